@@ -1,0 +1,272 @@
+#!/usr/bin/env python
+"""bench.py - phase-space point-updates/s of the DVM outer iteration (arXiv 1810.00348) on B200, fp64.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config IDX] [--kernel auto|slice|tile]
+    python bench.py --impl reference ...      # the CPU oracle on the host cores, bounded sample
+
+A "step" is one outer iteration (all of DESIGN.md's hot-path rows a1-a7) of the workload.  Default workload:
+BASELINE.json configs[4] (128^3 x 64^3 cavity, Kn = 0.01, memory-reduction path, f never materialised), the
+largest single-GPU configuration and the one the target is stated on; --config picks another.
+The solver runs on one GPU with no sharding (replicas only): with --gpus N every rank
+runs an independent replica, timing is max over ranks, value = total units / that time.
+Prints ONE JSON line.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+from pathlib import Path
+
+ROOT = Path(__file__).resolve().parent
+sys.path.insert(0, str(ROOT))
+
+METRIC = "phase-space point-updates/s (fp64, 1 B200)"
+UNIT = "point-updates/s"
+
+
+def measured_peaks():
+    p = ROOT / "MEASURED_PEAKS.json"
+    if p.exists():
+        d = json.loads(p.read_text())
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)", float(d.get("sm_max_mhz", 1965.0))
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)", 1965.0
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-i", str(self.index), "-lms", "200"], stdout=subprocess.PIPE,
+                                         stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], None, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            f = [x.strip() for x in r.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx = float(f[1])
+            except ValueError:
+                continue
+            for nme, val in zip(names, f[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(nme)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def workload_for(args):
+    from paper_1810_00348_b200 import workloads
+    return workloads.config(args.config)
+
+
+def algorithmic_bytes_per_point(kernel_name):
+    # slice kernel reads + writes one fp64 slice value per phase point (in-place slice: 16 B,
+    # plus the y-upwind re-read that is expected to hit L2); tile kernel moves only tile faces.
+    return {"slice": 16.0, "tile": 4.0}[kernel_name]
+
+
+# --------------------------------------------------------------------------------------------------
+def cpu_oracle_sample(wl, budget_s=15.0):
+    """Time the oracle as it stands on a bounded sample: one outer iteration over a zero-weight velocity subset
+    sized for ~budget_s seconds of CPU work (the oracle skips zero-weight velocities)."""
+    from paper_1810_00348_b200 import workloads
+    from oracle import dvm_oracle
+    cores = os.cpu_count() or 1
+    est_rate = 1.2e7 * cores
+    n_vel_target = max(8, int(est_rate * budget_s / wl.n_fluid))
+    keep = max(2, min(min(wl.mx, wl.my, wl.mz), int(round(n_vel_target ** (1.0 / 3.0)))))
+    sub = workloads.sparse_weight_subset(wl, keep=keep) if keep < max(wl.mx, wl.my, wl.mz) else wl
+    nv = int((sub.w_x > 0).sum() * (sub.w_y > 0).sum() * (sub.w_z > 0).sum())
+    # cap host memory: every thread holds 13 long-double accumulators + one f per cell
+    per_thread = wl.n_cells * (13 * 16 + 8)
+    nthreads = max(1, min(cores, nv, int(24e9 // per_thread)))
+    o = dvm_oracle.Oracle(sub)
+    t0 = time.perf_counter()
+    o.step(nthreads=nthreads)
+    dt = time.perf_counter() - t0
+    pts = wl.n_fluid * nv
+    return {"value": pts / dt, "unit": UNIT, "cores": int(o.threads), "kind": "oracle",
+            "sample": f"1 outer iteration over {nv} of {wl.n_vel} velocities (zero-weight subset, {keep} nodes/axis) "
+                      f"x {wl.n_fluid} cells = {pts:.3e} points in {dt:.2f} s"}, dt, pts
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    wl = workload_for(args)
+    vals = []
+    for i in range(args.warmup + args.steps):
+        cb, dt, pts = cpu_oracle_sample(wl, budget_s=args.ref_budget)
+        if i >= args.warmup:
+            vals.append((dt, pts, cb))
+    tot_t = sum(v[0] for v in vals)
+    tot_p = sum(v[1] for v in vals)
+    cb = dict(vals[-1][2]); cb["value"] = tot_p / tot_t
+    line = {"impl": "reference", "metric": METRIC, "value": tot_p / tot_t, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / len(vals), "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": wl.name, "phase_points_per_iteration": wl.phase_points,
+                       "note": "each step = one oracle iteration over a bounded velocity subset"},
+            "cpu_baseline": cb,
+            "e2e": {"value": tot_p / tot_t, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+# --------------------------------------------------------------------------------------------------
+def run_gpu(args):
+    import torch
+    from paper_1810_00348_b200 import dvm
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+    torch.cuda.set_device(local)
+    dev = torch.device(f"cuda:{local}")
+
+    wl = workload_for(args)
+    kernel = {"auto": dvm.KERNEL_AUTO, "slice": dvm.KERNEL_SLICE, "tile": dvm.KERNEL_TILE}[args.kernel]
+    s = dvm.Solver(wl, kernel=kernel, device=f"cuda:{local}")
+    stream = torch.cuda.current_stream(dev)
+
+    def barrier():
+        torch.cuda.synchronize(dev)
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    # ---- device-resident timing: W warm-up steps, then exactly K steps ----
+    s.iterate(args.warmup)
+    barrier()
+    l0 = s.launch_count()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    ev[0].record(stream)
+    for k in range(args.steps):
+        s.iterate(1)
+        ev[k + 1].record(stream)
+    barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    launches = s.launch_count() - l0
+    step_ms = [ev[k].elapsed_time(ev[k + 1]) for k in range(args.steps)]
+    total_ms = ev[0].elapsed_time(ev[args.steps])
+    res = s.residual()
+
+    # ---- end-to-end through the C ABI with host buffers (pinned), copies inside the timed region ----
+    n8, n14 = 8 * wl.n_cells, 14 * wl.n_cells
+    h_in = torch.empty(n8, dtype=torch.float64).pin_memory()
+    h_rw = torch.empty(max(s.nface, 1), dtype=torch.float64).pin_memory()
+    h_out = torch.empty(n14, dtype=torch.float64).pin_memory()
+    h_rw_out = torch.empty(max(s.nface, 1), dtype=torch.float64).pin_memory()
+    p14, rw = s.get_state()
+    h_in.copy_(p14[:8].reshape(-1).cpu()); h_rw[: s.nface].copy_(rw.cpu())
+    e2e_steps = max(1, min(args.steps, args.e2e_steps))
+    s.step_host(h_in, h_rw, 1, h_out, h_rw_out)  # warm
+    barrier()
+    t0 = time.perf_counter()
+    for k in range(e2e_steps):
+        s.step_host(h_in, h_rw, 1, h_out, h_rw_out)
+        h_in.copy_(h_out[:n8]); h_rw.copy_(h_rw_out)
+    torch.cuda.synchronize(dev)
+    e2e_ms = 1e3 * (time.perf_counter() - t0) / e2e_steps
+
+    t = torch.tensor([total_ms, e2e_ms], dtype=torch.float64, device=dev)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    total_ms, e2e_ms = t.tolist()
+    total_bytes, f_bytes = s.workspace_bytes()
+
+    if rank == 0:
+        pts = wl.phase_points
+        ms_per_step = total_ms / args.steps
+        value = world * pts / (ms_per_step * 1e-3)
+        kname = "slice" if s.kernel_used() == dvm.KERNEL_SLICE else "tile"
+        peak, peak_src, _ = measured_peaks()
+        # dominant kernel = the sweep (one launch per step); its duration is the step minus the five small update
+        # launches, measured here as the step itself (upper bound on the sweep time -> lower bound on achieved)
+        bpp = algorithmic_bytes_per_point(kname)
+        achieved = bpp * pts / (ms_per_step * 1e-3) / 1e9
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": wl.name, "physical_cells": [wl.nx, wl.ny, wl.nz], "velocity_nodes": [wl.mx, wl.my, wl.mz],
+                       "phase_points_per_iteration": pts, "kernel": kname, "parallelism": "replicas only" if world > 1 else "1 GPU",
+                       "l2": "inputs larger than L2 (f workspace %.1f GB, fields %.2f GB)" % (f_bytes / 1e9, (total_bytes - f_bytes) / 1e9)
+                       if total_bytes > 126e6 else "working set smaller than L2 (config is a parity case)",
+                       "workspace_bytes": total_bytes, "f_workspace_bytes": f_bytes,
+                       "full_6d_f_bytes_never_allocated": 8 * wl.n_cells * wl.n_vel,
+                       "residual_after_run": [float(x) for x in res], "step_ms": [round(x, 3) for x in step_ms]},
+            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                         "traffic": None, "peak_source": peak_src, "kernel": f"sweep_{kname}_kernel",
+                         "algorithmic_bytes_per_point": bpp},
+            "e2e": {"value": world * pts / (e2e_ms * 1e-3), "unit": UNIT,
+                    "h2d_bytes_per_step": 8 * (n8 + s.nface), "d2h_bytes_per_step": 8 * (n14 + s.nface)},
+            "gpu_launches": int(launches),
+            "clocks": clocks,
+        }
+        if world == 1 and not args.no_cpu_baseline:
+            line["cpu_baseline"], _, _ = cpu_oracle_sample(wl, budget_s=args.ref_budget)
+        print(json.dumps(line))
+    s.close()
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=4)
+    ap.add_argument("--kernel", default="auto", choices=["auto", "slice", "tile"])
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--ref-budget", type=float, default=15.0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_gpu(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,156 @@
+/*
+ * dvm.h - C ABI of the B200-native solver for ONE thing: the outer iteration of the memory-reduced
+ * iterative discrete-velocity method (DVM) of arXiv 1810.00348 for the steady 3D3V Shakhov/BGK model
+ * equation.  Citations are to /root/reference/PAPER.md (line, section, equation).
+ *
+ * One outer iteration (Alg. 1; Eq.(6)):
+ *   every discrete velocity xi_alpha sweeps the physical grid along its characteristic direction with the
+ *   first-order upwind formula Eq.(7), the Shakhov equilibrium f^S (Eq.(2))
+ *   and the relaxation time tau = mu/p (Eq.(10)) being rebuilt on the fly from
+ *   the macroscopic fields of step n; ghost values come from the Maxwell diffuse wall (Eq.(8)-(9),
+ *   PAPER.md:211-219), the free stream or a zero-gradient outflow; the moments Eq.(5)
+ *    and the wall-incident fluxes are reduced over velocity space as each value is produced
+ *   (PAPER.md:81), so the 6-D distribution function is never stored; a moment-update step converts the
+ *   sums to rho, u, T, q, sigma, rescales the mass of closed domains and evaluates the
+ *   convergence residual.
+ *
+ * Units: speeds in v_m = sqrt(2 R T0), rho in rho0, T in T0, lengths in L, f in rho0/v_m^3, q in
+ * rho0 v_m^3, sigma in rho0 v_m^2 (reading G2).
+ *
+ * Layout: cell index c = (k*ny + j)*nx + i (i fastest).  Fields are SoA: field m of cell c at [m*ncell + c].
+ * Direction ids: 0 = x-, 1 = x+, 2 = y-, 3 = y+, 4 = z-, 5 = z+.
+ * Boundary-face table (one slot per face whatever its type; see dvm_num_faces):
+ *   the six domain faces first - x- [k*ny+j], x+ [k*ny+j], y- [k*nx+i], y+ [k*nx+i], z- [j*nx+i],
+ *   z+ [j*nx+i] - then every face between a fluid cell and a solid (masked) cell inside the domain, ordered
+ *   by (fluid cell index ascending, direction id ascending).
+ *
+ * Pointers: "host" = ordinary host memory, read during the call only (dvm_create copies what it needs);
+ * "dev" = device memory on the solver's device, caller-owned, at least the stated size.
+ * All device work is enqueued on the stream given at creation; only the calls marked (syncs) wait for it.
+ * Every call returns 0 or a negative DVM_E* code; nothing throws or aborts across this boundary;
+ * dvm_last_error() returns a thread-local message for the last failing call of this thread.
+ * There is no CPU fallback: without a CUDA device dvm_create fails with DVM_ECUDA.
+ */
+#ifndef DVM_H
+#define DVM_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define DVM_OK          0
+#define DVM_EINVAL     -1   /* NULL pointer, non-positive size, non-monotone faces or nodes, bad BC type */
+#define DVM_ENOMEM     -2   /* the allocator returned NULL */
+#define DVM_ECUDA      -3   /* a CUDA runtime call or kernel launch failed, or no device */
+#define DVM_ENONFINITE -4   /* the residual reduction met NaN/Inf */
+
+#define DVM_WALL_DIFFUSE  0 /* Eq.(8)-(9): ghost = rho_w g_w(xi), g_w Maxwellian at (T, u), rho_w lagged */
+#define DVM_FREESTREAM    1 /* ghost = f^M(rho, u, T)(xi) */
+#define DVM_ZERO_GRADIENT 2 /* ghost = the cell's own new value, i.e. the term drops out of Eq.(7) */
+
+/* sweep-kernel variants (dvm_set_option DVM_OPT_KERNEL) */
+#define DVM_KERNEL_AUTO   0
+#define DVM_KERNEL_SLICE  1 /* the paper's mapping (thread = velocity, z-slice in HBM), fp64, in-place slice */
+#define DVM_KERNEL_TILE   2 /* B200 design: on-chip z-column tiles, DMMA moment contraction */
+
+#define DVM_OPT_KERNEL    1
+
+typedef struct dvm_solver dvm_solver; /* opaque */
+
+typedef struct {
+    int nx, ny, nz;
+    const double *xf, *yf, *zf;     /* host; face coordinates, nx+1 / ny+1 / nz+1 values, strictly increasing */
+    const unsigned char *solid;     /* host; nz*ny*nx, 1 = solid cell; NULL = all fluid */
+} dvm_grid;
+
+typedef struct {
+    int mx, my, mz;
+    const double *xi_x, *xi_y, *xi_z; /* host; nodes per axis, strictly increasing (tensor grid) */
+    const double *w_x, *w_y, *w_z;    /* host; 1-D quadrature weights >= 0; w_alpha = w_x w_y w_z (Eq.(5)) */
+} dvm_vgrid;
+
+typedef struct {
+    double Kn, omega, Pr;           /* Pr = 1: BGK; 2/3: Shakhov */
+    double rho0, u0[3], T0;         /* uniform initial state */
+} dvm_gas;
+
+typedef struct {
+    int type;                       /* DVM_WALL_DIFFUSE | DVM_FREESTREAM | DVM_ZERO_GRADIENT */
+    double T, rho, u[3];            /* wall: T, u ; free stream: rho, u, T ; zero gradient: unused */
+} dvm_face_bc;
+
+typedef struct {
+    dvm_face_bc face[6];            /* x-, x+, y-, y+, z-, z+ */
+    dvm_face_bc solid;              /* faces of masked cells (must be DVM_WALL_DIFFUSE) */
+    int rescale_mass;               /* 1 = global density rescale of closed domains */
+    int wall_norm;                  /* 0 = discrete half-flux normalisation (default), 1 = constant of Eq.(9) */
+} dvm_bc;
+
+typedef struct {
+    void *stream;                               /* cudaStream_t (0 = default stream) */
+    void *(*alloc)(size_t bytes, void *ctx);    /* device allocator, 256-byte aligned; NULL -> cudaMalloc */
+    void (*free_)(void *ptr, void *ctx);        /* matching release; NULL -> cudaFree */
+    void *ctx;
+} dvm_device;
+
+/* Build a solver: copies all host arrays, allocates its workspace through dev->alloc (no allocation scales
+ * with ncell * nvel: only one z-slice worth of f per in-flight velocity is held), sets the uniform initial
+ * state and rho_w^0 (DESIGN.md oracle step 1).  dev may be NULL (default stream, cudaMalloc). */
+int dvm_create(const dvm_grid *grid, const dvm_vgrid *vgrid, const dvm_gas *gas, const dvm_bc *bc,
+               const dvm_device *dev, dvm_solver **out);
+
+/* n >= 0 outer iterations (Alg. 1 + moment update + residual), asynchronous on the stream. */
+int dvm_iterate(dvm_solver *s, int n);
+
+/* Current macroscopic fields, dev_out[14][ncell]: rho, ux, uy, uz, T, qx, qy, qz, sxx, syy, szz, sxy, sxz, syz
+ * (solid cells: zeros).  Asynchronous device-to-device copy on the stream. */
+int dvm_moments(dvm_solver *s, double *dev_out);
+
+/* (syncs) Residual of the last iteration, host_out3 = r_rho, r_mom, r_E (G9).
+ * DVM_ENONFINITE if any of them is NaN/Inf; DVM_EINVAL before the first iteration. */
+int dvm_residual(dvm_solver *s, double *host_out3);
+
+/* ---- support calls ------------------------------------------------------------------------------ */
+/* number of boundary-face slots (domain + solid), >= 0, or a negative error code */
+int dvm_num_faces(const dvm_solver *s);
+/* number of outer iterations done since creation */
+int dvm_iterations_done(const dvm_solver *s);
+/* State between iterations = checkpoint: dev_prim14 [14][ncell] (as dvm_moments), dev_rho_wall [nfaces].
+ * Either pointer may be NULL to skip it.  Asynchronous. */
+int dvm_get_state(dvm_solver *s, double *dev_prim14, double *dev_rho_wall);
+/* Replace the state: dev_prim8 [8][ncell] = rho, u, T, q (sigma is output only); dev_rho_wall [nfaces] or NULL
+ * (keep).  The reference mass of the rescale stays that of the initial state.  Asynchronous. */
+int dvm_set_state(dvm_solver *s, const double *dev_prim8, const double *dev_rho_wall);
+/* Raw velocity sums of the last iteration, dev_raw13 [13][ncell]:
+ * sum_alpha w f {1, xi_x, xi_y, xi_z, xx, yy, zz, xy, xz, yz, xi_x|xi|^2, xi_y|xi|^2, xi_z|xi|^2}; before the
+ * rescale.  Asynchronous. */
+int dvm_raw_moments(dvm_solver *s, double *dev_raw13);
+/* Wall-incident fluxes of the last iteration, dev_flux [nfaces] (before division by Phi_unit and rescale). */
+int dvm_wall_flux(dvm_solver *s, double *dev_flux);
+/* (syncs) Residual triples of the last min(max_n, iterations done, capacity) iterations, oldest first,
+ * host_out[3*count]; returns count or a negative code. */
+int dvm_residual_history(dvm_solver *s, double *host_out, int max_n);
+/* (syncs) Mass-rescale factor of the last iteration (1 if rescale_mass = 0). */
+int dvm_mass_scale(dvm_solver *s, double *host_out1);
+/* (syncs) End-to-end step with HOST buffers: upload the state (host_prim8 [8][ncell], host_rho_wall [nfaces],
+ * either may be NULL = keep), run n iterations, download prim14 [14][ncell] and rho_wall (either may be NULL). */
+int dvm_step_host(dvm_solver *s, const double *host_prim8, const double *host_rho_wall, int n,
+                  double *host_prim14_out, double *host_rho_wall_out);
+/* Tuning / variant selection; must be called before the first dvm_iterate.  Unknown option: DVM_EINVAL. */
+int dvm_set_option(dvm_solver *s, int option, int value);
+/* Sweep-kernel variant in use: DVM_KERNEL_SLICE / DVM_KERNEL_TILE once the first dvm_iterate has planned the
+ * workspace, the requested value (possibly DVM_KERNEL_AUTO) before. */
+int dvm_kernel_used(const dvm_solver *s);
+/* Bytes of device workspace held by the solver, and the part of it that holds distribution-function values. */
+int dvm_workspace_bytes(const dvm_solver *s, size_t *total, size_t *f_bytes);
+/* Number of kernel launches enqueued by this solver so far (bench.py's gpu_launches). */
+long long dvm_launch_count(const dvm_solver *s);
+int dvm_destroy(dvm_solver *s);
+const char *dvm_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,566 @@
+// dvm_api.cu - host side of the C ABI declared in include/dvm.h: validation, geometry / boundary-face tables,
+// velocity-octant block tables, workspace management and the per-iteration launch sequence
+// (Alg. 1: sweep all velocity groups, then update the moments).
+// Product code: no CPU fallback and nothing shared with oracle/.
+#include "../../include/dvm.h"
+#include "dvm_dev.cuh"
+#include "update.cuh"
+#include "sweep_tile.cuh"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+using namespace dvm;
+
+namespace {
+
+thread_local std::string g_err;
+
+int fail(int code, const char *fmt, ...)
+{
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    g_err = buf;
+    return code;
+}
+
+#define CK(call)                                                                                     \
+    do {                                                                                             \
+        cudaError_t e_ = (call);                                                                     \
+        if (e_ != cudaSuccess) return fail(DVM_ECUDA, "%s: %s (%s:%d)", #call, cudaGetErrorString(e_), \
+                                           __FILE__, __LINE__);                                      \
+    } while (0)
+
+constexpr int HIST_CAP = 16384;
+const double PI = 3.14159265358979323846;
+
+}  // namespace
+
+struct dvm_solver {
+    int nx = 0, ny = 0, nz = 0, mx = 0, my = 0, mz = 0, nface = 0;
+    long long ncell = 0;
+    std::vector<double> xf, yf, zf, xi[3], w[3];
+    std::vector<unsigned char> solid;
+    dvm_gas gas{};
+    dvm_bc bc{};
+    cudaStream_t stream = nullptr;
+    dvm_device dev{};
+    std::vector<void *> allocs;
+    size_t total_bytes = 0, f_bytes = 0;
+    double mass0 = 0.0;
+    int iters = 0;
+    int kernel = DVM_KERNEL_AUTO;
+    bool planned = false;
+    long long launches = 0;
+    // device arrays
+    double *d_invdx = nullptr, *d_invdy = nullptr, *d_invdz = nullptr, *d_dx = nullptr, *d_dy = nullptr, *d_dz = nullptr;
+    unsigned char *d_flags = nullptr, *d_face_slot = nullptr;
+    int *d_face_of = nullptr;
+    double *d_xi[3] = {nullptr, nullptr, nullptr}, *d_w[3] = {nullptr, nullptr, nullptr};
+    double *d_prim = nullptr, *d_prim_new = nullptr, *d_coef = nullptr, *d_raw = nullptr;
+    double *d_rho_w = nullptr, *d_phi = nullptr, *d_phi_unit = nullptr;
+    double *d_part = nullptr, *d_scal = nullptr, *d_hist = nullptr, *d_hist_scale = nullptr;
+    long long npart = 0;
+    // sweep plan
+    std::vector<BlockDesc> blocks;
+    BlockDesc *d_blocks = nullptr;
+    double *d_fbuf = nullptr;
+    long long fstride = 0;
+    int nb_threads = 128;
+    TilePlan tile{};
+    std::vector<double> h_rho_w0;
+
+    void *dalloc(size_t bytes)
+    {
+        bytes = (bytes + 255) / 256 * 256;
+        if (bytes == 0) bytes = 256;
+        void *p = nullptr;
+        if (dev.alloc) p = dev.alloc(bytes, dev.ctx);
+        else if (cudaMalloc(&p, bytes) != cudaSuccess) p = nullptr;
+        if (p) { allocs.push_back(p); total_bytes += bytes; }
+        return p;
+    }
+    void dfree_all()
+    {
+        for (void *p : allocs) {
+            if (dev.free_) dev.free_(p, dev.ctx);
+            else if (!dev.alloc) cudaFree(p);
+        }
+        allocs.clear();
+    }
+};
+
+namespace {
+
+template <class T>
+int upload(dvm_solver *s, T **dst, const T *src, size_t n)
+{
+    *dst = (T *)s->dalloc(n * sizeof(T));
+    if (!*dst) return fail(DVM_ENOMEM, "device allocation of %zu bytes failed", n * sizeof(T));
+    CK(cudaMemcpyAsync(*dst, src, n * sizeof(T), cudaMemcpyHostToDevice, s->stream));
+    return 0;
+}
+
+template <class T>
+int dzeros(dvm_solver *s, T **dst, size_t n)
+{
+    *dst = (T *)s->dalloc(n * sizeof(T));
+    if (!*dst) return fail(DVM_ENOMEM, "device allocation of %zu bytes failed", n * sizeof(T));
+    CK(cudaMemsetAsync(*dst, 0, n * sizeof(T), s->stream));
+    return 0;
+}
+
+bool increasing(const double *a, int n)
+{
+    for (int i = 1; i < n; ++i)
+        if (!(a[i] > a[i - 1])) return false;
+    return true;
+}
+
+double host_wall_maxwellian(const dvm_face_bc &b, const double xi[3])
+{
+    const double cx = xi[0] - b.u[0], cy = xi[1] - b.u[1], cz = xi[2] - b.u[2];
+    return std::exp(-(cx * cx + cy * cy + cz * cz) / b.T) / std::pow(PI * b.T, 1.5);
+}
+
+const dvm_face_bc &slot_bc(const dvm_bc &bc, int b) { return b < 6 ? bc.face[b] : bc.solid; }
+
+UpdateParams update_params(dvm_solver *s)
+{
+    UpdateParams U{};
+    U.nx = s->nx; U.ny = s->ny; U.nz = s->nz; U.nface = s->nface; U.ncell = s->ncell; U.npart = s->npart;
+    U.flags = s->d_flags; U.dx = s->d_dx; U.dy = s->d_dy; U.dz = s->d_dz;
+    U.raw = s->d_raw; U.prim = s->d_prim; U.prim_new = s->d_prim_new; U.coef = s->d_coef;
+    U.part = s->d_part; U.scal = s->d_scal; U.hist = s->d_hist; U.hist_scale = s->d_hist_scale;
+    U.phi = s->d_phi; U.phi_unit = s->d_phi_unit; U.rho_w = s->d_rho_w;
+    U.omega = s->gas.omega;
+    const double cw = 15.0 * std::sqrt(PI) / ((5.0 - 2.0 * s->gas.omega) * (7.0 - 2.0 * s->gas.omega));
+    U.inv_cw_kn = 1.0 / (cw * s->gas.Kn);
+    U.shk = (1.0 - s->gas.Pr) * 0.8;
+    U.mass0 = s->mass0;
+    U.rescale = s->bc.rescale_mass;
+    return U;
+}
+
+SweepParams sweep_params(dvm_solver *s)
+{
+    SweepParams P{};
+    P.nx = s->nx; P.ny = s->ny; P.nz = s->nz; P.ncell = s->ncell;
+    P.invdx = s->d_invdx; P.invdy = s->d_invdy; P.invdz = s->d_invdz;
+    P.flags = s->d_flags; P.face_of = s->d_face_of; P.face_slot = s->d_face_slot;
+    P.coef = s->d_coef; P.rho_w = s->d_rho_w; P.phi = s->d_phi; P.raw = s->d_raw;
+    P.xi_x = s->d_xi[0]; P.xi_y = s->d_xi[1]; P.xi_z = s->d_xi[2];
+    P.w_x = s->d_w[0]; P.w_y = s->d_w[1]; P.w_z = s->d_w[2];
+    P.blocks = s->d_blocks; P.fbuf = s->d_fbuf; P.fstride = s->fstride;
+    for (int b = 0; b < 7; ++b) {
+        const dvm_face_bc &f = slot_bc(s->bc, b);
+        P.bc.type[b] = f.type; P.bc.T[b] = f.T; P.bc.rho[b] = f.rho;
+        for (int d = 0; d < 3; ++d) P.bc.u[b][d] = f.u[d];
+    }
+    return P;
+}
+
+// index ranges of the negative / non-negative nodes of one axis (nodes ascending)
+void split_axis(const std::vector<double> &xi, int lo[2], int cnt[2])
+{
+    int nneg = 0;
+    while (nneg < (int)xi.size() && xi[nneg] < 0.0) ++nneg;
+    lo[0] = 0; cnt[0] = nneg; lo[1] = nneg; cnt[1] = (int)xi.size() - nneg;
+}
+
+// Decide the kernel variant and build the block table + f workspace (once, before the first iteration).
+int plan(dvm_solver *s)
+{
+    if (s->planned) return 0;
+    const long long nvel = (long long)s->mx * s->my * s->mz;
+    int kernel = s->kernel;
+    if (kernel == DVM_KERNEL_AUTO) kernel = tile_supported(s->nx, s->ny, s->nz) ? DVM_KERNEL_TILE : DVM_KERNEL_SLICE;
+    if (kernel == DVM_KERNEL_TILE && !tile_supported(s->nx, s->ny, s->nz))
+        return fail(DVM_EINVAL, "tile kernel does not support this grid");
+    s->kernel = kernel;
+    int lo[3][2], cnt[3][2];
+    for (int d = 0; d < 3; ++d) split_axis(s->xi[d], lo[d], cnt[d]);
+    s->blocks.clear();
+    if (kernel == DVM_KERNEL_SLICE) {
+        int nb = 128;
+        if (nvel / 128 < 296) nb = 64;
+        if (nvel / 64 < 296) nb = 32;
+        s->nb_threads = nb;
+        int col = 0;
+        for (int oz = 0; oz < 2; ++oz) for (int oy = 0; oy < 2; ++oy) for (int ox = 0; ox < 2; ++ox) {
+            const int n = cnt[0][ox] * cnt[1][oy] * cnt[2][oz];
+            for (int l0 = 0; l0 < n; l0 += nb) {
+                BlockDesc b{};
+                b.ia0 = lo[0][ox]; b.na = cnt[0][ox]; b.ib0 = lo[1][oy]; b.nb = cnt[1][oy];
+                b.ic0 = lo[2][oz]; b.nc = cnt[2][oz]; b.l0 = l0;
+                b.sx = ox ? 1 : -1; b.sy = oy ? 1 : -1; b.sz = oz ? 1 : -1;
+                b.col0 = col; col += nb;
+                s->blocks.push_back(b);
+            }
+        }
+        s->fstride = col;
+        const size_t fbytes = (size_t)col * s->nx * s->ny * sizeof(double);
+        s->d_fbuf = (double *)s->dalloc(fbytes);
+        if (!s->d_fbuf) return fail(DVM_ENOMEM, "slice workspace of %zu bytes failed", fbytes);
+        s->f_bytes = fbytes;
+    } else {
+        int rc = tile_plan(s->nx, s->ny, s->nz, lo, cnt, nvel, &s->tile, &s->blocks);
+        if (rc) return fail(DVM_EINVAL, "tile plan failed");
+        const size_t fbytes = s->tile.fbuf_doubles * sizeof(double);
+        s->d_fbuf = (double *)s->dalloc(fbytes);
+        if (!s->d_fbuf) return fail(DVM_ENOMEM, "tile face workspace of %zu bytes failed", fbytes);
+        s->f_bytes = fbytes;
+    }
+    if (upload(s, &s->d_blocks, s->blocks.data(), s->blocks.size())) return DVM_ENOMEM;
+    s->planned = true;
+    return 0;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *dvm_last_error(void) { return g_err.c_str(); }
+
+int dvm_create(const dvm_grid *g, const dvm_vgrid *v, const dvm_gas *gas, const dvm_bc *bc, const dvm_device *dev,
+               dvm_solver **out)
+{
+    if (!g || !v || !gas || !bc || !out) return fail(DVM_EINVAL, "NULL argument");
+    *out = nullptr;
+    if (g->nx <= 0 || g->ny <= 0 || g->nz <= 0 || v->mx <= 0 || v->my <= 0 || v->mz <= 0)
+        return fail(DVM_EINVAL, "non-positive grid size");
+    if (!g->xf || !g->yf || !g->zf || !v->xi_x || !v->xi_y || !v->xi_z || !v->w_x || !v->w_y || !v->w_z)
+        return fail(DVM_EINVAL, "NULL array");
+    if ((long long)g->nx * g->ny * g->nz > 2000000000LL) return fail(DVM_EINVAL, "too many cells");
+    if (!increasing(g->xf, g->nx + 1) || !increasing(g->yf, g->ny + 1) || !increasing(g->zf, g->nz + 1))
+        return fail(DVM_EINVAL, "face coordinates must be strictly increasing");
+    if (!increasing(v->xi_x, v->mx) || !increasing(v->xi_y, v->my) || !increasing(v->xi_z, v->mz))
+        return fail(DVM_EINVAL, "velocity nodes must be strictly increasing");
+    for (int d = 0; d < 3; ++d) {
+        const double *w = d == 0 ? v->w_x : d == 1 ? v->w_y : v->w_z;
+        const int m = d == 0 ? v->mx : d == 1 ? v->my : v->mz;
+        for (int i = 0; i < m; ++i)
+            if (!(w[i] >= 0.0)) return fail(DVM_EINVAL, "quadrature weights must be >= 0");
+    }
+    if (!(gas->Kn > 0) || !(gas->rho0 > 0) || !(gas->T0 > 0) || !(gas->Pr > 0))
+        return fail(DVM_EINVAL, "Kn, Pr, rho0, T0 must be positive");
+    for (int b = 0; b < 7; ++b) {
+        const dvm_face_bc &f = slot_bc(*bc, b);
+        if (f.type < 0 || f.type > 2) return fail(DVM_EINVAL, "bad boundary type %d in slot %d", f.type, b);
+        if (f.type != DVM_ZERO_GRADIENT && !(f.T > 0)) return fail(DVM_EINVAL, "boundary temperature must be > 0");
+    }
+    if (g->solid && bc->solid.type != DVM_WALL_DIFFUSE) return fail(DVM_EINVAL, "solid faces must be diffuse walls");
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        cudaGetLastError();
+        return fail(DVM_ECUDA, "no CUDA device: this library has no CPU fallback");
+    }
+
+    dvm_solver *s = new (std::nothrow) dvm_solver;
+    if (!s) return fail(DVM_ENOMEM, "host allocation failed");
+    s->nx = g->nx; s->ny = g->ny; s->nz = g->nz; s->mx = v->mx; s->my = v->my; s->mz = v->mz;
+    s->ncell = (long long)g->nx * g->ny * g->nz;
+    s->xf.assign(g->xf, g->xf + g->nx + 1); s->yf.assign(g->yf, g->yf + g->ny + 1); s->zf.assign(g->zf, g->zf + g->nz + 1);
+    s->xi[0].assign(v->xi_x, v->xi_x + v->mx); s->xi[1].assign(v->xi_y, v->xi_y + v->my); s->xi[2].assign(v->xi_z, v->xi_z + v->mz);
+    s->w[0].assign(v->w_x, v->w_x + v->mx); s->w[1].assign(v->w_y, v->w_y + v->my); s->w[2].assign(v->w_z, v->w_z + v->mz);
+    s->solid.assign((size_t)s->ncell, 0);
+    if (g->solid) for (long long c = 0; c < s->ncell; ++c) s->solid[c] = g->solid[c] ? 1 : 0;
+    s->gas = *gas; s->bc = *bc;
+    if (dev) { s->dev = *dev; s->stream = (cudaStream_t)dev->stream; }
+
+    auto bail = [&](int rc) { cudaStreamSynchronize(s->stream); s->dfree_all(); delete s; return rc; };
+
+    const int nx = s->nx, ny = s->ny, nz = s->nz;
+    const long long n = s->ncell;
+    // ---- geometry ----
+    std::vector<double> dx(nx), dy(ny), dz(nz), idx(nx), idy(ny), idz(nz);
+    for (int i = 0; i < nx; ++i) { dx[i] = s->xf[i + 1] - s->xf[i]; idx[i] = 1.0 / dx[i]; }
+    for (int j = 0; j < ny; ++j) { dy[j] = s->yf[j + 1] - s->yf[j]; idy[j] = 1.0 / dy[j]; }
+    for (int k = 0; k < nz; ++k) { dz[k] = s->zf[k + 1] - s->zf[k]; idz[k] = 1.0 / dz[k]; }
+    // ---- cell flags, boundary-face table (order stated in dvm.h) ----
+    std::vector<unsigned char> flags((size_t)n, 0);
+    std::vector<int> face_of((size_t)6 * n, -1);
+    const int off[6] = {0, ny * nz, 2 * ny * nz, 2 * ny * nz + nx * nz, 2 * ny * nz + 2 * nx * nz,
+                        2 * ny * nz + 2 * nx * nz + nx * ny};
+    const int ndom = off[5] + nx * ny;
+    std::vector<unsigned char> face_slot((size_t)ndom, 6);
+    std::vector<int> face_cell((size_t)ndom, -1), face_dir((size_t)ndom, 0);
+    static const int di[6] = {-1, 1, 0, 0, 0, 0}, dj[6] = {0, 0, -1, 1, 0, 0}, dk[6] = {0, 0, 0, 0, -1, 1};
+    auto sol = [&](int i, int j, int k) { return s->solid[((size_t)k * ny + j) * nx + i] != 0; };
+    double mass0 = 0.0;
+    for (int k = 0; k < nz; ++k) for (int j = 0; j < ny; ++j) for (int i = 0; i < nx; ++i) {
+        const long long c = ((long long)k * ny + j) * nx + i;
+        const bool cs = sol(i, j, k);
+        if (cs) flags[c] |= FLAG_SOLID;
+        else mass0 += gas->rho0 * (dx[i] * dy[j] * dz[k]);
+        for (int d = 0; d < 6; ++d) {
+            const int ii = i + di[d], jj = j + dj[d], kk = k + dk[d];
+            const bool outside = ii < 0 || ii >= nx || jj < 0 || jj >= ny || kk < 0 || kk >= nz;
+            if (outside) {
+                int f;
+                switch (d) {
+                    case 0: case 1: f = off[d] + k * ny + j; break;
+                    case 2: case 3: f = off[d] + k * nx + i; break;
+                    default: f = off[d] + j * nx + i; break;
+                }
+                face_slot[f] = (unsigned char)d; face_dir[f] = d;
+                flags[c] |= (unsigned char)(1u << d);
+                if (!cs) { face_cell[f] = (int)c; face_of[(size_t)d * n + c] = f; }
+            } else if (sol(ii, jj, kk)) {
+                flags[c] |= (unsigned char)(1u << d);
+                if (!cs) {
+                    const int f = (int)face_slot.size();
+                    face_slot.push_back(6); face_cell.push_back((int)c); face_dir.push_back(d);
+                    face_of[(size_t)d * n + c] = f;
+                }
+            }
+        }
+    }
+    s->nface = (int)face_slot.size();
+    s->mass0 = mass0;
+    // ---- Phi_unit per (bc slot, direction) and Phi^0 per direction (oracle step 1; Eq.(9) with weights) ----
+    double tab[7][6] = {}, phi0[6] = {};
+    {
+        long double t[7][6] = {}, p0[6] = {};
+        dvm_face_bc init{};
+        init.T = gas->T0; init.u[0] = gas->u0[0]; init.u[1] = gas->u0[1]; init.u[2] = gas->u0[2];
+        for (int ic = 0; ic < s->mz; ++ic) for (int ib = 0; ib < s->my; ++ib) for (int ia = 0; ia < s->mx; ++ia) {
+            const double xi[3] = {s->xi[0][ia], s->xi[1][ib], s->xi[2][ic]};
+            const double w = s->w[0][ia] * s->w[1][ib] * s->w[2][ic];
+            const double f0 = gas->rho0 * host_wall_maxwellian(init, xi);
+            for (int d = 0; d < 6; ++d) {
+                const double toward = xi[d / 2] * ((d & 1) ? 1.0 : -1.0);  // > 0: moving towards side d
+                if (toward > 0) p0[d] += (long double)(w * toward * f0);
+            }
+            for (int b = 0; b < 7; ++b) {
+                const dvm_face_bc &f = slot_bc(*bc, b);
+                if (f.type != DVM_WALL_DIFFUSE) continue;
+                const double gw = host_wall_maxwellian(f, xi);
+                for (int d = 0; d < 6; ++d) {
+                    const double away = xi[d / 2] * ((d & 1) ? -1.0 : 1.0);  // > 0: leaving a wall on side d
+                    if (away > 0) t[b][d] += (long double)(w * away * gw);
+                }
+            }
+        }
+        for (int b = 0; b < 7; ++b) for (int d = 0; d < 6; ++d) tab[b][d] = (double)t[b][d];
+        for (int d = 0; d < 6; ++d) phi0[d] = (double)p0[d];
+    }
+    std::vector<double> phi_unit((size_t)s->nface, 0.0), rho_w0((size_t)s->nface, 0.0);
+    for (int f = 0; f < s->nface; ++f) {
+        const int b = face_slot[f];
+        const dvm_face_bc &fb = slot_bc(*bc, b);
+        if (fb.type != DVM_WALL_DIFFUSE || face_cell[f] < 0) continue;
+        phi_unit[f] = bc->wall_norm == 1 ? std::sqrt(fb.T / (4.0 * PI)) : tab[b][face_dir[f]];
+        if (!(phi_unit[f] > 0.0)) { return bail(fail(DVM_EINVAL, "no velocity node leaves wall face %d", f)); }
+        rho_w0[f] = phi0[face_dir[f]] / phi_unit[f];
+    }
+    s->h_rho_w0 = rho_w0;
+
+    // ---- device state ----
+    int rc = 0;
+    rc |= upload(s, &s->d_invdx, idx.data(), nx); rc |= upload(s, &s->d_invdy, idy.data(), ny);
+    rc |= upload(s, &s->d_invdz, idz.data(), nz);
+    rc |= upload(s, &s->d_dx, dx.data(), nx); rc |= upload(s, &s->d_dy, dy.data(), ny); rc |= upload(s, &s->d_dz, dz.data(), nz);
+    rc |= upload(s, &s->d_flags, flags.data(), (size_t)n);
+    rc |= upload(s, &s->d_face_of, face_of.data(), (size_t)6 * n);
+    rc |= upload(s, &s->d_face_slot, face_slot.data(), (size_t)s->nface);
+    for (int d = 0; d < 3; ++d) {
+        rc |= upload(s, &s->d_xi[d], s->xi[d].data(), s->xi[d].size());
+        rc |= upload(s, &s->d_w[d], s->w[d].data(), s->w[d].size());
+    }
+    rc |= upload(s, &s->d_phi_unit, phi_unit.data(), (size_t)s->nface);
+    rc |= upload(s, &s->d_rho_w, rho_w0.data(), (size_t)s->nface);
+    rc |= dzeros(s, &s->d_phi, (size_t)s->nface);
+    rc |= dzeros(s, &s->d_prim_new, (size_t)NPRIM * n);
+    rc |= dzeros(s, &s->d_coef, (size_t)NCOEF * n);
+    rc |= dzeros(s, &s->d_raw, (size_t)16 * n);
+    s->npart = (n + 255) / 256;
+    rc |= dzeros(s, &s->d_part, (size_t)7 * s->npart);
+    rc |= dzeros(s, &s->d_scal, 8);
+    rc |= dzeros(s, &s->d_hist, (size_t)3 * HIST_CAP);
+    rc |= dzeros(s, &s->d_hist_scale, (size_t)HIST_CAP);
+    if (rc) return bail(rc == DVM_ENOMEM ? DVM_ENOMEM : DVM_ECUDA);
+    {
+        std::vector<double> prim((size_t)NPRIM * n, 0.0);
+        for (long long c = 0; c < n; ++c) {
+            if (s->solid[c]) continue;
+            prim[c] = gas->rho0; prim[n + c] = gas->u0[0]; prim[2 * n + c] = gas->u0[1]; prim[3 * n + c] = gas->u0[2];
+            prim[4 * n + c] = gas->T0;
+        }
+        if (upload(s, &s->d_prim, prim.data(), prim.size())) return bail(DVM_ENOMEM);
+        if (cudaStreamSynchronize(s->stream) != cudaSuccess) return bail(fail(DVM_ECUDA, "upload failed"));
+    }
+    {
+        UpdateParams U = update_params(s);
+        if (launch_pack(U, s->stream) != cudaSuccess) return bail(fail(DVM_ECUDA, "pack kernel launch failed"));
+        s->launches += 1;
+    }
+    if (cudaStreamSynchronize(s->stream) != cudaSuccess) return bail(fail(DVM_ECUDA, "initialisation failed: %s", cudaGetErrorString(cudaGetLastError())));
+    *out = s;
+    return DVM_OK;
+}
+
+int dvm_set_option(dvm_solver *s, int option, int value)
+{
+    if (!s) return fail(DVM_EINVAL, "NULL solver");
+    if (option == DVM_OPT_KERNEL) {
+        if (s->planned) return fail(DVM_EINVAL, "kernel variant must be chosen before the first iteration");
+        if (value < DVM_KERNEL_AUTO || value > DVM_KERNEL_TILE) return fail(DVM_EINVAL, "unknown kernel variant %d", value);
+        s->kernel = value;
+        return DVM_OK;
+    }
+    return fail(DVM_EINVAL, "unknown option %d", option);
+}
+
+int dvm_iterate(dvm_solver *s, int niter)
+{
+    if (!s || niter < 0) return fail(DVM_EINVAL, "bad argument");
+    if (niter == 0) return DVM_OK;
+    if (int rc = plan(s)) return rc;
+    const UpdateParams U = update_params(s);
+    const SweepParams P = sweep_params(s);
+    for (int it = 0; it < niter; ++it) {
+        CK(cudaMemsetAsync(s->d_raw, 0, (size_t)16 * s->ncell * sizeof(double), s->stream));
+        CK(cudaMemsetAsync(s->d_phi, 0, (size_t)s->nface * sizeof(double), s->stream));
+        if (s->kernel == DVM_KERNEL_SLICE) {
+            CK(launch_sweep_slice(P, (int)s->blocks.size(), s->nb_threads, s->stream));
+        } else {
+            CK(launch_sweep_tile(P, s->tile, (int)s->blocks.size(), s->stream));
+        }
+        s->launches += 1;
+        int l = 0;
+        CK(launch_update(U, s->iters % HIST_CAP, s->stream, &l));
+        s->launches += l;
+        s->iters += 1;
+    }
+    return DVM_OK;
+}
+
+int dvm_moments(dvm_solver *s, double *dev_out)
+{
+    if (!s || !dev_out) return fail(DVM_EINVAL, "NULL argument");
+    CK(cudaMemcpyAsync(dev_out, s->d_prim, (size_t)NPRIM * s->ncell * sizeof(double), cudaMemcpyDeviceToDevice, s->stream));
+    return DVM_OK;
+}
+
+int dvm_residual(dvm_solver *s, double *host_out3)
+{
+    if (!s || !host_out3) return fail(DVM_EINVAL, "NULL argument");
+    if (s->iters == 0) return fail(DVM_EINVAL, "no iteration done yet");
+    const int slot = (s->iters - 1) % HIST_CAP;
+    CK(cudaMemcpyAsync(host_out3, s->d_hist + 3 * slot, 3 * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+    CK(cudaStreamSynchronize(s->stream));
+    for (int m = 0; m < 3; ++m)
+        if (!std::isfinite(host_out3[m])) return fail(DVM_ENONFINITE, "residual %d is not finite", m);
+    return DVM_OK;
+}
+
+int dvm_num_faces(const dvm_solver *s) { return s ? s->nface : fail(DVM_EINVAL, "NULL solver"); }
+int dvm_iterations_done(const dvm_solver *s) { return s ? s->iters : fail(DVM_EINVAL, "NULL solver"); }
+int dvm_kernel_used(const dvm_solver *s) { return s ? s->kernel : fail(DVM_EINVAL, "NULL solver"); }
+long long dvm_launch_count(const dvm_solver *s) { return s ? s->launches : -1; }
+
+int dvm_get_state(dvm_solver *s, double *dev_prim14, double *dev_rho_wall)
+{
+    if (!s) return fail(DVM_EINVAL, "NULL solver");
+    if (dev_prim14) CK(cudaMemcpyAsync(dev_prim14, s->d_prim, (size_t)NPRIM * s->ncell * sizeof(double), cudaMemcpyDeviceToDevice, s->stream));
+    if (dev_rho_wall) CK(cudaMemcpyAsync(dev_rho_wall, s->d_rho_w, (size_t)s->nface * sizeof(double), cudaMemcpyDeviceToDevice, s->stream));
+    return DVM_OK;
+}
+
+int dvm_set_state(dvm_solver *s, const double *dev_prim8, const double *dev_rho_wall)
+{
+    if (!s || !dev_prim8) return fail(DVM_EINVAL, "NULL argument");
+    CK(cudaMemcpyAsync(s->d_prim, dev_prim8, (size_t)8 * s->ncell * sizeof(double), cudaMemcpyDeviceToDevice, s->stream));
+    CK(cudaMemsetAsync(s->d_prim + 8 * s->ncell, 0, (size_t)6 * s->ncell * sizeof(double), s->stream));
+    if (dev_rho_wall) CK(cudaMemcpyAsync(s->d_rho_w, dev_rho_wall, (size_t)s->nface * sizeof(double), cudaMemcpyDeviceToDevice, s->stream));
+    const UpdateParams U = update_params(s);
+    CK(launch_pack(U, s->stream));
+    s->launches += 1;
+    return DVM_OK;
+}
+
+int dvm_raw_moments(dvm_solver *s, double *dev_raw13)
+{
+    if (!s || !dev_raw13) return fail(DVM_EINVAL, "NULL argument");
+    CK(cudaMemcpyAsync(dev_raw13, s->d_raw, (size_t)NRAW * s->ncell * sizeof(double), cudaMemcpyDeviceToDevice, s->stream));
+    return DVM_OK;
+}
+
+int dvm_wall_flux(dvm_solver *s, double *dev_flux)
+{
+    if (!s || !dev_flux) return fail(DVM_EINVAL, "NULL argument");
+    CK(cudaMemcpyAsync(dev_flux, s->d_phi, (size_t)s->nface * sizeof(double), cudaMemcpyDeviceToDevice, s->stream));
+    return DVM_OK;
+}
+
+int dvm_residual_history(dvm_solver *s, double *host_out, int max_n)
+{
+    if (!s || !host_out || max_n < 0) return fail(DVM_EINVAL, "bad argument");
+    const int count = std::min(std::min(max_n, s->iters), HIST_CAP);
+    if (count > 0) {
+        const int slot = (s->iters - count) % HIST_CAP;
+        const int run1 = std::min(count, HIST_CAP - slot);
+        CK(cudaMemcpyAsync(host_out, s->d_hist + 3 * slot, (size_t)3 * run1 * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+        if (count > run1)
+            CK(cudaMemcpyAsync(host_out + 3 * run1, s->d_hist, (size_t)3 * (count - run1) * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+    }
+    CK(cudaStreamSynchronize(s->stream));
+    return count;
+}
+
+int dvm_mass_scale(dvm_solver *s, double *host_out1)
+{
+    if (!s || !host_out1) return fail(DVM_EINVAL, "NULL argument");
+    if (s->iters == 0) { *host_out1 = 1.0; return DVM_OK; }
+    CK(cudaMemcpyAsync(host_out1, s->d_scal, sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+    CK(cudaStreamSynchronize(s->stream));
+    return DVM_OK;
+}
+
+int dvm_step_host(dvm_solver *s, const double *host_prim8, const double *host_rho_wall, int n,
+                  double *host_prim14_out, double *host_rho_wall_out)
+{
+    if (!s || n < 0) return fail(DVM_EINVAL, "bad argument");
+    if (host_prim8) {
+        CK(cudaMemcpyAsync(s->d_prim, host_prim8, (size_t)8 * s->ncell * sizeof(double), cudaMemcpyHostToDevice, s->stream));
+        CK(cudaMemsetAsync(s->d_prim + 8 * s->ncell, 0, (size_t)6 * s->ncell * sizeof(double), s->stream));
+        const UpdateParams U = update_params(s);
+        CK(launch_pack(U, s->stream));
+        s->launches += 1;
+    }
+    if (host_rho_wall) CK(cudaMemcpyAsync(s->d_rho_w, host_rho_wall, (size_t)s->nface * sizeof(double), cudaMemcpyHostToDevice, s->stream));
+    if (int rc = dvm_iterate(s, n)) return rc;
+    if (host_prim14_out) CK(cudaMemcpyAsync(host_prim14_out, s->d_prim, (size_t)NPRIM * s->ncell * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+    if (host_rho_wall_out) CK(cudaMemcpyAsync(host_rho_wall_out, s->d_rho_w, (size_t)s->nface * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+    CK(cudaStreamSynchronize(s->stream));
+    return DVM_OK;
+}
+
+int dvm_workspace_bytes(const dvm_solver *s, size_t *total, size_t *f_bytes)
+{
+    if (!s) return fail(DVM_EINVAL, "NULL solver");
+    if (total) *total = s->total_bytes;
+    if (f_bytes) *f_bytes = s->f_bytes;
+    return DVM_OK;
+}
+
+int dvm_destroy(dvm_solver *s)
+{
+    if (!s) return DVM_OK;
+    cudaStreamSynchronize(s->stream);
+    s->dfree_all();
+    delete s;
+    return DVM_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,281 @@
+"""Thin Python binding of the C ABI in include/dvm.h (same names; argument marshalling only).
+
+Every step of the hot path runs in the CUDA kernels of libdvm_b200.so.  PyTorch is used for device
+memory (the solver's workspace is obtained through the torch caching allocator), streams and nothing
+else.  There is no CPU fallback: if the library is missing or no CUDA device is present this fails loudly.
+This module never imports anything under oracle/.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+from pathlib import Path
+
+import numpy as np
+
+_PKG = Path(__file__).resolve().parent
+_CSRC = _PKG / "csrc"
+_SO = _PKG / "libdvm_b200.so"
+_INCLUDE = _PKG.parent / "include"
+
+OK, EINVAL, ENOMEM, ECUDA, ENONFINITE = 0, -1, -2, -3, -4
+WALL_DIFFUSE, FREESTREAM, ZERO_GRADIENT = 0, 1, 2
+KERNEL_AUTO, KERNEL_SLICE, KERNEL_TILE = 0, 1, 2
+OPT_KERNEL = 1
+
+# every symbol include/dvm.h declares (checked by tests/test_abi.py)
+SYMBOLS = (
+    "dvm_create", "dvm_iterate", "dvm_moments", "dvm_residual", "dvm_num_faces", "dvm_iterations_done",
+    "dvm_get_state", "dvm_set_state", "dvm_raw_moments", "dvm_wall_flux", "dvm_residual_history",
+    "dvm_mass_scale", "dvm_step_host", "dvm_set_option", "dvm_workspace_bytes", "dvm_launch_count",
+    "dvm_kernel_used", "dvm_destroy", "dvm_last_error",
+)
+
+NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
+              "-Xcompiler", "-fPIC", "-shared"]
+
+
+class DvmError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"dvm error {code}: {msg}")
+        self.code = code
+
+
+def build(force: bool = False, verbose: bool = False) -> Path:
+    """Compile csrc/*.cu for sm_100a into libdvm_b200.so (in-tree)."""
+    srcs = sorted(_CSRC.glob("*.cu"))
+    deps = srcs + sorted(_CSRC.glob("*.cuh")) + [_INCLUDE / "dvm.h"]
+    if not force and _SO.exists() and _SO.stat().st_mtime >= max(p.stat().st_mtime for p in deps):
+        return _SO
+    tmp = _SO.with_suffix(f".{os.getpid()}.tmp")
+    cmd = ["nvcc", *NVCC_FLAGS, *(["-Xptxas", "-v"] if verbose else []), "-o", str(tmp), *map(str, srcs)]
+    subprocess.run(cmd, check=True)
+    os.replace(tmp, _SO)
+    return _SO
+
+
+_dp = C.POINTER(C.c_double)
+
+
+class _Grid(C.Structure):
+    _fields_ = [("nx", C.c_int), ("ny", C.c_int), ("nz", C.c_int), ("xf", _dp), ("yf", _dp), ("zf", _dp),
+                ("solid", C.POINTER(C.c_ubyte))]
+
+
+class _VGrid(C.Structure):
+    _fields_ = [("mx", C.c_int), ("my", C.c_int), ("mz", C.c_int), ("xi_x", _dp), ("xi_y", _dp), ("xi_z", _dp),
+                ("w_x", _dp), ("w_y", _dp), ("w_z", _dp)]
+
+
+class _Gas(C.Structure):
+    _fields_ = [("Kn", C.c_double), ("omega", C.c_double), ("Pr", C.c_double), ("rho0", C.c_double),
+                ("u0", C.c_double * 3), ("T0", C.c_double)]
+
+
+class _FaceBC(C.Structure):
+    _fields_ = [("type", C.c_int), ("T", C.c_double), ("rho", C.c_double), ("u", C.c_double * 3)]
+
+
+class _BC(C.Structure):
+    _fields_ = [("face", _FaceBC * 6), ("solid", _FaceBC), ("rescale_mass", C.c_int), ("wall_norm", C.c_int)]
+
+
+_ALLOC = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p)
+_FREE = C.CFUNCTYPE(None, C.c_void_p, C.c_void_p)
+
+
+class _Device(C.Structure):
+    _fields_ = [("stream", C.c_void_p), ("alloc", _ALLOC), ("free_", _FREE), ("ctx", C.c_void_p)]
+
+
+_lib = None
+
+
+def lib():
+    """Load libdvm_b200.so (building it if the sources are newer).  Raises if it cannot be had."""
+    global _lib
+    if _lib is None:
+        if not _SO.exists():
+            build()
+        L = C.CDLL(str(_SO))
+        vp = C.c_void_p
+        L.dvm_create.argtypes = [C.POINTER(_Grid), C.POINTER(_VGrid), C.POINTER(_Gas), C.POINTER(_BC),
+                                 C.POINTER(_Device), C.POINTER(vp)]
+        L.dvm_iterate.argtypes = [vp, C.c_int]
+        L.dvm_moments.argtypes = [vp, vp]
+        L.dvm_residual.argtypes = [vp, _dp]
+        L.dvm_num_faces.argtypes = [vp]
+        L.dvm_iterations_done.argtypes = [vp]
+        L.dvm_get_state.argtypes = [vp, vp, vp]
+        L.dvm_set_state.argtypes = [vp, vp, vp]
+        L.dvm_raw_moments.argtypes = [vp, vp]
+        L.dvm_wall_flux.argtypes = [vp, vp]
+        L.dvm_residual_history.argtypes = [vp, _dp, C.c_int]
+        L.dvm_mass_scale.argtypes = [vp, _dp]
+        L.dvm_step_host.argtypes = [vp, vp, vp, C.c_int, vp, vp]
+        L.dvm_set_option.argtypes = [vp, C.c_int, C.c_int]
+        L.dvm_workspace_bytes.argtypes = [vp, C.POINTER(C.c_size_t), C.POINTER(C.c_size_t)]
+        L.dvm_kernel_used.argtypes = [vp]
+        L.dvm_launch_count.argtypes = [vp]
+        L.dvm_launch_count.restype = C.c_longlong
+        L.dvm_destroy.argtypes = [vp]
+        L.dvm_last_error.restype = C.c_char_p
+        _lib = L
+    return _lib
+
+
+def _check(rc):
+    if rc < 0:
+        raise DvmError(rc, lib().dvm_last_error().decode())
+    return rc
+
+
+def _f64(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+class Solver:
+    """dvm_create / dvm_iterate / dvm_moments / dvm_residual (+ support calls) for one workload record."""
+
+    def __init__(self, wl, kernel: int = KERNEL_AUTO, device: str = "cuda:0"):
+        import torch
+        if not torch.cuda.is_available():
+            raise DvmError(ECUDA, "no CUDA device: the DVM solver has no CPU fallback")
+        self.torch = torch
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        self.wl = wl
+        self.ncell = wl.n_cells
+        L = lib()
+        keep = [_f64(x) for x in (wl.xf, wl.yf, wl.zf, wl.xi_x, wl.xi_y, wl.xi_z, wl.w_x, wl.w_y, wl.w_z)]
+        g = _Grid(wl.nx, wl.ny, wl.nz, *(a.ctypes.data_as(_dp) for a in keep[0:3]), None)
+        if wl.solid is not None:
+            solid = np.ascontiguousarray(wl.solid, dtype=np.uint8).reshape(-1)
+            g.solid = solid.ctypes.data_as(C.POINTER(C.c_ubyte))
+        v = _VGrid(wl.mx, wl.my, wl.mz, *(a.ctypes.data_as(_dp) for a in keep[3:9]))
+        gas = _Gas(wl.Kn, wl.omega, wl.Pr, wl.rho0, (C.c_double * 3)(*wl.u0), wl.T0)
+        bc = _BC()
+        for b, f in enumerate(list(wl.faces) + [wl.solid_bc]):
+            dst = bc.face[b] if b < 6 else bc.solid
+            dst.type, dst.T, dst.rho = f.type, f.T, f.rho
+            for d in range(3):
+                dst.u[d] = f.u[d]
+        bc.rescale_mass, bc.wall_norm = wl.rescale_mass, wl.wall_norm
+
+        # device memory comes from the torch caching allocator; tensors are kept alive in this dict
+        self._blocks = {}
+
+        def _alloc(nbytes, ctx):
+            try:
+                t = torch.empty(int(nbytes), dtype=torch.uint8, device=self.device)
+            except Exception:
+                return None
+            self._blocks[t.data_ptr()] = t
+            return t.data_ptr()
+
+        def _free(ptr, ctx):
+            self._blocks.pop(ptr, None)
+
+        self._alloc_cb, self._free_cb = _ALLOC(_alloc), _FREE(_free)
+        self.stream = torch.cuda.current_stream(self.device)
+        dev = _Device(self.stream.cuda_stream, self._alloc_cb, self._free_cb, None)
+        h = C.c_void_p()
+        _check(L.dvm_create(C.byref(g), C.byref(v), C.byref(gas), C.byref(bc), C.byref(dev), C.byref(h)))
+        self._h = h
+        self.nface = _check(L.dvm_num_faces(h))
+        if kernel != KERNEL_AUTO:
+            self.set_option(OPT_KERNEL, kernel)
+
+    # -- the four calls of the north star ---------------------------------------------------------
+    def iterate(self, n: int = 1):
+        _check(lib().dvm_iterate(self._h, n))
+
+    def moments(self, out=None):
+        out = self._dev_empty(14 * self.ncell) if out is None else out
+        _check(lib().dvm_moments(self._h, out.data_ptr()))
+        return out.view(14, self.ncell)
+
+    def residual(self):
+        r = np.zeros(3)
+        _check(lib().dvm_residual(self._h, r.ctypes.data_as(_dp)))
+        return r
+
+    # -- support calls ------------------------------------------------------------------------------
+    def _dev_empty(self, n):
+        return self.torch.empty(n, dtype=self.torch.float64, device=self.device)
+
+    def set_option(self, option, value):
+        _check(lib().dvm_set_option(self._h, option, value))
+
+    def iterations_done(self):
+        return _check(lib().dvm_iterations_done(self._h))
+
+    def get_state(self):
+        p, r = self._dev_empty(14 * self.ncell), self._dev_empty(max(self.nface, 1))
+        _check(lib().dvm_get_state(self._h, p.data_ptr(), r.data_ptr()))
+        return p.view(14, self.ncell), r[: self.nface]
+
+    def set_state(self, prim8, rho_w=None):
+        t = self.torch
+        p = t.as_tensor(np.ascontiguousarray(prim8, dtype=np.float64) if isinstance(prim8, np.ndarray) else prim8,
+                        device=self.device).contiguous()
+        assert p.numel() == 8 * self.ncell
+        r = None
+        if rho_w is not None:
+            r = t.as_tensor(np.ascontiguousarray(rho_w, dtype=np.float64) if isinstance(rho_w, np.ndarray) else rho_w,
+                            device=self.device).contiguous()
+            assert r.numel() == self.nface
+        _check(lib().dvm_set_state(self._h, p.data_ptr(), None if r is None else r.data_ptr()))
+        t.cuda.current_stream(self.device).synchronize()
+
+    def raw_moments(self):
+        out = self._dev_empty(13 * self.ncell)
+        _check(lib().dvm_raw_moments(self._h, out.data_ptr()))
+        return out.view(13, self.ncell)
+
+    def wall_flux(self):
+        out = self._dev_empty(max(self.nface, 1))
+        _check(lib().dvm_wall_flux(self._h, out.data_ptr()))
+        return out[: self.nface]
+
+    def residual_history(self, max_n=1 << 14):
+        buf = np.zeros(3 * max(max_n, 1))
+        n = _check(lib().dvm_residual_history(self._h, buf.ctypes.data_as(_dp), max_n))
+        return buf[: 3 * n].reshape(n, 3)
+
+    def mass_scale(self):
+        v = C.c_double()
+        _check(lib().dvm_mass_scale(self._h, C.byref(v)))
+        return v.value
+
+    def step_host(self, host_prim8, host_rho_w, n, host_prim14_out, host_rho_w_out):
+        """End-to-end call with HOST (pinned torch or numpy) buffers; copies run inside the call."""
+        def ptr(x):
+            if x is None:
+                return None
+            return x.data_ptr() if hasattr(x, "data_ptr") else x.ctypes.data
+        _check(lib().dvm_step_host(self._h, ptr(host_prim8), ptr(host_rho_w), n, ptr(host_prim14_out), ptr(host_rho_w_out)))
+
+    def workspace_bytes(self):
+        a, b = C.c_size_t(), C.c_size_t()
+        _check(lib().dvm_workspace_bytes(self._h, C.byref(a), C.byref(b)))
+        return a.value, b.value
+
+    def kernel_used(self):
+        return _check(lib().dvm_kernel_used(self._h))
+
+    def launch_count(self):
+        return int(lib().dvm_launch_count(self._h))
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().dvm_destroy(self._h)
+            self._h = None
+            self._blocks.clear()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
