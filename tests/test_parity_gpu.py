@@ -53,7 +53,7 @@ def lockstep(wl, kernel, iters, oracle_mod, state=None, rho_w=None, check_raw=Tr
         assert_residual(s.residual(), o.resid, what=f"{wl.name} iteration {it + 1}")
         g_rw = s.get_state()[1].cpu().numpy()
         assert np.abs(g_rw - o.rho_w).max() <= 1e-11 * np.abs(o.rho_w).max()
-        assert abs(s.mass_scale() - o.scale) <= 1e-12
+        assert abs(s.mass_scale() - o.scale) <= 1e-12 * abs(o.scale)
         if check_raw:
             graw = s.raw_moments().cpu().numpy()
             for m in range(13):
