@@ -53,7 +53,7 @@ extern "C" {
 /* sweep-kernel variants (dvm_set_option DVM_OPT_KERNEL) */
 #define DVM_KERNEL_AUTO   0
 #define DVM_KERNEL_SLICE  1 /* the paper's mapping (thread = velocity, z-slice in HBM), fp64, in-place slice */
-#define DVM_KERNEL_TILE   2 /* B200 design: on-chip z-column tiles, DMMA moment contraction */
+#define DVM_KERNEL_TILE   2 /* B200 design: z-column tiles with the plane in registers, faces via TMA */
 
 #define DVM_OPT_KERNEL    1
 
@@ -143,6 +143,12 @@ int dvm_set_option(dvm_solver *s, int option, int value);
 /* Sweep-kernel variant in use: DVM_KERNEL_SLICE / DVM_KERNEL_TILE once the first dvm_iterate has planned the
  * workspace, the requested value (possibly DVM_KERNEL_AUTO) before. */
 int dvm_kernel_used(const dvm_solver *s);
+/* Host-only (needs no device): the work decomposition the tile kernel would use for an nx x ny x nz grid and the
+ * velocity nodes of v when target_ctas items should run concurrently.  counts4 = number of velocity blocks, tiles
+ * along x, tiles along y, band height P.  items8 (may be NULL) receives, for the first max_items work items in
+ * hand-out order, {velocity block, tile x, tile y, predecessor in x, predecessor in y, previous user of the x-face
+ * slot, x-face slot, octant bits}; predecessors are item indices or -1.  Returns the number of items. */
+int dvm_plan_query(int nx, int ny, int nz, const dvm_vgrid *v, int target_ctas, int *counts4, int *items8, int max_items);
 /* Bytes of device workspace held by the solver, and the part of it that holds distribution-function values. */
 int dvm_workspace_bytes(const dvm_solver *s, size_t *total, size_t *f_bytes);
 /* Number of kernel launches enqueued by this solver so far (bench.py's gpu_launches). */

@@ -77,6 +77,15 @@ struct dvm_solver {
     long long fstride = 0;
     int nb_threads = 128;
     TilePlan tile{};
+    unsigned char *d_sflags = nullptr;
+    double *d_gtab = nullptr;
+    int gstride = 0;
+    int foff[6] = {0, 0, 0, 0, 0, 0};
+    VBlock *d_vblocks = nullptr;
+    TileItem *d_items = nullptr;
+    int *d_done = nullptr, *d_counter = nullptr;
+    double *d_xface = nullptr, *d_yface = nullptr;
+    int tile_grid = 0, epoch = 0;
     std::vector<double> h_rho_w0;
 
     void *dalloc(size_t bytes)
@@ -169,6 +178,26 @@ SweepParams sweep_params(dvm_solver *s)
     return P;
 }
 
+TileParams tile_params(dvm_solver *s)
+{
+    TileParams P{};
+    P.nx = s->nx; P.ny = s->ny; P.nz = s->nz; P.ntx = s->tile.ntx; P.nty = s->tile.nty; P.P = s->tile.P;
+    P.ncell = s->ncell;
+    P.invdx = s->d_invdx; P.invdy = s->d_invdy; P.invdz = s->d_invdz;
+    P.flags = s->d_flags; P.sflags = s->d_sflags; P.face_of = s->d_face_of;
+    P.coef = s->d_coef; P.rho_w = s->d_rho_w; P.phi = s->d_phi; P.raw16 = s->d_raw;
+    P.xi_x = s->d_xi[0]; P.xi_y = s->d_xi[1]; P.xi_z = s->d_xi[2];
+    P.w_x = s->d_w[0]; P.w_y = s->d_w[1]; P.w_z = s->d_w[2];
+    P.gtab = s->d_gtab; P.gstride = s->gstride;
+    for (int b = 0; b < 7; ++b) P.bc_type[b] = slot_bc(s->bc, b).type;
+    for (int d = 0; d < 6; ++d) P.foff[d] = s->foff[d];
+    P.vblocks = s->d_vblocks; P.items = s->d_items; P.nitems = (int)s->tile.items.size();
+    P.done = s->d_done; P.counter = s->d_counter; P.epoch = s->epoch;
+    P.xface = s->d_xface; P.yface = s->d_yface;
+    P.slot_doubles = (long long)s->nz * TILE_TY * TILE_NVB;
+    return P;
+}
+
 // index ranges of the negative / non-negative nodes of one axis (nodes ascending)
 void split_axis(const std::vector<double> &xi, int lo[2], int cnt[2])
 {
@@ -183,9 +212,7 @@ int plan(dvm_solver *s)
     if (s->planned) return 0;
     const long long nvel = (long long)s->mx * s->my * s->mz;
     int kernel = s->kernel;
-    if (kernel == DVM_KERNEL_AUTO) kernel = tile_supported(s->nx, s->ny, s->nz) ? DVM_KERNEL_TILE : DVM_KERNEL_SLICE;
-    if (kernel == DVM_KERNEL_TILE && !tile_supported(s->nx, s->ny, s->nz))
-        return fail(DVM_EINVAL, "tile kernel does not support this grid");
+    if (kernel == DVM_KERNEL_AUTO) kernel = DVM_KERNEL_TILE;
     s->kernel = kernel;
     int lo[3][2], cnt[3][2];
     for (int d = 0; d < 3; ++d) split_axis(s->xi[d], lo[d], cnt[d]);
@@ -213,12 +240,27 @@ int plan(dvm_solver *s)
         if (!s->d_fbuf) return fail(DVM_ENOMEM, "slice workspace of %zu bytes failed", fbytes);
         s->f_bytes = fbytes;
     } else {
-        int rc = tile_plan(s->nx, s->ny, s->nz, lo, cnt, nvel, &s->tile, &s->blocks);
-        if (rc) return fail(DVM_EINVAL, "tile plan failed");
-        const size_t fbytes = s->tile.fbuf_doubles * sizeof(double);
-        s->d_fbuf = (double *)s->dalloc(fbytes);
-        if (!s->d_fbuf) return fail(DVM_ENOMEM, "tile face workspace of %zu bytes failed", fbytes);
+        int per_sm = 0, dev = 0, nsm = 0;
+        CK(tile_configure(&per_sm));
+        CK(cudaGetDevice(&dev));
+        CK(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
+        if (per_sm < 1) return fail(DVM_ECUDA, "tile kernel does not fit on an SM");
+        const int resident = per_sm * nsm;
+        if (tile_plan(s->nx, s->ny, s->nz, s->xi, resident, &s->tile)) return fail(DVM_EINVAL, "tile plan failed");
+        const size_t nitems = s->tile.items.size();
+        s->tile_grid = (int)std::min<size_t>((size_t)resident, nitems);
+        const size_t fbytes = (s->tile.xface_doubles + s->tile.yface_doubles) * sizeof(double);
+        s->d_xface = (double *)s->dalloc(s->tile.xface_doubles * sizeof(double));
+        s->d_yface = (double *)s->dalloc(s->tile.yface_doubles * sizeof(double));
+        if (!s->d_xface || !s->d_yface) return fail(DVM_ENOMEM, "tile face workspace of %zu bytes failed", fbytes);
         s->f_bytes = fbytes;
+        if (upload(s, &s->d_vblocks, s->tile.vblocks.data(), s->tile.vblocks.size())) return DVM_ENOMEM;
+        if (upload(s, &s->d_items, s->tile.items.data(), nitems)) return DVM_ENOMEM;
+        if (dzeros(s, &s->d_done, nitems)) return DVM_ENOMEM;
+        if (dzeros(s, &s->d_counter, 64)) return DVM_ENOMEM;
+        CK(cudaStreamSynchronize(s->stream));  // the host vectors above are read asynchronously
+        s->planned = true;
+        return 0;
     }
     if (upload(s, &s->d_blocks, s->blocks.data(), s->blocks.size())) return DVM_ENOMEM;
     s->planned = true;
@@ -287,7 +329,7 @@ int dvm_create(const dvm_grid *g, const dvm_vgrid *v, const dvm_gas *gas, const 
     for (int j = 0; j < ny; ++j) { dy[j] = s->yf[j + 1] - s->yf[j]; idy[j] = 1.0 / dy[j]; }
     for (int k = 0; k < nz; ++k) { dz[k] = s->zf[k + 1] - s->zf[k]; idz[k] = 1.0 / dz[k]; }
     // ---- cell flags, boundary-face table (order stated in dvm.h) ----
-    std::vector<unsigned char> flags((size_t)n, 0);
+    std::vector<unsigned char> flags((size_t)n, 0), sflags((size_t)n, 0);
     std::vector<int> face_of((size_t)6 * n, -1);
     const int off[6] = {0, ny * nz, 2 * ny * nz, 2 * ny * nz + nx * nz, 2 * ny * nz + 2 * nx * nz,
                         2 * ny * nz + 2 * nx * nz + nx * ny};
@@ -300,7 +342,7 @@ int dvm_create(const dvm_grid *g, const dvm_vgrid *v, const dvm_gas *gas, const 
     for (int k = 0; k < nz; ++k) for (int j = 0; j < ny; ++j) for (int i = 0; i < nx; ++i) {
         const long long c = ((long long)k * ny + j) * nx + i;
         const bool cs = sol(i, j, k);
-        if (cs) flags[c] |= FLAG_SOLID;
+        if (cs) { flags[c] |= FLAG_SOLID; sflags[c] |= FLAG_SOLID; }
         else mass0 += gas->rho0 * (dx[i] * dy[j] * dz[k]);
         for (int d = 0; d < 6; ++d) {
             const int ii = i + di[d], jj = j + dj[d], kk = k + dk[d];
@@ -317,6 +359,7 @@ int dvm_create(const dvm_grid *g, const dvm_vgrid *v, const dvm_gas *gas, const 
                 if (!cs) { face_cell[f] = (int)c; face_of[(size_t)d * n + c] = f; }
             } else if (sol(ii, jj, kk)) {
                 flags[c] |= (unsigned char)(1u << d);
+                sflags[c] |= (unsigned char)(1u << d);
                 if (!cs) {
                     const int f = (int)face_slot.size();
                     face_slot.push_back(6); face_cell.push_back((int)c); face_dir.push_back(d);
@@ -327,6 +370,22 @@ int dvm_create(const dvm_grid *g, const dvm_vgrid *v, const dvm_gas *gas, const 
     }
     s->nface = (int)face_slot.size();
     s->mass0 = mass0;
+    for (int d = 0; d < 6; ++d) s->foff[d] = off[d];
+    // ---- 1-D factors of the ghost distributions (tile kernel): per BC slot and axis, w(xi) exp(-(xi-u)^2/T), with
+    //      (pi T)^{-3/2} (and rho of a free stream) folded into the x factor; zero for zero-gradient slots ----
+    s->gstride = std::max(s->mx, std::max(s->my, s->mz));
+    std::vector<double> gtab((size_t)7 * 3 * s->gstride, 0.0);
+    for (int b = 0; b < 7; ++b) {
+        const dvm_face_bc &f = slot_bc(*bc, b);
+        if (f.type == DVM_ZERO_GRADIENT) continue;
+        for (int d = 0; d < 3; ++d) {
+            const double pref = d == 0 ? (f.type == DVM_FREESTREAM ? f.rho : 1.0) / std::pow(PI * f.T, 1.5) : 1.0;
+            for (size_t m = 0; m < s->xi[d].size(); ++m) {
+                const double c1 = s->xi[d][m] - f.u[d];
+                gtab[((size_t)b * 3 + d) * s->gstride + m] = pref * s->w[d][m] * std::exp(-c1 * c1 / f.T);
+            }
+        }
+    }
     // ---- Phi_unit per (bc slot, direction) and Phi^0 per direction (oracle step 1; Eq.(9) with weights) ----
     double tab[7][6] = {}, phi0[6] = {};
     {
@@ -371,6 +430,8 @@ int dvm_create(const dvm_grid *g, const dvm_vgrid *v, const dvm_gas *gas, const 
     rc |= upload(s, &s->d_invdz, idz.data(), nz);
     rc |= upload(s, &s->d_dx, dx.data(), nx); rc |= upload(s, &s->d_dy, dy.data(), ny); rc |= upload(s, &s->d_dz, dz.data(), nz);
     rc |= upload(s, &s->d_flags, flags.data(), (size_t)n);
+    rc |= upload(s, &s->d_sflags, sflags.data(), (size_t)n);
+    rc |= upload(s, &s->d_gtab, gtab.data(), gtab.size());
     rc |= upload(s, &s->d_face_of, face_of.data(), (size_t)6 * n);
     rc |= upload(s, &s->d_face_slot, face_slot.data(), (size_t)s->nface);
     for (int d = 0; d < 3; ++d) {
@@ -434,7 +495,10 @@ int dvm_iterate(dvm_solver *s, int niter)
         if (s->kernel == DVM_KERNEL_SLICE) {
             CK(launch_sweep_slice(P, (int)s->blocks.size(), s->nb_threads, s->stream));
         } else {
-            CK(launch_sweep_tile(P, s->tile, (int)s->blocks.size(), s->stream));
+            CK(cudaMemsetAsync(s->d_counter, 0, sizeof(int), s->stream));
+            s->epoch += 1;
+            const TileParams TP = tile_params(s);
+            CK(launch_sweep_tile(TP, s->tile_grid, s->stream));
         }
         s->launches += 1;
         int l = 0;
@@ -492,7 +556,8 @@ int dvm_set_state(dvm_solver *s, const double *dev_prim8, const double *dev_rho_
 int dvm_raw_moments(dvm_solver *s, double *dev_raw13)
 {
     if (!s || !dev_raw13) return fail(DVM_EINVAL, "NULL argument");
-    CK(cudaMemcpyAsync(dev_raw13, s->d_raw, (size_t)NRAW * s->ncell * sizeof(double), cudaMemcpyDeviceToDevice, s->stream));
+    CK(launch_raw_export(s->d_raw, dev_raw13, s->ncell, s->stream));
+    s->launches += 1;
     return DVM_OK;
 }
 
@@ -544,6 +609,28 @@ int dvm_step_host(dvm_solver *s, const double *host_prim8, const double *host_rh
     if (host_rho_wall_out) CK(cudaMemcpyAsync(host_rho_wall_out, s->d_rho_w, (size_t)s->nface * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
     CK(cudaStreamSynchronize(s->stream));
     return DVM_OK;
+}
+
+int dvm_plan_query(int nx, int ny, int nz, const dvm_vgrid *v, int target_ctas, int *counts4, int *items8, int max_items)
+{
+    if (!v || !counts4 || nx <= 0 || ny <= 0 || nz <= 0 || v->mx <= 0 || v->my <= 0 || v->mz <= 0 || !v->xi_x || !v->xi_y || !v->xi_z)
+        return fail(DVM_EINVAL, "bad argument");
+    std::vector<double> xi[3];
+    xi[0].assign(v->xi_x, v->xi_x + v->mx); xi[1].assign(v->xi_y, v->xi_y + v->my); xi[2].assign(v->xi_z, v->xi_z + v->mz);
+    TilePlan tp;
+    if (tile_plan(nx, ny, nz, xi, target_ctas, &tp)) return fail(DVM_EINVAL, "tile plan failed");
+    counts4[0] = (int)tp.vblocks.size(); counts4[1] = tp.ntx; counts4[2] = tp.nty; counts4[3] = tp.P;
+    const int n = (int)tp.items.size();
+    if (items8) {
+        for (int e = 0; e < n && e < max_items; ++e) {
+            const TileItem &it = tp.items[e];
+            const VBlock &vb = tp.vblocks[it.vb];
+            int *o = items8 + 8 * e;
+            o[0] = it.vb; o[1] = it.ti; o[2] = it.tj; o[3] = it.pred_x; o[4] = it.pred_y; o[5] = it.pred_s; o[6] = it.xslot;
+            o[7] = (vb.sx > 0) | ((vb.sy > 0) << 1) | ((vb.sz > 0) << 2);
+        }
+    }
+    return n;
 }
 
 int dvm_workspace_bytes(const dvm_solver *s, size_t *total, size_t *f_bytes)

@@ -37,7 +37,7 @@ struct SweepParams {
     const double *coef;             // [NCOEF][ncell]
     const double *rho_w;            // [nface]
     double *phi;                    // [nface] wall-incident flux accumulators
-    double *raw;                    // [NRAW][ncell] accumulators
+    double *raw;                    // [ncell][16] accumulators (NRAW used)
     const double *xi_x, *xi_y, *xi_z, *w_x, *w_y, *w_z;
     const BlockDesc *blocks;
     double *fbuf;                   // distribution-function workspace (slices / tile faces)

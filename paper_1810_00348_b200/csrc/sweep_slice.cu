@@ -115,7 +115,7 @@ __global__ void __launch_bounds__(NB) sweep_slice_kernel(const SweepParams P)
                 for (int q = 0; q < NRAW; ++q) m[q] = warp_sum(m[q]);
                 if (lane == 0) {
 #pragma unroll
-                    for (int q = 0; q < NRAW; ++q) atomicAdd(P.raw + q * nc + c, m[q]);
+                    for (int q = 0; q < NRAW; ++q) atomicAdd(P.raw + c * 16 + q, m[q]);
                     // wall-incident flux (Eq.(9)): all velocities of the block share the sign of xi_d, so
                     // sum w |xi_d| f = s_d * (first-moment partial)
                     if (fl & (1u << dnx)) atomicAdd(P.phi + P.face_of[dnx * nc + c], sx * m[1]);

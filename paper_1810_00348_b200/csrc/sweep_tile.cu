@@ -1,8 +1,604 @@
-// sweep_tile.cu - DVM_KERNEL_TILE (placeholder until the tile kernel lands: reports "unsupported")
+// sweep_tile.cu - DVM_KERNEL_TILE: the B200 sweep kernel of the DVM iteration (arXiv 1810.00348).
+//
+// What it computes is exactly Alg. 1-3 of the paper: for every discrete velocity the
+// first-order upwind recurrence Eq.(7) over the whole physical grid with the Shakhov
+// equilibrium Eq.(2) rebuilt on the fly, diffuse-wall / free-stream / zero-gradient ghosts
+// (Eq.(8)-(9)), and the velocity sums Eq.(5) plus the wall-incident fluxes
+// taken as each value is produced, so that f is never stored.  How it computes it is new:
+//
+//  * work item = (velocity block of 512 velocities of one sign octant) x (4 x 4 z-column of cells); a CTA of 128
+//    threads owns an item, a thread owns 4 velocities (consecutive xi_x nodes) and keeps the 4 x 4 x 4 values of
+//    the current z-plane in registers: x-, y- and z-upwind operands of interior cells are register operands;
+//  * what is carried is g = w_alpha f_alpha (the recurrence is linear in f), so quadrature weights cost nothing;
+//  * exp(-|xi-U|^2/T) factorises per axis on the tensor velocity grid: per cell and level the CTA builds tables of
+//    16 + nbb + ncb one-dimensional factors in shared memory (one exp per entry, not per phase point);
+//  * the division of Eq.(7) is MUFU.RCP64H + one cubic Newton step (3 DFMA, < 1 ulp);
+//  * the 13 velocity sums use the tensor structure: 4 power sums over the thread's xi_x nodes (4 DFMA / point),
+//    a lane-quad exchange over the 16 xi_x nodes of the block, then each lane expands its share of the 16
+//    (power of xi_x) x (monomial of xi_y, xi_z) products and a transposing butterfly over the 8 lane groups leaves
+//    one partial per lane, which goes to the [cell][16] accumulator in L2/HBM as one coalesced fp64 RED per
+//    (cell, warp);
+//  * the x- and y-faces of the column are the only f-traffic: written with coalesced 32-byte stores per thread,
+//    read back by the downwind item with TMA bulk copies (cp.async.bulk + mbarrier) two levels ahead;
+//  * items are handed out by an atomic counter in dependency order (tile_plan.cu); done-flags gate their start.
+//
+// Product code: shares nothing with oracle/.
 #include "sweep_tile.cuh"
 
+#include <cstdint>
+
 namespace dvm {
-bool tile_supported(int, int, int) { return false; }
-int tile_plan(int, int, int, const int[3][2], const int[3][2], long long, TilePlan *, std::vector<BlockDesc> *) { return -1; }
-cudaError_t launch_sweep_tile(const SweepParams &, const TilePlan &, int, cudaStream_t) { return cudaErrorNotSupported; }
+
+namespace {
+
+constexpr int NVB = TILE_NVB;
+constexpr int NCELL = TILE_NCELL;
+constexpr int LEVEL_DOUBLES = 4 * NVB;                 // one level of an x- or y-face slot
+constexpr unsigned LEVEL_BYTES = LEVEL_DOUBLES * 8u;   // 16 KB
+
+struct __align__(128) TileSmem {
+    double xface[2][TILE_TY][NVB];                 // staged x-face input, per level parity
+    double yface[2][TILE_TX][NVB];                 // staged y-face input
+    double4 xtab[2][NCELL][TILE_NA];               // per (cell, xi_x node): E, Q, e, a   (node index r*4 + ag)
+    double4 yztab[2][NCELL][TILE_MAXBC];           // per (cell, xi_y node) then (cell, xi_z node)
+    double nu[2][NCELL];                           // 1/tau (1 for dead cells)
+    double4 spec[2][NCELL];                        // rho_w of a solid ghost in x, y, z (special levels)
+    double stage[2][NCELL][10];                    // coef pack (9) of a level, prefetched two levels ahead
+    double rwb[2][8];                              // ghost densities of the domain faces: 4 x-face rows, 4 y-face columns
+    double invdz[2];
+    double xi_a[TILE_NA], w_a[TILE_NA];            // nodes / weights of the block (0 beyond the box)
+    double xi_bc[TILE_MAXBC], w_bc[TILE_MAXBC];
+    double g[4][3][16];                            // ghost Maxwellian 1-D factors: upwind x, y, z face and solid
+    double invdx[TILE_TX], invdy[TILE_TY];
+    int cflag[2][NCELL];                           // flags | sflags << 8 | in-domain << 16, staged
+    int code[2][NCELL];                            // 1: x-up solid ghost, 2: y-up, 4: z-up, 8: dead cell
+    int cidx[2][NCELL];                            // global cell index or -1 (dead)
+    int dnface[2][NCELL][4];                       // wall face downwind in x, y, z (or -1); [3] = -1
+    unsigned long long mbar[2];
+    int item;
+};
+
+// ---- PTX helpers -----------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(unsigned long long *b, unsigned count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(b)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long *b, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(b)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long *b, unsigned parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(b)), "r"(parity) : "memory");
+}
+// TMA 1-D bulk copy global -> shared, completion counted on an mbarrier
+__device__ __forceinline__ void tma_load(void *dst, const void *src, unsigned bytes, unsigned long long *b)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(smem_u32(b))
+                 : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async()
+{
+    asm volatile("fence.proxy.async;" ::: "memory");
+}
+__device__ __forceinline__ int ld_acquire(const int *p)
+{
+    int v;
+    asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_release(int *p, int v)
+{
+    asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+// 1/d: MUFU.RCP64H seed (about 20 bits) + one cubic Newton step: e = 1 - d y, y (1 + e + e^2); error ~ e^3
+__device__ __forceinline__ double fast_rcp(double d)
+{
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(d));
+    const double e = fma(-d, y, 1.0);
+    const double t = fma(e, e, e);
+    return fma(y, t, y);
+}
+__device__ __forceinline__ double shx(double v, int m) { return __shfl_xor_sync(0xffffffffu, v, m); }
+
+// moment index (order of dvm_raw_moments) of output j of lane type q = lane & 3
+//   q = 0: S0 {1, xi_y, xi_z, xi_y^2}        q = 1: S1 {1, xi_y, xi_z, xi_y^2 + xi_z^2}
+//   q = 2: S0 {xi_z^2, xi_y xi_z, xi_y r2, xi_z r2}   q = 3: S2 {1, xi_y, xi_z}, S3 {1}
+__constant__ int c_mom[4][4] = {{0, 2, 3, 5}, {1, 7, 8, 10}, {6, 9, 11, 12}, {4, 11, 12, 10}};
+
+// per-item constants, uniform over the CTA
+struct ItemCtx {
+    int sx, sy, sz;
+    int i0, j0;          // sweep-relative origin of the tile
+    int upx, upy, upz;   // direction ids of the upwind sides
+    int tpx, tpy, tpz;   // BC types of the upwind domain faces
+    int first_x, first_y;
+    int nbb, ncb;
+};
+
+__device__ __forceinline__ bool cell_of(const TileParams &P, const ItemCtx &I, int ii, int jj, int kp, int &i, int &j,
+                                        int &k)
+{
+    const int ip = I.i0 + ii, jp = I.j0 + jj;
+    i = I.sx > 0 ? ip : P.nx - 1 - ip;
+    j = I.sy > 0 ? jp : P.ny - 1 - jp;
+    k = I.sz > 0 ? kp : P.nz - 1 - kp;
+    return ip < P.nx && jp < P.ny;
+}
+
+// ghost density of a domain face cell: rho_w of a wall, 1 for a free stream (rho_inf is folded into the factors),
+// 0 for a dropped (zero-gradient) term
+__device__ __forceinline__ double face_density(const TileParams &P, int type, int slot)
+{
+    if (type == 0) return P.rho_w[slot];
+    return type == 1 ? 1.0 : 0.0;
+}
+
+// Loads of the per-level metadata of level kp (two values per thread, roles by tid); kept in registers while the
+// current level is computed, then written to shared memory by stage_store.
+__device__ __forceinline__ void stage_load(const TileParams &P, const ItemCtx &I, int kp, int tid, double &v0, double &v1)
+{
+    v0 = 0.0; v1 = 0.0;
+    if (kp >= P.nz) return;
+    int i, j, k;
+    {
+        const int cell = tid & 15, f = tid >> 4;
+        if (cell_of(P, I, cell & 3, cell >> 2, kp, i, j, k)) v0 = P.coef[(long long)f * P.ncell + ((long long)k * P.ny + j) * P.nx + i];
+    }
+    if (tid < 16) {
+        if (cell_of(P, I, tid & 3, tid >> 2, kp, i, j, k)) v1 = P.coef[8ll * P.ncell + ((long long)k * P.ny + j) * P.nx + i];
+    } else if (tid < 32) {
+        const int cell = tid - 16;
+        if (cell_of(P, I, cell & 3, cell >> 2, kp, i, j, k)) {
+            const long long c = ((long long)k * P.ny + j) * P.nx + i;
+            v1 = (double)((int)P.flags[c] | ((int)P.sflags[c] << 8) | (1 << 16));
+        }
+    } else if (tid < 36) {
+        if (I.first_x && cell_of(P, I, 0, tid - 32, kp, i, j, k)) v1 = face_density(P, I.tpx, P.foff[I.upx] + k * P.ny + j);
+    } else if (tid < 40) {
+        if (I.first_y && cell_of(P, I, tid - 36, 0, kp, i, j, k)) v1 = face_density(P, I.tpy, P.foff[I.upy] + k * P.nx + i);
+    } else if (tid == 40) {
+        cell_of(P, I, 0, 0, kp, i, j, k);
+        v1 = P.invdz[k];
+    }
+}
+
+__device__ __forceinline__ void stage_store(TileSmem &s, int b, int tid, double v0, double v1)
+{
+    s.stage[b][tid & 15][tid >> 4] = v0;
+    if (tid < 16) s.stage[b][tid][8] = v1;
+    else if (tid < 32) s.cflag[b][tid - 16] = (int)v1;
+    else if (tid < 40) s.rwb[b][tid - 32] = v1;
+    else if (tid == 40) s.invdz[b] = v1;
+}
+
+// Tables of level kp into buffer b = kp & 1 (reads stage[b], cflag[b], invdz[b]).  Returns 1 if this thread saw a
+// cell that needs the special path (solid ghost, solid or out-of-domain cell).
+__device__ __forceinline__ int build_tables(const TileParams &P, const ItemCtx &I, TileSmem &s, int kp, int tid)
+{
+    const int b = kp & 1;
+    int special = 0;
+    if (tid < 16) {
+        const int cell = tid, fl = s.cflag[b][cell];
+        int i, j, k;
+        cell_of(P, I, cell & 3, cell >> 2, kp, i, j, k);
+        const long long c = ((long long)k * P.ny + j) * P.nx + i;
+        const int flags = fl & 0xff, sfl = (fl >> 8) & 0xff;
+        const bool dead = !((fl >> 16) & 1) || (sfl & 64);
+        int code = 8;
+        double4 sp = make_double4(0.0, 0.0, 0.0, 0.0);
+        int dn[3] = {-1, -1, -1};
+        if (!dead) {
+            code = ((sfl >> I.upx) & 1) | (((sfl >> I.upy) & 1) << 1) | (((sfl >> I.upz) & 1) << 2);
+            if (code & 1) sp.x = P.rho_w[P.face_of[(long long)I.upx * P.ncell + c]];
+            if (code & 2) sp.y = P.rho_w[P.face_of[(long long)I.upy * P.ncell + c]];
+            if (code & 4) sp.z = P.rho_w[P.face_of[(long long)I.upz * P.ncell + c]];
+            const int up[3] = {I.upx, I.upy, I.upz};
+#pragma unroll
+            for (int d = 0; d < 3; ++d) {
+                const int dd = up[d] ^ 1;
+                if ((flags >> dd) & 1) dn[d] = P.face_of[(long long)dd * P.ncell + c];
+            }
+        }
+        s.code[b][cell] = code;
+        s.spec[b][cell] = sp;
+        s.cidx[b][cell] = dead ? -1 : (int)c;
+        s.nu[b][cell] = dead ? 1.0 : s.stage[b][cell][0];
+        s.dnface[b][cell][0] = dn[0]; s.dnface[b][cell][1] = dn[1]; s.dnface[b][cell][2] = dn[2];
+        s.dnface[b][cell][3] = -1;
+        special = code != 0;
+    }
+    const int nent = 16 * (TILE_NA + I.nbb + I.ncb);
+    for (int e = tid; e < nent; e += TILE_THREADS) {
+        const int cell = e & 15, n = e >> 4;
+        const int fl = s.cflag[b][cell];
+        const bool dead = !((fl >> 16) & 1) || ((fl >> 8) & 64);
+        const double *st = s.stage[b][cell];
+        const double invT = st[2];
+        double xi, w, u, q, h;
+        bool drop;
+        if (n < TILE_NA) {
+            const int al = 4 * (n & 3) + (n >> 2);   // table position r*4+ag  <->  node 4*ag + r
+            xi = s.xi_a[al]; w = s.w_a[al] * (st[0] * st[1]); u = st[3]; q = st[6];
+            h = s.invdx[cell & 3]; drop = (I.i0 + (cell & 3) == 0) && I.tpx == 2;
+        } else if (n < TILE_NA + I.nbb) {
+            const int bl = n - TILE_NA;
+            xi = s.xi_bc[bl]; w = s.w_bc[bl]; u = st[4]; q = st[7];
+            h = s.invdy[cell >> 2]; drop = (I.j0 + (cell >> 2) == 0) && I.tpy == 2;
+        } else {
+            const int cl = n - TILE_NA;
+            xi = s.xi_bc[cl]; w = s.w_bc[cl]; u = st[5]; q = st[8];
+            h = s.invdz[b]; drop = (kp == 0) && I.tpz == 2;
+        }
+        const double c1 = xi - u, t = c1 * c1 * invT;
+        double4 ent;
+        ent.x = w * exp(-t);
+        ent.y = q * c1;
+        ent.z = n < TILE_NA ? 2.0 * t - 5.0 : 2.0 * t;
+        ent.w = drop ? 0.0 : fabs(xi) * h;
+        if (dead) ent = make_double4(0.0, 0.0, 0.0, 0.0);
+        if (n < TILE_NA) s.xtab[b][cell][n] = ent;
+        else s.yztab[b][cell][n - TILE_NA] = ent;
+    }
+    return special;
+}
+
+// Ghost values of the domain faces of level kp (buffer b) for a tile at the upwind x / y edge of the domain
+__device__ __forceinline__ void fill_faces(const ItemCtx &I, TileSmem &s, int b, int tid, int ag, int yidx, int zidx)
+{
+    if (I.first_x) {
+        const double gyz = s.g[0][1][yidx] * s.g[0][2][zidx];
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+            const double G = s.g[0][0][4 * ag + r] * gyz;
+#pragma unroll
+            for (int jj = 0; jj < 4; ++jj) s.xface[b][jj][tid * 4 + r] = s.rwb[b][jj] * G;
+        }
+    }
+    if (I.first_y) {
+        const double gyz = s.g[1][1][yidx] * s.g[1][2][zidx];
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+            const double G = s.g[1][0][4 * ag + r] * gyz;
+#pragma unroll
+            for (int ii = 0; ii < 4; ++ii) s.yface[b][ii][tid * 4 + r] = s.rwb[b][4 + ii] * G;
+        }
+    }
+}
+
+// Reduction of the four power sums S_p = sum_r xi_x^p g_r of a lane over the warp (see the header comment):
+// returns, in every lane, one of the 16 partial products of the cell; lane & 15 names it (c_mom).
+__device__ __forceinline__ double reduce16(double S0, double S1, double S2, double S3, const double (&cf)[4], int lane)
+{
+    const bool b0 = lane & 1, b1 = lane & 2, b2 = lane & 4, b3 = lane & 8;
+    // lane quad = the 4 xi_x groups of one (xi_y, xi_z) pair
+    S0 += shx(S0, 1);
+    S0 += shx(S0, 2);
+    double u = (b1 ? S2 : S1) + shx(b1 ? S1 : S2, 2);
+    double v = S3 + shx(b1 ? 0.0 : S3, 2);
+    u += shx(u, 1);
+    v += shx(v, 1);
+    // lanes 0, 2 expand S0, lane 1 expands S1, lane 3 expands S2 (3 outputs) and S3 (1 output)
+    const double U = b0 ? u : S0;
+    const double V = (b0 && b1) ? v : U;
+    const double o0 = cf[0] * U, o1 = cf[1] * U, o2 = cf[2] * U, o3 = cf[3] * V;
+    // transposing butterfly over the 8 (xi_y, xi_z) pairs of the warp
+    const double k0 = (b2 ? o2 : o0) + shx(b2 ? o0 : o2, 4);
+    const double k1 = (b2 ? o3 : o1) + shx(b2 ? o1 : o3, 4);
+    double kk = (b3 ? k1 : k0) + shx(b3 ? k0 : k1, 8);
+    kk += shx(kk, 16);
+    return kk;
+}
+
+// per-thread constants of an item
+struct ThreadCtx {
+    double X1[4], X2[4], X3[4];  // xi_x, xi_x^2, xi_x^3 of the thread's nodes
+    double cf[4];                // expansion coefficients of this lane
+    double dsgn;                 // sign of the wall-flux contribution of this lane
+    int ag, yi, zi;              // xi_x group, table rows of the thread's xi_y and xi_z nodes
+    int mom, dsel;               // moment slot and wall-flux direction (3 = none) of this lane
+};
+
+// One level of the column: 4 rows x 4 cells x 4 velocities per thread, fully unrolled so that the plane lives in
+// registers.  SPECIAL adds solid ghosts and dead cells.
+template <bool SPECIAL>
+__device__ __forceinline__ void compute_level(const TileParams &P, TileSmem &s, const int b, double (&pl)[4][4][4],
+                                              const ThreadCtx &T, const int tid, const int lane, double *xout,
+                                              double *yout)
+{
+    double Pg[4] = {0.0, 0.0, 0.0, 0.0};
+    if (SPECIAL) {
+        const double gyz = s.g[3][1][T.yi] * s.g[3][2][T.zi];
+#pragma unroll
+        for (int r = 0; r < 4; ++r) Pg[r] = s.g[3][0][4 * T.ag + r] * gyz;
+    }
+#pragma unroll
+    for (int jj = 0; jj < 4; ++jj) {
+        double fx[4];
+        {
+            const double2 *p = reinterpret_cast<const double2 *>(&s.xface[b][jj][tid * 4]);
+            const double2 v0 = p[0], v1 = p[1];
+            fx[0] = v0.x; fx[1] = v0.y; fx[2] = v1.x; fx[3] = v1.y;
+        }
+#pragma unroll
+        for (int ii = 0; ii < 4; ++ii) {
+            const int cell = jj * 4 + ii;
+            const double4 yt = s.yztab[b][cell][T.yi];
+            const double4 zt = s.yztab[b][cell][T.zi];
+            const double Eyz = yt.x * zt.x, Qyz = yt.y + zt.y, eyz = yt.z + zt.z;
+            const double ay = yt.w, az = zt.w;
+            const double dyz = (ay + az) + s.nu[b][cell];
+            double yup[4];
+            if (jj == 0) {
+                const double2 *p = reinterpret_cast<const double2 *>(&s.yface[b][ii][tid * 4]);
+                const double2 v0 = p[0], v1 = p[1];
+                yup[0] = v0.x; yup[1] = v0.y; yup[2] = v1.x; yup[3] = v1.y;
+            } else {
+#pragma unroll
+                for (int r = 0; r < 4; ++r) yup[r] = pl[jj - 1][ii][r];
+            }
+            int code = 0;
+            double4 sp = make_double4(0.0, 0.0, 0.0, 0.0);
+            if (SPECIAL) { code = s.code[b][cell]; sp = s.spec[b][cell]; }
+            double S0 = 0.0, S1 = 0.0, S2 = 0.0, S3 = 0.0;
+#pragma unroll
+            for (int r = 0; r < 4; ++r) {
+                const double4 xt = s.xtab[b][cell][r * 4 + T.ag];
+                double xu = fx[r], yu = yup[r], zu = pl[jj][ii][r];
+                if (SPECIAL) {
+                    if (code & 1) xu = sp.x * Pg[r];
+                    if (code & 2) yu = sp.y * Pg[r];
+                    if (code & 4) zu = sp.z * Pg[r];
+                }
+                const double src = (xt.x * Eyz) * fma(xt.y + Qyz, xt.z + eyz, 1.0);
+                const double inv = fast_rcp(xt.w + dyz);
+                double num = fma(ay, yu, src);
+                num = fma(az, zu, num);
+                num = fma(xt.w, xu, num);
+                double gg = num * inv;
+                if (SPECIAL) { if (code & 8) gg = 0.0; }
+                fx[r] = gg;
+                pl[jj][ii][r] = gg;
+                S0 += gg;
+                S1 = fma(T.X1[r], gg, S1);
+                S2 = fma(T.X2[r], gg, S2);
+                S3 = fma(T.X3[r], gg, S3);
+            }
+            const double kk = reduce16(S0, S1, S2, S3, T.cf, lane);
+            if (lane < 16) {
+                const int c = s.cidx[b][cell];
+                if (!SPECIAL || c >= 0) {
+                    atomicAdd(P.raw16 + (long long)c * 16 + T.mom, kk);
+                    const int f = s.dnface[b][cell][T.dsel];
+                    if (f >= 0) atomicAdd(P.phi + f, T.dsgn * kk);
+                }
+            }
+        }
+        if (xout) {
+            double2 *p = reinterpret_cast<double2 *>(xout + jj * NVB + tid * 4);
+            p[0] = make_double2(fx[0], fx[1]);
+            p[1] = make_double2(fx[2], fx[3]);
+        }
+    }
+    if (yout) {
+#pragma unroll
+        for (int ii = 0; ii < 4; ++ii) {
+            double2 *p = reinterpret_cast<double2 *>(yout + ii * NVB + tid * 4);
+            p[0] = make_double2(pl[3][ii][0], pl[3][ii][1]);
+            p[1] = make_double2(pl[3][ii][2], pl[3][ii][3]);
+        }
+    }
+}
+
+__global__ void __launch_bounds__(TILE_THREADS, 2) sweep_tile_kernel(const TileParams P)
+{
+    extern __shared__ unsigned char smem_raw[];
+    TileSmem &s = *reinterpret_cast<TileSmem *>((reinterpret_cast<uintptr_t>(smem_raw) + 127) & ~uintptr_t(127));
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    if (tid == 0) {
+        mbar_init(&s.mbar[0], 1);
+        mbar_init(&s.mbar[1], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        fence_proxy_async();
+    }
+    __syncthreads();
+    unsigned par[2] = {0u, 0u};
+    const long long slot = P.slot_doubles;
+
+    for (;;) {
+        // ---- next item (dependency order), wait for its upwind items ----
+        if (tid == 0) {
+            const int n = atomicAdd(P.counter, 1);
+            s.item = n;
+            if (n < P.nitems) {
+                const TileItem it = P.items[n];
+                const int pred[3] = {it.pred_x, it.pred_y, it.pred_s};
+#pragma unroll
+                for (int q = 0; q < 3; ++q)
+                    if (pred[q] >= 0)
+                        while (ld_acquire(P.done + pred[q]) != P.epoch) __nanosleep(64);
+                fence_proxy_async();  // the upwind items' face stores (generic proxy) before our TMA reads
+                // faces of levels 0 and 1 (the staging buffers are free: every thread passed the end-of-item barrier)
+                const bool fx = it.ti == 0, fy = it.tj == 0;
+                const unsigned bytes = (fx ? 0u : LEVEL_BYTES) + (fy ? 0u : LEVEL_BYTES);
+                const double *xs = P.xface + ((long long)it.vb * P.P + it.xslot) * slot;
+                const double *ys = P.yface + ((long long)it.vb * P.ntx + it.ti) * slot;
+                for (int kp = 0; kp < 2 && kp < P.nz; ++kp) {
+                    mbar_expect_tx(&s.mbar[kp], bytes);
+                    if (!fx) tma_load(&s.xface[kp][0][0], xs + (long long)kp * LEVEL_DOUBLES, LEVEL_BYTES, &s.mbar[kp]);
+                    if (!fy) tma_load(&s.yface[kp][0][0], ys + (long long)kp * LEVEL_DOUBLES, LEVEL_BYTES, &s.mbar[kp]);
+                }
+            }
+        }
+        __syncthreads();
+        const int n = s.item;
+        if (n >= P.nitems) break;
+        const TileItem it = P.items[n];
+        const VBlock vb = P.vblocks[it.vb];
+        ItemCtx I;
+        I.sx = vb.sx; I.sy = vb.sy; I.sz = vb.sz;
+        I.i0 = it.ti * TILE_TX; I.j0 = it.tj * TILE_TY;
+        I.upx = vb.sx > 0 ? 0 : 1; I.upy = vb.sy > 0 ? 2 : 3; I.upz = vb.sz > 0 ? 4 : 5;
+        I.tpx = P.bc_type[I.upx]; I.tpy = P.bc_type[I.upy]; I.tpz = P.bc_type[I.upz];
+        I.first_x = it.ti == 0; I.first_y = it.tj == 0;
+        I.nbb = vb.nbb; I.ncb = vb.ncb;
+
+        // ---- per-item tables: nodes, weights, ghost factors, cell widths ----
+        {
+            const int slotid[4] = {I.upx, I.upy, I.upz, 6};
+            if (tid < 16) {
+                const bool ok = tid < vb.na;
+                const int idx = vb.a0 + tid;
+                s.xi_a[tid] = ok ? P.xi_x[idx] : 0.0;
+                s.w_a[tid] = ok ? P.w_x[idx] : 0.0;
+#pragma unroll
+                for (int f = 0; f < 4; ++f) s.g[f][0][tid] = ok ? P.gtab[(long long)(slotid[f] * 3 + 0) * P.gstride + idx] : 0.0;
+            } else if (tid < 16 + vb.nbb) {
+                const int bl = tid - 16;
+                const bool ok = bl < vb.nb;
+                const int idx = vb.b0 + bl;
+                s.xi_bc[bl] = ok ? P.xi_y[idx] : 0.0;
+                s.w_bc[bl] = ok ? P.w_y[idx] : 0.0;
+#pragma unroll
+                for (int f = 0; f < 4; ++f) s.g[f][1][bl] = ok ? P.gtab[(long long)(slotid[f] * 3 + 1) * P.gstride + idx] : 0.0;
+            } else if (tid >= 32 && tid < 32 + vb.ncb) {
+                const int cl = tid - 32;
+                const bool ok = cl < vb.nc;
+                const int idx = vb.c0 + cl;
+                s.xi_bc[vb.nbb + cl] = ok ? P.xi_z[idx] : 0.0;
+                s.w_bc[vb.nbb + cl] = ok ? P.w_z[idx] : 0.0;
+#pragma unroll
+                for (int f = 0; f < 4; ++f)
+                    s.g[f][2][vb.nbb + cl] = ok ? P.gtab[(long long)(slotid[f] * 3 + 2) * P.gstride + idx] : 0.0;
+            } else if (tid >= 48 && tid < 52) {
+                const int ip = I.i0 + (tid - 48);
+                s.invdx[tid - 48] = ip < P.nx ? P.invdx[vb.sx > 0 ? ip : P.nx - 1 - ip] : 0.0;
+            } else if (tid >= 52 && tid < 56) {
+                const int jp = I.j0 + (tid - 52);
+                s.invdy[tid - 52] = jp < P.ny ? P.invdy[vb.sy > 0 ? jp : P.ny - 1 - jp] : 0.0;
+            }
+        }
+        // metadata of levels 0 and 1
+        {
+            double v0, v1;
+            stage_load(P, I, 0, tid, v0, v1);
+            stage_store(s, 0, tid, v0, v1);
+            stage_load(P, I, 1, tid, v0, v1);
+            stage_store(s, 1, tid, v0, v1);
+        }
+        __syncthreads();
+
+        ThreadCtx T;
+        T.ag = lane & 3;
+        {
+            const int pair = warp * 8 + (lane >> 2);
+            T.yi = pair % vb.nbb;
+            T.zi = vb.nbb + pair / vb.nbb;
+            const double xb = s.xi_bc[T.yi], xc = s.xi_bc[T.zi], r2 = xb * xb + xc * xc;
+            const int q = lane & 3, j = ((lane >> 2) & 1) * 2 + ((lane >> 3) & 1);
+            if (q == 0) { T.cf[0] = 1.0; T.cf[1] = xb; T.cf[2] = xc; T.cf[3] = xb * xb; }
+            else if (q == 1) { T.cf[0] = 1.0; T.cf[1] = xb; T.cf[2] = xc; T.cf[3] = r2; }
+            else if (q == 2) { T.cf[0] = xc * xc; T.cf[1] = xb * xc; T.cf[2] = xb * r2; T.cf[3] = xc * r2; }
+            else { T.cf[0] = 1.0; T.cf[1] = xb; T.cf[2] = xc; T.cf[3] = 1.0; }
+            T.mom = c_mom[q][j];
+            T.dsel = 3; T.dsgn = 0.0;
+            if (q == 1 && j == 0) { T.dsel = 0; T.dsgn = (double)vb.sx; }
+            if (q == 0 && j == 1) { T.dsel = 1; T.dsgn = (double)vb.sy; }
+            if (q == 0 && j == 2) { T.dsel = 2; T.dsgn = (double)vb.sz; }
+#pragma unroll
+            for (int r = 0; r < 4; ++r) {
+                const double x = s.xi_a[4 * T.ag + r];
+                T.X1[r] = x; T.X2[r] = x * x; T.X3[r] = x * x * x;
+            }
+        }
+
+        // tables and boundary faces of level 0
+        int special = build_tables(P, I, s, 0, tid);
+        fill_faces(I, s, 0, tid, T.ag, T.yi, T.zi);
+        // plane = ghost of the upwind z face of the domain
+        double pl[4][4][4];
+        {
+            const double gyz = s.g[2][1][T.yi] * s.g[2][2][T.zi];
+            double G[4];
+#pragma unroll
+            for (int r = 0; r < 4; ++r) G[r] = s.g[2][0][4 * T.ag + r] * gyz;
+#pragma unroll
+            for (int jj = 0; jj < 4; ++jj)
+#pragma unroll
+                for (int ii = 0; ii < 4; ++ii) {
+                    int i, j, k;
+                    double rw = 0.0;
+                    if (cell_of(P, I, ii, jj, 0, i, j, k)) rw = face_density(P, I.tpz, P.foff[I.upz] + j * P.nx + i);
+#pragma unroll
+                    for (int r = 0; r < 4; ++r) pl[jj][ii][r] = rw * G[r];
+                }
+        }
+        special = __syncthreads_or(special);
+
+        const bool write_x = it.ti < P.ntx - 1, write_y = it.tj < P.nty - 1;
+        double *xdst = P.xface + ((long long)it.vb * P.P + it.xslot) * slot;
+        double *ydst = P.yface + ((long long)it.vb * P.ntx + it.ti) * slot;
+
+        for (int kp = 0; kp < P.nz; ++kp) {
+            const int b = kp & 1;
+            double v0, v1;
+            stage_load(P, I, kp + 2, tid, v0, v1);
+            mbar_wait(&s.mbar[b], par[b]);
+            par[b] ^= 1u;
+            double *xout = write_x ? xdst + (long long)kp * LEVEL_DOUBLES : nullptr;
+            double *yout = write_y ? ydst + (long long)kp * LEVEL_DOUBLES : nullptr;
+            if (special) compute_level<true>(P, s, b, pl, T, tid, lane, xout, yout);
+            else compute_level<false>(P, s, b, pl, T, tid, lane, xout, yout);
+            stage_store(s, b, tid, v0, v1);
+            int sp = 0;
+            if (kp + 1 < P.nz) {
+                sp = build_tables(P, I, s, kp + 1, tid);
+                fill_faces(I, s, b ^ 1, tid, T.ag, T.yi, T.zi);
+            }
+            special = __syncthreads_or(sp);
+            if (tid == 0 && kp + 2 < P.nz) {
+                const unsigned bytes = (I.first_x ? 0u : LEVEL_BYTES) + (I.first_y ? 0u : LEVEL_BYTES);
+                fence_proxy_async();
+                mbar_expect_tx(&s.mbar[b], bytes);
+                if (!I.first_x) tma_load(&s.xface[b][0][0], xdst + (long long)(kp + 2) * LEVEL_DOUBLES, LEVEL_BYTES, &s.mbar[b]);
+                if (!I.first_y) tma_load(&s.yface[b][0][0], ydst + (long long)(kp + 2) * LEVEL_DOUBLES, LEVEL_BYTES, &s.mbar[b]);
+            }
+        }
+        // ---- publish: faces of this item are complete ----
+        __threadfence();
+        __syncthreads();
+        if (tid == 0) st_release(P.done + n, P.epoch);
+    }
+}
+
+}  // namespace
+
+size_t tile_smem_bytes() { return sizeof(TileSmem) + 128; }
+
+cudaError_t tile_configure(int *ctas_per_sm)
+{
+    cudaError_t e = cudaFuncSetAttribute(sweep_tile_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tile_smem_bytes());
+    if (e != cudaSuccess) return e;
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, sweep_tile_kernel, TILE_THREADS, tile_smem_bytes());
+}
+
+cudaError_t launch_sweep_tile(const TileParams &P, int grid, cudaStream_t st)
+{
+    sweep_tile_kernel<<<grid, TILE_THREADS, tile_smem_bytes(), st>>>(P);
+    return cudaGetLastError();
+}
+
 }  // namespace dvm

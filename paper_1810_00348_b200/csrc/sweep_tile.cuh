@@ -1,4 +1,14 @@
-// sweep_tile.cuh - host interface of the tile sweep kernel (sweep_tile.cu)
+// sweep_tile.cuh - host interface and shared records of the tile sweep kernel (sweep_tile.cu, tile_plan.cu).
+//
+// DVM_KERNEL_TILE in one paragraph: the sweep of Eq.(7) is cut into
+// work items (velocity block V, z-column tile (I', J')).  A velocity block is 512 discrete velocities of one
+// sign octant (a box 16 x nbb x ncb of node indices); a column tile is TX x TY = 4 x 4 cells wide and spans
+// all nz levels.  One CTA of 128 threads owns an item: every thread carries 4 velocities (consecutive xi_x
+// nodes, same xi_y, xi_z) and keeps their 4 x 4 x 4 values of the current z-plane of the tile in REGISTERS, so the
+// z-upwind and y-upwind operands never leave the register file; only the x- and y-faces of the column go to HBM
+// (8 B per phase point instead of the 16 B of an in-place slice, 32 B in the paper's two-slice form,
+// PAPER.md:104-106, 233-235).  Items are handed out by an atomic counter in an order that respects the upwind
+// dependencies (x-face of (I'-1, J'), y-face of (I', J'-1)); done-flags in global memory gate the start of an item.
 #pragma once
 #include <cuda_runtime.h>
 #include <vector>
@@ -6,15 +16,78 @@
 
 namespace dvm {
 
-struct TilePlan {
-    size_t fbuf_doubles = 0;
-    int nthreads = 0;
-    size_t smem = 0;
+constexpr int TILE_TX = 4;                 // cells per tile along the sweep-relative x
+constexpr int TILE_TY = 4;                 // cells per tile along the sweep-relative y
+constexpr int TILE_NCELL = TILE_TX * TILE_TY;
+constexpr int TILE_RV = 4;                 // velocities per thread (consecutive xi_x nodes)
+constexpr int TILE_GA = 4;                 // xi_x groups per lane quad
+constexpr int TILE_NA = TILE_RV * TILE_GA; // xi_x nodes per velocity block
+constexpr int TILE_THREADS = 128;
+constexpr int TILE_WARPS = TILE_THREADS / 32;
+constexpr int TILE_NVB = TILE_THREADS * TILE_RV;  // velocities per block (incl. padding)
+constexpr int TILE_NPAIR = TILE_THREADS / TILE_GA; // (xi_y, xi_z) pairs per block
+constexpr int TILE_MAXBC = 12;             // nbb + ncb of a block
+
+// velocity block: node-index box [a0, a0+na) x [b0, b0+nb) x [c0, c0+nc), na <= 16, nb <= nbb, nc <= ncb,
+// nbb * ncb = 32; lanes beyond the box carry weight 0
+struct VBlock {
+    int a0, na, b0, nb, c0, nc;
+    int nbb, ncb;
+    int sx, sy, sz;   // sweep direction per axis: +1 ascending (xi >= 0), -1 descending
+    int pad;
 };
 
-bool tile_supported(int nx, int ny, int nz);
-int tile_plan(int nx, int ny, int nz, const int lo[3][2], const int cnt[3][2], long long nvel, TilePlan *plan,
-              std::vector<BlockDesc> *blocks);
-cudaError_t launch_sweep_tile(const SweepParams &P, const TilePlan &plan, int nblocks, cudaStream_t st);
+// work item; ti, tj are sweep-relative tile coordinates (0 = most upwind)
+struct TileItem {
+    int vb;
+    int ti, tj;
+    int pred_x;       // item index of (vb, ti-1, tj) or -1
+    int pred_y;       // item index of (vb, ti, tj-1) or -1
+    int pred_s;       // item index of the last reader of this item's x-face slot, (vb, ntx-1, tj-P), or -1
+    int xslot;        // tj % P
+    int pad;
+};
+
+struct TilePlan {
+    int ntx = 0, nty = 0, P = 1;
+    std::vector<VBlock> vblocks;
+    std::vector<TileItem> items;
+    size_t xface_doubles = 0, yface_doubles = 0;
+};
+
+struct TileParams {
+    int nx, ny, nz, ntx, nty, P;
+    long long ncell;
+    const double *invdx, *invdy, *invdz;
+    const unsigned char *flags;   // [ncell] bits 0..5: neighbour in direction d is not a fluid cell; bit 6: solid
+    const unsigned char *sflags;  // [ncell] bits 0..5: neighbour in direction d is a solid cell; bit 6: solid
+    const int *face_of;           // [6][ncell] boundary-face slot or -1
+    const double *coef;           // [NCOEF][ncell]
+    const double *rho_w;          // [nface]
+    double *phi;                  // [nface]
+    double *raw16;                // [ncell][16] velocity sums (13 used)
+    const double *xi_x, *xi_y, *xi_z, *w_x, *w_y, *w_z;
+    const double *gtab;           // [7][3][gstride] per BC slot and axis: weighted 1-D factors of the ghost Maxwellian
+    int gstride;
+    int bc_type[7];
+    int foff[6];                  // first slot of each domain face in the boundary-face table
+    const VBlock *vblocks;
+    const TileItem *items;
+    int nitems;
+    int *done;                    // [nitems] epoch of completion
+    int *counter;                 // next item
+    int epoch;
+    double *xface, *yface;
+    long long slot_doubles;       // nz * 4 * TILE_NVB
+};
+
+// Build velocity blocks, items and their order for a grid and a set of velocity nodes.  target_ctas = number of
+// items that should be able to run concurrently (sets the band height P).  Pure host code (tests call it through
+// dvm_plan_query without a GPU).
+int tile_plan(int nx, int ny, int nz, const std::vector<double> xi[3], int target_ctas, TilePlan *plan);
+
+size_t tile_smem_bytes();
+cudaError_t tile_configure(int *ctas_per_sm);
+cudaError_t launch_sweep_tile(const TileParams &P, int grid, cudaStream_t st);
 
 }  // namespace dvm

@@ -1,0 +1,99 @@
+// tile_plan.cu - host planner of the tile sweep kernel: velocity blocks, work items, their hand-out order and
+// the dependency edges (see sweep_tile.cuh).  Pure host code, no CUDA calls.
+//
+// Order.  Tile rows (sweep-relative tj) are grouped into bands of P rows.  Bands are processed one after the
+// other; inside a band items are ordered by the diagonal d = ti + (tj mod P), then by row, then by velocity
+// block.  Every predecessor of an item (the tile upwind in x, the tile upwind in y, and the last reader of the
+// x-face slot the item is about to overwrite) is therefore earlier in the order, which - with items handed out
+// by a monotone counter - rules out deadlock: an item only ever waits for items that are running or done.
+#include "sweep_tile.cuh"
+
+#include <algorithm>
+#include <map>
+
+namespace dvm {
+
+namespace {
+
+// index ranges of the negative / non-negative nodes of one axis (nodes ascending)
+void split_axis(const std::vector<double> &xi, int lo[2], int cnt[2])
+{
+    int nneg = 0;
+    while (nneg < (int)xi.size() && xi[nneg] < 0.0) ++nneg;
+    lo[0] = 0; cnt[0] = nneg; lo[1] = nneg; cnt[1] = (int)xi.size() - nneg;
+}
+
+int ceil_div(int a, int b) { return (a + b - 1) / b; }
+
+}  // namespace
+
+int tile_plan(int nx, int ny, int nz, const std::vector<double> xi[3], int target_ctas, TilePlan *plan)
+{
+    if (nx <= 0 || ny <= 0 || nz <= 0 || !plan) return -1;
+    plan->vblocks.clear();
+    plan->items.clear();
+    int lo[3][2], cnt[3][2];
+    for (int d = 0; d < 3; ++d) split_axis(xi[d], lo[d], cnt[d]);
+
+    // ---- velocity blocks: per octant, chunks of 16 x nbb x ncb node indices ----
+    for (int oz = 0; oz < 2; ++oz) for (int oy = 0; oy < 2; ++oy) for (int ox = 0; ox < 2; ++ox) {
+        const int na = cnt[0][ox], nb = cnt[1][oy], nc = cnt[2][oz];
+        if (na == 0 || nb == 0 || nc == 0) continue;
+        // (nbb, ncb) with nbb * ncb = 32 and nbb + ncb <= TILE_MAXBC: the shape wasting the fewest lanes
+        int best_bb = 8, best_cb = 4;
+        long best = -1;
+        const int shapes[2][2] = {{8, 4}, {4, 8}};
+        for (auto &s : shapes) {
+            const long slots = (long)ceil_div(nb, s[0]) * ceil_div(nc, s[1]);
+            if (best < 0 || slots < best) { best = slots; best_bb = s[0]; best_cb = s[1]; }
+        }
+        for (int c0 = 0; c0 < nc; c0 += best_cb) for (int b0 = 0; b0 < nb; b0 += best_bb)
+            for (int a0 = 0; a0 < na; a0 += TILE_NA) {
+                VBlock v{};
+                v.a0 = lo[0][ox] + a0; v.na = std::min(TILE_NA, na - a0);
+                v.b0 = lo[1][oy] + b0; v.nb = std::min(best_bb, nb - b0);
+                v.c0 = lo[2][oz] + c0; v.nc = std::min(best_cb, nc - c0);
+                v.nbb = best_bb; v.ncb = best_cb;
+                v.sx = ox ? 1 : -1; v.sy = oy ? 1 : -1; v.sz = oz ? 1 : -1;
+                plan->vblocks.push_back(v);
+            }
+    }
+    const int nvb = (int)plan->vblocks.size();
+    if (nvb == 0) return -1;
+    const int ntx = ceil_div(nx, TILE_TX), nty = ceil_div(ny, TILE_TY);
+    plan->ntx = ntx; plan->nty = nty;
+    // band height: enough independent tiles per diagonal to keep target_ctas items in flight
+    int P = ceil_div(std::max(target_ctas, 1) * 2, nvb);
+    P = std::max(1, std::min(P, nty));
+    plan->P = P;
+
+    // ---- items in hand-out order ----
+    std::vector<int> index((size_t)nvb * ntx * nty, -1);
+    auto at = [&](int vb, int ti, int tj) -> int & { return index[((size_t)vb * nty + tj) * ntx + ti]; };
+    for (int band = 0; band * P < nty; ++band) {
+        const int j0 = band * P, rows = std::min(P, nty - j0);
+        for (int d = 0; d < ntx + rows - 1; ++d)
+            for (int r = 0; r < rows; ++r) {
+                const int ti = d - r, tj = j0 + r;
+                if (ti < 0 || ti >= ntx) continue;
+                for (int vb = 0; vb < nvb; ++vb) {
+                    TileItem it{};
+                    it.vb = vb; it.ti = ti; it.tj = tj; it.xslot = tj % P;
+                    it.pred_x = it.pred_y = it.pred_s = -1;
+                    at(vb, ti, tj) = (int)plan->items.size();
+                    plan->items.push_back(it);
+                }
+            }
+    }
+    for (auto &it : plan->items) {
+        if (it.ti > 0) it.pred_x = at(it.vb, it.ti - 1, it.tj);
+        if (it.tj > 0) it.pred_y = at(it.vb, it.ti, it.tj - 1);
+        if (it.ti == 0 && it.tj >= P) it.pred_s = at(it.vb, ntx - 1, it.tj - P);
+    }
+    const size_t slot = (size_t)nz * TILE_TY * TILE_NVB;
+    plan->xface_doubles = (size_t)nvb * P * slot;
+    plan->yface_doubles = (size_t)nvb * ntx * slot;
+    return 0;
+}
+
+}  // namespace dvm

@@ -68,20 +68,20 @@ __global__ void __launch_bounds__(UB) convert_kernel(const UpdateParams U)
         if (U.flags[c] & FLAG_SOLID) {
             for (int m = 0; m < NPRIM; ++m) U.prim_new[m * n + c] = 0.0;
         } else {
-            const double *r = U.raw;
-            const double rho = r[c];
+            const double *r = U.raw + c * 16;   // [cell][16] accumulator, 13 used
+            const double rho = r[0];
             const double ir = 1.0 / rho;
-            const double ux = r[n + c] * ir, uy = r[2 * n + c] * ir, uz = r[3 * n + c] * ir;
-            const double mxx = r[4 * n + c], myy = r[5 * n + c], mzz = r[6 * n + c];
-            const double mxy = r[7 * n + c], mxz = r[8 * n + c], myz = r[9 * n + c];
+            const double ux = r[1] * ir, uy = r[2] * ir, uz = r[3] * ir;
+            const double mxx = r[4], myy = r[5], mzz = r[6];
+            const double mxy = r[7], mxz = r[8], myz = r[9];
             const double pxx = mxx - rho * ux * ux, pyy = myy - rho * uy * uy, pzz = mzz - rho * uz * uz;
             const double pxy = mxy - rho * ux * uy, pxz = mxz - rho * ux * uz, pyz = myz - rho * uy * uz;
             const double trP = pxx + pyy + pzz, trm = mxx + myy + mzz;
             const double u2 = ux * ux + uy * uy + uz * uz;
             const double T = (2.0 / 3.0) * trP * ir;
-            const double qx = 0.5 * (r[10 * n + c] - 2.0 * (ux * mxx + uy * mxy + uz * mxz) - ux * trm + 2.0 * rho * ux * u2);
-            const double qy = 0.5 * (r[11 * n + c] - 2.0 * (ux * mxy + uy * myy + uz * myz) - uy * trm + 2.0 * rho * uy * u2);
-            const double qz = 0.5 * (r[12 * n + c] - 2.0 * (ux * mxz + uy * myz + uz * mzz) - uz * trm + 2.0 * rho * uz * u2);
+            const double qx = 0.5 * (r[10] - 2.0 * (ux * mxx + uy * mxy + uz * mxz) - ux * trm + 2.0 * rho * ux * u2);
+            const double qy = 0.5 * (r[11] - 2.0 * (ux * mxy + uy * myy + uz * myz) - uy * trm + 2.0 * rho * uy * u2);
+            const double qz = 0.5 * (r[12] - 2.0 * (ux * mxz + uy * myz + uz * mzz) - uz * trm + 2.0 * rho * uz * u2);
             double *o = U.prim_new;
             o[c] = rho; o[n + c] = ux; o[2 * n + c] = uy; o[3 * n + c] = uz; o[4 * n + c] = T;
             o[5 * n + c] = qx; o[6 * n + c] = qy; o[7 * n + c] = qz;
@@ -180,11 +180,25 @@ __global__ void __launch_bounds__(UB) faces_kernel(const UpdateParams U)
     U.rho_w[f] = pu > 0.0 ? U.phi[f] / pu * U.scal[0] : 0.0;
 }
 
+// [cell][16] accumulator -> [13][ncell] (dvm_raw_moments)
+__global__ void __launch_bounds__(UB) raw_export_kernel(const double *raw16, double *out13, long long n)
+{
+    const long long c = (long long)blockIdx.x * UB + threadIdx.x;
+    if (c >= n) return;
+    for (int m = 0; m < NRAW; ++m) out13[m * n + c] = raw16[c * 16 + m];
+}
+
 static inline int nblk(long long n) { return (int)((n + UB - 1) / UB); }
 
 cudaError_t launch_pack(const UpdateParams &U, cudaStream_t st)
 {
     pack_kernel<<<nblk(U.ncell), UB, 0, st>>>(U);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_raw_export(const double *raw16, double *out13, long long n, cudaStream_t st)
+{
+    raw_export_kernel<<<nblk(n), UB, 0, st>>>(raw16, out13, n);
     return cudaGetLastError();
 }
 

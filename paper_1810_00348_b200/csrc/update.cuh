@@ -10,7 +10,7 @@ struct UpdateParams {
     long long npart;            // stride of the partial-sum table (>= number of update blocks)
     const unsigned char *flags;
     const double *dx, *dy, *dz; // cell widths
-    const double *raw;          // [13][ncell]
+    const double *raw;          // [ncell][16] velocity sums (13 used)
     double *prim;               // [14][ncell] state n -> n+1 (in place, in finish_kernel)
     double *prim_new;           // [14][ncell] unscaled conversion of this iteration
     double *coef;               // [9][ncell]
@@ -27,6 +27,7 @@ struct UpdateParams {
 
 struct SweepParams;
 
+cudaError_t launch_raw_export(const double *raw16, double *out13, long long n, cudaStream_t st);
 cudaError_t launch_pack(const UpdateParams &U, cudaStream_t st);
 cudaError_t launch_update(const UpdateParams &U, int hist_slot, cudaStream_t st, int *launches);
 cudaError_t launch_sweep_slice(const SweepParams &P, int nblocks, int nb, cudaStream_t st);

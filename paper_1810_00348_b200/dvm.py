@@ -29,7 +29,7 @@ SYMBOLS = (
     "dvm_create", "dvm_iterate", "dvm_moments", "dvm_residual", "dvm_num_faces", "dvm_iterations_done",
     "dvm_get_state", "dvm_set_state", "dvm_raw_moments", "dvm_wall_flux", "dvm_residual_history",
     "dvm_mass_scale", "dvm_step_host", "dvm_set_option", "dvm_workspace_bytes", "dvm_launch_count",
-    "dvm_kernel_used", "dvm_destroy", "dvm_last_error",
+    "dvm_kernel_used", "dvm_plan_query", "dvm_destroy", "dvm_last_error",
 )
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
@@ -117,6 +117,8 @@ def lib():
         L.dvm_set_option.argtypes = [vp, C.c_int, C.c_int]
         L.dvm_workspace_bytes.argtypes = [vp, C.POINTER(C.c_size_t), C.POINTER(C.c_size_t)]
         L.dvm_kernel_used.argtypes = [vp]
+        L.dvm_plan_query.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(_VGrid), C.c_int, C.POINTER(C.c_int),
+                                     C.POINTER(C.c_int), C.c_int]
         L.dvm_launch_count.argtypes = [vp]
         L.dvm_launch_count.restype = C.c_longlong
         L.dvm_destroy.argtypes = [vp]
@@ -133,6 +135,18 @@ def _check(rc):
 
 def _f64(a):
     return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def plan_query(nx, ny, nz, xi_x, xi_y, xi_z, target_ctas=296, max_items=1 << 22):
+    """dvm_plan_query: (counts dict, items int32 [n][8]) of the tile kernel's work decomposition (host only)."""
+    keep = [_f64(a) for a in (xi_x, xi_y, xi_z)]
+    v = _VGrid(len(keep[0]), len(keep[1]), len(keep[2]), *(a.ctypes.data_as(_dp) for a in keep), None, None, None)
+    counts = (C.c_int * 4)()
+    n = _check(lib().dvm_plan_query(nx, ny, nz, C.byref(v), target_ctas, counts, None, 0))
+    items = np.zeros((min(n, max_items), 8), dtype=np.int32)
+    _check(lib().dvm_plan_query(nx, ny, nz, C.byref(v), target_ctas, counts, items.ctypes.data_as(C.POINTER(C.c_int)),
+                                len(items)))
+    return {"n_vblocks": counts[0], "ntx": counts[1], "nty": counts[2], "P": counts[3], "n_items": n}, items
 
 
 class Solver:
