@@ -219,11 +219,12 @@ __device__ __forceinline__ int build_tables(const TileParams &P, const ItemCtx &
         s.nu[b][cell] = dead ? 1.0 : s.stage[b][cell][0];
         s.dnface[b][cell][0] = dn[0]; s.dnface[b][cell][1] = dn[1]; s.dnface[b][cell][2] = dn[2];
         s.dnface[b][cell][3] = -1;
-        special = code != 0;
+        special = (code & 7) != 0;
     }
-    const int nent = 16 * (TILE_NA + I.nbb + I.ncb);
-    for (int e = tid; e < nent; e += TILE_THREADS) {
-        const int cell = e & 15, n = e >> 4;
+    // TILE_NA + nbb + ncb = 28 entries per cell; consecutive threads write consecutive entries of one cell
+    constexpr int NENT = TILE_NA + TILE_MAXBC;
+    for (int e = tid; e < 16 * NENT; e += TILE_THREADS) {
+        const int cell = e / NENT, n = e - cell * NENT;
         const int fl = s.cflag[b][cell];
         const bool dead = !((fl >> 16) & 1) || ((fl >> 8) & 64);
         const double *st = s.stage[b][cell];
@@ -279,9 +280,10 @@ __device__ __forceinline__ void fill_faces(const ItemCtx &I, TileSmem &s, int b,
     }
 }
 
-// Reduction of the four power sums S_p = sum_r xi_x^p g_r of a lane over the warp (see the header comment):
-// returns, in every lane, one of the 16 partial products of the cell; lane & 15 names it (c_mom).
-__device__ __forceinline__ double reduce16(double S0, double S1, double S2, double S3, const double (&cf)[4], int lane)
+// Reduction of the four power sums S_p = sum_r xi_x^p g_r of a lane over the 4 x-groups of a lane quad and the
+// (xi_y, xi_z) pairs with lane bits 2 and 3 (see the header comment).  Returns, in every lane, the partial sum over
+// its half-warp of one of the 16 products of the cell; lane & 15 names it (c_mom).
+__device__ __forceinline__ double reduce_half(double S0, double S1, double S2, double S3, const double (&cf)[4], int lane)
 {
     const bool b0 = lane & 1, b1 = lane & 2, b2 = lane & 4, b3 = lane & 8;
     // lane quad = the 4 xi_x groups of one (xi_y, xi_z) pair
@@ -295,12 +297,10 @@ __device__ __forceinline__ double reduce16(double S0, double S1, double S2, doub
     const double U = b0 ? u : S0;
     const double V = (b0 && b1) ? v : U;
     const double o0 = cf[0] * U, o1 = cf[1] * U, o2 = cf[2] * U, o3 = cf[3] * V;
-    // transposing butterfly over the 8 (xi_y, xi_z) pairs of the warp
+    // transposing butterfly over the (xi_y, xi_z) pairs of the half-warp
     const double k0 = (b2 ? o2 : o0) + shx(b2 ? o0 : o2, 4);
     const double k1 = (b2 ? o3 : o1) + shx(b2 ? o1 : o3, 4);
-    double kk = (b3 ? k1 : k0) + shx(b3 ? k0 : k1, 8);
-    kk += shx(kk, 16);
-    return kk;
+    return (b3 ? k1 : k0) + shx(b3 ? k0 : k1, 8);
 }
 
 // per-thread constants of an item
@@ -308,23 +308,34 @@ struct ThreadCtx {
     double X1[4], X2[4], X3[4];  // xi_x, xi_x^2, xi_x^3 of the thread's nodes
     double cf[4];                // expansion coefficients of this lane
     double dsgn;                 // sign of the wall-flux contribution of this lane
+    double *rawm;                // raw16 + moment slot of this lane
     int ag, yi, zi;              // xi_x group, table rows of the thread's xi_y and xi_z nodes
-    int mom, dsel;               // moment slot and wall-flux direction (3 = none) of this lane
+    int dsel;                    // wall-flux direction (3 = none) of this lane
 };
 
-// One level of the column: 4 rows x 4 cells x 4 velocities per thread, fully unrolled so that the plane lives in
-// registers.  SPECIAL adds solid ghosts and dead cells.
-template <bool SPECIAL>
+// velocity sums of two cells (A: lower half-warp keeps it, B: upper half-warp) -> accumulators, one RED per lane
+__device__ __forceinline__ void emit_pair(const TileParams &P, TileSmem &s, const int b, const int cellA, double kA, double kB,
+                                          const ThreadCtx &T, const int lane)
+{
+    const bool hi = lane & 16;
+    const double keep = hi ? kB : kA, send = hi ? kA : kB;
+    const double tot = keep + shx(send, 16);
+    const int cell = cellA + (hi ? 1 : 0);
+    const int c = s.cidx[b][cell];
+    if (c >= 0) {
+        atomicAdd(T.rawm + (long long)c * 16, tot);
+        const int f = s.dnface[b][cell][T.dsel];
+        if (f >= 0) atomicAdd(P.phi + f, T.dsgn * tot);
+    }
+}
+
+// One level of the column, fast path (no solid ghost in the level): 4 rows x 4 cells x 4 velocities per thread,
+// fully unrolled so that the plane lives in registers.  Dead cells (outside the domain / solid) have all-zero table
+// entries and nu = 1, so they produce g = 0 by the same arithmetic.
 __device__ __forceinline__ void compute_level(const TileParams &P, TileSmem &s, const int b, double (&pl)[4][4][4],
                                               const ThreadCtx &T, const int tid, const int lane, double *xout,
                                               double *yout)
 {
-    double Pg[4] = {0.0, 0.0, 0.0, 0.0};
-    if (SPECIAL) {
-        const double gyz = s.g[3][1][T.yi] * s.g[3][2][T.zi];
-#pragma unroll
-        for (int r = 0; r < 4; ++r) Pg[r] = s.g[3][0][4 * T.ag + r] * gyz;
-    }
 #pragma unroll
     for (int jj = 0; jj < 4; ++jj) {
         double fx[4];
@@ -333,6 +344,7 @@ __device__ __forceinline__ void compute_level(const TileParams &P, TileSmem &s, 
             const double2 v0 = p[0], v1 = p[1];
             fx[0] = v0.x; fx[1] = v0.y; fx[2] = v1.x; fx[3] = v1.y;
         }
+        double kprev = 0.0;
 #pragma unroll
         for (int ii = 0; ii < 4; ++ii) {
             const int cell = jj * 4 + ii;
@@ -350,26 +362,16 @@ __device__ __forceinline__ void compute_level(const TileParams &P, TileSmem &s, 
 #pragma unroll
                 for (int r = 0; r < 4; ++r) yup[r] = pl[jj - 1][ii][r];
             }
-            int code = 0;
-            double4 sp = make_double4(0.0, 0.0, 0.0, 0.0);
-            if (SPECIAL) { code = s.code[b][cell]; sp = s.spec[b][cell]; }
             double S0 = 0.0, S1 = 0.0, S2 = 0.0, S3 = 0.0;
 #pragma unroll
             for (int r = 0; r < 4; ++r) {
                 const double4 xt = s.xtab[b][cell][r * 4 + T.ag];
-                double xu = fx[r], yu = yup[r], zu = pl[jj][ii][r];
-                if (SPECIAL) {
-                    if (code & 1) xu = sp.x * Pg[r];
-                    if (code & 2) yu = sp.y * Pg[r];
-                    if (code & 4) zu = sp.z * Pg[r];
-                }
                 const double src = (xt.x * Eyz) * fma(xt.y + Qyz, xt.z + eyz, 1.0);
                 const double inv = fast_rcp(xt.w + dyz);
-                double num = fma(ay, yu, src);
-                num = fma(az, zu, num);
-                num = fma(xt.w, xu, num);
-                double gg = num * inv;
-                if (SPECIAL) { if (code & 8) gg = 0.0; }
+                double num = fma(ay, yup[r], src);
+                num = fma(az, pl[jj][ii][r], num);
+                num = fma(xt.w, fx[r], num);
+                const double gg = num * inv;
                 fx[r] = gg;
                 pl[jj][ii][r] = gg;
                 S0 += gg;
@@ -377,15 +379,9 @@ __device__ __forceinline__ void compute_level(const TileParams &P, TileSmem &s, 
                 S2 = fma(T.X2[r], gg, S2);
                 S3 = fma(T.X3[r], gg, S3);
             }
-            const double kk = reduce16(S0, S1, S2, S3, T.cf, lane);
-            if (lane < 16) {
-                const int c = s.cidx[b][cell];
-                if (!SPECIAL || c >= 0) {
-                    atomicAdd(P.raw16 + (long long)c * 16 + T.mom, kk);
-                    const int f = s.dnface[b][cell][T.dsel];
-                    if (f >= 0) atomicAdd(P.phi + f, T.dsgn * kk);
-                }
-            }
+            const double kk = reduce_half(S0, S1, S2, S3, T.cf, lane);
+            if (ii & 1) emit_pair(P, s, b, cell - 1, kprev, kk, T, lane);
+            else kprev = kk;
         }
         if (xout) {
             double2 *p = reinterpret_cast<double2 *>(xout + jj * NVB + tid * 4);
@@ -403,10 +399,77 @@ __device__ __forceinline__ void compute_level(const TileParams &P, TileSmem &s, 
     }
 }
 
+// One level that holds a solid ghost (a fluid cell whose upwind neighbour is a masked cell): the same arithmetic
+// written as compact loops over a copy of the plane in local memory.  Rare (the surface of a masked body), so its
+// speed does not matter; keeping it out of the unrolled path halves the code the instruction cache has to hold.
+__device__ __forceinline__ void compute_level_slow(const TileParams &P, TileSmem &s, const int b, double *pl,
+                                                   const ThreadCtx &T, const int tid, const int lane, double *xout,
+                                                   double *yout)
+{
+    const double gyz = s.g[3][1][T.yi] * s.g[3][2][T.zi];
+#pragma unroll 1
+    for (int jj = 0; jj < 4; ++jj) {
+        double fx[4];
+#pragma unroll
+        for (int r = 0; r < 4; ++r) fx[r] = s.xface[b][jj][tid * 4 + r];
+        double kprev = 0.0;
+#pragma unroll 1
+        for (int ii = 0; ii < 4; ++ii) {
+            const int cell = jj * 4 + ii;
+            const double4 yt = s.yztab[b][cell][T.yi];
+            const double4 zt = s.yztab[b][cell][T.zi];
+            const double Eyz = yt.x * zt.x, Qyz = yt.y + zt.y, eyz = yt.z + zt.z;
+            const double ay = yt.w, az = zt.w;
+            const double dyz = (ay + az) + s.nu[b][cell];
+            const int code = s.code[b][cell];
+            const double4 sp = s.spec[b][cell];
+            double S0 = 0.0, S1 = 0.0, S2 = 0.0, S3 = 0.0;
+#pragma unroll
+            for (int r = 0; r < 4; ++r) {
+                const double Pg = s.g[3][0][4 * T.ag + r] * gyz;
+                const double4 xt = s.xtab[b][cell][r * 4 + T.ag];
+                double xu = fx[r], zu = pl[cell * 4 + r];
+                double yu = jj == 0 ? s.yface[b][ii][tid * 4 + r] : pl[(cell - 4) * 4 + r];
+                if (code & 1) xu = sp.x * Pg;
+                if (code & 2) yu = sp.y * Pg;
+                if (code & 4) zu = sp.z * Pg;
+                const double src = (xt.x * Eyz) * fma(xt.y + Qyz, xt.z + eyz, 1.0);
+                const double inv = fast_rcp(xt.w + dyz);
+                double num = fma(ay, yu, src);
+                num = fma(az, zu, num);
+                num = fma(xt.w, xu, num);
+                double gg = num * inv;
+                if (code & 8) gg = 0.0;
+                fx[r] = gg;
+                pl[cell * 4 + r] = gg;
+                S0 += gg;
+                S1 = fma(T.X1[r], gg, S1);
+                S2 = fma(T.X2[r], gg, S2);
+                S3 = fma(T.X3[r], gg, S3);
+            }
+            const double kk = reduce_half(S0, S1, S2, S3, T.cf, lane);
+            if (ii & 1) emit_pair(P, s, b, cell - 1, kprev, kk, T, lane);
+            else kprev = kk;
+        }
+        if (xout) {
+#pragma unroll
+            for (int r = 0; r < 4; ++r) xout[jj * NVB + tid * 4 + r] = fx[r];
+        }
+    }
+    if (yout) {
+#pragma unroll 1
+        for (int ii = 0; ii < 4; ++ii)
+#pragma unroll
+            for (int r = 0; r < 4; ++r) yout[ii * NVB + tid * 4 + r] = pl[(12 + ii) * 4 + r];
+    }
+}
+
 __global__ void __launch_bounds__(TILE_THREADS, 2) sweep_tile_kernel(const TileParams P)
 {
-    extern __shared__ unsigned char smem_raw[];
-    TileSmem &s = *reinterpret_cast<TileSmem *>((reinterpret_cast<uintptr_t>(smem_raw) + 127) & ~uintptr_t(127));
+    // dynamic shared memory starts at offset 0 of the CTA's window (no static __shared__ in this kernel), so the
+    // 128-byte alignment holds; casting without pointer arithmetic keeps the address space visible (LDS / STS)
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    TileSmem &s = *reinterpret_cast<TileSmem *>(smem_raw);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     if (tid == 0) {
         mbar_init(&s.mbar[0], 1);
@@ -444,7 +507,8 @@ __global__ void __launch_bounds__(TILE_THREADS, 2) sweep_tile_kernel(const TileP
             }
         }
         __syncthreads();
-        const int n = s.item;
+        // every thread reads the same value; the lane-0 broadcast tells the compiler it is warp-uniform
+        const int n = __shfl_sync(0xffffffffu, s.item, 0);
         if (n >= P.nitems) break;
         const TileItem it = P.items[n];
         const VBlock vb = P.vblocks[it.vb];
@@ -513,7 +577,7 @@ __global__ void __launch_bounds__(TILE_THREADS, 2) sweep_tile_kernel(const TileP
             else if (q == 1) { T.cf[0] = 1.0; T.cf[1] = xb; T.cf[2] = xc; T.cf[3] = r2; }
             else if (q == 2) { T.cf[0] = xc * xc; T.cf[1] = xb * xc; T.cf[2] = xb * r2; T.cf[3] = xc * r2; }
             else { T.cf[0] = 1.0; T.cf[1] = xb; T.cf[2] = xc; T.cf[3] = 1.0; }
-            T.mom = c_mom[q][j];
+            T.rawm = P.raw16 + c_mom[q][j];
             T.dsel = 3; T.dsgn = 0.0;
             if (q == 1 && j == 0) { T.dsel = 0; T.dsgn = (double)vb.sx; }
             if (q == 0 && j == 1) { T.dsel = 1; T.dsgn = (double)vb.sy; }
@@ -546,7 +610,7 @@ __global__ void __launch_bounds__(TILE_THREADS, 2) sweep_tile_kernel(const TileP
                     for (int r = 0; r < 4; ++r) pl[jj][ii][r] = rw * G[r];
                 }
         }
-        special = __syncthreads_or(special);
+        special = __shfl_sync(0xffffffffu, __syncthreads_or(special), 0);
 
         const bool write_x = it.ti < P.ntx - 1, write_y = it.tj < P.nty - 1;
         double *xdst = P.xface + ((long long)it.vb * P.P + it.xslot) * slot;
@@ -560,15 +624,27 @@ __global__ void __launch_bounds__(TILE_THREADS, 2) sweep_tile_kernel(const TileP
             par[b] ^= 1u;
             double *xout = write_x ? xdst + (long long)kp * LEVEL_DOUBLES : nullptr;
             double *yout = write_y ? ydst + (long long)kp * LEVEL_DOUBLES : nullptr;
-            if (special) compute_level<true>(P, s, b, pl, T, tid, lane, xout, yout);
-            else compute_level<false>(P, s, b, pl, T, tid, lane, xout, yout);
+            if (special) {
+                double tmp[64];
+#pragma unroll
+                for (int c = 0; c < 16; ++c)
+#pragma unroll
+                    for (int r = 0; r < 4; ++r) tmp[c * 4 + r] = pl[c >> 2][c & 3][r];
+                compute_level_slow(P, s, b, tmp, T, tid, lane, xout, yout);
+#pragma unroll
+                for (int c = 0; c < 16; ++c)
+#pragma unroll
+                    for (int r = 0; r < 4; ++r) pl[c >> 2][c & 3][r] = tmp[c * 4 + r];
+            } else {
+                compute_level(P, s, b, pl, T, tid, lane, xout, yout);
+            }
             stage_store(s, b, tid, v0, v1);
             int sp = 0;
             if (kp + 1 < P.nz) {
                 sp = build_tables(P, I, s, kp + 1, tid);
                 fill_faces(I, s, b ^ 1, tid, T.ag, T.yi, T.zi);
             }
-            special = __syncthreads_or(sp);
+            special = __shfl_sync(0xffffffffu, __syncthreads_or(sp), 0);
             if (tid == 0 && kp + 2 < P.nz) {
                 const unsigned bytes = (I.first_x ? 0u : LEVEL_BYTES) + (I.first_y ? 0u : LEVEL_BYTES);
                 fence_proxy_async();
@@ -586,7 +662,7 @@ __global__ void __launch_bounds__(TILE_THREADS, 2) sweep_tile_kernel(const TileP
 
 }  // namespace
 
-size_t tile_smem_bytes() { return sizeof(TileSmem) + 128; }
+size_t tile_smem_bytes() { return sizeof(TileSmem); }
 
 cudaError_t tile_configure(int *ctas_per_sm)
 {
