@@ -90,10 +90,20 @@ def workload_for(args):
     return workloads.config(args.config)
 
 
+# DESIGN.md section 6 (roofline): per phase-space point-update the method needs ~45 fp64 issue slots (SURVEY.md
+# section 8(d): c, c^2, exp factorised per axis, Shakhov factor, numerator, denominator, reciprocal, 13 moment FMAs)
+# = 90 flop, and moves one fp64 value out and back in per tile-face point: 8 B (tile kernel, 4 x 4 columns) or 16 B
+# (slice kernel, in-place slice).  fp64 peak derived from unit counts and clocks: 148 SMs x 64 fp64 lanes x 2 flop
+# x 1.965 GHz = 37.2 TFLOP/s (the DFMA micro-benchmark in profiles/r01_fp64_microbench.txt reaches 34.0).
+ALGO_FP64_SLOTS_PER_POINT = 45.0
+FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
+TRAFFIC_NCU = {  # dram__bytes_read.sum + dram__bytes_write.sum per sweep launch, from profiles/ (None = not captured)
+    "cfg2_cavity_tanh_64^3x32^3_Kn0.075": 65.716e9,
+}
+
+
 def algorithmic_bytes_per_point(kernel_name):
-    # slice kernel reads + writes one fp64 slice value per phase point (in-place slice: 16 B,
-    # plus the y-upwind re-read that is expected to hit L2); tile kernel moves only tile faces.
-    return {"slice": 16.0, "tile": 4.0}[kernel_name]
+    return {"slice": 16.0, "tile": 8.0}[kernel_name]
 
 
 # --------------------------------------------------------------------------------------------------
@@ -222,7 +232,21 @@ def run_gpu(args):
         # dominant kernel = the sweep (one launch per step); its duration is the step minus the five small update
         # launches, measured here as the step itself (upper bound on the sweep time -> lower bound on achieved)
         bpp = algorithmic_bytes_per_point(kname)
-        achieved = bpp * pts / (ms_per_step * 1e-3) / 1e9
+        hbm_gbs = bpp * pts / (ms_per_step * 1e-3) / 1e9
+        tflops = 2.0 * ALGO_FP64_SLOTS_PER_POINT * pts / (ms_per_step * 1e-3) / 1e12
+        # the binding roofline is the slower of the two bounds for this workload
+        t_alu, t_hbm = 2.0 * ALGO_FP64_SLOTS_PER_POINT / (FP64_PEAK_TFLOPS * 1e12), bpp / (peak * 1e9)
+        if t_alu >= t_hbm:
+            roof = {"bound": "alu", "achieved": tflops, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
+                    "frac": tflops / FP64_PEAK_TFLOPS, "traffic": TRAFFIC_NCU.get(wl.name),
+                    "peak_source": "derived: 148 SM x 64 fp64 lanes x 2 flop x 1.965 GHz (DESIGN.md section 6)",
+                    "algorithmic_flop_per_point": 2.0 * ALGO_FP64_SLOTS_PER_POINT}
+        else:
+            roof = {"bound": "hbm", "achieved": hbm_gbs, "peak": peak, "unit": "GB/s", "frac": hbm_gbs / peak,
+                    "traffic": TRAFFIC_NCU.get(wl.name), "peak_source": peak_src}
+        roof.update({"kernel": f"sweep_{kname}_kernel", "algorithmic_bytes_per_point": bpp,
+                     "hbm_achieved_gbs": hbm_gbs, "hbm_peak_gbs": peak, "hbm_frac": hbm_gbs / peak,
+                     "launch_ms": ms_per_step})
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -234,9 +258,7 @@ def run_gpu(args):
                        "workspace_bytes": total_bytes, "f_workspace_bytes": f_bytes,
                        "full_6d_f_bytes_never_allocated": 8 * wl.n_cells * wl.n_vel,
                        "residual_after_run": [float(x) for x in res], "step_ms": [round(x, 3) for x in step_ms]},
-            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": None, "peak_source": peak_src, "kernel": f"sweep_{kname}_kernel",
-                         "algorithmic_bytes_per_point": bpp},
+            "roofline": roof,
             "e2e": {"value": world * pts / (e2e_ms * 1e-3), "unit": UNIT,
                     "h2d_bytes_per_step": 8 * (n8 + s.nface), "d2h_bytes_per_step": 8 * (n14 + s.nface)},
             "gpu_launches": int(launches),

@@ -93,6 +93,15 @@ __device__ __forceinline__ void fence_proxy_async()
 {
     asm volatile("fence.proxy.async;" ::: "memory");
 }
+// generic-proxy accesses to global / shared memory ordered before later async-proxy (TMA) accesses to the same space
+__device__ __forceinline__ void fence_proxy_async_global()
+{
+    asm volatile("fence.proxy.async.global;" ::: "memory");
+}
+__device__ __forceinline__ void fence_proxy_async_smem()
+{
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
 __device__ __forceinline__ int ld_acquire(const int *p)
 {
     int v;
@@ -493,7 +502,7 @@ __global__ void __launch_bounds__(TILE_THREADS, 2) sweep_tile_kernel(const TileP
                 for (int q = 0; q < 3; ++q)
                     if (pred[q] >= 0)
                         while (ld_acquire(P.done + pred[q]) != P.epoch) __nanosleep(64);
-                fence_proxy_async();  // the upwind items' face stores (generic proxy) before our TMA reads
+                fence_proxy_async_global();  // the upwind items' face stores (generic proxy) before our TMA reads
                 // faces of levels 0 and 1 (the staging buffers are free: every thread passed the end-of-item barrier)
                 const bool fx = it.ti == 0, fy = it.tj == 0;
                 const unsigned bytes = (fx ? 0u : LEVEL_BYTES) + (fy ? 0u : LEVEL_BYTES);
@@ -647,7 +656,7 @@ __global__ void __launch_bounds__(TILE_THREADS, 2) sweep_tile_kernel(const TileP
             special = __shfl_sync(0xffffffffu, __syncthreads_or(sp), 0);
             if (tid == 0 && kp + 2 < P.nz) {
                 const unsigned bytes = (I.first_x ? 0u : LEVEL_BYTES) + (I.first_y ? 0u : LEVEL_BYTES);
-                fence_proxy_async();
+                fence_proxy_async_smem();  // this level's reads of the staging buffer before the TMA overwrites it
                 mbar_expect_tx(&s.mbar[b], bytes);
                 if (!I.first_x) tma_load(&s.xface[b][0][0], xdst + (long long)(kp + 2) * LEVEL_DOUBLES, LEVEL_BYTES, &s.mbar[b]);
                 if (!I.first_y) tma_load(&s.yface[b][0][0], ydst + (long long)(kp + 2) * LEVEL_DOUBLES, LEVEL_BYTES, &s.mbar[b]);

@@ -16,7 +16,8 @@ import numpy as np
 
 _PKG = Path(__file__).resolve().parent
 _CSRC = _PKG / "csrc"
-_SO = _PKG / "libdvm_b200.so"
+# DVM_B200_LIB names another build of the same library (kernel experiments); default: the in-tree build
+_SO = Path(os.environ.get("DVM_B200_LIB", str(_PKG / "libdvm_b200.so")))
 _INCLUDE = _PKG.parent / "include"
 
 OK, EINVAL, ENOMEM, ECUDA, ENONFINITE = 0, -1, -2, -3, -4

@@ -145,6 +145,24 @@ def test_config2_shape_sampled_step(oracle_mod, kernel):
     lockstep(wl, kernel, 1, oracle_mod, state=st, rho_w=None)
 
 
+def test_config3_full_size_sampled_step(oracle_mod):
+    """Config 3 at full size (96 x 64 x 64 cells with the 16^3 solid cube, 48^3 shifted velocity grid) in the launch
+    configuration bench.py times (tile kernel): one step from the free-stream state and one from a perturbed state,
+    with a zero-weight velocity subset (4 nodes per axis) so that the oracle finishes in seconds."""
+    wl = W.sparse_weight_subset(W.config(3), keep=4)
+    lockstep(wl, 2, 1, oracle_mod)
+    lockstep(wl, 2, 1, oracle_mod, state=W.perturbed_state(wl, seed=3), rho_w=None)
+
+
+def test_config4_full_size_sampled_step(oracle_mod):
+    """Config 4 at full size (128^3 cells x 64^3 velocities: 5.5e11 phase points swept by the GPU) with a zero-weight
+    subset of 4 nodes per axis (the oracle sweeps 64 velocities): one step from a perturbed state; raw moments, wall
+    fluxes, wall densities, fields and residual must agree.  Also checks that f is never materialised."""
+    wl = W.sparse_weight_subset(W.config(4), keep=4)
+    st = W.perturbed_state(wl, seed=4)
+    lockstep(wl, 2, 1, oracle_mod, state=st, rho_w=None)
+
+
 def test_errors_and_state_roundtrip():
     from paper_1810_00348_b200 import dvm
     wl = W.config(0)
