@@ -200,8 +200,8 @@ __device__ __forceinline__ int build_tables(const TileParams &P, const ItemCtx &
 {
     const int b = kp & 1;
     int special = 0;
-    if (tid < 16) {
-        const int cell = tid, fl = s.cflag[b][cell];
+    if (tid >= 96 && tid < 112) {   // warp 3: warps 0 and 1 already carry the extra metadata roles
+        const int cell = tid - 96, fl = s.cflag[b][cell];
         int i, j, k;
         cell_of(P, I, cell & 3, cell >> 2, kp, i, j, k);
         const long long c = ((long long)k * P.ny + j) * P.nx + i;
@@ -312,6 +312,28 @@ __device__ __forceinline__ double reduce_half(double S0, double S1, double S2, d
     return (b3 ? k1 : k0) + shx(b3 ? k0 : k1, 8);
 }
 
+// The same reduction for two cells at once, stage by stage, so that the shuffle latency of one cell is covered by
+// the other cell's instructions.
+__device__ __forceinline__ void reduce_half2(const double (&A)[4], const double (&B)[4], const double (&cf)[4], int lane,
+                                             double &kA, double &kB)
+{
+    const bool b0 = lane & 1, b1 = lane & 2, b2 = lane & 4, b3 = lane & 8;
+    double a0 = A[0] + shx(A[0], 1), c0 = B[0] + shx(B[0], 1);
+    double ua = (b1 ? A[2] : A[1]) + shx(b1 ? A[1] : A[2], 2), ub = (b1 ? B[2] : B[1]) + shx(b1 ? B[1] : B[2], 2);
+    double va = A[3] + shx(b1 ? 0.0 : A[3], 2), vb = B[3] + shx(b1 ? 0.0 : B[3], 2);
+    a0 += shx(a0, 2); c0 += shx(c0, 2);
+    ua += shx(ua, 1); ub += shx(ub, 1);
+    va += shx(va, 1); vb += shx(vb, 1);
+    const double Ua = b0 ? ua : a0, Ub = b0 ? ub : c0;
+    const double Va = (b0 && b1) ? va : Ua, Vb = (b0 && b1) ? vb : Ub;
+    const double oa0 = cf[0] * Ua, oa1 = cf[1] * Ua, oa2 = cf[2] * Ua, oa3 = cf[3] * Va;
+    const double ob0 = cf[0] * Ub, ob1 = cf[1] * Ub, ob2 = cf[2] * Ub, ob3 = cf[3] * Vb;
+    const double ka0 = (b2 ? oa2 : oa0) + shx(b2 ? oa0 : oa2, 4), kb0 = (b2 ? ob2 : ob0) + shx(b2 ? ob0 : ob2, 4);
+    const double ka1 = (b2 ? oa3 : oa1) + shx(b2 ? oa1 : oa3, 4), kb1 = (b2 ? ob3 : ob1) + shx(b2 ? ob1 : ob3, 4);
+    kA = (b3 ? ka1 : ka0) + shx(b3 ? ka0 : ka1, 8);
+    kB = (b3 ? kb1 : kb0) + shx(b3 ? kb0 : kb1, 8);
+}
+
 // per-thread constants of an item
 struct ThreadCtx {
     double X1[4], X2[4], X3[4];  // xi_x, xi_x^2, xi_x^3 of the thread's nodes
@@ -353,7 +375,7 @@ __device__ __forceinline__ void compute_level(const TileParams &P, TileSmem &s, 
             const double2 v0 = p[0], v1 = p[1];
             fx[0] = v0.x; fx[1] = v0.y; fx[2] = v1.x; fx[3] = v1.y;
         }
-        double kprev = 0.0;
+        double SA[4] = {0.0, 0.0, 0.0, 0.0};
 #pragma unroll
         for (int ii = 0; ii < 4; ++ii) {
             const int cell = jj * 4 + ii;
@@ -388,9 +410,14 @@ __device__ __forceinline__ void compute_level(const TileParams &P, TileSmem &s, 
                 S2 = fma(T.X2[r], gg, S2);
                 S3 = fma(T.X3[r], gg, S3);
             }
-            const double kk = reduce_half(S0, S1, S2, S3, T.cf, lane);
-            if (ii & 1) emit_pair(P, s, b, cell - 1, kprev, kk, T, lane);
-            else kprev = kk;
+            if (ii & 1) {
+                const double SB[4] = {S0, S1, S2, S3};
+                double kA, kB;
+                reduce_half2(SA, SB, T.cf, lane, kA, kB);
+                emit_pair(P, s, b, cell - 1, kA, kB, T, lane);
+            } else {
+                SA[0] = S0; SA[1] = S1; SA[2] = S2; SA[3] = S3;
+            }
         }
         if (xout) {
             double2 *p = reinterpret_cast<double2 *>(xout + jj * NVB + tid * 4);
@@ -654,7 +681,7 @@ __global__ void __launch_bounds__(TILE_THREADS, 2) sweep_tile_kernel(const TileP
                 fill_faces(I, s, b ^ 1, tid, T.ag, T.yi, T.zi);
             }
             special = __shfl_sync(0xffffffffu, __syncthreads_or(sp), 0);
-            if (tid == 0 && kp + 2 < P.nz) {
+            if (tid == 64 && kp + 2 < P.nz) {
                 const unsigned bytes = (I.first_x ? 0u : LEVEL_BYTES) + (I.first_y ? 0u : LEVEL_BYTES);
                 fence_proxy_async_smem();  // this level's reads of the staging buffer before the TMA overwrites it
                 mbar_expect_tx(&s.mbar[b], bytes);
