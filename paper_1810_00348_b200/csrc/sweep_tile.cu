@@ -33,6 +33,7 @@ namespace {
 
 constexpr int NVB = TILE_NVB;
 constexpr int NCELL = TILE_NCELL;
+constexpr int RB = 4;                                  // cells of a row whose moment reductions are interleaved
 constexpr int LEVEL_DOUBLES = 4 * NVB;                 // one level of an x- or y-face slot
 constexpr unsigned LEVEL_BYTES = LEVEL_DOUBLES * 8u;   // 16 KB
 
@@ -312,26 +313,36 @@ __device__ __forceinline__ double reduce_half(double S0, double S1, double S2, d
     return (b3 ? k1 : k0) + shx(b3 ? k0 : k1, 8);
 }
 
-// The same reduction for two cells at once, stage by stage, so that the shuffle latency of one cell is covered by
-// the other cell's instructions.
-__device__ __forceinline__ void reduce_half2(const double (&A)[4], const double (&B)[4], const double (&cf)[4], int lane,
-                                             double &kA, double &kB)
+// The same reduction for N cells at once, stage by stage, so that the shuffle latency of one cell is covered by the
+// other cells' instructions.  S[c][p] = power sum p of cell c; k[c] = result of cell c.
+template <int N>
+__device__ __forceinline__ void reduce_halfN(const double (&S)[N][4], const double (&cf)[4], int lane, double (&k)[N])
 {
     const bool b0 = lane & 1, b1 = lane & 2, b2 = lane & 4, b3 = lane & 8;
-    double a0 = A[0] + shx(A[0], 1), c0 = B[0] + shx(B[0], 1);
-    double ua = (b1 ? A[2] : A[1]) + shx(b1 ? A[1] : A[2], 2), ub = (b1 ? B[2] : B[1]) + shx(b1 ? B[1] : B[2], 2);
-    double va = A[3] + shx(b1 ? 0.0 : A[3], 2), vb = B[3] + shx(b1 ? 0.0 : B[3], 2);
-    a0 += shx(a0, 2); c0 += shx(c0, 2);
-    ua += shx(ua, 1); ub += shx(ub, 1);
-    va += shx(va, 1); vb += shx(vb, 1);
-    const double Ua = b0 ? ua : a0, Ub = b0 ? ub : c0;
-    const double Va = (b0 && b1) ? va : Ua, Vb = (b0 && b1) ? vb : Ub;
-    const double oa0 = cf[0] * Ua, oa1 = cf[1] * Ua, oa2 = cf[2] * Ua, oa3 = cf[3] * Va;
-    const double ob0 = cf[0] * Ub, ob1 = cf[1] * Ub, ob2 = cf[2] * Ub, ob3 = cf[3] * Vb;
-    const double ka0 = (b2 ? oa2 : oa0) + shx(b2 ? oa0 : oa2, 4), kb0 = (b2 ? ob2 : ob0) + shx(b2 ? ob0 : ob2, 4);
-    const double ka1 = (b2 ? oa3 : oa1) + shx(b2 ? oa1 : oa3, 4), kb1 = (b2 ? ob3 : ob1) + shx(b2 ? ob1 : ob3, 4);
-    kA = (b3 ? ka1 : ka0) + shx(b3 ? ka0 : ka1, 8);
-    kB = (b3 ? kb1 : kb0) + shx(b3 ? kb0 : kb1, 8);
+    double a0[N], u[N], v[N];
+#pragma unroll
+    for (int c = 0; c < N; ++c) a0[c] = S[c][0] + shx(S[c][0], 1);
+#pragma unroll
+    for (int c = 0; c < N; ++c) u[c] = (b1 ? S[c][2] : S[c][1]) + shx(b1 ? S[c][1] : S[c][2], 2);
+#pragma unroll
+    for (int c = 0; c < N; ++c) v[c] = S[c][3] + shx(b1 ? 0.0 : S[c][3], 2);
+#pragma unroll
+    for (int c = 0; c < N; ++c) a0[c] += shx(a0[c], 2);
+#pragma unroll
+    for (int c = 0; c < N; ++c) u[c] += shx(u[c], 1);
+#pragma unroll
+    for (int c = 0; c < N; ++c) v[c] += shx(v[c], 1);
+    double k0[N], k1[N];
+#pragma unroll
+    for (int c = 0; c < N; ++c) {
+        const double U = b0 ? u[c] : a0[c];
+        const double V = (b0 && b1) ? v[c] : U;
+        const double o0 = cf[0] * U, o1 = cf[1] * U, o2 = cf[2] * U, o3 = cf[3] * V;
+        k0[c] = (b2 ? o2 : o0) + shx(b2 ? o0 : o2, 4);
+        k1[c] = (b2 ? o3 : o1) + shx(b2 ? o1 : o3, 4);
+    }
+#pragma unroll
+    for (int c = 0; c < N; ++c) k[c] = (b3 ? k1[c] : k0[c]) + shx(b3 ? k0[c] : k1[c], 8);
 }
 
 // per-thread constants of an item
@@ -375,7 +386,7 @@ __device__ __forceinline__ void compute_level(const TileParams &P, TileSmem &s, 
             const double2 v0 = p[0], v1 = p[1];
             fx[0] = v0.x; fx[1] = v0.y; fx[2] = v1.x; fx[3] = v1.y;
         }
-        double SA[4] = {0.0, 0.0, 0.0, 0.0};
+        double SR[RB][4];
 #pragma unroll
         for (int ii = 0; ii < 4; ++ii) {
             const int cell = jj * 4 + ii;
@@ -410,13 +421,12 @@ __device__ __forceinline__ void compute_level(const TileParams &P, TileSmem &s, 
                 S2 = fma(T.X2[r], gg, S2);
                 S3 = fma(T.X3[r], gg, S3);
             }
-            if (ii & 1) {
-                const double SB[4] = {S0, S1, S2, S3};
-                double kA, kB;
-                reduce_half2(SA, SB, T.cf, lane, kA, kB);
-                emit_pair(P, s, b, cell - 1, kA, kB, T, lane);
-            } else {
-                SA[0] = S0; SA[1] = S1; SA[2] = S2; SA[3] = S3;
+            SR[ii % RB][0] = S0; SR[ii % RB][1] = S1; SR[ii % RB][2] = S2; SR[ii % RB][3] = S3;
+            if (ii % RB == RB - 1) {
+                double k[RB];
+                reduce_halfN<RB>(SR, T.cf, lane, k);
+#pragma unroll
+                for (int c = 0; c < RB; c += 2) emit_pair(P, s, b, cell - (RB - 1) + c, k[c], k[c + 1], T, lane);
             }
         }
         if (xout) {
