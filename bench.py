@@ -98,7 +98,8 @@ def workload_for(args):
 ALGO_FP64_SLOTS_PER_POINT = 45.0
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 TRAFFIC_NCU = {  # dram__bytes_read.sum + dram__bytes_write.sum per sweep launch, from profiles/ (None = not captured)
-    "cfg2_cavity_tanh_64^3x32^3_Kn0.075": 65.716e9,
+    "cfg2_cavity_tanh_64^3x32^3_Kn0.075": 65.510e9,   # profiles/r01_sweep_tile.md (b)
+    "cfg4_cavity_128^3x64^3_Kn0.01": 4.2717e12,       # profiles/r01_sweep_tile.md (a)
 }
 
 
