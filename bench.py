@@ -85,6 +85,20 @@ class ClockSampler:
         return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons), "samples": len(sm)}
 
 
+def max_over_ranks(values, dist, device):
+    """Device-timed figures are taken as the max over ranks (every rank ends up with the same list)."""
+    import torch
+    t = torch.tensor(list(values), dtype=torch.float64, device=device)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return t.tolist()
+
+
+def whole_job_value(world, units_per_rank_step, ms_per_step):
+    """Replicas only: every rank processes the same number of units per step."""
+    return world * units_per_rank_step / (ms_per_step * 1e-3)
+
+
 def workload_for(args):
     from paper_1810_00348_b200 import workloads
     return workloads.config(args.config)
@@ -218,16 +232,13 @@ def run_gpu(args):
     torch.cuda.synchronize(dev)
     e2e_ms = 1e3 * (time.perf_counter() - t0) / e2e_steps
 
-    t = torch.tensor([total_ms, e2e_ms], dtype=torch.float64, device=dev)
-    if dist is not None:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    total_ms, e2e_ms = t.tolist()
+    total_ms, e2e_ms = max_over_ranks([total_ms, e2e_ms], dist, dev)
     total_bytes, f_bytes = s.workspace_bytes()
 
     if rank == 0:
         pts = wl.phase_points
         ms_per_step = total_ms / args.steps
-        value = world * pts / (ms_per_step * 1e-3)
+        value = whole_job_value(world, pts, ms_per_step)
         kname = "slice" if s.kernel_used() == dvm.KERNEL_SLICE else "tile"
         peak, peak_src, _ = measured_peaks()
         # dominant kernel = the sweep (one launch per step); its duration is the step minus the five small update
@@ -260,7 +271,7 @@ def run_gpu(args):
                        "full_6d_f_bytes_never_allocated": 8 * wl.n_cells * wl.n_vel,
                        "residual_after_run": [float(x) for x in res], "step_ms": [round(x, 3) for x in step_ms]},
             "roofline": roof,
-            "e2e": {"value": world * pts / (e2e_ms * 1e-3), "unit": UNIT,
+            "e2e": {"value": whole_job_value(world, pts, e2e_ms), "unit": UNIT,
                     "h2d_bytes_per_step": 8 * (n8 + s.nface), "d2h_bytes_per_step": 8 * (n14 + s.nface)},
             "gpu_launches": int(launches),
             "clocks": clocks,

@@ -1,0 +1,60 @@
+"""Host logic of the tile sweep (no GPU): the work decomposition returned by dvm_plan_query must hand items out in an
+order in which every dependency comes earlier - the property that rules out deadlock of the persistent kernel."""
+import numpy as np
+import pytest
+
+from paper_1810_00348_b200 import dvm, workloads as W
+
+
+def plan(wl, target=296):
+    return dvm.plan_query(wl.nx, wl.ny, wl.nz, wl.xi_x, wl.xi_y, wl.xi_z, target_ctas=target)
+
+
+@pytest.mark.parametrize("wl,target", [
+    (W.config(0), 296), (W.config(1), 296), (W.config(2), 296), (W.config(3), 296),
+    (W.cavity(0, 0, 0.1, nxyz=(13, 9, 11), mxyz=(10, 7, 9)), 296),
+    (W.cavity(0, 0, 0.1, nxyz=(13, 9, 11), mxyz=(10, 7, 9)), 4),
+    (W.cube_flow(4, 12, box=(6, 4, 4), vrange=8.0), 37),
+])
+def test_items_cover_everything_once_in_dependency_order(wl, target):
+    counts, items = plan(wl, target)
+    n = counts["n_items"]
+    assert len(items) == n == counts["n_vblocks"] * counts["ntx"] * counts["nty"]
+    assert counts["ntx"] == -(-wl.nx // 4) and counts["nty"] == -(-wl.ny // 4)
+    vb, ti, tj, px, py, ps, xslot, octant = items.T
+    # every (velocity block, tile) exactly once
+    key = (vb.astype(np.int64) * counts["nty"] + tj) * counts["ntx"] + ti
+    assert len(np.unique(key)) == n
+    idx = np.arange(n)
+    # predecessors are earlier items (or absent) ...
+    for p in (px, py, ps):
+        assert np.all((p == -1) | ((p >= 0) & (p < idx)))
+    # ... and are the right ones: upwind tile in x / y of the same velocity block
+    has = px >= 0
+    assert np.array_equal(ti > 0, has)
+    assert np.all(vb[px[has]] == vb[has]) and np.all(ti[px[has]] == ti[has] - 1) and np.all(tj[px[has]] == tj[has])
+    has = py >= 0
+    assert np.array_equal(tj > 0, has)
+    assert np.all(vb[py[has]] == vb[has]) and np.all(tj[py[has]] == tj[has] - 1) and np.all(ti[py[has]] == ti[has])
+    # x-face slot reuse: the item that overwrites slot tj % P waits for the last reader of the previous user
+    P = counts["P"]
+    assert np.array_equal(xslot, tj % P)
+    has = ps >= 0
+    assert np.array_equal(has, (ti == 0) & (tj >= P))
+    assert np.all(vb[ps[has]] == vb[has]) and np.all(ti[ps[has]] == counts["ntx"] - 1) and np.all(tj[ps[has]] == tj[has] - P)
+
+
+def test_velocity_blocks_partition_the_velocity_grid():
+    """Octants come from node signs (the cube case has a shifted xi_x grid: unequal halves)."""
+    wl = W.config(3)
+    counts, items = plan(wl)
+    assert (wl.xi_x < 0).sum() != (wl.xi_x >= 0).sum()
+    # blocks of 16 x (8 x 4 | 4 x 8) nodes: at least ceil(n/512) per octant, all octants present
+    assert set(np.unique(items[:, 7])) == set(range(8))
+    assert counts["n_vblocks"] >= -(-wl.n_vel // 512)
+
+
+def test_plan_rejects_bad_input():
+    wl = W.config(0)
+    with pytest.raises(dvm.DvmError):
+        dvm.plan_query(0, 8, 8, wl.xi_x, wl.xi_y, wl.xi_z)
