@@ -87,6 +87,13 @@ struct dvm_solver {
     double *d_xface = nullptr, *d_yface = nullptr;
     int tile_grid = 0, epoch = 0;
     std::vector<double> h_rho_w0;
+    // factor tables of the tile kernel (tables.cu)
+    std::vector<CellRec> h_rec;
+    CellRec *d_rec = nullptr;
+    double4 *d_TX = nullptr, *d_TY = nullptr, *d_TZ = nullptr;
+    int *d_xnode = nullptr, *d_ynode = nullptr, *d_znode = nullptr;
+    int nxp = 0, nyp = 0, nxb = 0, nyb = 0, nzb = 0;
+    size_t table_bytes = 0;
 
     void *dalloc(size_t bytes)
     {
@@ -195,7 +202,24 @@ TileParams tile_params(dvm_solver *s)
     P.done = s->d_done; P.counter = s->d_counter; P.epoch = s->epoch;
     P.xface = s->d_xface; P.yface = s->d_yface;
     P.slot_doubles = (long long)s->nz * TILE_TY * TILE_NVB;
+    P.TX = s->d_TX; P.TY = s->d_TY; P.TZ = s->d_TZ; P.rec = s->d_rec;
+    P.nxp = s->nxp; P.nyp = s->nyp; P.nbb = s->tile.nbb; P.ncb = s->tile.ncb;
     return P;
+}
+
+TableParams table_params(dvm_solver *s)
+{
+    TableParams T{};
+    T.nx = s->nx; T.ny = s->ny; T.nz = s->nz; T.nxp = s->nxp; T.nyp = s->nyp;
+    T.nbb = s->tile.nbb; T.ncb = s->tile.ncb; T.nxb = s->nxb; T.nyb = s->nyb; T.nzb = s->nzb;
+    T.ncell = s->ncell; T.coef = s->d_coef; T.flags = s->d_flags;
+    T.invdx = s->d_invdx; T.invdy = s->d_invdy; T.invdz = s->d_invdz;
+    T.xi_x = s->d_xi[0]; T.xi_y = s->d_xi[1]; T.xi_z = s->d_xi[2];
+    T.w_x = s->d_w[0]; T.w_y = s->d_w[1]; T.w_z = s->d_w[2];
+    T.xnode = s->d_xnode; T.ynode = s->d_ynode; T.znode = s->d_znode;
+    for (int d = 0; d < 6; ++d) T.bc_type[d] = s->bc.face[d].type;
+    T.TX = s->d_TX; T.TY = s->d_TY; T.TZ = s->d_TZ; T.rec = s->d_rec;
+    return T;
 }
 
 // index ranges of the negative / non-negative nodes of one axis (nodes ascending)
@@ -254,11 +278,26 @@ int plan(dvm_solver *s)
         s->d_yface = (double *)s->dalloc(s->tile.yface_doubles * sizeof(double));
         if (!s->d_xface || !s->d_yface) return fail(DVM_ENOMEM, "tile face workspace of %zu bytes failed", fbytes);
         s->f_bytes = fbytes;
+        // factor tables on the padded grid: [1-D block][nz][nyp][nxp][width] entries of 32 bytes, zero in the padding
+        {
+            s->nxb = (int)s->tile.xnode.size() / TILE_NA;
+            s->nyb = (int)s->tile.ynode.size() / s->tile.nbb;
+            s->nzb = (int)s->tile.znode.size() / s->tile.ncb;
+            const size_t npc = (size_t)s->nz * s->nyp * s->nxp;
+            const size_t ex = npc * s->tile.xnode.size(), ey = npc * s->tile.ynode.size(), ez = npc * s->tile.znode.size();
+            if (dzeros(s, &s->d_TX, ex) || dzeros(s, &s->d_TY, ey) || dzeros(s, &s->d_TZ, ez)) return DVM_ENOMEM;
+            s->table_bytes = (ex + ey + ez) * sizeof(double4);
+            if (upload(s, &s->d_rec, s->h_rec.data(), s->h_rec.size())) return DVM_ENOMEM;
+            if (upload(s, &s->d_xnode, s->tile.xnode.data(), s->tile.xnode.size())) return DVM_ENOMEM;
+            if (upload(s, &s->d_ynode, s->tile.ynode.data(), s->tile.ynode.size())) return DVM_ENOMEM;
+            if (upload(s, &s->d_znode, s->tile.znode.data(), s->tile.znode.size())) return DVM_ENOMEM;
+        }
         if (upload(s, &s->d_vblocks, s->tile.vblocks.data(), s->tile.vblocks.size())) return DVM_ENOMEM;
         if (upload(s, &s->d_items, s->tile.items.data(), nitems)) return DVM_ENOMEM;
         if (dzeros(s, &s->d_done, nitems)) return DVM_ENOMEM;
         if (dzeros(s, &s->d_counter, 64)) return DVM_ENOMEM;
         CK(cudaStreamSynchronize(s->stream));  // the host vectors above are read asynchronously
+        s->h_rec.clear(); s->h_rec.shrink_to_fit();
         s->planned = true;
         return 0;
     }
@@ -370,6 +409,22 @@ int dvm_create(const dvm_grid *g, const dvm_vgrid *v, const dvm_gas *gas, const 
     }
     s->nface = (int)face_slot.size();
     s->mass0 = mass0;
+    // per-cell records of the padded grid for the tile kernel (static part; nu is written every iteration)
+    s->nxp = nx + 2 * TILE_PAD; s->nyp = ny + 2 * TILE_PAD;
+    {
+        CellRec dead{};
+        dead.nu = 1.0; dead.cidx = -1; dead.flags = 0;
+        for (int d = 0; d < 6; ++d) dead.face[d] = -1;
+        s->h_rec.assign((size_t)nz * s->nyp * s->nxp, dead);
+        for (int k = 0; k < nz; ++k) for (int j = 0; j < ny; ++j) for (int i = 0; i < nx; ++i) {
+            const long long c = ((long long)k * ny + j) * nx + i;
+            if (s->solid[c]) continue;
+            CellRec &r = s->h_rec[((size_t)k * s->nyp + j + TILE_PAD) * s->nxp + i + TILE_PAD];
+            r.cidx = (int)c;
+            r.flags = (int)(flags[c] & 63) | ((int)(sflags[c] & 63) << 8);
+            for (int d = 0; d < 6; ++d) r.face[d] = face_of[(size_t)d * n + c];
+        }
+    }
     for (int d = 0; d < 6; ++d) s->foff[d] = off[d];
     // ---- 1-D factors of the ghost distributions (tile kernel): per BC slot and axis, w(xi) exp(-(xi-u)^2/T), with
     //      (pi T)^{-3/2} (and rho of a free stream) folded into the x factor; zero for zero-gradient slots ----
@@ -495,6 +550,8 @@ int dvm_iterate(dvm_solver *s, int niter)
         if (s->kernel == DVM_KERNEL_SLICE) {
             CK(launch_sweep_slice(P, (int)s->blocks.size(), s->nb_threads, s->stream));
         } else {
+            CK(launch_tables(table_params(s), s->stream));
+            s->launches += 1;
             CK(cudaMemsetAsync(s->d_counter, 0, sizeof(int), s->stream));
             s->epoch += 1;
             const TileParams TP = tile_params(s);

@@ -26,6 +26,7 @@
 #include "sweep_tile.cuh"
 
 #include <cstdint>
+#include <cstdio>
 
 namespace dvm {
 
@@ -37,24 +38,28 @@ constexpr int RB = 4;                                  // cells of a row whose m
 constexpr int LEVEL_DOUBLES = 4 * NVB;                 // one level of an x- or y-face slot
 constexpr unsigned LEVEL_BYTES = LEVEL_DOUBLES * 8u;   // 16 KB
 
+constexpr unsigned XROW_BYTES = 4 * TILE_NA * 32u;      // one 4-cell row of x entries
+constexpr unsigned REC_ROW_BYTES = 4 * (unsigned)sizeof(CellRec);
+
 struct __align__(128) TileSmem {
-    double xface[2][TILE_TY][NVB];                 // staged x-face input, per level parity
-    double yface[2][TILE_TX][NVB];                 // staged y-face input
-    double4 xtab[2][NCELL][TILE_NA];               // per (cell, xi_x node): E, Q, e, a   (node index r*4 + ag)
-    double4 yztab[2][NCELL][TILE_MAXBC];           // per (cell, xi_y node) then (cell, xi_z node)
+    // ---- staged by TMA two levels ahead (index = level parity) ----
+    double xface[2][TILE_TY][NVB];                 // x-face input of the level
+    double yface[2][TILE_TX][NVB];                 // y-face input
+    double4 xtab[2][NCELL][TILE_NA];               // per (cell', xi_x node): E, Q, e, a   (slot r*4 + ag); cell' = row * 4 +
+    double4 ytab[2][NCELL * 8];                    // position of the cell in ascending absolute x;  [cell'][nbb]
+    double4 ztab[2][NCELL * 8];                    // [cell'][ncb]
+    CellRec rec[2][NCELL];                         // per cell': 1/tau, cell index, neighbour flags, boundary faces
+    // ---- decoded per level by 16 threads (sweep-relative cell = jj * 4 + ii) ----
     double nu[2][NCELL];                           // 1/tau (1 for dead cells)
-    double4 spec[2][NCELL];                        // rho_w of a solid ghost in x, y, z (special levels)
-    double stage[2][NCELL][10];                    // coef pack (9) of a level, prefetched two levels ahead
-    double rwb[2][8];                              // ghost densities of the domain faces: 4 x-face rows, 4 y-face columns
-    double invdz[2];
-    double xi_a[TILE_NA], w_a[TILE_NA];            // nodes / weights of the block (0 beyond the box)
-    double xi_bc[TILE_MAXBC], w_bc[TILE_MAXBC];
-    double g[4][3][16];                            // ghost Maxwellian 1-D factors: upwind x, y, z face and solid
-    double invdx[TILE_TX], invdy[TILE_TY];
-    int cflag[2][NCELL];                           // flags | sflags << 8 | in-domain << 16, staged
+    double4 spec[2][NCELL];                        // rho_w of a solid ghost in x, y, z (slow-path levels)
     int code[2][NCELL];                            // 1: x-up solid ghost, 2: y-up, 4: z-up, 8: dead cell
     int cidx[2][NCELL];                            // global cell index or -1 (dead)
     int dnface[2][NCELL][4];                       // wall face downwind in x, y, z (or -1); [3] = -1
+    double rwb[2][8];                              // ghost densities of the domain faces: 4 x-face rows, 4 y-face columns
+    // ---- per item ----
+    double xi_a[TILE_NA];                          // nodes of the block (0 beyond the box)
+    double xi_bc[TILE_MAXBC];
+    double g[4][3][16];                            // ghost Maxwellian 1-D factors: upwind x, y, z face and solid
     unsigned long long mbar[2];
     int item;
 };
@@ -85,6 +90,10 @@ __device__ __forceinline__ void mbar_wait(unsigned long long *b, unsigned parity
 // TMA 1-D bulk copy global -> shared, completion counted on an mbarrier
 __device__ __forceinline__ void tma_load(void *dst, const void *src, unsigned bytes, unsigned long long *b)
 {
+#ifdef DVM_DEBUG_TMA
+    if ((smem_u32(dst) & 15u) || ((unsigned long long)src & 15ull) || (bytes & 15u) || bytes == 0)
+        printf("tma misaligned: dst %u src %p bytes %u (thread %d)\n", smem_u32(dst), src, bytes, (int)threadIdx.x);
+#endif
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
                      smem_u32(dst)),
                  "l"(src), "r"(bytes), "r"(smem_u32(b))
@@ -157,112 +166,85 @@ __device__ __forceinline__ double face_density(const TileParams &P, int type, in
     return type == 1 ? 1.0 : 0.0;
 }
 
-// Loads of the per-level metadata of level kp (two values per thread, roles by tid); kept in registers while the
-// current level is computed, then written to shared memory by stage_store.
-__device__ __forceinline__ void stage_load(const TileParams &P, const ItemCtx &I, int kp, int tid, double &v0, double &v1)
+// Ghost densities of the domain faces of level kp for a tile at the upwind x / y edge of the domain (one value per
+// thread 32..39), loaded two levels ahead into a register and written to shared memory by rwb_store.
+__device__ __forceinline__ double rwb_load(const TileParams &P, const ItemCtx &I, int kp, int tid)
 {
-    v0 = 0.0; v1 = 0.0;
-    if (kp >= P.nz) return;
+    double v = 0.0;
+    if (kp >= P.nz) return v;
     int i, j, k;
-    {
-        const int cell = tid & 15, f = tid >> 4;
-        if (cell_of(P, I, cell & 3, cell >> 2, kp, i, j, k)) v0 = P.coef[(long long)f * P.ncell + ((long long)k * P.ny + j) * P.nx + i];
+    if (tid >= 32 && tid < 36) {
+        if (I.first_x && cell_of(P, I, 0, tid - 32, kp, i, j, k)) v = face_density(P, I.tpx, P.foff[I.upx] + k * P.ny + j);
+    } else if (tid >= 36 && tid < 40) {
+        if (I.first_y && cell_of(P, I, tid - 36, 0, kp, i, j, k)) v = face_density(P, I.tpy, P.foff[I.upy] + k * P.nx + i);
     }
-    if (tid < 16) {
-        if (cell_of(P, I, tid & 3, tid >> 2, kp, i, j, k)) v1 = P.coef[8ll * P.ncell + ((long long)k * P.ny + j) * P.nx + i];
-    } else if (tid < 32) {
-        const int cell = tid - 16;
-        if (cell_of(P, I, cell & 3, cell >> 2, kp, i, j, k)) {
-            const long long c = ((long long)k * P.ny + j) * P.nx + i;
-            v1 = (double)((int)P.flags[c] | ((int)P.sflags[c] << 8) | (1 << 16));
-        }
-    } else if (tid < 36) {
-        if (I.first_x && cell_of(P, I, 0, tid - 32, kp, i, j, k)) v1 = face_density(P, I.tpx, P.foff[I.upx] + k * P.ny + j);
-    } else if (tid < 40) {
-        if (I.first_y && cell_of(P, I, tid - 36, 0, kp, i, j, k)) v1 = face_density(P, I.tpy, P.foff[I.upy] + k * P.nx + i);
-    } else if (tid == 40) {
-        cell_of(P, I, 0, 0, kp, i, j, k);
-        v1 = P.invdz[k];
-    }
+    return v;
 }
 
-__device__ __forceinline__ void stage_store(TileSmem &s, int b, int tid, double v0, double v1)
+__device__ __forceinline__ void rwb_store(TileSmem &s, int b, int tid, double v)
 {
-    s.stage[b][tid & 15][tid >> 4] = v0;
-    if (tid < 16) s.stage[b][tid][8] = v1;
-    else if (tid < 32) s.cflag[b][tid - 16] = (int)v1;
-    else if (tid < 40) s.rwb[b][tid - 32] = v1;
-    else if (tid == 40) s.invdz[b] = v1;
+    if (tid >= 32 && tid < 40) s.rwb[b][tid - 32] = v;
 }
 
-// Tables of level kp into buffer b = kp & 1 (reads stage[b], cflag[b], invdz[b]).  Returns 1 if this thread saw a
-// cell that needs the special path (solid ghost, solid or out-of-domain cell).
-__device__ __forceinline__ int build_tables(const TileParams &P, const ItemCtx &I, TileSmem &s, int kp, int tid)
+// TMA copies of level kp into buffer b = kp & 1: the x- / y-face input and, per 4-cell row, the x, y, z factor-table
+// rows and the cell records (tables.cu; every row is one contiguous run of the padded grid).  Executed by threads
+// 64..79 (one row copy each); thread 64 also posts the byte count and fetches the faces.
+__device__ __forceinline__ void issue_level(const TileParams &P, const ItemCtx &I, TileSmem &s, const VBlock &vb, int kp,
+                                            int tid, const double *xsrc, const double *ysrc)
+{
+    const int b = kp & 1, q = tid - 64;
+    if (q < 0 || q >= 16) return;
+    const unsigned ybytes = 4u * vb.nbb * 32u, zbytes = 4u * vb.ncb * 32u;
+    if (q == 0) {
+        const unsigned faces = (I.first_x ? 0u : LEVEL_BYTES) + (I.first_y ? 0u : LEVEL_BYTES);
+        mbar_expect_tx(&s.mbar[b], faces + 4u * (XROW_BYTES + ybytes + zbytes + REC_ROW_BYTES));
+        if (!I.first_x) tma_load(&s.xface[b][0][0], xsrc + (long long)kp * LEVEL_DOUBLES, LEVEL_BYTES, &s.mbar[b]);
+        if (!I.first_y) tma_load(&s.yface[b][0][0], ysrc + (long long)kp * LEVEL_DOUBLES, LEVEL_BYTES, &s.mbar[b]);
+    }
+    const int jj = q & 3, kind = q >> 2;
+    // first cell (lowest absolute x) of row jj on the padded grid; rows may lie in the dead padding
+    const int jp = I.j0 + jj, ip0 = I.i0;
+    const int j = I.sy > 0 ? jp : P.ny - 1 - jp;
+    const int i = I.sx > 0 ? ip0 : P.nx - 4 - ip0;
+    const int k = I.sz > 0 ? kp : P.nz - 1 - kp;
+    const long long npc = (long long)P.nz * P.nyp * P.nxp;
+    const long long pc = ((long long)k * P.nyp + (j + TILE_PAD)) * P.nxp + (i + TILE_PAD);
+    if (kind == 0) tma_load(&s.xtab[b][jj * 4][0], P.TX + ((long long)vb.xb * npc + pc) * TILE_NA, XROW_BYTES, &s.mbar[b]);
+    else if (kind == 1) tma_load(&s.ytab[b][jj * 4 * vb.nbb], P.TY + ((long long)vb.yb * npc + pc) * vb.nbb, ybytes, &s.mbar[b]);
+    else if (kind == 2) tma_load(&s.ztab[b][jj * 4 * vb.ncb], P.TZ + ((long long)vb.zb * npc + pc) * vb.ncb, zbytes, &s.mbar[b]);
+    else tma_load(&s.rec[b][jj * 4], P.rec + pc, REC_ROW_BYTES, &s.mbar[b]);
+}
+
+// Per-cell records of level kp (buffer b = kp & 1) decoded from the staged CellRec rows by threads 96..111; the caller
+// has waited for the level's TMA copies.  Returns 1 if this thread saw a fluid cell with a solid upwind ghost.
+__device__ __forceinline__ int decode_records(const TileParams &P, const ItemCtx &I, TileSmem &s, int kp, int tid)
 {
     const int b = kp & 1;
     int special = 0;
-    if (tid >= 96 && tid < 112) {   // warp 3: warps 0 and 1 already carry the extra metadata roles
-        const int cell = tid - 96, fl = s.cflag[b][cell];
-        int i, j, k;
-        cell_of(P, I, cell & 3, cell >> 2, kp, i, j, k);
-        const long long c = ((long long)k * P.ny + j) * P.nx + i;
-        const int flags = fl & 0xff, sfl = (fl >> 8) & 0xff;
-        const bool dead = !((fl >> 16) & 1) || (sfl & 64);
+    if (tid >= 96 && tid < 112) {
+        const int cell = tid - 96, ii = cell & 3, jj = cell >> 2;
+        const CellRec &r = s.rec[b][jj * 4 + (I.sx > 0 ? ii : 3 - ii)];
+        const bool dead = r.cidx < 0;
+        const int flags = r.flags & 0xff, sfl = (r.flags >> 8) & 0xff;
         int code = 8;
         double4 sp = make_double4(0.0, 0.0, 0.0, 0.0);
         int dn[3] = {-1, -1, -1};
         if (!dead) {
             code = ((sfl >> I.upx) & 1) | (((sfl >> I.upy) & 1) << 1) | (((sfl >> I.upz) & 1) << 2);
-            if (code & 1) sp.x = P.rho_w[P.face_of[(long long)I.upx * P.ncell + c]];
-            if (code & 2) sp.y = P.rho_w[P.face_of[(long long)I.upy * P.ncell + c]];
-            if (code & 4) sp.z = P.rho_w[P.face_of[(long long)I.upz * P.ncell + c]];
-            const int up[3] = {I.upx, I.upy, I.upz};
-#pragma unroll
-            for (int d = 0; d < 3; ++d) {
-                const int dd = up[d] ^ 1;
-                if ((flags >> dd) & 1) dn[d] = P.face_of[(long long)dd * P.ncell + c];
-            }
+            if (code & 1) sp.x = P.rho_w[r.face[I.upx]];
+            if (code & 2) sp.y = P.rho_w[r.face[I.upy]];
+            if (code & 4) sp.z = P.rho_w[r.face[I.upz]];
+            if ((flags >> (I.upx ^ 1)) & 1) dn[0] = r.face[I.upx ^ 1];
+            if ((flags >> (I.upy ^ 1)) & 1) dn[1] = r.face[I.upy ^ 1];
+            if ((flags >> (I.upz ^ 1)) & 1) dn[2] = r.face[I.upz ^ 1];
         }
         s.code[b][cell] = code;
         s.spec[b][cell] = sp;
-        s.cidx[b][cell] = dead ? -1 : (int)c;
-        s.nu[b][cell] = dead ? 1.0 : s.stage[b][cell][0];
+        s.cidx[b][cell] = r.cidx;
+        s.nu[b][cell] = dead ? 1.0 : r.nu;
         s.dnface[b][cell][0] = dn[0]; s.dnface[b][cell][1] = dn[1]; s.dnface[b][cell][2] = dn[2];
         s.dnface[b][cell][3] = -1;
         special = (code & 7) != 0;
-    }
-    // TILE_NA + nbb + ncb = 28 entries per cell; consecutive threads write consecutive entries of one cell
-    constexpr int NENT = TILE_NA + TILE_MAXBC;
-    for (int e = tid; e < 16 * NENT; e += TILE_THREADS) {
-        const int cell = e / NENT, n = e - cell * NENT;
-        const int fl = s.cflag[b][cell];
-        const bool dead = !((fl >> 16) & 1) || ((fl >> 8) & 64);
-        const double *st = s.stage[b][cell];
-        const double invT = st[2];
-        double xi, w, u, q, h;
-        bool drop;
-        if (n < TILE_NA) {
-            const int al = 4 * (n & 3) + (n >> 2);   // table position r*4+ag  <->  node 4*ag + r
-            xi = s.xi_a[al]; w = s.w_a[al] * (st[0] * st[1]); u = st[3]; q = st[6];
-            h = s.invdx[cell & 3]; drop = (I.i0 + (cell & 3) == 0) && I.tpx == 2;
-        } else if (n < TILE_NA + I.nbb) {
-            const int bl = n - TILE_NA;
-            xi = s.xi_bc[bl]; w = s.w_bc[bl]; u = st[4]; q = st[7];
-            h = s.invdy[cell >> 2]; drop = (I.j0 + (cell >> 2) == 0) && I.tpy == 2;
-        } else {
-            const int cl = n - TILE_NA;
-            xi = s.xi_bc[cl]; w = s.w_bc[cl]; u = st[5]; q = st[8];
-            h = s.invdz[b]; drop = (kp == 0) && I.tpz == 2;
-        }
-        const double c1 = xi - u, t = c1 * c1 * invT;
-        double4 ent;
-        ent.x = w * exp(-t);
-        ent.y = q * c1;
-        ent.z = n < TILE_NA ? 2.0 * t - 5.0 : 2.0 * t;
-        ent.w = drop ? 0.0 : fabs(xi) * h;
-        if (dead) ent = make_double4(0.0, 0.0, 0.0, 0.0);
-        if (n < TILE_NA) s.xtab[b][cell][n] = ent;
-        else s.yztab[b][cell][n - TILE_NA] = ent;
     }
     return special;
 }
@@ -351,7 +333,9 @@ struct ThreadCtx {
     double cf[4];                // expansion coefficients of this lane
     double dsgn;                 // sign of the wall-flux contribution of this lane
     double *rawm;                // raw16 + moment slot of this lane
-    int ag, yi, zi;              // xi_x group, table rows of the thread's xi_y and xi_z nodes
+    int ag, yi, zi;              // xi_x group, rows of the thread's xi_y and xi_z nodes in xi_bc / g
+    int yl, zl, nbb, ncb;        // local xi_y / xi_z index in the block, block shape
+    int xrev;                    // 3 if the sweep runs against x (table rows are in ascending absolute x), else 0
     int dsel;                    // wall-flux direction (3 = none) of this lane
 };
 
@@ -378,7 +362,11 @@ __device__ __forceinline__ void compute_level(const TileParams &P, TileSmem &s, 
                                               const ThreadCtx &T, const int tid, const int lane, double *xout,
                                               double *yout)
 {
-#pragma unroll
+    // The 4 rows of the tile are a real loop: the B200 instruction cache holds 32 KB, and a level loop larger than
+    // that is fetch-bound at 1/3 instruction per clock and scheduler (profiles/r01_ifetch_microbench.txt); the
+    // fully unrolled level was 48 KB.  The plane stays in registers with static indices: every iteration works on
+    // row slot 0 (old values of row jj -> new values) with the new row jj - 1 in slot 3, then the slots rotate.
+#pragma unroll 1
     for (int jj = 0; jj < 4; ++jj) {
         double fx[4];
         {
@@ -386,36 +374,42 @@ __device__ __forceinline__ void compute_level(const TileParams &P, TileSmem &s, 
             const double2 v0 = p[0], v1 = p[1];
             fx[0] = v0.x; fx[1] = v0.y; fx[2] = v1.x; fx[3] = v1.y;
         }
+        // y-upwind operands: the staged y-face for the first row, else the row computed in the previous iteration
+        double yu[4][4];
+#pragma unroll
+        for (int ii = 0; ii < 4; ++ii)
+#pragma unroll
+            for (int r = 0; r < 4; ++r) yu[ii][r] = pl[3][ii][r];
+        if (jj == 0) {
+#pragma unroll
+            for (int ii = 0; ii < 4; ++ii) {
+                const double2 *p = reinterpret_cast<const double2 *>(&s.yface[b][ii][tid * 4]);
+                const double2 v0 = p[0], v1 = p[1];
+                yu[ii][0] = v0.x; yu[ii][1] = v0.y; yu[ii][2] = v1.x; yu[ii][3] = v1.y;
+            }
+        }
         double SR[RB][4];
 #pragma unroll
         for (int ii = 0; ii < 4; ++ii) {
             const int cell = jj * 4 + ii;
-            const double4 yt = s.yztab[b][cell][T.yi];
-            const double4 zt = s.yztab[b][cell][T.zi];
+            const int cp = jj * 4 + (ii ^ T.xrev);   // position of the cell in the staged table rows
+            const double4 yt = s.ytab[b][cp * T.nbb + T.yl];
+            const double4 zt = s.ztab[b][cp * T.ncb + T.zl];
             const double Eyz = yt.x * zt.x, Qyz = yt.y + zt.y, eyz = yt.z + zt.z;
             const double ay = yt.w, az = zt.w;
             const double dyz = (ay + az) + s.nu[b][cell];
-            double yup[4];
-            if (jj == 0) {
-                const double2 *p = reinterpret_cast<const double2 *>(&s.yface[b][ii][tid * 4]);
-                const double2 v0 = p[0], v1 = p[1];
-                yup[0] = v0.x; yup[1] = v0.y; yup[2] = v1.x; yup[3] = v1.y;
-            } else {
-#pragma unroll
-                for (int r = 0; r < 4; ++r) yup[r] = pl[jj - 1][ii][r];
-            }
             double S0 = 0.0, S1 = 0.0, S2 = 0.0, S3 = 0.0;
 #pragma unroll
             for (int r = 0; r < 4; ++r) {
-                const double4 xt = s.xtab[b][cell][r * 4 + T.ag];
+                const double4 xt = s.xtab[b][cp][r * 4 + T.ag];
                 const double src = (xt.x * Eyz) * fma(xt.y + Qyz, xt.z + eyz, 1.0);
                 const double inv = fast_rcp(xt.w + dyz);
-                double num = fma(ay, yup[r], src);
-                num = fma(az, pl[jj][ii][r], num);
+                double num = fma(ay, yu[ii][r], src);
+                num = fma(az, pl[0][ii][r], num);
                 num = fma(xt.w, fx[r], num);
                 const double gg = num * inv;
                 fx[r] = gg;
-                pl[jj][ii][r] = gg;
+                pl[0][ii][r] = gg;
                 S0 += gg;
                 S1 = fma(T.X1[r], gg, S1);
                 S2 = fma(T.X2[r], gg, S2);
@@ -434,6 +428,14 @@ __device__ __forceinline__ void compute_level(const TileParams &P, TileSmem &s, 
             p[0] = make_double2(fx[0], fx[1]);
             p[1] = make_double2(fx[2], fx[3]);
         }
+        // rotate the row slots: (0, 1, 2, 3) <- (1, 2, 3, 0); after the 4th iteration the rows are back in place
+#pragma unroll
+        for (int ii = 0; ii < 4; ++ii)
+#pragma unroll
+            for (int r = 0; r < 4; ++r) {
+                const double t = pl[0][ii][r];
+                pl[0][ii][r] = pl[1][ii][r]; pl[1][ii][r] = pl[2][ii][r]; pl[2][ii][r] = pl[3][ii][r]; pl[3][ii][r] = t;
+            }
     }
     if (yout) {
 #pragma unroll
@@ -462,8 +464,9 @@ __device__ __forceinline__ void compute_level_slow(const TileParams &P, TileSmem
 #pragma unroll 1
         for (int ii = 0; ii < 4; ++ii) {
             const int cell = jj * 4 + ii;
-            const double4 yt = s.yztab[b][cell][T.yi];
-            const double4 zt = s.yztab[b][cell][T.zi];
+            const int cp = jj * 4 + (ii ^ T.xrev);   // position of the cell in the staged table rows
+            const double4 yt = s.ytab[b][cp * T.nbb + T.yl];
+            const double4 zt = s.ztab[b][cp * T.ncb + T.zl];
             const double Eyz = yt.x * zt.x, Qyz = yt.y + zt.y, eyz = yt.z + zt.z;
             const double ay = yt.w, az = zt.w;
             const double dyz = (ay + az) + s.nu[b][cell];
@@ -473,7 +476,7 @@ __device__ __forceinline__ void compute_level_slow(const TileParams &P, TileSmem
 #pragma unroll
             for (int r = 0; r < 4; ++r) {
                 const double Pg = s.g[3][0][4 * T.ag + r] * gyz;
-                const double4 xt = s.xtab[b][cell][r * 4 + T.ag];
+                const double4 xt = s.xtab[b][cp][r * 4 + T.ag];
                 double xu = fx[r], zu = pl[cell * 4 + r];
                 double yu = jj == 0 ? s.yface[b][ii][tid * 4 + r] : pl[(cell - 4) * 4 + r];
                 if (code & 1) xu = sp.x * Pg;
@@ -539,17 +542,6 @@ __global__ void __launch_bounds__(TILE_THREADS, 2) sweep_tile_kernel(const TileP
                 for (int q = 0; q < 3; ++q)
                     if (pred[q] >= 0)
                         while (ld_acquire(P.done + pred[q]) != P.epoch) __nanosleep(64);
-                fence_proxy_async_global();  // the upwind items' face stores (generic proxy) before our TMA reads
-                // faces of levels 0 and 1 (the staging buffers are free: every thread passed the end-of-item barrier)
-                const bool fx = it.ti == 0, fy = it.tj == 0;
-                const unsigned bytes = (fx ? 0u : LEVEL_BYTES) + (fy ? 0u : LEVEL_BYTES);
-                const double *xs = P.xface + ((long long)it.vb * P.P + it.xslot) * slot;
-                const double *ys = P.yface + ((long long)it.vb * P.ntx + it.ti) * slot;
-                for (int kp = 0; kp < 2 && kp < P.nz; ++kp) {
-                    mbar_expect_tx(&s.mbar[kp], bytes);
-                    if (!fx) tma_load(&s.xface[kp][0][0], xs + (long long)kp * LEVEL_DOUBLES, LEVEL_BYTES, &s.mbar[kp]);
-                    if (!fy) tma_load(&s.yface[kp][0][0], ys + (long long)kp * LEVEL_DOUBLES, LEVEL_BYTES, &s.mbar[kp]);
-                }
             }
         }
         __syncthreads();
@@ -565,15 +557,23 @@ __global__ void __launch_bounds__(TILE_THREADS, 2) sweep_tile_kernel(const TileP
         I.tpx = P.bc_type[I.upx]; I.tpy = P.bc_type[I.upy]; I.tpz = P.bc_type[I.upz];
         I.first_x = it.ti == 0; I.first_y = it.tj == 0;
         I.nbb = vb.nbb; I.ncb = vb.ncb;
+        double *xdst = P.xface + ((long long)it.vb * P.P + it.xslot) * slot;
+        double *ydst = P.yface + ((long long)it.vb * P.ntx + it.ti) * slot;
 
-        // ---- per-item tables: nodes, weights, ghost factors, cell widths ----
+        // ---- TMA copies of levels 0 and 1 (the staging buffers are free: every thread passed the end-of-item
+        //      barrier; the upwind items' face stores were made with the generic proxy) ----
+        if (tid >= 64 && tid < 80) {
+            fence_proxy_async_global();
+            issue_level(P, I, s, vb, 0, tid, xdst, ydst);
+            if (P.nz > 1) issue_level(P, I, s, vb, 1, tid, xdst, ydst);
+        }
+        // ---- per-item tables: nodes, ghost factors; ghost densities of the domain faces of levels 0 and 1 ----
         {
             const int slotid[4] = {I.upx, I.upy, I.upz, 6};
             if (tid < 16) {
                 const bool ok = tid < vb.na;
                 const int idx = vb.a0 + tid;
                 s.xi_a[tid] = ok ? P.xi_x[idx] : 0.0;
-                s.w_a[tid] = ok ? P.w_x[idx] : 0.0;
 #pragma unroll
                 for (int f = 0; f < 4; ++f) s.g[f][0][tid] = ok ? P.gtab[(long long)(slotid[f] * 3 + 0) * P.gstride + idx] : 0.0;
             } else if (tid < 16 + vb.nbb) {
@@ -581,7 +581,6 @@ __global__ void __launch_bounds__(TILE_THREADS, 2) sweep_tile_kernel(const TileP
                 const bool ok = bl < vb.nb;
                 const int idx = vb.b0 + bl;
                 s.xi_bc[bl] = ok ? P.xi_y[idx] : 0.0;
-                s.w_bc[bl] = ok ? P.w_y[idx] : 0.0;
 #pragma unroll
                 for (int f = 0; f < 4; ++f) s.g[f][1][bl] = ok ? P.gtab[(long long)(slotid[f] * 3 + 1) * P.gstride + idx] : 0.0;
             } else if (tid >= 32 && tid < 32 + vb.ncb) {
@@ -589,34 +588,24 @@ __global__ void __launch_bounds__(TILE_THREADS, 2) sweep_tile_kernel(const TileP
                 const bool ok = cl < vb.nc;
                 const int idx = vb.c0 + cl;
                 s.xi_bc[vb.nbb + cl] = ok ? P.xi_z[idx] : 0.0;
-                s.w_bc[vb.nbb + cl] = ok ? P.w_z[idx] : 0.0;
 #pragma unroll
                 for (int f = 0; f < 4; ++f)
                     s.g[f][2][vb.nbb + cl] = ok ? P.gtab[(long long)(slotid[f] * 3 + 2) * P.gstride + idx] : 0.0;
-            } else if (tid >= 48 && tid < 52) {
-                const int ip = I.i0 + (tid - 48);
-                s.invdx[tid - 48] = ip < P.nx ? P.invdx[vb.sx > 0 ? ip : P.nx - 1 - ip] : 0.0;
-            } else if (tid >= 52 && tid < 56) {
-                const int jp = I.j0 + (tid - 52);
-                s.invdy[tid - 52] = jp < P.ny ? P.invdy[vb.sy > 0 ? jp : P.ny - 1 - jp] : 0.0;
             }
-        }
-        // metadata of levels 0 and 1
-        {
-            double v0, v1;
-            stage_load(P, I, 0, tid, v0, v1);
-            stage_store(s, 0, tid, v0, v1);
-            stage_load(P, I, 1, tid, v0, v1);
-            stage_store(s, 1, tid, v0, v1);
+            rwb_store(s, 0, tid, rwb_load(P, I, 0, tid));
+            rwb_store(s, 1, tid, rwb_load(P, I, 1, tid));
         }
         __syncthreads();
 
         ThreadCtx T;
         T.ag = lane & 3;
+        T.nbb = vb.nbb; T.ncb = vb.ncb;
+        T.xrev = vb.sx > 0 ? 0 : 3;
         {
             const int pair = warp * 8 + (lane >> 2);
-            T.yi = pair % vb.nbb;
-            T.zi = vb.nbb + pair / vb.nbb;
+            T.yl = pair % vb.nbb; T.zl = pair / vb.nbb;
+            T.yi = T.yl;
+            T.zi = vb.nbb + T.zl;
             const double xb = s.xi_bc[T.yi], xc = s.xi_bc[T.zi], r2 = xb * xb + xc * xc;
             const int q = lane & 3, j = ((lane >> 2) & 1) * 2 + ((lane >> 3) & 1);
             if (q == 0) { T.cf[0] = 1.0; T.cf[1] = xb; T.cf[2] = xc; T.cf[3] = xb * xb; }
@@ -635,8 +624,12 @@ __global__ void __launch_bounds__(TILE_THREADS, 2) sweep_tile_kernel(const TileP
             }
         }
 
-        // tables and boundary faces of level 0
-        int special = build_tables(P, I, s, 0, tid);
+        // records and boundary faces of level 0 (its copies were issued above; the wait does not consume the phase)
+        int special = 0;
+        if (tid >= 96 && tid < 112) {
+            mbar_wait(&s.mbar[0], par[0]);
+            special = decode_records(P, I, s, 0, tid);
+        }
         fill_faces(I, s, 0, tid, T.ag, T.yi, T.zi);
         // plane = ghost of the upwind z face of the domain
         double pl[4][4][4];
@@ -659,13 +652,10 @@ __global__ void __launch_bounds__(TILE_THREADS, 2) sweep_tile_kernel(const TileP
         special = __shfl_sync(0xffffffffu, __syncthreads_or(special), 0);
 
         const bool write_x = it.ti < P.ntx - 1, write_y = it.tj < P.nty - 1;
-        double *xdst = P.xface + ((long long)it.vb * P.P + it.xslot) * slot;
-        double *ydst = P.yface + ((long long)it.vb * P.ntx + it.ti) * slot;
 
         for (int kp = 0; kp < P.nz; ++kp) {
             const int b = kp & 1;
-            double v0, v1;
-            stage_load(P, I, kp + 2, tid, v0, v1);
+            const double vrw = rwb_load(P, I, kp + 2, tid);
             mbar_wait(&s.mbar[b], par[b]);
             par[b] ^= 1u;
             double *xout = write_x ? xdst + (long long)kp * LEVEL_DOUBLES : nullptr;
@@ -684,19 +674,19 @@ __global__ void __launch_bounds__(TILE_THREADS, 2) sweep_tile_kernel(const TileP
             } else {
                 compute_level(P, s, b, pl, T, tid, lane, xout, yout);
             }
-            stage_store(s, b, tid, v0, v1);
+            rwb_store(s, b, tid, vrw);
             int sp = 0;
             if (kp + 1 < P.nz) {
-                sp = build_tables(P, I, s, kp + 1, tid);
+                if (tid >= 96 && tid < 112) {
+                    mbar_wait(&s.mbar[b ^ 1], par[b ^ 1]);   // level kp + 1 has landed (issued a level ago)
+                    sp = decode_records(P, I, s, kp + 1, tid);
+                }
                 fill_faces(I, s, b ^ 1, tid, T.ag, T.yi, T.zi);
             }
             special = __shfl_sync(0xffffffffu, __syncthreads_or(sp), 0);
-            if (tid == 64 && kp + 2 < P.nz) {
-                const unsigned bytes = (I.first_x ? 0u : LEVEL_BYTES) + (I.first_y ? 0u : LEVEL_BYTES);
-                fence_proxy_async_smem();  // this level's reads of the staging buffer before the TMA overwrites it
-                mbar_expect_tx(&s.mbar[b], bytes);
-                if (!I.first_x) tma_load(&s.xface[b][0][0], xdst + (long long)(kp + 2) * LEVEL_DOUBLES, LEVEL_BYTES, &s.mbar[b]);
-                if (!I.first_y) tma_load(&s.yface[b][0][0], ydst + (long long)(kp + 2) * LEVEL_DOUBLES, LEVEL_BYTES, &s.mbar[b]);
+            if (tid >= 64 && tid < 80 && kp + 2 < P.nz) {
+                fence_proxy_async_smem();  // this level's reads of the staging buffers before the TMA overwrites them
+                issue_level(P, I, s, vb, kp + 2, tid, xdst, ydst);
             }
         }
         // ---- publish: faces of this item are complete ----

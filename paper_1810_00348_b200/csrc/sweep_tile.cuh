@@ -27,6 +27,17 @@ constexpr int TILE_WARPS = TILE_THREADS / 32;
 constexpr int TILE_NVB = TILE_THREADS * TILE_RV;  // velocities per block (incl. padding)
 constexpr int TILE_NPAIR = TILE_THREADS / TILE_GA; // (xi_y, xi_z) pairs per block
 constexpr int TILE_MAXBC = 12;             // nbb + ncb of a block
+constexpr int TILE_PAD = 4;                // dead cells around the grid in the factor tables (tiles may overhang by 3)
+
+// per-cell record of the padded grid, fetched by TMA with the factor tables (48 bytes)
+struct CellRec {
+    double nu;        // 1/tau of step n (written by the table kernel every iteration)
+    int cidx;         // cell index, -1 for padding and solid cells
+    int flags;        // bits 0..5: neighbour in direction d is not fluid; bits 8..13: it is a solid cell
+    int face[6];      // boundary-face slot in direction d or -1
+    int pad[2];       // 48 bytes: every row of records starts on a 16-byte boundary (TMA)
+};
+static_assert(sizeof(CellRec) == 48, "CellRec rows must be 16-byte aligned");
 
 // velocity block: node-index box [a0, a0+na) x [b0, b0+nb) x [c0, c0+nc), na <= 16, nb <= nbb, nc <= ncb,
 // nbb * ncb = 32; lanes beyond the box carry weight 0
@@ -34,7 +45,8 @@ struct VBlock {
     int a0, na, b0, nb, c0, nc;
     int nbb, ncb;
     int sx, sy, sz;   // sweep direction per axis: +1 ascending (xi >= 0), -1 descending
-    int pad;
+    int xb, yb, zb;   // 1-D block ids: rows of the factor tables TX / TY / TZ this block reads
+    int pad[2];
 };
 
 // work item; ti, tj are sweep-relative tile coordinates (0 = most upwind)
@@ -50,6 +62,9 @@ struct TileItem {
 
 struct TilePlan {
     int ntx = 0, nty = 0, P = 1;
+    int nbb = 8, ncb = 4;              // one (xi_y, xi_z) block shape for the whole problem
+    std::vector<int> xnode, ynode, znode;   // node index per 1-D block slot (-1 = padding): [nxb][16], [nyb][nbb], [nzb][ncb];
+                                            // xnode is in table order: slot r*4 + ag holds node 4*ag + r of the block
     std::vector<VBlock> vblocks;
     std::vector<TileItem> items;
     size_t xface_doubles = 0, yface_doubles = 0;
@@ -79,6 +94,23 @@ struct TileParams {
     int epoch;
     double *xface, *yface;
     long long slot_doubles;       // nz * 4 * TILE_NVB
+    // factor tables of step n (tables_kernel), padded grid nxp x nyp x nz, entries double4 (E, Q, e, a):
+    const double4 *TX, *TY, *TZ;  // [nxb][nz][nyp][nxp][16], [nyb][nz][nyp][nxp][nbb], [nzb][nz][nyp][nxp][ncb]
+    const CellRec *rec;           // [nz][nyp][nxp]
+    int nxp, nyp, nbb, ncb;
+};
+
+struct TableParams {
+    int nx, ny, nz, nxp, nyp, nbb, ncb, nxb, nyb, nzb;
+    long long ncell;
+    const double *coef;           // [NCOEF][ncell]
+    const unsigned char *flags;   // bit 6: solid
+    const double *invdx, *invdy, *invdz;
+    const double *xi_x, *xi_y, *xi_z, *w_x, *w_y, *w_z;
+    const int *xnode, *ynode, *znode;
+    int bc_type[6];
+    double4 *TX, *TY, *TZ;
+    CellRec *rec;
 };
 
 // Build velocity blocks, items and their order for a grid and a set of velocity nodes.  target_ctas = number of
@@ -89,5 +121,6 @@ int tile_plan(int nx, int ny, int nz, const std::vector<double> xi[3], int targe
 size_t tile_smem_bytes();
 cudaError_t tile_configure(int *ctas_per_sm);
 cudaError_t launch_sweep_tile(const TileParams &P, int grid, cudaStream_t st);
+cudaError_t launch_tables(const TableParams &T, cudaStream_t st);
 
 }  // namespace dvm

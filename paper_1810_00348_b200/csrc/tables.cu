@@ -1,0 +1,64 @@
+// tables.cu - the 1-D factor tables of the tile sweep kernel, rebuilt once per outer iteration from the per-cell pack
+// of step n (a1/a2 of DESIGN.md): on the tensor velocity grid the source term of Eq.(7) factorises,
+//   f^S / tau = [E_x E_y E_z] [1 + (Q_x + Q_y + Q_z)(e_x + e_y + e_z)]      (Eq.(2)),
+// so one entry (E, Q, e, a) per (cell, 1-D node) is all the sweep needs: E = w exp(-(xi-u)^2/T) (the x entry also
+// carries rho (pi T)^{-3/2} / tau), Q = q'(xi-u), e = 2 (xi-u)^2/T (- 5 in x), a = |xi| / cell width (Eq.(7),
+// PAPER.md:77; 0 where the upwind face is a zero-gradient boundary, i.e. the term is dropped).
+// The tables live on a grid padded by TILE_PAD dead cells (all-zero entries) so that every 4-cell row of a tile is one
+// contiguous run the sweep kernel fetches with a single TMA bulk copy.  O(cells x (mx + my + mz)) work and bytes.
+// Product code: shares nothing with oracle/.
+#include "sweep_tile.cuh"
+
+namespace dvm {
+
+__global__ void __launch_bounds__(256) tables_kernel(const TableParams T)
+{
+    const int sx = T.nxb * TILE_NA, sy = T.nyb * T.nbb, sz = T.nzb * T.ncb;
+    const long long nslot = sx + sy + sz;
+    const long long npc = (long long)T.nz * T.nyp * T.nxp;   // padded cells
+    const long long n = T.ncell;
+    for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < n * nslot;
+         idx += (long long)gridDim.x * blockDim.x) {
+        const long long c = idx / nslot;
+        const int sl = (int)(idx - c * nslot);
+        const int i = (int)(c % T.nx), j = (int)((c / T.nx) % T.ny), k = (int)(c / ((long long)T.nx * T.ny));
+        const long long pc = ((long long)k * T.nyp + (j + TILE_PAD)) * T.nxp + (i + TILE_PAD);
+        int d, m, pos, width, blk;
+        double4 *dst;
+        if (sl < sx) { d = 0; width = TILE_NA; blk = sl / width; pos = sl - blk * width; m = T.xnode[sl]; dst = T.TX; }
+        else if (sl < sx + sy) { d = 1; width = T.nbb; const int t = sl - sx; blk = t / width; pos = t - blk * width; m = T.ynode[t]; dst = T.TY; }
+        else { d = 2; width = T.ncb; const int t = sl - sx - sy; blk = t / width; pos = t - blk * width; m = T.znode[t]; dst = T.TZ; }
+        const bool solid = T.flags[c] & FLAG_SOLID;
+        const double nu = T.coef[c];
+        double4 ent = make_double4(0.0, 0.0, 0.0, 0.0);
+        if (!solid && m >= 0) {
+            const double invT = T.coef[2 * n + c], u = T.coef[(3 + d) * n + c], q = T.coef[(6 + d) * n + c];
+            const double xi = d == 0 ? T.xi_x[m] : d == 1 ? T.xi_y[m] : T.xi_z[m];
+            double w = d == 0 ? T.w_x[m] : d == 1 ? T.w_y[m] : T.w_z[m];
+            if (d == 0) w *= nu * T.coef[n + c];
+            const int id = d == 0 ? i : d == 1 ? j : k, nd = d == 0 ? T.nx : d == 1 ? T.ny : T.nz;
+            const double h = d == 0 ? T.invdx[i] : d == 1 ? T.invdy[j] : T.invdz[k];
+            const bool pos_dir = xi >= 0.0;   // sweeps ascending: the upwind face is the low one
+            const bool first = pos_dir ? id == 0 : id == nd - 1;
+            const bool drop = first && T.bc_type[2 * d + (pos_dir ? 0 : 1)] == 2;
+            const double c1 = xi - u, t = c1 * c1 * invT;
+            ent.x = w * exp(-t);
+            ent.y = q * c1;
+            ent.z = d == 0 ? 2.0 * t - 5.0 : 2.0 * t;
+            ent.w = drop ? 0.0 : fabs(xi) * h;
+        }
+        dst[((long long)blk * npc + pc) * width + pos] = ent;
+        if (sl == 0) T.rec[pc].nu = solid ? 1.0 : nu;
+    }
+}
+
+cudaError_t launch_tables(const TableParams &T, cudaStream_t st)
+{
+    const long long work = T.ncell * ((long long)T.nxb * TILE_NA + (long long)T.nyb * T.nbb + (long long)T.nzb * T.ncb);
+    const long long blocks = (work + 255) / 256;
+    const int grid = (int)(blocks < 148LL * 32 ? blocks : 148LL * 32);
+    tables_kernel<<<grid, 256, 0, st>>>(T);
+    return cudaGetLastError();
+}
+
+}  // namespace dvm
