@@ -366,6 +366,14 @@ __device__ __forceinline__ void compute_level(const TileParams &P, TileSmem &s, 
     // that is fetch-bound at 1/3 instruction per clock and scheduler (profiles/r01_ifetch_microbench.txt); the
     // fully unrolled level was 48 KB.  The plane stays in registers with static indices: every iteration works on
     // row slot 0 (old values of row jj -> new values) with the new row jj - 1 in slot 3, then the slots rotate.
+    // y-upwind operands of the row: the staged y-face for the first row, then the row just computed
+    double yu[4][4];
+#pragma unroll
+    for (int ii = 0; ii < 4; ++ii) {
+        const double2 *p = reinterpret_cast<const double2 *>(&s.yface[b][ii][tid * 4]);
+        const double2 v0 = p[0], v1 = p[1];
+        yu[ii][0] = v0.x; yu[ii][1] = v0.y; yu[ii][2] = v1.x; yu[ii][3] = v1.y;
+    }
 #pragma unroll 1
     for (int jj = 0; jj < 4; ++jj) {
         double fx[4];
@@ -373,20 +381,6 @@ __device__ __forceinline__ void compute_level(const TileParams &P, TileSmem &s, 
             const double2 *p = reinterpret_cast<const double2 *>(&s.xface[b][jj][tid * 4]);
             const double2 v0 = p[0], v1 = p[1];
             fx[0] = v0.x; fx[1] = v0.y; fx[2] = v1.x; fx[3] = v1.y;
-        }
-        // y-upwind operands: the staged y-face for the first row, else the row computed in the previous iteration
-        double yu[4][4];
-#pragma unroll
-        for (int ii = 0; ii < 4; ++ii)
-#pragma unroll
-            for (int r = 0; r < 4; ++r) yu[ii][r] = pl[3][ii][r];
-        if (jj == 0) {
-#pragma unroll
-            for (int ii = 0; ii < 4; ++ii) {
-                const double2 *p = reinterpret_cast<const double2 *>(&s.yface[b][ii][tid * 4]);
-                const double2 v0 = p[0], v1 = p[1];
-                yu[ii][0] = v0.x; yu[ii][1] = v0.y; yu[ii][2] = v1.x; yu[ii][3] = v1.y;
-            }
         }
         double SR[RB][4];
 #pragma unroll
@@ -410,6 +404,7 @@ __device__ __forceinline__ void compute_level(const TileParams &P, TileSmem &s, 
                 const double gg = num * inv;
                 fx[r] = gg;
                 pl[0][ii][r] = gg;
+                yu[ii][r] = gg;
                 S0 += gg;
                 S1 = fma(T.X1[r], gg, S1);
                 S2 = fma(T.X2[r], gg, S2);
