@@ -96,7 +96,8 @@ typedef struct {
 } dvm_device;
 
 /* Build a solver: copies all host arrays, allocates its workspace through dev->alloc (no allocation scales
- * with ncell * nvel: only one z-slice worth of f per in-flight velocity is held), sets the uniform initial
+ * with ncell * nvel: the f workspace holds tile faces / one z-slice per in-flight velocity, the factor tables of the tile
+ * kernel ncell * (mx + my + mz) entries), sets the uniform initial
  * state and rho_w^0 (DESIGN.md oracle step 1).  dev may be NULL (default stream, cudaMalloc). */
 int dvm_create(const dvm_grid *grid, const dvm_vgrid *vgrid, const dvm_gas *gas, const dvm_bc *bc,
                const dvm_device *dev, dvm_solver **out);
