@@ -6,7 +6,8 @@
 
 A "step" is one outer iteration (all of DESIGN.md's hot-path rows a1-a7) of the workload.  Default workload:
 BASELINE.json configs[4] (128^3 x 64^3 cavity, Kn = 0.01, memory-reduction path, f never materialised), the
-largest single-GPU configuration and the one the target is stated on; --config picks another.
+largest single-GPU configuration and the one the target is stated on; --config picks another (0-4: BASELINE.json;
+5: the paper's own cube run, 191 x 181 x 181 stretched cells x 48^3 velocities).
 The solver runs on one GPU with no sharding (replicas only): with --gpus N every rank
 runs an independent replica, timing is max over ranks, value = total units / that time.
 Prints ONE JSON line.

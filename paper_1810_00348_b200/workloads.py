@@ -175,6 +175,39 @@ def cube_flow(cells_per_side: int = 16, m: int = 48, *, box=(6, 4, 4), Kn: float
                     faces, FaceBC(WALL_DIFFUSE, 1.0, 1.0, (0.0, 0.0, 0.0)), 0, 0, iterations)
 
 
+def geometric_faces(n_lo: int, n_mid: int, n_hi: int, r_lo: float, r_hi: float, side: float = 1.0) -> np.ndarray:
+    """Faces of an axis with n_mid uniform cells across a body of length `side` centred at 0, and cells growing by the
+    cell-by-cell ratios r_lo / r_hi away from it (1.02 in front and at the sides, 1.03 behind the cube)."""
+    h = side / n_mid
+    lo = -0.5 * side - np.cumsum(h * r_lo ** np.arange(1, n_lo + 1))
+    hi = 0.5 * side + np.cumsum(h * r_hi ** np.arange(1, n_hi + 1))
+    mid = -0.5 * side + h * np.arange(n_mid + 1)
+    return np.concatenate([lo[::-1], mid, hi]).astype(np.float64)
+
+
+def cube_flow_paper(n_cube: int = 31, n_front: int = 75, n_side: int = 75, n_rear: int = 85, m: int = 48, *,
+                    Kn: float = 1.0, Ma: float = 2.0, vrange: float = 4.0, iterations: int = 41, name: str = "") -> Workload:
+    """The paper's own cube workload shape: 191 x 181 x 181 cells with
+    geometric expansion 1.02 (front, sides) / 1.03 (rear) away from a unit cube of n_cube^3 solid cells, Ma = 2, Kn = 1,
+    48^3 velocities on [-4, 4]^3 (not shifted), free-stream Maxwellian for every entering particle.
+    The paper does not give its grid cell by cell: with 31 cells across the cube the lateral count (2 x 75 + 31 = 181) and
+    half-width (6.0) match its 181 cells / 12 units; the streamwise split 75 + 31 + 85 = 191 is ours."""
+    xf = geometric_faces(n_front, n_cube, n_rear, 1.02, 1.03)
+    yf = geometric_faces(n_side, n_cube, n_side, 1.02, 1.02)
+    zf = yf.copy()
+    nx, ny, nz = len(xf) - 1, len(yf) - 1, len(zf) - 1
+    solid = np.zeros((nz, ny, nx), dtype=np.uint8)
+    solid[n_side:n_side + n_cube, n_side:n_side + n_cube, n_front:n_front + n_cube] = 1
+    U_inf = Ma * math.sqrt(5.0 / 6.0)
+    xi_x, w_x = trapezoid_nodes(m, -vrange, vrange)
+    xi_y, w_y = trapezoid_nodes(m, -vrange, vrange)
+    xi_z, w_z = trapezoid_nodes(m, -vrange, vrange)
+    fs = FaceBC(FREESTREAM, 1.0, 1.0, (U_inf, 0.0, 0.0))
+    return Workload(name or f"cube_paper_{nx}x{ny}x{nz}_v{m}", xf, yf, zf, solid,
+                    xi_x, xi_y, xi_z, w_x, w_y, w_z, Kn, 0.81, 2.0 / 3.0, 1.0, (U_inf, 0.0, 0.0), 1.0,
+                    [fs] * 6, FaceBC(WALL_DIFFUSE, 1.0, 1.0, (0.0, 0.0, 0.0)), 0, 0, iterations)
+
+
 def config(idx: int) -> Workload:
     """BASELINE.json configs[idx] as concrete arrays."""
     if idx == 0:
@@ -187,6 +220,8 @@ def config(idx: int) -> Workload:
         return cube_flow(16, 48, iterations=50, name="cfg3_cube_96x64x64_v48^3_Ma2")
     if idx == 4:
         return cavity(128, 64, 0.01, iterations=50, name="cfg4_cavity_128^3x64^3_Kn0.01")
+    if idx == 5:   # not in BASELINE.json: the paper's own cube run
+        return cube_flow_paper(name="cfg5_cube_paper_191x181x181_v48^3_Ma2_Kn1")
     raise ValueError(f"no config {idx}")
 
 

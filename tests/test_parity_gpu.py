@@ -163,6 +163,15 @@ def test_config4_full_size_sampled_step(oracle_mod):
     lockstep(wl, 2, 1, oracle_mod, state=st, rho_w=None)
 
 
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_paper_cube_grid_small(oracle_mod, kernel):
+    """The paper's own cube workload shape at reduced size: geometric
+    cell expansion 1.02 / 1.03 away from the solid cube, unshifted velocity grid on [-4, 4]^3, free stream on all six
+    outer faces, Kn = 1; sizes that are not multiples of the tile (18 x 17 x 17 cells)."""
+    wl = W.cube_flow_paper(5, 6, 6, 7, 12)
+    lockstep(wl, kernel, 3, oracle_mod)
+
+
 def test_P10_paper_iteration_count_soft_pin():
     """Soft pin P10: the paper's cavity run (Kn = 1, 64^3 x 64^3, U_w = 0.1 v_m, velocity range
     [-4, 4]^3, trapezoid rule) reaches its 1e-9 criterion in 36 iterations on a K40.  The criterion's exact form is our
