@@ -59,6 +59,7 @@ struct dvm_solver {
     double mass0 = 0.0;
     int iters = 0;
     int kernel = DVM_KERNEL_AUTO;
+    long long max_f_mbytes = 0;   // cap on the f workspace of the tile kernel (0 = none)
     bool planned = false;
     long long launches = 0;
     // device arrays
@@ -189,6 +190,7 @@ TileParams tile_params(dvm_solver *s)
 {
     TileParams P{};
     P.nx = s->nx; P.ny = s->ny; P.nz = s->nz; P.ntx = s->tile.ntx; P.nty = s->tile.nty; P.P = s->tile.P;
+    P.batch = s->tile.batch;
     P.ncell = s->ncell;
     P.invdx = s->d_invdx; P.invdy = s->d_invdy; P.invdz = s->d_invdz;
     P.flags = s->d_flags; P.sflags = s->d_sflags; P.face_of = s->d_face_of;
@@ -270,7 +272,19 @@ int plan(dvm_solver *s)
         CK(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
         if (per_sm < 1) return fail(DVM_ECUDA, "tile kernel does not fit on an SM");
         const int resident = per_sm * nsm;
-        if (tile_plan(s->nx, s->ny, s->nz, s->xi, resident, &s->tile)) return fail(DVM_EINVAL, "tile plan failed");
+        if (tile_plan(s->nx, s->ny, s->nz, s->xi, resident, 0, &s->tile)) return fail(DVM_EINVAL, "tile plan failed");
+        if (s->max_f_mbytes > 0) {
+            // cap on the f workspace: fewer velocity blocks in flight (batches); the band height P
+            // grows as the batch shrinks, so iterate to a fixed point; one block is the floor
+            const double cap = (double)s->max_f_mbytes * 1048576.0, slot_bytes = (double)s->nz * TILE_TY * TILE_NVB * 8.0;
+            int B = (int)s->tile.vblocks.size();
+            for (int pass = 0; pass < 8; ++pass) {
+                const double need = (double)(s->tile.xface_doubles + s->tile.yface_doubles) * 8.0;
+                if (need <= cap || B == 1) break;
+                B = std::max(1, std::min(B - 1, (int)(cap / ((s->tile.P + s->tile.ntx) * slot_bytes))));
+                if (tile_plan(s->nx, s->ny, s->nz, s->xi, resident, B, &s->tile)) return fail(DVM_EINVAL, "tile plan failed");
+            }
+        }
         const size_t nitems = s->tile.items.size();
         s->tile_grid = (int)std::min<size_t>((size_t)resident, nitems);
         const size_t fbytes = (s->tile.xface_doubles + s->tile.yface_doubles) * sizeof(double);
@@ -534,6 +548,12 @@ int dvm_set_option(dvm_solver *s, int option, int value)
         s->kernel = value;
         return DVM_OK;
     }
+    if (option == DVM_OPT_MAX_F_MBYTES) {
+        if (s->planned) return fail(DVM_EINVAL, "the workspace cap must be set before the first iteration");
+        if (value < 0) return fail(DVM_EINVAL, "negative workspace cap");
+        s->max_f_mbytes = value;
+        return DVM_OK;
+    }
     return fail(DVM_EINVAL, "unknown option %d", option);
 }
 
@@ -668,23 +688,25 @@ int dvm_step_host(dvm_solver *s, const double *host_prim8, const double *host_rh
     return DVM_OK;
 }
 
-int dvm_plan_query(int nx, int ny, int nz, const dvm_vgrid *v, int target_ctas, int *counts4, int *items8, int max_items)
+int dvm_plan_query(int nx, int ny, int nz, const dvm_vgrid *v, int target_ctas, int max_blocks, int *counts5, int *items9,
+                   int max_items)
 {
-    if (!v || !counts4 || nx <= 0 || ny <= 0 || nz <= 0 || v->mx <= 0 || v->my <= 0 || v->mz <= 0 || !v->xi_x || !v->xi_y || !v->xi_z)
+    if (!v || !counts5 || max_blocks < 0 || nx <= 0 || ny <= 0 || nz <= 0 || v->mx <= 0 || v->my <= 0 || v->mz <= 0 || !v->xi_x || !v->xi_y || !v->xi_z)
         return fail(DVM_EINVAL, "bad argument");
     std::vector<double> xi[3];
     xi[0].assign(v->xi_x, v->xi_x + v->mx); xi[1].assign(v->xi_y, v->xi_y + v->my); xi[2].assign(v->xi_z, v->xi_z + v->mz);
     TilePlan tp;
-    if (tile_plan(nx, ny, nz, xi, target_ctas, &tp)) return fail(DVM_EINVAL, "tile plan failed");
-    counts4[0] = (int)tp.vblocks.size(); counts4[1] = tp.ntx; counts4[2] = tp.nty; counts4[3] = tp.P;
+    if (tile_plan(nx, ny, nz, xi, target_ctas, max_blocks, &tp)) return fail(DVM_EINVAL, "tile plan failed");
+    counts5[0] = (int)tp.vblocks.size(); counts5[1] = tp.ntx; counts5[2] = tp.nty; counts5[3] = tp.P; counts5[4] = tp.batch;
     const int n = (int)tp.items.size();
-    if (items8) {
+    if (items9) {
         for (int e = 0; e < n && e < max_items; ++e) {
             const TileItem &it = tp.items[e];
             const VBlock &vb = tp.vblocks[it.vb];
-            int *o = items8 + 8 * e;
+            int *o = items9 + 9 * e;
             o[0] = it.vb; o[1] = it.ti; o[2] = it.tj; o[3] = it.pred_x; o[4] = it.pred_y; o[5] = it.pred_s; o[6] = it.xslot;
             o[7] = (vb.sx > 0) | ((vb.sy > 0) << 1) | ((vb.sz > 0) << 2);
+            o[8] = it.fslot;
         }
     }
     return n;

@@ -552,8 +552,8 @@ __global__ void __launch_bounds__(TILE_THREADS, 2) sweep_tile_kernel(const TileP
         I.tpx = P.bc_type[I.upx]; I.tpy = P.bc_type[I.upy]; I.tpz = P.bc_type[I.upz];
         I.first_x = it.ti == 0; I.first_y = it.tj == 0;
         I.nbb = vb.nbb; I.ncb = vb.ncb;
-        double *xdst = P.xface + ((long long)it.vb * P.P + it.xslot) * slot;
-        double *ydst = P.yface + ((long long)it.vb * P.ntx + it.ti) * slot;
+        double *xdst = P.xface + ((long long)(it.vb % P.batch) * P.P + it.xslot) * slot;
+        double *ydst = P.yface + ((long long)(it.vb % P.batch) * P.ntx + it.ti) * slot;
 
         // ---- TMA copies of levels 0 and 1 (the staging buffers are free: every thread passed the end-of-item
         //      barrier; the upwind items' face stores were made with the generic proxy) ----

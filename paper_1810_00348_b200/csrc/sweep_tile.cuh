@@ -57,11 +57,12 @@ struct TileItem {
     int pred_y;       // item index of (vb, ti, tj-1) or -1
     int pred_s;       // item index of the last reader of this item's x-face slot, (vb, ntx-1, tj-P), or -1
     int xslot;        // tj % P
-    int pad;
+    int fslot;        // face-slot set of the block: index within its batch
 };
 
 struct TilePlan {
     int ntx = 0, nty = 0, P = 1;
+    int batch = 0;                     // velocity blocks in flight at once (= face-slot sets)
     int nbb = 8, ncb = 4;              // one (xi_y, xi_z) block shape for the whole problem
     std::vector<int> xnode, ynode, znode;   // node index per 1-D block slot (-1 = padding): [nxb][16], [nyb][nbb], [nzb][ncb];
                                             // xnode is in table order: slot r*4 + ag holds node 4*ag + r of the block
@@ -72,6 +73,7 @@ struct TilePlan {
 
 struct TileParams {
     int nx, ny, nz, ntx, nty, P;
+    int batch;                    // velocity blocks per batch: block vb uses face-slot set vb % batch
     long long ncell;
     const double *invdx, *invdy, *invdz;
     const unsigned char *flags;   // [ncell] bits 0..5: neighbour in direction d is not a fluid cell; bit 6: solid
@@ -114,9 +116,10 @@ struct TableParams {
 };
 
 // Build velocity blocks, items and their order for a grid and a set of velocity nodes.  target_ctas = number of
-// items that should be able to run concurrently (sets the band height P).  Pure host code (tests call it through
+// items that should be able to run concurrently (sets the band height P); max_blocks > 0 caps the velocity blocks in
+// flight at once (batches).  Pure host code (tests call it through
 // dvm_plan_query without a GPU).
-int tile_plan(int nx, int ny, int nz, const std::vector<double> xi[3], int target_ctas, TilePlan *plan);
+int tile_plan(int nx, int ny, int nz, const std::vector<double> xi[3], int target_ctas, int max_blocks, TilePlan *plan);
 
 size_t tile_smem_bytes();
 cudaError_t tile_configure(int *ctas_per_sm);

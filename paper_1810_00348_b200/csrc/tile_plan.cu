@@ -27,7 +27,7 @@ int ceil_div(int a, int b) { return (a + b - 1) / b; }
 
 }  // namespace
 
-int tile_plan(int nx, int ny, int nz, const std::vector<double> xi[3], int target_ctas, TilePlan *plan)
+int tile_plan(int nx, int ny, int nz, const std::vector<double> xi[3], int target_ctas, int max_blocks, TilePlan *plan)
 {
     if (nx <= 0 || ny <= 0 || nz <= 0 || !plan) return -1;
     plan->vblocks.clear();
@@ -86,37 +86,50 @@ int tile_plan(int nx, int ny, int nz, const std::vector<double> xi[3], int targe
     if (nvb == 0) return -1;
     const int ntx = ceil_div(nx, TILE_TX), nty = ceil_div(ny, TILE_TY);
     plan->ntx = ntx; plan->nty = nty;
+    // velocity blocks in flight at once (smaller batches cap the memory of the stored f): the face
+    // workspace holds one slot set per block of a batch; batches sweep the grid one after the other
+    const int B = max_blocks > 0 ? std::min(max_blocks, nvb) : nvb;
+    plan->batch = B;
     // band height: enough independent tiles per diagonal to keep target_ctas items in flight
-    int P = ceil_div(std::max(target_ctas, 1) * 2, nvb);
+    int P = ceil_div(std::max(target_ctas, 1) * 2, B);
     P = std::max(1, std::min(P, nty));
     plan->P = P;
 
-    // ---- items in hand-out order ----
+    // ---- items in hand-out order: batch, band of P tile rows, diagonal, row, velocity block ----
     std::vector<int> index((size_t)nvb * ntx * nty, -1);
     auto at = [&](int vb, int ti, int tj) -> int & { return index[((size_t)vb * nty + tj) * ntx + ti]; };
-    for (int band = 0; band * P < nty; ++band) {
-        const int j0 = band * P, rows = std::min(P, nty - j0);
-        for (int d = 0; d < ntx + rows - 1; ++d)
-            for (int r = 0; r < rows; ++r) {
-                const int ti = d - r, tj = j0 + r;
-                if (ti < 0 || ti >= ntx) continue;
-                for (int vb = 0; vb < nvb; ++vb) {
-                    TileItem it{};
-                    it.vb = vb; it.ti = ti; it.tj = tj; it.xslot = tj % P;
-                    it.pred_x = it.pred_y = it.pred_s = -1;
-                    at(vb, ti, tj) = (int)plan->items.size();
-                    plan->items.push_back(it);
+    for (int v0 = 0; v0 < nvb; v0 += B)
+        for (int band = 0; band * P < nty; ++band) {
+            const int j0 = band * P, rows = std::min(P, nty - j0);
+            for (int d = 0; d < ntx + rows - 1; ++d)
+                for (int r = 0; r < rows; ++r) {
+                    const int ti = d - r, tj = j0 + r;
+                    if (ti < 0 || ti >= ntx) continue;
+                    for (int vb = v0; vb < std::min(nvb, v0 + B); ++vb) {
+                        TileItem it{};
+                        it.vb = vb; it.ti = ti; it.tj = tj; it.xslot = tj % P; it.fslot = vb - v0;
+                        it.pred_x = it.pred_y = it.pred_s = -1;
+                        at(vb, ti, tj) = (int)plan->items.size();
+                        plan->items.push_back(it);
+                    }
                 }
-            }
-    }
+        }
     for (auto &it : plan->items) {
         if (it.ti > 0) it.pred_x = at(it.vb, it.ti - 1, it.tj);
         if (it.tj > 0) it.pred_y = at(it.vb, it.ti, it.tj - 1);
         if (it.ti == 0 && it.tj >= P) it.pred_s = at(it.vb, ntx - 1, it.tj - P);
+        // face slots are shared with the block B places earlier (previous batch): wait for its last readers
+        if (it.vb >= B) {
+            if (it.tj == 0) it.pred_y = at(it.vb - B, it.ti, nty - 1);          // y-face slot (fslot, ti)
+            if (it.ti == 0 && it.tj < P) {                                      // x-face slot (fslot, tj % P)
+                const int last = it.tj + ((nty - 1 - it.tj) / P) * P;
+                it.pred_s = at(it.vb - B, ntx - 1, last);
+            }
+        }
     }
     const size_t slot = (size_t)nz * TILE_TY * TILE_NVB;
-    plan->xface_doubles = (size_t)nvb * P * slot;
-    plan->yface_doubles = (size_t)nvb * ntx * slot;
+    plan->xface_doubles = (size_t)B * P * slot;
+    plan->yface_doubles = (size_t)B * ntx * slot;
     return 0;
 }
 

@@ -24,6 +24,7 @@ OK, EINVAL, ENOMEM, ECUDA, ENONFINITE = 0, -1, -2, -3, -4
 WALL_DIFFUSE, FREESTREAM, ZERO_GRADIENT = 0, 1, 2
 KERNEL_AUTO, KERNEL_SLICE, KERNEL_TILE = 0, 1, 2
 OPT_KERNEL = 1
+OPT_MAX_F_MBYTES = 2
 
 # every symbol include/dvm.h declares (checked by tests/test_abi.py)
 SYMBOLS = (
@@ -118,7 +119,7 @@ def lib():
         L.dvm_set_option.argtypes = [vp, C.c_int, C.c_int]
         L.dvm_workspace_bytes.argtypes = [vp, C.POINTER(C.c_size_t), C.POINTER(C.c_size_t)]
         L.dvm_kernel_used.argtypes = [vp]
-        L.dvm_plan_query.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(_VGrid), C.c_int, C.POINTER(C.c_int),
+        L.dvm_plan_query.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(_VGrid), C.c_int, C.c_int, C.POINTER(C.c_int),
                                      C.POINTER(C.c_int), C.c_int]
         L.dvm_launch_count.argtypes = [vp]
         L.dvm_launch_count.restype = C.c_longlong
@@ -138,22 +139,23 @@ def _f64(a):
     return np.ascontiguousarray(a, dtype=np.float64)
 
 
-def plan_query(nx, ny, nz, xi_x, xi_y, xi_z, target_ctas=296, max_items=1 << 22):
-    """dvm_plan_query: (counts dict, items int32 [n][8]) of the tile kernel's work decomposition (host only)."""
+def plan_query(nx, ny, nz, xi_x, xi_y, xi_z, target_ctas=296, max_blocks=0, max_items=1 << 22):
+    """dvm_plan_query: (counts dict, items int32 [n][9]) of the tile kernel's work decomposition (host only)."""
     keep = [_f64(a) for a in (xi_x, xi_y, xi_z)]
     v = _VGrid(len(keep[0]), len(keep[1]), len(keep[2]), *(a.ctypes.data_as(_dp) for a in keep), None, None, None)
-    counts = (C.c_int * 4)()
-    n = _check(lib().dvm_plan_query(nx, ny, nz, C.byref(v), target_ctas, counts, None, 0))
-    items = np.zeros((min(n, max_items), 8), dtype=np.int32)
-    _check(lib().dvm_plan_query(nx, ny, nz, C.byref(v), target_ctas, counts, items.ctypes.data_as(C.POINTER(C.c_int)),
-                                len(items)))
-    return {"n_vblocks": counts[0], "ntx": counts[1], "nty": counts[2], "P": counts[3], "n_items": n}, items
+    counts = (C.c_int * 5)()
+    n = _check(lib().dvm_plan_query(nx, ny, nz, C.byref(v), target_ctas, max_blocks, counts, None, 0))
+    items = np.zeros((min(n, max_items), 9), dtype=np.int32)
+    _check(lib().dvm_plan_query(nx, ny, nz, C.byref(v), target_ctas, max_blocks, counts,
+                                items.ctypes.data_as(C.POINTER(C.c_int)), len(items)))
+    return {"n_vblocks": counts[0], "ntx": counts[1], "nty": counts[2], "P": counts[3], "batch": counts[4],
+            "n_items": n}, items
 
 
 class Solver:
     """dvm_create / dvm_iterate / dvm_moments / dvm_residual (+ support calls) for one workload record."""
 
-    def __init__(self, wl, kernel: int = KERNEL_AUTO, device: str = "cuda:0"):
+    def __init__(self, wl, kernel: int = KERNEL_AUTO, device: str = "cuda:0", max_f_mbytes: int = 0):
         import torch
         if not torch.cuda.is_available():
             raise DvmError(ECUDA, "no CUDA device: the DVM solver has no CPU fallback")
@@ -201,6 +203,8 @@ class Solver:
         self.nface = _check(L.dvm_num_faces(h))
         if kernel != KERNEL_AUTO:
             self.set_option(OPT_KERNEL, kernel)
+        if max_f_mbytes:
+            self.set_option(OPT_MAX_F_MBYTES, int(max_f_mbytes))
 
     # -- the four calls of the north star ---------------------------------------------------------
     def iterate(self, n: int = 1):

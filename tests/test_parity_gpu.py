@@ -172,6 +172,28 @@ def test_paper_cube_grid_small(oracle_mod, kernel):
     lockstep(wl, kernel, 3, oracle_mod)
 
 
+def test_workspace_cap_batches(oracle_mod):
+    """DVM_OPT_MAX_F_MBYTES (smaller velocity batches cap the memory of the stored f): config 1 with the f
+    workspace capped well below the uncapped size sweeps its 27 velocity blocks in batches; same results."""
+    from paper_1810_00348_b200 import dvm
+    wl = W.config(1)
+    s0 = dvm.Solver(wl, kernel=2)
+    s0.iterate(1)
+    _, f_full = s0.workspace_bytes()
+    s0.close()
+    cap_mb = max(1, int(f_full / 4 / 2**20))
+    o = oracle_mod.Oracle(wl)
+    s = dvm.Solver(wl, kernel=2, max_f_mbytes=cap_mb)
+    for it in range(3):
+        s.iterate(1)
+        c14 = o.step()
+        assert_fields(s.moments().cpu().numpy(), c14, what=f"capped workspace, iteration {it + 1}")
+        assert_residual(s.residual(), o.resid)
+    _, f_cap = s.workspace_bytes()
+    assert f_cap <= cap_mb * 2**20 and f_cap < f_full / 3
+    s.close()
+
+
 def test_P10_paper_iteration_count_soft_pin():
     """Soft pin P10: the paper's cavity run (Kn = 1, 64^3 x 64^3, U_w = 0.1 v_m, velocity range
     [-4, 4]^3, trapezoid rule) reaches its 1e-9 criterion in 36 iterations on a K40.  The criterion's exact form is our

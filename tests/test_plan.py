@@ -6,22 +6,28 @@ import pytest
 from paper_1810_00348_b200 import dvm, workloads as W
 
 
-def plan(wl, target=296):
-    return dvm.plan_query(wl.nx, wl.ny, wl.nz, wl.xi_x, wl.xi_y, wl.xi_z, target_ctas=target)
+def plan(wl, target=296, max_blocks=0):
+    return dvm.plan_query(wl.nx, wl.ny, wl.nz, wl.xi_x, wl.xi_y, wl.xi_z, target_ctas=target, max_blocks=max_blocks)
 
 
-@pytest.mark.parametrize("wl,target", [
-    (W.config(0), 296), (W.config(1), 296), (W.config(2), 296), (W.config(3), 296),
-    (W.cavity(0, 0, 0.1, nxyz=(13, 9, 11), mxyz=(10, 7, 9)), 296),
-    (W.cavity(0, 0, 0.1, nxyz=(13, 9, 11), mxyz=(10, 7, 9)), 4),
-    (W.cube_flow(4, 12, box=(6, 4, 4), vrange=8.0), 37),
+@pytest.mark.parametrize("wl,target,max_blocks", [
+    (W.config(0), 296, 0), (W.config(1), 296, 0), (W.config(2), 296, 0), (W.config(3), 296, 0),
+    (W.cavity(0, 0, 0.1, nxyz=(13, 9, 11), mxyz=(10, 7, 9)), 296, 0),
+    (W.cavity(0, 0, 0.1, nxyz=(13, 9, 11), mxyz=(10, 7, 9)), 4, 0),
+    (W.cube_flow(4, 12, box=(6, 4, 4), vrange=8.0), 37, 0),
+    (W.config(1), 296, 5), (W.config(2), 296, 24), (W.config(0), 296, 1),
+    (W.cavity(0, 0, 0.1, nxyz=(13, 9, 11), mxyz=(10, 7, 9)), 16, 3),
 ])
-def test_items_cover_everything_once_in_dependency_order(wl, target):
-    counts, items = plan(wl, target)
+def test_items_cover_everything_once_in_dependency_order(wl, target, max_blocks):
+    counts, items = plan(wl, target, max_blocks)
     n = counts["n_items"]
     assert len(items) == n == counts["n_vblocks"] * counts["ntx"] * counts["nty"]
     assert counts["ntx"] == -(-wl.nx // 4) and counts["nty"] == -(-wl.ny // 4)
-    vb, ti, tj, px, py, ps, xslot, octant = items.T
+    vb, ti, tj, px, py, ps, xslot, octant, fslot = items.T
+    B = counts["batch"]
+    assert B == (min(max_blocks, counts["n_vblocks"]) if max_blocks else counts["n_vblocks"])
+    assert np.array_equal(fslot, vb % B)
+    later = vb >= B   # items of a later batch share their face slots with the block B places earlier
     # every (velocity block, tile) exactly once
     key = (vb.astype(np.int64) * counts["nty"] + tj) * counts["ntx"] + ti
     assert len(np.unique(key)) == n
@@ -33,15 +39,27 @@ def test_items_cover_everything_once_in_dependency_order(wl, target):
     has = px >= 0
     assert np.array_equal(ti > 0, has)
     assert np.all(vb[px[has]] == vb[has]) and np.all(ti[px[has]] == ti[has] - 1) and np.all(tj[px[has]] == tj[has])
-    has = py >= 0
+    has = (py >= 0) & (tj > 0)
     assert np.array_equal(tj > 0, has)
     assert np.all(vb[py[has]] == vb[has]) and np.all(tj[py[has]] == tj[has] - 1) and np.all(ti[py[has]] == ti[has])
+    # first tile row of a later batch: waits for the last reader of its y-face slot in the previous batch
+    first = (tj == 0)
+    assert np.array_equal(py[first] >= 0, later[first])
+    sel = first & later
+    assert np.all(vb[py[sel]] == vb[sel] - B) and np.all(ti[py[sel]] == ti[sel]) and np.all(tj[py[sel]] == counts["nty"] - 1)
     # x-face slot reuse: the item that overwrites slot tj % P waits for the last reader of the previous user
     P = counts["P"]
     assert np.array_equal(xslot, tj % P)
-    has = ps >= 0
+    has = (ps >= 0) & (tj >= P)
     assert np.array_equal(has, (ti == 0) & (tj >= P))
     assert np.all(vb[ps[has]] == vb[has]) and np.all(ti[ps[has]] == counts["ntx"] - 1) and np.all(tj[ps[has]] == tj[has] - P)
+    sel = (ti == 0) & (tj < P)
+    assert np.array_equal(ps[sel] >= 0, later[sel])
+    sel = sel & later
+    assert np.all(vb[ps[sel]] == vb[sel] - B) and np.all(ti[ps[sel]] == counts["ntx"] - 1)
+    assert np.all(tj[ps[sel]] % P == tj[sel] % P) and np.all(tj[ps[sel]] + P >= counts["nty"])
+    # batches are handed out one after the other
+    assert np.all(np.diff(vb // B) >= 0)
 
 
 def test_velocity_blocks_partition_the_velocity_grid():
