@@ -10,14 +10,17 @@
 //    threads owns an item, a thread owns 4 velocities (consecutive xi_x nodes) and keeps the 4 x 4 x 4 values of
 //    the current z-plane in registers: x-, y- and z-upwind operands of interior cells are register operands;
 //  * what is carried is g = w_alpha f_alpha (the recurrence is linear in f), so quadrature weights cost nothing;
-//  * exp(-|xi-U|^2/T) factorises per axis on the tensor velocity grid: per cell and level the CTA builds tables of
-//    16 + nbb + ncb one-dimensional factors in shared memory (one exp per entry, not per phase point);
+//  * exp(-|xi-U|^2/T) and the Shakhov polynomial factorise per axis on the tensor velocity grid: tables.cu tabulates
+//    one entry (E, Q, e, a) per (cell, 1-D node) once per iteration; per level the CTA receives the 16 + nbb + ncb
+//    entries of its 16 cells as TMA row copies, together with the cell records (1/tau, cell index, faces);
 //  * the division of Eq.(7) is MUFU.RCP64H + one cubic Newton step (3 DFMA, < 1 ulp);
 //  * the 13 velocity sums use the tensor structure: 4 power sums over the thread's xi_x nodes (4 DFMA / point),
 //    a lane-quad exchange over the 16 xi_x nodes of the block, then each lane expands its share of the 16
 //    (power of xi_x) x (monomial of xi_y, xi_z) products and a transposing butterfly over the 8 lane groups leaves
 //    one partial per lane, which goes to the [cell][16] accumulator in L2/HBM as one coalesced fp64 RED per
-//    (cell, warp);
+//    (2 cells, warp);
+//  * the 4 rows of a level are a loop with rotating register slots: the level loop must fit the 32 KB instruction
+//    cache (profiles/r01_ifetch_microbench.txt), the fully unrolled level did not;
 //  * the x- and y-faces of the column are the only f-traffic: written with coalesced 32-byte stores per thread,
 //    read back by the downwind item with TMA bulk copies (cp.async.bulk + mbarrier) two levels ahead;
 //  * items are handed out by an atomic counter in dependency order (tile_plan.cu); done-flags gate their start.

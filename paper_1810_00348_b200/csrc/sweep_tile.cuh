@@ -9,6 +9,8 @@
 // (8 B per phase point instead of the 16 B of an in-place slice, 32 B in the paper's two-slice form,
 // PAPER.md:104-106, 233-235).  Items are handed out by an atomic counter in an order that respects the upwind
 // dependencies (x-face of (I'-1, J'), y-face of (I', J'-1)); done-flags in global memory gate the start of an item.
+// The equilibrium enters through 1-D factor tables (tables.cu) staged by TMA with the faces; velocity blocks may
+// sweep in batches that share face-slot sets when the f workspace is capped (DVM_OPT_MAX_F_MBYTES).
 #pragma once
 #include <cuda_runtime.h>
 #include <vector>
