@@ -203,7 +203,8 @@ TileParams tile_params(dvm_solver *s)
     P.vblocks = s->d_vblocks; P.items = s->d_items; P.nitems = (int)s->tile.items.size();
     P.done = s->d_done; P.counter = s->d_counter; P.epoch = s->epoch;
     P.xface = s->d_xface; P.yface = s->d_yface;
-    P.slot_doubles = (long long)s->nz * TILE_TY * TILE_NVB;
+    P.xslot_doubles = (long long)s->nz * TILE_TY * TILE_NVB;
+    P.yslot_doubles = (long long)s->nz * TILE_TX * TILE_NVB;
     P.TX = s->d_TX; P.TY = s->d_TY; P.TZ = s->d_TZ; P.rec = s->d_rec;
     P.nxp = s->nxp; P.nyp = s->nyp; P.nbb = s->tile.nbb; P.ncb = s->tile.ncb;
     return P;
@@ -276,12 +277,12 @@ int plan(dvm_solver *s)
         if (s->max_f_mbytes > 0) {
             // cap on the f workspace: fewer velocity blocks in flight (batches); the band height P
             // grows as the batch shrinks, so iterate to a fixed point; one block is the floor
-            const double cap = (double)s->max_f_mbytes * 1048576.0, slot_bytes = (double)s->nz * TILE_TY * TILE_NVB * 8.0;
+            const double cap = (double)s->max_f_mbytes * 1048576.0, lvl = (double)s->nz * TILE_NVB * 8.0;
             int B = (int)s->tile.vblocks.size();
             for (int pass = 0; pass < 8; ++pass) {
                 const double need = (double)(s->tile.xface_doubles + s->tile.yface_doubles) * 8.0;
                 if (need <= cap || B == 1) break;
-                B = std::max(1, std::min(B - 1, (int)(cap / ((s->tile.P + s->tile.ntx) * slot_bytes))));
+                B = std::max(1, std::min(B - 1, (int)(cap / ((s->tile.P * TILE_TY + s->tile.ntx * TILE_TX) * lvl))));
                 if (tile_plan(s->nx, s->ny, s->nz, s->xi, resident, B, &s->tile)) return fail(DVM_EINVAL, "tile plan failed");
             }
         }

@@ -38,8 +38,9 @@ namespace {
 constexpr int NVB = TILE_NVB;
 constexpr int NCELL = TILE_NCELL;
 constexpr int RB = 4;                                  // cells of a row whose moment reductions are interleaved
-constexpr int LEVEL_DOUBLES = 4 * NVB;                 // one level of an x- or y-face slot
-constexpr unsigned LEVEL_BYTES = LEVEL_DOUBLES * 8u;   // 16 KB
+constexpr int XLEVEL_DOUBLES = TILE_TY * NVB;          // one level of an x-face slot
+constexpr int YLEVEL_DOUBLES = TILE_TX * NVB;          // one level of a y-face slot
+constexpr unsigned XLEVEL_BYTES = XLEVEL_DOUBLES * 8u, YLEVEL_BYTES = YLEVEL_DOUBLES * 8u;
 
 constexpr unsigned XROW_BYTES = 4 * TILE_NA * 32u;      // one 4-cell row of x entries
 constexpr unsigned REC_ROW_BYTES = 4 * (unsigned)sizeof(CellRec);
@@ -176,7 +177,7 @@ __device__ __forceinline__ double rwb_load(const TileParams &P, const ItemCtx &I
     double v = 0.0;
     if (kp >= P.nz) return v;
     int i, j, k;
-    if (tid >= 32 && tid < 36) {
+    if (tid >= 32 && tid < 32 + TILE_TY) {
         if (I.first_x && cell_of(P, I, 0, tid - 32, kp, i, j, k)) v = face_density(P, I.tpx, P.foff[I.upx] + k * P.ny + j);
     } else if (tid >= 36 && tid < 40) {
         if (I.first_y && cell_of(P, I, tid - 36, 0, kp, i, j, k)) v = face_density(P, I.tpy, P.foff[I.upy] + k * P.nx + i);
@@ -196,15 +197,15 @@ __device__ __forceinline__ void issue_level(const TileParams &P, const ItemCtx &
                                             int tid, const double *xsrc, const double *ysrc)
 {
     const int b = kp & 1, q = tid - 64;
-    if (q < 0 || q >= 16) return;
+    if (q < 0 || q >= 4 * TILE_TY) return;
     const unsigned ybytes = 4u * vb.nbb * 32u, zbytes = 4u * vb.ncb * 32u;
     if (q == 0) {
-        const unsigned faces = (I.first_x ? 0u : LEVEL_BYTES) + (I.first_y ? 0u : LEVEL_BYTES);
-        mbar_expect_tx(&s.mbar[b], faces + 4u * (XROW_BYTES + ybytes + zbytes + REC_ROW_BYTES));
-        if (!I.first_x) tma_load(&s.xface[b][0][0], xsrc + (long long)kp * LEVEL_DOUBLES, LEVEL_BYTES, &s.mbar[b]);
-        if (!I.first_y) tma_load(&s.yface[b][0][0], ysrc + (long long)kp * LEVEL_DOUBLES, LEVEL_BYTES, &s.mbar[b]);
+        const unsigned faces = (I.first_x ? 0u : XLEVEL_BYTES) + (I.first_y ? 0u : YLEVEL_BYTES);
+        mbar_expect_tx(&s.mbar[b], faces + (unsigned)TILE_TY * (XROW_BYTES + ybytes + zbytes + REC_ROW_BYTES));
+        if (!I.first_x) tma_load(&s.xface[b][0][0], xsrc + (long long)kp * XLEVEL_DOUBLES, XLEVEL_BYTES, &s.mbar[b]);
+        if (!I.first_y) tma_load(&s.yface[b][0][0], ysrc + (long long)kp * YLEVEL_DOUBLES, YLEVEL_BYTES, &s.mbar[b]);
     }
-    const int jj = q & 3, kind = q >> 2;
+    const int jj = q % TILE_TY, kind = q / TILE_TY;
     // first cell (lowest absolute x) of row jj on the padded grid; rows may lie in the dead padding
     const int jp = I.j0 + jj, ip0 = I.i0;
     const int j = I.sy > 0 ? jp : P.ny - 1 - jp;
@@ -224,7 +225,7 @@ __device__ __forceinline__ int decode_records(const TileParams &P, const ItemCtx
 {
     const int b = kp & 1;
     int special = 0;
-    if (tid >= 96 && tid < 112) {
+    if (tid >= 96 && tid < 96 + NCELL) {
         const int cell = tid - 96, ii = cell & 3, jj = cell >> 2;
         const CellRec &r = s.rec[b][jj * 4 + (I.sx > 0 ? ii : 3 - ii)];
         const bool dead = r.cidx < 0;
@@ -261,7 +262,7 @@ __device__ __forceinline__ void fill_faces(const ItemCtx &I, TileSmem &s, int b,
         for (int r = 0; r < 4; ++r) {
             const double G = s.g[0][0][4 * ag + r] * gyz;
 #pragma unroll
-            for (int jj = 0; jj < 4; ++jj) s.xface[b][jj][tid * 4 + r] = s.rwb[b][jj] * G;
+            for (int jj = 0; jj < TILE_TY; ++jj) s.xface[b][jj][tid * 4 + r] = s.rwb[b][jj] * G;
         }
     }
     if (I.first_y) {
@@ -361,7 +362,7 @@ __device__ __forceinline__ void emit_pair(const TileParams &P, TileSmem &s, cons
 // One level of the column, fast path (no solid ghost in the level): 4 rows x 4 cells x 4 velocities per thread,
 // fully unrolled so that the plane lives in registers.  Dead cells (outside the domain / solid) have all-zero table
 // entries and nu = 1, so they produce g = 0 by the same arithmetic.
-__device__ __forceinline__ void compute_level(const TileParams &P, TileSmem &s, const int b, double (&pl)[4][4][4],
+__device__ __forceinline__ void compute_level(const TileParams &P, TileSmem &s, const int b, double (&pl)[TILE_TY][4][4],
                                               const ThreadCtx &T, const int tid, const int lane, double *xout,
                                               double *yout)
 {
@@ -378,7 +379,7 @@ __device__ __forceinline__ void compute_level(const TileParams &P, TileSmem &s, 
         yu[ii][0] = v0.x; yu[ii][1] = v0.y; yu[ii][2] = v1.x; yu[ii][3] = v1.y;
     }
 #pragma unroll 1
-    for (int jj = 0; jj < 4; ++jj) {
+    for (int jj = 0; jj < TILE_TY; ++jj) {
         double fx[4];
         {
             const double2 *p = reinterpret_cast<const double2 *>(&s.xface[b][jj][tid * 4]);
@@ -432,15 +433,17 @@ __device__ __forceinline__ void compute_level(const TileParams &P, TileSmem &s, 
 #pragma unroll
             for (int r = 0; r < 4; ++r) {
                 const double t = pl[0][ii][r];
-                pl[0][ii][r] = pl[1][ii][r]; pl[1][ii][r] = pl[2][ii][r]; pl[2][ii][r] = pl[3][ii][r]; pl[3][ii][r] = t;
+#pragma unroll
+                for (int q = 0; q + 1 < TILE_TY; ++q) pl[q][ii][r] = pl[q + 1][ii][r];
+                pl[TILE_TY - 1][ii][r] = t;
             }
     }
     if (yout) {
 #pragma unroll
         for (int ii = 0; ii < 4; ++ii) {
             double2 *p = reinterpret_cast<double2 *>(yout + ii * NVB + tid * 4);
-            p[0] = make_double2(pl[3][ii][0], pl[3][ii][1]);
-            p[1] = make_double2(pl[3][ii][2], pl[3][ii][3]);
+            p[0] = make_double2(pl[TILE_TY - 1][ii][0], pl[TILE_TY - 1][ii][1]);
+            p[1] = make_double2(pl[TILE_TY - 1][ii][2], pl[TILE_TY - 1][ii][3]);
         }
     }
 }
@@ -454,7 +457,7 @@ __device__ __forceinline__ void compute_level_slow(const TileParams &P, TileSmem
 {
     const double gyz = s.g[3][1][T.yi] * s.g[3][2][T.zi];
 #pragma unroll 1
-    for (int jj = 0; jj < 4; ++jj) {
+    for (int jj = 0; jj < TILE_TY; ++jj) {
         double fx[4];
 #pragma unroll
         for (int r = 0; r < 4; ++r) fx[r] = s.xface[b][jj][tid * 4 + r];
@@ -507,11 +510,11 @@ __device__ __forceinline__ void compute_level_slow(const TileParams &P, TileSmem
 #pragma unroll 1
         for (int ii = 0; ii < 4; ++ii)
 #pragma unroll
-            for (int r = 0; r < 4; ++r) yout[ii * NVB + tid * 4 + r] = pl[(12 + ii) * 4 + r];
+            for (int r = 0; r < 4; ++r) yout[ii * NVB + tid * 4 + r] = pl[((TILE_TY - 1) * 4 + ii) * 4 + r];
     }
 }
 
-__global__ void __launch_bounds__(TILE_THREADS, 2) sweep_tile_kernel(const TileParams P)
+__global__ void __launch_bounds__(TILE_THREADS, TILE_MIN_CTAS) sweep_tile_kernel(const TileParams P)
 {
     // dynamic shared memory starts at offset 0 of the CTA's window (no static __shared__ in this kernel), so the
     // 128-byte alignment holds; casting without pointer arithmetic keeps the address space visible (LDS / STS)
@@ -526,7 +529,6 @@ __global__ void __launch_bounds__(TILE_THREADS, 2) sweep_tile_kernel(const TileP
     }
     __syncthreads();
     unsigned par[2] = {0u, 0u};
-    const long long slot = P.slot_doubles;
 
     for (;;) {
         // ---- next item (dependency order), wait for its upwind items ----
@@ -555,12 +557,12 @@ __global__ void __launch_bounds__(TILE_THREADS, 2) sweep_tile_kernel(const TileP
         I.tpx = P.bc_type[I.upx]; I.tpy = P.bc_type[I.upy]; I.tpz = P.bc_type[I.upz];
         I.first_x = it.ti == 0; I.first_y = it.tj == 0;
         I.nbb = vb.nbb; I.ncb = vb.ncb;
-        double *xdst = P.xface + ((long long)(it.vb % P.batch) * P.P + it.xslot) * slot;
-        double *ydst = P.yface + ((long long)(it.vb % P.batch) * P.ntx + it.ti) * slot;
+        double *xdst = P.xface + ((long long)(it.vb % P.batch) * P.P + it.xslot) * P.xslot_doubles;
+        double *ydst = P.yface + ((long long)(it.vb % P.batch) * P.ntx + it.ti) * P.yslot_doubles;
 
         // ---- TMA copies of levels 0 and 1 (the staging buffers are free: every thread passed the end-of-item
         //      barrier; the upwind items' face stores were made with the generic proxy) ----
-        if (tid >= 64 && tid < 80) {
+        if (tid >= 64 && tid < 64 + 4 * TILE_TY) {
             fence_proxy_async_global();
             issue_level(P, I, s, vb, 0, tid, xdst, ydst);
             if (P.nz > 1) issue_level(P, I, s, vb, 1, tid, xdst, ydst);
@@ -624,20 +626,20 @@ __global__ void __launch_bounds__(TILE_THREADS, 2) sweep_tile_kernel(const TileP
 
         // records and boundary faces of level 0 (its copies were issued above; the wait does not consume the phase)
         int special = 0;
-        if (tid >= 96 && tid < 112) {
+        if (tid >= 96 && tid < 96 + NCELL) {
             mbar_wait(&s.mbar[0], par[0]);
             special = decode_records(P, I, s, 0, tid);
         }
         fill_faces(I, s, 0, tid, T.ag, T.yi, T.zi);
         // plane = ghost of the upwind z face of the domain
-        double pl[4][4][4];
+        double pl[TILE_TY][4][4];
         {
             const double gyz = s.g[2][1][T.yi] * s.g[2][2][T.zi];
             double G[4];
 #pragma unroll
             for (int r = 0; r < 4; ++r) G[r] = s.g[2][0][4 * T.ag + r] * gyz;
 #pragma unroll
-            for (int jj = 0; jj < 4; ++jj)
+            for (int jj = 0; jj < TILE_TY; ++jj)
 #pragma unroll
                 for (int ii = 0; ii < 4; ++ii) {
                     int i, j, k;
@@ -656,17 +658,17 @@ __global__ void __launch_bounds__(TILE_THREADS, 2) sweep_tile_kernel(const TileP
             const double vrw = rwb_load(P, I, kp + 2, tid);
             mbar_wait(&s.mbar[b], par[b]);
             par[b] ^= 1u;
-            double *xout = write_x ? xdst + (long long)kp * LEVEL_DOUBLES : nullptr;
-            double *yout = write_y ? ydst + (long long)kp * LEVEL_DOUBLES : nullptr;
+            double *xout = write_x ? xdst + (long long)kp * XLEVEL_DOUBLES : nullptr;
+            double *yout = write_y ? ydst + (long long)kp * YLEVEL_DOUBLES : nullptr;
             if (special) {
-                double tmp[64];
+                double tmp[NCELL * 4];
 #pragma unroll
-                for (int c = 0; c < 16; ++c)
+                for (int c = 0; c < NCELL; ++c)
 #pragma unroll
                     for (int r = 0; r < 4; ++r) tmp[c * 4 + r] = pl[c >> 2][c & 3][r];
                 compute_level_slow(P, s, b, tmp, T, tid, lane, xout, yout);
 #pragma unroll
-                for (int c = 0; c < 16; ++c)
+                for (int c = 0; c < NCELL; ++c)
 #pragma unroll
                     for (int r = 0; r < 4; ++r) pl[c >> 2][c & 3][r] = tmp[c * 4 + r];
             } else {
@@ -675,14 +677,14 @@ __global__ void __launch_bounds__(TILE_THREADS, 2) sweep_tile_kernel(const TileP
             rwb_store(s, b, tid, vrw);
             int sp = 0;
             if (kp + 1 < P.nz) {
-                if (tid >= 96 && tid < 112) {
+                if (tid >= 96 && tid < 96 + NCELL) {
                     mbar_wait(&s.mbar[b ^ 1], par[b ^ 1]);   // level kp + 1 has landed (issued a level ago)
                     sp = decode_records(P, I, s, kp + 1, tid);
                 }
                 fill_faces(I, s, b ^ 1, tid, T.ag, T.yi, T.zi);
             }
             special = __shfl_sync(0xffffffffu, __syncthreads_or(sp), 0);
-            if (tid >= 64 && tid < 80 && kp + 2 < P.nz) {
+            if (tid >= 64 && tid < 64 + 4 * TILE_TY && kp + 2 < P.nz) {
                 fence_proxy_async_smem();  // this level's reads of the staging buffers before the TMA overwrites them
                 issue_level(P, I, s, vb, kp + 2, tid, xdst, ydst);
             }

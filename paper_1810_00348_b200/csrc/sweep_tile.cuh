@@ -19,7 +19,11 @@
 namespace dvm {
 
 constexpr int TILE_TX = 4;                 // cells per tile along the sweep-relative x
-constexpr int TILE_TY = 4;                 // cells per tile along the sweep-relative y
+#ifndef DVM_TILE_TY
+#define DVM_TILE_TY 4
+#endif
+constexpr int TILE_TY = DVM_TILE_TY;        // cells per tile along the sweep-relative y (4, or 2: 3 CTAs per SM)
+constexpr int TILE_MIN_CTAS = TILE_TY <= 2 ? 3 : 2;   // resident CTAs per SM the kernel is compiled for
 constexpr int TILE_NCELL = TILE_TX * TILE_TY;
 constexpr int TILE_RV = 4;                 // velocities per thread (consecutive xi_x nodes)
 constexpr int TILE_GA = 4;                 // xi_x groups per lane quad
@@ -97,7 +101,7 @@ struct TileParams {
     int *counter;                 // next item
     int epoch;
     double *xface, *yface;
-    long long slot_doubles;       // nz * 4 * TILE_NVB
+    long long xslot_doubles, yslot_doubles;   // nz * TILE_TY * TILE_NVB, nz * TILE_TX * TILE_NVB
     // factor tables of step n (tables_kernel), padded grid nxp x nyp x nz, entries double4 (E, Q, e, a):
     const double4 *TX, *TY, *TZ;  // [nxb][nz][nyp][nxp][16], [nyb][nz][nyp][nxp][nbb], [nzb][nz][nyp][nxp][ncb]
     const CellRec *rec;           // [nz][nyp][nxp]

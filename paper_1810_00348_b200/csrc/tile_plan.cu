@@ -127,9 +127,8 @@ int tile_plan(int nx, int ny, int nz, const std::vector<double> xi[3], int targe
             }
         }
     }
-    const size_t slot = (size_t)nz * TILE_TY * TILE_NVB;
-    plan->xface_doubles = (size_t)B * P * slot;
-    plan->yface_doubles = (size_t)B * ntx * slot;
+    plan->xface_doubles = (size_t)B * P * nz * TILE_TY * TILE_NVB;
+    plan->yface_doubles = (size_t)B * ntx * nz * TILE_TX * TILE_NVB;
     return 0;
 }
 
