@@ -277,34 +277,14 @@ __device__ __forceinline__ void fill_faces(const ItemCtx &I, TileSmem &s, int b,
 }
 
 // Reduction of the four power sums S_p = sum_r xi_x^p g_r of a lane over the 4 x-groups of a lane quad and the
-// (xi_y, xi_z) pairs with lane bits 2 and 3 (see the header comment).  Returns, in every lane, the partial sum over
-// its half-warp of one of the 16 products of the cell; lane & 15 names it (c_mom).
-__device__ __forceinline__ double reduce_half(double S0, double S1, double S2, double S3, const double (&cf)[4], int lane)
-{
-    const bool b0 = lane & 1, b1 = lane & 2, b2 = lane & 4, b3 = lane & 8;
-    // lane quad = the 4 xi_x groups of one (xi_y, xi_z) pair
-    S0 += shx(S0, 1);
-    S0 += shx(S0, 2);
-    double u = (b1 ? S2 : S1) + shx(b1 ? S1 : S2, 2);
-    double v = S3 + shx(b1 ? 0.0 : S3, 2);
-    u += shx(u, 1);
-    v += shx(v, 1);
-    // lanes 0, 2 expand S0, lane 1 expands S1, lane 3 expands S2 (3 outputs) and S3 (1 output)
-    const double U = b0 ? u : S0;
-    const double V = (b0 && b1) ? v : U;
-    const double o0 = cf[0] * U, o1 = cf[1] * U, o2 = cf[2] * U, o3 = cf[3] * V;
-    // transposing butterfly over the (xi_y, xi_z) pairs of the half-warp
-    const double k0 = (b2 ? o2 : o0) + shx(b2 ? o0 : o2, 4);
-    const double k1 = (b2 ? o3 : o1) + shx(b2 ? o1 : o3, 4);
-    return (b3 ? k1 : k0) + shx(b3 ? k0 : k1, 8);
-}
-
-// The same reduction for N cells at once, stage by stage, so that the shuffle latency of one cell is covered by the
-// other cells' instructions.  S[c][p] = power sum p of cell c; k[c] = result of cell c.
+// (xi_y, xi_z) pairs with lane bits 2 and 3 (see the header comment), for N cells at once, stage by stage, so that
+// the shuffle latency of one cell is covered by the other cells' instructions.  Leaves, in every lane, the partial
+// sum over its half-warp of one of the 16 products of the cell; lane & 15 names it (c_mom).  S[c][p] = power sum p of cell c; k[c] = result of cell c.
 template <int N>
-__device__ __forceinline__ void reduce_halfN(const double (&S)[N][4], const double (&cf)[4], int lane, double (&k)[N])
+__device__ __forceinline__ void reduce_halfN(const double (&S)[N][4], const double (&cf)[4], const int vsel, int lane,
+                                             double (&k)[N])
 {
-    const bool b0 = lane & 1, b1 = lane & 2, b2 = lane & 4, b3 = lane & 8;
+    const bool b0 = lane & 1, b1 = lane & 2;
     double a0[N], u[N], v[N];
 #pragma unroll
     for (int c = 0; c < N; ++c) a0[c] = S[c][0] + shx(S[c][0], 1);
@@ -318,23 +298,28 @@ __device__ __forceinline__ void reduce_halfN(const double (&S)[N][4], const doub
     for (int c = 0; c < N; ++c) u[c] += shx(u[c], 1);
 #pragma unroll
     for (int c = 0; c < N; ++c) v[c] += shx(v[c], 1);
-    double k0[N], k1[N];
+    // Pair stage without selects between the shuffles: the lane with pair bits m = 2 b2 + b3 keeps its four products in
+    // the order r_k = o_(k xor m) (cf is stored permuted), so that both exchange steps send fixed registers; only the
+    // operand of the S3 product (lane role 3, product 3, register 3 xor m: bit k of vsel) is chosen per register.
+    const bool s0 = vsel & 1, s1 = vsel & 2, s2 = vsel & 4, s3 = vsel & 8;
+    double r0[N], r1[N];
 #pragma unroll
     for (int c = 0; c < N; ++c) {
         const double U = b0 ? u[c] : a0[c];
-        const double V = (b0 && b1) ? v[c] : U;
-        const double o0 = cf[0] * U, o1 = cf[1] * U, o2 = cf[2] * U, o3 = cf[3] * V;
-        k0[c] = (b2 ? o2 : o0) + shx(b2 ? o0 : o2, 4);
-        k1[c] = (b2 ? o3 : o1) + shx(b2 ? o1 : o3, 4);
+        const double p0 = cf[0] * (s0 ? v[c] : U), p1 = cf[1] * (s1 ? v[c] : U);
+        const double p2 = cf[2] * (s2 ? v[c] : U), p3 = cf[3] * (s3 ? v[c] : U);
+        r0[c] = p0 + shx(p2, 4);
+        r1[c] = p1 + shx(p3, 4);
     }
 #pragma unroll
-    for (int c = 0; c < N; ++c) k[c] = (b3 ? k1[c] : k0[c]) + shx(b3 ? k0[c] : k1[c], 8);
+    for (int c = 0; c < N; ++c) k[c] = r0[c] + shx(r1[c], 8);
 }
 
 // per-thread constants of an item
 struct ThreadCtx {
     double X1[4], X2[4], X3[4];  // xi_x, xi_x^2, xi_x^3 of the thread's nodes
-    double cf[4];                // expansion coefficients of this lane
+    double cf[4];                // expansion coefficients of this lane, in the order cf[k] = c[k xor m] (reduce_halfN)
+    int vsel;                    // bit k: product k of this lane takes the S3 sum
     double dsgn;                 // sign of the wall-flux contribution of this lane
     double *rawm;                // raw16 + moment slot of this lane
     int ag, yi, zi;              // xi_x group, rows of the thread's xi_y and xi_z nodes in xi_bc / g
@@ -417,7 +402,7 @@ __device__ __forceinline__ void compute_level(const TileParams &P, TileSmem &s, 
             SR[ii % RB][0] = S0; SR[ii % RB][1] = S1; SR[ii % RB][2] = S2; SR[ii % RB][3] = S3;
             if (ii % RB == RB - 1) {
                 double k[RB];
-                reduce_halfN<RB>(SR, T.cf, lane, k);
+                reduce_halfN<RB>(SR, T.cf, T.vsel, lane, k);
 #pragma unroll
                 for (int c = 0; c < RB; c += 2) emit_pair(P, s, b, cell - (RB - 1) + c, k[c], k[c + 1], T, lane);
             }
@@ -497,7 +482,10 @@ __device__ __forceinline__ void compute_level_slow(const TileParams &P, TileSmem
                 S2 = fma(T.X2[r], gg, S2);
                 S3 = fma(T.X3[r], gg, S3);
             }
-            const double kk = reduce_half(S0, S1, S2, S3, T.cf, lane);
+            const double S1c[1][4] = {{S0, S1, S2, S3}};
+            double k1[1];
+            reduce_halfN<1>(S1c, T.cf, T.vsel, lane, k1);
+            const double kk = k1[0];
             if (ii & 1) emit_pair(P, s, b, cell - 1, kprev, kk, T, lane);
             else kprev = kk;
         }
@@ -608,10 +596,16 @@ __global__ void __launch_bounds__(TILE_THREADS, TILE_MIN_CTAS) sweep_tile_kernel
             T.zi = vb.nbb + T.zl;
             const double xb = s.xi_bc[T.yi], xc = s.xi_bc[T.zi], r2 = xb * xb + xc * xc;
             const int q = lane & 3, j = ((lane >> 2) & 1) * 2 + ((lane >> 3) & 1);
-            if (q == 0) { T.cf[0] = 1.0; T.cf[1] = xb; T.cf[2] = xc; T.cf[3] = xb * xb; }
-            else if (q == 1) { T.cf[0] = 1.0; T.cf[1] = xb; T.cf[2] = xc; T.cf[3] = r2; }
-            else if (q == 2) { T.cf[0] = xc * xc; T.cf[1] = xb * xc; T.cf[2] = xb * r2; T.cf[3] = xc * r2; }
-            else { T.cf[0] = 1.0; T.cf[1] = xb; T.cf[2] = xc; T.cf[3] = 1.0; }
+            double cq[4];
+            if (q == 0) { cq[0] = 1.0; cq[1] = xb; cq[2] = xc; cq[3] = xb * xb; }
+            else if (q == 1) { cq[0] = 1.0; cq[1] = xb; cq[2] = xc; cq[3] = r2; }
+            else if (q == 2) { cq[0] = xc * xc; cq[1] = xb * xc; cq[2] = xb * r2; cq[3] = xc * r2; }
+            else { cq[0] = 1.0; cq[1] = xb; cq[2] = xc; cq[3] = 1.0; }
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {   // static indices only: cf[k] = cq[k ^ j]
+                T.cf[k] = j == 0 ? cq[k] : j == 1 ? cq[k ^ 1] : j == 2 ? cq[k ^ 2] : cq[k ^ 3];
+            }
+            T.vsel = q == 3 ? 1 << (3 ^ j) : 0;
             T.rawm = P.raw16 + c_mom[q][j];
             T.dsel = 3; T.dsgn = 0.0;
             if (q == 1 && j == 0) { T.dsel = 0; T.dsgn = (double)vb.sx; }
