@@ -234,6 +234,28 @@ def test_P7_closed_box_fixed_point(oracle_mod):
     assert np.abs(pa[0] - 1).max() > 1e-4
 
 
+def test_P11_uniform_free_stream_is_preserved(oracle_mod):
+    """An empty box whose six faces are free-stream boundaries at the state of the gas: every upwind value
+    and the source are the same Maxwellian, so Eq.(7) returns it for every velocity whatever the (non-uniform) grid, and
+    the new moments are its discrete moments: the uniform state up to the quadrature error of a 24-node grid.  A sign or
+    direction mistake in the free-stream ghost, or a ghost at the wrong face, breaks it."""
+    fs = W.FaceBC(W.FREESTREAM, 1.1, 0.9, (0.3, -0.2, 0.1))
+    wl = W.cavity(0, 24, 0.2, stretch=1.5, nxyz=(6, 5, 4)).with_(
+        faces=[fs] * 6, rescale_mass=0, rho0=0.9, u0=(0.3, -0.2, 0.1), T0=1.1)
+    o = oracle_mod.Oracle(wl)
+    for it in range(2):
+        p = o.step()
+        # tolerance = quadrature error of the 24-node grid (tail truncation at |xi| = 6 of a Maxwellian centred at 0.3)
+        assert np.abs(p[0] - 0.9).max() < 1e-11 and np.abs(p[4] - 1.1).max() < 1e-11
+        assert np.abs(p[1] - 0.3).max() < 1e-11 and np.abs(p[2] + 0.2).max() < 1e-11 and np.abs(p[3] - 0.1).max() < 1e-11
+        assert np.abs(p[5:]).max() < 1e-11
+    # one velocity, from the exact initial state: the field is the free-stream Maxwellian itself
+    f = oracle_mod.Oracle(wl).sweep_velocity(20, 3, 11)
+    xi = np.array([wl.xi_x[20], wl.xi_y[3], wl.xi_z[11]])
+    fm = 0.9 / (np.pi * 1.1) ** 1.5 * np.exp(-((xi - np.array([0.3, -0.2, 0.1])) ** 2).sum() / 1.1)
+    assert np.abs(f / fm - 1).max() < 1e-12
+
+
 def test_P8_mirror_symmetry_and_mass(oracle_mod):
     wl = W.cavity(6, 8, 1.0)
     o = oracle_mod.Oracle(wl)

@@ -137,6 +137,24 @@ def test_closed_box_fixed_point(oracle_mod, kernel):
 
 
 @pytest.mark.parametrize("kernel", KERNELS)
+def test_uniform_free_stream_is_preserved(oracle_mod, kernel):
+    """P11 on the GPU: an empty box with free-stream faces at the state of the gas keeps that state, and agrees with the
+    oracle; non-uniform ragged grid."""
+    fs = W.FaceBC(W.FREESTREAM, 1.1, 0.9, (0.3, -0.2, 0.1))
+    wl = W.cavity(0, 24, 0.2, stretch=1.5, nxyz=(6, 5, 7)).with_(
+        faces=[fs] * 6, rescale_mass=0, rho0=0.9, u0=(0.3, -0.2, 0.1), T0=1.1)
+    s = make(wl, kernel)
+    o = oracle_mod.Oracle(wl)
+    for it in range(2):
+        s.iterate(1)
+        c = o.step()
+        g = s.moments().cpu().numpy()
+        assert np.abs(g[0] - 0.9).max() < 1e-11 and np.abs(g[4] - 1.1).max() < 1e-11 and np.abs(g[1] - 0.3).max() < 1e-11
+        assert np.abs(g - c).max() < 1e-13   # q and sigma are ~1e-12 here: absolute comparison with the oracle
+    s.close()
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
 def test_config2_shape_sampled_step(oracle_mod, kernel):
     """Config 2 at full physical size (64^3 tanh grid, 32^3 velocities) with a zero-weight velocity subset so the
     oracle finishes in seconds: one step from a perturbed state; raw moments and wall densities must agree."""
