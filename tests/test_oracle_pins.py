@@ -234,6 +234,25 @@ def test_P7_closed_box_fixed_point(oracle_mod):
     assert np.abs(pa[0] - 1).max() > 1e-4
 
 
+def test_P12_closed_box_with_solid_block_fixed_point(oracle_mod):
+    """P7 with a masked block inside the box: all walls, including the faces of the solid cells, are stationary and at the
+    gas temperature, so the uniform state stays a fixed point; checks the solid-face table, its ghosts and its wall-flux
+    normalisation (reading G20)."""
+    wl = W.cavity(6, 24, 0.1, U_w=0.0)
+    solid = np.zeros((6, 6, 6), dtype=np.uint8)
+    solid[2:4, 1:3, 3:5] = 1
+    wl = wl.with_(solid=solid)
+    o = oracle_mod.Oracle(wl)
+    assert o.nface == 6 * 36 + 6 * 4    # 6 domain faces + the 24 faces of the 2 x 2 x 2 block
+    fluid = solid.reshape(-1) == 0
+    for it in range(2):
+        p = o.step()
+        assert np.abs(p[0][fluid] - 1).max() < 1e-13 and np.abs(p[4][fluid] - 1).max() < 2e-13
+        assert np.abs(p[1:4][:, fluid]).max() < 1e-13 and np.abs(p[5:][:, fluid]).max() < 1e-13
+        assert np.abs(p[:, ~fluid]).max() == 0.0
+        assert np.abs(o.rho_w[-24:] - 1).max() < 1e-13 and abs(o.scale - 1) < 1e-13
+
+
 def test_P11_uniform_free_stream_is_preserved(oracle_mod):
     """An empty box whose six faces are free-stream boundaries at the state of the gas: every upwind value
     and the source are the same Maxwellian, so Eq.(7) returns it for every velocity whatever the (non-uniform) grid, and
