@@ -375,3 +375,146 @@ def test_config0_history_reference_digits(oracle_mod):
     assert all(h2 < h1 for h1, h2 in zip(hist[2:], hist[3:]))
     assert hist[-1] < 1e-5
     assert o.total_mass(o.prim8[0]) == pytest.approx(1.0, rel=1e-14)
+
+
+# ------------------------------------------------------------------------------------------------
+# Pins added in round 2 for the wall Maxwellian (Eq.(8), reading G3) and the mass rescale
+# (reading G8): the round-1 pins were blind to the sign of U_w, to T_w != 1 and to what is rescaled.
+def test_P13_wall_maxwellian_is_scipy_gaussian(oracle_mod):
+    """g_w = trivariate normal pdf with mean U_w and variance T_w/2 per axis (Eq.(8) in v_m units with the wall velocity in
+    the exponent, G3), for T_w != 1 and a wall velocity with three different non-zero components: a wrong sign of U_w or
+    a wrong power of T_w in the normalisation fails."""
+    from scipy.stats import multivariate_normal
+    rng = np.random.default_rng(13)
+    for Tw, Uw in [(0.7, (0.16, -0.05, 0.08)), (1.3, (-0.3, 0.2, 0.11)), (1.0, (0.16, 0.0, 0.0))]:
+        faces = [W.FaceBC(W.WALL_DIFFUSE, Tw, 1.0, Uw) for _ in range(6)]
+        wl = W.cavity(2, 4, 1.0).with_(faces=faces, solid_bc=W.FaceBC(W.WALL_DIFFUSE, Tw, 1.0, Uw))
+        o = oracle_mod.Oracle(wl)
+        ref = multivariate_normal(mean=np.array(Uw), cov=np.eye(3) * Tw / 2)
+        for xi in rng.uniform(-2.5, 2.5, (12, 3)):
+            for b in (0, 3, 5, 6):
+                assert o.gwall(b, xi) == pytest.approx(ref.pdf(xi), rel=1e-13)
+        # not symmetric in the sign of U_w
+        xi = np.array([0.9, -0.4, 0.3])
+        assert abs(o.gwall(5, xi) / ref.pdf(-xi) - 1) > 1e-2 or max(abs(u) for u in Uw) == 0
+
+
+def test_P3b_phi_unit_hot_and_cold_moving_walls(oracle_mod):
+    """Phi_unit of a wall at T_w != 1 moving tangentially: equals the half-range flux of the scipy normal pdf summed over
+    the nodes (no formula of ours), tends to sqrt(T_w / 4 pi) with relative gap ~ h^2 / (12 T_w)."""
+    from scipy.stats import multivariate_normal
+    for Tw in (0.7, 1.3):
+        Uw = (0.2, -0.1, 0.0)    # tangential to the z walls
+        m = 32
+        wl = W.cavity(2, m, 1.0, vrange=7.0)
+        faces = list(wl.faces)
+        faces[4] = W.FaceBC(W.WALL_DIFFUSE, Tw, 1.0, Uw)
+        faces[5] = W.FaceBC(W.WALL_DIFFUSE, Tw, 1.0, Uw)
+        wl = wl.with_(faces=faces)
+        o = oracle_mod.Oracle(wl)
+        phi = o.phi_unit()
+        cell, dirn, area = o.face_table()
+        X, Y, Z, Wt = vel_arrays(wl)
+        g = multivariate_normal(mean=np.array(Uw), cov=np.eye(3) * Tw / 2).pdf(np.stack([X, Y, Z], axis=-1))
+        lo = (Wt * np.where(Z > 0, Z, 0.0) * g).sum()      # z- wall: leaving = xi_z > 0
+        hi = (Wt * np.where(Z < 0, -Z, 0.0) * g).sum()     # z+ wall: leaving = xi_z < 0
+        assert phi[dirn == 4][0] == pytest.approx(lo, rel=1e-13)
+        assert phi[dirn == 5][0] == pytest.approx(hi, rel=1e-13)
+        exact = math.sqrt(Tw / (4 * math.pi))
+        h = 14.0 / (m - 1)
+        gap = abs(phi[dirn == 4][0] / exact - 1)
+        assert 0.5 * h * h / (12 * Tw) < gap < 2.0 * h * h / (12 * Tw)
+        # the stationary T_w = 1 walls keep their own value
+        assert phi[dirn == 0][0] == pytest.approx((Wt * np.where(X > 0, X, 0.0)
+                                                   * multivariate_normal(mean=np.zeros(3), cov=np.eye(3) / 2).pdf(
+                                                       np.stack([X, Y, Z], axis=-1))).sum(), rel=1e-13)
+
+
+def _moving_channel(Uw=(0.3, 0.0, 0.0), Tw=1.2, rho=0.9):
+    """Gas drifting with the four side walls (y+-, z+-: tangential motion at U_w, temperature T_w); the x faces are free
+    stream at the same state.  In the frame of the walls this is P7 + P11."""
+    fs = W.FaceBC(W.FREESTREAM, Tw, rho, Uw)
+    wall = W.FaceBC(W.WALL_DIFFUSE, Tw, 1.0, Uw)
+    return W.cavity(0, 32, 0.2, vrange=7.0, stretch=1.5, nxyz=(5, 4, 6)).with_(
+        faces=[fs, fs, wall, wall, wall, wall], rescale_mass=0, rho0=rho, u0=Uw, T0=Tw)
+
+
+def test_P14_gas_moving_with_the_walls_is_a_fixed_point(oracle_mod):
+    """Eq.(8) with the wall velocity in the exponent (G3): a uniform gas at (rho, U_w, T_w) between walls that move
+    tangentially at U_w with temperature T_w (free stream at the same state on the two open faces) is a fixed point: every
+    ghost, every upwind value and the source are the same Maxwellian.  With the sign of U_w flipped in g_w, or T_w entering
+    the normalisation with the wrong power, the wall ghost differs from the gas and the state moves at O(1e-2)."""
+    wl = _moving_channel()
+    o = oracle_mod.Oracle(wl)
+    assert np.abs(o.rho_w[o.face_table()[1] >= 2] - 0.9).max() < 1e-11   # rho_w^0 of the walls = rho0
+    for it in range(2):
+        p = o.step()
+        assert np.abs(p[0] - 0.9).max() < 1e-11 and np.abs(p[4] - 1.2).max() < 1e-11
+        assert np.abs(p[1] - 0.3).max() < 1e-11 and np.abs(p[2:4]).max() < 1e-11
+        assert np.abs(p[5:]).max() < 1e-11
+        cell, dirn, area = o.face_table()
+        assert np.abs(o.rho_w[dirn >= 2] - 0.9).max() < 1e-11
+    # the pin has teeth: walls moving the other way are not a fixed point
+    bad = wl.with_(faces=wl.faces[:2] + [W.FaceBC(W.WALL_DIFFUSE, 1.2, 1.0, (-0.3, 0.0, 0.0))] * 4)
+    pb = oracle_mod.Oracle(bad).step()
+    assert np.abs(pb[1] - 0.3).max() > 1e-3
+
+
+def test_P15_lid_drags_the_gas_in_its_direction(oracle_mod):
+    """Cavity, a few iterations: the gas layer next to the lid moves in the direction of U_w (G3, G11), and reversing the
+    lid mirrors the solution in x."""
+    wl = W.cavity(6, 12, 1.0)
+    o = oracle_mod.Oracle(wl)
+    for it in range(4):
+        p = o.step()
+    F = p.reshape(14, wl.nz, wl.ny, wl.nx)
+    assert F[1][-1].mean() > 1e-2            # top layer follows the lid (U_w = +0.16 along x)
+    assert F[1][-1].min() > 0
+    assert F[1][0].mean() < F[1][-1].mean() * 0.5   # return flow / weaker at the bottom
+    wr = W.cavity(6, 12, 1.0, U_w=-0.16)
+    orv = oracle_mod.Oracle(wr)
+    for it in range(4):
+        pr = orv.step()
+    Fr = pr.reshape(14, wl.nz, wl.ny, wl.nx)
+    assert np.abs(Fr[1] + F[1][:, :, ::-1]).max() < 1e-13
+    assert np.abs(Fr[0] - F[0][:, :, ::-1]).max() < 1e-13
+
+
+def test_P16_mass_rescale_scales_everything_linear_in_f(oracle_mod):
+    """Reading G8 of PAPER.md:257 ('scale the density of the whole field'): the state after the rescale is the set of
+    moments of s * f^{n+1}, s = mass0 / sum rho V.  Brute force: store the 6-D f, scale it, take the central moments
+    of Eq.(3) directly; rho, q and sigma carry the factor, u and T do not, and rho_w carries it too."""
+    wl = W.cavity(4, 8, 0.5, stretch=1.2)     # rescale_mass = 1; the 8-node quadrature makes s differ from 1 by O(0.1)
+    o = oracle_mod.Oracle(wl)
+    prim = W.perturbed_state(wl, seed=16, amp_q=0.01)
+    rng = np.random.default_rng(16)
+    rho_w = rng.uniform(0.9, 1.1, o.nface)
+    o.set_state(prim, rho_w)
+    p14 = o.step()
+    n = wl.n_cells
+    X, Y, Z, Wt = vel_arrays(wl)
+    f6 = np.empty((wl.mx, wl.my, wl.mz, n))
+    for ia in range(wl.mx):
+        for ib in range(wl.my):
+            for ic in range(wl.mz):
+                f6[ia, ib, ic] = o.sweep_velocity(ia, ib, ic, prim, rho_w).reshape(-1)
+    rho_raw = np.einsum("abc,abcn->n", Wt, f6)
+    dx, dy, dz = np.diff(wl.xf), np.diff(wl.yf), np.diff(wl.zf)
+    V = (dz[:, None, None] * dy[None, :, None] * dx[None, None, :]).reshape(-1)
+    s = o.mass0 / (rho_raw * V).sum()
+    assert abs(s - 1) > 1e-3 and o.scale == pytest.approx(s, rel=1e-13)
+    for c in range(0, n, 5):
+        r, u, t, q, sig = central_moments(s * f6[..., c], X, Y, Z, Wt)
+        assert p14[0, c] == pytest.approx(r, rel=1e-13)
+        assert np.allclose(p14[1:4, c], u, atol=1e-14)
+        assert p14[4, c] == pytest.approx(t, rel=1e-13)
+        assert np.allclose(p14[5:8, c], q, atol=1e-14)
+        assert np.allclose(p14[8:14, c], sig, atol=1e-14)
+    cell, dirn, area = o.face_table()
+    phi_u = o.phi_unit()
+    comp = [X, X, Y, Y, Z, Z]
+    for fidx in range(0, o.nface, 7):
+        c, d = cell[fidx], dirn[fidx]
+        xin = comp[d] * (1.0 if d & 1 else -1.0)
+        bf = (Wt * np.where(xin > 0, xin, 0.0) * (s * f6[..., c])).sum()
+        assert o.rho_w[fidx] == pytest.approx(bf / phi_u[fidx], rel=1e-13)
