@@ -41,6 +41,7 @@ int fail(int code, const char *fmt, ...)
     } while (0)
 
 constexpr int HIST_CAP = 16384;
+constexpr int RAW_SINK_ROWS = 1024;   // accumulator rows past the last cell: one per CTA of the tile sweep, for dead cells
 const double PI = 3.14159265358979323846;
 
 }  // namespace
@@ -65,7 +66,7 @@ struct dvm_solver {
     // device arrays
     double *d_invdx = nullptr, *d_invdy = nullptr, *d_invdz = nullptr, *d_dx = nullptr, *d_dy = nullptr, *d_dz = nullptr;
     unsigned char *d_flags = nullptr, *d_face_slot = nullptr;
-    int *d_face_of = nullptr;
+    int *d_face_of = nullptr, *d_face_cell = nullptr, *d_face_dir = nullptr;
     double *d_xi[3] = {nullptr, nullptr, nullptr}, *d_w[3] = {nullptr, nullptr, nullptr};
     double *d_prim = nullptr, *d_prim_new = nullptr, *d_coef = nullptr, *d_raw = nullptr;
     double *d_rho_w = nullptr, *d_phi = nullptr, *d_phi_unit = nullptr;
@@ -287,7 +288,7 @@ int plan(dvm_solver *s)
             }
         }
         const size_t nitems = s->tile.items.size();
-        s->tile_grid = (int)std::min<size_t>((size_t)resident, nitems);
+        s->tile_grid = (int)std::min<size_t>(std::min<size_t>((size_t)resident, nitems), (size_t)RAW_SINK_ROWS);
         const size_t fbytes = (s->tile.xface_doubles + s->tile.yface_doubles) * sizeof(double);
         s->d_xface = (double *)s->dalloc(s->tile.xface_doubles * sizeof(double));
         s->d_yface = (double *)s->dalloc(s->tile.yface_doubles * sizeof(double));
@@ -504,6 +505,8 @@ int dvm_create(const dvm_grid *g, const dvm_vgrid *v, const dvm_gas *gas, const 
     rc |= upload(s, &s->d_gtab, gtab.data(), gtab.size());
     rc |= upload(s, &s->d_face_of, face_of.data(), (size_t)6 * n);
     rc |= upload(s, &s->d_face_slot, face_slot.data(), (size_t)s->nface);
+    rc |= upload(s, &s->d_face_cell, face_cell.data(), (size_t)s->nface);
+    rc |= upload(s, &s->d_face_dir, face_dir.data(), (size_t)s->nface);
     for (int d = 0; d < 3; ++d) {
         rc |= upload(s, &s->d_xi[d], s->xi[d].data(), s->xi[d].size());
         rc |= upload(s, &s->d_w[d], s->w[d].data(), s->w[d].size());
@@ -513,7 +516,7 @@ int dvm_create(const dvm_grid *g, const dvm_vgrid *v, const dvm_gas *gas, const 
     rc |= dzeros(s, &s->d_phi, (size_t)s->nface);
     rc |= dzeros(s, &s->d_prim_new, (size_t)NPRIM * n);
     rc |= dzeros(s, &s->d_coef, (size_t)NCOEF * n);
-    rc |= dzeros(s, &s->d_raw, (size_t)16 * n);
+    rc |= dzeros(s, &s->d_raw, (size_t)16 * (n + RAW_SINK_ROWS));
     s->npart = (n + 255) / 256;
     rc |= dzeros(s, &s->d_part, (size_t)7 * s->npart);
     rc |= dzeros(s, &s->d_scal, 8);
@@ -566,7 +569,7 @@ int dvm_iterate(dvm_solver *s, int niter)
     const UpdateParams U = update_params(s);
     const SweepParams P = sweep_params(s);
     for (int it = 0; it < niter; ++it) {
-        CK(cudaMemsetAsync(s->d_raw, 0, (size_t)16 * s->ncell * sizeof(double), s->stream));
+        CK(cudaMemsetAsync(s->d_raw, 0, (size_t)16 * (s->ncell + RAW_SINK_ROWS) * sizeof(double), s->stream));
         CK(cudaMemsetAsync(s->d_phi, 0, (size_t)s->nface * sizeof(double), s->stream));
         if (s->kernel == DVM_KERNEL_SLICE) {
             CK(launch_sweep_slice(P, (int)s->blocks.size(), s->nb_threads, s->stream));
@@ -577,6 +580,8 @@ int dvm_iterate(dvm_solver *s, int niter)
             s->epoch += 1;
             const TileParams TP = tile_params(s);
             CK(launch_sweep_tile(TP, s->tile_grid, s->stream));
+            CK(launch_phi_from_raw(s->d_raw, s->d_face_cell, s->d_face_dir, s->d_phi, s->nface, s->stream));
+            s->launches += 1;
         }
         s->launches += 1;
         int l = 0;

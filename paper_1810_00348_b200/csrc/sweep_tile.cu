@@ -28,6 +28,7 @@
 // Product code: shares nothing with oracle/.
 #include "sweep_tile.cuh"
 
+#include <cstddef>
 #include <cstdint>
 #include <cstdio>
 
@@ -37,7 +38,6 @@ namespace {
 
 constexpr int NVB = TILE_NVB;
 constexpr int NCELL = TILE_NCELL;
-constexpr int RB = 4;                                  // cells of a row whose moment reductions are interleaved
 constexpr int XLEVEL_DOUBLES = TILE_TY * NVB;          // one level of an x-face slot
 constexpr int YLEVEL_DOUBLES = TILE_TX * NVB;          // one level of a y-face slot
 constexpr unsigned XLEVEL_BYTES = XLEVEL_DOUBLES * 8u, YLEVEL_BYTES = YLEVEL_DOUBLES * 8u;
@@ -45,26 +45,48 @@ constexpr unsigned XLEVEL_BYTES = XLEVEL_DOUBLES * 8u, YLEVEL_BYTES = YLEVEL_DOU
 constexpr unsigned XROW_BYTES = 4 * TILE_NA * 32u;      // one 4-cell row of x entries
 constexpr unsigned REC_ROW_BYTES = 4 * (unsigned)sizeof(CellRec);
 
+// One tile row (4 cells along x) of one level: everything the row's arithmetic reads sits at a static offset from the
+// row's base address, whatever the row index and the level parity are.
+// One TMA bulk copy per level: source of level 0, byte step per level, destination in a LevelBuf; bytes = 0: skipped.
+struct CopyDesc {
+    const unsigned char *src;
+    long long step;
+    unsigned dst, bytes;
+    unsigned pad[2];
+};
+constexpr int NCOPY = 4 * TILE_TY + 2;              // per row: x, y, z factor rows and cell records; x-face and y-face input
+
+struct __align__(128) RowBuf {
+    // ---- staged by TMA two levels ahead ----
+    double4 xtab[4][TILE_NA];                      // per (cell', xi_x node): E, Q, e, a (slot r*4 + ag); cell' = position of
+    double4 ytab[4 * 8];                           // the cell in ascending absolute x;  [cell'][nbb]
+    double4 ztab[4 * 8];                           // [cell'][ncb]
+    CellRec rec[4];                                // per cell': 1/tau, cell index, neighbour flags, boundary faces
+    // ---- decoded per level by 16 threads (sweep-relative cell ii) ----
+    double4 spec[4];                               // rho_w of a solid ghost in x, y, z (slow-path levels)
+    double nu[4];                                  // 1/tau (1 for dead cells)
+    int code[4];                                   // 1: x-up solid ghost, 2: y-up, 4: z-up, 8: dead cell
+    int cidx[4];                                   // row of the [cell][16] accumulator: the cell index, or the CTA's sink row (dead)
+    int pad_[16];
+};
+static_assert(sizeof(RowBuf) % 128 == 0, "rows of the staging buffer must keep the TMA alignment");
+
+struct __align__(128) LevelBuf {
+    RowBuf row[TILE_TY];
+    double xface[TILE_TY][NVB];                    // x-face input of the level
+    double yface[TILE_TX][NVB];                    // y-face input of the level
+    double rwb[8];                                 // ghost densities of the domain faces: 4 x-face rows, 4 y-face columns
+};
+
 struct __align__(128) TileSmem {
-    // ---- staged by TMA two levels ahead (index = level parity) ----
-    double xface[2][TILE_TY][NVB];                 // x-face input of the level
-    double yface[2][TILE_TX][NVB];                 // y-face input
-    double4 xtab[2][NCELL][TILE_NA];               // per (cell', xi_x node): E, Q, e, a   (slot r*4 + ag); cell' = row * 4 +
-    double4 ytab[2][NCELL * 8];                    // position of the cell in ascending absolute x;  [cell'][nbb]
-    double4 ztab[2][NCELL * 8];                    // [cell'][ncb]
-    CellRec rec[2][NCELL];                         // per cell': 1/tau, cell index, neighbour flags, boundary faces
-    // ---- decoded per level by 16 threads (sweep-relative cell = jj * 4 + ii) ----
-    double nu[2][NCELL];                           // 1/tau (1 for dead cells)
-    double4 spec[2][NCELL];                        // rho_w of a solid ghost in x, y, z (slow-path levels)
-    int code[2][NCELL];                            // 1: x-up solid ghost, 2: y-up, 4: z-up, 8: dead cell
-    int cidx[2][NCELL];                            // global cell index or -1 (dead)
-    int dnface[2][NCELL][4];                       // wall face downwind in x, y, z (or -1); [3] = -1
-    double rwb[2][8];                              // ghost densities of the domain faces: 4 x-face rows, 4 y-face columns
+    LevelBuf lv[2];                                // index = level parity
     // ---- per item ----
     double xi_a[TILE_NA];                          // nodes of the block (0 beyond the box)
     double xi_bc[TILE_MAXBC];
     double g[4][3][16];                            // ghost Maxwellian 1-D factors: upwind x, y, z face and solid
+    CopyDesc desc[NCOPY];                          // the TMA copies of one level of this item (issue_level)
     unsigned long long mbar[2];
+    unsigned txbytes;                              // bytes the copies of one level deliver
     int item;
 };
 
@@ -135,12 +157,45 @@ __device__ __forceinline__ double fast_rcp(double d)
     const double t = fma(e, e, e);
     return fma(y, t, y);
 }
-__device__ __forceinline__ double shx(double v, int m) { return __shfl_xor_sync(0xffffffffu, v, m); }
+// Global REDs and face stores are volatile asm statements: they keep their program order, so ptxas cannot sink the
+// stores of a whole level to its end, where the burst would stall the warp on the load/store unit.
+__device__ __forceinline__ void red_f64(double *addr, double v)
+{
+    asm volatile("red.global.add.f64 [%0], %1;" ::"l"(addr), "d"(v));
+}
+__device__ __forceinline__ void st_f64x2(double *addr, double a, double b)
+{
+    asm volatile("st.global.v2.f64 [%0], {%1, %2};" ::"l"(addr), "d"(a), "d"(b));
+}
 
-// moment index (order of dvm_raw_moments) of output j of lane type q = lane & 3
-//   q = 0: S0 {1, xi_y, xi_z, xi_y^2}        q = 1: S1 {1, xi_y, xi_z, xi_y^2 + xi_z^2}
-//   q = 2: S0 {xi_z^2, xi_y xi_z, xi_y r2, xi_z r2}   q = 3: S2 {1, xi_y, xi_z}, S3 {1}
-__constant__ int c_mom[4][4] = {{0, 2, 3, 5}, {1, 7, 8, 10}, {6, 9, 11, 12}, {4, 11, 12, 10}};
+// D (8 x 8) += A (8 x 4, row-major) * B (4 x 8, column-major) in fp64 on the tensor cores (DMMA).  Fragments of lane l:
+// A[l >> 2][l & 3], B[l & 3][l >> 2], C/D[l >> 2][2 (l & 3) + {0, 1}].
+__device__ __forceinline__ void dmma(double &c0, double &c1, const double a, const double b)
+{
+    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+}
+
+// Velocity sums of Eq.(5) as two small matrix products per pair of cells (A, B) and warp.
+//   stage 1, once per computed value g (4 per cell and thread): C[p][pair] += X[p][ag] * g[ag][pair], the lane supplying
+//     its own g as the B fragment (k = its xi_x group ag = lane & 3, n = its (xi_y, xi_z) pair lane >> 2) and xi_x^p of
+//     its own node as the A fragment (p = (lane >> 2) & 3: rows 4..7 repeat rows 0..3).  After the 4 products
+//     C[p][pair] = sum over the 16 xi_x nodes of the block of xi_x^p g, for the warp's 8 pairs.  Cell A and cell B have
+//     an accumulator each; lanes 0..15 (rows 0..3) then keep A's, lanes 16..31 (rows 4..7) B's.
+//   stage 2, once per cell pair: D[row][j] = sum_pair C[row][pair] * M_j(pair), M = {1, y^2, y, z^2, z, yz, y r2, z r2},
+//     r2 = y^2 + z^2.  The C fragment of stage 1 (columns 2q, 2q + 1) is the A fragment of the two k-steps (pairs 0, 2, 4, 6
+//     and 1, 3, 5, 7) as it stands; every lane supplies M_(lane >> 2) of pairs 2q and 2q + 1 as B fragments.
+// 17 of the 32 values D[p][j] of a cell are products the 13 sums need; each lane adds its two results (j = 2q and
+// 2q + 1, p = (lane >> 2) & 3, q = lane & 3) to the [cell][16] accumulator row in L2 / HBM with a fp64 RED; sums made of
+// several products (xi_x |xi|^2 ...) simply receive several REDs.  Slots of the row: 0..12 = the 13 sums in the order of
+// dvm_raw_moments, except that slots 1, 2, 3 hold the first moments of the velocities with xi_d >= 0 only and slots 13,
+// 14, 15 those of xi_d < 0: every velocity block lies in one sign octant, so this costs nothing, and the half-range
+// sums are the wall-incident fluxes of Eq.(9): update.cu reads them from here, the sweep needs no flux
+// atomics.  c_slot0 / c_slot1: slot of the first / second result; c_use: 1 if the sums need it (a result they do not
+// need is added as 0 to a slot no other lane of the same instruction targets).
+__constant__ signed char c_slot0[4][4] = {{0, 2, 3, 11}, {1, 7, 8, 5}, {4, 11, 12, 6}, {10, 9, 2, 3}};
+__constant__ signed char c_use0[4][4] = {{1, 1, 1, 1}, {1, 1, 1, 0}, {1, 1, 1, 0}, {1, 0, 0, 0}};
+__constant__ signed char c_slot1[4][4] = {{5, 6, 9, 12}, {10, 10, 0, 1}, {2, 3, 4, 7}, {8, 11, 13, 14}};
+__constant__ signed char c_use1[4][4] = {{1, 1, 1, 1}, {1, 1, 0, 0}, {0, 0, 0, 0}, {0, 0, 0, 0}};
 
 // per-item constants, uniform over the CTA
 struct ItemCtx {
@@ -187,67 +242,93 @@ __device__ __forceinline__ double rwb_load(const TileParams &P, const ItemCtx &I
 
 __device__ __forceinline__ void rwb_store(TileSmem &s, int b, int tid, double v)
 {
-    if (tid >= 32 && tid < 40) s.rwb[b][tid - 32] = v;
+    if (tid >= 32 && tid < 40) s.lv[b].rwb[tid - 32] = v;
 }
 
-// TMA copies of level kp into buffer b = kp & 1: the x- / y-face input and, per 4-cell row, the x, y, z factor-table
-// rows and the cell records (tables.cu; every row is one contiguous run of the padded grid).  Executed by threads
-// 64..79 (one row copy each); thread 64 also posts the byte count and fetches the faces.
-__device__ __forceinline__ void issue_level(const TileParams &P, const ItemCtx &I, TileSmem &s, const VBlock &vb, int kp,
-                                            int tid, const double *xsrc, const double *ysrc)
+// The TMA copies of a level are described once per item (setup_copies: per 4-cell row the x, y, z factor-table rows and
+// the cell records - tables.cu; every row is one contiguous run of the padded grid - plus the x- and y-face input) and
+// issued per level by thread (q & 3) * 32 + (q >> 2) for copy q (issue_level), so every warp issues at most 5.
+__device__ __forceinline__ int copy_of_thread(int tid) { return (tid & 31) * 4 + (tid >> 5); }
+
+__device__ __forceinline__ void setup_copies(const TileParams &P, const ItemCtx &I, TileSmem &s, const VBlock &vb, int tid,
+                                             const double *xsrc, const double *ysrc)
 {
-    const int b = kp & 1, q = tid - 64;
-    if (q < 0 || q >= 4 * TILE_TY) return;
+    const int q = copy_of_thread(tid);
+    if (q >= NCOPY) return;
     const unsigned ybytes = 4u * vb.nbb * 32u, zbytes = 4u * vb.ncb * 32u;
-    if (q == 0) {
-        const unsigned faces = (I.first_x ? 0u : XLEVEL_BYTES) + (I.first_y ? 0u : YLEVEL_BYTES);
-        mbar_expect_tx(&s.mbar[b], faces + (unsigned)TILE_TY * (XROW_BYTES + ybytes + zbytes + REC_ROW_BYTES));
-        if (!I.first_x) tma_load(&s.xface[b][0][0], xsrc + (long long)kp * XLEVEL_DOUBLES, XLEVEL_BYTES, &s.mbar[b]);
-        if (!I.first_y) tma_load(&s.yface[b][0][0], ysrc + (long long)kp * YLEVEL_DOUBLES, YLEVEL_BYTES, &s.mbar[b]);
+    CopyDesc d;
+    d.pad[0] = d.pad[1] = 0;
+    if (q == 4 * TILE_TY) {
+        d.src = reinterpret_cast<const unsigned char *>(xsrc); d.step = XLEVEL_BYTES;
+        d.dst = (unsigned)offsetof(LevelBuf, xface); d.bytes = I.first_x ? 0u : XLEVEL_BYTES;
+    } else if (q == 4 * TILE_TY + 1) {
+        d.src = reinterpret_cast<const unsigned char *>(ysrc); d.step = YLEVEL_BYTES;
+        d.dst = (unsigned)offsetof(LevelBuf, yface); d.bytes = I.first_y ? 0u : YLEVEL_BYTES;
+    } else {
+        const int jj = q % TILE_TY, kind = q / TILE_TY;
+        // first cell (lowest absolute x) of row jj on the padded grid at level 0; rows may lie in the dead padding
+        const int jp = I.j0 + jj, ip0 = I.i0;
+        const int j = I.sy > 0 ? jp : P.ny - 1 - jp;
+        const int i = I.sx > 0 ? ip0 : P.nx - 4 - ip0;
+        const int k = I.sz > 0 ? 0 : P.nz - 1;
+        const long long npc = (long long)P.nz * P.nyp * P.nxp, lvl = (long long)P.nyp * P.nxp * I.sz;
+        const long long pc = ((long long)k * P.nyp + (j + TILE_PAD)) * P.nxp + (i + TILE_PAD);
+        const unsigned rowoff = (unsigned)(offsetof(LevelBuf, row) + jj * sizeof(RowBuf));
+        if (kind == 0) {
+            d.src = reinterpret_cast<const unsigned char *>(P.TX + ((long long)vb.xb * npc + pc) * TILE_NA);
+            d.step = lvl * TILE_NA * 32; d.dst = rowoff + (unsigned)offsetof(RowBuf, xtab); d.bytes = XROW_BYTES;
+        } else if (kind == 1) {
+            d.src = reinterpret_cast<const unsigned char *>(P.TY + ((long long)vb.yb * npc + pc) * vb.nbb);
+            d.step = lvl * vb.nbb * 32; d.dst = rowoff + (unsigned)offsetof(RowBuf, ytab); d.bytes = ybytes;
+        } else if (kind == 2) {
+            d.src = reinterpret_cast<const unsigned char *>(P.TZ + ((long long)vb.zb * npc + pc) * vb.ncb);
+            d.step = lvl * vb.ncb * 32; d.dst = rowoff + (unsigned)offsetof(RowBuf, ztab); d.bytes = zbytes;
+        } else {
+            d.src = reinterpret_cast<const unsigned char *>(P.rec + pc);
+            d.step = lvl * (long long)sizeof(CellRec); d.dst = rowoff + (unsigned)offsetof(RowBuf, rec); d.bytes = REC_ROW_BYTES;
+        }
     }
-    const int jj = q % TILE_TY, kind = q / TILE_TY;
-    // first cell (lowest absolute x) of row jj on the padded grid; rows may lie in the dead padding
-    const int jp = I.j0 + jj, ip0 = I.i0;
-    const int j = I.sy > 0 ? jp : P.ny - 1 - jp;
-    const int i = I.sx > 0 ? ip0 : P.nx - 4 - ip0;
-    const int k = I.sz > 0 ? kp : P.nz - 1 - kp;
-    const long long npc = (long long)P.nz * P.nyp * P.nxp;
-    const long long pc = ((long long)k * P.nyp + (j + TILE_PAD)) * P.nxp + (i + TILE_PAD);
-    if (kind == 0) tma_load(&s.xtab[b][jj * 4][0], P.TX + ((long long)vb.xb * npc + pc) * TILE_NA, XROW_BYTES, &s.mbar[b]);
-    else if (kind == 1) tma_load(&s.ytab[b][jj * 4 * vb.nbb], P.TY + ((long long)vb.yb * npc + pc) * vb.nbb, ybytes, &s.mbar[b]);
-    else if (kind == 2) tma_load(&s.ztab[b][jj * 4 * vb.ncb], P.TZ + ((long long)vb.zb * npc + pc) * vb.ncb, zbytes, &s.mbar[b]);
-    else tma_load(&s.rec[b][jj * 4], P.rec + pc, REC_ROW_BYTES, &s.mbar[b]);
+    s.desc[q] = d;
+    if (q == 0)
+        s.txbytes = (I.first_x ? 0u : XLEVEL_BYTES) + (I.first_y ? 0u : YLEVEL_BYTES) +
+                    (unsigned)TILE_TY * (XROW_BYTES + ybytes + zbytes + REC_ROW_BYTES);
+}
+
+// issue the copies of level kp into buffer kp & 1 (the descriptors were written by the same threads)
+__device__ __forceinline__ void issue_level(TileSmem &s, int kp, int tid)
+{
+    const int q = copy_of_thread(tid);
+    if (q >= NCOPY) return;
+    const int b = kp & 1;
+    if (q == 0) mbar_expect_tx(&s.mbar[b], s.txbytes);
+    const CopyDesc d = s.desc[q];
+    if (d.bytes) tma_load(reinterpret_cast<unsigned char *>(&s.lv[b]) + d.dst, d.src + (long long)kp * d.step, d.bytes, &s.mbar[b]);
 }
 
 // Per-cell records of level kp (buffer b = kp & 1) decoded from the staged CellRec rows by threads 96..111; the caller
 // has waited for the level's TMA copies.  Returns 1 if this thread saw a fluid cell with a solid upwind ghost.
-__device__ __forceinline__ int decode_records(const TileParams &P, const ItemCtx &I, TileSmem &s, int kp, int tid)
+__device__ __forceinline__ int decode_records(const TileParams &P, const ItemCtx &I, TileSmem &s, int kp, int tid, int sink)
 {
     const int b = kp & 1;
     int special = 0;
     if (tid >= 96 && tid < 96 + NCELL) {
         const int cell = tid - 96, ii = cell & 3, jj = cell >> 2;
-        const CellRec &r = s.rec[b][jj * 4 + (I.sx > 0 ? ii : 3 - ii)];
+        RowBuf &R = s.lv[b].row[jj];
+        const CellRec &r = R.rec[I.sx > 0 ? ii : 3 - ii];
         const bool dead = r.cidx < 0;
-        const int flags = r.flags & 0xff, sfl = (r.flags >> 8) & 0xff;
+        const int sfl = (r.flags >> 8) & 0xff;
         int code = 8;
         double4 sp = make_double4(0.0, 0.0, 0.0, 0.0);
-        int dn[3] = {-1, -1, -1};
         if (!dead) {
             code = ((sfl >> I.upx) & 1) | (((sfl >> I.upy) & 1) << 1) | (((sfl >> I.upz) & 1) << 2);
             if (code & 1) sp.x = P.rho_w[r.face[I.upx]];
             if (code & 2) sp.y = P.rho_w[r.face[I.upy]];
             if (code & 4) sp.z = P.rho_w[r.face[I.upz]];
-            if ((flags >> (I.upx ^ 1)) & 1) dn[0] = r.face[I.upx ^ 1];
-            if ((flags >> (I.upy ^ 1)) & 1) dn[1] = r.face[I.upy ^ 1];
-            if ((flags >> (I.upz ^ 1)) & 1) dn[2] = r.face[I.upz ^ 1];
         }
-        s.code[b][cell] = code;
-        s.spec[b][cell] = sp;
-        s.cidx[b][cell] = r.cidx;
-        s.nu[b][cell] = dead ? 1.0 : r.nu;
-        s.dnface[b][cell][0] = dn[0]; s.dnface[b][cell][1] = dn[1]; s.dnface[b][cell][2] = dn[2];
-        s.dnface[b][cell][3] = -1;
+        R.code[ii] = code;
+        R.spec[ii] = sp;
+        R.cidx[ii] = dead ? sink : r.cidx;
+        R.nu[ii] = dead ? 1.0 : r.nu;
         special = (code & 7) != 0;
     }
     return special;
@@ -256,13 +337,14 @@ __device__ __forceinline__ int decode_records(const TileParams &P, const ItemCtx
 // Ghost values of the domain faces of level kp (buffer b) for a tile at the upwind x / y edge of the domain
 __device__ __forceinline__ void fill_faces(const ItemCtx &I, TileSmem &s, int b, int tid, int ag, int yidx, int zidx)
 {
+    LevelBuf &L = s.lv[b];
     if (I.first_x) {
         const double gyz = s.g[0][1][yidx] * s.g[0][2][zidx];
 #pragma unroll
         for (int r = 0; r < 4; ++r) {
             const double G = s.g[0][0][4 * ag + r] * gyz;
 #pragma unroll
-            for (int jj = 0; jj < TILE_TY; ++jj) s.xface[b][jj][tid * 4 + r] = s.rwb[b][jj] * G;
+            for (int jj = 0; jj < TILE_TY; ++jj) L.xface[jj][tid * 4 + r] = L.rwb[jj] * G;
         }
     }
     if (I.first_y) {
@@ -271,164 +353,188 @@ __device__ __forceinline__ void fill_faces(const ItemCtx &I, TileSmem &s, int b,
         for (int r = 0; r < 4; ++r) {
             const double G = s.g[1][0][4 * ag + r] * gyz;
 #pragma unroll
-            for (int ii = 0; ii < 4; ++ii) s.yface[b][ii][tid * 4 + r] = s.rwb[b][4 + ii] * G;
+            for (int ii = 0; ii < 4; ++ii) L.yface[ii][tid * 4 + r] = L.rwb[4 + ii] * G;
         }
     }
-}
-
-// Reduction of the four power sums S_p = sum_r xi_x^p g_r of a lane over the 4 x-groups of a lane quad and the
-// (xi_y, xi_z) pairs with lane bits 2 and 3 (see the header comment), for N cells at once, stage by stage, so that
-// the shuffle latency of one cell is covered by the other cells' instructions.  Leaves, in every lane, the partial
-// sum over its half-warp of one of the 16 products of the cell; lane & 15 names it (c_mom).  S[c][p] = power sum p of cell c; k[c] = result of cell c.
-template <int N>
-__device__ __forceinline__ void reduce_halfN(const double (&S)[N][4], const double (&cf)[4], const int vsel, int lane,
-                                             double (&k)[N])
-{
-    const bool b0 = lane & 1, b1 = lane & 2;
-    double a0[N], u[N], v[N];
-#pragma unroll
-    for (int c = 0; c < N; ++c) a0[c] = S[c][0] + shx(S[c][0], 1);
-#pragma unroll
-    for (int c = 0; c < N; ++c) u[c] = (b1 ? S[c][2] : S[c][1]) + shx(b1 ? S[c][1] : S[c][2], 2);
-#pragma unroll
-    for (int c = 0; c < N; ++c) v[c] = S[c][3] + shx(b1 ? 0.0 : S[c][3], 2);
-#pragma unroll
-    for (int c = 0; c < N; ++c) a0[c] += shx(a0[c], 2);
-#pragma unroll
-    for (int c = 0; c < N; ++c) u[c] += shx(u[c], 1);
-#pragma unroll
-    for (int c = 0; c < N; ++c) v[c] += shx(v[c], 1);
-    // Pair stage without selects between the shuffles: the lane with pair bits m = 2 b2 + b3 keeps its four products in
-    // the order r_k = o_(k xor m) (cf is stored permuted), so that both exchange steps send fixed registers; only the
-    // operand of the S3 product (lane role 3, product 3, register 3 xor m: bit k of vsel) is chosen per register.
-    const bool s0 = vsel & 1, s1 = vsel & 2, s2 = vsel & 4, s3 = vsel & 8;
-    double r0[N], r1[N];
-#pragma unroll
-    for (int c = 0; c < N; ++c) {
-        const double U = b0 ? u[c] : a0[c];
-        const double p0 = cf[0] * (s0 ? v[c] : U), p1 = cf[1] * (s1 ? v[c] : U);
-        const double p2 = cf[2] * (s2 ? v[c] : U), p3 = cf[3] * (s3 ? v[c] : U);
-        r0[c] = p0 + shx(p2, 4);
-        r1[c] = p1 + shx(p3, 4);
-    }
-#pragma unroll
-    for (int c = 0; c < N; ++c) k[c] = r0[c] + shx(r1[c], 8);
 }
 
 // per-thread constants of an item
 struct ThreadCtx {
-    double X1[4], X2[4], X3[4];  // xi_x, xi_x^2, xi_x^3 of the thread's nodes
-    double cf[4];                // expansion coefficients of this lane, in the order cf[k] = c[k xor m] (reduce_halfN)
-    int vsel;                    // bit k: product k of this lane takes the S3 sum
-    double dsgn;                 // sign of the wall-flux contribution of this lane
-    double *rawm;                // raw16 + moment slot of this lane
+    double aX[4];                // stage-1 A fragments per node r: xi_x^p, p = (lane >> 2) & 3
+    double yz0, yz1;             // stage-2 B fragments: monomial lane >> 2 of the warp's pairs 2 (lane & 3), 2 (lane & 3) + 1
+    double *raw0, *raw1;         // raw16 + accumulator slot of the lane's two results
+    double use0, use1;           // 1 if the result is one of the products the sums need, else 0 (the RED then adds 0)
+    int xo[4], yo[4], zo[4];     // byte offsets in a RowBuf of the thread's table entries of cell ii (r = 0 for x)
     int ag, yi, zi;              // xi_x group, rows of the thread's xi_y and xi_z nodes in xi_bc / g
-    int yl, zl, nbb, ncb;        // local xi_y / xi_z index in the block, block shape
     int xrev;                    // 3 if the sweep runs against x (table rows are in ascending absolute x), else 0
-    int dsel;                    // wall-flux direction (3 = none) of this lane
 };
 
-// velocity sums of two cells (A: lower half-warp keeps it, B: upper half-warp) -> accumulators, one RED per lane
-__device__ __forceinline__ void emit_pair(const TileParams &P, TileSmem &s, const int b, const int cellA, double kA, double kB,
-                                          const ThreadCtx &T, const int lane)
+__device__ __forceinline__ const double4 &entry(const RowBuf &R, int byte_off)
+{
+    return *reinterpret_cast<const double4 *>(reinterpret_cast<const unsigned char *>(&R) + byte_off);
+}
+
+// stage 2 for the cell pair (iiA, iiA + 1) of a row and the REDs of its results (lanes 0..15: cell A, 16..31: cell B).
+// No predicates and no branches (the row stays one basic block): a result the sums do not need is multiplied by 0 and
+// added to a slot no other lane of the instruction targets; dead cells carry the CTA's sink row and g = 0.
+__device__ __forceinline__ void emit_pair(const RowBuf &R, const int iiA, const double a0, const double a1, const double b0,
+                                          const double b1, const ThreadCtx &T, const int lane)
 {
     const bool hi = lane & 16;
-    const double keep = hi ? kB : kA, send = hi ? kA : kB;
-    const double tot = keep + shx(send, 16);
-    const int cell = cellA + (hi ? 1 : 0);
-    const int c = s.cidx[b][cell];
-    if (c >= 0) {
-        atomicAdd(T.rawm + (long long)c * 16, tot);
-        const int f = s.dnface[b][cell][T.dsel];
-        if (f >= 0) atomicAdd(P.phi + f, T.dsgn * tot);
+    double d0 = 0.0, d1 = 0.0;
+    dmma(d0, d1, hi ? b0 : a0, T.yz0);
+    dmma(d0, d1, hi ? b1 : a1, T.yz1);
+    const long long c = R.cidx[iiA + (hi ? 1 : 0)];
+    red_f64(T.raw0 + c * 16, d0 * T.use0);
+    red_f64(T.raw1 + c * 16, d1 * T.use1);
+}
+
+// One row (4 cells along the sweep-relative x) of a level, fast path: zrow holds the values of the row in the previous
+// z-plane (the z-upwind operands) and receives the new ones, yup holds the y-upwind operands (the staged y-face for the
+// first row of the tile, else the row just computed).  Dead cells (outside the domain / solid) have all-zero table
+// entries and nu = 1, so they produce g = 0 by the same arithmetic.
+__device__ __forceinline__ void compute_row(const RowBuf &R, const double *xin, double (&zrow)[4][4], const double (&yup)[4][4],
+                                            const ThreadCtx &T, const int tid, const int lane, double *xout, const bool wx)
+{
+    double fx[4];
+    {
+        const double2 *p = reinterpret_cast<const double2 *>(xin + tid * 4);
+        const double2 v0 = p[0], v1 = p[1];
+        fx[0] = v0.x; fx[1] = v0.y; fx[2] = v1.x; fx[3] = v1.y;
+    }
+    double acc[2][2];
+#pragma unroll
+    for (int ii = 0; ii < 4; ++ii) {
+        const double4 yt = entry(R, T.yo[ii]);
+        const double4 zt = entry(R, T.zo[ii]);
+        const double Eyz = yt.x * zt.x, Qyz = yt.y + zt.y, eyz = yt.z + zt.z;
+        const double ay = yt.w, az = zt.w;
+        const double dyz = (ay + az) + R.nu[ii];
+        // Everything that does not depend on the x-upwind value, for the 4 nodes of the thread in lock step (dependent
+        // instructions 4 apart: the fp64 pipe takes a warp instruction every 2 clocks and has a latency of ~10): the cell
+        // value is g = W g_xup + V with W = a_x / den and V = (a_y g_yup + a_z g_zup + src) / den, Eq.(7) PAPER.md:75-79.
+        double4 xt[4];
+        double t1[4], t2[4], d[4], y0[4], sE[4], e[4], W[4], V[4];
+#pragma unroll
+        for (int r = 0; r < 4; ++r) xt[r] = entry(R, T.xo[ii] + r * 4 * 32);
+#pragma unroll
+        for (int r = 0; r < 4; ++r) d[r] = xt[r].w + dyz;
+#pragma unroll
+        for (int r = 0; r < 4; ++r) t1[r] = xt[r].y + Qyz;
+#pragma unroll
+        for (int r = 0; r < 4; ++r) asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y0[r]) : "d"(d[r]));
+#pragma unroll
+        for (int r = 0; r < 4; ++r) t2[r] = xt[r].z + eyz;
+#pragma unroll
+        for (int r = 0; r < 4; ++r) sE[r] = xt[r].x * Eyz;
+#pragma unroll
+        for (int r = 0; r < 4; ++r) e[r] = fma(-d[r], y0[r], 1.0);
+#pragma unroll
+        for (int r = 0; r < 4; ++r) t1[r] = fma(t1[r], t2[r], 1.0);
+#pragma unroll
+        for (int r = 0; r < 4; ++r) e[r] = fma(e[r], e[r], e[r]);
+#pragma unroll
+        for (int r = 0; r < 4; ++r) V[r] = sE[r] * t1[r];
+#pragma unroll
+        for (int r = 0; r < 4; ++r) y0[r] = fma(y0[r], e[r], y0[r]);       // 1 / den (MUFU seed + cubic Newton step)
+#pragma unroll
+        for (int r = 0; r < 4; ++r) V[r] = fma(ay, yup[ii][r], V[r]);
+#pragma unroll
+        for (int r = 0; r < 4; ++r) W[r] = xt[r].w * y0[r];
+#pragma unroll
+        for (int r = 0; r < 4; ++r) V[r] = fma(az, zrow[ii][r], V[r]);
+#pragma unroll
+        for (int r = 0; r < 4; ++r) V[r] *= y0[r];
+        // the recurrence along x: one DFMA per value
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+            const double gg = fma(W[r], fx[r], V[r]);
+            fx[r] = gg;
+            zrow[ii][r] = gg;
+        }
+        acc[ii & 1][0] = 0.0; acc[ii & 1][1] = 0.0;
+#pragma unroll
+        for (int r = 0; r < 4; ++r) dmma(acc[ii & 1][0], acc[ii & 1][1], T.aX[r], zrow[ii][r]);
+        if (ii & 1) emit_pair(R, ii - 1, acc[0][0], acc[0][1], acc[1][0], acc[1][1], T, lane);
+    }
+    if (wx) {
+        st_f64x2(xout + tid * 4, fx[0], fx[1]);
+        st_f64x2(xout + tid * 4 + 2, fx[2], fx[3]);
     }
 }
 
-// One level of the column, fast path (no solid ghost in the level): 4 rows x 4 cells x 4 velocities per thread,
-// fully unrolled so that the plane lives in registers.  Dead cells (outside the domain / solid) have all-zero table
-// entries and nu = 1, so they produce g = 0 by the same arithmetic.
-__device__ __forceinline__ void compute_level(const TileParams &P, TileSmem &s, const int b, double (&pl)[TILE_TY][4][4],
-                                              const ThreadCtx &T, const int tid, const int lane, double *xout,
+// One level of the column, fast path (no solid ghost in the level): 4 rows x 4 cells x 4 velocities per thread with the
+// plane in registers (static indices only).  The B200 instruction cache holds 32 KB, and a level loop larger than that is
+// fetch-bound at 1/3 instruction per clock and scheduler (profiles/r01_ifetch_microbench.txt), so how many rows are
+// unrolled is a code-size decision.  DVM_ROW_UNROLL = 4: all rows unrolled, the y-upwind operands of a row are the
+// registers of the row before, no register moves; = 2: a 2-iteration loop over row pairs whose body works on row slots
+// 0, 1 and then swaps them with slots 2, 3; = 1: a 4-iteration loop that works on slot 0 and rotates the slots.
+#ifndef DVM_ROW_UNROLL
+#define DVM_ROW_UNROLL 2
+#endif
+__device__ __forceinline__ void compute_level(const TileParams &P, const LevelBuf &L, double (&pl)[TILE_TY][4][4],
+                                              const ThreadCtx &T, const int tid, const int lane, double *xout, const bool wx,
                                               double *yout)
 {
-    // The 4 rows of the tile are a real loop: the B200 instruction cache holds 32 KB, and a level loop larger than
-    // that is fetch-bound at 1/3 instruction per clock and scheduler (profiles/r01_ifetch_microbench.txt); the
-    // fully unrolled level was 48 KB.  The plane stays in registers with static indices: every iteration works on
-    // row slot 0 (old values of row jj -> new values) with the new row jj - 1 in slot 3, then the slots rotate.
-    // y-upwind operands of the row: the staged y-face for the first row, then the row just computed
     double yu[4][4];
 #pragma unroll
     for (int ii = 0; ii < 4; ++ii) {
-        const double2 *p = reinterpret_cast<const double2 *>(&s.yface[b][ii][tid * 4]);
+        const double2 *p = reinterpret_cast<const double2 *>(&L.yface[ii][tid * 4]);
         const double2 v0 = p[0], v1 = p[1];
         yu[ii][0] = v0.x; yu[ii][1] = v0.y; yu[ii][2] = v1.x; yu[ii][3] = v1.y;
     }
-#pragma unroll 1
-    for (int jj = 0; jj < TILE_TY; ++jj) {
-        double fx[4];
-        {
-            const double2 *p = reinterpret_cast<const double2 *>(&s.xface[b][jj][tid * 4]);
-            const double2 v0 = p[0], v1 = p[1];
-            fx[0] = v0.x; fx[1] = v0.y; fx[2] = v1.x; fx[3] = v1.y;
-        }
-        double SR[RB][4];
+#if DVM_ROW_UNROLL == 4
+    compute_row(L.row[0], L.xface[0], pl[0], yu, T, tid, lane, xout, wx);
 #pragma unroll
-        for (int ii = 0; ii < 4; ++ii) {
-            const int cell = jj * 4 + ii;
-            const int cp = jj * 4 + (ii ^ T.xrev);   // position of the cell in the staged table rows
-            const double4 yt = s.ytab[b][cp * T.nbb + T.yl];
-            const double4 zt = s.ztab[b][cp * T.ncb + T.zl];
-            const double Eyz = yt.x * zt.x, Qyz = yt.y + zt.y, eyz = yt.z + zt.z;
-            const double ay = yt.w, az = zt.w;
-            const double dyz = (ay + az) + s.nu[b][cell];
-            double S0 = 0.0, S1 = 0.0, S2 = 0.0, S3 = 0.0;
+    for (int jj = 1; jj < TILE_TY; ++jj) compute_row(L.row[jj], L.xface[jj], pl[jj], pl[jj - 1], T, tid, lane, xout + jj * NVB, wx);
+#elif DVM_ROW_UNROLL == 2
+    static_assert(TILE_TY == 4, "row pairs");
+    const RowBuf *R = &L.row[0];
+    const double *xin = &L.xface[0][0];
+#pragma unroll 1
+    for (int h = 0; h < 2; ++h) {
+        compute_row(R[0], xin, pl[0], yu, T, tid, lane, xout, wx);
+        compute_row(R[1], xin + NVB, pl[1], pl[0], T, tid, lane, xout + NVB, wx);
+        R += 2;
+        xin += 2 * NVB;
+        xout += 2 * NVB;
+#pragma unroll
+        for (int ii = 0; ii < 4; ++ii)
 #pragma unroll
             for (int r = 0; r < 4; ++r) {
-                const double4 xt = s.xtab[b][cp][r * 4 + T.ag];
-                const double src = (xt.x * Eyz) * fma(xt.y + Qyz, xt.z + eyz, 1.0);
-                const double inv = fast_rcp(xt.w + dyz);
-                double num = fma(ay, yu[ii][r], src);
-                num = fma(az, pl[0][ii][r], num);
-                num = fma(xt.w, fx[r], num);
-                const double gg = num * inv;
-                fx[r] = gg;
-                pl[0][ii][r] = gg;
-                yu[ii][r] = gg;
-                S0 += gg;
-                S1 = fma(T.X1[r], gg, S1);
-                S2 = fma(T.X2[r], gg, S2);
-                S3 = fma(T.X3[r], gg, S3);
+                const double t0 = pl[0][ii][r], t1 = pl[1][ii][r];
+                yu[ii][r] = t1;
+                pl[0][ii][r] = pl[2][ii][r]; pl[1][ii][r] = pl[3][ii][r];
+                pl[2][ii][r] = t0; pl[3][ii][r] = t1;
             }
-            SR[ii % RB][0] = S0; SR[ii % RB][1] = S1; SR[ii % RB][2] = S2; SR[ii % RB][3] = S3;
-            if (ii % RB == RB - 1) {
-                double k[RB];
-                reduce_halfN<RB>(SR, T.cf, T.vsel, lane, k);
-#pragma unroll
-                for (int c = 0; c < RB; c += 2) emit_pair(P, s, b, cell - (RB - 1) + c, k[c], k[c + 1], T, lane);
-            }
-        }
-        if (xout) {
-            double2 *p = reinterpret_cast<double2 *>(xout + jj * NVB + tid * 4);
-            p[0] = make_double2(fx[0], fx[1]);
-            p[1] = make_double2(fx[2], fx[3]);
-        }
+    }
+#else
+    const RowBuf *R = &L.row[0];
+    const double *xin = &L.xface[0][0];
+#pragma unroll 1
+    for (int jj = 0; jj < TILE_TY; ++jj) {
+        compute_row(*R, xin, pl[0], yu, T, tid, lane, xout, wx);
+        ++R;
+        xin += NVB;
+        xout += NVB;
         // rotate the row slots: (0, 1, 2, 3) <- (1, 2, 3, 0); after the 4th iteration the rows are back in place
 #pragma unroll
         for (int ii = 0; ii < 4; ++ii)
 #pragma unroll
             for (int r = 0; r < 4; ++r) {
                 const double t = pl[0][ii][r];
+                yu[ii][r] = t;
 #pragma unroll
                 for (int q = 0; q + 1 < TILE_TY; ++q) pl[q][ii][r] = pl[q + 1][ii][r];
                 pl[TILE_TY - 1][ii][r] = t;
             }
     }
+#endif
     if (yout) {
 #pragma unroll
         for (int ii = 0; ii < 4; ++ii) {
-            double2 *p = reinterpret_cast<double2 *>(yout + ii * NVB + tid * 4);
-            p[0] = make_double2(pl[TILE_TY - 1][ii][0], pl[TILE_TY - 1][ii][1]);
-            p[1] = make_double2(pl[TILE_TY - 1][ii][2], pl[TILE_TY - 1][ii][3]);
+            st_f64x2(yout + ii * NVB + tid * 4, pl[TILE_TY - 1][ii][0], pl[TILE_TY - 1][ii][1]);
+            st_f64x2(yout + ii * NVB + tid * 4 + 2, pl[TILE_TY - 1][ii][2], pl[TILE_TY - 1][ii][3]);
         }
     }
 }
@@ -436,35 +542,38 @@ __device__ __forceinline__ void compute_level(const TileParams &P, TileSmem &s, 
 // One level that holds a solid ghost (a fluid cell whose upwind neighbour is a masked cell): the same arithmetic
 // written as compact loops over a copy of the plane in local memory.  Rare (the surface of a masked body), so its
 // speed does not matter; keeping it out of the unrolled path halves the code the instruction cache has to hold.
-__device__ __forceinline__ void compute_level_slow(const TileParams &P, TileSmem &s, const int b, double *pl,
+__device__ __forceinline__ void compute_level_slow(const TileParams &P, TileSmem &s, const LevelBuf &L, double *pl,
                                                    const ThreadCtx &T, const int tid, const int lane, double *xout,
                                                    double *yout)
 {
     const double gyz = s.g[3][1][T.yi] * s.g[3][2][T.zi];
 #pragma unroll 1
     for (int jj = 0; jj < TILE_TY; ++jj) {
+        const RowBuf &R = L.row[jj];
         double fx[4];
 #pragma unroll
-        for (int r = 0; r < 4; ++r) fx[r] = s.xface[b][jj][tid * 4 + r];
-        double kprev = 0.0;
+        for (int r = 0; r < 4; ++r) fx[r] = L.xface[jj][tid * 4 + r];
+        double acc[2][2] = {{0.0, 0.0}, {0.0, 0.0}};
 #pragma unroll 1
         for (int ii = 0; ii < 4; ++ii) {
             const int cell = jj * 4 + ii;
-            const int cp = jj * 4 + (ii ^ T.xrev);   // position of the cell in the staged table rows
-            const double4 yt = s.ytab[b][cp * T.nbb + T.yl];
-            const double4 zt = s.ztab[b][cp * T.ncb + T.zl];
+            const int xo = ii == 0 ? T.xo[0] : ii == 1 ? T.xo[1] : ii == 2 ? T.xo[2] : T.xo[3];
+            const int yo = ii == 0 ? T.yo[0] : ii == 1 ? T.yo[1] : ii == 2 ? T.yo[2] : T.yo[3];
+            const int zo = ii == 0 ? T.zo[0] : ii == 1 ? T.zo[1] : ii == 2 ? T.zo[2] : T.zo[3];
+            const double4 yt = entry(R, yo);
+            const double4 zt = entry(R, zo);
             const double Eyz = yt.x * zt.x, Qyz = yt.y + zt.y, eyz = yt.z + zt.z;
             const double ay = yt.w, az = zt.w;
-            const double dyz = (ay + az) + s.nu[b][cell];
-            const int code = s.code[b][cell];
-            const double4 sp = s.spec[b][cell];
-            double S0 = 0.0, S1 = 0.0, S2 = 0.0, S3 = 0.0;
+            const double dyz = (ay + az) + R.nu[ii];
+            const int code = R.code[ii];
+            const double4 sp = R.spec[ii];
+            double c0 = 0.0, c1 = 0.0;
 #pragma unroll
             for (int r = 0; r < 4; ++r) {
                 const double Pg = s.g[3][0][4 * T.ag + r] * gyz;
-                const double4 xt = s.xtab[b][cp][r * 4 + T.ag];
+                const double4 xt = entry(R, xo + r * 4 * 32);
                 double xu = fx[r], zu = pl[cell * 4 + r];
-                double yu = jj == 0 ? s.yface[b][ii][tid * 4 + r] : pl[(cell - 4) * 4 + r];
+                double yu = jj == 0 ? L.yface[ii][tid * 4 + r] : pl[(cell - 4) * 4 + r];
                 if (code & 1) xu = sp.x * Pg;
                 if (code & 2) yu = sp.y * Pg;
                 if (code & 4) zu = sp.z * Pg;
@@ -477,17 +586,13 @@ __device__ __forceinline__ void compute_level_slow(const TileParams &P, TileSmem
                 if (code & 8) gg = 0.0;
                 fx[r] = gg;
                 pl[cell * 4 + r] = gg;
-                S0 += gg;
-                S1 = fma(T.X1[r], gg, S1);
-                S2 = fma(T.X2[r], gg, S2);
-                S3 = fma(T.X3[r], gg, S3);
+                dmma(c0, c1, T.aX[r], gg);
             }
-            const double S1c[1][4] = {{S0, S1, S2, S3}};
-            double k1[1];
-            reduce_halfN<1>(S1c, T.cf, T.vsel, lane, k1);
-            const double kk = k1[0];
-            if (ii & 1) emit_pair(P, s, b, cell - 1, kprev, kk, T, lane);
-            else kprev = kk;
+            if (ii & 1) {
+                emit_pair(R, ii - 1, acc[0][0], acc[0][1], c0, c1, T, lane);
+            } else {
+                acc[0][0] = c0; acc[0][1] = c1;
+            }
         }
         if (xout) {
 #pragma unroll
@@ -517,6 +622,7 @@ __global__ void __launch_bounds__(TILE_THREADS, TILE_MIN_CTAS) sweep_tile_kernel
     }
     __syncthreads();
     unsigned par[2] = {0u, 0u};
+    const int sink = (int)P.ncell + (int)blockIdx.x;   // accumulator row that takes the (zero) sums of dead cells
 
     for (;;) {
         // ---- next item (dependency order), wait for its upwind items ----
@@ -550,10 +656,11 @@ __global__ void __launch_bounds__(TILE_THREADS, TILE_MIN_CTAS) sweep_tile_kernel
 
         // ---- TMA copies of levels 0 and 1 (the staging buffers are free: every thread passed the end-of-item
         //      barrier; the upwind items' face stores were made with the generic proxy) ----
-        if (tid >= 64 && tid < 64 + 4 * TILE_TY) {
+        setup_copies(P, I, s, vb, tid, xdst, ydst);
+        if (copy_of_thread(tid) < NCOPY) {
             fence_proxy_async_global();
-            issue_level(P, I, s, vb, 0, tid, xdst, ydst);
-            if (P.nz > 1) issue_level(P, I, s, vb, 1, tid, xdst, ydst);
+            issue_level(s, 0, tid);
+            if (P.nz > 1) issue_level(s, 1, tid);
         }
         // ---- per-item tables: nodes, ghost factors; ghost densities of the domain faces of levels 0 and 1 ----
         {
@@ -587,42 +694,56 @@ __global__ void __launch_bounds__(TILE_THREADS, TILE_MIN_CTAS) sweep_tile_kernel
 
         ThreadCtx T;
         T.ag = lane & 3;
-        T.nbb = vb.nbb; T.ncb = vb.ncb;
         T.xrev = vb.sx > 0 ? 0 : 3;
         {
             const int pair = warp * 8 + (lane >> 2);
-            T.yl = pair % vb.nbb; T.zl = pair / vb.nbb;
-            T.yi = T.yl;
-            T.zi = vb.nbb + T.zl;
-            const double xb = s.xi_bc[T.yi], xc = s.xi_bc[T.zi], r2 = xb * xb + xc * xc;
-            const int q = lane & 3, j = ((lane >> 2) & 1) * 2 + ((lane >> 3) & 1);
-            double cq[4];
-            if (q == 0) { cq[0] = 1.0; cq[1] = xb; cq[2] = xc; cq[3] = xb * xb; }
-            else if (q == 1) { cq[0] = 1.0; cq[1] = xb; cq[2] = xc; cq[3] = r2; }
-            else if (q == 2) { cq[0] = xc * xc; cq[1] = xb * xc; cq[2] = xb * r2; cq[3] = xc * r2; }
-            else { cq[0] = 1.0; cq[1] = xb; cq[2] = xc; cq[3] = 1.0; }
+            const int yl = pair % vb.nbb, zl = pair / vb.nbb;
+            T.yi = yl;
+            T.zi = vb.nbb + zl;
+            // table entries of the thread in a row buffer: cell ii sits at position ii ^ xrev of the staged rows
 #pragma unroll
-            for (int k = 0; k < 4; ++k) {   // static indices only: cf[k] = cq[k ^ j]
-                T.cf[k] = j == 0 ? cq[k] : j == 1 ? cq[k ^ 1] : j == 2 ? cq[k ^ 2] : cq[k ^ 3];
+            for (int ii = 0; ii < 4; ++ii) {
+                const int cp = ii ^ T.xrev;
+                T.xo[ii] = (int)offsetof(RowBuf, xtab) + (cp * TILE_NA + T.ag) * 32;
+                T.yo[ii] = (int)offsetof(RowBuf, ytab) + (cp * vb.nbb + yl) * 32;
+                T.zo[ii] = (int)offsetof(RowBuf, ztab) + (cp * vb.ncb + zl) * 32;
             }
-            T.vsel = q == 3 ? 1 << (3 ^ j) : 0;
-            T.rawm = P.raw16 + c_mom[q][j];
-            T.dsel = 3; T.dsgn = 0.0;
-            if (q == 1 && j == 0) { T.dsel = 0; T.dsgn = (double)vb.sx; }
-            if (q == 0 && j == 1) { T.dsel = 1; T.dsgn = (double)vb.sy; }
-            if (q == 0 && j == 2) { T.dsel = 2; T.dsgn = (double)vb.sz; }
+            // stage-1 A fragments: xi_x^p of the thread's own nodes, p = (lane >> 2) & 3
+            const int row = lane >> 2, pw = row & 3;
 #pragma unroll
             for (int r = 0; r < 4; ++r) {
                 const double x = s.xi_a[4 * T.ag + r];
-                T.X1[r] = x; T.X2[r] = x * x; T.X3[r] = x * x * x;
+                T.aX[r] = pw == 0 ? 1.0 : pw == 1 ? x : pw == 2 ? x * x : x * x * x;
             }
+            // stage-2 B fragments: monomial j = lane >> 2 of the (xi_y, xi_z) nodes of pairs 2q and 2q + 1 of this warp
+            const int j = lane >> 2, q = lane & 3;
+            double mono[2];
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+                const int pr = warp * 8 + 2 * q + e;
+                const double y = s.xi_bc[pr % vb.nbb], z = s.xi_bc[vb.nbb + pr / vb.nbb], r2 = y * y + z * z;
+                mono[e] = j == 0 ? 1.0 : j == 1 ? y * y : j == 2 ? y : j == 3 ? z * z : j == 4 ? z : j == 5 ? y * z
+                        : j == 6 ? y * r2 : z * r2;
+            }
+            T.yz0 = mono[0]; T.yz1 = mono[1];
+            // results of this lane: D[p][2q], D[p][2q + 1] and their accumulator slots
+            int s0 = c_slot0[pw][q];
+            const int s1 = c_slot1[pw][q];
+            const bool u0 = c_use0[pw][q], u1 = c_use1[pw][q];
+            if (s0 >= 1 && s0 <= 3) {
+                // first moments: half-range slot by the sign of the block; an unneeded result goes to the other one
+                const int sg = s0 == 1 ? vb.sx : s0 == 2 ? vb.sy : vb.sz;
+                if ((sg < 0) == u0) s0 += 12;
+            }
+            T.raw0 = P.raw16 + s0; T.raw1 = P.raw16 + s1;
+            T.use0 = u0 ? 1.0 : 0.0; T.use1 = u1 ? 1.0 : 0.0;
         }
 
         // records and boundary faces of level 0 (its copies were issued above; the wait does not consume the phase)
         int special = 0;
         if (tid >= 96 && tid < 96 + NCELL) {
             mbar_wait(&s.mbar[0], par[0]);
-            special = decode_records(P, I, s, 0, tid);
+            special = decode_records(P, I, s, 0, tid, sink);
         }
         fill_faces(I, s, 0, tid, T.ag, T.yi, T.zi);
         // plane = ghost of the upwind z face of the domain
@@ -660,30 +781,31 @@ __global__ void __launch_bounds__(TILE_THREADS, TILE_MIN_CTAS) sweep_tile_kernel
                 for (int c = 0; c < NCELL; ++c)
 #pragma unroll
                     for (int r = 0; r < 4; ++r) tmp[c * 4 + r] = pl[c >> 2][c & 3][r];
-                compute_level_slow(P, s, b, tmp, T, tid, lane, xout, yout);
+                compute_level_slow(P, s, s.lv[b], tmp, T, tid, lane, xout, yout);
 #pragma unroll
                 for (int c = 0; c < NCELL; ++c)
 #pragma unroll
                     for (int r = 0; r < 4; ++r) pl[c >> 2][c & 3][r] = tmp[c * 4 + r];
             } else {
-                compute_level(P, s, b, pl, T, tid, lane, xout, yout);
+                compute_level(P, s.lv[b], pl, T, tid, lane, xdst + (long long)kp * XLEVEL_DOUBLES, write_x, yout);
             }
             rwb_store(s, b, tid, vrw);
             int sp = 0;
             if (kp + 1 < P.nz) {
                 if (tid >= 96 && tid < 96 + NCELL) {
                     mbar_wait(&s.mbar[b ^ 1], par[b ^ 1]);   // level kp + 1 has landed (issued a level ago)
-                    sp = decode_records(P, I, s, kp + 1, tid);
+                    sp = decode_records(P, I, s, kp + 1, tid, sink);
                 }
                 fill_faces(I, s, b ^ 1, tid, T.ag, T.yi, T.zi);
             }
             special = __shfl_sync(0xffffffffu, __syncthreads_or(sp), 0);
-            if (tid >= 64 && tid < 64 + 4 * TILE_TY && kp + 2 < P.nz) {
+            if (copy_of_thread(tid) < NCOPY && kp + 2 < P.nz) {
                 fence_proxy_async_smem();  // this level's reads of the staging buffers before the TMA overwrites them
-                issue_level(P, I, s, vb, kp + 2, tid, xdst, ydst);
+                issue_level(s, kp + 2, tid);
             }
         }
         // ---- publish: faces of this item are complete ----
+        asm volatile("" ::: "memory");
         __threadfence();
         __syncthreads();
         if (tid == 0) st_release(P.done + n, P.epoch);

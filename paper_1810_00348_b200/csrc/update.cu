@@ -68,10 +68,12 @@ __global__ void __launch_bounds__(UB) convert_kernel(const UpdateParams U)
         if (U.flags[c] & FLAG_SOLID) {
             for (int m = 0; m < NPRIM; ++m) U.prim_new[m * n + c] = 0.0;
         } else {
-            const double *r = U.raw + c * 16;   // [cell][16] accumulator, 13 used
+            // [cell][16] accumulator: 13 sums; the first moments are kept as two half-range sums (slots 1..3: xi_d >= 0,
+            // slots 13..15: xi_d < 0; the slice kernel leaves the latter 0), see sweep_tile.cu
+            const double *r = U.raw + c * 16;
             const double rho = r[0];
             const double ir = 1.0 / rho;
-            const double ux = r[1] * ir, uy = r[2] * ir, uz = r[3] * ir;
+            const double ux = (r[1] + r[13]) * ir, uy = (r[2] + r[14]) * ir, uz = (r[3] + r[15]) * ir;
             const double mxx = r[4], myy = r[5], mzz = r[6];
             const double mxy = r[7], mxz = r[8], myz = r[9];
             const double pxx = mxx - rho * ux * ux, pyy = myy - rho * uy * uy, pzz = mzz - rho * uz * uz;
@@ -185,7 +187,23 @@ __global__ void __launch_bounds__(UB) raw_export_kernel(const double *raw16, dou
 {
     const long long c = (long long)blockIdx.x * UB + threadIdx.x;
     if (c >= n) return;
-    for (int m = 0; m < NRAW; ++m) out13[m * n + c] = raw16[c * 16 + m];
+    for (int m = 0; m < NRAW; ++m) out13[m * n + c] = raw16[c * 16 + m] + (m >= 1 && m <= 3 ? raw16[c * 16 + 12 + m] : 0.0);
+}
+
+// Wall-incident fluxes of Eq.(9) from the half-range first moments the tile sweep leaves in the accumulator
+// rows: a face on side d of its cell is hit by the velocities moving towards d, Phi = sum w |xi_n| f over them.
+__global__ void __launch_bounds__(UB) phi_from_raw_kernel(const double *raw16, const int *face_cell, const int *face_dir, double *phi,
+                                                          int nface)
+{
+    const int f = blockIdx.x * UB + threadIdx.x;
+    if (f >= nface) return;
+    const int c = face_cell[f], d = face_dir[f];
+    double v = 0.0;
+    if (c >= 0) {
+        const double *r = raw16 + (long long)c * 16;
+        v = (d & 1) ? r[1 + (d >> 1)] : -r[13 + (d >> 1)];
+    }
+    phi[f] = v;
 }
 
 static inline int nblk(long long n) { return (int)((n + UB - 1) / UB); }
@@ -199,6 +217,12 @@ cudaError_t launch_pack(const UpdateParams &U, cudaStream_t st)
 cudaError_t launch_raw_export(const double *raw16, double *out13, long long n, cudaStream_t st)
 {
     raw_export_kernel<<<nblk(n), UB, 0, st>>>(raw16, out13, n);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_phi_from_raw(const double *raw16, const int *face_cell, const int *face_dir, double *phi, int nface, cudaStream_t st)
+{
+    phi_from_raw_kernel<<<nblk(nface), UB, 0, st>>>(raw16, face_cell, face_dir, phi, nface);
     return cudaGetLastError();
 }
 

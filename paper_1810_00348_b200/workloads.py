@@ -222,6 +222,9 @@ def config(idx: int) -> Workload:
         return cavity(128, 64, 0.01, iterations=50, name="cfg4_cavity_128^3x64^3_Kn0.01")
     if idx == 5:   # not in BASELINE.json: the paper's own cube run
         return cube_flow_paper(name="cfg5_cube_paper_191x181x181_v48^3_Ma2_Kn1")
+    if idx == 6:   # not in BASELINE.json: a 16-level slab of config 4 (same x-y plane, velocity grid and gas), the stand-in
+        # for config 4 under `ncu --set full`, whose replay passes save and restore the whole 52 GB workspace of config 4
+        return cavity(0, 64, 0.01, iterations=50, nxyz=(128, 128, 16), name="cfg6_slab_of_cfg4_128x128x16_v64^3_Kn0.01")
     raise ValueError(f"no config {idx}")
 
 
