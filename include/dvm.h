@@ -57,6 +57,8 @@ extern "C" {
 
 #define DVM_OPT_KERNEL    1
 #define DVM_OPT_MAX_F_MBYTES 2 /* tile kernel: cap (MiB) on the f workspace; velocity blocks then sweep in batches (0 = none) */
+#define DVM_OPT_TILE_RV   3 /* tile kernel: velocities per thread, 4 (128-thread CTAs, velocity blocks of 16 x 8 x 4 nodes) or 2
+                             (256-thread CTAs, blocks of 8 x 8 x 8 nodes); 0 = the library chooses by lane use (default) */
 
 typedef struct dvm_solver dvm_solver; /* opaque */
 
@@ -145,15 +147,18 @@ int dvm_set_option(dvm_solver *s, int option, int value);
 /* Sweep-kernel variant in use: DVM_KERNEL_SLICE / DVM_KERNEL_TILE once the first dvm_iterate has planned the
  * workspace, the requested value (possibly DVM_KERNEL_AUTO) before. */
 int dvm_kernel_used(const dvm_solver *s);
+/* Velocities per thread of the tile kernel: 2 or 4 once the first dvm_iterate has planned, the requested value before. */
+int dvm_tile_rv(const dvm_solver *s);
 /* Host-only (needs no device): the work decomposition the tile kernel would use for an nx x ny x nz grid and the
- * velocity nodes of v when target_ctas items should run concurrently and at most max_blocks velocity blocks are in
- * flight at once (0 = all; "smaller batches").  counts5 = number of velocity blocks, tiles along x, tiles
+ * velocity nodes of v when target_ctas items should run concurrently, at most max_blocks velocity blocks are in
+ * flight at once (0 = all; "smaller batches") and a thread carries rv velocities (2, 4, or 0 = the
+ * library's choice for these nodes).  counts5 = number of velocity blocks, tiles along x, tiles
  * along y, band height P, blocks per batch.  items9 (may be NULL) receives, for the first max_items work items in
  * hand-out order, {velocity block, tile x, tile y, predecessor in x, predecessor in y (for tile y = 0 of a later batch:
  * the last reader of the y-face slot), previous user of the x-face slot, x-face slot, octant bits, face-slot set};
  * predecessors are item indices or -1.  Returns the number of items. */
-int dvm_plan_query(int nx, int ny, int nz, const dvm_vgrid *v, int target_ctas, int max_blocks, int *counts5, int *items9,
-                   int max_items);
+int dvm_plan_query(int nx, int ny, int nz, const dvm_vgrid *v, int target_ctas, int max_blocks, int rv, int *counts5,
+                   int *items9, int max_items);
 /* Bytes of device workspace held by the solver, and the part of it that holds distribution-function values. */
 int dvm_workspace_bytes(const dvm_solver *s, size_t *total, size_t *f_bytes);
 /* Number of kernel launches enqueued by this solver so far (bench.py's gpu_launches). */

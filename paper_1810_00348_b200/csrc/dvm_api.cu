@@ -11,6 +11,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -61,6 +62,7 @@ struct dvm_solver {
     int iters = 0;
     int kernel = DVM_KERNEL_AUTO;
     long long max_f_mbytes = 0;   // cap on the f workspace of the tile kernel (0 = none)
+    int tile_rv = 0;              // velocities per thread of the tile kernel: 0 = choose, 2, 4
     bool planned = false;
     long long launches = 0;
     // device arrays
@@ -215,7 +217,7 @@ TableParams table_params(dvm_solver *s)
 {
     TableParams T{};
     T.nx = s->nx; T.ny = s->ny; T.nz = s->nz; T.nxp = s->nxp; T.nyp = s->nyp;
-    T.nbb = s->tile.nbb; T.ncb = s->tile.ncb; T.nxb = s->nxb; T.nyb = s->nyb; T.nzb = s->nzb;
+    T.na = tile_na(s->tile.rv); T.nbb = s->tile.nbb; T.ncb = s->tile.ncb; T.nxb = s->nxb; T.nyb = s->nyb; T.nzb = s->nzb;
     T.ncell = s->ncell; T.coef = s->d_coef; T.flags = s->d_flags;
     T.invdx = s->d_invdx; T.invdy = s->d_invdy; T.invdz = s->d_invdz;
     T.xi_x = s->d_xi[0]; T.xi_y = s->d_xi[1]; T.xi_z = s->d_xi[2];
@@ -232,6 +234,26 @@ void split_axis(const std::vector<double> &xi, int lo[2], int cnt[2])
     int nneg = 0;
     while (nneg < (int)xi.size() && xi[nneg] < 0.0) ++nneg;
     lo[0] = 0; cnt[0] = nneg; lo[1] = nneg; cnt[1] = (int)xi.size() - nneg;
+}
+
+// Variant of the tile kernel for a velocity grid when the caller leaves the choice open: the one whose velocity blocks
+// (16 x 8 x 4 nodes for RV = 4, 8 x 8 x 8 for RV = 2) waste fewer lanes on padding; RV_BIAS is the measured throughput of
+// RV = 2 relative to RV = 4 when both fill their blocks.
+constexpr double RV_BIAS = 0.8;
+int choose_rv(const std::vector<double> xi[3])
+{
+    if (const char *e = std::getenv("DVM_TILE_RV")) {
+        const int v = std::atoi(e);
+        if (v == 2 || v == 4) return v;
+    }
+    const long long nvel = (long long)xi[0].size() * xi[1].size() * xi[2].size();
+    double fill[2] = {0.0, 0.0};
+    for (int t = 0; t < 2; ++t) {
+        TilePlan tp;
+        if (tile_plan(4, 4, 1, xi, 1, 0, t == 0 ? 4 : 2, &tp)) return 4;
+        fill[t] = (double)nvel / ((double)tp.vblocks.size() * TILE_NVB);
+    }
+    return fill[1] * RV_BIAS > fill[0] ? 2 : 4;
 }
 
 // Decide the kernel variant and build the block table + f workspace (once, before the first iteration).
@@ -269,12 +291,14 @@ int plan(dvm_solver *s)
         s->f_bytes = fbytes;
     } else {
         int per_sm = 0, dev = 0, nsm = 0;
-        CK(tile_configure(&per_sm));
+        const int rv = s->tile_rv ? s->tile_rv : choose_rv(s->xi);
+        s->tile_rv = rv;
+        CK(tile_configure(rv, &per_sm));
         CK(cudaGetDevice(&dev));
         CK(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
         if (per_sm < 1) return fail(DVM_ECUDA, "tile kernel does not fit on an SM");
         const int resident = per_sm * nsm;
-        if (tile_plan(s->nx, s->ny, s->nz, s->xi, resident, 0, &s->tile)) return fail(DVM_EINVAL, "tile plan failed");
+        if (tile_plan(s->nx, s->ny, s->nz, s->xi, resident, 0, rv, &s->tile)) return fail(DVM_EINVAL, "tile plan failed");
         if (s->max_f_mbytes > 0) {
             // cap on the f workspace: fewer velocity blocks in flight (batches); the band height P
             // grows as the batch shrinks, so iterate to a fixed point; one block is the floor
@@ -284,7 +308,7 @@ int plan(dvm_solver *s)
                 const double need = (double)(s->tile.xface_doubles + s->tile.yface_doubles) * 8.0;
                 if (need <= cap || B == 1) break;
                 B = std::max(1, std::min(B - 1, (int)(cap / ((s->tile.P * TILE_TY + s->tile.ntx * TILE_TX) * lvl))));
-                if (tile_plan(s->nx, s->ny, s->nz, s->xi, resident, B, &s->tile)) return fail(DVM_EINVAL, "tile plan failed");
+                if (tile_plan(s->nx, s->ny, s->nz, s->xi, resident, B, rv, &s->tile)) return fail(DVM_EINVAL, "tile plan failed");
             }
         }
         const size_t nitems = s->tile.items.size();
@@ -296,7 +320,7 @@ int plan(dvm_solver *s)
         s->f_bytes = fbytes;
         // factor tables on the padded grid: [1-D block][nz][nyp][nxp][width] entries of 32 bytes, zero in the padding
         {
-            s->nxb = (int)s->tile.xnode.size() / TILE_NA;
+            s->nxb = (int)s->tile.xnode.size() / tile_na(rv);
             s->nyb = (int)s->tile.ynode.size() / s->tile.nbb;
             s->nzb = (int)s->tile.znode.size() / s->tile.ncb;
             const size_t npc = (size_t)s->nz * s->nyp * s->nxp;
@@ -552,6 +576,12 @@ int dvm_set_option(dvm_solver *s, int option, int value)
         s->kernel = value;
         return DVM_OK;
     }
+    if (option == DVM_OPT_TILE_RV) {
+        if (s->planned) return fail(DVM_EINVAL, "the tile-kernel variant must be chosen before the first iteration");
+        if (value != 0 && value != 2 && value != 4) return fail(DVM_EINVAL, "velocities per thread must be 0 (choose), 2 or 4");
+        s->tile_rv = value;
+        return DVM_OK;
+    }
     if (option == DVM_OPT_MAX_F_MBYTES) {
         if (s->planned) return fail(DVM_EINVAL, "the workspace cap must be set before the first iteration");
         if (value < 0) return fail(DVM_EINVAL, "negative workspace cap");
@@ -579,7 +609,7 @@ int dvm_iterate(dvm_solver *s, int niter)
             CK(cudaMemsetAsync(s->d_counter, 0, sizeof(int), s->stream));
             s->epoch += 1;
             const TileParams TP = tile_params(s);
-            CK(launch_sweep_tile(TP, s->tile_grid, s->stream));
+            CK(launch_sweep_tile(TP, s->tile_rv, s->tile_grid, s->stream));
             CK(launch_phi_from_raw(s->d_raw, s->d_face_cell, s->d_face_dir, s->d_phi, s->nface, s->stream));
             s->launches += 1;
         }
@@ -614,6 +644,7 @@ int dvm_residual(dvm_solver *s, double *host_out3)
 int dvm_num_faces(const dvm_solver *s) { return s ? s->nface : fail(DVM_EINVAL, "NULL solver"); }
 int dvm_iterations_done(const dvm_solver *s) { return s ? s->iters : fail(DVM_EINVAL, "NULL solver"); }
 int dvm_kernel_used(const dvm_solver *s) { return s ? s->kernel : fail(DVM_EINVAL, "NULL solver"); }
+int dvm_tile_rv(const dvm_solver *s) { return s ? s->tile_rv : fail(DVM_EINVAL, "NULL solver"); }
 long long dvm_launch_count(const dvm_solver *s) { return s ? s->launches : -1; }
 
 int dvm_get_state(dvm_solver *s, double *dev_prim14, double *dev_rho_wall)
@@ -694,15 +725,16 @@ int dvm_step_host(dvm_solver *s, const double *host_prim8, const double *host_rh
     return DVM_OK;
 }
 
-int dvm_plan_query(int nx, int ny, int nz, const dvm_vgrid *v, int target_ctas, int max_blocks, int *counts5, int *items9,
+int dvm_plan_query(int nx, int ny, int nz, const dvm_vgrid *v, int target_ctas, int max_blocks, int rv, int *counts5, int *items9,
                    int max_items)
 {
-    if (!v || !counts5 || max_blocks < 0 || nx <= 0 || ny <= 0 || nz <= 0 || v->mx <= 0 || v->my <= 0 || v->mz <= 0 || !v->xi_x || !v->xi_y || !v->xi_z)
+    if (!v || !counts5 || max_blocks < 0 || (rv != 0 && rv != 2 && rv != 4) || nx <= 0 || ny <= 0 || nz <= 0 || v->mx <= 0 || v->my <= 0 || v->mz <= 0 || !v->xi_x || !v->xi_y || !v->xi_z)
         return fail(DVM_EINVAL, "bad argument");
     std::vector<double> xi[3];
     xi[0].assign(v->xi_x, v->xi_x + v->mx); xi[1].assign(v->xi_y, v->xi_y + v->my); xi[2].assign(v->xi_z, v->xi_z + v->mz);
     TilePlan tp;
-    if (tile_plan(nx, ny, nz, xi, target_ctas, max_blocks, &tp)) return fail(DVM_EINVAL, "tile plan failed");
+    if (rv == 0) rv = choose_rv(xi);
+    if (tile_plan(nx, ny, nz, xi, target_ctas, max_blocks, rv, &tp)) return fail(DVM_EINVAL, "tile plan failed");
     counts5[0] = (int)tp.vblocks.size(); counts5[1] = tp.ntx; counts5[2] = tp.nty; counts5[3] = tp.P; counts5[4] = tp.batch;
     const int n = (int)tp.items.size();
     if (items9) {

@@ -6,22 +6,22 @@
 // (Eq.(8)-(9)), and the velocity sums Eq.(5) plus the wall-incident fluxes
 // taken as each value is produced, so that f is never stored.  How it computes it is new:
 //
-//  * work item = (velocity block of 512 velocities of one sign octant) x (4 x 4 z-column of cells); a CTA of 128
-//    threads owns an item, a thread owns 4 velocities (consecutive xi_x nodes) and keeps the 4 x 4 x 4 values of
-//    the current z-plane in registers: x-, y- and z-upwind operands of interior cells are register operands;
+//  * work item = (velocity block of 512 velocities of one sign octant) x (4 x 4 z-column of cells); a CTA owns an
+//    item, a thread owns RV velocities (consecutive xi_x nodes) and keeps their 4 x 4 values of the current z-plane
+//    in registers: x-, y- and z-upwind operands of interior cells are register operands.  Two variants: RV = 4
+//    (128 threads, blocks of 16 x 32 nodes, 8 warps per SM) and RV = 2 (256 threads, blocks of 8 x 64 nodes, 16 warps
+//    per SM);
 //  * what is carried is g = w_alpha f_alpha (the recurrence is linear in f), so quadrature weights cost nothing;
 //  * exp(-|xi-U|^2/T) and the Shakhov polynomial factorise per axis on the tensor velocity grid: tables.cu tabulates
-//    one entry (E, Q, e, a) per (cell, 1-D node) once per iteration; per level the CTA receives the 16 + nbb + ncb
-//    entries of its 16 cells as TMA row copies, together with the cell records (1/tau, cell index, faces);
-//  * the division of Eq.(7) is MUFU.RCP64H + one cubic Newton step (3 DFMA, < 1 ulp);
-//  * the 13 velocity sums use the tensor structure: 4 power sums over the thread's xi_x nodes (4 DFMA / point),
-//    a lane-quad exchange over the 16 xi_x nodes of the block, then each lane expands its share of the 16
-//    (power of xi_x) x (monomial of xi_y, xi_z) products and a transposing butterfly over the 8 lane groups leaves
-//    one partial per lane, which goes to the [cell][16] accumulator in L2/HBM as one coalesced fp64 RED per
-//    (2 cells, warp);
-//  * the 4 rows of a level are a loop with rotating register slots: the level loop must fit the 32 KB instruction
-//    cache (profiles/r01_ifetch_microbench.txt), the fully unrolled level did not;
-//  * the x- and y-faces of the column are the only f-traffic: written with coalesced 32-byte stores per thread,
+//    one entry (E, Q, e, a) per (cell, 1-D node) once per iteration; per level the CTA receives the entries of its
+//    16 cells as TMA row copies, together with the cell records (1/tau, cell index, faces);
+//  * the cell value is written as g = W g_xup + V, so that the recurrence along x is ONE fp64 FMA per value and
+//    everything else (W, V: source term, reciprocal of the denominator by MUFU.RCP64H + one cubic Newton step) is
+//    independent work, done for the RV nodes of a thread in lock step;
+//  * the 13 velocity sums are two small matrix products on the fp64 tensor cores (mma.sync m8n8k4 = SASS DMMA, a
+//    pipe of its own beside the fp64 FMA pipe): powers of xi_x times the values over the lane quad, then monomials
+//    of (xi_y, xi_z) over the 8 pairs of a warp; results go to the [cell][16] accumulator in L2 / HBM as fp64 REDs;
+//  * the x- and y-faces of the column are the only f-traffic: written with ordered 16-byte stores,
 //    read back by the downwind item with TMA bulk copies (cp.async.bulk + mbarrier) two levels ahead;
 //  * items are handed out by an atomic counter in dependency order (tile_plan.cu); done-flags gate their start.
 //
@@ -38,15 +38,12 @@ namespace {
 
 constexpr int NVB = TILE_NVB;
 constexpr int NCELL = TILE_NCELL;
+constexpr int GA = TILE_GA;
 constexpr int XLEVEL_DOUBLES = TILE_TY * NVB;          // one level of an x-face slot
 constexpr int YLEVEL_DOUBLES = TILE_TX * NVB;          // one level of a y-face slot
 constexpr unsigned XLEVEL_BYTES = XLEVEL_DOUBLES * 8u, YLEVEL_BYTES = YLEVEL_DOUBLES * 8u;
-
-constexpr unsigned XROW_BYTES = 4 * TILE_NA * 32u;      // one 4-cell row of x entries
 constexpr unsigned REC_ROW_BYTES = 4 * (unsigned)sizeof(CellRec);
 
-// One tile row (4 cells along x) of one level: everything the row's arithmetic reads sits at a static offset from the
-// row's base address, whatever the row index and the level parity are.
 // One TMA bulk copy per level: source of level 0, byte step per level, destination in a LevelBuf; bytes = 0: skipped.
 struct CopyDesc {
     const unsigned char *src;
@@ -56,9 +53,12 @@ struct CopyDesc {
 };
 constexpr int NCOPY = 4 * TILE_TY + 2;              // per row: x, y, z factor rows and cell records; x-face and y-face input
 
+// One tile row (4 cells along x) of one level: everything the row's arithmetic reads sits at a static offset from the
+// row's base address, whatever the row index and the level parity are.
+template <int RV>
 struct __align__(128) RowBuf {
     // ---- staged by TMA two levels ahead ----
-    double4 xtab[4][TILE_NA];                      // per (cell', xi_x node): E, Q, e, a (slot r*4 + ag); cell' = position of
+    double4 xtab[4][GA * RV];                      // per (cell', xi_x node): E, Q, e, a (slot r*4 + ag); cell' = position of
     double4 ytab[4 * 8];                           // the cell in ascending absolute x;  [cell'][nbb]
     double4 ztab[4 * 8];                           // [cell'][ncb]
     CellRec rec[4];                                // per cell': 1/tau, cell index, neighbour flags, boundary faces
@@ -67,21 +67,21 @@ struct __align__(128) RowBuf {
     double nu[4];                                  // 1/tau (1 for dead cells)
     int code[4];                                   // 1: x-up solid ghost, 2: y-up, 4: z-up, 8: dead cell
     int cidx[4];                                   // row of the [cell][16] accumulator: the cell index, or the CTA's sink row (dead)
-    int pad_[16];
 };
-static_assert(sizeof(RowBuf) % 128 == 0, "rows of the staging buffer must keep the TMA alignment");
 
+template <int RV>
 struct __align__(128) LevelBuf {
-    RowBuf row[TILE_TY];
+    RowBuf<RV> row[TILE_TY];
     double xface[TILE_TY][NVB];                    // x-face input of the level
     double yface[TILE_TX][NVB];                    // y-face input of the level
     double rwb[8];                                 // ghost densities of the domain faces: 4 x-face rows, 4 y-face columns
 };
 
+template <int RV>
 struct __align__(128) TileSmem {
-    LevelBuf lv[2];                                // index = level parity
+    LevelBuf<RV> lv[2];                            // index = level parity
     // ---- per item ----
-    double xi_a[TILE_NA];                          // nodes of the block (0 beyond the box)
+    double xi_a[16];                               // nodes of the block (0 beyond the box)
     double xi_bc[TILE_MAXBC];
     double g[4][3][16];                            // ghost Maxwellian 1-D factors: upwind x, y, z face and solid
     CopyDesc desc[NCOPY];                          // the TMA copies of one level of this item (issue_level)
@@ -176,10 +176,10 @@ __device__ __forceinline__ void dmma(double &c0, double &c1, const double a, con
 }
 
 // Velocity sums of Eq.(5) as two small matrix products per pair of cells (A, B) and warp.
-//   stage 1, once per computed value g (4 per cell and thread): C[p][pair] += X[p][ag] * g[ag][pair], the lane supplying
+//   stage 1, once per computed value g (RV per cell and thread): C[p][pair] += X[p][ag] * g[ag][pair], the lane supplying
 //     its own g as the B fragment (k = its xi_x group ag = lane & 3, n = its (xi_y, xi_z) pair lane >> 2) and xi_x^p of
-//     its own node as the A fragment (p = (lane >> 2) & 3: rows 4..7 repeat rows 0..3).  After the 4 products
-//     C[p][pair] = sum over the 16 xi_x nodes of the block of xi_x^p g, for the warp's 8 pairs.  Cell A and cell B have
+//     its own node as the A fragment (p = (lane >> 2) & 3: rows 4..7 repeat rows 0..3).  After the RV products
+//     C[p][pair] = sum over the xi_x nodes of the block of xi_x^p g, for the warp's 8 pairs.  Cell A and cell B have
 //     an accumulator each; lanes 0..15 (rows 0..3) then keep A's, lanes 16..31 (rows 4..7) B's.
 //   stage 2, once per cell pair: D[row][j] = sum_pair C[row][pair] * M_j(pair), M = {1, y^2, y, z^2, z, yz, y r2, z r2},
 //     r2 = y^2 + z^2.  The C fragment of stage 1 (columns 2q, 2q + 1) is the A fragment of the two k-steps (pairs 0, 2, 4, 6
@@ -240,30 +240,34 @@ __device__ __forceinline__ double rwb_load(const TileParams &P, const ItemCtx &I
     return v;
 }
 
-__device__ __forceinline__ void rwb_store(TileSmem &s, int b, int tid, double v)
+template <int RV>
+__device__ __forceinline__ void rwb_store(TileSmem<RV> &s, int b, int tid, double v)
 {
     if (tid >= 32 && tid < 40) s.lv[b].rwb[tid - 32] = v;
 }
 
 // The TMA copies of a level are described once per item (setup_copies: per 4-cell row the x, y, z factor-table rows and
 // the cell records - tables.cu; every row is one contiguous run of the padded grid - plus the x- and y-face input) and
-// issued per level by thread (q & 3) * 32 + (q >> 2) for copy q (issue_level), so every warp issues at most 5.
-__device__ __forceinline__ int copy_of_thread(int tid) { return (tid & 31) * 4 + (tid >> 5); }
+// issued per level by lane q / WARPS of warp q % WARPS for copy q (issue_level), so the copies are spread over the warps.
+template <int RV>
+__device__ __forceinline__ int copy_of_thread(int tid) { return (tid & 31) * (NVB / RV / 32) + (tid >> 5); }
 
-__device__ __forceinline__ void setup_copies(const TileParams &P, const ItemCtx &I, TileSmem &s, const VBlock &vb, int tid,
+template <int RV>
+__device__ __forceinline__ void setup_copies(const TileParams &P, const ItemCtx &I, TileSmem<RV> &s, const VBlock &vb, int tid,
                                              const double *xsrc, const double *ysrc)
 {
-    const int q = copy_of_thread(tid);
+    constexpr int NA = GA * RV;
+    const int q = copy_of_thread<RV>(tid);
     if (q >= NCOPY) return;
-    const unsigned ybytes = 4u * vb.nbb * 32u, zbytes = 4u * vb.ncb * 32u;
+    const unsigned xbytes = 4u * NA * 32u, ybytes = 4u * vb.nbb * 32u, zbytes = 4u * vb.ncb * 32u;
     CopyDesc d;
     d.pad[0] = d.pad[1] = 0;
     if (q == 4 * TILE_TY) {
         d.src = reinterpret_cast<const unsigned char *>(xsrc); d.step = XLEVEL_BYTES;
-        d.dst = (unsigned)offsetof(LevelBuf, xface); d.bytes = I.first_x ? 0u : XLEVEL_BYTES;
+        d.dst = (unsigned)offsetof(LevelBuf<RV>, xface); d.bytes = I.first_x ? 0u : XLEVEL_BYTES;
     } else if (q == 4 * TILE_TY + 1) {
         d.src = reinterpret_cast<const unsigned char *>(ysrc); d.step = YLEVEL_BYTES;
-        d.dst = (unsigned)offsetof(LevelBuf, yface); d.bytes = I.first_y ? 0u : YLEVEL_BYTES;
+        d.dst = (unsigned)offsetof(LevelBuf<RV>, yface); d.bytes = I.first_y ? 0u : YLEVEL_BYTES;
     } else {
         const int jj = q % TILE_TY, kind = q / TILE_TY;
         // first cell (lowest absolute x) of row jj on the padded grid at level 0; rows may lie in the dead padding
@@ -273,31 +277,32 @@ __device__ __forceinline__ void setup_copies(const TileParams &P, const ItemCtx 
         const int k = I.sz > 0 ? 0 : P.nz - 1;
         const long long npc = (long long)P.nz * P.nyp * P.nxp, lvl = (long long)P.nyp * P.nxp * I.sz;
         const long long pc = ((long long)k * P.nyp + (j + TILE_PAD)) * P.nxp + (i + TILE_PAD);
-        const unsigned rowoff = (unsigned)(offsetof(LevelBuf, row) + jj * sizeof(RowBuf));
+        const unsigned rowoff = (unsigned)(offsetof(LevelBuf<RV>, row) + jj * sizeof(RowBuf<RV>));
         if (kind == 0) {
-            d.src = reinterpret_cast<const unsigned char *>(P.TX + ((long long)vb.xb * npc + pc) * TILE_NA);
-            d.step = lvl * TILE_NA * 32; d.dst = rowoff + (unsigned)offsetof(RowBuf, xtab); d.bytes = XROW_BYTES;
+            d.src = reinterpret_cast<const unsigned char *>(P.TX + ((long long)vb.xb * npc + pc) * NA);
+            d.step = lvl * NA * 32; d.dst = rowoff + (unsigned)offsetof(RowBuf<RV>, xtab); d.bytes = xbytes;
         } else if (kind == 1) {
             d.src = reinterpret_cast<const unsigned char *>(P.TY + ((long long)vb.yb * npc + pc) * vb.nbb);
-            d.step = lvl * vb.nbb * 32; d.dst = rowoff + (unsigned)offsetof(RowBuf, ytab); d.bytes = ybytes;
+            d.step = lvl * vb.nbb * 32; d.dst = rowoff + (unsigned)offsetof(RowBuf<RV>, ytab); d.bytes = ybytes;
         } else if (kind == 2) {
             d.src = reinterpret_cast<const unsigned char *>(P.TZ + ((long long)vb.zb * npc + pc) * vb.ncb);
-            d.step = lvl * vb.ncb * 32; d.dst = rowoff + (unsigned)offsetof(RowBuf, ztab); d.bytes = zbytes;
+            d.step = lvl * vb.ncb * 32; d.dst = rowoff + (unsigned)offsetof(RowBuf<RV>, ztab); d.bytes = zbytes;
         } else {
             d.src = reinterpret_cast<const unsigned char *>(P.rec + pc);
-            d.step = lvl * (long long)sizeof(CellRec); d.dst = rowoff + (unsigned)offsetof(RowBuf, rec); d.bytes = REC_ROW_BYTES;
+            d.step = lvl * (long long)sizeof(CellRec); d.dst = rowoff + (unsigned)offsetof(RowBuf<RV>, rec); d.bytes = REC_ROW_BYTES;
         }
     }
     s.desc[q] = d;
     if (q == 0)
         s.txbytes = (I.first_x ? 0u : XLEVEL_BYTES) + (I.first_y ? 0u : YLEVEL_BYTES) +
-                    (unsigned)TILE_TY * (XROW_BYTES + ybytes + zbytes + REC_ROW_BYTES);
+                    (unsigned)TILE_TY * (xbytes + ybytes + zbytes + REC_ROW_BYTES);
 }
 
 // issue the copies of level kp into buffer kp & 1 (the descriptors were written by the same threads)
-__device__ __forceinline__ void issue_level(TileSmem &s, int kp, int tid)
+template <int RV>
+__device__ __forceinline__ void issue_level(TileSmem<RV> &s, int kp, int tid)
 {
-    const int q = copy_of_thread(tid);
+    const int q = copy_of_thread<RV>(tid);
     if (q >= NCOPY) return;
     const int b = kp & 1;
     if (q == 0) mbar_expect_tx(&s.mbar[b], s.txbytes);
@@ -305,15 +310,18 @@ __device__ __forceinline__ void issue_level(TileSmem &s, int kp, int tid)
     if (d.bytes) tma_load(reinterpret_cast<unsigned char *>(&s.lv[b]) + d.dst, d.src + (long long)kp * d.step, d.bytes, &s.mbar[b]);
 }
 
-// Per-cell records of level kp (buffer b = kp & 1) decoded from the staged CellRec rows by threads 96..111; the caller
-// has waited for the level's TMA copies.  Returns 1 if this thread saw a fluid cell with a solid upwind ghost.
-__device__ __forceinline__ int decode_records(const TileParams &P, const ItemCtx &I, TileSmem &s, int kp, int tid, int sink)
+// Per-cell records of level kp (buffer b = kp & 1) decoded from the staged CellRec rows by the first 16 threads of the
+// last warp; the caller has waited for the level's TMA copies.  Returns 1 if this thread saw a fluid cell with a solid
+// upwind ghost.
+template <int RV>
+__device__ __forceinline__ int decode_records(const TileParams &P, const ItemCtx &I, TileSmem<RV> &s, int kp, int tid, int sink)
 {
+    constexpr int T0 = NVB / RV - 32;
     const int b = kp & 1;
     int special = 0;
-    if (tid >= 96 && tid < 96 + NCELL) {
-        const int cell = tid - 96, ii = cell & 3, jj = cell >> 2;
-        RowBuf &R = s.lv[b].row[jj];
+    if (tid >= T0 && tid < T0 + NCELL) {
+        const int cell = tid - T0, ii = cell & 3, jj = cell >> 2;
+        RowBuf<RV> &R = s.lv[b].row[jj];
         const CellRec &r = R.rec[I.sx > 0 ? ii : 3 - ii];
         const bool dead = r.cidx < 0;
         const int sfl = (r.flags >> 8) & 0xff;
@@ -335,32 +343,34 @@ __device__ __forceinline__ int decode_records(const TileParams &P, const ItemCtx
 }
 
 // Ghost values of the domain faces of level kp (buffer b) for a tile at the upwind x / y edge of the domain
-__device__ __forceinline__ void fill_faces(const ItemCtx &I, TileSmem &s, int b, int tid, int ag, int yidx, int zidx)
+template <int RV>
+__device__ __forceinline__ void fill_faces(const ItemCtx &I, TileSmem<RV> &s, int b, int tid, int ag, int yidx, int zidx)
 {
-    LevelBuf &L = s.lv[b];
+    LevelBuf<RV> &L = s.lv[b];
     if (I.first_x) {
         const double gyz = s.g[0][1][yidx] * s.g[0][2][zidx];
 #pragma unroll
-        for (int r = 0; r < 4; ++r) {
-            const double G = s.g[0][0][4 * ag + r] * gyz;
+        for (int r = 0; r < RV; ++r) {
+            const double G = s.g[0][0][RV * ag + r] * gyz;
 #pragma unroll
-            for (int jj = 0; jj < TILE_TY; ++jj) L.xface[jj][tid * 4 + r] = L.rwb[jj] * G;
+            for (int jj = 0; jj < TILE_TY; ++jj) L.xface[jj][tid * RV + r] = L.rwb[jj] * G;
         }
     }
     if (I.first_y) {
         const double gyz = s.g[1][1][yidx] * s.g[1][2][zidx];
 #pragma unroll
-        for (int r = 0; r < 4; ++r) {
-            const double G = s.g[1][0][4 * ag + r] * gyz;
+        for (int r = 0; r < RV; ++r) {
+            const double G = s.g[1][0][RV * ag + r] * gyz;
 #pragma unroll
-            for (int ii = 0; ii < 4; ++ii) L.yface[ii][tid * 4 + r] = L.rwb[4 + ii] * G;
+            for (int ii = 0; ii < 4; ++ii) L.yface[ii][tid * RV + r] = L.rwb[4 + ii] * G;
         }
     }
 }
 
 // per-thread constants of an item
+template <int RV>
 struct ThreadCtx {
-    double aX[4];                // stage-1 A fragments per node r: xi_x^p, p = (lane >> 2) & 3
+    double aX[RV];               // stage-1 A fragments per node r: xi_x^p, p = (lane >> 2) & 3
     double yz0, yz1;             // stage-2 B fragments: monomial lane >> 2 of the warp's pairs 2 (lane & 3), 2 (lane & 3) + 1
     double *raw0, *raw1;         // raw16 + accumulator slot of the lane's two results
     double use0, use1;           // 1 if the result is one of the products the sums need, else 0 (the RED then adds 0)
@@ -369,16 +379,35 @@ struct ThreadCtx {
     int xrev;                    // 3 if the sweep runs against x (table rows are in ascending absolute x), else 0
 };
 
-__device__ __forceinline__ const double4 &entry(const RowBuf &R, int byte_off)
+template <int RV>
+__device__ __forceinline__ const double4 &entry(const RowBuf<RV> &R, int byte_off)
 {
     return *reinterpret_cast<const double4 *>(reinterpret_cast<const unsigned char *>(&R) + byte_off);
+}
+
+// RV consecutive doubles of a face row (16-byte aligned)
+template <int RV>
+__device__ __forceinline__ void load_face(const double *p, double (&v)[RV])
+{
+#pragma unroll
+    for (int h = 0; h < RV / 2; ++h) {
+        const double2 t = reinterpret_cast<const double2 *>(p)[h];
+        v[2 * h] = t.x; v[2 * h + 1] = t.y;
+    }
+}
+template <int RV>
+__device__ __forceinline__ void store_face(double *p, const double (&v)[RV])
+{
+#pragma unroll
+    for (int h = 0; h < RV / 2; ++h) st_f64x2(p + 2 * h, v[2 * h], v[2 * h + 1]);
 }
 
 // stage 2 for the cell pair (iiA, iiA + 1) of a row and the REDs of its results (lanes 0..15: cell A, 16..31: cell B).
 // No predicates and no branches (the row stays one basic block): a result the sums do not need is multiplied by 0 and
 // added to a slot no other lane of the instruction targets; dead cells carry the CTA's sink row and g = 0.
-__device__ __forceinline__ void emit_pair(const RowBuf &R, const int iiA, const double a0, const double a1, const double b0,
-                                          const double b1, const ThreadCtx &T, const int lane)
+template <int RV>
+__device__ __forceinline__ void emit_pair(const RowBuf<RV> &R, const int iiA, const double a0, const double a1, const double b0,
+                                          const double b1, const ThreadCtx<RV> &T, const int lane)
 {
     const bool hi = lane & 16;
     double d0 = 0.0, d1 = 0.0;
@@ -393,15 +422,12 @@ __device__ __forceinline__ void emit_pair(const RowBuf &R, const int iiA, const 
 // z-plane (the z-upwind operands) and receives the new ones, yup holds the y-upwind operands (the staged y-face for the
 // first row of the tile, else the row just computed).  Dead cells (outside the domain / solid) have all-zero table
 // entries and nu = 1, so they produce g = 0 by the same arithmetic.
-__device__ __forceinline__ void compute_row(const RowBuf &R, const double *xin, double (&zrow)[4][4], const double (&yup)[4][4],
-                                            const ThreadCtx &T, const int tid, const int lane, double *xout, const bool wx)
+template <int RV>
+__device__ __forceinline__ void compute_row(const RowBuf<RV> &R, const double *xin, double (&zrow)[4][RV], const double (&yup)[4][RV],
+                                            const ThreadCtx<RV> &T, const int tid, const int lane, double *xout, const bool wx)
 {
-    double fx[4];
-    {
-        const double2 *p = reinterpret_cast<const double2 *>(xin + tid * 4);
-        const double2 v0 = p[0], v1 = p[1];
-        fx[0] = v0.x; fx[1] = v0.y; fx[2] = v1.x; fx[3] = v1.y;
-    }
+    double fx[RV];
+    load_face<RV>(xin + tid * RV, fx);
     double acc[2][2];
 #pragma unroll
     for (int ii = 0; ii < 4; ++ii) {
@@ -410,98 +436,91 @@ __device__ __forceinline__ void compute_row(const RowBuf &R, const double *xin, 
         const double Eyz = yt.x * zt.x, Qyz = yt.y + zt.y, eyz = yt.z + zt.z;
         const double ay = yt.w, az = zt.w;
         const double dyz = (ay + az) + R.nu[ii];
-        // Everything that does not depend on the x-upwind value, for the 4 nodes of the thread in lock step (dependent
-        // instructions 4 apart: the fp64 pipe takes a warp instruction every 2 clocks and has a latency of ~10): the cell
-        // value is g = W g_xup + V with W = a_x / den and V = (a_y g_yup + a_z g_zup + src) / den, Eq.(7) PAPER.md:75-79.
-        double4 xt[4];
-        double t1[4], t2[4], d[4], y0[4], sE[4], e[4], W[4], V[4];
+        // Everything that does not depend on the x-upwind value, for the RV nodes of the thread in lock step (the fp64
+        // pipe takes a warp instruction every 2 clocks and has a latency of ~10): the cell value is g = W g_xup + V with
+        // W = a_x / den and V = (a_y g_yup + a_z g_zup + src) / den, Eq.(7) PAPER.md:75-79.
+        double4 xt[RV];
+        double t1[RV], t2[RV], d[RV], y0[RV], sE[RV], e[RV], W[RV], V[RV];
 #pragma unroll
-        for (int r = 0; r < 4; ++r) xt[r] = entry(R, T.xo[ii] + r * 4 * 32);
+        for (int r = 0; r < RV; ++r) xt[r] = entry(R, T.xo[ii] + r * GA * 32);
 #pragma unroll
-        for (int r = 0; r < 4; ++r) d[r] = xt[r].w + dyz;
+        for (int r = 0; r < RV; ++r) d[r] = xt[r].w + dyz;
 #pragma unroll
-        for (int r = 0; r < 4; ++r) t1[r] = xt[r].y + Qyz;
+        for (int r = 0; r < RV; ++r) t1[r] = xt[r].y + Qyz;
 #pragma unroll
-        for (int r = 0; r < 4; ++r) asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y0[r]) : "d"(d[r]));
+        for (int r = 0; r < RV; ++r) asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y0[r]) : "d"(d[r]));
 #pragma unroll
-        for (int r = 0; r < 4; ++r) t2[r] = xt[r].z + eyz;
+        for (int r = 0; r < RV; ++r) t2[r] = xt[r].z + eyz;
 #pragma unroll
-        for (int r = 0; r < 4; ++r) sE[r] = xt[r].x * Eyz;
+        for (int r = 0; r < RV; ++r) sE[r] = xt[r].x * Eyz;
 #pragma unroll
-        for (int r = 0; r < 4; ++r) e[r] = fma(-d[r], y0[r], 1.0);
+        for (int r = 0; r < RV; ++r) e[r] = fma(-d[r], y0[r], 1.0);
 #pragma unroll
-        for (int r = 0; r < 4; ++r) t1[r] = fma(t1[r], t2[r], 1.0);
+        for (int r = 0; r < RV; ++r) t1[r] = fma(t1[r], t2[r], 1.0);
 #pragma unroll
-        for (int r = 0; r < 4; ++r) e[r] = fma(e[r], e[r], e[r]);
+        for (int r = 0; r < RV; ++r) e[r] = fma(e[r], e[r], e[r]);
 #pragma unroll
-        for (int r = 0; r < 4; ++r) V[r] = sE[r] * t1[r];
+        for (int r = 0; r < RV; ++r) V[r] = sE[r] * t1[r];
 #pragma unroll
-        for (int r = 0; r < 4; ++r) y0[r] = fma(y0[r], e[r], y0[r]);       // 1 / den (MUFU seed + cubic Newton step)
+        for (int r = 0; r < RV; ++r) y0[r] = fma(y0[r], e[r], y0[r]);       // 1 / den (MUFU seed + cubic Newton step)
 #pragma unroll
-        for (int r = 0; r < 4; ++r) V[r] = fma(ay, yup[ii][r], V[r]);
+        for (int r = 0; r < RV; ++r) V[r] = fma(ay, yup[ii][r], V[r]);
 #pragma unroll
-        for (int r = 0; r < 4; ++r) W[r] = xt[r].w * y0[r];
+        for (int r = 0; r < RV; ++r) W[r] = xt[r].w * y0[r];
 #pragma unroll
-        for (int r = 0; r < 4; ++r) V[r] = fma(az, zrow[ii][r], V[r]);
+        for (int r = 0; r < RV; ++r) V[r] = fma(az, zrow[ii][r], V[r]);
 #pragma unroll
-        for (int r = 0; r < 4; ++r) V[r] *= y0[r];
+        for (int r = 0; r < RV; ++r) V[r] *= y0[r];
         // the recurrence along x: one DFMA per value
 #pragma unroll
-        for (int r = 0; r < 4; ++r) {
+        for (int r = 0; r < RV; ++r) {
             const double gg = fma(W[r], fx[r], V[r]);
             fx[r] = gg;
             zrow[ii][r] = gg;
         }
         acc[ii & 1][0] = 0.0; acc[ii & 1][1] = 0.0;
 #pragma unroll
-        for (int r = 0; r < 4; ++r) dmma(acc[ii & 1][0], acc[ii & 1][1], T.aX[r], zrow[ii][r]);
-        if (ii & 1) emit_pair(R, ii - 1, acc[0][0], acc[0][1], acc[1][0], acc[1][1], T, lane);
+        for (int r = 0; r < RV; ++r) dmma(acc[ii & 1][0], acc[ii & 1][1], T.aX[r], zrow[ii][r]);
+        if (ii & 1) emit_pair<RV>(R, ii - 1, acc[0][0], acc[0][1], acc[1][0], acc[1][1], T, lane);
     }
-    if (wx) {
-        st_f64x2(xout + tid * 4, fx[0], fx[1]);
-        st_f64x2(xout + tid * 4 + 2, fx[2], fx[3]);
-    }
+    if (wx) store_face<RV>(xout + tid * RV, fx);
 }
 
-// One level of the column, fast path (no solid ghost in the level): 4 rows x 4 cells x 4 velocities per thread with the
+// One level of the column, fast path (no solid ghost in the level): 4 rows x 4 cells x RV velocities per thread with the
 // plane in registers (static indices only).  The B200 instruction cache holds 32 KB, and a level loop larger than that is
 // fetch-bound at 1/3 instruction per clock and scheduler (profiles/r01_ifetch_microbench.txt), so how many rows are
 // unrolled is a code-size decision.  DVM_ROW_UNROLL = 4: all rows unrolled, the y-upwind operands of a row are the
 // registers of the row before, no register moves; = 2: a 2-iteration loop over row pairs whose body works on row slots
 // 0, 1 and then swaps them with slots 2, 3; = 1: a 4-iteration loop that works on slot 0 and rotates the slots.
 #ifndef DVM_ROW_UNROLL
-#define DVM_ROW_UNROLL 2
+#define DVM_ROW_UNROLL 4
 #endif
-__device__ __forceinline__ void compute_level(const TileParams &P, const LevelBuf &L, double (&pl)[TILE_TY][4][4],
-                                              const ThreadCtx &T, const int tid, const int lane, double *xout, const bool wx,
-                                              double *yout)
+template <int RV>
+__device__ __forceinline__ void compute_level(const LevelBuf<RV> &L, double (&pl)[TILE_TY][4][RV], const ThreadCtx<RV> &T,
+                                              const int tid, const int lane, double *xout, const bool wx, double *yout)
 {
-    double yu[4][4];
+    double yu[4][RV];
 #pragma unroll
-    for (int ii = 0; ii < 4; ++ii) {
-        const double2 *p = reinterpret_cast<const double2 *>(&L.yface[ii][tid * 4]);
-        const double2 v0 = p[0], v1 = p[1];
-        yu[ii][0] = v0.x; yu[ii][1] = v0.y; yu[ii][2] = v1.x; yu[ii][3] = v1.y;
-    }
+    for (int ii = 0; ii < 4; ++ii) load_face<RV>(&L.yface[ii][tid * RV], yu[ii]);
 #if DVM_ROW_UNROLL == 4
-    compute_row(L.row[0], L.xface[0], pl[0], yu, T, tid, lane, xout, wx);
+    compute_row<RV>(L.row[0], L.xface[0], pl[0], yu, T, tid, lane, xout, wx);
 #pragma unroll
-    for (int jj = 1; jj < TILE_TY; ++jj) compute_row(L.row[jj], L.xface[jj], pl[jj], pl[jj - 1], T, tid, lane, xout + jj * NVB, wx);
+    for (int jj = 1; jj < TILE_TY; ++jj) compute_row<RV>(L.row[jj], L.xface[jj], pl[jj], pl[jj - 1], T, tid, lane, xout + jj * NVB, wx);
 #elif DVM_ROW_UNROLL == 2
     static_assert(TILE_TY == 4, "row pairs");
-    const RowBuf *R = &L.row[0];
+    const RowBuf<RV> *R = &L.row[0];
     const double *xin = &L.xface[0][0];
 #pragma unroll 1
     for (int h = 0; h < 2; ++h) {
-        compute_row(R[0], xin, pl[0], yu, T, tid, lane, xout, wx);
-        compute_row(R[1], xin + NVB, pl[1], pl[0], T, tid, lane, xout + NVB, wx);
+        compute_row<RV>(R[0], xin, pl[0], yu, T, tid, lane, xout, wx);
+        compute_row<RV>(R[1], xin + NVB, pl[1], pl[0], T, tid, lane, xout + NVB, wx);
         R += 2;
         xin += 2 * NVB;
         xout += 2 * NVB;
 #pragma unroll
         for (int ii = 0; ii < 4; ++ii)
 #pragma unroll
-            for (int r = 0; r < 4; ++r) {
+            for (int r = 0; r < RV; ++r) {
                 const double t0 = pl[0][ii][r], t1 = pl[1][ii][r];
                 yu[ii][r] = t1;
                 pl[0][ii][r] = pl[2][ii][r]; pl[1][ii][r] = pl[3][ii][r];
@@ -509,11 +528,11 @@ __device__ __forceinline__ void compute_level(const TileParams &P, const LevelBu
             }
     }
 #else
-    const RowBuf *R = &L.row[0];
+    const RowBuf<RV> *R = &L.row[0];
     const double *xin = &L.xface[0][0];
 #pragma unroll 1
     for (int jj = 0; jj < TILE_TY; ++jj) {
-        compute_row(*R, xin, pl[0], yu, T, tid, lane, xout, wx);
+        compute_row<RV>(*R, xin, pl[0], yu, T, tid, lane, xout, wx);
         ++R;
         xin += NVB;
         xout += NVB;
@@ -521,7 +540,7 @@ __device__ __forceinline__ void compute_level(const TileParams &P, const LevelBu
 #pragma unroll
         for (int ii = 0; ii < 4; ++ii)
 #pragma unroll
-            for (int r = 0; r < 4; ++r) {
+            for (int r = 0; r < RV; ++r) {
                 const double t = pl[0][ii][r];
                 yu[ii][r] = t;
 #pragma unroll
@@ -532,28 +551,25 @@ __device__ __forceinline__ void compute_level(const TileParams &P, const LevelBu
 #endif
     if (yout) {
 #pragma unroll
-        for (int ii = 0; ii < 4; ++ii) {
-            st_f64x2(yout + ii * NVB + tid * 4, pl[TILE_TY - 1][ii][0], pl[TILE_TY - 1][ii][1]);
-            st_f64x2(yout + ii * NVB + tid * 4 + 2, pl[TILE_TY - 1][ii][2], pl[TILE_TY - 1][ii][3]);
-        }
+        for (int ii = 0; ii < 4; ++ii) store_face<RV>(yout + ii * NVB + tid * RV, pl[TILE_TY - 1][ii]);
     }
 }
 
 // One level that holds a solid ghost (a fluid cell whose upwind neighbour is a masked cell): the same arithmetic
 // written as compact loops over a copy of the plane in local memory.  Rare (the surface of a masked body), so its
 // speed does not matter; keeping it out of the unrolled path halves the code the instruction cache has to hold.
-__device__ __forceinline__ void compute_level_slow(const TileParams &P, TileSmem &s, const LevelBuf &L, double *pl,
-                                                   const ThreadCtx &T, const int tid, const int lane, double *xout,
-                                                   double *yout)
+template <int RV>
+__device__ __forceinline__ void compute_level_slow(TileSmem<RV> &s, const LevelBuf<RV> &L, double *pl, const ThreadCtx<RV> &T,
+                                                   const int tid, const int lane, double *xout, double *yout)
 {
     const double gyz = s.g[3][1][T.yi] * s.g[3][2][T.zi];
 #pragma unroll 1
     for (int jj = 0; jj < TILE_TY; ++jj) {
-        const RowBuf &R = L.row[jj];
-        double fx[4];
+        const RowBuf<RV> &R = L.row[jj];
+        double fx[RV];
 #pragma unroll
-        for (int r = 0; r < 4; ++r) fx[r] = L.xface[jj][tid * 4 + r];
-        double acc[2][2] = {{0.0, 0.0}, {0.0, 0.0}};
+        for (int r = 0; r < RV; ++r) fx[r] = L.xface[jj][tid * RV + r];
+        double accA0 = 0.0, accA1 = 0.0;
 #pragma unroll 1
         for (int ii = 0; ii < 4; ++ii) {
             const int cell = jj * 4 + ii;
@@ -569,11 +585,11 @@ __device__ __forceinline__ void compute_level_slow(const TileParams &P, TileSmem
             const double4 sp = R.spec[ii];
             double c0 = 0.0, c1 = 0.0;
 #pragma unroll
-            for (int r = 0; r < 4; ++r) {
-                const double Pg = s.g[3][0][4 * T.ag + r] * gyz;
-                const double4 xt = entry(R, xo + r * 4 * 32);
-                double xu = fx[r], zu = pl[cell * 4 + r];
-                double yu = jj == 0 ? L.yface[ii][tid * 4 + r] : pl[(cell - 4) * 4 + r];
+            for (int r = 0; r < RV; ++r) {
+                const double Pg = s.g[3][0][RV * T.ag + r] * gyz;
+                const double4 xt = entry(R, xo + r * GA * 32);
+                double xu = fx[r], zu = pl[cell * RV + r];
+                double yu = jj == 0 ? L.yface[ii][tid * RV + r] : pl[(cell - 4) * RV + r];
                 if (code & 1) xu = sp.x * Pg;
                 if (code & 2) yu = sp.y * Pg;
                 if (code & 4) zu = sp.z * Pg;
@@ -585,34 +601,36 @@ __device__ __forceinline__ void compute_level_slow(const TileParams &P, TileSmem
                 double gg = num * inv;
                 if (code & 8) gg = 0.0;
                 fx[r] = gg;
-                pl[cell * 4 + r] = gg;
+                pl[cell * RV + r] = gg;
                 dmma(c0, c1, T.aX[r], gg);
             }
             if (ii & 1) {
-                emit_pair(R, ii - 1, acc[0][0], acc[0][1], c0, c1, T, lane);
+                emit_pair<RV>(R, ii - 1, accA0, accA1, c0, c1, T, lane);
             } else {
-                acc[0][0] = c0; acc[0][1] = c1;
+                accA0 = c0; accA1 = c1;
             }
         }
         if (xout) {
 #pragma unroll
-            for (int r = 0; r < 4; ++r) xout[jj * NVB + tid * 4 + r] = fx[r];
+            for (int r = 0; r < RV; ++r) xout[jj * NVB + tid * RV + r] = fx[r];
         }
     }
     if (yout) {
 #pragma unroll 1
         for (int ii = 0; ii < 4; ++ii)
 #pragma unroll
-            for (int r = 0; r < 4; ++r) yout[ii * NVB + tid * 4 + r] = pl[((TILE_TY - 1) * 4 + ii) * 4 + r];
+            for (int r = 0; r < RV; ++r) yout[ii * NVB + tid * RV + r] = pl[((TILE_TY - 1) * 4 + ii) * RV + r];
     }
 }
 
-__global__ void __launch_bounds__(TILE_THREADS, TILE_MIN_CTAS) sweep_tile_kernel(const TileParams P)
+template <int RV>
+__global__ void __launch_bounds__(NVB / RV, 2) sweep_tile_kernel(const TileParams P)
 {
+    constexpr int THREADS = NVB / RV, NA = GA * RV;
     // dynamic shared memory starts at offset 0 of the CTA's window (no static __shared__ in this kernel), so the
     // 128-byte alignment holds; casting without pointer arithmetic keeps the address space visible (LDS / STS)
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    TileSmem &s = *reinterpret_cast<TileSmem *>(smem_raw);
+    TileSmem<RV> &s = *reinterpret_cast<TileSmem<RV> *>(smem_raw);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     if (tid == 0) {
         mbar_init(&s.mbar[0], 1);
@@ -656,11 +674,11 @@ __global__ void __launch_bounds__(TILE_THREADS, TILE_MIN_CTAS) sweep_tile_kernel
 
         // ---- TMA copies of levels 0 and 1 (the staging buffers are free: every thread passed the end-of-item
         //      barrier; the upwind items' face stores were made with the generic proxy) ----
-        setup_copies(P, I, s, vb, tid, xdst, ydst);
-        if (copy_of_thread(tid) < NCOPY) {
+        setup_copies<RV>(P, I, s, vb, tid, xdst, ydst);
+        if (copy_of_thread<RV>(tid) < NCOPY) {
             fence_proxy_async_global();
-            issue_level(s, 0, tid);
-            if (P.nz > 1) issue_level(s, 1, tid);
+            issue_level<RV>(s, 0, tid);
+            if (P.nz > 1) issue_level<RV>(s, 1, tid);
         }
         // ---- per-item tables: nodes, ghost factors; ghost densities of the domain faces of levels 0 and 1 ----
         {
@@ -687,12 +705,12 @@ __global__ void __launch_bounds__(TILE_THREADS, TILE_MIN_CTAS) sweep_tile_kernel
                 for (int f = 0; f < 4; ++f)
                     s.g[f][2][vb.nbb + cl] = ok ? P.gtab[(long long)(slotid[f] * 3 + 2) * P.gstride + idx] : 0.0;
             }
-            rwb_store(s, 0, tid, rwb_load(P, I, 0, tid));
-            rwb_store(s, 1, tid, rwb_load(P, I, 1, tid));
+            rwb_store<RV>(s, 0, tid, rwb_load(P, I, 0, tid));
+            rwb_store<RV>(s, 1, tid, rwb_load(P, I, 1, tid));
         }
         __syncthreads();
 
-        ThreadCtx T;
+        ThreadCtx<RV> T;
         T.ag = lane & 3;
         T.xrev = vb.sx > 0 ? 0 : 3;
         {
@@ -704,15 +722,15 @@ __global__ void __launch_bounds__(TILE_THREADS, TILE_MIN_CTAS) sweep_tile_kernel
 #pragma unroll
             for (int ii = 0; ii < 4; ++ii) {
                 const int cp = ii ^ T.xrev;
-                T.xo[ii] = (int)offsetof(RowBuf, xtab) + (cp * TILE_NA + T.ag) * 32;
-                T.yo[ii] = (int)offsetof(RowBuf, ytab) + (cp * vb.nbb + yl) * 32;
-                T.zo[ii] = (int)offsetof(RowBuf, ztab) + (cp * vb.ncb + zl) * 32;
+                T.xo[ii] = (int)offsetof(RowBuf<RV>, xtab) + (cp * NA + T.ag) * 32;
+                T.yo[ii] = (int)offsetof(RowBuf<RV>, ytab) + (cp * vb.nbb + yl) * 32;
+                T.zo[ii] = (int)offsetof(RowBuf<RV>, ztab) + (cp * vb.ncb + zl) * 32;
             }
             // stage-1 A fragments: xi_x^p of the thread's own nodes, p = (lane >> 2) & 3
             const int row = lane >> 2, pw = row & 3;
 #pragma unroll
-            for (int r = 0; r < 4; ++r) {
-                const double x = s.xi_a[4 * T.ag + r];
+            for (int r = 0; r < RV; ++r) {
+                const double x = s.xi_a[RV * T.ag + r];
                 T.aX[r] = pw == 0 ? 1.0 : pw == 1 ? x : pw == 2 ? x * x : x * x * x;
             }
             // stage-2 B fragments: monomial j = lane >> 2 of the (xi_y, xi_z) nodes of pairs 2q and 2q + 1 of this warp
@@ -739,20 +757,23 @@ __global__ void __launch_bounds__(TILE_THREADS, TILE_MIN_CTAS) sweep_tile_kernel
             T.use0 = u0 ? 1.0 : 0.0; T.use1 = u1 ? 1.0 : 0.0;
         }
 
-        // records and boundary faces of level 0 (its copies were issued above; the wait does not consume the phase)
+        // Records and boundary faces of level 0.  Only the 16 decoding threads wait on the mbarrier of a level's copies
+        // (a try_wait round trip costs several hundred clocks); they do so one level ahead, and the CTA barrier that
+        // follows hands their observation of the completed copies on to every other thread.
         int special = 0;
-        if (tid >= 96 && tid < 96 + NCELL) {
+        if (tid >= THREADS - 32 && tid < THREADS - 32 + NCELL) {
             mbar_wait(&s.mbar[0], par[0]);
-            special = decode_records(P, I, s, 0, tid, sink);
+            par[0] ^= 1u;
+            special = decode_records<RV>(P, I, s, 0, tid, sink);
         }
-        fill_faces(I, s, 0, tid, T.ag, T.yi, T.zi);
+        fill_faces<RV>(I, s, 0, tid, T.ag, T.yi, T.zi);
         // plane = ghost of the upwind z face of the domain
-        double pl[TILE_TY][4][4];
+        double pl[TILE_TY][4][RV];
         {
             const double gyz = s.g[2][1][T.yi] * s.g[2][2][T.zi];
-            double G[4];
+            double G[RV];
 #pragma unroll
-            for (int r = 0; r < 4; ++r) G[r] = s.g[2][0][4 * T.ag + r] * gyz;
+            for (int r = 0; r < RV; ++r) G[r] = s.g[2][0][RV * T.ag + r] * gyz;
 #pragma unroll
             for (int jj = 0; jj < TILE_TY; ++jj)
 #pragma unroll
@@ -761,7 +782,7 @@ __global__ void __launch_bounds__(TILE_THREADS, TILE_MIN_CTAS) sweep_tile_kernel
                     double rw = 0.0;
                     if (cell_of(P, I, ii, jj, 0, i, j, k)) rw = face_density(P, I.tpz, P.foff[I.upz] + j * P.nx + i);
 #pragma unroll
-                    for (int r = 0; r < 4; ++r) pl[jj][ii][r] = rw * G[r];
+                    for (int r = 0; r < RV; ++r) pl[jj][ii][r] = rw * G[r];
                 }
         }
         special = __shfl_sync(0xffffffffu, __syncthreads_or(special), 0);
@@ -771,37 +792,36 @@ __global__ void __launch_bounds__(TILE_THREADS, TILE_MIN_CTAS) sweep_tile_kernel
         for (int kp = 0; kp < P.nz; ++kp) {
             const int b = kp & 1;
             const double vrw = rwb_load(P, I, kp + 2, tid);
-            mbar_wait(&s.mbar[b], par[b]);
-            par[b] ^= 1u;
             double *xout = write_x ? xdst + (long long)kp * XLEVEL_DOUBLES : nullptr;
             double *yout = write_y ? ydst + (long long)kp * YLEVEL_DOUBLES : nullptr;
             if (special) {
-                double tmp[NCELL * 4];
+                double tmp[NCELL * RV];
 #pragma unroll
                 for (int c = 0; c < NCELL; ++c)
 #pragma unroll
-                    for (int r = 0; r < 4; ++r) tmp[c * 4 + r] = pl[c >> 2][c & 3][r];
-                compute_level_slow(P, s, s.lv[b], tmp, T, tid, lane, xout, yout);
+                    for (int r = 0; r < RV; ++r) tmp[c * RV + r] = pl[c >> 2][c & 3][r];
+                compute_level_slow<RV>(s, s.lv[b], tmp, T, tid, lane, xout, yout);
 #pragma unroll
                 for (int c = 0; c < NCELL; ++c)
 #pragma unroll
-                    for (int r = 0; r < 4; ++r) pl[c >> 2][c & 3][r] = tmp[c * 4 + r];
+                    for (int r = 0; r < RV; ++r) pl[c >> 2][c & 3][r] = tmp[c * RV + r];
             } else {
-                compute_level(P, s.lv[b], pl, T, tid, lane, xdst + (long long)kp * XLEVEL_DOUBLES, write_x, yout);
+                compute_level<RV>(s.lv[b], pl, T, tid, lane, xdst + (long long)kp * XLEVEL_DOUBLES, write_x, yout);
             }
-            rwb_store(s, b, tid, vrw);
+            rwb_store<RV>(s, b, tid, vrw);
             int sp = 0;
             if (kp + 1 < P.nz) {
-                if (tid >= 96 && tid < 96 + NCELL) {
+                if (tid >= THREADS - 32 && tid < THREADS - 32 + NCELL) {
                     mbar_wait(&s.mbar[b ^ 1], par[b ^ 1]);   // level kp + 1 has landed (issued a level ago)
-                    sp = decode_records(P, I, s, kp + 1, tid, sink);
+                    par[b ^ 1] ^= 1u;
+                    sp = decode_records<RV>(P, I, s, kp + 1, tid, sink);
                 }
-                fill_faces(I, s, b ^ 1, tid, T.ag, T.yi, T.zi);
+                fill_faces<RV>(I, s, b ^ 1, tid, T.ag, T.yi, T.zi);
             }
             special = __shfl_sync(0xffffffffu, __syncthreads_or(sp), 0);
-            if (copy_of_thread(tid) < NCOPY && kp + 2 < P.nz) {
+            if (copy_of_thread<RV>(tid) < NCOPY && kp + 2 < P.nz) {
                 fence_proxy_async_smem();  // this level's reads of the staging buffers before the TMA overwrites them
-                issue_level(s, kp + 2, tid);
+                issue_level<RV>(s, kp + 2, tid);
             }
         }
         // ---- publish: faces of this item are complete ----
@@ -812,20 +832,24 @@ __global__ void __launch_bounds__(TILE_THREADS, TILE_MIN_CTAS) sweep_tile_kernel
     }
 }
 
-}  // namespace
-
-size_t tile_smem_bytes() { return sizeof(TileSmem); }
-
-cudaError_t tile_configure(int *ctas_per_sm)
+template <int RV>
+cudaError_t configure(int *ctas_per_sm)
 {
-    cudaError_t e = cudaFuncSetAttribute(sweep_tile_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tile_smem_bytes());
+    cudaError_t e = cudaFuncSetAttribute(sweep_tile_kernel<RV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(TileSmem<RV>));
     if (e != cudaSuccess) return e;
-    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, sweep_tile_kernel, TILE_THREADS, tile_smem_bytes());
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, sweep_tile_kernel<RV>, NVB / RV, sizeof(TileSmem<RV>));
 }
 
-cudaError_t launch_sweep_tile(const TileParams &P, int grid, cudaStream_t st)
+}  // namespace
+
+size_t tile_smem_bytes(int rv) { return rv == 2 ? sizeof(TileSmem<2>) : sizeof(TileSmem<4>); }
+
+cudaError_t tile_configure(int rv, int *ctas_per_sm) { return rv == 2 ? configure<2>(ctas_per_sm) : configure<4>(ctas_per_sm); }
+
+cudaError_t launch_sweep_tile(const TileParams &P, int rv, int grid, cudaStream_t st)
 {
-    sweep_tile_kernel<<<grid, TILE_THREADS, tile_smem_bytes(), st>>>(P);
+    if (rv == 2) sweep_tile_kernel<2><<<grid, NVB / 2, sizeof(TileSmem<2>), st>>>(P);
+    else sweep_tile_kernel<4><<<grid, NVB / 4, sizeof(TileSmem<4>), st>>>(P);
     return cudaGetLastError();
 }
 

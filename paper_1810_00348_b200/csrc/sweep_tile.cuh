@@ -2,15 +2,17 @@
 //
 // DVM_KERNEL_TILE in one paragraph: the sweep of Eq.(7) is cut into
 // work items (velocity block V, z-column tile (I', J')).  A velocity block is 512 discrete velocities of one
-// sign octant (a box 16 x nbb x ncb of node indices); a column tile is TX x TY = 4 x 4 cells wide and spans
-// all nz levels.  One CTA of 128 threads owns an item: every thread carries 4 velocities (consecutive xi_x
-// nodes, same xi_y, xi_z) and keeps their 4 x 4 x 4 values of the current z-plane of the tile in REGISTERS, so the
+// sign octant (a box NA x nbb x ncb of node indices); a column tile is TX x TY = 4 x 4 cells wide and spans
+// all nz levels.  One CTA owns an item: every thread carries RV velocities (consecutive xi_x nodes, same xi_y, xi_z)
+// and keeps their 4 x 4 values of the current z-plane of the tile in REGISTERS, so the
 // z-upwind and y-upwind operands never leave the register file; only the x- and y-faces of the column go to HBM
 // (8 B per phase point instead of the 16 B of an in-place slice, 32 B in the paper's two-slice form,
 // PAPER.md:104-106, 233-235).  Items are handed out by an atomic counter in an order that respects the upwind
 // dependencies (x-face of (I'-1, J'), y-face of (I', J'-1)); done-flags in global memory gate the start of an item.
 // The equilibrium enters through 1-D factor tables (tables.cu) staged by TMA with the faces; velocity blocks may
 // sweep in batches that share face-slot sets when the f workspace is capped (DVM_OPT_MAX_F_MBYTES).
+// Two variants of the kernel (DVM_OPT_TILE_RV): RV = 4: CTAs of 128 threads, blocks of 16 x 32 nodes (nbb x ncb = 8 x 4
+// or 4 x 8); RV = 2: CTAs of 256 threads, blocks of 8 x 8 x 8 nodes, twice the warps per SM.
 #pragma once
 #include <cuda_runtime.h>
 #include <vector>
@@ -22,18 +24,15 @@ constexpr int TILE_TX = 4;                 // cells per tile along the sweep-rel
 #ifndef DVM_TILE_TY
 #define DVM_TILE_TY 4
 #endif
-constexpr int TILE_TY = DVM_TILE_TY;        // cells per tile along the sweep-relative y (4, or 2: 3 CTAs per SM)
-constexpr int TILE_MIN_CTAS = TILE_TY <= 2 ? 3 : 2;   // resident CTAs per SM the kernel is compiled for
+constexpr int TILE_TY = DVM_TILE_TY;        // cells per tile along the sweep-relative y
 constexpr int TILE_NCELL = TILE_TX * TILE_TY;
-constexpr int TILE_RV = 4;                 // velocities per thread (consecutive xi_x nodes)
 constexpr int TILE_GA = 4;                 // xi_x groups per lane quad
-constexpr int TILE_NA = TILE_RV * TILE_GA; // xi_x nodes per velocity block
-constexpr int TILE_THREADS = 128;
-constexpr int TILE_WARPS = TILE_THREADS / 32;
-constexpr int TILE_NVB = TILE_THREADS * TILE_RV;  // velocities per block (incl. padding)
-constexpr int TILE_NPAIR = TILE_THREADS / TILE_GA; // (xi_y, xi_z) pairs per block
-constexpr int TILE_MAXBC = 12;             // nbb + ncb of a block
+constexpr int TILE_NVB = 512;              // velocities per block (incl. padding) = threads x RV
+constexpr int TILE_MAXBC = 16;             // nbb + ncb of a block
 constexpr int TILE_PAD = 4;                // dead cells around the grid in the factor tables (tiles may overhang by 3)
+inline int tile_threads(int rv) { return TILE_NVB / rv; }
+inline int tile_na(int rv) { return TILE_GA * rv; }          // xi_x nodes per velocity block
+inline int tile_npair(int rv) { return TILE_NVB / rv / TILE_GA; }   // (xi_y, xi_z) pairs per block = nbb * ncb
 
 // per-cell record of the padded grid, fetched by TMA with the factor tables (48 bytes)
 struct CellRec {
@@ -45,8 +44,8 @@ struct CellRec {
 };
 static_assert(sizeof(CellRec) == 48, "CellRec rows must be 16-byte aligned");
 
-// velocity block: node-index box [a0, a0+na) x [b0, b0+nb) x [c0, c0+nc), na <= 16, nb <= nbb, nc <= ncb,
-// nbb * ncb = 32; lanes beyond the box carry weight 0
+// velocity block: node-index box [a0, a0+na) x [b0, b0+nb) x [c0, c0+nc), na <= NA, nb <= nbb, nc <= ncb,
+// nbb * ncb = pairs per block; lanes beyond the box carry weight 0
 struct VBlock {
     int a0, na, b0, nb, c0, nc;
     int nbb, ncb;
@@ -68,10 +67,11 @@ struct TileItem {
 
 struct TilePlan {
     int ntx = 0, nty = 0, P = 1;
+    int rv = 4;                        // velocities per thread of the kernel variant this plan is for
     int batch = 0;                     // velocity blocks in flight at once (= face-slot sets)
     int nbb = 8, ncb = 4;              // one (xi_y, xi_z) block shape for the whole problem
-    std::vector<int> xnode, ynode, znode;   // node index per 1-D block slot (-1 = padding): [nxb][16], [nyb][nbb], [nzb][ncb];
-                                            // xnode is in table order: slot r*4 + ag holds node 4*ag + r of the block
+    std::vector<int> xnode, ynode, znode;   // node index per 1-D block slot (-1 = padding): [nxb][NA], [nyb][nbb], [nzb][ncb];
+                                            // xnode is in table order: slot r*4 + ag holds node RV*ag + r of the block
     std::vector<VBlock> vblocks;
     std::vector<TileItem> items;
     size_t xface_doubles = 0, yface_doubles = 0;
@@ -103,13 +103,13 @@ struct TileParams {
     double *xface, *yface;
     long long xslot_doubles, yslot_doubles;   // nz * TILE_TY * TILE_NVB, nz * TILE_TX * TILE_NVB
     // factor tables of step n (tables_kernel), padded grid nxp x nyp x nz, entries double4 (E, Q, e, a):
-    const double4 *TX, *TY, *TZ;  // [nxb][nz][nyp][nxp][16], [nyb][nz][nyp][nxp][nbb], [nzb][nz][nyp][nxp][ncb]
+    const double4 *TX, *TY, *TZ;  // [nxb][nz][nyp][nxp][NA], [nyb][nz][nyp][nxp][nbb], [nzb][nz][nyp][nxp][ncb]
     const CellRec *rec;           // [nz][nyp][nxp]
     int nxp, nyp, nbb, ncb;
 };
 
 struct TableParams {
-    int nx, ny, nz, nxp, nyp, nbb, ncb, nxb, nyb, nzb;
+    int nx, ny, nz, nxp, nyp, na, nbb, ncb, nxb, nyb, nzb;
     long long ncell;
     const double *coef;           // [NCOEF][ncell]
     const unsigned char *flags;   // bit 6: solid
@@ -125,11 +125,11 @@ struct TableParams {
 // items that should be able to run concurrently (sets the band height P); max_blocks > 0 caps the velocity blocks in
 // flight at once (batches).  Pure host code (tests call it through
 // dvm_plan_query without a GPU).
-int tile_plan(int nx, int ny, int nz, const std::vector<double> xi[3], int target_ctas, int max_blocks, TilePlan *plan);
+int tile_plan(int nx, int ny, int nz, const std::vector<double> xi[3], int target_ctas, int max_blocks, int rv, TilePlan *plan);
 
-size_t tile_smem_bytes();
-cudaError_t tile_configure(int *ctas_per_sm);
-cudaError_t launch_sweep_tile(const TileParams &P, int grid, cudaStream_t st);
+size_t tile_smem_bytes(int rv);
+cudaError_t tile_configure(int rv, int *ctas_per_sm);
+cudaError_t launch_sweep_tile(const TileParams &P, int rv, int grid, cudaStream_t st);
 cudaError_t launch_tables(const TableParams &T, cudaStream_t st);
 
 }  // namespace dvm

@@ -13,7 +13,7 @@ namespace dvm {
 
 __global__ void __launch_bounds__(256) tables_kernel(const TableParams T)
 {
-    const int sx = T.nxb * TILE_NA, sy = T.nyb * T.nbb, sz = T.nzb * T.ncb;
+    const int sx = T.nxb * T.na, sy = T.nyb * T.nbb, sz = T.nzb * T.ncb;
     const long long nslot = sx + sy + sz;
     const long long npc = (long long)T.nz * T.nyp * T.nxp;   // padded cells
     const long long n = T.ncell;
@@ -25,7 +25,7 @@ __global__ void __launch_bounds__(256) tables_kernel(const TableParams T)
         const long long pc = ((long long)k * T.nyp + (j + TILE_PAD)) * T.nxp + (i + TILE_PAD);
         int d, m, pos, width, blk;
         double4 *dst;
-        if (sl < sx) { d = 0; width = TILE_NA; blk = sl / width; pos = sl - blk * width; m = T.xnode[sl]; dst = T.TX; }
+        if (sl < sx) { d = 0; width = T.na; blk = sl / width; pos = sl - blk * width; m = T.xnode[sl]; dst = T.TX; }
         else if (sl < sx + sy) { d = 1; width = T.nbb; const int t = sl - sx; blk = t / width; pos = t - blk * width; m = T.ynode[t]; dst = T.TY; }
         else { d = 2; width = T.ncb; const int t = sl - sx - sy; blk = t / width; pos = t - blk * width; m = T.znode[t]; dst = T.TZ; }
         const bool solid = T.flags[c] & FLAG_SOLID;
@@ -54,7 +54,7 @@ __global__ void __launch_bounds__(256) tables_kernel(const TableParams T)
 
 cudaError_t launch_tables(const TableParams &T, cudaStream_t st)
 {
-    const long long work = T.ncell * ((long long)T.nxb * TILE_NA + (long long)T.nyb * T.nbb + (long long)T.nzb * T.ncb);
+    const long long work = T.ncell * ((long long)T.nxb * T.na + (long long)T.nyb * T.nbb + (long long)T.nzb * T.ncb);
     const long long blocks = (work + 255) / 256;
     const int grid = (int)(blocks < 148LL * 32 ? blocks : 148LL * 32);
     tables_kernel<<<grid, 256, 0, st>>>(T);

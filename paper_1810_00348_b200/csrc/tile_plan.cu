@@ -27,21 +27,23 @@ int ceil_div(int a, int b) { return (a + b - 1) / b; }
 
 }  // namespace
 
-int tile_plan(int nx, int ny, int nz, const std::vector<double> xi[3], int target_ctas, int max_blocks, TilePlan *plan)
+int tile_plan(int nx, int ny, int nz, const std::vector<double> xi[3], int target_ctas, int max_blocks, int rv, TilePlan *plan)
 {
-    if (nx <= 0 || ny <= 0 || nz <= 0 || !plan) return -1;
+    if (nx <= 0 || ny <= 0 || nz <= 0 || !plan || (rv != 2 && rv != 4)) return -1;
+    const int NA = tile_na(rv);
+    plan->rv = rv;
     plan->vblocks.clear();
     plan->items.clear();
     int lo[3][2], cnt[3][2];
     for (int d = 0; d < 3; ++d) split_axis(xi[d], lo[d], cnt[d]);
 
-    // ---- (nbb, ncb) with nbb * ncb = 32 and nbb + ncb <= TILE_MAXBC: one shape for the whole problem (the factor
-    //      tables are laid out by 1-D block), the one wasting the fewest lanes ----
-    int best_bb = 8, best_cb = 4;
+    // ---- (nbb, ncb) with nbb * ncb = pairs per block and nbb + ncb <= TILE_MAXBC: one shape for the whole problem (the
+    //      factor tables are laid out by 1-D block), the one wasting the fewest lanes ----
+    int best_bb = 8, best_cb = rv == 2 ? 8 : 4;
     {
         long best = -1;
-        const int shapes[2][2] = {{8, 4}, {4, 8}};
-        for (auto &s : shapes) {
+        const int shapes4[2][2] = {{8, 4}, {4, 8}}, shapes2[2][2] = {{8, 8}, {8, 8}};
+        for (auto &s : (rv == 2 ? shapes2 : shapes4)) {
             long slots = 0;
             for (int oz = 0; oz < 2; ++oz) for (int oy = 0; oy < 2; ++oy)
                 slots += (long)ceil_div(cnt[1][oy], s[0]) * ceil_div(cnt[2][oz], s[1]);
@@ -51,7 +53,7 @@ int tile_plan(int nx, int ny, int nz, const std::vector<double> xi[3], int targe
     plan->nbb = best_bb; plan->ncb = best_cb;
     // ---- 1-D blocks per axis and sign half; first block id of each half ----
     int first[3][2];
-    const int width[3] = {TILE_NA, best_bb, best_cb};
+    const int width[3] = {NA, best_bb, best_cb};
     std::vector<int> *nodes[3] = {&plan->xnode, &plan->ynode, &plan->znode};
     for (int d = 0; d < 3; ++d) {
         nodes[d]->clear();
@@ -60,25 +62,25 @@ int tile_plan(int nx, int ny, int nz, const std::vector<double> xi[3], int targe
             first[d][h] = nblk;
             for (int k0 = 0; k0 < cnt[d][h]; k0 += width[d], ++nblk)
                 for (int sl = 0; sl < width[d]; ++sl) {
-                    // x: table slot r*4 + ag holds node 4*ag + r of the block (conflict-free reads, sweep_tile.cu)
-                    const int local = d == 0 ? 4 * (sl & 3) + (sl >> 2) : sl;
+                    // x: table slot r*4 + ag holds node RV*ag + r of the block (conflict-free reads, sweep_tile.cu)
+                    const int local = d == 0 ? rv * (sl & 3) + (sl >> 2) : sl;
                     nodes[d]->push_back(k0 + local < cnt[d][h] ? lo[d][h] + k0 + local : -1);
                 }
         }
     }
-    // ---- velocity blocks: per octant, chunks of 16 x nbb x ncb node indices ----
+    // ---- velocity blocks: per octant, chunks of NA x nbb x ncb node indices ----
     for (int oz = 0; oz < 2; ++oz) for (int oy = 0; oy < 2; ++oy) for (int ox = 0; ox < 2; ++ox) {
         const int na = cnt[0][ox], nb = cnt[1][oy], nc = cnt[2][oz];
         if (na == 0 || nb == 0 || nc == 0) continue;
         for (int c0 = 0; c0 < nc; c0 += best_cb) for (int b0 = 0; b0 < nb; b0 += best_bb)
-            for (int a0 = 0; a0 < na; a0 += TILE_NA) {
+            for (int a0 = 0; a0 < na; a0 += NA) {
                 VBlock v{};
-                v.a0 = lo[0][ox] + a0; v.na = std::min(TILE_NA, na - a0);
+                v.a0 = lo[0][ox] + a0; v.na = std::min(NA, na - a0);
                 v.b0 = lo[1][oy] + b0; v.nb = std::min(best_bb, nb - b0);
                 v.c0 = lo[2][oz] + c0; v.nc = std::min(best_cb, nc - c0);
                 v.nbb = best_bb; v.ncb = best_cb;
                 v.sx = ox ? 1 : -1; v.sy = oy ? 1 : -1; v.sz = oz ? 1 : -1;
-                v.xb = first[0][ox] + a0 / TILE_NA; v.yb = first[1][oy] + b0 / best_bb; v.zb = first[2][oz] + c0 / best_cb;
+                v.xb = first[0][ox] + a0 / NA; v.yb = first[1][oy] + b0 / best_bb; v.zb = first[2][oz] + c0 / best_cb;
                 plan->vblocks.push_back(v);
             }
     }

@@ -25,13 +25,14 @@ WALL_DIFFUSE, FREESTREAM, ZERO_GRADIENT = 0, 1, 2
 KERNEL_AUTO, KERNEL_SLICE, KERNEL_TILE = 0, 1, 2
 OPT_KERNEL = 1
 OPT_MAX_F_MBYTES = 2
+OPT_TILE_RV = 3
 
 # every symbol include/dvm.h declares (checked by tests/test_abi.py)
 SYMBOLS = (
     "dvm_create", "dvm_iterate", "dvm_moments", "dvm_residual", "dvm_num_faces", "dvm_iterations_done",
     "dvm_get_state", "dvm_set_state", "dvm_raw_moments", "dvm_wall_flux", "dvm_residual_history",
     "dvm_mass_scale", "dvm_step_host", "dvm_set_option", "dvm_workspace_bytes", "dvm_launch_count",
-    "dvm_kernel_used", "dvm_plan_query", "dvm_destroy", "dvm_last_error",
+    "dvm_kernel_used", "dvm_tile_rv", "dvm_plan_query", "dvm_destroy", "dvm_last_error",
 )
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
@@ -119,7 +120,8 @@ def lib():
         L.dvm_set_option.argtypes = [vp, C.c_int, C.c_int]
         L.dvm_workspace_bytes.argtypes = [vp, C.POINTER(C.c_size_t), C.POINTER(C.c_size_t)]
         L.dvm_kernel_used.argtypes = [vp]
-        L.dvm_plan_query.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(_VGrid), C.c_int, C.c_int, C.POINTER(C.c_int),
+        L.dvm_tile_rv.argtypes = [vp]
+        L.dvm_plan_query.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(_VGrid), C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int),
                                      C.POINTER(C.c_int), C.c_int]
         L.dvm_launch_count.argtypes = [vp]
         L.dvm_launch_count.restype = C.c_longlong
@@ -139,14 +141,14 @@ def _f64(a):
     return np.ascontiguousarray(a, dtype=np.float64)
 
 
-def plan_query(nx, ny, nz, xi_x, xi_y, xi_z, target_ctas=296, max_blocks=0, max_items=1 << 22):
+def plan_query(nx, ny, nz, xi_x, xi_y, xi_z, target_ctas=296, max_blocks=0, max_items=1 << 22, rv=0):
     """dvm_plan_query: (counts dict, items int32 [n][9]) of the tile kernel's work decomposition (host only)."""
     keep = [_f64(a) for a in (xi_x, xi_y, xi_z)]
     v = _VGrid(len(keep[0]), len(keep[1]), len(keep[2]), *(a.ctypes.data_as(_dp) for a in keep), None, None, None)
     counts = (C.c_int * 5)()
-    n = _check(lib().dvm_plan_query(nx, ny, nz, C.byref(v), target_ctas, max_blocks, counts, None, 0))
+    n = _check(lib().dvm_plan_query(nx, ny, nz, C.byref(v), target_ctas, max_blocks, rv, counts, None, 0))
     items = np.zeros((min(n, max_items), 9), dtype=np.int32)
-    _check(lib().dvm_plan_query(nx, ny, nz, C.byref(v), target_ctas, max_blocks, counts,
+    _check(lib().dvm_plan_query(nx, ny, nz, C.byref(v), target_ctas, max_blocks, rv, counts,
                                 items.ctypes.data_as(C.POINTER(C.c_int)), len(items)))
     return {"n_vblocks": counts[0], "ntx": counts[1], "nty": counts[2], "P": counts[3], "batch": counts[4],
             "n_items": n}, items
@@ -155,7 +157,7 @@ def plan_query(nx, ny, nz, xi_x, xi_y, xi_z, target_ctas=296, max_blocks=0, max_
 class Solver:
     """dvm_create / dvm_iterate / dvm_moments / dvm_residual (+ support calls) for one workload record."""
 
-    def __init__(self, wl, kernel: int = KERNEL_AUTO, device: str = "cuda:0", max_f_mbytes: int = 0):
+    def __init__(self, wl, kernel: int = KERNEL_AUTO, device: str = "cuda:0", max_f_mbytes: int = 0, tile_rv: int = 0):
         import torch
         if not torch.cuda.is_available():
             raise DvmError(ECUDA, "no CUDA device: the DVM solver has no CPU fallback")
@@ -205,6 +207,8 @@ class Solver:
             self.set_option(OPT_KERNEL, kernel)
         if max_f_mbytes:
             self.set_option(OPT_MAX_F_MBYTES, int(max_f_mbytes))
+        if tile_rv:
+            self.set_option(OPT_TILE_RV, int(tile_rv))
 
     # -- the four calls of the north star ---------------------------------------------------------
     def iterate(self, n: int = 1):
@@ -283,6 +287,9 @@ class Solver:
 
     def kernel_used(self):
         return _check(lib().dvm_kernel_used(self._h))
+
+    def tile_rv(self):
+        return _check(lib().dvm_tile_rv(self._h))
 
     def launch_count(self):
         return int(lib().dvm_launch_count(self._h))
