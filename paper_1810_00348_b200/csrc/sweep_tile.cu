@@ -342,6 +342,27 @@ __device__ __forceinline__ int decode_records(const TileParams &P, const ItemCtx
     return special;
 }
 
+// The RV values of a thread in a face row of NVB doubles are stored as RV / 2 pairs, pair h of thread t at double
+// (h * threads + t) * 2: every 16-byte access of a warp then covers 512 contiguous bytes (full sectors in L2 / HBM, no
+// bank conflict in shared memory).  row = start of the face row.
+template <int RV>
+__device__ __forceinline__ int face_index(int tid, int r) { return ((r >> 1) * (NVB / RV) + tid) * 2 + (r & 1); }
+template <int RV>
+__device__ __forceinline__ void load_face(const double *row, int tid, double (&v)[RV])
+{
+#pragma unroll
+    for (int h = 0; h < RV / 2; ++h) {
+        const double2 t = reinterpret_cast<const double2 *>(row)[h * (NVB / RV) + tid];
+        v[2 * h] = t.x; v[2 * h + 1] = t.y;
+    }
+}
+template <int RV>
+__device__ __forceinline__ void store_face(double *row, int tid, const double (&v)[RV])
+{
+#pragma unroll
+    for (int h = 0; h < RV / 2; ++h) st_f64x2(row + (h * (NVB / RV) + tid) * 2, v[2 * h], v[2 * h + 1]);
+}
+
 // Ghost values of the domain faces of level kp (buffer b) for a tile at the upwind x / y edge of the domain
 template <int RV>
 __device__ __forceinline__ void fill_faces(const ItemCtx &I, TileSmem<RV> &s, int b, int tid, int ag, int yidx, int zidx)
@@ -353,7 +374,7 @@ __device__ __forceinline__ void fill_faces(const ItemCtx &I, TileSmem<RV> &s, in
         for (int r = 0; r < RV; ++r) {
             const double G = s.g[0][0][RV * ag + r] * gyz;
 #pragma unroll
-            for (int jj = 0; jj < TILE_TY; ++jj) L.xface[jj][tid * RV + r] = L.rwb[jj] * G;
+            for (int jj = 0; jj < TILE_TY; ++jj) L.xface[jj][face_index<RV>(tid, r)] = L.rwb[jj] * G;
         }
     }
     if (I.first_y) {
@@ -362,7 +383,7 @@ __device__ __forceinline__ void fill_faces(const ItemCtx &I, TileSmem<RV> &s, in
         for (int r = 0; r < RV; ++r) {
             const double G = s.g[1][0][RV * ag + r] * gyz;
 #pragma unroll
-            for (int ii = 0; ii < 4; ++ii) L.yface[ii][tid * RV + r] = L.rwb[4 + ii] * G;
+            for (int ii = 0; ii < 4; ++ii) L.yface[ii][face_index<RV>(tid, r)] = L.rwb[4 + ii] * G;
         }
     }
 }
@@ -383,23 +404,6 @@ template <int RV>
 __device__ __forceinline__ const double4 &entry(const RowBuf<RV> &R, int byte_off)
 {
     return *reinterpret_cast<const double4 *>(reinterpret_cast<const unsigned char *>(&R) + byte_off);
-}
-
-// RV consecutive doubles of a face row (16-byte aligned)
-template <int RV>
-__device__ __forceinline__ void load_face(const double *p, double (&v)[RV])
-{
-#pragma unroll
-    for (int h = 0; h < RV / 2; ++h) {
-        const double2 t = reinterpret_cast<const double2 *>(p)[h];
-        v[2 * h] = t.x; v[2 * h + 1] = t.y;
-    }
-}
-template <int RV>
-__device__ __forceinline__ void store_face(double *p, const double (&v)[RV])
-{
-#pragma unroll
-    for (int h = 0; h < RV / 2; ++h) st_f64x2(p + 2 * h, v[2 * h], v[2 * h + 1]);
 }
 
 // stage 2 for the cell pair (iiA, iiA + 1) of a row and the REDs of its results (lanes 0..15: cell A, 16..31: cell B).
@@ -427,7 +431,7 @@ __device__ __forceinline__ void compute_row(const RowBuf<RV> &R, const double *x
                                             const ThreadCtx<RV> &T, const int tid, const int lane, double *xout, const bool wx)
 {
     double fx[RV];
-    load_face<RV>(xin + tid * RV, fx);
+    load_face<RV>(xin, tid, fx);
     double acc[2][2];
 #pragma unroll
     for (int ii = 0; ii < 4; ++ii) {
@@ -483,7 +487,7 @@ __device__ __forceinline__ void compute_row(const RowBuf<RV> &R, const double *x
         for (int r = 0; r < RV; ++r) dmma(acc[ii & 1][0], acc[ii & 1][1], T.aX[r], zrow[ii][r]);
         if (ii & 1) emit_pair<RV>(R, ii - 1, acc[0][0], acc[0][1], acc[1][0], acc[1][1], T, lane);
     }
-    if (wx) store_face<RV>(xout + tid * RV, fx);
+    if (wx) store_face<RV>(xout, tid, fx);
 }
 
 // One level of the column, fast path (no solid ghost in the level): 4 rows x 4 cells x RV velocities per thread with the
@@ -501,7 +505,7 @@ __device__ __forceinline__ void compute_level(const LevelBuf<RV> &L, double (&pl
 {
     double yu[4][RV];
 #pragma unroll
-    for (int ii = 0; ii < 4; ++ii) load_face<RV>(&L.yface[ii][tid * RV], yu[ii]);
+    for (int ii = 0; ii < 4; ++ii) load_face<RV>(&L.yface[ii][0], tid, yu[ii]);
 #if DVM_ROW_UNROLL == 4
     compute_row<RV>(L.row[0], L.xface[0], pl[0], yu, T, tid, lane, xout, wx);
 #pragma unroll
@@ -551,7 +555,7 @@ __device__ __forceinline__ void compute_level(const LevelBuf<RV> &L, double (&pl
 #endif
     if (yout) {
 #pragma unroll
-        for (int ii = 0; ii < 4; ++ii) store_face<RV>(yout + ii * NVB + tid * RV, pl[TILE_TY - 1][ii]);
+        for (int ii = 0; ii < 4; ++ii) store_face<RV>(yout + ii * NVB, tid, pl[TILE_TY - 1][ii]);
     }
 }
 
@@ -568,7 +572,7 @@ __device__ __forceinline__ void compute_level_slow(TileSmem<RV> &s, const LevelB
         const RowBuf<RV> &R = L.row[jj];
         double fx[RV];
 #pragma unroll
-        for (int r = 0; r < RV; ++r) fx[r] = L.xface[jj][tid * RV + r];
+        for (int r = 0; r < RV; ++r) fx[r] = L.xface[jj][face_index<RV>(tid, r)];
         double accA0 = 0.0, accA1 = 0.0;
 #pragma unroll 1
         for (int ii = 0; ii < 4; ++ii) {
@@ -589,7 +593,7 @@ __device__ __forceinline__ void compute_level_slow(TileSmem<RV> &s, const LevelB
                 const double Pg = s.g[3][0][RV * T.ag + r] * gyz;
                 const double4 xt = entry(R, xo + r * GA * 32);
                 double xu = fx[r], zu = pl[cell * RV + r];
-                double yu = jj == 0 ? L.yface[ii][tid * RV + r] : pl[(cell - 4) * RV + r];
+                double yu = jj == 0 ? L.yface[ii][face_index<RV>(tid, r)] : pl[(cell - 4) * RV + r];
                 if (code & 1) xu = sp.x * Pg;
                 if (code & 2) yu = sp.y * Pg;
                 if (code & 4) zu = sp.z * Pg;
@@ -612,14 +616,14 @@ __device__ __forceinline__ void compute_level_slow(TileSmem<RV> &s, const LevelB
         }
         if (xout) {
 #pragma unroll
-            for (int r = 0; r < RV; ++r) xout[jj * NVB + tid * RV + r] = fx[r];
+            for (int r = 0; r < RV; ++r) xout[jj * NVB + face_index<RV>(tid, r)] = fx[r];
         }
     }
     if (yout) {
 #pragma unroll 1
         for (int ii = 0; ii < 4; ++ii)
 #pragma unroll
-            for (int r = 0; r < RV; ++r) yout[ii * NVB + tid * RV + r] = pl[((TILE_TY - 1) * 4 + ii) * RV + r];
+            for (int r = 0; r < RV; ++r) yout[ii * NVB + face_index<RV>(tid, r)] = pl[((TILE_TY - 1) * 4 + ii) * RV + r];
     }
 }
 
