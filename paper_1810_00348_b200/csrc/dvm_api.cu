@@ -42,7 +42,6 @@ int fail(int code, const char *fmt, ...)
     } while (0)
 
 constexpr int HIST_CAP = 16384;
-constexpr int RAW_SINK_ROWS = 1024;   // accumulator rows past the last cell: one per CTA of the tile sweep, for dead cells
 const double PI = 3.14159265358979323846;
 
 }  // namespace
@@ -312,7 +311,7 @@ int plan(dvm_solver *s)
             }
         }
         const size_t nitems = s->tile.items.size();
-        s->tile_grid = (int)std::min<size_t>(std::min<size_t>((size_t)resident, nitems), (size_t)RAW_SINK_ROWS);
+        s->tile_grid = (int)std::min<size_t>((size_t)resident, nitems);
         const size_t fbytes = (s->tile.xface_doubles + s->tile.yface_doubles) * sizeof(double);
         s->d_xface = (double *)s->dalloc(s->tile.xface_doubles * sizeof(double));
         s->d_yface = (double *)s->dalloc(s->tile.yface_doubles * sizeof(double));
@@ -452,15 +451,16 @@ int dvm_create(const dvm_grid *g, const dvm_vgrid *v, const dvm_gas *gas, const 
     // per-cell records of the padded grid for the tile kernel (static part; nu is written every iteration)
     s->nxp = nx + 2 * TILE_PAD; s->nyp = ny + 2 * TILE_PAD;
     {
-        CellRec dead{};
-        dead.nu = 1.0; dead.cidx = -1; dead.flags = 0;
-        for (int d = 0; d < 6; ++d) dead.face[d] = -1;
-        s->h_rec.assign((size_t)nz * s->nyp * s->nxp, dead);
-        for (int k = 0; k < nz; ++k) for (int j = 0; j < ny; ++j) for (int i = 0; i < nx; ++i) {
-            const long long c = ((long long)k * ny + j) * nx + i;
-            if (s->solid[c]) continue;
-            CellRec &r = s->h_rec[((size_t)k * s->nyp + j + TILE_PAD) * s->nxp + i + TILE_PAD];
-            r.cidx = (int)c;
+        s->h_rec.resize((size_t)nz * s->nyp * s->nxp);
+        for (int k = 0; k < nz; ++k) for (int jp = 0; jp < s->nyp; ++jp) for (int ip = 0; ip < s->nxp; ++ip) {
+            const int i = ip - TILE_PAD, j = jp - TILE_PAD;
+            const bool inside = i >= 0 && i < nx && j >= 0 && j < ny;
+            const int ic = std::min(std::max(i, 0), nx - 1), jc = std::min(std::max(j, 0), ny - 1);
+            const long long c = ((long long)k * ny + jc) * nx + ic;
+            CellRec &r = s->h_rec[((size_t)k * s->nyp + jp) * s->nxp + ip];
+            r.nu = 1.0; r.cidx = (int)c; r.flags = REC_DEAD; r.pad[0] = r.pad[1] = 0;
+            for (int d = 0; d < 6; ++d) r.face[d] = -1;
+            if (!inside || s->solid[c]) continue;
             r.flags = (int)(flags[c] & 63) | ((int)(sflags[c] & 63) << 8);
             for (int d = 0; d < 6; ++d) r.face[d] = face_of[(size_t)d * n + c];
         }
@@ -540,7 +540,7 @@ int dvm_create(const dvm_grid *g, const dvm_vgrid *v, const dvm_gas *gas, const 
     rc |= dzeros(s, &s->d_phi, (size_t)s->nface);
     rc |= dzeros(s, &s->d_prim_new, (size_t)NPRIM * n);
     rc |= dzeros(s, &s->d_coef, (size_t)NCOEF * n);
-    rc |= dzeros(s, &s->d_raw, (size_t)16 * (n + RAW_SINK_ROWS));
+    rc |= dzeros(s, &s->d_raw, (size_t)16 * n);
     s->npart = (n + 255) / 256;
     rc |= dzeros(s, &s->d_part, (size_t)7 * s->npart);
     rc |= dzeros(s, &s->d_scal, 8);
@@ -599,7 +599,7 @@ int dvm_iterate(dvm_solver *s, int niter)
     const UpdateParams U = update_params(s);
     const SweepParams P = sweep_params(s);
     for (int it = 0; it < niter; ++it) {
-        CK(cudaMemsetAsync(s->d_raw, 0, (size_t)16 * (s->ncell + RAW_SINK_ROWS) * sizeof(double), s->stream));
+        CK(cudaMemsetAsync(s->d_raw, 0, (size_t)16 * s->ncell * sizeof(double), s->stream));
         CK(cudaMemsetAsync(s->d_phi, 0, (size_t)s->nface * sizeof(double), s->stream));
         if (s->kernel == DVM_KERNEL_SLICE) {
             CK(launch_sweep_slice(P, (int)s->blocks.size(), s->nb_threads, s->stream));

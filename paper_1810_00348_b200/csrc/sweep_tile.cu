@@ -61,12 +61,10 @@ struct __align__(128) RowBuf {
     double4 xtab[4][GA * RV];                      // per (cell', xi_x node): E, Q, e, a (slot r*4 + ag); cell' = position of
     double4 ytab[4 * 8];                           // the cell in ascending absolute x;  [cell'][nbb]
     double4 ztab[4 * 8];                           // [cell'][ncb]
-    CellRec rec[4];                                // per cell': 1/tau, cell index, neighbour flags, boundary faces
-    // ---- decoded per level by 16 threads (sweep-relative cell ii) ----
-    double4 spec[4];                               // rho_w of a solid ghost in x, y, z (slow-path levels)
-    double nu[4];                                  // 1/tau (1 for dead cells)
+    CellRec rec[4];                                // per cell': 1/tau, accumulator row, neighbour flags, boundary faces
+    // ---- decoded by 16 threads on levels that hold a solid ghost (slow path; sweep-relative cell ii) ----
+    double4 spec[4];                               // rho_w of a solid ghost in x, y, z
     int code[4];                                   // 1: x-up solid ghost, 2: y-up, 4: z-up, 8: dead cell
-    int cidx[4];                                   // row of the [cell][16] accumulator: the cell index, or the CTA's sink row (dead)
 };
 
 template <int RV>
@@ -88,6 +86,7 @@ struct __align__(128) TileSmem {
     unsigned long long mbar[2];
     unsigned txbytes;                              // bytes the copies of one level deliver
     int item;
+    int special[2];                                // the level in buffer b holds a fluid cell with a solid upwind ghost
 };
 
 // ---- PTX helpers -----------------------------------------------------------------------------------
@@ -310,20 +309,30 @@ __device__ __forceinline__ void issue_level(TileSmem<RV> &s, int kp, int tid)
     if (d.bytes) tma_load(reinterpret_cast<unsigned char *>(&s.lv[b]) + d.dst, d.src + (long long)kp * d.step, d.bytes, &s.mbar[b]);
 }
 
-// Per-cell records of level kp (buffer b = kp & 1) decoded from the staged CellRec rows by the first 16 threads of the
-// last warp; the caller has waited for the level's TMA copies.  Returns 1 if this thread saw a fluid cell with a solid
-// upwind ghost.
+// Does the level staged in buffer b hold a fluid cell whose upwind neighbour is a masked cell?  Asked by lanes 0..15 of
+// warp 0 (one record each) right after they have waited for the level's copies; the answer reaches the other threads
+// through the CTA barrier that ends the level before.
 template <int RV>
-__device__ __forceinline__ int decode_records(const TileParams &P, const ItemCtx &I, TileSmem<RV> &s, int kp, int tid, int sink)
+__device__ __forceinline__ void detect_special(const ItemCtx &I, TileSmem<RV> &s, int b, int lane)
+{
+    const CellRec &r = s.lv[b].row[lane >> 2].rec[lane & 3];
+    const int upmask = (1 << I.upx) | (1 << I.upy) | (1 << I.upz);
+    const bool hit = (((r.flags >> 8) & 0x3f) & upmask) != 0;
+    const unsigned any = __ballot_sync(0x0000ffffu, hit);
+    if (lane == 0) s.special[b] = any != 0u;
+}
+
+// Slow path only: per-cell ghost codes of the level in buffer b, decoded from the staged records by the first 16 threads
+// of the last warp.
+template <int RV>
+__device__ __forceinline__ void decode_records(const TileParams &P, const ItemCtx &I, TileSmem<RV> &s, int b, int tid)
 {
     constexpr int T0 = NVB / RV - 32;
-    const int b = kp & 1;
-    int special = 0;
     if (tid >= T0 && tid < T0 + NCELL) {
         const int cell = tid - T0, ii = cell & 3, jj = cell >> 2;
         RowBuf<RV> &R = s.lv[b].row[jj];
         const CellRec &r = R.rec[I.sx > 0 ? ii : 3 - ii];
-        const bool dead = r.cidx < 0;
+        const bool dead = (r.flags & REC_DEAD) != 0;
         const int sfl = (r.flags >> 8) & 0xff;
         int code = 8;
         double4 sp = make_double4(0.0, 0.0, 0.0, 0.0);
@@ -335,11 +344,7 @@ __device__ __forceinline__ int decode_records(const TileParams &P, const ItemCtx
         }
         R.code[ii] = code;
         R.spec[ii] = sp;
-        R.cidx[ii] = dead ? sink : r.cidx;
-        R.nu[ii] = dead ? 1.0 : r.nu;
-        special = (code & 7) != 0;
     }
-    return special;
 }
 
 // The RV values of a thread in a face row of NVB doubles are stored as RV / 2 pairs, pair h of thread t at double
@@ -396,6 +401,7 @@ struct ThreadCtx {
     double *raw0, *raw1;         // raw16 + accumulator slot of the lane's two results
     double use0, use1;           // 1 if the result is one of the products the sums need, else 0 (the RED then adds 0)
     int xo[4], yo[4], zo[4];     // byte offsets in a RowBuf of the thread's table entries of cell ii (r = 0 for x)
+    int ro[4];                   // byte offset in a RowBuf of the record of cell ii
     int ag, yi, zi;              // xi_x group, rows of the thread's xi_y and xi_z nodes in xi_bc / g
     int xrev;                    // 3 if the sweep runs against x (table rows are in ascending absolute x), else 0
 };
@@ -405,19 +411,26 @@ __device__ __forceinline__ const double4 &entry(const RowBuf<RV> &R, int byte_of
 {
     return *reinterpret_cast<const double4 *>(reinterpret_cast<const unsigned char *>(&R) + byte_off);
 }
-
-// stage 2 for the cell pair (iiA, iiA + 1) of a row and the REDs of its results (lanes 0..15: cell A, 16..31: cell B).
-// No predicates and no branches (the row stays one basic block): a result the sums do not need is multiplied by 0 and
-// added to a slot no other lane of the instruction targets; dead cells carry the CTA's sink row and g = 0.
 template <int RV>
-__device__ __forceinline__ void emit_pair(const RowBuf<RV> &R, const int iiA, const double a0, const double a1, const double b0,
-                                          const double b1, const ThreadCtx<RV> &T, const int lane)
+__device__ __forceinline__ const CellRec &record(const RowBuf<RV> &R, int byte_off)
+{
+    return *reinterpret_cast<const CellRec *>(reinterpret_cast<const unsigned char *>(&R) + byte_off);
+}
+
+// stage 2 for a pair of cells (A, B; roA, roB: their records) of a row and the REDs of its results (lanes 0..15: cell A,
+// 16..31: cell B).
+// No predicates and no branches (the row stays one basic block): a result the sums do not need is multiplied by 0 and
+// added to a slot no other lane of the instruction targets; dead cells have g = 0 and name a row of their own or, in
+// the padding, of the nearest cell of the grid.
+template <int RV>
+__device__ __forceinline__ void emit_pair(const RowBuf<RV> &R, const int roA, const int roB, const double a0, const double a1,
+                                          const double b0, const double b1, const ThreadCtx<RV> &T, const int lane)
 {
     const bool hi = lane & 16;
     double d0 = 0.0, d1 = 0.0;
     dmma(d0, d1, hi ? b0 : a0, T.yz0);
     dmma(d0, d1, hi ? b1 : a1, T.yz1);
-    const long long c = R.cidx[iiA + (hi ? 1 : 0)];
+    const long long c = record(R, hi ? roB : roA).cidx;
     red_f64(T.raw0 + c * 16, d0 * T.use0);
     red_f64(T.raw1 + c * 16, d1 * T.use1);
 }
@@ -425,10 +438,12 @@ __device__ __forceinline__ void emit_pair(const RowBuf<RV> &R, const int iiA, co
 // One row (4 cells along the sweep-relative x) of a level, fast path: zrow holds the values of the row in the previous
 // z-plane (the z-upwind operands) and receives the new ones, yup holds the y-upwind operands (the staged y-face for the
 // first row of the tile, else the row just computed).  Dead cells (outside the domain / solid) have all-zero table
-// entries and nu = 1, so they produce g = 0 by the same arithmetic.
-template <int RV>
+// entries and nu = 1, so they produce g = 0 by the same arithmetic.  The last row of the tile (LAST) also writes the
+// y-face output, cell by cell, so that the stores are spread over the row.
+template <int RV, bool LAST>
 __device__ __forceinline__ void compute_row(const RowBuf<RV> &R, const double *xin, double (&zrow)[4][RV], const double (&yup)[4][RV],
-                                            const ThreadCtx<RV> &T, const int tid, const int lane, double *xout, const bool wx)
+                                            const ThreadCtx<RV> &T, const int tid, const int lane, double *xout, const bool wx,
+                                            double *yout, const bool wy)
 {
     double fx[RV];
     load_face<RV>(xin, tid, fx);
@@ -439,7 +454,7 @@ __device__ __forceinline__ void compute_row(const RowBuf<RV> &R, const double *x
         const double4 zt = entry(R, T.zo[ii]);
         const double Eyz = yt.x * zt.x, Qyz = yt.y + zt.y, eyz = yt.z + zt.z;
         const double ay = yt.w, az = zt.w;
-        const double dyz = (ay + az) + R.nu[ii];
+        const double dyz = (ay + az) + record(R, T.ro[ii]).nu;
         // Everything that does not depend on the x-upwind value, for the RV nodes of the thread in lock step (the fp64
         // pipe takes a warp instruction every 2 clocks and has a latency of ~10): the cell value is g = W g_xup + V with
         // W = a_x / den and V = (a_y g_yup + a_z g_zup + src) / den, Eq.(7) PAPER.md:75-79.
@@ -485,77 +500,34 @@ __device__ __forceinline__ void compute_row(const RowBuf<RV> &R, const double *x
         acc[ii & 1][0] = 0.0; acc[ii & 1][1] = 0.0;
 #pragma unroll
         for (int r = 0; r < RV; ++r) dmma(acc[ii & 1][0], acc[ii & 1][1], T.aX[r], zrow[ii][r]);
-        if (ii & 1) emit_pair<RV>(R, ii - 1, acc[0][0], acc[0][1], acc[1][0], acc[1][1], T, lane);
+        if (ii & 1) emit_pair<RV>(R, T.ro[ii - 1], T.ro[ii], acc[0][0], acc[0][1], acc[1][0], acc[1][1], T, lane);
+        if (LAST && wy) store_face<RV>(yout + ii * NVB, tid, zrow[ii]);
     }
     if (wx) store_face<RV>(xout, tid, fx);
 }
 
 // One level of the column, fast path (no solid ghost in the level): 4 rows x 4 cells x RV velocities per thread with the
-// plane in registers (static indices only).  The B200 instruction cache holds 32 KB, and a level loop larger than that is
-// fetch-bound at 1/3 instruction per clock and scheduler (profiles/r01_ifetch_microbench.txt), so how many rows are
-// unrolled is a code-size decision.  DVM_ROW_UNROLL = 4: all rows unrolled, the y-upwind operands of a row are the
-// registers of the row before, no register moves; = 2: a 2-iteration loop over row pairs whose body works on row slots
-// 0, 1 and then swaps them with slots 2, 3; = 1: a 4-iteration loop that works on slot 0 and rotates the slots.
-#ifndef DVM_ROW_UNROLL
-#define DVM_ROW_UNROLL 4
-#endif
+// plane in registers (static indices only); the rows are unrolled, the y-upwind operands of a row are the registers of
+// the row before.  The B200 instruction cache holds 32 KB, and a level loop larger than that is fetch-bound at 1/3
+// instruction per clock and scheduler (profiles/r01_ifetch_microbench.txt): the instructions a level executes on
+// this path (about 1900 for RV = 4) stay below that; rolled variants with rotating row slots were slower (profiles/).
 template <int RV>
 __device__ __forceinline__ void compute_level(const LevelBuf<RV> &L, double (&pl)[TILE_TY][4][RV], const ThreadCtx<RV> &T,
-                                              const int tid, const int lane, double *xout, const bool wx, double *yout)
+                                              const int tid, const int lane, double *xout, const bool wx, double *yout,
+                                              const bool wy)
 {
     double yu[4][RV];
 #pragma unroll
     for (int ii = 0; ii < 4; ++ii) load_face<RV>(&L.yface[ii][0], tid, yu[ii]);
-#if DVM_ROW_UNROLL == 4
-    compute_row<RV>(L.row[0], L.xface[0], pl[0], yu, T, tid, lane, xout, wx);
+    if (TILE_TY == 1) {
+        compute_row<RV, true>(L.row[0], L.xface[0], pl[0], yu, T, tid, lane, xout, wx, yout, wy);
+    } else {
+        compute_row<RV, false>(L.row[0], L.xface[0], pl[0], yu, T, tid, lane, xout, wx, yout, wy);
 #pragma unroll
-    for (int jj = 1; jj < TILE_TY; ++jj) compute_row<RV>(L.row[jj], L.xface[jj], pl[jj], pl[jj - 1], T, tid, lane, xout + jj * NVB, wx);
-#elif DVM_ROW_UNROLL == 2
-    static_assert(TILE_TY == 4, "row pairs");
-    const RowBuf<RV> *R = &L.row[0];
-    const double *xin = &L.xface[0][0];
-#pragma unroll 1
-    for (int h = 0; h < 2; ++h) {
-        compute_row<RV>(R[0], xin, pl[0], yu, T, tid, lane, xout, wx);
-        compute_row<RV>(R[1], xin + NVB, pl[1], pl[0], T, tid, lane, xout + NVB, wx);
-        R += 2;
-        xin += 2 * NVB;
-        xout += 2 * NVB;
-#pragma unroll
-        for (int ii = 0; ii < 4; ++ii)
-#pragma unroll
-            for (int r = 0; r < RV; ++r) {
-                const double t0 = pl[0][ii][r], t1 = pl[1][ii][r];
-                yu[ii][r] = t1;
-                pl[0][ii][r] = pl[2][ii][r]; pl[1][ii][r] = pl[3][ii][r];
-                pl[2][ii][r] = t0; pl[3][ii][r] = t1;
-            }
-    }
-#else
-    const RowBuf<RV> *R = &L.row[0];
-    const double *xin = &L.xface[0][0];
-#pragma unroll 1
-    for (int jj = 0; jj < TILE_TY; ++jj) {
-        compute_row<RV>(*R, xin, pl[0], yu, T, tid, lane, xout, wx);
-        ++R;
-        xin += NVB;
-        xout += NVB;
-        // rotate the row slots: (0, 1, 2, 3) <- (1, 2, 3, 0); after the 4th iteration the rows are back in place
-#pragma unroll
-        for (int ii = 0; ii < 4; ++ii)
-#pragma unroll
-            for (int r = 0; r < RV; ++r) {
-                const double t = pl[0][ii][r];
-                yu[ii][r] = t;
-#pragma unroll
-                for (int q = 0; q + 1 < TILE_TY; ++q) pl[q][ii][r] = pl[q + 1][ii][r];
-                pl[TILE_TY - 1][ii][r] = t;
-            }
-    }
-#endif
-    if (yout) {
-#pragma unroll
-        for (int ii = 0; ii < 4; ++ii) store_face<RV>(yout + ii * NVB, tid, pl[TILE_TY - 1][ii]);
+        for (int jj = 1; jj < TILE_TY - 1; ++jj)
+            compute_row<RV, false>(L.row[jj], L.xface[jj], pl[jj], pl[jj - 1], T, tid, lane, xout + jj * NVB, wx, yout, wy);
+        compute_row<RV, true>(L.row[TILE_TY - 1], L.xface[TILE_TY - 1], pl[TILE_TY - 1], pl[TILE_TY > 1 ? TILE_TY - 2 : 0], T, tid, lane,
+                              xout + (TILE_TY - 1) * NVB, wx, yout, wy);
     }
 }
 
@@ -574,6 +546,7 @@ __device__ __forceinline__ void compute_level_slow(TileSmem<RV> &s, const LevelB
 #pragma unroll
         for (int r = 0; r < RV; ++r) fx[r] = L.xface[jj][face_index<RV>(tid, r)];
         double accA0 = 0.0, accA1 = 0.0;
+        int roPrev = 0;
 #pragma unroll 1
         for (int ii = 0; ii < 4; ++ii) {
             const int cell = jj * 4 + ii;
@@ -584,7 +557,8 @@ __device__ __forceinline__ void compute_level_slow(TileSmem<RV> &s, const LevelB
             const double4 zt = entry(R, zo);
             const double Eyz = yt.x * zt.x, Qyz = yt.y + zt.y, eyz = yt.z + zt.z;
             const double ay = yt.w, az = zt.w;
-            const double dyz = (ay + az) + R.nu[ii];
+            const int ro = ii == 0 ? T.ro[0] : ii == 1 ? T.ro[1] : ii == 2 ? T.ro[2] : T.ro[3];
+            const double dyz = (ay + az) + record(R, ro).nu;
             const int code = R.code[ii];
             const double4 sp = R.spec[ii];
             double c0 = 0.0, c1 = 0.0;
@@ -609,10 +583,11 @@ __device__ __forceinline__ void compute_level_slow(TileSmem<RV> &s, const LevelB
                 dmma(c0, c1, T.aX[r], gg);
             }
             if (ii & 1) {
-                emit_pair<RV>(R, ii - 1, accA0, accA1, c0, c1, T, lane);
+                emit_pair<RV>(R, roPrev, ro, accA0, accA1, c0, c1, T, lane);
             } else {
                 accA0 = c0; accA1 = c1;
             }
+            roPrev = ro;
         }
         if (xout) {
 #pragma unroll
@@ -644,7 +619,6 @@ __global__ void __launch_bounds__(NVB / RV, 2) sweep_tile_kernel(const TileParam
     }
     __syncthreads();
     unsigned par[2] = {0u, 0u};
-    const int sink = (int)P.ncell + (int)blockIdx.x;   // accumulator row that takes the (zero) sums of dead cells
 
     for (;;) {
         // ---- next item (dependency order), wait for its upwind items ----
@@ -729,6 +703,7 @@ __global__ void __launch_bounds__(NVB / RV, 2) sweep_tile_kernel(const TileParam
                 T.xo[ii] = (int)offsetof(RowBuf<RV>, xtab) + (cp * NA + T.ag) * 32;
                 T.yo[ii] = (int)offsetof(RowBuf<RV>, ytab) + (cp * vb.nbb + yl) * 32;
                 T.zo[ii] = (int)offsetof(RowBuf<RV>, ztab) + (cp * vb.ncb + zl) * 32;
+                T.ro[ii] = (int)offsetof(RowBuf<RV>, rec) + cp * (int)sizeof(CellRec);
             }
             // stage-1 A fragments: xi_x^p of the thread's own nodes, p = (lane >> 2) & 3
             const int row = lane >> 2, pw = row & 3;
@@ -761,14 +736,13 @@ __global__ void __launch_bounds__(NVB / RV, 2) sweep_tile_kernel(const TileParam
             T.use0 = u0 ? 1.0 : 0.0; T.use1 = u1 ? 1.0 : 0.0;
         }
 
-        // Records and boundary faces of level 0.  Only the 16 decoding threads wait on the mbarrier of a level's copies
-        // (a try_wait round trip costs several hundred clocks); they do so one level ahead, and the CTA barrier that
-        // follows hands their observation of the completed copies on to every other thread.
-        int special = 0;
-        if (tid >= THREADS - 32 && tid < THREADS - 32 + NCELL) {
+        // Level 0 has landed?  Only lanes 0..15 of warp 0 ever wait on the mbarrier of a level's copies (a try_wait round
+        // trip costs several hundred clocks); they do so one level ahead, look for solid ghosts in the staged records, and
+        // the CTA barrier that follows hands their observation of the completed copies on to every other thread.
+        if (tid < NCELL) {
             mbar_wait(&s.mbar[0], par[0]);
             par[0] ^= 1u;
-            special = decode_records<RV>(P, I, s, 0, tid, sink);
+            detect_special<RV>(I, s, 0, lane);
         }
         fill_faces<RV>(I, s, 0, tid, T.ag, T.yi, T.zi);
         // plane = ghost of the upwind z face of the domain
@@ -789,40 +763,45 @@ __global__ void __launch_bounds__(NVB / RV, 2) sweep_tile_kernel(const TileParam
                     for (int r = 0; r < RV; ++r) pl[jj][ii][r] = rw * G[r];
                 }
         }
-        special = __shfl_sync(0xffffffffu, __syncthreads_or(special), 0);
+        __syncthreads();
 
         const bool write_x = it.ti < P.ntx - 1, write_y = it.tj < P.nty - 1;
+        const bool edge = I.first_x | I.first_y;
 
         for (int kp = 0; kp < P.nz; ++kp) {
             const int b = kp & 1;
-            const double vrw = rwb_load(P, I, kp + 2, tid);
-            double *xout = write_x ? xdst + (long long)kp * XLEVEL_DOUBLES : nullptr;
-            double *yout = write_y ? ydst + (long long)kp * YLEVEL_DOUBLES : nullptr;
+            // level kp + 1 (issued a level ago): wait for it and look for solid ghosts, for the barrier at the end
+            if (tid < NCELL && kp + 1 < P.nz) {
+                mbar_wait(&s.mbar[b ^ 1], par[b ^ 1]);
+                par[b ^ 1] ^= 1u;
+                detect_special<RV>(I, s, b ^ 1, lane);
+            }
+            double vrw = 0.0;
+            if (edge) vrw = rwb_load(P, I, kp + 2, tid);
+            const int special = __shfl_sync(0xffffffffu, s.special[b], 0);
+            double *xout = xdst + (long long)kp * XLEVEL_DOUBLES, *yout = ydst + (long long)kp * YLEVEL_DOUBLES;
             if (special) {
+                // every thread of the CTA takes this branch together
+                decode_records<RV>(P, I, s, b, tid);
+                __syncthreads();
                 double tmp[NCELL * RV];
 #pragma unroll
                 for (int c = 0; c < NCELL; ++c)
 #pragma unroll
                     for (int r = 0; r < RV; ++r) tmp[c * RV + r] = pl[c >> 2][c & 3][r];
-                compute_level_slow<RV>(s, s.lv[b], tmp, T, tid, lane, xout, yout);
+                compute_level_slow<RV>(s, s.lv[b], tmp, T, tid, lane, write_x ? xout : nullptr, write_y ? yout : nullptr);
 #pragma unroll
                 for (int c = 0; c < NCELL; ++c)
 #pragma unroll
                     for (int r = 0; r < RV; ++r) pl[c >> 2][c & 3][r] = tmp[c * RV + r];
             } else {
-                compute_level<RV>(s.lv[b], pl, T, tid, lane, xdst + (long long)kp * XLEVEL_DOUBLES, write_x, yout);
+                compute_level<RV>(s.lv[b], pl, T, tid, lane, xout, write_x, yout, write_y);
             }
-            rwb_store<RV>(s, b, tid, vrw);
-            int sp = 0;
-            if (kp + 1 < P.nz) {
-                if (tid >= THREADS - 32 && tid < THREADS - 32 + NCELL) {
-                    mbar_wait(&s.mbar[b ^ 1], par[b ^ 1]);   // level kp + 1 has landed (issued a level ago)
-                    par[b ^ 1] ^= 1u;
-                    sp = decode_records<RV>(P, I, s, kp + 1, tid, sink);
-                }
-                fill_faces<RV>(I, s, b ^ 1, tid, T.ag, T.yi, T.zi);
+            if (edge) {
+                rwb_store<RV>(s, b, tid, vrw);
+                if (kp + 1 < P.nz) fill_faces<RV>(I, s, b ^ 1, tid, T.ag, T.yi, T.zi);
             }
-            special = __shfl_sync(0xffffffffu, __syncthreads_or(sp), 0);
+            __syncthreads();
             if (copy_of_thread<RV>(tid) < NCOPY && kp + 2 < P.nz) {
                 fence_proxy_async_smem();  // this level's reads of the staging buffers before the TMA overwrites them
                 issue_level<RV>(s, kp + 2, tid);

@@ -35,10 +35,12 @@ inline int tile_na(int rv) { return TILE_GA * rv; }          // xi_x nodes per v
 inline int tile_npair(int rv) { return TILE_NVB / rv / TILE_GA; }   // (xi_y, xi_z) pairs per block = nbb * ncb
 
 // per-cell record of the padded grid, fetched by TMA with the factor tables (48 bytes)
+constexpr int REC_DEAD = 1 << 16;
 struct CellRec {
-    double nu;        // 1/tau of step n (written by the table kernel every iteration)
-    int cidx;         // cell index, -1 for padding and solid cells
-    int flags;        // bits 0..5: neighbour in direction d is not fluid; bits 8..13: it is a solid cell
+    double nu;        // 1/tau of step n (written by the table kernel every iteration); 1 for dead cells
+    int cidx;         // row of the [cell][16] accumulator the sums of this cell go to: the cell index; a dead cell (solid, or
+                      // in the padding) produces exact zeros and names its own row / that of the nearest cell of the grid
+    int flags;        // bits 0..5: neighbour in direction d is not fluid; bits 8..13: it is a solid cell; REC_DEAD
     int face[6];      // boundary-face slot in direction d or -1
     int pad[2];       // 48 bytes: every row of records starts on a 16-byte boundary (TMA)
 };
