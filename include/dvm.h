@@ -57,6 +57,8 @@ extern "C" {
 
 #define DVM_OPT_KERNEL    1
 #define DVM_OPT_MAX_F_MBYTES 2 /* tile kernel: cap (MiB) on the f workspace; velocity blocks then sweep in batches (0 = none) */
+#define DVM_OPT_MAX_CTAS  4 /* tile kernel: cap on the persistent grid (0 = every resident CTA); 1 runs the work items strictly in
+                             hand-out order on one CTA - for tests of the dependency protocol, not for speed */
 #define DVM_OPT_TILE_RV   3 /* tile kernel: velocities per thread, 4 (128-thread CTAs, velocity blocks of 16 x 8 x 4 nodes) or 2
                              (256-thread CTAs, blocks of 8 x 8 x 8 nodes); 0 = the library chooses by lane use (default) */
 
@@ -159,6 +161,11 @@ int dvm_tile_rv(const dvm_solver *s);
  * predecessors are item indices or -1.  Returns the number of items. */
 int dvm_plan_query(int nx, int ny, int nz, const dvm_vgrid *v, int target_ctas, int max_blocks, int rv, int *counts5,
                    int *items9, int max_items);
+/* Host-only: the velocity blocks of the tile kernel for the nodes of v (rv as in dvm_plan_query), in block-id order (the
+ * order of dvm_plan_query's items9[0]).  boxes8 (may be NULL) receives for the first max_blocks blocks {a0, na, b0, nb, c0,
+ * nc, NA, 256 nbb + ncb}: the block holds the nodes [a0, a0+na) x [b0, b0+nb) x [c0, c0+nc) of one sign octant, in a box
+ * of NA x nbb x ncb lanes.  Returns the number of blocks. */
+int dvm_plan_vblocks(const dvm_vgrid *v, int rv, int *boxes8, int max_blocks);
 /* Bytes of device workspace held by the solver, and the part of it that holds distribution-function values. */
 int dvm_workspace_bytes(const dvm_solver *s, size_t *total, size_t *f_bytes);
 /* Number of kernel launches enqueued by this solver so far (bench.py's gpu_launches). */

@@ -62,6 +62,7 @@ struct dvm_solver {
     int kernel = DVM_KERNEL_AUTO;
     long long max_f_mbytes = 0;   // cap on the f workspace of the tile kernel (0 = none)
     int tile_rv = 0;              // velocities per thread of the tile kernel: 0 = choose, 2, 4
+    int max_ctas = 0;             // cap on the persistent grid of the tile kernel (0 = all resident CTAs)
     bool planned = false;
     long long launches = 0;
     // device arrays
@@ -312,6 +313,7 @@ int plan(dvm_solver *s)
         }
         const size_t nitems = s->tile.items.size();
         s->tile_grid = (int)std::min<size_t>((size_t)resident, nitems);
+        if (s->max_ctas > 0) s->tile_grid = std::min(s->tile_grid, s->max_ctas);
         const size_t fbytes = (s->tile.xface_doubles + s->tile.yface_doubles) * sizeof(double);
         s->d_xface = (double *)s->dalloc(s->tile.xface_doubles * sizeof(double));
         s->d_yface = (double *)s->dalloc(s->tile.yface_doubles * sizeof(double));
@@ -582,6 +584,12 @@ int dvm_set_option(dvm_solver *s, int option, int value)
         s->tile_rv = value;
         return DVM_OK;
     }
+    if (option == DVM_OPT_MAX_CTAS) {
+        if (s->planned) return fail(DVM_EINVAL, "the grid cap must be set before the first iteration");
+        if (value < 0) return fail(DVM_EINVAL, "negative grid cap");
+        s->max_ctas = value;
+        return DVM_OK;
+    }
     if (option == DVM_OPT_MAX_F_MBYTES) {
         if (s->planned) return fail(DVM_EINVAL, "the workspace cap must be set before the first iteration");
         if (value < 0) return fail(DVM_EINVAL, "negative workspace cap");
@@ -747,6 +755,25 @@ int dvm_plan_query(int nx, int ny, int nz, const dvm_vgrid *v, int target_ctas, 
             o[8] = it.fslot;
         }
     }
+    return n;
+}
+
+int dvm_plan_vblocks(const dvm_vgrid *v, int rv, int *boxes8, int max_blocks)
+{
+    if (!v || max_blocks < 0 || (rv != 0 && rv != 2 && rv != 4) || v->mx <= 0 || v->my <= 0 || v->mz <= 0 || !v->xi_x || !v->xi_y || !v->xi_z)
+        return fail(DVM_EINVAL, "bad argument");
+    std::vector<double> xi[3];
+    xi[0].assign(v->xi_x, v->xi_x + v->mx); xi[1].assign(v->xi_y, v->xi_y + v->my); xi[2].assign(v->xi_z, v->xi_z + v->mz);
+    if (rv == 0) rv = choose_rv(xi);
+    TilePlan tp;
+    if (tile_plan(4, 4, 1, xi, 1, 0, rv, &tp)) return fail(DVM_EINVAL, "tile plan failed");
+    const int n = (int)tp.vblocks.size();
+    if (boxes8)
+        for (int e = 0; e < n && e < max_blocks; ++e) {
+            const VBlock &b = tp.vblocks[e];
+            int *o = boxes8 + 8 * e;
+            o[0] = b.a0; o[1] = b.na; o[2] = b.b0; o[3] = b.nb; o[4] = b.c0; o[5] = b.nc; o[6] = tile_na(rv); o[7] = b.nbb * 256 + b.ncb;
+        }
     return n;
 }
 

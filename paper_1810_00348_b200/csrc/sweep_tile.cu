@@ -605,7 +605,7 @@ __device__ __forceinline__ void compute_level_slow(TileSmem<RV> &s, const LevelB
 template <int RV>
 __global__ void __launch_bounds__(NVB / RV, 2) sweep_tile_kernel(const TileParams P)
 {
-    constexpr int THREADS = NVB / RV, NA = GA * RV;
+    constexpr int NA = GA * RV;
     // dynamic shared memory starts at offset 0 of the CTA's window (no static __shared__ in this kernel), so the
     // 128-byte alignment holds; casting without pointer arithmetic keeps the address space visible (LDS / STS)
     extern __shared__ __align__(128) unsigned char smem_raw[];

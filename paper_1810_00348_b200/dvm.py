@@ -26,13 +26,14 @@ KERNEL_AUTO, KERNEL_SLICE, KERNEL_TILE = 0, 1, 2
 OPT_KERNEL = 1
 OPT_MAX_F_MBYTES = 2
 OPT_TILE_RV = 3
+OPT_MAX_CTAS = 4
 
 # every symbol include/dvm.h declares (checked by tests/test_abi.py)
 SYMBOLS = (
     "dvm_create", "dvm_iterate", "dvm_moments", "dvm_residual", "dvm_num_faces", "dvm_iterations_done",
     "dvm_get_state", "dvm_set_state", "dvm_raw_moments", "dvm_wall_flux", "dvm_residual_history",
     "dvm_mass_scale", "dvm_step_host", "dvm_set_option", "dvm_workspace_bytes", "dvm_launch_count",
-    "dvm_kernel_used", "dvm_tile_rv", "dvm_plan_query", "dvm_destroy", "dvm_last_error",
+    "dvm_kernel_used", "dvm_tile_rv", "dvm_plan_query", "dvm_plan_vblocks", "dvm_destroy", "dvm_last_error",
 )
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
@@ -99,8 +100,8 @@ def lib():
     """Load libdvm_b200.so (building it if the sources are newer).  Raises if it cannot be had."""
     global _lib
     if _lib is None:
-        if not _SO.exists():
-            build()
+        if "DVM_B200_LIB" not in os.environ:
+            build()   # no-op when the library is newer than every source
         L = C.CDLL(str(_SO))
         vp = C.c_void_p
         L.dvm_create.argtypes = [C.POINTER(_Grid), C.POINTER(_VGrid), C.POINTER(_Gas), C.POINTER(_BC),
@@ -123,6 +124,7 @@ def lib():
         L.dvm_tile_rv.argtypes = [vp]
         L.dvm_plan_query.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(_VGrid), C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int),
                                      C.POINTER(C.c_int), C.c_int]
+        L.dvm_plan_vblocks.argtypes = [C.POINTER(_VGrid), C.c_int, C.POINTER(C.c_int), C.c_int]
         L.dvm_launch_count.argtypes = [vp]
         L.dvm_launch_count.restype = C.c_longlong
         L.dvm_destroy.argtypes = [vp]
@@ -154,10 +156,21 @@ def plan_query(nx, ny, nz, xi_x, xi_y, xi_z, target_ctas=296, max_blocks=0, max_
             "n_items": n}, items
 
 
+def plan_vblocks(xi_x, xi_y, xi_z, rv=0):
+    """dvm_plan_vblocks: int32 [n][8] = a0, na, b0, nb, c0, nc, NA, 256 nbb + ncb per velocity block (host only)."""
+    keep = [_f64(a) for a in (xi_x, xi_y, xi_z)]
+    v = _VGrid(len(keep[0]), len(keep[1]), len(keep[2]), *(a.ctypes.data_as(_dp) for a in keep), None, None, None)
+    n = _check(lib().dvm_plan_vblocks(C.byref(v), rv, None, 0))
+    out = np.zeros((n, 8), dtype=np.int32)
+    _check(lib().dvm_plan_vblocks(C.byref(v), rv, out.ctypes.data_as(C.POINTER(C.c_int)), n))
+    return out
+
+
 class Solver:
     """dvm_create / dvm_iterate / dvm_moments / dvm_residual (+ support calls) for one workload record."""
 
-    def __init__(self, wl, kernel: int = KERNEL_AUTO, device: str = "cuda:0", max_f_mbytes: int = 0, tile_rv: int = 0):
+    def __init__(self, wl, kernel: int = KERNEL_AUTO, device: str = "cuda:0", max_f_mbytes: int = 0, tile_rv: int = 0,
+                 max_ctas: int = 0):
         import torch
         if not torch.cuda.is_available():
             raise DvmError(ECUDA, "no CUDA device: the DVM solver has no CPU fallback")
@@ -209,6 +222,8 @@ class Solver:
             self.set_option(OPT_MAX_F_MBYTES, int(max_f_mbytes))
         if tile_rv:
             self.set_option(OPT_TILE_RV, int(tile_rv))
+        if max_ctas:
+            self.set_option(OPT_MAX_CTAS, int(max_ctas))
 
     # -- the four calls of the north star ---------------------------------------------------------
     def iterate(self, n: int = 1):

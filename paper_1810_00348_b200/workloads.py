@@ -283,3 +283,28 @@ def sparse_weight_subset(wl: Workload, keep: int = 8, seed: int = 100348) -> Wor
 
     return wl.with_(w_x=thin(wl.xi_x, wl.w_x), w_y=thin(wl.xi_y, wl.w_y), w_z=thin(wl.xi_z, wl.w_z),
                     name=wl.name + f"_wsub{keep}")
+
+
+def stratified_weight_subset(wl: Workload, boxes, seed: int = 0) -> Workload:
+    """Zero all but ONE node per 1-D velocity block and axis in the 1-D weights, so that the kept velocities (their tensor
+    product) put exactly one velocity into every velocity block of the CUDA tile kernel.
+
+    `boxes` is the block table of `dvm.plan_vblocks` (rows a0, na, b0, nb, c0, nc, ...): only its node ranges are used
+    here.  The position of the kept node inside its 1-D block rotates with the block and with `seed`, so that the kept
+    velocities visit different register slots, lane-quad roles and lane positions of the kernel.  The oracle skips the
+    zero-weight velocities; the CUDA path sweeps everything (full-size one-step parity).
+    """
+    boxes = np.asarray(boxes)
+
+    def thin(w, starts_counts, stride):
+        out = np.zeros_like(w)
+        for n, (lo, cnt) in enumerate(sorted(set(starts_counts))):
+            pos = (stride * n + 1 + seed) % cnt
+            out[lo + pos] = w[lo + pos]
+        return out
+
+    bx = [(int(r[0]), int(r[1])) for r in boxes]
+    by = [(int(r[2]), int(r[3])) for r in boxes]
+    bz = [(int(r[4]), int(r[5])) for r in boxes]
+    return wl.with_(w_x=thin(wl.w_x, bx, 5), w_y=thin(wl.w_y, by, 3), w_z=thin(wl.w_z, bz, 1),
+                    name=wl.name + f"_strat{seed}")

@@ -76,3 +76,28 @@ def test_plan_rejects_bad_input():
     wl = W.config(0)
     with pytest.raises(dvm.DvmError):
         dvm.plan_query(0, 8, 8, wl.xi_x, wl.xi_y, wl.xi_z)
+
+
+@pytest.mark.parametrize("cfg", [2, 3, 4])
+@pytest.mark.parametrize("rv", [4, 2])
+def test_stratified_subset_puts_one_velocity_in_every_block(cfg, rv):
+    """The full-size one-step parity cases keep one velocity per velocity block of the tile kernel (a zero-weight
+    velocity is identically zero inside that kernel): exactly one kept velocity in each block of dvm_plan_vblocks, both
+    signs present on every axis, and the in-block positions of the two seeds differ."""
+    wl = W.config(cfg)
+    boxes = dvm.plan_vblocks(wl.xi_x, wl.xi_y, wl.xi_z, rv)
+    counts, items = dvm.plan_query(wl.nx, wl.ny, wl.nz, wl.xi_x, wl.xi_y, wl.xi_z, rv=rv, max_items=1)
+    assert len(boxes) == counts["n_vblocks"]
+    kept = []
+    for seed in (0, 1):
+        sub = W.stratified_weight_subset(wl, boxes, seed)
+        kx, ky, kz = (np.flatnonzero(w) for w in (sub.w_x, sub.w_y, sub.w_z))
+        for b in boxes:
+            n = (((kx >= b[0]) & (kx < b[0] + b[1])).sum() * ((ky >= b[2]) & (ky < b[2] + b[3])).sum()
+                 * ((kz >= b[4]) & (kz < b[4] + b[5])).sum())
+            assert n == 1
+        assert len(kx) * len(ky) * len(kz) == len(boxes)
+        for xi, k in ((wl.xi_x, kx), (wl.xi_y, ky), (wl.xi_z, kz)):
+            assert (xi[k] < 0).any() and (xi[k] >= 0).any()
+        kept.append((kx, ky, kz))
+    assert not np.array_equal(kept[0][0], kept[1][0])
