@@ -7,6 +7,11 @@
  * form of ref. [60]), direct exp() / pow() / division per phase point, long-double
  * accumulation of the velocity sums in a fixed alpha order per thread.  OpenMP over velocities only
  * (velocities are independent inside an iteration).
+ *
+ * order = 2 ("extend the first order upwind scheme to second order by
+ * storing three consecutive slices"): the paper gives no formula; reading G21 of DESIGN.md is the finite-volume
+ * second-order upwind scheme, i.e. Eq.(7) with the cell values at the two faces of a cell replaced by values
+ * extrapolated linearly from the two upwind cell centres, first order where the second upwind cell is missing.
  */
 #include "dvm_oracle.h"
 
@@ -305,12 +310,37 @@ static void sweep_one(const odvm_problem *p, const face_tab *t, const double *pr
                 double num = odvm_feq(p, W, xi) / tau;
                 double den = 1.0 / tau;
                 int zg_face[3] = {-1, -1, -1};
+                double psi[3] = {0.0, 0.0, 0.0}, f1v[3] = {0.0, 0.0, 0.0};
                 for (int d = 0; d < 3; ++d) {
                     const int up = 2 * d + (s[d] > 0 ? 0 : 1); /* side of the cell the flow comes from */
                     const int face = t->face_of[up][c];
                     double fu;
                     if (face < 0) {
-                        fu = f[c - (size_t)((long)s[d] * (long)stride[d])];
+                        const size_t c1 = c - (size_t)((long)s[d] * (long)stride[d]);
+                        fu = f[c1];
+                        if (p->order == 2) {
+                            /* Reading G21.  Value at the downwind face of a cell = its value extrapolated linearly
+                             * from the two upwind centres: F(c) = f_c + psi_c (f_c - f_c1), psi_c = w_c / (w_c + w_c1)
+                             * (w = cell widths along d); F(c) = f_c if c1 is not a fluid cell.  The transport term of
+                             * Eq.(7) along d becomes a_d (F(c) - F(c1)); F(c1) likewise needs c2. */
+                            const int idx[3] = {i, j, k};
+                            const double *xfd = d == 0 ? p->xf : d == 1 ? p->yf : p->zf;
+                            const int q = idx[d], q1 = q - s[d];
+                            const double wc = xfd[q + 1] - xfd[q], w1 = xfd[q1 + 1] - xfd[q1];
+                            psi[d] = wc / (wc + w1);
+                            f1v[d] = fu;
+                            double Fup = fu;
+                            if (t->face_of[up][c1] < 0) {
+                                const size_t c2 = c1 - (size_t)((long)s[d] * (long)stride[d]);
+                                const int q2 = q1 - s[d];
+                                const double w2 = xfd[q2 + 1] - xfd[q2];
+                                Fup = fu + w1 / (w1 + w2) * (fu - f[c2]);
+                            }
+                            /* a_d [(1 + psi) f_c - psi f_c1 - Fup] : the f_c part goes to the denominator */
+                            num += a[d] * (psi[d] * fu + Fup);
+                            den += a[d] * (1.0 + psi[d]);
+                            continue;
+                        }
                     } else {
                         const int b = t->bc_slot[face];
                         if (p->bc_type[b] == ODVM_WALL_DIFFUSE) fu = rho_w[face] * gw[b];
@@ -324,8 +354,11 @@ static void sweep_one(const odvm_problem *p, const face_tab *t, const double *pr
                 const double fc = num / den;
                 f[c] = fc;
                 if (!acc) continue;
+                /* value at the downwind faces of the cell: f_c (order 1), extrapolated (order 2, G21) */
+                double Fdn[3];
+                for (int d = 0; d < 3; ++d) Fdn[d] = fc + psi[d] * (fc - f1v[d]);
                 for (int d = 0; d < 3; ++d)
-                    if (zg_face[d] >= 0 && acc->flux_in) acc->flux_in[zg_face[d]] += (long double)(w * fabs(xi[d]) * fc);
+                    if (zg_face[d] >= 0 && acc->flux_in) acc->flux_in[zg_face[d]] += (long double)(w * fabs(xi[d]) * Fdn[d]);
                 /* ---- Step 3: raw moments (Eq.(5)) ---- */
                 if (acc->raw) {
                     const long double wf = (long double)w * (long double)fc;
@@ -349,7 +382,7 @@ static void sweep_one(const odvm_problem *p, const face_tab *t, const double *pr
                     for (int d = 0; d < 3; ++d) {
                         const int dn = 2 * d + (s[d] > 0 ? 1 : 0);
                         const int face = t->face_of[dn][c];
-                        if (face >= 0) acc->flux_out[face] += (long double)(w * fabs(xi[d]) * fc);
+                        if (face >= 0) acc->flux_out[face] += (long double)(w * fabs(xi[d]) * Fdn[d]);
                     }
                 }
             }

@@ -1,6 +1,7 @@
 /*
  * dvm_oracle.h - CPU ORACLE for one outer iteration of the iterative discrete-velocity method of
- * arXiv 1810.00348 (steady 3D3V Shakhov/BGK model equation, first-order upwind sweep).
+ * arXiv 1810.00348 (steady 3D3V Shakhov/BGK model equation, first-order upwind sweep; second-order upwind as the
+ * paper's stated extension).
  *
  * THIS IS TEST INFRASTRUCTURE.  It is a plain, slow, obviously-correct restatement of the paper's
  * scheme (one full 3-D array f[k][j][i] per discrete velocity, direct exp/pow, division, no slices, no
@@ -41,6 +42,7 @@ typedef struct {
     double bc_T[7], bc_rho[7], bc_u[7][3];
     int rescale_mass;               /* 1 = apply the global mass rescale */
     int wall_norm;                  /* 0 = discrete Phi_unit (G4), 1 = analytic constant of Eq.(9) */
+    int order;                      /* 1 = first-order upwind, Eq.(7); 2 = second-order upwind (reading G21) */
 } odvm_problem;
 
 /* number of boundary faces (domain + solid); fills nothing */
@@ -73,7 +75,7 @@ double odvm_total_mass(const odvm_problem *p, const double *rho);
  *   prim8_in  [8][ncell]  rho,ux,uy,uz,T,qx,qy,qz           rho_w_in [nface]
  *   raw13_out [13][ncell] sum w f {1, xi_x,xi_y,xi_z, xx,yy,zz,xy,xz,yz, x|xi|^2,y|xi|^2,z|xi|^2}
  *   prim14_out[14][ncell] rho,ux,uy,uz,T,qx,qy,qz,sxx,syy,szz,sxy,sxz,syz (after the rescale)
- *   rho_w_out [nface], flux_out [nface] = sum_{leaving the domain} w |xi_n| f_cell,
+ *   rho_w_out [nface], flux_out [nface] = sum_{leaving the domain} w |xi_n| f_face (f_face = f_cell for order 1),
  *   flux_in [nface] = sum_{entering} w |xi_n| f_ghost (diagnostic for pin P4),
  *   resid[3] = r_rho, r_mom, r_E;  *scale = mass-rescale factor s (1 if off).
  * Velocities whose weight is exactly 0 are skipped.  nthreads <= 0 -> all OpenMP threads.

@@ -33,7 +33,7 @@ class _Problem(C.Structure):
         ("Kn", C.c_double), ("omega", C.c_double), ("Pr", C.c_double),
         ("bc_type", C.c_int * 7),
         ("bc_T", C.c_double * 7), ("bc_rho", C.c_double * 7), ("bc_u", (C.c_double * 3) * 7),
-        ("rescale_mass", C.c_int), ("wall_norm", C.c_int),
+        ("rescale_mass", C.c_int), ("wall_norm", C.c_int), ("order", C.c_int),
     ]
 
 
@@ -111,6 +111,7 @@ class Oracle:
             for d in range(3):
                 p.bc_u[b][d] = bc.u[d]
         p.rescale_mass, p.wall_norm = wl.rescale_mass, wl.wall_norm
+        p.order = getattr(wl, "order", 1)
         self.p = p
         self.n = wl.n_cells
         self.nface = lib().odvm_num_faces(C.byref(p))

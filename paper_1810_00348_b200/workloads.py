@@ -63,6 +63,7 @@ class Workload:
     rescale_mass: int = 1
     wall_norm: int = 0
     iterations: int = 1
+    order: int = 1          # 1 = first-order upwind Eq.(7); 2 = second-order upwind (G21)
 
     @property
     def nx(self):
