@@ -57,6 +57,11 @@ extern "C" {
 
 #define DVM_OPT_KERNEL    1
 #define DVM_OPT_MAX_F_MBYTES 2 /* tile kernel: cap (MiB) on the f workspace; velocity blocks then sweep in batches (0 = none) */
+#define DVM_OPT_ORDER     5 /* order of the upwind sweep: 1 = Eq.(7) (default); 2 = second-order upwind, the extension PAPER.md:393 names
+                             ("second order by storing three consecutive slices"): Eq.(7) in flux-difference form with the value
+                             at a cell's downwind face extrapolated linearly from the two upwind cell centres (the cell value
+                             where the upwind neighbour is not a fluid cell; reading G21); the wall-incident flux of
+                             Eq.(9) takes the extrapolated face value.  Slice kernel only (two stored slices + the one written) */
 #define DVM_OPT_MAX_CTAS  4 /* tile kernel: cap on the persistent grid (0 = every resident CTA); 1 runs the work items strictly in
                              hand-out order on one CTA - for tests of the dependency protocol, not for speed */
 #define DVM_OPT_TILE_RV   3 /* tile kernel: velocities per thread, 4 (128-thread CTAs, velocity blocks of 16 x 8 x 4 nodes) or 2

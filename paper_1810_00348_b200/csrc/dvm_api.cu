@@ -63,6 +63,7 @@ struct dvm_solver {
     long long max_f_mbytes = 0;   // cap on the f workspace of the tile kernel (0 = none)
     int tile_rv = 0;              // velocities per thread of the tile kernel: 0 = choose, 2, 4
     int max_ctas = 0;             // cap on the persistent grid of the tile kernel (0 = all resident CTAs)
+    int order = 1;                // 1: first-order upwind Eq.(7); 2: second-order upwind
     bool planned = false;
     long long launches = 0;
     // device arrays
@@ -78,7 +79,7 @@ struct dvm_solver {
     std::vector<BlockDesc> blocks;
     BlockDesc *d_blocks = nullptr;
     double *d_fbuf = nullptr;
-    long long fstride = 0;
+    long long fstride = 0, fslice = 0;
     int nb_threads = 128;
     TilePlan tile{};
     unsigned char *d_sflags = nullptr;
@@ -176,6 +177,7 @@ SweepParams sweep_params(dvm_solver *s)
     SweepParams P{};
     P.nx = s->nx; P.ny = s->ny; P.nz = s->nz; P.ncell = s->ncell;
     P.invdx = s->d_invdx; P.invdy = s->d_invdy; P.invdz = s->d_invdz;
+    P.dx = s->d_dx; P.dy = s->d_dy; P.dz = s->d_dz; P.order = s->order; P.fslice = s->fslice;
     P.flags = s->d_flags; P.face_of = s->d_face_of; P.face_slot = s->d_face_slot;
     P.coef = s->d_coef; P.rho_w = s->d_rho_w; P.phi = s->d_phi; P.raw = s->d_raw;
     P.xi_x = s->d_xi[0]; P.xi_y = s->d_xi[1]; P.xi_z = s->d_xi[2];
@@ -262,7 +264,9 @@ int plan(dvm_solver *s)
     if (s->planned) return 0;
     const long long nvel = (long long)s->mx * s->my * s->mz;
     int kernel = s->kernel;
-    if (kernel == DVM_KERNEL_AUTO) kernel = DVM_KERNEL_TILE;
+    if (kernel == DVM_KERNEL_AUTO) kernel = s->order == 2 ? DVM_KERNEL_SLICE : DVM_KERNEL_TILE;
+    if (kernel == DVM_KERNEL_TILE && s->order == 2)
+        return fail(DVM_EINVAL, "the second-order sweep (DVM_OPT_ORDER = 2) is implemented by the slice kernel only");
     s->kernel = kernel;
     int lo[3][2], cnt[3][2];
     for (int d = 0; d < 3; ++d) split_axis(s->xi[d], lo[d], cnt[d]);
@@ -285,7 +289,8 @@ int plan(dvm_solver *s)
             }
         }
         s->fstride = col;
-        const size_t fbytes = (size_t)col * s->nx * s->ny * sizeof(double);
+        s->fslice = s->order == 2 ? (long long)col * s->nx * s->ny : 0;
+        const size_t fbytes = (size_t)col * s->nx * s->ny * sizeof(double) * (s->order == 2 ? 2 : 1);
         s->d_fbuf = (double *)s->dalloc(fbytes);
         if (!s->d_fbuf) return fail(DVM_ENOMEM, "slice workspace of %zu bytes failed", fbytes);
         s->f_bytes = fbytes;
@@ -582,6 +587,12 @@ int dvm_set_option(dvm_solver *s, int option, int value)
         if (s->planned) return fail(DVM_EINVAL, "the tile-kernel variant must be chosen before the first iteration");
         if (value != 0 && value != 2 && value != 4) return fail(DVM_EINVAL, "velocities per thread must be 0 (choose), 2 or 4");
         s->tile_rv = value;
+        return DVM_OK;
+    }
+    if (option == DVM_OPT_ORDER) {
+        if (s->planned) return fail(DVM_EINVAL, "the order of the sweep must be chosen before the first iteration");
+        if (value != 1 && value != 2) return fail(DVM_EINVAL, "the order of the upwind sweep is 1 or 2");
+        s->order = value;
         return DVM_OK;
     }
     if (option == DVM_OPT_MAX_CTAS) {

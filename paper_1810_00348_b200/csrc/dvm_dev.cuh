@@ -31,6 +31,9 @@ struct SweepParams {
     int nx, ny, nz;
     long long ncell;
     const double *invdx, *invdy, *invdz;
+    const double *dx, *dy, *dz;     // cell widths (second-order sweep)
+    int order;                      // 1: first-order upwind Eq.(7); 2: second-order upwind (G21)
+    long long fslice;               // order 2: offset (doubles) of the second stored slice in fbuf
     const unsigned char *flags;     // [ncell]
     const int *face_of;             // [6][ncell], face slot or -1
     const unsigned char *face_slot; // [nface] -> bc slot 0..6

@@ -4,6 +4,12 @@
 // from a 9-double per-cell pack staged row by row in shared memory, and the moment / wall-flux sums
 // (Alg. 3) taken from registers right after each update, so the slice is never re-read.
 // It is the baseline variant; the tile kernel (sweep_tile.cu) is the B200 design.
+//
+// order = 2 (DVM_OPT_ORDER; "extend the first order upwind scheme to second order by storing three
+// consecutive slices"; reading G21 of DESIGN.md): the transport term of Eq.(7) along d becomes a_d (F(c) - F(c1)) with
+// F = value at a cell's downwind face, extrapolated linearly from the two upwind centres (the cell value itself where the
+// upwind neighbour is not a fluid cell).  A second in-place slice keeps level k-2 under level k-1, so with the slice being
+// written this is the paper's three slices; the wall-incident flux of Eq.(9) takes the extrapolated face value.
 #include "dvm_dev.cuh"
 
 namespace dvm {
@@ -56,7 +62,8 @@ __global__ void __launch_bounds__(NB) sweep_slice_kernel(const SweepParams P)
             }
             for (int t = threadIdx.x; t < nx; t += NB) s_flag[t] = P.flags[row + t];
             __syncthreads();
-            double fprev = 0.0;
+            double fprev = 0.0, fprev2 = 0.0;
+            unsigned flprev = 0xffu;   // flags of the cell fprev belongs to
             for (int ii = 0; ii < nx; ++ii) {
                 const int i = sx > 0 ? ii : nx - 1 - ii;
                 const unsigned fl = s_flag[i];
@@ -70,6 +77,9 @@ __global__ void __launch_bounds__(NB) sweep_slice_kernel(const SweepParams P)
                 const double fS = A * exp(-e) * (1.0 + Qc * (2.0 * e - 5.0));
                 const double ax = axx * P.invdx[i];
                 double num = nu * fS, den = nu;
+                const bool o2 = P.order == 2;
+                double px = 0.0, py = 0.0, pz = 0.0;     // psi of reading G21 per direction (0: first order there)
+                double f1x = 0.0, f1y = 0.0, f1z = 0.0;  // value of the first upwind cell per direction
                 // x upwind
                 if (fl & (1u << upx)) {
                     const bool dom = (i == (sx > 0 ? 0 : nx - 1));
@@ -79,7 +89,15 @@ __global__ void __launch_bounds__(NB) sweep_slice_kernel(const SweepParams P)
                         const double g = dom ? (tx == 0 ? P.rho_w[face] * gx : gx) : P.rho_w[face] * gs;
                         num += ax * g; den += ax;
                     }
-                } else { num += ax * fprev; den += ax; }
+                } else if (!o2) { num += ax * fprev; den += ax; }
+                else {
+                    // G21: a_x [(1 + psi) f_c - psi f_c1 - F(c1)], F(c1) = f_c1 + psi_1 (f_c1 - f_c2) if c2 is a fluid cell
+                    const double wc = P.dx[i], w1 = P.dx[i - sx];
+                    px = wc / (wc + w1); f1x = fprev;
+                    double Fup = fprev;
+                    if (!(flprev & (1u << upx))) { const double w2 = P.dx[i - 2 * sx]; Fup = fprev + w1 / (w1 + w2) * (fprev - fprev2); }
+                    num += ax * (px * fprev + Fup); den += ax * (1.0 + px);
+                }
                 // y upwind
                 if (fl & (1u << upy)) {
                     const bool dom = (j == (sy > 0 ? 0 : ny - 1));
@@ -89,7 +107,18 @@ __global__ void __launch_bounds__(NB) sweep_slice_kernel(const SweepParams P)
                         const double g = dom ? (ty == 0 ? P.rho_w[face] * gy : gy) : P.rho_w[face] * gs;
                         num += ay * g; den += ay;
                     }
-                } else { num += ay * col[((long long)(j - sy) * nx + i) * S]; den += ay; }
+                } else if (!o2) { num += ay * col[((long long)(j - sy) * nx + i) * S]; den += ay; }
+                else {
+                    const double f1 = col[((long long)(j - sy) * nx + i) * S];
+                    const double wc = P.dy[j], w1 = P.dy[j - sy];
+                    py = wc / (wc + w1); f1y = f1;
+                    double Fup = f1;
+                    if (!(P.flags[c - (long long)sy * nx] & (1u << upy))) {
+                        const double w2 = P.dy[j - 2 * sy];
+                        Fup = f1 + w1 / (w1 + w2) * (f1 - col[((long long)(j - 2 * sy) * nx + i) * S]);
+                    }
+                    num += ay * (py * f1 + Fup); den += ay * (1.0 + py);
+                }
                 // z upwind: the in-place slice still holds level k -/+ 1 at (i, j)
                 if (fl & (1u << upz)) {
                     const bool dom = (k == (sz > 0 ? 0 : nz - 1));
@@ -99,10 +128,23 @@ __global__ void __launch_bounds__(NB) sweep_slice_kernel(const SweepParams P)
                         const double g = dom ? (tz == 0 ? P.rho_w[face] * gz : gz) : P.rho_w[face] * gs;
                         num += az * g; den += az;
                     }
-                } else { num += az * col[((long long)j * nx + i) * S]; den += az; }
+                } else if (!o2) { num += az * col[((long long)j * nx + i) * S]; den += az; }
+                else {
+                    const double f1 = col[((long long)j * nx + i) * S];
+                    const double wc = P.dz[k], w1 = P.dz[k - sz];
+                    pz = wc / (wc + w1); f1z = f1;
+                    double Fup = f1;
+                    if (!(P.flags[c - (long long)sz * nx * ny] & (1u << upz))) {
+                        const double w2 = P.dz[k - 2 * sz];
+                        Fup = f1 + w1 / (w1 + w2) * (f1 - col[P.fslice + ((long long)j * nx + i) * S]);
+                    }
+                    num += az * (pz * f1 + Fup); den += az * (1.0 + pz);
+                }
                 const double f = num / den;
+                // second slice: level k-1 moves under the value being written (stale where k-1 is not fluid: never read)
+                if (o2) col[P.fslice + ((long long)j * nx + i) * S] = col[((long long)j * nx + i) * S];
                 col[((long long)j * nx + i) * S] = f;
-                fprev = f;
+                fprev2 = fprev; fprev = f; flprev = fl;
 
                 // moments (Eq.(5)) reduced over the warp, one atomic per warp and moment
                 const double wf = w * f;
@@ -118,9 +160,23 @@ __global__ void __launch_bounds__(NB) sweep_slice_kernel(const SweepParams P)
                     for (int q = 0; q < NRAW; ++q) atomicAdd(P.raw + c * 16 + q, m[q]);
                     // wall-incident flux (Eq.(9)): all velocities of the block share the sign of xi_d, so
                     // sum w |xi_d| f = s_d * (first-moment partial)
-                    if (fl & (1u << dnx)) atomicAdd(P.phi + P.face_of[dnx * nc + c], sx * m[1]);
-                    if (fl & (1u << dny)) atomicAdd(P.phi + P.face_of[dny * nc + c], sy * m[2]);
-                    if (fl & (1u << dnz)) atomicAdd(P.phi + P.face_of[dnz * nc + c], sz * m[3]);
+                    if (!o2) {
+                        if (fl & (1u << dnx)) atomicAdd(P.phi + P.face_of[dnx * nc + c], sx * m[1]);
+                        if (fl & (1u << dny)) atomicAdd(P.phi + P.face_of[dny * nc + c], sy * m[2]);
+                        if (fl & (1u << dnz)) atomicAdd(P.phi + P.face_of[dnz * nc + c], sz * m[3]);
+                    }
+                }
+                if (o2 && (fl & ((1u << dnx) | (1u << dny) | (1u << dnz)))) {
+                    // order 2: the flux through a downwind boundary face takes the extrapolated face value (G21); the
+                    // condition is the same for every thread (they all sit in the same cell)
+                    const double hx = warp_sum(w * axx * (f + px * (f - f1x)));
+                    const double hy = warp_sum(w * axy * (f + py * (f - f1y)));
+                    const double hz = warp_sum(w * axz * (f + pz * (f - f1z)));
+                    if (lane == 0) {
+                        if (fl & (1u << dnx)) atomicAdd(P.phi + P.face_of[dnx * nc + c], hx);
+                        if (fl & (1u << dny)) atomicAdd(P.phi + P.face_of[dny * nc + c], hy);
+                        if (fl & (1u << dnz)) atomicAdd(P.phi + P.face_of[dnz * nc + c], hz);
+                    }
                 }
             }
         }

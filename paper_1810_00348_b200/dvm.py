@@ -27,6 +27,7 @@ OPT_KERNEL = 1
 OPT_MAX_F_MBYTES = 2
 OPT_TILE_RV = 3
 OPT_MAX_CTAS = 4
+OPT_ORDER = 5
 
 # every symbol include/dvm.h declares (checked by tests/test_abi.py)
 SYMBOLS = (
@@ -170,7 +171,7 @@ class Solver:
     """dvm_create / dvm_iterate / dvm_moments / dvm_residual (+ support calls) for one workload record."""
 
     def __init__(self, wl, kernel: int = KERNEL_AUTO, device: str = "cuda:0", max_f_mbytes: int = 0, tile_rv: int = 0,
-                 max_ctas: int = 0):
+                 max_ctas: int = 0, order: int = 0):
         import torch
         if not torch.cuda.is_available():
             raise DvmError(ECUDA, "no CUDA device: the DVM solver has no CPU fallback")
@@ -216,6 +217,9 @@ class Solver:
         _check(L.dvm_create(C.byref(g), C.byref(v), C.byref(gas), C.byref(bc), C.byref(dev), C.byref(h)))
         self._h = h
         self.nface = _check(L.dvm_num_faces(h))
+        order = order or getattr(wl, "order", 1)
+        if order != 1:
+            self.set_option(OPT_ORDER, int(order))
         if kernel != KERNEL_AUTO:
             self.set_option(OPT_KERNEL, kernel)
         if max_f_mbytes:
