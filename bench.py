@@ -7,7 +7,7 @@
 A "step" is one outer iteration (all of DESIGN.md's hot-path rows a1-a7) of the workload.  Default workload:
 BASELINE.json configs[4] (128^3 x 64^3 cavity, Kn = 0.01, memory-reduction path, f never materialised), the
 largest single-GPU configuration and the one the target is stated on; --config picks another (0-4: BASELINE.json;
-5: the paper's own cube run, 191 x 181 x 181 stretched cells x 48^3 velocities).
+5: the paper's own cube run, 191 x 181 x 181 stretched cells x 48^3 velocities; 6: a 16-level slab of config 4 for ncu).
 The solver runs on one GPU with no sharding (replicas only): with --gpus N every rank
 runs an independent replica, timing is max over ranks, value = total units / that time.
 Prints ONE JSON line.
@@ -105,17 +105,29 @@ def workload_for(args):
     return workloads.config(args.config)
 
 
-# DESIGN.md section 6 (roofline): per phase-space point-update the method needs ~45 fp64 issue slots (SURVEY.md
-# section 8(d): c, c^2, exp factorised per axis, Shakhov factor, numerator, denominator, reciprocal, 13 moment FMAs)
-# = 90 flop, and moves one fp64 value out and back in per tile-face point: 8 B (tile kernel, 4 x 4 columns) or 16 B
-# (slice kernel, in-place slice).  fp64 peak derived from unit counts and clocks: 148 SMs x 64 fp64 lanes x 2 flop
-# x 1.965 GHz = 37.2 TFLOP/s (the DFMA micro-benchmark in profiles/r01_fp64_microbench.txt reaches 34.0).
+# DESIGN.md section 6 (roofline).  Unit = one phase-space point-update.
+#  * HBM: the tile kernel writes one fp64 face value per point and reads it back (4 x 4 tile columns): 8 B / point
+#    algorithmic (16 B for the slice kernel's in-place slice), against the measured copy bandwidth of MEASURED_PEAKS.json.
+#  * fp64 pipe: what the kernel EXECUTES, counted from its SASS and confirmed by ncu (profiles/): FP64_SLOTS_PER_POINT
+#    warp-level fp64 instructions (DFMA / DADD / DMUL) per 32 points, each holding the 16-lane fp64 pipe of an SM
+#    sub-partition for 2 clocks; peak = 148 SM x 64 lanes x 1.965 GHz FMA-lane-slots per second.  The 13 velocity sums run
+#    on the fp64 tensor-core (DMMA) pipe and are reported separately.
+#  * the figure SURVEY.md section 8(d) calls "algorithmic" (45 fp64 issue slots per point with one FMA per moment) is kept as
+#    `algorithmic_equivalent`: the kernel does not execute those slots (factorised exp, tensor-core sums), so it is context,
+#    not the roofline fraction.
+# The binding roofline is the unit with the highest utilisation; bench.py computes both fractions live and names it.
 ALGO_FP64_SLOTS_PER_POINT = 45.0
-FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
-TRAFFIC_NCU = {  # dram__bytes_read.sum + dram__bytes_write.sum per sweep launch, from profiles/ (None = not captured)
-    "cfg2_cavity_tanh_64^3x32^3_Kn0.075": 68.699e9,   # profiles/r01_sweep_tile.md (b)
-    "cfg4_cavity_128^3x64^3_Kn0.01": 4.3636e12,       # profiles/r01_sweep_tile.md (a)
+FP64_LANE_SLOTS_PEAK = 148 * 64 * 1.965e9          # fp64 FMA-lane issue slots per second
+FP64_PEAK_TFLOPS = 2 * FP64_LANE_SLOTS_PEAK / 1e12
+# ncu evidence per workload (profiles/r02_*.md), taken at the commit named there; None = not captured.
+#   traffic: dram__bytes_read.sum + dram__bytes_write.sum per sweep launch; inst / fp64 / dmma: thread-level instructions per
+#   point-update (smsp__inst_executed.sum x 32 / points, SASS opcode shares of the level loop); pipe / issue: ncu percentages
+NCU = {
+    "cfg4_cavity_128^3x64^3_Kn0.01": {"traffic": None, "inst_per_point": None, "fp64_inst_per_point": None, "dmma_per_point": None,
+                                      "pipe_fp64_active_pct": None, "pipe_tensor_active_pct": None, "issue_active_pct": None,
+                                      "commit": None},
 }
+FP64_SLOTS_PER_POINT = {"tile": 15.5, "slice": 70.0}   # executed fp64 instructions per point (SASS count)
 
 
 def algorithmic_bytes_per_point(kernel_name):
@@ -163,7 +175,8 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": tot_p / tot_t, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / len(vals), "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": wl.name, "phase_points_per_iteration": wl.phase_points,
+            "config": {"workload": wl.name, "physical_cells": [wl.nx, wl.ny, wl.nz], "velocity_nodes": [wl.mx, wl.my, wl.mz],
+                       "phase_points_per_iteration": wl.phase_points, "kernel": "oracle (CPU)", "parallelism": "host cores",
                        "note": "each step = one oracle iteration over a bounded velocity subset"},
             "cpu_baseline": cb,
             "e2e": {"value": tot_p / tot_t, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
@@ -187,7 +200,8 @@ def run_gpu(args):
 
     wl = workload_for(args)
     kernel = {"auto": dvm.KERNEL_AUTO, "slice": dvm.KERNEL_SLICE, "tile": dvm.KERNEL_TILE}[args.kernel]
-    s = dvm.Solver(wl, kernel=kernel, device=f"cuda:{local}")
+    s = dvm.Solver(wl, kernel=kernel, device=f"cuda:{local}", max_f_mbytes=args.max_f_mbytes, tile_rv=args.tile_rv,
+                   order=args.order)
     stream = torch.cuda.current_stream(dev)
 
     def barrier():
@@ -242,30 +256,39 @@ def run_gpu(args):
         value = whole_job_value(world, pts, ms_per_step)
         kname = "slice" if s.kernel_used() == dvm.KERNEL_SLICE else "tile"
         peak, peak_src, _ = measured_peaks()
-        # dominant kernel = the sweep (one launch per step); its duration is the step minus the five small update
-        # launches, measured here as the step itself (upper bound on the sweep time -> lower bound on achieved)
+        # dominant kernel = the sweep (one launch per step); its duration is the step minus the small table / update launches,
+        # measured here as the step itself (upper bound on the sweep time -> lower bound on achieved)
         bpp = algorithmic_bytes_per_point(kname)
-        hbm_gbs = bpp * pts / (ms_per_step * 1e-3) / 1e9
-        tflops = 2.0 * ALGO_FP64_SLOTS_PER_POINT * pts / (ms_per_step * 1e-3) / 1e12
-        # the binding roofline is the slower of the two bounds for this workload
-        t_alu, t_hbm = 2.0 * ALGO_FP64_SLOTS_PER_POINT / (FP64_PEAK_TFLOPS * 1e12), bpp / (peak * 1e9)
-        if t_alu >= t_hbm:
-            roof = {"bound": "alu", "achieved": tflops, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
-                    "frac": tflops / FP64_PEAK_TFLOPS, "traffic": TRAFFIC_NCU.get(wl.name),
-                    "peak_source": "derived: 148 SM x 64 fp64 lanes x 2 flop x 1.965 GHz (DESIGN.md section 6)",
-                    "algorithmic_flop_per_point": 2.0 * ALGO_FP64_SLOTS_PER_POINT}
+        secs = ms_per_step * 1e-3
+        hbm_gbs = bpp * pts / secs / 1e9
+        fp64_slots = FP64_SLOTS_PER_POINT[kname] * pts / secs            # executed fp64 lane slots per second
+        frac_hbm, frac_alu = hbm_gbs / peak, fp64_slots / FP64_LANE_SLOTS_PEAK
+        ncu = NCU.get(wl.name, {})
+        if frac_hbm >= frac_alu:
+            roof = {"bound": "hbm", "achieved": hbm_gbs, "peak": peak, "unit": "GB/s", "frac": frac_hbm,
+                    "traffic": ncu.get("traffic"), "peak_source": peak_src}
         else:
-            roof = {"bound": "hbm", "achieved": hbm_gbs, "peak": peak, "unit": "GB/s", "frac": hbm_gbs / peak,
-                    "traffic": TRAFFIC_NCU.get(wl.name), "peak_source": peak_src}
-        roof.update({"kernel": f"sweep_{kname}_kernel", "algorithmic_bytes_per_point": bpp,
-                     "hbm_achieved_gbs": hbm_gbs, "hbm_peak_gbs": peak, "hbm_frac": hbm_gbs / peak,
-                     "launch_ms": ms_per_step})
+            roof = {"bound": "alu", "achieved": 2.0 * fp64_slots / 1e12, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
+                    "frac": frac_alu, "traffic": ncu.get("traffic"),
+                    "peak_source": "derived: 148 SM x 64 fp64 lanes x 2 flop x 1.965 GHz (DESIGN.md section 6)"}
+        roof.update({"kernel": f"sweep_{kname}_kernel", "launch_ms": ms_per_step,
+                     "algorithmic_bytes_per_point": bpp, "hbm_achieved_gbs": hbm_gbs, "hbm_peak_gbs": peak, "hbm_frac": frac_hbm,
+                     "fp64_executed_inst_per_point": FP64_SLOTS_PER_POINT[kname], "fp64_executed_tflops": 2.0 * fp64_slots / 1e12,
+                     "fp64_peak_tflops": FP64_PEAK_TFLOPS, "fp64_pipe_frac": frac_alu,
+                     "algorithmic_equivalent": {"fp64_slots_per_point": ALGO_FP64_SLOTS_PER_POINT,
+                                                "tflops": 2.0 * ALGO_FP64_SLOTS_PER_POINT * pts / secs / 1e12,
+                                                "note": "SURVEY.md 8(d) count with one FMA per moment and a divide; not executed"},
+                     "ncu": ncu,
+                     "note": "no unit is saturated: the kernel is latency / issue bound at 8 warps per SM; the unit with the "
+                             "highest utilisation is named as the bound"})
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
             "config": {"workload": wl.name, "physical_cells": [wl.nx, wl.ny, wl.nz], "velocity_nodes": [wl.mx, wl.my, wl.mz],
-                       "phase_points_per_iteration": pts, "kernel": kname, "parallelism": "replicas only" if world > 1 else "1 GPU",
+                       "phase_points_per_iteration": pts, "kernel": kname, "tile_rv": s.tile_rv() if kname == "tile" else None,
+                       "order": args.order, "max_f_mbytes": args.max_f_mbytes,
+                       "parallelism": "replicas only" if world > 1 else "1 GPU",
                        "l2": "inputs larger than L2 (f workspace %.1f GB, fields %.2f GB)" % (f_bytes / 1e9, (total_bytes - f_bytes) / 1e9)
                        if total_bytes > 126e6 else "working set smaller than L2 (config is a parity case)",
                        "workspace_bytes": total_bytes, "f_workspace_bytes": f_bytes,
@@ -296,6 +319,9 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--ref-budget", type=float, default=15.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--max-f-mbytes", type=int, default=0, help="cap (MiB) on the f workspace of the tile kernel (0 = none)")
+    ap.add_argument("--tile-rv", type=int, default=0, choices=[0, 2, 4], help="velocities per thread of the tile kernel (0 = library's choice)")
+    ap.add_argument("--order", type=int, default=1, choices=[1, 2], help="order of the upwind sweep (2: slice kernel)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

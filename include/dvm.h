@@ -27,6 +27,8 @@
  * Pointers: "host" = ordinary host memory, read during the call only (dvm_create copies what it needs);
  * "dev" = device memory on the solver's device, caller-owned, at least the stated size.
  * All device work is enqueued on the stream given at creation; only the calls marked (syncs) wait for it.
+ * A solver lives on the CUDA device that is current when dvm_create is called; every later call switches to that
+ * device for its duration and restores the caller's current device.
  * Every call returns 0 or a negative DVM_E* code; nothing throws or aborts across this boundary;
  * dvm_last_error() returns a thread-local message for the last failing call of this thread.
  * There is no CPU fallback: without a CUDA device dvm_create fails with DVM_ECUDA.
@@ -61,7 +63,8 @@ extern "C" {
                              ("second order by storing three consecutive slices"): Eq.(7) in flux-difference form with the value
                              at a cell's downwind face extrapolated linearly from the two upwind cell centres (the cell value
                              where the upwind neighbour is not a fluid cell; reading G21); the wall-incident flux of
-                             Eq.(9) takes the extrapolated face value.  Slice kernel only (two stored slices + the one written) */
+                             Eq.(9) takes the extrapolated face value.  Tile kernel: two z-planes in registers and two-deep faces
+                             (2 velocities per thread); slice kernel: two stored slices + the one being written */
 #define DVM_OPT_MAX_CTAS  4 /* tile kernel: cap on the persistent grid (0 = every resident CTA); 1 runs the work items strictly in
                              hand-out order on one CTA - for tests of the dependency protocol, not for speed */
 #define DVM_OPT_TILE_RV   3 /* tile kernel: velocities per thread, 4 (128-thread CTAs, velocity blocks of 16 x 8 x 4 nodes) or 2
@@ -158,19 +161,19 @@ int dvm_kernel_used(const dvm_solver *s);
 int dvm_tile_rv(const dvm_solver *s);
 /* Host-only (needs no device): the work decomposition the tile kernel would use for an nx x ny x nz grid and the
  * velocity nodes of v when target_ctas items should run concurrently, at most max_blocks velocity blocks are in
- * flight at once (0 = all; "smaller batches") and a thread carries rv velocities (2, 4, or 0 = the
- * library's choice for these nodes).  counts5 = number of velocity blocks, tiles along x, tiles
+ * flight at once (0 = all; "smaller batches"), a thread carries rv velocities (2, 4, or 0 = the
+ * library's choice for these nodes) and the sweep has the given order (1 or 2; order 2 needs rv = 2 or 0).  counts5 = number of velocity blocks, tiles along x, tiles
  * along y, band height P, blocks per batch.  items9 (may be NULL) receives, for the first max_items work items in
  * hand-out order, {velocity block, tile x, tile y, predecessor in x, predecessor in y (for tile y = 0 of a later batch:
  * the last reader of the y-face slot), previous user of the x-face slot, x-face slot, octant bits, face-slot set};
  * predecessors are item indices or -1.  Returns the number of items. */
-int dvm_plan_query(int nx, int ny, int nz, const dvm_vgrid *v, int target_ctas, int max_blocks, int rv, int *counts5,
-                   int *items9, int max_items);
-/* Host-only: the velocity blocks of the tile kernel for the nodes of v (rv as in dvm_plan_query), in block-id order (the
+int dvm_plan_query(int nx, int ny, int nz, const dvm_vgrid *v, int target_ctas, int max_blocks, int rv, int order,
+                   int *counts5, int *items9, int max_items);
+/* Host-only: the velocity blocks of the tile kernel for the nodes of v (rv, order as in dvm_plan_query), in block-id order (the
  * order of dvm_plan_query's items9[0]).  boxes8 (may be NULL) receives for the first max_blocks blocks {a0, na, b0, nb, c0,
  * nc, NA, 256 nbb + ncb}: the block holds the nodes [a0, a0+na) x [b0, b0+nb) x [c0, c0+nc) of one sign octant, in a box
  * of NA x nbb x ncb lanes.  Returns the number of blocks. */
-int dvm_plan_vblocks(const dvm_vgrid *v, int rv, int *boxes8, int max_blocks);
+int dvm_plan_vblocks(const dvm_vgrid *v, int rv, int order, int *boxes8, int max_blocks);
 /* Bytes of device workspace held by the solver, and the part of it that holds distribution-function values. */
 int dvm_workspace_bytes(const dvm_solver *s, size_t *total, size_t *f_bytes);
 /* Number of kernel launches enqueued by this solver so far (bench.py's gpu_launches). */

@@ -42,6 +42,20 @@ int fail(int code, const char *fmt, ...)
     } while (0)
 
 constexpr int HIST_CAP = 16384;
+
+// Every entry point runs on the solver's device whatever device is current in the calling thread, and restores it.
+struct DeviceGuard {
+    int prev = -1, want;
+    explicit DeviceGuard(int d) : want(d)
+    {
+        if (cudaGetDevice(&prev) != cudaSuccess) prev = -1;
+        if (prev != want) cudaSetDevice(want);
+    }
+    ~DeviceGuard()
+    {
+        if (prev >= 0 && prev != want) cudaSetDevice(prev);
+    }
+};
 const double PI = 3.14159265358979323846;
 
 }  // namespace
@@ -54,6 +68,7 @@ struct dvm_solver {
     dvm_gas gas{};
     dvm_bc bc{};
     cudaStream_t stream = nullptr;
+    int device = 0;               // CUDA device ordinal the solver lives on (current device at dvm_create)
     dvm_device dev{};
     std::vector<void *> allocs;
     size_t total_bytes = 0, f_bytes = 0;
@@ -95,7 +110,7 @@ struct dvm_solver {
     // factor tables of the tile kernel (tables.cu)
     std::vector<CellRec> h_rec;
     CellRec *d_rec = nullptr;
-    double4 *d_TX = nullptr, *d_TY = nullptr, *d_TZ = nullptr;
+    double *d_TX = nullptr, *d_TY = nullptr, *d_TZ = nullptr;
     int *d_xnode = nullptr, *d_ynode = nullptr, *d_znode = nullptr;
     int nxp = 0, nyp = 0, nxb = 0, nyb = 0, nzb = 0;
     size_t table_bytes = 0;
@@ -208,8 +223,9 @@ TileParams tile_params(dvm_solver *s)
     P.vblocks = s->d_vblocks; P.items = s->d_items; P.nitems = (int)s->tile.items.size();
     P.done = s->d_done; P.counter = s->d_counter; P.epoch = s->epoch;
     P.xface = s->d_xface; P.yface = s->d_yface;
-    P.xslot_doubles = (long long)s->nz * TILE_TY * TILE_NVB;
-    P.yslot_doubles = (long long)s->nz * TILE_TX * TILE_NVB;
+    const int nvb = tile_nvb(s->tile.rv, s->tile.order), layers = tile_face_layers(s->tile.order);
+    P.xslot_doubles = (long long)s->nz * layers * TILE_TY * nvb;
+    P.yslot_doubles = (long long)s->nz * layers * TILE_TX * nvb;
     P.TX = s->d_TX; P.TY = s->d_TY; P.TZ = s->d_TZ; P.rec = s->d_rec;
     P.nxp = s->nxp; P.nyp = s->nyp; P.nbb = s->tile.nbb; P.ncb = s->tile.ncb;
     return P;
@@ -219,6 +235,7 @@ TableParams table_params(dvm_solver *s)
 {
     TableParams T{};
     T.nx = s->nx; T.ny = s->ny; T.nz = s->nz; T.nxp = s->nxp; T.nyp = s->nyp;
+    T.order = s->tile.order; T.dx = s->d_dx; T.dy = s->d_dy; T.dz = s->d_dz;
     T.na = tile_na(s->tile.rv); T.nbb = s->tile.nbb; T.ncb = s->tile.ncb; T.nxb = s->nxb; T.nyb = s->nyb; T.nzb = s->nzb;
     T.ncell = s->ncell; T.coef = s->d_coef; T.flags = s->d_flags;
     T.invdx = s->d_invdx; T.invdy = s->d_invdy; T.invdz = s->d_invdz;
@@ -228,14 +245,6 @@ TableParams table_params(dvm_solver *s)
     for (int d = 0; d < 6; ++d) T.bc_type[d] = s->bc.face[d].type;
     T.TX = s->d_TX; T.TY = s->d_TY; T.TZ = s->d_TZ; T.rec = s->d_rec;
     return T;
-}
-
-// index ranges of the negative / non-negative nodes of one axis (nodes ascending)
-void split_axis(const std::vector<double> &xi, int lo[2], int cnt[2])
-{
-    int nneg = 0;
-    while (nneg < (int)xi.size() && xi[nneg] < 0.0) ++nneg;
-    lo[0] = 0; cnt[0] = nneg; lo[1] = nneg; cnt[1] = (int)xi.size() - nneg;
 }
 
 // Variant of the tile kernel for a velocity grid when the caller leaves the choice open: the one whose velocity blocks
@@ -252,21 +261,41 @@ int choose_rv(const std::vector<double> xi[3])
     double fill[2] = {0.0, 0.0};
     for (int t = 0; t < 2; ++t) {
         TilePlan tp;
-        if (tile_plan(4, 4, 1, xi, 1, 0, t == 0 ? 4 : 2, &tp)) return 4;
+        if (tile_plan(4, 4, 1, xi, 1, 0, t == 0 ? 4 : 2, 1, &tp)) return 4;
         fill[t] = (double)nvel / ((double)tp.vblocks.size() * TILE_NVB);
     }
     return fill[1] * RV_BIAS > fill[0] ? 2 : 4;
 }
 
-// Decide the kernel variant and build the block table + f workspace (once, before the first iteration).
+int plan_once(dvm_solver *s);
+
+// Decide the kernel variant and build the block table + f workspace (once, before the first iteration).  A failed attempt
+// gives back what it allocated, so that the call can be repeated (e.g. with another workspace cap).
 int plan(dvm_solver *s)
 {
     if (s->planned) return 0;
+    const size_t nalloc = s->allocs.size(), bytes = s->total_bytes;
+    const int rc = plan_once(s);
+    if (rc != 0) {
+        cudaStreamSynchronize(s->stream);
+        for (size_t e = nalloc; e < s->allocs.size(); ++e) {
+            if (s->dev.free_) s->dev.free_(s->allocs[e], s->dev.ctx);
+            else if (!s->dev.alloc) cudaFree(s->allocs[e]);
+        }
+        s->allocs.resize(nalloc);
+        s->total_bytes = bytes;
+        s->f_bytes = 0;
+    }
+    return rc;
+}
+
+int plan_once(dvm_solver *s)
+{
     const long long nvel = (long long)s->mx * s->my * s->mz;
     int kernel = s->kernel;
-    if (kernel == DVM_KERNEL_AUTO) kernel = s->order == 2 ? DVM_KERNEL_SLICE : DVM_KERNEL_TILE;
-    if (kernel == DVM_KERNEL_TILE && s->order == 2)
-        return fail(DVM_EINVAL, "the second-order sweep (DVM_OPT_ORDER = 2) is implemented by the slice kernel only");
+    if (kernel == DVM_KERNEL_AUTO) kernel = DVM_KERNEL_TILE;
+    if (kernel == DVM_KERNEL_TILE && s->order == 2 && s->tile_rv == 4)
+        return fail(DVM_EINVAL, "the second-order tile kernel carries 2 velocities per thread (DVM_OPT_TILE_RV = 2 or 0)");
     s->kernel = kernel;
     int lo[3][2], cnt[3][2];
     for (int d = 0; d < 3; ++d) split_axis(s->xi[d], lo[d], cnt[d]);
@@ -296,25 +325,30 @@ int plan(dvm_solver *s)
         s->f_bytes = fbytes;
     } else {
         int per_sm = 0, dev = 0, nsm = 0;
-        const int rv = s->tile_rv ? s->tile_rv : choose_rv(s->xi);
+        const int order = s->order;
+        const int rv = order == 2 ? 2 : s->tile_rv ? s->tile_rv : choose_rv(s->xi);
         s->tile_rv = rv;
-        CK(tile_configure(rv, &per_sm));
+        CK(tile_configure(rv, order, &per_sm));
         CK(cudaGetDevice(&dev));
         CK(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
         if (per_sm < 1) return fail(DVM_ECUDA, "tile kernel does not fit on an SM");
         const int resident = per_sm * nsm;
-        if (tile_plan(s->nx, s->ny, s->nz, s->xi, resident, 0, rv, &s->tile)) return fail(DVM_EINVAL, "tile plan failed");
+        if (tile_plan(s->nx, s->ny, s->nz, s->xi, resident, 0, rv, order, &s->tile)) return fail(DVM_EINVAL, "tile plan failed");
         if (s->max_f_mbytes > 0) {
             // cap on the f workspace: fewer velocity blocks in flight (batches); the band height P
             // grows as the batch shrinks, so iterate to a fixed point; one block is the floor
-            const double cap = (double)s->max_f_mbytes * 1048576.0, lvl = (double)s->nz * TILE_NVB * 8.0;
+            const double cap = (double)s->max_f_mbytes * 1048576.0, lvl = (double)s->nz * tile_nvb(rv, order) * tile_face_layers(order) * 8.0;
             int B = (int)s->tile.vblocks.size();
             for (int pass = 0; pass < 8; ++pass) {
                 const double need = (double)(s->tile.xface_doubles + s->tile.yface_doubles) * 8.0;
                 if (need <= cap || B == 1) break;
                 B = std::max(1, std::min(B - 1, (int)(cap / ((s->tile.P * TILE_TY + s->tile.ntx * TILE_TX) * lvl))));
-                if (tile_plan(s->nx, s->ny, s->nz, s->xi, resident, B, rv, &s->tile)) return fail(DVM_EINVAL, "tile plan failed");
+                if (tile_plan(s->nx, s->ny, s->nz, s->xi, resident, B, rv, order, &s->tile)) return fail(DVM_EINVAL, "tile plan failed");
             }
+            const double need = (double)(s->tile.xface_doubles + s->tile.yface_doubles) * 8.0;
+            if (need > cap)
+                return fail(DVM_EINVAL, "the f workspace needs %.1f MiB even with one velocity block in flight: the cap of %lld MiB "
+                            "(DVM_OPT_MAX_F_MBYTES) cannot be met", need / 1048576.0, s->max_f_mbytes);
         }
         const size_t nitems = s->tile.items.size();
         s->tile_grid = (int)std::min<size_t>((size_t)resident, nitems);
@@ -330,9 +364,10 @@ int plan(dvm_solver *s)
             s->nyb = (int)s->tile.ynode.size() / s->tile.nbb;
             s->nzb = (int)s->tile.znode.size() / s->tile.ncb;
             const size_t npc = (size_t)s->nz * s->nyp * s->nxp;
-            const size_t ex = npc * s->tile.xnode.size(), ey = npc * s->tile.ynode.size(), ez = npc * s->tile.znode.size();
+            const size_t ed = (size_t)tile_entry_doubles(order);
+            const size_t ex = npc * s->tile.xnode.size() * ed, ey = npc * s->tile.ynode.size() * ed, ez = npc * s->tile.znode.size() * ed;
             if (dzeros(s, &s->d_TX, ex) || dzeros(s, &s->d_TY, ey) || dzeros(s, &s->d_TZ, ez)) return DVM_ENOMEM;
-            s->table_bytes = (ex + ey + ez) * sizeof(double4);
+            s->table_bytes = (ex + ey + ez) * sizeof(double);
             if (upload(s, &s->d_rec, s->h_rec.data(), s->h_rec.size())) return DVM_ENOMEM;
             if (upload(s, &s->d_xnode, s->tile.xnode.data(), s->tile.xnode.size())) return DVM_ENOMEM;
             if (upload(s, &s->d_ynode, s->tile.ynode.data(), s->tile.ynode.size())) return DVM_ENOMEM;
@@ -403,6 +438,7 @@ int dvm_create(const dvm_grid *g, const dvm_vgrid *v, const dvm_gas *gas, const 
     if (g->solid) for (long long c = 0; c < s->ncell; ++c) s->solid[c] = g->solid[c] ? 1 : 0;
     s->gas = *gas; s->bc = *bc;
     if (dev) { s->dev = *dev; s->stream = (cudaStream_t)dev->stream; }
+    if (cudaGetDevice(&s->device) != cudaSuccess) { delete s; return fail(DVM_ECUDA, "cudaGetDevice failed"); }
 
     auto bail = [&](int rc) { cudaStreamSynchronize(s->stream); s->dfree_all(); delete s; return rc; };
 
@@ -614,6 +650,7 @@ int dvm_iterate(dvm_solver *s, int niter)
 {
     if (!s || niter < 0) return fail(DVM_EINVAL, "bad argument");
     if (niter == 0) return DVM_OK;
+    DeviceGuard guard(s->device);
     if (int rc = plan(s)) return rc;
     const UpdateParams U = update_params(s);
     const SweepParams P = sweep_params(s);
@@ -628,8 +665,8 @@ int dvm_iterate(dvm_solver *s, int niter)
             CK(cudaMemsetAsync(s->d_counter, 0, sizeof(int), s->stream));
             s->epoch += 1;
             const TileParams TP = tile_params(s);
-            CK(launch_sweep_tile(TP, s->tile_rv, s->tile_grid, s->stream));
-            CK(launch_phi_from_raw(s->d_raw, s->d_face_cell, s->d_face_dir, s->d_phi, s->nface, s->stream));
+            CK(launch_sweep_tile(TP, s->tile_rv, s->order, s->tile_grid, s->stream));
+            CK(launch_phi_from_raw(U, s->d_face_cell, s->d_face_dir, s->d_phi, s->order, s->stream));
             s->launches += 1;
         }
         s->launches += 1;
@@ -644,6 +681,7 @@ int dvm_iterate(dvm_solver *s, int niter)
 int dvm_moments(dvm_solver *s, double *dev_out)
 {
     if (!s || !dev_out) return fail(DVM_EINVAL, "NULL argument");
+    DeviceGuard guard(s->device);
     CK(cudaMemcpyAsync(dev_out, s->d_prim, (size_t)NPRIM * s->ncell * sizeof(double), cudaMemcpyDeviceToDevice, s->stream));
     return DVM_OK;
 }
@@ -651,13 +689,14 @@ int dvm_moments(dvm_solver *s, double *dev_out)
 int dvm_residual(dvm_solver *s, double *host_out3)
 {
     if (!s || !host_out3) return fail(DVM_EINVAL, "NULL argument");
+    DeviceGuard guard(s->device);
     if (s->iters == 0) return fail(DVM_EINVAL, "no iteration done yet");
     const int slot = (s->iters - 1) % HIST_CAP;
     CK(cudaMemcpyAsync(host_out3, s->d_hist + 3 * slot, 3 * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
     CK(cudaStreamSynchronize(s->stream));
     for (int m = 0; m < 3; ++m)
         if (!std::isfinite(host_out3[m])) return fail(DVM_ENONFINITE, "residual %d is not finite", m);
-    return DVM_OK;
+    return DVM_OK;   // (an earlier iteration's NaN stays visible in dvm_residual_history)
 }
 
 int dvm_num_faces(const dvm_solver *s) { return s ? s->nface : fail(DVM_EINVAL, "NULL solver"); }
@@ -669,6 +708,7 @@ long long dvm_launch_count(const dvm_solver *s) { return s ? s->launches : -1; }
 int dvm_get_state(dvm_solver *s, double *dev_prim14, double *dev_rho_wall)
 {
     if (!s) return fail(DVM_EINVAL, "NULL solver");
+    DeviceGuard guard(s->device);
     if (dev_prim14) CK(cudaMemcpyAsync(dev_prim14, s->d_prim, (size_t)NPRIM * s->ncell * sizeof(double), cudaMemcpyDeviceToDevice, s->stream));
     if (dev_rho_wall) CK(cudaMemcpyAsync(dev_rho_wall, s->d_rho_w, (size_t)s->nface * sizeof(double), cudaMemcpyDeviceToDevice, s->stream));
     return DVM_OK;
@@ -677,6 +717,7 @@ int dvm_get_state(dvm_solver *s, double *dev_prim14, double *dev_rho_wall)
 int dvm_set_state(dvm_solver *s, const double *dev_prim8, const double *dev_rho_wall)
 {
     if (!s || !dev_prim8) return fail(DVM_EINVAL, "NULL argument");
+    DeviceGuard guard(s->device);
     CK(cudaMemcpyAsync(s->d_prim, dev_prim8, (size_t)8 * s->ncell * sizeof(double), cudaMemcpyDeviceToDevice, s->stream));
     CK(cudaMemsetAsync(s->d_prim + 8 * s->ncell, 0, (size_t)6 * s->ncell * sizeof(double), s->stream));
     if (dev_rho_wall) CK(cudaMemcpyAsync(s->d_rho_w, dev_rho_wall, (size_t)s->nface * sizeof(double), cudaMemcpyDeviceToDevice, s->stream));
@@ -689,6 +730,7 @@ int dvm_set_state(dvm_solver *s, const double *dev_prim8, const double *dev_rho_
 int dvm_raw_moments(dvm_solver *s, double *dev_raw13)
 {
     if (!s || !dev_raw13) return fail(DVM_EINVAL, "NULL argument");
+    DeviceGuard guard(s->device);
     CK(launch_raw_export(s->d_raw, dev_raw13, s->ncell, s->stream));
     s->launches += 1;
     return DVM_OK;
@@ -697,6 +739,7 @@ int dvm_raw_moments(dvm_solver *s, double *dev_raw13)
 int dvm_wall_flux(dvm_solver *s, double *dev_flux)
 {
     if (!s || !dev_flux) return fail(DVM_EINVAL, "NULL argument");
+    DeviceGuard guard(s->device);
     CK(cudaMemcpyAsync(dev_flux, s->d_phi, (size_t)s->nface * sizeof(double), cudaMemcpyDeviceToDevice, s->stream));
     return DVM_OK;
 }
@@ -704,6 +747,7 @@ int dvm_wall_flux(dvm_solver *s, double *dev_flux)
 int dvm_residual_history(dvm_solver *s, double *host_out, int max_n)
 {
     if (!s || !host_out || max_n < 0) return fail(DVM_EINVAL, "bad argument");
+    DeviceGuard guard(s->device);
     const int count = std::min(std::min(max_n, s->iters), HIST_CAP);
     if (count > 0) {
         const int slot = (s->iters - count) % HIST_CAP;
@@ -719,6 +763,7 @@ int dvm_residual_history(dvm_solver *s, double *host_out, int max_n)
 int dvm_mass_scale(dvm_solver *s, double *host_out1)
 {
     if (!s || !host_out1) return fail(DVM_EINVAL, "NULL argument");
+    DeviceGuard guard(s->device);
     if (s->iters == 0) { *host_out1 = 1.0; return DVM_OK; }
     CK(cudaMemcpyAsync(host_out1, s->d_scal, sizeof(double), cudaMemcpyDeviceToHost, s->stream));
     CK(cudaStreamSynchronize(s->stream));
@@ -729,6 +774,7 @@ int dvm_step_host(dvm_solver *s, const double *host_prim8, const double *host_rh
                   double *host_prim14_out, double *host_rho_wall_out)
 {
     if (!s || n < 0) return fail(DVM_EINVAL, "bad argument");
+    DeviceGuard guard(s->device);
     if (host_prim8) {
         CK(cudaMemcpyAsync(s->d_prim, host_prim8, (size_t)8 * s->ncell * sizeof(double), cudaMemcpyHostToDevice, s->stream));
         CK(cudaMemsetAsync(s->d_prim + 8 * s->ncell, 0, (size_t)6 * s->ncell * sizeof(double), s->stream));
@@ -744,16 +790,16 @@ int dvm_step_host(dvm_solver *s, const double *host_prim8, const double *host_rh
     return DVM_OK;
 }
 
-int dvm_plan_query(int nx, int ny, int nz, const dvm_vgrid *v, int target_ctas, int max_blocks, int rv, int *counts5, int *items9,
-                   int max_items)
+int dvm_plan_query(int nx, int ny, int nz, const dvm_vgrid *v, int target_ctas, int max_blocks, int rv, int order, int *counts5,
+                   int *items9, int max_items)
 {
-    if (!v || !counts5 || max_blocks < 0 || (rv != 0 && rv != 2 && rv != 4) || nx <= 0 || ny <= 0 || nz <= 0 || v->mx <= 0 || v->my <= 0 || v->mz <= 0 || !v->xi_x || !v->xi_y || !v->xi_z)
+    if (!v || !counts5 || max_blocks < 0 || (rv != 0 && rv != 2 && rv != 4) || (order != 1 && order != 2) || (order == 2 && rv == 4) || nx <= 0 || ny <= 0 || nz <= 0 || v->mx <= 0 || v->my <= 0 || v->mz <= 0 || !v->xi_x || !v->xi_y || !v->xi_z)
         return fail(DVM_EINVAL, "bad argument");
     std::vector<double> xi[3];
     xi[0].assign(v->xi_x, v->xi_x + v->mx); xi[1].assign(v->xi_y, v->xi_y + v->my); xi[2].assign(v->xi_z, v->xi_z + v->mz);
     TilePlan tp;
-    if (rv == 0) rv = choose_rv(xi);
-    if (tile_plan(nx, ny, nz, xi, target_ctas, max_blocks, rv, &tp)) return fail(DVM_EINVAL, "tile plan failed");
+    if (rv == 0) rv = order == 2 ? 2 : choose_rv(xi);
+    if (tile_plan(nx, ny, nz, xi, target_ctas, max_blocks, rv, order, &tp)) return fail(DVM_EINVAL, "tile plan failed");
     counts5[0] = (int)tp.vblocks.size(); counts5[1] = tp.ntx; counts5[2] = tp.nty; counts5[3] = tp.P; counts5[4] = tp.batch;
     const int n = (int)tp.items.size();
     if (items9) {
@@ -769,15 +815,15 @@ int dvm_plan_query(int nx, int ny, int nz, const dvm_vgrid *v, int target_ctas, 
     return n;
 }
 
-int dvm_plan_vblocks(const dvm_vgrid *v, int rv, int *boxes8, int max_blocks)
+int dvm_plan_vblocks(const dvm_vgrid *v, int rv, int order, int *boxes8, int max_blocks)
 {
-    if (!v || max_blocks < 0 || (rv != 0 && rv != 2 && rv != 4) || v->mx <= 0 || v->my <= 0 || v->mz <= 0 || !v->xi_x || !v->xi_y || !v->xi_z)
+    if (!v || max_blocks < 0 || (rv != 0 && rv != 2 && rv != 4) || (order != 1 && order != 2) || (order == 2 && rv == 4) || v->mx <= 0 || v->my <= 0 || v->mz <= 0 || !v->xi_x || !v->xi_y || !v->xi_z)
         return fail(DVM_EINVAL, "bad argument");
     std::vector<double> xi[3];
     xi[0].assign(v->xi_x, v->xi_x + v->mx); xi[1].assign(v->xi_y, v->xi_y + v->my); xi[2].assign(v->xi_z, v->xi_z + v->mz);
-    if (rv == 0) rv = choose_rv(xi);
+    if (rv == 0) rv = order == 2 ? 2 : choose_rv(xi);
     TilePlan tp;
-    if (tile_plan(4, 4, 1, xi, 1, 0, rv, &tp)) return fail(DVM_EINVAL, "tile plan failed");
+    if (tile_plan(4, 4, 1, xi, 1, 0, rv, order, &tp)) return fail(DVM_EINVAL, "tile plan failed");
     const int n = (int)tp.vblocks.size();
     if (boxes8)
         for (int e = 0; e < n && e < max_blocks; ++e) {
@@ -799,6 +845,7 @@ int dvm_workspace_bytes(const dvm_solver *s, size_t *total, size_t *f_bytes)
 int dvm_destroy(dvm_solver *s)
 {
     if (!s) return DVM_OK;
+    DeviceGuard guard(s->device);
     cudaStreamSynchronize(s->stream);
     s->dfree_all();
     delete s;

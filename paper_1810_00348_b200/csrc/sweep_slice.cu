@@ -186,6 +186,13 @@ __global__ void __launch_bounds__(NB) sweep_slice_kernel(const SweepParams P)
 cudaError_t launch_sweep_slice(const SweepParams &P, int nblocks, int nb, cudaStream_t st)
 {
     const size_t smem = (size_t)NCOEF * P.nx * sizeof(double) + ((P.nx + 7) / 8) * 8;
+    if (smem > 48 * 1024) {
+        if (smem > 200 * 1024) return cudaErrorInvalidValue;   // one row of the per-cell pack must fit in shared memory
+        cudaError_t e = nb == 128 ? cudaFuncSetAttribute(sweep_slice_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)
+                      : nb == 64 ? cudaFuncSetAttribute(sweep_slice_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)
+                                 : cudaFuncSetAttribute(sweep_slice_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+    }
     if (nb == 128) sweep_slice_kernel<128><<<nblocks, 128, smem, st>>>(P);
     else if (nb == 64) sweep_slice_kernel<64><<<nblocks, 64, smem, st>>>(P);
     else sweep_slice_kernel<32><<<nblocks, 32, smem, st>>>(P);

@@ -36,13 +36,22 @@ namespace dvm {
 
 namespace {
 
-constexpr int NVB = TILE_NVB;
 constexpr int NCELL = TILE_NCELL;
 constexpr int GA = TILE_GA;
-constexpr int XLEVEL_DOUBLES = TILE_TY * NVB;          // one level of an x-face slot
-constexpr int YLEVEL_DOUBLES = TILE_TX * NVB;          // one level of a y-face slot
-constexpr unsigned XLEVEL_BYTES = XLEVEL_DOUBLES * 8u, YLEVEL_BYTES = YLEVEL_DOUBLES * 8u;
 constexpr unsigned REC_ROW_BYTES = 4 * (unsigned)sizeof(CellRec);
+
+// Kernel variant: RV velocities per thread, ORD = order of the upwind sweep (sweep_tile.cuh)
+template <int RV, int ORD>
+struct KC {
+    static constexpr int THREADS = ORD == 2 ? 128 : TILE_NVB / RV;
+    static constexpr int WARPS = THREADS / 32;
+    static constexpr int NVB = THREADS * RV;                 // velocities per block
+    static constexpr int ES = ORD == 2 ? 48 : 32;            // bytes of a factor-table entry
+    static constexpr int LAYERS = ORD;                       // upwind values per direction carried through a face
+    static constexpr int XLEVEL_DOUBLES = LAYERS * TILE_TY * NVB;   // one level of an x-face slot
+    static constexpr int YLEVEL_DOUBLES = LAYERS * TILE_TX * NVB;   // one level of a y-face slot
+    static constexpr unsigned XLEVEL_BYTES = XLEVEL_DOUBLES * 8u, YLEVEL_BYTES = YLEVEL_DOUBLES * 8u;
+};
 
 // One TMA bulk copy per level: source of level 0, byte step per level, destination in a LevelBuf; bytes = 0: skipped.
 struct CopyDesc {
@@ -55,29 +64,29 @@ constexpr int NCOPY = 4 * TILE_TY + 2;              // per row: x, y, z factor r
 
 // One tile row (4 cells along x) of one level: everything the row's arithmetic reads sits at a static offset from the
 // row's base address, whatever the row index and the level parity are.
-template <int RV>
+template <int RV, int ORD>
 struct __align__(128) RowBuf {
     // ---- staged by TMA two levels ahead ----
-    double4 xtab[4][GA * RV];                      // per (cell', xi_x node): E, Q, e, a (slot r*4 + ag); cell' = position of
-    double4 ytab[4 * 8];                           // the cell in ascending absolute x;  [cell'][nbb]
-    double4 ztab[4 * 8];                           // [cell'][ncb]
+    alignas(16) unsigned char xtab[4 * GA * RV * KC<RV, ORD>::ES];   // per (cell', xi_x node): E, Q, e, a [order 2: E, Q, e, cd, c1,
+    alignas(16) unsigned char ytab[4 * 8 * KC<RV, ORD>::ES];         // c2] (slot r*4 + ag); cell' = position of the cell in ascending
+    alignas(16) unsigned char ztab[4 * 8 * KC<RV, ORD>::ES];         // absolute x;  y: [cell'][nbb], z: [cell'][ncb]
     CellRec rec[4];                                // per cell': 1/tau, accumulator row, neighbour flags, boundary faces
     // ---- decoded by 16 threads on levels that hold a solid ghost (slow path; sweep-relative cell ii) ----
     double4 spec[4];                               // rho_w of a solid ghost in x, y, z
     int code[4];                                   // 1: x-up solid ghost, 2: y-up, 4: z-up, 8: dead cell
 };
 
-template <int RV>
+template <int RV, int ORD>
 struct __align__(128) LevelBuf {
-    RowBuf<RV> row[TILE_TY];
-    double xface[TILE_TY][NVB];                    // x-face input of the level
-    double yface[TILE_TX][NVB];                    // y-face input of the level
+    RowBuf<RV, ORD> row[TILE_TY];
+    double xface[KC<RV, ORD>::LAYERS][TILE_TY][KC<RV, ORD>::NVB];   // x-face input of the level (layer 0: nearest upwind cell)
+    double yface[KC<RV, ORD>::LAYERS][TILE_TX][KC<RV, ORD>::NVB];   // y-face input of the level
     double rwb[8];                                 // ghost densities of the domain faces: 4 x-face rows, 4 y-face columns
 };
 
-template <int RV>
+template <int RV, int ORD>
 struct __align__(128) TileSmem {
-    LevelBuf<RV> lv[2];                            // index = level parity
+    LevelBuf<RV, ORD> lv[2];                            // index = level parity
     // ---- per item ----
     double xi_a[16];                               // nodes of the block (0 beyond the box)
     double xi_bc[TILE_MAXBC];
@@ -239,8 +248,8 @@ __device__ __forceinline__ double rwb_load(const TileParams &P, const ItemCtx &I
     return v;
 }
 
-template <int RV>
-__device__ __forceinline__ void rwb_store(TileSmem<RV> &s, int b, int tid, double v)
+template <int RV, int ORD>
+__device__ __forceinline__ void rwb_store(TileSmem<RV, ORD> &s, int b, int tid, double v)
 {
     if (tid >= 32 && tid < 40) s.lv[b].rwb[tid - 32] = v;
 }
@@ -248,25 +257,28 @@ __device__ __forceinline__ void rwb_store(TileSmem<RV> &s, int b, int tid, doubl
 // The TMA copies of a level are described once per item (setup_copies: per 4-cell row the x, y, z factor-table rows and
 // the cell records - tables.cu; every row is one contiguous run of the padded grid - plus the x- and y-face input) and
 // issued per level by lane q / WARPS of warp q % WARPS for copy q (issue_level), so the copies are spread over the warps.
-template <int RV>
-__device__ __forceinline__ int copy_of_thread(int tid) { return (tid & 31) * (NVB / RV / 32) + (tid >> 5); }
+template <int RV, int ORD>
+__device__ __forceinline__ int copy_of_thread(int tid) { return (tid & 31) * KC<RV, ORD>::WARPS + (tid >> 5); }
 
-template <int RV>
-__device__ __forceinline__ void setup_copies(const TileParams &P, const ItemCtx &I, TileSmem<RV> &s, const VBlock &vb, int tid,
+template <int RV, int ORD>
+__device__ __forceinline__ void setup_copies(const TileParams &P, const ItemCtx &I, TileSmem<RV, ORD> &s, const VBlock &vb, int tid,
                                              const double *xsrc, const double *ysrc)
 {
-    constexpr int NA = GA * RV;
-    const int q = copy_of_thread<RV>(tid);
+    using RB = RowBuf<RV, ORD>;
+    using LB = LevelBuf<RV, ORD>;
+    constexpr int NA = GA * RV, ES = KC<RV, ORD>::ES;
+    constexpr unsigned XLEVEL_BYTES = KC<RV, ORD>::XLEVEL_BYTES, YLEVEL_BYTES = KC<RV, ORD>::YLEVEL_BYTES;
+    const int q = copy_of_thread<RV, ORD>(tid);
     if (q >= NCOPY) return;
-    const unsigned xbytes = 4u * NA * 32u, ybytes = 4u * vb.nbb * 32u, zbytes = 4u * vb.ncb * 32u;
+    const unsigned xbytes = 4u * NA * ES, ybytes = 4u * vb.nbb * ES, zbytes = 4u * vb.ncb * ES;
     CopyDesc d;
     d.pad[0] = d.pad[1] = 0;
     if (q == 4 * TILE_TY) {
         d.src = reinterpret_cast<const unsigned char *>(xsrc); d.step = XLEVEL_BYTES;
-        d.dst = (unsigned)offsetof(LevelBuf<RV>, xface); d.bytes = I.first_x ? 0u : XLEVEL_BYTES;
+        d.dst = (unsigned)offsetof(LB, xface); d.bytes = I.first_x ? 0u : XLEVEL_BYTES;
     } else if (q == 4 * TILE_TY + 1) {
         d.src = reinterpret_cast<const unsigned char *>(ysrc); d.step = YLEVEL_BYTES;
-        d.dst = (unsigned)offsetof(LevelBuf<RV>, yface); d.bytes = I.first_y ? 0u : YLEVEL_BYTES;
+        d.dst = (unsigned)offsetof(LB, yface); d.bytes = I.first_y ? 0u : YLEVEL_BYTES;
     } else {
         const int jj = q % TILE_TY, kind = q / TILE_TY;
         // first cell (lowest absolute x) of row jj on the padded grid at level 0; rows may lie in the dead padding
@@ -276,19 +288,19 @@ __device__ __forceinline__ void setup_copies(const TileParams &P, const ItemCtx 
         const int k = I.sz > 0 ? 0 : P.nz - 1;
         const long long npc = (long long)P.nz * P.nyp * P.nxp, lvl = (long long)P.nyp * P.nxp * I.sz;
         const long long pc = ((long long)k * P.nyp + (j + TILE_PAD)) * P.nxp + (i + TILE_PAD);
-        const unsigned rowoff = (unsigned)(offsetof(LevelBuf<RV>, row) + jj * sizeof(RowBuf<RV>));
+        const unsigned rowoff = (unsigned)(offsetof(LB, row) + jj * sizeof(RowBuf<RV, ORD>));
         if (kind == 0) {
-            d.src = reinterpret_cast<const unsigned char *>(P.TX + ((long long)vb.xb * npc + pc) * NA);
-            d.step = lvl * NA * 32; d.dst = rowoff + (unsigned)offsetof(RowBuf<RV>, xtab); d.bytes = xbytes;
+            d.src = reinterpret_cast<const unsigned char *>(P.TX) + ((long long)vb.xb * npc + pc) * NA * ES;
+            d.step = lvl * NA * ES; d.dst = rowoff + (unsigned)offsetof(RB, xtab); d.bytes = xbytes;
         } else if (kind == 1) {
-            d.src = reinterpret_cast<const unsigned char *>(P.TY + ((long long)vb.yb * npc + pc) * vb.nbb);
-            d.step = lvl * vb.nbb * 32; d.dst = rowoff + (unsigned)offsetof(RowBuf<RV>, ytab); d.bytes = ybytes;
+            d.src = reinterpret_cast<const unsigned char *>(P.TY) + ((long long)vb.yb * npc + pc) * vb.nbb * ES;
+            d.step = lvl * vb.nbb * ES; d.dst = rowoff + (unsigned)offsetof(RB, ytab); d.bytes = ybytes;
         } else if (kind == 2) {
-            d.src = reinterpret_cast<const unsigned char *>(P.TZ + ((long long)vb.zb * npc + pc) * vb.ncb);
-            d.step = lvl * vb.ncb * 32; d.dst = rowoff + (unsigned)offsetof(RowBuf<RV>, ztab); d.bytes = zbytes;
+            d.src = reinterpret_cast<const unsigned char *>(P.TZ) + ((long long)vb.zb * npc + pc) * vb.ncb * ES;
+            d.step = lvl * vb.ncb * ES; d.dst = rowoff + (unsigned)offsetof(RB, ztab); d.bytes = zbytes;
         } else {
             d.src = reinterpret_cast<const unsigned char *>(P.rec + pc);
-            d.step = lvl * (long long)sizeof(CellRec); d.dst = rowoff + (unsigned)offsetof(RowBuf<RV>, rec); d.bytes = REC_ROW_BYTES;
+            d.step = lvl * (long long)sizeof(CellRec); d.dst = rowoff + (unsigned)offsetof(RB, rec); d.bytes = REC_ROW_BYTES;
         }
     }
     s.desc[q] = d;
@@ -298,10 +310,10 @@ __device__ __forceinline__ void setup_copies(const TileParams &P, const ItemCtx 
 }
 
 // issue the copies of level kp into buffer kp & 1 (the descriptors were written by the same threads)
-template <int RV>
-__device__ __forceinline__ void issue_level(TileSmem<RV> &s, int kp, int tid)
+template <int RV, int ORD>
+__device__ __forceinline__ void issue_level(TileSmem<RV, ORD> &s, int kp, int tid)
 {
-    const int q = copy_of_thread<RV>(tid);
+    const int q = copy_of_thread<RV, ORD>(tid);
     if (q >= NCOPY) return;
     const int b = kp & 1;
     if (q == 0) mbar_expect_tx(&s.mbar[b], s.txbytes);
@@ -312,8 +324,8 @@ __device__ __forceinline__ void issue_level(TileSmem<RV> &s, int kp, int tid)
 // Does the level staged in buffer b hold a fluid cell whose upwind neighbour is a masked cell?  Asked by lanes 0..15 of
 // warp 0 (one record each) right after they have waited for the level's copies; the answer reaches the other threads
 // through the CTA barrier that ends the level before.
-template <int RV>
-__device__ __forceinline__ void detect_special(const ItemCtx &I, TileSmem<RV> &s, int b, int lane)
+template <int RV, int ORD>
+__device__ __forceinline__ void detect_special(const ItemCtx &I, TileSmem<RV, ORD> &s, int b, int lane)
 {
     const CellRec &r = s.lv[b].row[lane >> 2].rec[lane & 3];
     const int upmask = (1 << I.upx) | (1 << I.upy) | (1 << I.upz);
@@ -324,13 +336,13 @@ __device__ __forceinline__ void detect_special(const ItemCtx &I, TileSmem<RV> &s
 
 // Slow path only: per-cell ghost codes of the level in buffer b, decoded from the staged records by the first 16 threads
 // of the last warp.
-template <int RV>
-__device__ __forceinline__ void decode_records(const TileParams &P, const ItemCtx &I, TileSmem<RV> &s, int b, int tid)
+template <int RV, int ORD>
+__device__ __forceinline__ void decode_records(const TileParams &P, const ItemCtx &I, TileSmem<RV, ORD> &s, int b, int tid)
 {
-    constexpr int T0 = NVB / RV - 32;
+    constexpr int T0 = KC<RV, ORD>::THREADS - 32;
     if (tid >= T0 && tid < T0 + NCELL) {
         const int cell = tid - T0, ii = cell & 3, jj = cell >> 2;
-        RowBuf<RV> &R = s.lv[b].row[jj];
+        RowBuf<RV, ORD> &R = s.lv[b].row[jj];
         const CellRec &r = R.rec[I.sx > 0 ? ii : 3 - ii];
         const bool dead = (r.flags & REC_DEAD) != 0;
         const int sfl = (r.flags >> 8) & 0xff;
@@ -350,36 +362,39 @@ __device__ __forceinline__ void decode_records(const TileParams &P, const ItemCt
 // The RV values of a thread in a face row of NVB doubles are stored as RV / 2 pairs, pair h of thread t at double
 // (h * threads + t) * 2: every 16-byte access of a warp then covers 512 contiguous bytes (full sectors in L2 / HBM, no
 // bank conflict in shared memory).  row = start of the face row.
-template <int RV>
-__device__ __forceinline__ int face_index(int tid, int r) { return ((r >> 1) * (NVB / RV) + tid) * 2 + (r & 1); }
-template <int RV>
+template <int RV, int ORD>
+__device__ __forceinline__ int face_index(int tid, int r) { return ((r >> 1) * KC<RV, ORD>::THREADS + tid) * 2 + (r & 1); }
+template <int RV, int ORD>
 __device__ __forceinline__ void load_face(const double *row, int tid, double (&v)[RV])
 {
 #pragma unroll
     for (int h = 0; h < RV / 2; ++h) {
-        const double2 t = reinterpret_cast<const double2 *>(row)[h * (NVB / RV) + tid];
+        const double2 t = reinterpret_cast<const double2 *>(row)[h * KC<RV, ORD>::THREADS + tid];
         v[2 * h] = t.x; v[2 * h + 1] = t.y;
     }
 }
-template <int RV>
+template <int RV, int ORD>
 __device__ __forceinline__ void store_face(double *row, int tid, const double (&v)[RV])
 {
 #pragma unroll
-    for (int h = 0; h < RV / 2; ++h) st_f64x2(row + (h * (NVB / RV) + tid) * 2, v[2 * h], v[2 * h + 1]);
+    for (int h = 0; h < RV / 2; ++h) st_f64x2(row + (h * KC<RV, ORD>::THREADS + tid) * 2, v[2 * h], v[2 * h + 1]);
 }
 
 // Ghost values of the domain faces of level kp (buffer b) for a tile at the upwind x / y edge of the domain
-template <int RV>
-__device__ __forceinline__ void fill_faces(const ItemCtx &I, TileSmem<RV> &s, int b, int tid, int ag, int yidx, int zidx)
+template <int RV, int ORD>
+__device__ __forceinline__ void fill_faces(const ItemCtx &I, TileSmem<RV, ORD> &s, int b, int tid, int ag, int yidx, int zidx)
 {
-    LevelBuf<RV> &L = s.lv[b];
+    LevelBuf<RV, ORD> &L = s.lv[b];
     if (I.first_x) {
         const double gyz = s.g[0][1][yidx] * s.g[0][2][zidx];
 #pragma unroll
         for (int r = 0; r < RV; ++r) {
             const double G = s.g[0][0][RV * ag + r] * gyz;
 #pragma unroll
-            for (int jj = 0; jj < TILE_TY; ++jj) L.xface[jj][face_index<RV>(tid, r)] = L.rwb[jj] * G;
+            for (int jj = 0; jj < TILE_TY; ++jj) {
+                L.xface[0][jj][face_index<RV, ORD>(tid, r)] = L.rwb[jj] * G;
+                if (ORD == 2) L.xface[ORD - 1][jj][face_index<RV, ORD>(tid, r)] = 0.0;   // second upwind value: its coefficient is 0
+            }
         }
     }
     if (I.first_y) {
@@ -388,13 +403,16 @@ __device__ __forceinline__ void fill_faces(const ItemCtx &I, TileSmem<RV> &s, in
         for (int r = 0; r < RV; ++r) {
             const double G = s.g[1][0][RV * ag + r] * gyz;
 #pragma unroll
-            for (int ii = 0; ii < 4; ++ii) L.yface[ii][face_index<RV>(tid, r)] = L.rwb[4 + ii] * G;
+            for (int ii = 0; ii < 4; ++ii) {
+                L.yface[0][ii][face_index<RV, ORD>(tid, r)] = L.rwb[4 + ii] * G;
+                if (ORD == 2) L.yface[ORD - 1][ii][face_index<RV, ORD>(tid, r)] = 0.0;
+            }
         }
     }
 }
 
 // per-thread constants of an item
-template <int RV>
+template <int RV, int ORD>
 struct ThreadCtx {
     double aX[RV];               // stage-1 A fragments per node r: xi_x^p, p = (lane >> 2) & 3
     double yz0, yz1;             // stage-2 B fragments: monomial lane >> 2 of the warp's pairs 2 (lane & 3), 2 (lane & 3) + 1
@@ -406,13 +424,19 @@ struct ThreadCtx {
     int xrev;                    // 3 if the sweep runs against x (table rows are in ascending absolute x), else 0
 };
 
-template <int RV>
-__device__ __forceinline__ const double4 &entry(const RowBuf<RV> &R, int byte_off)
+template <int RV, int ORD>
+__device__ __forceinline__ const double4 &entry(const RowBuf<RV, ORD> &R, int byte_off)
 {
     return *reinterpret_cast<const double4 *>(reinterpret_cast<const unsigned char *>(&R) + byte_off);
 }
-template <int RV>
-__device__ __forceinline__ const CellRec &record(const RowBuf<RV> &R, int byte_off)
+// order 2: the two stencil coefficients c1, c2 that follow (E, Q, e, cd) in an entry
+template <int RV, int ORD>
+__device__ __forceinline__ const double2 &entry_c(const RowBuf<RV, ORD> &R, int byte_off)
+{
+    return *reinterpret_cast<const double2 *>(reinterpret_cast<const unsigned char *>(&R) + byte_off + 32);
+}
+template <int RV, int ORD>
+__device__ __forceinline__ const CellRec &record(const RowBuf<RV, ORD> &R, int byte_off)
 {
     return *reinterpret_cast<const CellRec *>(reinterpret_cast<const unsigned char *>(&R) + byte_off);
 }
@@ -422,15 +446,15 @@ __device__ __forceinline__ const CellRec &record(const RowBuf<RV> &R, int byte_o
 // No predicates and no branches (the row stays one basic block): a result the sums do not need is multiplied by 0 and
 // added to a slot no other lane of the instruction targets; dead cells have g = 0 and name a row of their own or, in
 // the padding, of the nearest cell of the grid.
-template <int RV>
-__device__ __forceinline__ void emit_pair(const RowBuf<RV> &R, const int roA, const int roB, const double a0, const double a1,
-                                          const double b0, const double b1, const ThreadCtx<RV> &T, const int lane)
+template <int RV, int ORD>
+__device__ __forceinline__ void emit_pair(const RowBuf<RV, ORD> &R, const int roA, const int roB, const double a0, const double a1,
+                                          const double b0, const double b1, const ThreadCtx<RV, ORD> &T, const int lane)
 {
     const bool hi = lane & 16;
     double d0 = 0.0, d1 = 0.0;
     dmma(d0, d1, hi ? b0 : a0, T.yz0);
     dmma(d0, d1, hi ? b1 : a1, T.yz1);
-    const long long c = record(R, hi ? roB : roA).cidx;
+    const long long c = record<RV, ORD>(R, hi ? roB : roA).cidx;
     red_f64(T.raw0 + c * 16, d0 * T.use0);
     red_f64(T.raw1 + c * 16, d1 * T.use1);
 }
@@ -440,28 +464,44 @@ __device__ __forceinline__ void emit_pair(const RowBuf<RV> &R, const int roA, co
 // first row of the tile, else the row just computed).  Dead cells (outside the domain / solid) have all-zero table
 // entries and nu = 1, so they produce g = 0 by the same arithmetic.  The last row of the tile (LAST) also writes the
 // y-face output, cell by cell, so that the stores are spread over the row.
-template <int RV, bool LAST>
-__device__ __forceinline__ void compute_row(const RowBuf<RV> &R, const double *xin, double (&zrow)[4][RV], const double (&yup)[4][RV],
-                                            const ThreadCtx<RV> &T, const int tid, const int lane, double *xout, const bool wx,
+// ORD = 2 (second-order upwind, G21): z2row / yup2 / the second x-face layer hold the second upwind values; the
+// table entries carry the stencil coefficients (cd, c1, c2) per direction, so the cell value is
+// g = [src + sum_d (c1_d g_1d + c2_d g_2d)] / (nu + sum_d cd_d); the recurrence along x is still one DFMA per value
+// (the c2 term uses the value two cells back, known a cell earlier).  YL: y-face layer this row's values go to (-1: none).
+template <int RV, int ORD, int YL>
+__device__ __forceinline__ void compute_row(const RowBuf<RV, ORD> &R, const double *xin, const double *xin2, double (&zrow)[4][RV],
+                                            double (&z2row)[4][RV], const double (&yup)[4][RV], const double (&yup2)[4][RV],
+                                            const ThreadCtx<RV, ORD> &T, const int tid, const int lane, double *xout, const bool wx,
                                             double *yout, const bool wy)
 {
-    double fx[RV];
-    load_face<RV>(xin, tid, fx);
+    constexpr int NVB = KC<RV, ORD>::NVB, ES = KC<RV, ORD>::ES;
+    double fx[RV], fx2[RV];
+    load_face<RV, ORD>(xin, tid, fx);
+    if (ORD == 2) load_face<RV, ORD>(xin2, tid, fx2);
     double acc[2][2];
 #pragma unroll
     for (int ii = 0; ii < 4; ++ii) {
-        const double4 yt = entry(R, T.yo[ii]);
-        const double4 zt = entry(R, T.zo[ii]);
+        const double4 yt = entry<RV, ORD>(R, T.yo[ii]);
+        const double4 zt = entry<RV, ORD>(R, T.zo[ii]);
         const double Eyz = yt.x * zt.x, Qyz = yt.y + zt.y, eyz = yt.z + zt.z;
-        const double ay = yt.w, az = zt.w;
-        const double dyz = (ay + az) + record(R, T.ro[ii]).nu;
+        const double dyz = (yt.w + zt.w) + record<RV, ORD>(R, T.ro[ii]).nu;
+        double c1y = yt.w, c1z = zt.w, c2y = 0.0, c2z = 0.0;
+        if (ORD == 2) {
+            const double2 yc = entry_c<RV, ORD>(R, T.yo[ii]), zc = entry_c<RV, ORD>(R, T.zo[ii]);
+            c1y = yc.x; c2y = yc.y; c1z = zc.x; c2z = zc.y;
+        }
         // Everything that does not depend on the x-upwind value, for the RV nodes of the thread in lock step (the fp64
         // pipe takes a warp instruction every 2 clocks and has a latency of ~10): the cell value is g = W g_xup + V with
         // W = a_x / den and V = (a_y g_yup + a_z g_zup + src) / den, Eq.(7) PAPER.md:75-79.
         double4 xt[RV];
+        double2 xc[RV];
         double t1[RV], t2[RV], d[RV], y0[RV], sE[RV], e[RV], W[RV], V[RV];
 #pragma unroll
-        for (int r = 0; r < RV; ++r) xt[r] = entry(R, T.xo[ii] + r * GA * 32);
+        for (int r = 0; r < RV; ++r) xt[r] = entry<RV, ORD>(R, T.xo[ii] + r * GA * ES);
+        if (ORD == 2) {
+#pragma unroll
+            for (int r = 0; r < RV; ++r) xc[r] = entry_c<RV, ORD>(R, T.xo[ii] + r * GA * ES);
+        }
 #pragma unroll
         for (int r = 0; r < RV; ++r) d[r] = xt[r].w + dyz;
 #pragma unroll
@@ -483,27 +523,41 @@ __device__ __forceinline__ void compute_row(const RowBuf<RV> &R, const double *x
 #pragma unroll
         for (int r = 0; r < RV; ++r) y0[r] = fma(y0[r], e[r], y0[r]);       // 1 / den (MUFU seed + cubic Newton step)
 #pragma unroll
-        for (int r = 0; r < RV; ++r) V[r] = fma(ay, yup[ii][r], V[r]);
+        for (int r = 0; r < RV; ++r) V[r] = fma(c1y, yup[ii][r], V[r]);
+        if (ORD == 2) {
 #pragma unroll
-        for (int r = 0; r < RV; ++r) W[r] = xt[r].w * y0[r];
+            for (int r = 0; r < RV; ++r) V[r] = fma(c2y, yup2[ii][r], V[r]);
+        }
 #pragma unroll
-        for (int r = 0; r < RV; ++r) V[r] = fma(az, zrow[ii][r], V[r]);
+        for (int r = 0; r < RV; ++r) W[r] = (ORD == 2 ? xc[r].x : xt[r].w) * y0[r];
+#pragma unroll
+        for (int r = 0; r < RV; ++r) V[r] = fma(c1z, zrow[ii][r], V[r]);
+        if (ORD == 2) {
+#pragma unroll
+            for (int r = 0; r < RV; ++r) V[r] = fma(c2z, z2row[ii][r], V[r]);
+#pragma unroll
+            for (int r = 0; r < RV; ++r) V[r] = fma(xc[r].y, fx2[r], V[r]);
+        }
 #pragma unroll
         for (int r = 0; r < RV; ++r) V[r] *= y0[r];
         // the recurrence along x: one DFMA per value
 #pragma unroll
         for (int r = 0; r < RV; ++r) {
             const double gg = fma(W[r], fx[r], V[r]);
+            if (ORD == 2) { fx2[r] = fx[r]; z2row[ii][r] = zrow[ii][r]; }
             fx[r] = gg;
             zrow[ii][r] = gg;
         }
         acc[ii & 1][0] = 0.0; acc[ii & 1][1] = 0.0;
 #pragma unroll
         for (int r = 0; r < RV; ++r) dmma(acc[ii & 1][0], acc[ii & 1][1], T.aX[r], zrow[ii][r]);
-        if (ii & 1) emit_pair<RV>(R, T.ro[ii - 1], T.ro[ii], acc[0][0], acc[0][1], acc[1][0], acc[1][1], T, lane);
-        if (LAST && wy) store_face<RV>(yout + ii * NVB, tid, zrow[ii]);
+        if (ii & 1) emit_pair<RV, ORD>(R, T.ro[ii - 1], T.ro[ii], acc[0][0], acc[0][1], acc[1][0], acc[1][1], T, lane);
+        if (YL >= 0 && wy) store_face<RV, ORD>(yout + (YL * TILE_TX + ii) * NVB, tid, zrow[ii]);
     }
-    if (wx) store_face<RV>(xout, tid, fx);
+    if (wx) {
+        store_face<RV, ORD>(xout, tid, fx);
+        if (ORD == 2) store_face<RV, ORD>(xout + TILE_TY * NVB, tid, fx2);
+    }
 }
 
 // One level of the column, fast path (no solid ghost in the level): 4 rows x 4 cells x RV velocities per thread with the
@@ -511,40 +565,60 @@ __device__ __forceinline__ void compute_row(const RowBuf<RV> &R, const double *x
 // the row before.  The B200 instruction cache holds 32 KB, and a level loop larger than that is fetch-bound at 1/3
 // instruction per clock and scheduler (profiles/r01_ifetch_microbench.txt): the instructions a level executes on
 // this path (about 1900 for RV = 4) stay below that; rolled variants with rotating row slots were slower (profiles/).
-template <int RV>
-__device__ __forceinline__ void compute_level(const LevelBuf<RV> &L, double (&pl)[TILE_TY][4][RV], const ThreadCtx<RV> &T,
-                                              const int tid, const int lane, double *xout, const bool wx, double *yout,
-                                              const bool wy)
+template <int RV, int ORD>
+__device__ __forceinline__ void compute_level(const LevelBuf<RV, ORD> &L, double (&pl)[TILE_TY][4][RV], double (&pl2)[ORD == 2 ? TILE_TY : 1][4][RV],
+                                              const ThreadCtx<RV, ORD> &T, const int tid, const int lane, double *xout, const bool wx,
+                                              double *yout, const bool wy)
 {
-    double yu[4][RV];
+    constexpr int NVB = KC<RV, ORD>::NVB, L2 = ORD - 1;
+    static_assert(TILE_TY >= 2 || ORD == 1, "the second-order tile kernel needs at least two rows per tile");
+    double yu[4][RV], yu2[4][RV];
 #pragma unroll
-    for (int ii = 0; ii < 4; ++ii) load_face<RV>(&L.yface[ii][0], tid, yu[ii]);
+    for (int ii = 0; ii < 4; ++ii) load_face<RV, ORD>(&L.yface[0][ii][0], tid, yu[ii]);
+    if (ORD == 2) {
+#pragma unroll
+        for (int ii = 0; ii < 4; ++ii) load_face<RV, ORD>(&L.yface[L2][ii][0], tid, yu2[ii]);
+    }
+    // y-face layer a row's values go to: the last row -> layer 0, the one before (order 2) -> layer 1
     if (TILE_TY == 1) {
-        compute_row<RV, true>(L.row[0], L.xface[0], pl[0], yu, T, tid, lane, xout, wx, yout, wy);
+        compute_row<RV, ORD, 0>(L.row[0], L.xface[0][0], L.xface[L2][0], pl[0], pl2[0], yu, yu2, T, tid, lane, xout, wx, yout, wy);
     } else {
-        compute_row<RV, false>(L.row[0], L.xface[0], pl[0], yu, T, tid, lane, xout, wx, yout, wy);
+        compute_row<RV, ORD, (ORD == 2 && TILE_TY == 2) ? 1 : -1>(L.row[0], L.xface[0][0], L.xface[L2][0], pl[0], pl2[0], yu, yu2, T, tid, lane,
+                                                                xout, wx, yout, wy);
 #pragma unroll
-        for (int jj = 1; jj < TILE_TY - 1; ++jj)
-            compute_row<RV, false>(L.row[jj], L.xface[jj], pl[jj], pl[jj - 1], T, tid, lane, xout + jj * NVB, wx, yout, wy);
-        compute_row<RV, true>(L.row[TILE_TY - 1], L.xface[TILE_TY - 1], pl[TILE_TY - 1], pl[TILE_TY > 1 ? TILE_TY - 2 : 0], T, tid, lane,
-                              xout + (TILE_TY - 1) * NVB, wx, yout, wy);
+        for (int jj = 1; jj < TILE_TY - 1; ++jj) {
+            if (ORD == 2 && jj == TILE_TY - 2)
+                compute_row<RV, ORD, 1>(L.row[jj], L.xface[0][jj], L.xface[L2][jj], pl[jj], pl2[ORD == 2 ? jj : 0], pl[jj - 1], jj >= 2 ? pl[jj >= 2 ? jj - 2 : 0] : yu,
+                                        T, tid, lane, xout + jj * NVB, wx, yout, wy);
+            else
+                compute_row<RV, ORD, -1>(L.row[jj], L.xface[0][jj], L.xface[L2][jj], pl[jj], pl2[ORD == 2 ? jj : 0], pl[jj - 1], jj >= 2 ? pl[jj >= 2 ? jj - 2 : 0] : yu,
+                                         T, tid, lane, xout + jj * NVB, wx, yout, wy);
+        }
+        constexpr int J = TILE_TY - 1;
+        compute_row<RV, ORD, 0>(L.row[J], L.xface[0][J], L.xface[L2][J], pl[J], pl2[ORD == 2 ? J : 0], pl[J - 1], J >= 2 ? pl[J >= 2 ? J - 2 : 0] : yu, T, tid, lane,
+                                xout + J * NVB, wx, yout, wy);
     }
 }
 
 // One level that holds a solid ghost (a fluid cell whose upwind neighbour is a masked cell): the same arithmetic
-// written as compact loops over a copy of the plane in local memory.  Rare (the surface of a masked body), so its
+// written as compact loops over a copy of the plane(s) in local memory.  Rare (the surface of a masked body), so its
 // speed does not matter; keeping it out of the unrolled path halves the code the instruction cache has to hold.
-template <int RV>
-__device__ __forceinline__ void compute_level_slow(TileSmem<RV> &s, const LevelBuf<RV> &L, double *pl, const ThreadCtx<RV> &T,
-                                                   const int tid, const int lane, double *xout, double *yout)
+// A solid ghost replaces the first upwind value; the coefficient of the second one is 0 there (tables.cu).
+template <int RV, int ORD>
+__device__ __forceinline__ void compute_level_slow(TileSmem<RV, ORD> &s, const LevelBuf<RV, ORD> &L, double *pl, double *pl2,
+                                                   const ThreadCtx<RV, ORD> &T, const int tid, const int lane, double *xout, double *yout)
 {
+    constexpr int NVB = KC<RV, ORD>::NVB, ES = KC<RV, ORD>::ES, L2 = ORD - 1;
     const double gyz = s.g[3][1][T.yi] * s.g[3][2][T.zi];
 #pragma unroll 1
     for (int jj = 0; jj < TILE_TY; ++jj) {
-        const RowBuf<RV> &R = L.row[jj];
-        double fx[RV];
+        const RowBuf<RV, ORD> &R = L.row[jj];
+        double fx[RV], fx2[RV];
 #pragma unroll
-        for (int r = 0; r < RV; ++r) fx[r] = L.xface[jj][face_index<RV>(tid, r)];
+        for (int r = 0; r < RV; ++r) {
+            fx[r] = L.xface[0][jj][face_index<RV, ORD>(tid, r)];
+            fx2[r] = ORD == 2 ? L.xface[L2][jj][face_index<RV, ORD>(tid, r)] : 0.0;
+        }
         double accA0 = 0.0, accA1 = 0.0;
         int roPrev = 0;
 #pragma unroll 1
@@ -553,37 +627,56 @@ __device__ __forceinline__ void compute_level_slow(TileSmem<RV> &s, const LevelB
             const int xo = ii == 0 ? T.xo[0] : ii == 1 ? T.xo[1] : ii == 2 ? T.xo[2] : T.xo[3];
             const int yo = ii == 0 ? T.yo[0] : ii == 1 ? T.yo[1] : ii == 2 ? T.yo[2] : T.yo[3];
             const int zo = ii == 0 ? T.zo[0] : ii == 1 ? T.zo[1] : ii == 2 ? T.zo[2] : T.zo[3];
-            const double4 yt = entry(R, yo);
-            const double4 zt = entry(R, zo);
+            const double4 yt = entry<RV, ORD>(R, yo);
+            const double4 zt = entry<RV, ORD>(R, zo);
             const double Eyz = yt.x * zt.x, Qyz = yt.y + zt.y, eyz = yt.z + zt.z;
-            const double ay = yt.w, az = zt.w;
+            double c1y = yt.w, c1z = zt.w, c2y = 0.0, c2z = 0.0;
+            if (ORD == 2) {
+                const double2 yc = entry_c<RV, ORD>(R, yo), zc = entry_c<RV, ORD>(R, zo);
+                c1y = yc.x; c2y = yc.y; c1z = zc.x; c2z = zc.y;
+            }
             const int ro = ii == 0 ? T.ro[0] : ii == 1 ? T.ro[1] : ii == 2 ? T.ro[2] : T.ro[3];
-            const double dyz = (ay + az) + record(R, ro).nu;
+            const double dyz = (yt.w + zt.w) + record<RV, ORD>(R, ro).nu;
             const int code = R.code[ii];
             const double4 sp = R.spec[ii];
             double c0 = 0.0, c1 = 0.0;
 #pragma unroll
             for (int r = 0; r < RV; ++r) {
                 const double Pg = s.g[3][0][RV * T.ag + r] * gyz;
-                const double4 xt = entry(R, xo + r * GA * 32);
+                const double4 xt = entry<RV, ORD>(R, xo + r * GA * ES);
+                double c1x = xt.w, c2x = 0.0;
+                if (ORD == 2) { const double2 xc = entry_c<RV, ORD>(R, xo + r * GA * ES); c1x = xc.x; c2x = xc.y; }
                 double xu = fx[r], zu = pl[cell * RV + r];
-                double yu = jj == 0 ? L.yface[ii][face_index<RV>(tid, r)] : pl[(cell - 4) * RV + r];
+                double yu = jj == 0 ? L.yface[0][ii][face_index<RV, ORD>(tid, r)] : pl[(cell - 4) * RV + r];
+                double xu2 = fx2[r], zu2 = 0.0, yu2 = 0.0;
+                if (ORD == 2) {
+                    zu2 = pl2[cell * RV + r];
+                    yu2 = jj == 0 ? L.yface[L2][ii][face_index<RV, ORD>(tid, r)]
+                        : jj == 1 ? L.yface[0][ii][face_index<RV, ORD>(tid, r)] : pl[(cell - 8) * RV + r];
+                }
                 if (code & 1) xu = sp.x * Pg;
                 if (code & 2) yu = sp.y * Pg;
                 if (code & 4) zu = sp.z * Pg;
                 const double src = (xt.x * Eyz) * fma(xt.y + Qyz, xt.z + eyz, 1.0);
                 const double inv = fast_rcp(xt.w + dyz);
-                double num = fma(ay, yu, src);
-                num = fma(az, zu, num);
-                num = fma(xt.w, xu, num);
+                double num = fma(c1y, yu, src);
+                num = fma(c1z, zu, num);
+                num = fma(c1x, xu, num);
+                if (ORD == 2) {
+                    num = fma(c2y, yu2, num);
+                    num = fma(c2z, zu2, num);
+                    num = fma(c2x, xu2, num);
+                }
                 double gg = num * inv;
                 if (code & 8) gg = 0.0;
+                fx2[r] = fx[r];
                 fx[r] = gg;
+                if (ORD == 2) pl2[cell * RV + r] = pl[cell * RV + r];
                 pl[cell * RV + r] = gg;
                 dmma(c0, c1, T.aX[r], gg);
             }
             if (ii & 1) {
-                emit_pair<RV>(R, roPrev, ro, accA0, accA1, c0, c1, T, lane);
+                emit_pair<RV, ORD>(R, roPrev, ro, accA0, accA1, c0, c1, T, lane);
             } else {
                 accA0 = c0; accA1 = c1;
             }
@@ -591,25 +684,33 @@ __device__ __forceinline__ void compute_level_slow(TileSmem<RV> &s, const LevelB
         }
         if (xout) {
 #pragma unroll
-            for (int r = 0; r < RV; ++r) xout[jj * NVB + face_index<RV>(tid, r)] = fx[r];
+            for (int r = 0; r < RV; ++r) {
+                xout[jj * NVB + face_index<RV, ORD>(tid, r)] = fx[r];
+                if (ORD == 2) xout[(TILE_TY + jj) * NVB + face_index<RV, ORD>(tid, r)] = fx2[r];
+            }
         }
     }
     if (yout) {
 #pragma unroll 1
         for (int ii = 0; ii < 4; ++ii)
 #pragma unroll
-            for (int r = 0; r < RV; ++r) yout[ii * NVB + face_index<RV>(tid, r)] = pl[((TILE_TY - 1) * 4 + ii) * RV + r];
+            for (int r = 0; r < RV; ++r) {
+                yout[ii * NVB + face_index<RV, ORD>(tid, r)] = pl[((TILE_TY - 1) * 4 + ii) * RV + r];
+                if (ORD == 2) yout[(TILE_TX + ii) * NVB + face_index<RV, ORD>(tid, r)] = pl[((TILE_TY >= 2 ? TILE_TY - 2 : 0) * 4 + ii) * RV + r];
+            }
     }
 }
 
-template <int RV>
-__global__ void __launch_bounds__(NVB / RV, 2) sweep_tile_kernel(const TileParams P)
+template <int RV, int ORD>
+__global__ void __launch_bounds__(KC<RV, ORD>::THREADS, 2) sweep_tile_kernel(const TileParams P)
 {
-    constexpr int NA = GA * RV;
+    constexpr int NA = GA * RV, THREADS = KC<RV, ORD>::THREADS, XLEVEL_DOUBLES = KC<RV, ORD>::XLEVEL_DOUBLES, YLEVEL_DOUBLES = KC<RV, ORD>::YLEVEL_DOUBLES;
+    (void)THREADS;
+    using RB = RowBuf<RV, ORD>;
     // dynamic shared memory starts at offset 0 of the CTA's window (no static __shared__ in this kernel), so the
     // 128-byte alignment holds; casting without pointer arithmetic keeps the address space visible (LDS / STS)
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    TileSmem<RV> &s = *reinterpret_cast<TileSmem<RV> *>(smem_raw);
+    TileSmem<RV, ORD> &s = *reinterpret_cast<TileSmem<RV, ORD> *>(smem_raw);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     if (tid == 0) {
         mbar_init(&s.mbar[0], 1);
@@ -652,11 +753,11 @@ __global__ void __launch_bounds__(NVB / RV, 2) sweep_tile_kernel(const TileParam
 
         // ---- TMA copies of levels 0 and 1 (the staging buffers are free: every thread passed the end-of-item
         //      barrier; the upwind items' face stores were made with the generic proxy) ----
-        setup_copies<RV>(P, I, s, vb, tid, xdst, ydst);
-        if (copy_of_thread<RV>(tid) < NCOPY) {
+        setup_copies<RV, ORD>(P, I, s, vb, tid, xdst, ydst);
+        if (copy_of_thread<RV, ORD>(tid) < NCOPY) {
             fence_proxy_async_global();
-            issue_level<RV>(s, 0, tid);
-            if (P.nz > 1) issue_level<RV>(s, 1, tid);
+            issue_level<RV, ORD>(s, 0, tid);
+            if (P.nz > 1) issue_level<RV, ORD>(s, 1, tid);
         }
         // ---- per-item tables: nodes, ghost factors; ghost densities of the domain faces of levels 0 and 1 ----
         {
@@ -683,12 +784,12 @@ __global__ void __launch_bounds__(NVB / RV, 2) sweep_tile_kernel(const TileParam
                 for (int f = 0; f < 4; ++f)
                     s.g[f][2][vb.nbb + cl] = ok ? P.gtab[(long long)(slotid[f] * 3 + 2) * P.gstride + idx] : 0.0;
             }
-            rwb_store<RV>(s, 0, tid, rwb_load(P, I, 0, tid));
-            rwb_store<RV>(s, 1, tid, rwb_load(P, I, 1, tid));
+            rwb_store<RV, ORD>(s, 0, tid, rwb_load(P, I, 0, tid));
+            rwb_store<RV, ORD>(s, 1, tid, rwb_load(P, I, 1, tid));
         }
         __syncthreads();
 
-        ThreadCtx<RV> T;
+        ThreadCtx<RV, ORD> T;
         T.ag = lane & 3;
         T.xrev = vb.sx > 0 ? 0 : 3;
         {
@@ -700,10 +801,10 @@ __global__ void __launch_bounds__(NVB / RV, 2) sweep_tile_kernel(const TileParam
 #pragma unroll
             for (int ii = 0; ii < 4; ++ii) {
                 const int cp = ii ^ T.xrev;
-                T.xo[ii] = (int)offsetof(RowBuf<RV>, xtab) + (cp * NA + T.ag) * 32;
-                T.yo[ii] = (int)offsetof(RowBuf<RV>, ytab) + (cp * vb.nbb + yl) * 32;
-                T.zo[ii] = (int)offsetof(RowBuf<RV>, ztab) + (cp * vb.ncb + zl) * 32;
-                T.ro[ii] = (int)offsetof(RowBuf<RV>, rec) + cp * (int)sizeof(CellRec);
+                T.xo[ii] = (int)offsetof(RB, xtab) + (cp * NA + T.ag) * KC<RV, ORD>::ES;
+                T.yo[ii] = (int)offsetof(RB, ytab) + (cp * vb.nbb + yl) * KC<RV, ORD>::ES;
+                T.zo[ii] = (int)offsetof(RB, ztab) + (cp * vb.ncb + zl) * KC<RV, ORD>::ES;
+                T.ro[ii] = (int)offsetof(RB, rec) + cp * (int)sizeof(CellRec);
             }
             // stage-1 A fragments: xi_x^p of the thread's own nodes, p = (lane >> 2) & 3
             const int row = lane >> 2, pw = row & 3;
@@ -742,11 +843,18 @@ __global__ void __launch_bounds__(NVB / RV, 2) sweep_tile_kernel(const TileParam
         if (tid < NCELL) {
             mbar_wait(&s.mbar[0], par[0]);
             par[0] ^= 1u;
-            detect_special<RV>(I, s, 0, lane);
+            detect_special<RV, ORD>(I, s, 0, lane);
         }
-        fill_faces<RV>(I, s, 0, tid, T.ag, T.yi, T.zi);
-        // plane = ghost of the upwind z face of the domain
-        double pl[TILE_TY][4][RV];
+        fill_faces<RV, ORD>(I, s, 0, tid, T.ag, T.yi, T.zi);
+        // plane = ghost of the upwind z face of the domain (order 2: the plane before it is never used, its coefficient
+        // is 0 in the first level; it must only be finite)
+        double pl[TILE_TY][4][RV], pl2[ORD == 2 ? TILE_TY : 1][4][RV];
+#pragma unroll
+        for (int jj = 0; jj < (ORD == 2 ? TILE_TY : 1); ++jj)
+#pragma unroll
+            for (int ii = 0; ii < 4; ++ii)
+#pragma unroll
+                for (int r = 0; r < RV; ++r) pl2[jj][ii][r] = 0.0;
         {
             const double gyz = s.g[2][1][T.yi] * s.g[2][2][T.zi];
             double G[RV];
@@ -774,7 +882,7 @@ __global__ void __launch_bounds__(NVB / RV, 2) sweep_tile_kernel(const TileParam
             if (tid < NCELL && kp + 1 < P.nz) {
                 mbar_wait(&s.mbar[b ^ 1], par[b ^ 1]);
                 par[b ^ 1] ^= 1u;
-                detect_special<RV>(I, s, b ^ 1, lane);
+                detect_special<RV, ORD>(I, s, b ^ 1, lane);
             }
             double vrw = 0.0;
             if (edge) vrw = rwb_load(P, I, kp + 2, tid);
@@ -782,29 +890,35 @@ __global__ void __launch_bounds__(NVB / RV, 2) sweep_tile_kernel(const TileParam
             double *xout = xdst + (long long)kp * XLEVEL_DOUBLES, *yout = ydst + (long long)kp * YLEVEL_DOUBLES;
             if (special) {
                 // every thread of the CTA takes this branch together
-                decode_records<RV>(P, I, s, b, tid);
+                decode_records<RV, ORD>(P, I, s, b, tid);
                 __syncthreads();
-                double tmp[NCELL * RV];
+                double tmp[NCELL * RV], tmp2[ORD == 2 ? NCELL * RV : 1];
 #pragma unroll
                 for (int c = 0; c < NCELL; ++c)
 #pragma unroll
-                    for (int r = 0; r < RV; ++r) tmp[c * RV + r] = pl[c >> 2][c & 3][r];
-                compute_level_slow<RV>(s, s.lv[b], tmp, T, tid, lane, write_x ? xout : nullptr, write_y ? yout : nullptr);
+                    for (int r = 0; r < RV; ++r) {
+                        tmp[c * RV + r] = pl[c >> 2][c & 3][r];
+                        if (ORD == 2) tmp2[c * RV + r] = pl2[ORD == 2 ? c >> 2 : 0][c & 3][r];
+                    }
+                compute_level_slow<RV, ORD>(s, s.lv[b], tmp, tmp2, T, tid, lane, write_x ? xout : nullptr, write_y ? yout : nullptr);
 #pragma unroll
                 for (int c = 0; c < NCELL; ++c)
 #pragma unroll
-                    for (int r = 0; r < RV; ++r) pl[c >> 2][c & 3][r] = tmp[c * RV + r];
+                    for (int r = 0; r < RV; ++r) {
+                        pl[c >> 2][c & 3][r] = tmp[c * RV + r];
+                        if (ORD == 2) pl2[ORD == 2 ? c >> 2 : 0][c & 3][r] = tmp2[c * RV + r];
+                    }
             } else {
-                compute_level<RV>(s.lv[b], pl, T, tid, lane, xout, write_x, yout, write_y);
+                compute_level<RV, ORD>(s.lv[b], pl, pl2, T, tid, lane, xout, write_x, yout, write_y);
             }
             if (edge) {
-                rwb_store<RV>(s, b, tid, vrw);
-                if (kp + 1 < P.nz) fill_faces<RV>(I, s, b ^ 1, tid, T.ag, T.yi, T.zi);
+                rwb_store<RV, ORD>(s, b, tid, vrw);
+                if (kp + 1 < P.nz) fill_faces<RV, ORD>(I, s, b ^ 1, tid, T.ag, T.yi, T.zi);
             }
             __syncthreads();
-            if (copy_of_thread<RV>(tid) < NCOPY && kp + 2 < P.nz) {
+            if (copy_of_thread<RV, ORD>(tid) < NCOPY && kp + 2 < P.nz) {
                 fence_proxy_async_smem();  // this level's reads of the staging buffers before the TMA overwrites them
-                issue_level<RV>(s, kp + 2, tid);
+                issue_level<RV, ORD>(s, kp + 2, tid);
             }
         }
         // ---- publish: faces of this item are complete ----
@@ -815,24 +929,31 @@ __global__ void __launch_bounds__(NVB / RV, 2) sweep_tile_kernel(const TileParam
     }
 }
 
-template <int RV>
+template <int RV, int ORD>
 cudaError_t configure(int *ctas_per_sm)
 {
-    cudaError_t e = cudaFuncSetAttribute(sweep_tile_kernel<RV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(TileSmem<RV>));
+    cudaError_t e = cudaFuncSetAttribute(sweep_tile_kernel<RV, ORD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(TileSmem<RV, ORD>));
     if (e != cudaSuccess) return e;
-    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, sweep_tile_kernel<RV>, NVB / RV, sizeof(TileSmem<RV>));
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, sweep_tile_kernel<RV, ORD>, KC<RV, ORD>::THREADS, sizeof(TileSmem<RV, ORD>));
 }
 
 }  // namespace
 
-size_t tile_smem_bytes(int rv) { return rv == 2 ? sizeof(TileSmem<2>) : sizeof(TileSmem<4>); }
-
-cudaError_t tile_configure(int rv, int *ctas_per_sm) { return rv == 2 ? configure<2>(ctas_per_sm) : configure<4>(ctas_per_sm); }
-
-cudaError_t launch_sweep_tile(const TileParams &P, int rv, int grid, cudaStream_t st)
+size_t tile_smem_bytes(int rv, int order)
 {
-    if (rv == 2) sweep_tile_kernel<2><<<grid, NVB / 2, sizeof(TileSmem<2>), st>>>(P);
-    else sweep_tile_kernel<4><<<grid, NVB / 4, sizeof(TileSmem<4>), st>>>(P);
+    return order == 2 ? sizeof(TileSmem<2, 2>) : rv == 2 ? sizeof(TileSmem<2, 1>) : sizeof(TileSmem<4, 1>);
+}
+
+cudaError_t tile_configure(int rv, int order, int *ctas_per_sm)
+{
+    return order == 2 ? configure<2, 2>(ctas_per_sm) : rv == 2 ? configure<2, 1>(ctas_per_sm) : configure<4, 1>(ctas_per_sm);
+}
+
+cudaError_t launch_sweep_tile(const TileParams &P, int rv, int order, int grid, cudaStream_t st)
+{
+    if (order == 2) sweep_tile_kernel<2, 2><<<grid, KC<2, 2>::THREADS, sizeof(TileSmem<2, 2>), st>>>(P);
+    else if (rv == 2) sweep_tile_kernel<2, 1><<<grid, KC<2, 1>::THREADS, sizeof(TileSmem<2, 1>), st>>>(P);
+    else sweep_tile_kernel<4, 1><<<grid, KC<4, 1>::THREADS, sizeof(TileSmem<4, 1>), st>>>(P);
     return cudaGetLastError();
 }
 

@@ -27,12 +27,24 @@ constexpr int TILE_TX = 4;                 // cells per tile along the sweep-rel
 constexpr int TILE_TY = DVM_TILE_TY;        // cells per tile along the sweep-relative y
 constexpr int TILE_NCELL = TILE_TX * TILE_TY;
 constexpr int TILE_GA = 4;                 // xi_x groups per lane quad
-constexpr int TILE_NVB = 512;              // velocities per block (incl. padding) = threads x RV
+constexpr int TILE_NVB = 512;              // velocities per block (incl. padding) = threads x RV, first-order kernels
 constexpr int TILE_MAXBC = 16;             // nbb + ncb of a block
 constexpr int TILE_PAD = 4;                // dead cells around the grid in the factor tables (tiles may overhang by 3)
-inline int tile_threads(int rv) { return TILE_NVB / rv; }
+// index ranges of the negative / non-negative nodes of one axis (nodes ascending): the two sweep directions
+inline void split_axis(const std::vector<double> &xi, int lo[2], int cnt[2])
+{
+    int nneg = 0;
+    while (nneg < (int)xi.size() && xi[nneg] < 0.0) ++nneg;
+    lo[0] = 0; cnt[0] = nneg; lo[1] = nneg; cnt[1] = (int)xi.size() - nneg;
+}
+// Kernel variants: (rv, order) = (4, 1): 128 threads x 4 velocities; (2, 1): 256 x 2; (2, 2): the second-order sweep
+// (DVM_OPT_ORDER = 2) keeps two z-planes in registers: 128 threads x 2 velocities, 256 velocities per block.
+inline int tile_threads(int rv, int order = 1) { return order == 2 ? 128 : TILE_NVB / rv; }
+inline int tile_nvb(int rv, int order = 1) { return tile_threads(rv, order) * rv; }   // velocities per block
 inline int tile_na(int rv) { return TILE_GA * rv; }          // xi_x nodes per velocity block
-inline int tile_npair(int rv) { return TILE_NVB / rv / TILE_GA; }   // (xi_y, xi_z) pairs per block = nbb * ncb
+inline int tile_npair(int rv, int order = 1) { return tile_threads(rv, order) / TILE_GA; }   // (xi_y, xi_z) pairs per block
+inline int tile_entry_doubles(int order) { return order == 2 ? 6 : 4; }   // factor-table entry: (E, Q, e, a) or (E, Q, e, cd, c1, c2)
+inline int tile_face_layers(int order) { return order == 2 ? 2 : 1; }     // upwind values per direction carried through a face
 
 // per-cell record of the padded grid, fetched by TMA with the factor tables (48 bytes)
 constexpr int REC_DEAD = 1 << 16;
@@ -69,7 +81,7 @@ struct TileItem {
 
 struct TilePlan {
     int ntx = 0, nty = 0, P = 1;
-    int rv = 4;                        // velocities per thread of the kernel variant this plan is for
+    int rv = 4, order = 1;             // kernel variant this plan is for: velocities per thread, order of the sweep
     int batch = 0;                     // velocity blocks in flight at once (= face-slot sets)
     int nbb = 8, ncb = 4;              // one (xi_y, xi_z) block shape for the whole problem
     std::vector<int> xnode, ynode, znode;   // node index per 1-D block slot (-1 = padding): [nxb][NA], [nyb][nbb], [nzb][ncb];
@@ -103,23 +115,24 @@ struct TileParams {
     int *counter;                 // next item
     int epoch;
     double *xface, *yface;
-    long long xslot_doubles, yslot_doubles;   // nz * TILE_TY * TILE_NVB, nz * TILE_TX * TILE_NVB
-    // factor tables of step n (tables_kernel), padded grid nxp x nyp x nz, entries double4 (E, Q, e, a):
-    const double4 *TX, *TY, *TZ;  // [nxb][nz][nyp][nxp][NA], [nyb][nz][nyp][nxp][nbb], [nzb][nz][nyp][nxp][ncb]
+    long long xslot_doubles, yslot_doubles;   // nz * layers * TILE_TY * NVB, nz * layers * TILE_TX * NVB
+    // factor tables of step n (tables_kernel), padded grid nxp x nyp x nz, entries (E, Q, e, a) [order 2: (E, Q, e, cd, c1, c2)]:
+    const double *TX, *TY, *TZ;   // [nxb][nz][nyp][nxp][NA][4 or 6], [nyb][nz][nyp][nxp][nbb][.], [nzb][nz][nyp][nxp][ncb][.]
     const CellRec *rec;           // [nz][nyp][nxp]
     int nxp, nyp, nbb, ncb;
 };
 
 struct TableParams {
-    int nx, ny, nz, nxp, nyp, na, nbb, ncb, nxb, nyb, nzb;
+    int nx, ny, nz, nxp, nyp, na, nbb, ncb, nxb, nyb, nzb, order;
     long long ncell;
     const double *coef;           // [NCOEF][ncell]
     const unsigned char *flags;   // bit 6: solid
     const double *invdx, *invdy, *invdz;
+    const double *dx, *dy, *dz;   // cell widths (order 2)
     const double *xi_x, *xi_y, *xi_z, *w_x, *w_y, *w_z;
     const int *xnode, *ynode, *znode;
     int bc_type[6];
-    double4 *TX, *TY, *TZ;
+    double *TX, *TY, *TZ;
     CellRec *rec;
 };
 
@@ -127,11 +140,12 @@ struct TableParams {
 // items that should be able to run concurrently (sets the band height P); max_blocks > 0 caps the velocity blocks in
 // flight at once (batches).  Pure host code (tests call it through
 // dvm_plan_query without a GPU).
-int tile_plan(int nx, int ny, int nz, const std::vector<double> xi[3], int target_ctas, int max_blocks, int rv, TilePlan *plan);
+int tile_plan(int nx, int ny, int nz, const std::vector<double> xi[3], int target_ctas, int max_blocks, int rv, int order,
+              TilePlan *plan);
 
-size_t tile_smem_bytes(int rv);
-cudaError_t tile_configure(int rv, int *ctas_per_sm);
-cudaError_t launch_sweep_tile(const TileParams &P, int rv, int grid, cudaStream_t st);
+size_t tile_smem_bytes(int rv, int order);
+cudaError_t tile_configure(int rv, int order, int *ctas_per_sm);
+cudaError_t launch_sweep_tile(const TileParams &P, int rv, int order, int grid, cudaStream_t st);
 cudaError_t launch_tables(const TableParams &T, cudaStream_t st);
 
 }  // namespace dvm

@@ -15,23 +15,16 @@ namespace dvm {
 
 namespace {
 
-// index ranges of the negative / non-negative nodes of one axis (nodes ascending)
-void split_axis(const std::vector<double> &xi, int lo[2], int cnt[2])
-{
-    int nneg = 0;
-    while (nneg < (int)xi.size() && xi[nneg] < 0.0) ++nneg;
-    lo[0] = 0; cnt[0] = nneg; lo[1] = nneg; cnt[1] = (int)xi.size() - nneg;
-}
-
 int ceil_div(int a, int b) { return (a + b - 1) / b; }
 
 }  // namespace
 
-int tile_plan(int nx, int ny, int nz, const std::vector<double> xi[3], int target_ctas, int max_blocks, int rv, TilePlan *plan)
+int tile_plan(int nx, int ny, int nz, const std::vector<double> xi[3], int target_ctas, int max_blocks, int rv, int order,
+              TilePlan *plan)
 {
-    if (nx <= 0 || ny <= 0 || nz <= 0 || !plan || (rv != 2 && rv != 4)) return -1;
-    const int NA = tile_na(rv);
-    plan->rv = rv;
+    if (nx <= 0 || ny <= 0 || nz <= 0 || !plan || (rv != 2 && rv != 4) || (order != 1 && order != 2) || (order == 2 && rv != 2)) return -1;
+    const int NA = tile_na(rv), NVB = tile_nvb(rv, order), npair = tile_npair(rv, order), layers = tile_face_layers(order);
+    plan->rv = rv; plan->order = order;
     plan->vblocks.clear();
     plan->items.clear();
     int lo[3][2], cnt[3][2];
@@ -39,11 +32,11 @@ int tile_plan(int nx, int ny, int nz, const std::vector<double> xi[3], int targe
 
     // ---- (nbb, ncb) with nbb * ncb = pairs per block and nbb + ncb <= TILE_MAXBC: one shape for the whole problem (the
     //      factor tables are laid out by 1-D block), the one wasting the fewest lanes ----
-    int best_bb = 8, best_cb = rv == 2 ? 8 : 4;
+    int best_bb = 8, best_cb = npair / 8;
     {
         long best = -1;
         const int shapes4[2][2] = {{8, 4}, {4, 8}}, shapes2[2][2] = {{8, 8}, {8, 8}};
-        for (auto &s : (rv == 2 ? shapes2 : shapes4)) {
+        for (auto &s : (npair == 64 ? shapes2 : shapes4)) {
             long slots = 0;
             for (int oz = 0; oz < 2; ++oz) for (int oy = 0; oy < 2; ++oy)
                 slots += (long)ceil_div(cnt[1][oy], s[0]) * ceil_div(cnt[2][oz], s[1]);
@@ -129,8 +122,8 @@ int tile_plan(int nx, int ny, int nz, const std::vector<double> xi[3], int targe
             }
         }
     }
-    plan->xface_doubles = (size_t)B * P * nz * TILE_TY * TILE_NVB;
-    plan->yface_doubles = (size_t)B * ntx * nz * TILE_TX * TILE_NVB;
+    plan->xface_doubles = (size_t)B * P * nz * layers * TILE_TY * NVB;
+    plan->yface_doubles = (size_t)B * ntx * nz * layers * TILE_TX * NVB;
     return 0;
 }
 

@@ -160,17 +160,14 @@ __global__ void __launch_bounds__(UB) residual_kernel(const UpdateParams U, int 
     }
     __syncthreads();
     if (threadIdx.x == 0) {
-        int bad = 0;
         for (int m = 0; m < 3; ++m) {
             const double num = tot[2 * m], den = tot[2 * m + 1];
             double r;
             if (den > 0.0) r = sqrt(num / den);
             else r = num > 0.0 ? __longlong_as_double(0x7ff0000000000000LL) : (num == 0.0 ? 0.0 : num);
-            if (!isfinite(r)) bad = 1;
             U.hist[3 * slot + m] = r;
         }
         U.hist_scale[slot] = U.scal[0];
-        if (bad) U.scal[2] = 1.0;
     }
 }
 
@@ -191,17 +188,35 @@ __global__ void __launch_bounds__(UB) raw_export_kernel(const double *raw16, dou
 }
 
 // Wall-incident fluxes of Eq.(9) from the half-range first moments the tile sweep leaves in the accumulator
-// rows: a face on side d of its cell is hit by the velocities moving towards d, Phi = sum w |xi_n| f over them.
+// rows: a face on side d of its cell is hit by the velocities moving towards d, Phi = sum w |xi_n| f over them.  With the
+// second-order sweep (reading G21) the flux takes the value extrapolated to the face, f_c + psi (f_c - f_c1): the same
+// combination of the half-range sums of the cell and of its upwind neighbour c1 (psi = 0 if c1 is not a fluid cell).
+struct PhiGeom {
+    int order, nx, ny, nz;
+    const unsigned char *flags;
+    const double *dx, *dy, *dz;
+};
 __global__ void __launch_bounds__(UB) phi_from_raw_kernel(const double *raw16, const int *face_cell, const int *face_dir, double *phi,
-                                                          int nface)
+                                                          int nface, const PhiGeom G)
 {
     const int f = blockIdx.x * UB + threadIdx.x;
     if (f >= nface) return;
     const int c = face_cell[f], d = face_dir[f];
     double v = 0.0;
     if (c >= 0) {
-        const double *r = raw16 + (long long)c * 16;
-        v = (d & 1) ? r[1 + (d >> 1)] : -r[13 + (d >> 1)];
+        const int slot = (d & 1) ? 1 + (d >> 1) : 13 + (d >> 1);
+        const double sgn = (d & 1) ? 1.0 : -1.0;
+        v = sgn * raw16[(long long)c * 16 + slot];
+        if (G.order == 2 && !((G.flags[c] >> (d ^ 1)) & 1u)) {
+            const int ax = d >> 1, s = (d & 1) ? 1 : -1;
+            const int i = c % G.nx, j = (c / G.nx) % G.ny, k = c / (G.nx * G.ny);
+            const int id = ax == 0 ? i : ax == 1 ? j : k;
+            const double *w = ax == 0 ? G.dx : ax == 1 ? G.dy : G.dz;
+            const long long stride = ax == 0 ? 1 : ax == 1 ? G.nx : (long long)G.nx * G.ny;
+            const double psi = w[id] / (w[id] + w[id - s]);
+            const double v1 = sgn * raw16[((long long)c - s * stride) * 16 + slot];
+            v += psi * (v - v1);
+        }
     }
     phi[f] = v;
 }
@@ -220,9 +235,10 @@ cudaError_t launch_raw_export(const double *raw16, double *out13, long long n, c
     return cudaGetLastError();
 }
 
-cudaError_t launch_phi_from_raw(const double *raw16, const int *face_cell, const int *face_dir, double *phi, int nface, cudaStream_t st)
+cudaError_t launch_phi_from_raw(const UpdateParams &U, const int *face_cell, const int *face_dir, double *phi, int order, cudaStream_t st)
 {
-    phi_from_raw_kernel<<<nblk(nface), UB, 0, st>>>(raw16, face_cell, face_dir, phi, nface);
+    PhiGeom G{order, U.nx, U.ny, U.nz, U.flags, U.dx, U.dy, U.dz};
+    phi_from_raw_kernel<<<nblk(U.nface), UB, 0, st>>>(U.raw, face_cell, face_dir, phi, U.nface, G);
     return cudaGetLastError();
 }
 

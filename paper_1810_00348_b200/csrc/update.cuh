@@ -15,7 +15,7 @@ struct UpdateParams {
     double *prim_new;           // [14][ncell] unscaled conversion of this iteration
     double *coef;               // [9][ncell]
     double *part;               // [7][npart] block partials: mass, 6 residual sums
-    double *scal;               // [0] rescale factor, [1] total mass before rescale, [2] non-finite flag
+    double *scal;               // [0] rescale factor, [1] total mass before rescale
     double *hist;               // [cap][3] residual history ring
     double *hist_scale;         // [cap]
     const double *phi;          // [nface]
@@ -29,7 +29,7 @@ struct SweepParams;
 
 cudaError_t launch_raw_export(const double *raw16, double *out13, long long n, cudaStream_t st);
 cudaError_t launch_pack(const UpdateParams &U, cudaStream_t st);
-cudaError_t launch_phi_from_raw(const double *raw16, const int *face_cell, const int *face_dir, double *phi, int nface, cudaStream_t st);
+cudaError_t launch_phi_from_raw(const UpdateParams &U, const int *face_cell, const int *face_dir, double *phi, int order, cudaStream_t st);
 cudaError_t launch_update(const UpdateParams &U, int hist_slot, cudaStream_t st, int *launches);
 cudaError_t launch_sweep_slice(const SweepParams &P, int nblocks, int nb, cudaStream_t st);
 

@@ -123,9 +123,9 @@ def lib():
         L.dvm_workspace_bytes.argtypes = [vp, C.POINTER(C.c_size_t), C.POINTER(C.c_size_t)]
         L.dvm_kernel_used.argtypes = [vp]
         L.dvm_tile_rv.argtypes = [vp]
-        L.dvm_plan_query.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(_VGrid), C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int),
-                                     C.POINTER(C.c_int), C.c_int]
-        L.dvm_plan_vblocks.argtypes = [C.POINTER(_VGrid), C.c_int, C.POINTER(C.c_int), C.c_int]
+        L.dvm_plan_query.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(_VGrid), C.c_int, C.c_int, C.c_int, C.c_int,
+                                     C.POINTER(C.c_int), C.POINTER(C.c_int), C.c_int]
+        L.dvm_plan_vblocks.argtypes = [C.POINTER(_VGrid), C.c_int, C.c_int, C.POINTER(C.c_int), C.c_int]
         L.dvm_launch_count.argtypes = [vp]
         L.dvm_launch_count.restype = C.c_longlong
         L.dvm_destroy.argtypes = [vp]
@@ -144,26 +144,26 @@ def _f64(a):
     return np.ascontiguousarray(a, dtype=np.float64)
 
 
-def plan_query(nx, ny, nz, xi_x, xi_y, xi_z, target_ctas=296, max_blocks=0, max_items=1 << 22, rv=0):
+def plan_query(nx, ny, nz, xi_x, xi_y, xi_z, target_ctas=296, max_blocks=0, max_items=1 << 22, rv=0, order=1):
     """dvm_plan_query: (counts dict, items int32 [n][9]) of the tile kernel's work decomposition (host only)."""
     keep = [_f64(a) for a in (xi_x, xi_y, xi_z)]
     v = _VGrid(len(keep[0]), len(keep[1]), len(keep[2]), *(a.ctypes.data_as(_dp) for a in keep), None, None, None)
     counts = (C.c_int * 5)()
-    n = _check(lib().dvm_plan_query(nx, ny, nz, C.byref(v), target_ctas, max_blocks, rv, counts, None, 0))
+    n = _check(lib().dvm_plan_query(nx, ny, nz, C.byref(v), target_ctas, max_blocks, rv, order, counts, None, 0))
     items = np.zeros((min(n, max_items), 9), dtype=np.int32)
-    _check(lib().dvm_plan_query(nx, ny, nz, C.byref(v), target_ctas, max_blocks, rv, counts,
+    _check(lib().dvm_plan_query(nx, ny, nz, C.byref(v), target_ctas, max_blocks, rv, order, counts,
                                 items.ctypes.data_as(C.POINTER(C.c_int)), len(items)))
     return {"n_vblocks": counts[0], "ntx": counts[1], "nty": counts[2], "P": counts[3], "batch": counts[4],
             "n_items": n}, items
 
 
-def plan_vblocks(xi_x, xi_y, xi_z, rv=0):
+def plan_vblocks(xi_x, xi_y, xi_z, rv=0, order=1):
     """dvm_plan_vblocks: int32 [n][8] = a0, na, b0, nb, c0, nc, NA, 256 nbb + ncb per velocity block (host only)."""
     keep = [_f64(a) for a in (xi_x, xi_y, xi_z)]
     v = _VGrid(len(keep[0]), len(keep[1]), len(keep[2]), *(a.ctypes.data_as(_dp) for a in keep), None, None, None)
-    n = _check(lib().dvm_plan_vblocks(C.byref(v), rv, None, 0))
+    n = _check(lib().dvm_plan_vblocks(C.byref(v), rv, order, None, 0))
     out = np.zeros((n, 8), dtype=np.int32)
-    _check(lib().dvm_plan_vblocks(C.byref(v), rv, out.ctypes.data_as(C.POINTER(C.c_int)), n))
+    _check(lib().dvm_plan_vblocks(C.byref(v), rv, order, out.ctypes.data_as(C.POINTER(C.c_int)), n))
     return out
 
 

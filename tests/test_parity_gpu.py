@@ -453,42 +453,60 @@ def test_dependency_protocol_under_stress(oracle_mod, ctas, rv):
 
 
 # ---------------------------------------------------------------------------------------------------------------------
-# Second-order upwind sweep (DVM_OPT_ORDER = 2; oracle pins in tests/test_oracle_order2.py)
-def test_order2_config0_every_iteration(oracle_mod):
-    lockstep(W.config(0).with_(order=2), 0, 20, oracle_mod)
+# Second-order upwind sweep (DVM_OPT_ORDER = 2; oracle pins in tests/test_oracle_order2.py), both kernels:
+# the slice kernel with a second stored slice, the tile kernel with two z-planes in registers and two-deep faces.
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_order2_config0_every_iteration(oracle_mod, kernel):
+    lockstep(W.config(0).with_(order=2), kernel, 20, oracle_mod)
 
 
-def test_order2_ragged_stretched_cavity(oracle_mod):
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_order2_ragged_stretched_cavity(oracle_mod, kernel):
     wl = W.cavity(0, 0, 0.075, stretch=1.5, nxyz=(13, 9, 11), mxyz=(10, 7, 9)).with_(order=2)
-    lockstep(wl, 0, 3, oracle_mod)
+    lockstep(wl, kernel, 3, oracle_mod)
+    wide = W.cavity(0, 0, 0.3, nxyz=(6, 5, 7), mxyz=(40, 10, 9)).with_(order=2)
+    lockstep(wide, kernel, 2, oracle_mod, state=W.perturbed_state(wide, seed=41, amp_q=0.01), rho_w=None)
 
 
-def test_order2_cube_flows(oracle_mod):
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_order2_cube_flows(oracle_mod, kernel):
     """free stream + zero-gradient outflow + solid mask; then the paper's stretched cube grid at reduced size"""
-    lockstep(W.cube_flow(4, 12, box=(6, 4, 4), vrange=8.0).with_(order=2), 0, 3, oracle_mod)
-    lockstep(W.cube_flow_paper(5, 6, 6, 7, 12).with_(order=2), 0, 3, oracle_mod)
+    lockstep(W.cube_flow(4, 12, box=(6, 4, 4), vrange=8.0).with_(order=2), kernel, 3, oracle_mod)
+    lockstep(W.cube_flow_paper(5, 6, 6, 7, 12).with_(order=2), kernel, 3, oracle_mod)
 
 
-def test_order2_degenerate_and_solid_block(oracle_mod):
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_order2_degenerate_and_solid_block(oracle_mod, kernel):
     wl = W.cavity(1, 6, 0.5, nxyz=(12, 1, 1))
     zg = W.FaceBC(W.ZERO_GRADIENT)
     wl = wl.with_(faces=[W.FaceBC(W.WALL_DIFFUSE, 1.2, 1.0, (0, 0, 0)), W.FaceBC(W.FREESTREAM, 0.9, 1.1, (0.1, 0, 0)),
                          zg, zg, zg, zg], rescale_mass=0, order=2)
-    lockstep(wl, 0, 2, oracle_mod)
+    lockstep(wl, kernel, 2, oracle_mod)
     solid = np.zeros((6, 6, 6), dtype=np.uint8)
     solid[2:4, 1:3, 3:5] = 1
-    lockstep(W.cavity(6, 12, 0.3).with_(solid=solid, order=2), 0, 3, oracle_mod)
-    lockstep(W.cavity(3, 2, 1.0).with_(order=2), 0, 2, oracle_mod)
+    lockstep(W.cavity(6, 12, 0.3).with_(solid=solid, order=2), kernel, 3, oracle_mod)
+    lockstep(W.cavity(3, 2, 1.0).with_(order=2), kernel, 2, oracle_mod)
 
 
-def test_order2_config1_first_iterations(oracle_mod):
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_order2_config1_first_iterations(oracle_mod, kernel):
     wl = W.config(1).with_(order=2)
-    s = lockstep(wl, 0, 3, oracle_mod, state=W.perturbed_state(wl, seed=1810, amp_q=0.01), rho_w=np.ones(6 * 32 * 32))
+    lockstep(wl, kernel, 3, oracle_mod, state=W.perturbed_state(wl, seed=1810, amp_q=0.01), rho_w=np.ones(6 * 32 * 32))
 
 
-def test_order2_is_refused_by_the_tile_kernel():
+def test_order2_config3_full_size_stratified_step(oracle_mod):
+    """second-order tile kernel on config 3 at full size, one velocity in each of its (256-velocity) blocks"""
     from paper_1810_00348_b200 import dvm
-    s = dvm.Solver(W.config(0).with_(order=2), kernel=dvm.KERNEL_TILE)
-    with pytest.raises(dvm.DvmError):
-        s.iterate(1)
+    wl = W.config(3).with_(order=2)
+    sub = W.stratified_weight_subset(wl, dvm.plan_vblocks(wl.xi_x, wl.xi_y, wl.xi_z, 2, 2), 1)
+    lockstep(sub, 2, 1, oracle_mod, state=W.perturbed_state(sub, seed=35, amp_q=0.01), rho_w=None)
+
+
+def test_order2_fixed_points_on_the_tile_kernel():
+    wl = W.cavity(8, 24, 0.1, U_w=0.0).with_(order=2)
+    s = make(wl, 2)
+    s.iterate(2)
+    g = s.moments().cpu().numpy()
+    assert np.abs(g[0] - 1).max() < 1e-12 and np.abs(g[4] - 1).max() < 1e-12 and np.abs(g[1:4]).max() < 1e-12
+    assert s.tile_rv() == 2
     s.close()
