@@ -510,3 +510,57 @@ def test_order2_fixed_points_on_the_tile_kernel():
     assert np.abs(g[0] - 1).max() < 1e-12 and np.abs(g[4] - 1).max() < 1e-12 and np.abs(g[1:4]).max() < 1e-12
     assert s.tile_rv() == 2
     s.close()
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# Full-weight steps against the archived oracle: tests/golden/full_step_cfg<N>.txt is written by
+# tests/golden/make_full_step_goldens.py (oracle only; config 4 took ~1.9 h of 16 host cores) - every velocity of the
+# configuration contributes, not a subset.
+def _golden_full_steps():
+    from pathlib import Path
+    return sorted(int(p.stem.split("cfg")[1]) for p in (Path(__file__).parent / "golden").glob("full_step_cfg*.txt"))
+
+
+@pytest.mark.parametrize("cfg", _golden_full_steps())
+def test_full_weight_step_against_archived_oracle(cfg):
+    from pathlib import Path
+    import importlib.util
+    spec = importlib.util.spec_from_file_location("make_goldens", Path(__file__).parent / "golden" / "make_full_step_goldens.py")
+    mg = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mg)                      # imports oracle/ (test infrastructure) for the writer; not used here
+    wl, prim, cells = mg.seeded_state(cfg)
+    gold = {"cell": {}, "face": {}, "field": {}}
+    for line in (Path(__file__).parent / "golden" / f"full_step_cfg{cfg}.txt").read_text().splitlines():
+        if line.startswith("#") or not line.strip():
+            continue
+        k, *v = line.split()
+        if k == "resid":
+            gold["resid"] = np.array([float(x) for x in v])
+        elif k == "scale":
+            gold["scale"] = float(v[0])
+        else:
+            gold[k][int(v[0])] = np.array([float(x) for x in v[1:]])
+    s = make(wl, 2)
+    s.set_state(prim, None)
+    s.iterate(1)
+    g14 = s.moments().cpu().numpy()
+    rw = s.get_state()[1].cpu().numpy()
+    assert sorted(gold["cell"]) == [int(c) for c in cells]
+    fmax = np.array([gold["field"][m][0] for m in range(14)])
+    groups = {"rho": [0], "u": [1, 2, 3], "T": [4], "q": [5, 6, 7], "sigma": [8, 9, 10, 11, 12, 13]}
+    for name, idx in groups.items():
+        scale = fmax[idx].max()
+        err = max(np.abs(g14[idx, c] - gold["cell"][c][idx]).max() for c in gold["cell"])
+        assert err <= 1e-11 * scale, (name, err / scale)
+    fluid = np.ones(wl.n_cells, bool) if wl.solid is None else wl.solid.reshape(-1) == 0
+    for m in range(14):
+        f = g14[m][fluid]
+        amax, ssum, ssq = gold["field"][m]
+        assert abs(np.abs(f).max() - amax) <= 1e-11 * fmax[[i for i in groups.values() if m in i][0]].max()
+        assert abs((f * f).sum() - ssq) <= 1e-10 * max(ssq, 1e-300)
+        assert abs(f.sum() - ssum) <= 1e-10 * np.abs(f).sum()
+    for fidx, val in gold["face"].items():
+        assert abs(rw[fidx] - val[0]) <= 1e-11 * abs(val[0])
+    assert_residual(s.residual(), gold["resid"], what=f"archived full-weight step of config {cfg}")
+    assert abs(s.mass_scale() - gold["scale"]) <= 1e-12 * abs(gold["scale"])
+    s.close()
