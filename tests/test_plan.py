@@ -6,8 +6,9 @@ import pytest
 from paper_1810_00348_b200 import dvm, workloads as W
 
 
-def plan(wl, target=296, max_blocks=0):
-    return dvm.plan_query(wl.nx, wl.ny, wl.nz, wl.xi_x, wl.xi_y, wl.xi_z, target_ctas=target, max_blocks=max_blocks)
+def plan(wl, target=296, max_blocks=0, rv=0, order=1):
+    return dvm.plan_query(wl.nx, wl.ny, wl.nz, wl.xi_x, wl.xi_y, wl.xi_z, target_ctas=target, max_blocks=max_blocks, rv=rv,
+                          order=order)
 
 
 @pytest.mark.parametrize("wl,target,max_blocks", [
@@ -18,8 +19,9 @@ def plan(wl, target=296, max_blocks=0):
     (W.config(1), 296, 5), (W.config(2), 296, 24), (W.config(0), 296, 1),
     (W.cavity(0, 0, 0.1, nxyz=(13, 9, 11), mxyz=(10, 7, 9)), 16, 3),
 ])
-def test_items_cover_everything_once_in_dependency_order(wl, target, max_blocks):
-    counts, items = plan(wl, target, max_blocks)
+@pytest.mark.parametrize("rv,order", [(4, 1), (2, 1), (2, 2)])
+def test_items_cover_everything_once_in_dependency_order(wl, target, max_blocks, rv, order):
+    counts, items = plan(wl, target, max_blocks, rv, order)
     n = counts["n_items"]
     assert len(items) == n == counts["n_vblocks"] * counts["ntx"] * counts["nty"]
     assert counts["ntx"] == -(-wl.nx // 4) and counts["nty"] in (-(-wl.ny // 4), -(-wl.ny // 2))   # tiles are 4 x 4 or 4 x 2
@@ -101,3 +103,23 @@ def test_stratified_subset_puts_one_velocity_in_every_block(cfg, rv):
             assert (xi[k] < 0).any() and (xi[k] >= 0).any()
         kept.append((kx, ky, kz))
     assert not np.array_equal(kept[0][0], kept[1][0])
+
+
+@pytest.mark.parametrize("rv,order,nvb,na", [(4, 1, 512, 16), (2, 1, 512, 8), (2, 2, 256, 8)])
+def test_velocity_block_boxes(rv, order, nvb, na):
+    """dvm_plan_vblocks: the boxes tile the velocity grid exactly once, stay inside one sign octant, and fit the lanes of
+    the kernel variant (NA x nbb x ncb = velocities per block)."""
+    wl = W.config(3)
+    boxes = dvm.plan_vblocks(wl.xi_x, wl.xi_y, wl.xi_z, rv, order)
+    cover = np.zeros((wl.mx, wl.my, wl.mz), dtype=np.int32)
+    for a0, n_a, b0, n_b, c0, n_c, NA, shape in boxes:
+        nbb, ncb = shape // 256, shape % 256
+        assert NA == na and NA * nbb * ncb == nvb
+        assert 0 < n_a <= NA and 0 < n_b <= nbb and 0 < n_c <= ncb
+        cover[a0:a0 + n_a, b0:b0 + n_b, c0:c0 + n_c] += 1
+        for xi, lo, cnt in ((wl.xi_x, a0, n_a), (wl.xi_y, b0, n_b), (wl.xi_z, c0, n_c)):
+            s = xi[lo:lo + cnt] >= 0
+            assert s.all() or not s.any()
+    assert (cover == 1).all()
+    with pytest.raises(dvm.DvmError):
+        dvm.plan_vblocks(wl.xi_x, wl.xi_y, wl.xi_z, 4, 2)      # the second-order kernel carries 2 velocities per thread
