@@ -320,7 +320,7 @@ def main():
     ap.add_argument("--ref-budget", type=float, default=15.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--max-f-mbytes", type=int, default=0, help="cap (MiB) on the f workspace of the tile kernel (0 = none)")
-    ap.add_argument("--tile-rv", type=int, default=0, choices=[0, 2, 4], help="velocities per thread of the tile kernel (0 = library's choice)")
+    ap.add_argument("--tile-rv", type=int, default=0, choices=[0, 2, 3, 4], help="velocities per thread of the tile kernel (0 = library's choice)")
     ap.add_argument("--order", type=int, default=1, choices=[1, 2], help="order of the upwind sweep (2: slice kernel)")
     args = ap.parse_args()
     if args.impl == "reference":

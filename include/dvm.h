@@ -59,6 +59,8 @@ extern "C" {
 
 #define DVM_OPT_KERNEL    1
 #define DVM_OPT_MAX_F_MBYTES 2 /* tile kernel: cap (MiB) on the f workspace; velocity blocks then sweep in batches (0 = none) */
+#define DVM_OPT_TILE_AXIS 6 /* tile kernel: velocity axis that plays the wide role (RV nodes per thread x 4 lane groups): 1 = xi_x,
+                             2 = xi_y, 3 = xi_z; 0 = the library chooses the axis (and RV) that wastes the fewest lanes (default) */
 #define DVM_OPT_ORDER     5 /* order of the upwind sweep: 1 = Eq.(7) (default); 2 = second-order upwind, the extension PAPER.md:393 names
                              ("second order by storing three consecutive slices"): Eq.(7) in flux-difference form with the value
                              at a cell's downwind face extrapolated linearly from the two upwind cell centres (the cell value
@@ -67,8 +69,9 @@ extern "C" {
                              (2 velocities per thread); slice kernel: two stored slices + the one being written */
 #define DVM_OPT_MAX_CTAS  4 /* tile kernel: cap on the persistent grid (0 = every resident CTA); 1 runs the work items strictly in
                              hand-out order on one CTA - for tests of the dependency protocol, not for speed */
-#define DVM_OPT_TILE_RV   3 /* tile kernel: velocities per thread, 4 (128-thread CTAs, velocity blocks of 16 x 8 x 4 nodes) or 2
-                             (256-thread CTAs, blocks of 8 x 8 x 8 nodes); 0 = the library chooses by lane use (default) */
+#define DVM_OPT_TILE_RV   3 /* tile kernel: velocities per thread, 4 (128-thread CTAs, velocity blocks of 16 x 8 x 4 nodes), 3 (128
+                             threads, 12 x 8 x 4: fills sign halves of 12 k nodes) or 2 (256-thread CTAs, blocks of 8 x 8 x 8
+                             nodes); 0 = the library chooses by lane use x measured speed of the variant (default) */
 
 typedef struct dvm_solver dvm_solver; /* opaque */
 
@@ -159,21 +162,24 @@ int dvm_set_option(dvm_solver *s, int option, int value);
 int dvm_kernel_used(const dvm_solver *s);
 /* Velocities per thread of the tile kernel: 2 or 4 once the first dvm_iterate has planned, the requested value before. */
 int dvm_tile_rv(const dvm_solver *s);
+/* 1 + velocity axis in the wide role of the tile kernel once planned (DVM_OPT_TILE_AXIS), the requested value before. */
+int dvm_tile_axis(const dvm_solver *s);
 /* Host-only (needs no device): the work decomposition the tile kernel would use for an nx x ny x nz grid and the
  * velocity nodes of v when target_ctas items should run concurrently, at most max_blocks velocity blocks are in
  * flight at once (0 = all; "smaller batches"), a thread carries rv velocities (2, 4, or 0 = the
- * library's choice for these nodes) and the sweep has the given order (1 or 2; order 2 needs rv = 2 or 0).  counts5 = number of velocity blocks, tiles along x, tiles
+ * library's choice for these nodes; 3 is a variant too), the sweep has the given order (1 or 2; order 2 needs rv = 2 or 0)
+ * and wide_axis is as DVM_OPT_TILE_AXIS (0 = the library's choice).  counts5 = number of velocity blocks, tiles along x, tiles
  * along y, band height P, blocks per batch.  items9 (may be NULL) receives, for the first max_items work items in
  * hand-out order, {velocity block, tile x, tile y, predecessor in x, predecessor in y (for tile y = 0 of a later batch:
  * the last reader of the y-face slot), previous user of the x-face slot, x-face slot, octant bits, face-slot set};
  * predecessors are item indices or -1.  Returns the number of items. */
-int dvm_plan_query(int nx, int ny, int nz, const dvm_vgrid *v, int target_ctas, int max_blocks, int rv, int order,
+int dvm_plan_query(int nx, int ny, int nz, const dvm_vgrid *v, int target_ctas, int max_blocks, int rv, int order, int wide_axis,
                    int *counts5, int *items9, int max_items);
 /* Host-only: the velocity blocks of the tile kernel for the nodes of v (rv, order as in dvm_plan_query), in block-id order (the
- * order of dvm_plan_query's items9[0]).  boxes8 (may be NULL) receives for the first max_blocks blocks {a0, na, b0, nb, c0,
- * nc, NA, 256 nbb + ncb}: the block holds the nodes [a0, a0+na) x [b0, b0+nb) x [c0, c0+nc) of one sign octant, in a box
- * of NA x nbb x ncb lanes.  Returns the number of blocks. */
-int dvm_plan_vblocks(const dvm_vgrid *v, int rv, int order, int *boxes8, int max_blocks);
+ * order of dvm_plan_query's items9[0]).  boxes8 (may be NULL) receives for the first max_blocks blocks {x0, nx, y0, ny, z0,
+ * nz, NA + 65536 (1 + wide axis), 256 nbb + ncb}: the block holds the nodes [x0, x0+nx) x [y0, y0+ny) x [z0, z0+nz) of xi_x,
+ * xi_y, xi_z, all of one sign octant, in a box of NA (along the wide axis) x nbb x ncb lanes.  Returns the number of blocks. */
+int dvm_plan_vblocks(const dvm_vgrid *v, int rv, int order, int wide_axis, int *boxes8, int max_blocks);
 /* Bytes of device workspace held by the solver, and the part of it that holds distribution-function values. */
 int dvm_workspace_bytes(const dvm_solver *s, size_t *total, size_t *f_bytes);
 /* Number of kernel launches enqueued by this solver so far (bench.py's gpu_launches). */

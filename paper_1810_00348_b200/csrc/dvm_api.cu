@@ -76,7 +76,8 @@ struct dvm_solver {
     int iters = 0;
     int kernel = DVM_KERNEL_AUTO;
     long long max_f_mbytes = 0;   // cap on the f workspace of the tile kernel (0 = none)
-    int tile_rv = 0;              // velocities per thread of the tile kernel: 0 = choose, 2, 4
+    int tile_rv = 0;              // velocities per thread of the tile kernel: 0 = choose, 2, 3, 4
+    int tile_axis = 0;            // velocity axis in the wide role of the tile kernel: 0 = choose, 1 + axis
     int max_ctas = 0;             // cap on the persistent grid of the tile kernel (0 = all resident CTAs)
     int order = 1;                // 1: first-order upwind Eq.(7); 2: second-order upwind
     bool planned = false;
@@ -235,6 +236,7 @@ TableParams table_params(dvm_solver *s)
 {
     TableParams T{};
     T.nx = s->nx; T.ny = s->ny; T.nz = s->nz; T.nxp = s->nxp; T.nyp = s->nyp;
+    for (int r = 0; r < 3; ++r) T.ax[r] = s->tile.ax[r];
     T.order = s->tile.order; T.dx = s->d_dx; T.dy = s->d_dy; T.dz = s->d_dz;
     T.na = tile_na(s->tile.rv); T.nbb = s->tile.nbb; T.ncb = s->tile.ncb; T.nxb = s->nxb; T.nyb = s->nyb; T.nzb = s->nzb;
     T.ncell = s->ncell; T.coef = s->d_coef; T.flags = s->d_flags;
@@ -247,24 +249,32 @@ TableParams table_params(dvm_solver *s)
     return T;
 }
 
-// Variant of the tile kernel for a velocity grid when the caller leaves the choice open: the one whose velocity blocks
-// (16 x 8 x 4 nodes for RV = 4, 8 x 8 x 8 for RV = 2) waste fewer lanes on padding; RV_BIAS is the measured throughput of
-// RV = 2 relative to RV = 4 when both fill their blocks.
-constexpr double RV_BIAS = 0.8;
-int choose_rv(const std::vector<double> xi[3])
+// Variant of the tile kernel for a velocity grid when the caller leaves the choice open: the (velocities per thread, wide
+// axis) pair with the highest expected throughput = (share of its lanes that carry a velocity: blocks of 16 x 32, 12 x 32
+// or 8 x 64 nodes per sign octant, the wide side along the chosen velocity axis) x (measured throughput of the variant
+// relative to RV = 4 when all fill their blocks).  rv / axis > 0 (resp. >= 0) fix that part.
+constexpr double RV_SPEED[5] = {0.0, 0.0, 0.80, 0.90, 1.0};
+void choose_variant(const std::vector<double> xi[3], int order, int rv_fixed, int axis_fixed, int *rv_out, int *axis_out)
 {
-    if (const char *e = std::getenv("DVM_TILE_RV")) {
-        const int v = std::atoi(e);
-        if (v == 2 || v == 4) return v;
-    }
+    if (rv_fixed == 0)
+        if (const char *e = std::getenv("DVM_TILE_RV")) { const int v = std::atoi(e); if (v >= 2 && v <= 4) rv_fixed = v; }
+    if (axis_fixed < 0)
+        if (const char *e = std::getenv("DVM_TILE_AXIS")) { const int v = std::atoi(e); if (v >= 0 && v <= 2) axis_fixed = v; }
+    if (order == 2) rv_fixed = 2;
     const long long nvel = (long long)xi[0].size() * xi[1].size() * xi[2].size();
-    double fill[2] = {0.0, 0.0};
-    for (int t = 0; t < 2; ++t) {
-        TilePlan tp;
-        if (tile_plan(4, 4, 1, xi, 1, 0, t == 0 ? 4 : 2, 1, &tp)) return 4;
-        fill[t] = (double)nvel / ((double)tp.vblocks.size() * TILE_NVB);
+    int best_rv = rv_fixed ? rv_fixed : 4, best_ax = axis_fixed >= 0 ? axis_fixed : 0;
+    double best_score = -1.0;
+    for (int rv = 4; rv >= 2; --rv) {
+        if (rv_fixed && rv != rv_fixed) continue;
+        for (int ax = 0; ax < 3; ++ax) {
+            if (axis_fixed >= 0 && ax != axis_fixed) continue;
+            TilePlan tp;
+            if (tile_plan(4, 4, 1, xi, 1, 0, rv, order, ax, &tp)) continue;
+            const double fill = (double)nvel / ((double)tp.vblocks.size() * tile_nvb(rv, order));
+            if (fill * RV_SPEED[rv] > best_score * 1.0000001) { best_score = fill * RV_SPEED[rv]; best_rv = rv; best_ax = ax; }
+        }
     }
-    return fill[1] * RV_BIAS > fill[0] ? 2 : 4;
+    *rv_out = best_rv; *axis_out = best_ax;
 }
 
 int plan_once(dvm_solver *s);
@@ -294,7 +304,7 @@ int plan_once(dvm_solver *s)
     const long long nvel = (long long)s->mx * s->my * s->mz;
     int kernel = s->kernel;
     if (kernel == DVM_KERNEL_AUTO) kernel = DVM_KERNEL_TILE;
-    if (kernel == DVM_KERNEL_TILE && s->order == 2 && s->tile_rv == 4)
+    if (kernel == DVM_KERNEL_TILE && s->order == 2 && s->tile_rv > 2)
         return fail(DVM_EINVAL, "the second-order tile kernel carries 2 velocities per thread (DVM_OPT_TILE_RV = 2 or 0)");
     s->kernel = kernel;
     int lo[3][2], cnt[3][2];
@@ -326,14 +336,15 @@ int plan_once(dvm_solver *s)
     } else {
         int per_sm = 0, dev = 0, nsm = 0;
         const int order = s->order;
-        const int rv = order == 2 ? 2 : s->tile_rv ? s->tile_rv : choose_rv(s->xi);
-        s->tile_rv = rv;
-        CK(tile_configure(rv, order, &per_sm));
+        int rv = 0, wide = 0;
+        choose_variant(s->xi, order, s->tile_rv, s->tile_axis - 1, &rv, &wide);
+        s->tile_rv = rv; s->tile_axis = wide + 1;
+        CK(tile_configure(rv, order, wide, &per_sm));
         CK(cudaGetDevice(&dev));
         CK(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
         if (per_sm < 1) return fail(DVM_ECUDA, "tile kernel does not fit on an SM");
         const int resident = per_sm * nsm;
-        if (tile_plan(s->nx, s->ny, s->nz, s->xi, resident, 0, rv, order, &s->tile)) return fail(DVM_EINVAL, "tile plan failed");
+        if (tile_plan(s->nx, s->ny, s->nz, s->xi, resident, 0, rv, order, wide, &s->tile)) return fail(DVM_EINVAL, "tile plan failed");
         if (s->max_f_mbytes > 0) {
             // cap on the f workspace: fewer velocity blocks in flight (batches); the band height P
             // grows as the batch shrinks, so iterate to a fixed point; one block is the floor
@@ -343,7 +354,7 @@ int plan_once(dvm_solver *s)
                 const double need = (double)(s->tile.xface_doubles + s->tile.yface_doubles) * 8.0;
                 if (need <= cap || B == 1) break;
                 B = std::max(1, std::min(B - 1, (int)(cap / ((s->tile.P * TILE_TY + s->tile.ntx * TILE_TX) * lvl))));
-                if (tile_plan(s->nx, s->ny, s->nz, s->xi, resident, B, rv, order, &s->tile)) return fail(DVM_EINVAL, "tile plan failed");
+                if (tile_plan(s->nx, s->ny, s->nz, s->xi, resident, B, rv, order, wide, &s->tile)) return fail(DVM_EINVAL, "tile plan failed");
             }
             const double need = (double)(s->tile.xface_doubles + s->tile.yface_doubles) * 8.0;
             if (need > cap)
@@ -621,8 +632,14 @@ int dvm_set_option(dvm_solver *s, int option, int value)
     }
     if (option == DVM_OPT_TILE_RV) {
         if (s->planned) return fail(DVM_EINVAL, "the tile-kernel variant must be chosen before the first iteration");
-        if (value != 0 && value != 2 && value != 4) return fail(DVM_EINVAL, "velocities per thread must be 0 (choose), 2 or 4");
+        if (value != 0 && (value < 2 || value > 4)) return fail(DVM_EINVAL, "velocities per thread must be 0 (choose), 2, 3 or 4");
         s->tile_rv = value;
+        return DVM_OK;
+    }
+    if (option == DVM_OPT_TILE_AXIS) {
+        if (s->planned) return fail(DVM_EINVAL, "the wide axis of the tile kernel must be chosen before the first iteration");
+        if (value < 0 || value > 3) return fail(DVM_EINVAL, "wide axis: 0 (choose), 1 = xi_x, 2 = xi_y, 3 = xi_z");
+        s->tile_axis = value;
         return DVM_OK;
     }
     if (option == DVM_OPT_ORDER) {
@@ -665,7 +682,7 @@ int dvm_iterate(dvm_solver *s, int niter)
             CK(cudaMemsetAsync(s->d_counter, 0, sizeof(int), s->stream));
             s->epoch += 1;
             const TileParams TP = tile_params(s);
-            CK(launch_sweep_tile(TP, s->tile_rv, s->order, s->tile_grid, s->stream));
+            CK(launch_sweep_tile(TP, s->tile_rv, s->order, s->tile.ax[0], s->tile_grid, s->stream));
             CK(launch_phi_from_raw(U, s->d_face_cell, s->d_face_dir, s->d_phi, s->order, s->stream));
             s->launches += 1;
         }
@@ -703,6 +720,7 @@ int dvm_num_faces(const dvm_solver *s) { return s ? s->nface : fail(DVM_EINVAL, 
 int dvm_iterations_done(const dvm_solver *s) { return s ? s->iters : fail(DVM_EINVAL, "NULL solver"); }
 int dvm_kernel_used(const dvm_solver *s) { return s ? s->kernel : fail(DVM_EINVAL, "NULL solver"); }
 int dvm_tile_rv(const dvm_solver *s) { return s ? s->tile_rv : fail(DVM_EINVAL, "NULL solver"); }
+int dvm_tile_axis(const dvm_solver *s) { return s ? s->tile_axis : fail(DVM_EINVAL, "NULL solver"); }
 long long dvm_launch_count(const dvm_solver *s) { return s ? s->launches : -1; }
 
 int dvm_get_state(dvm_solver *s, double *dev_prim14, double *dev_rho_wall)
@@ -790,16 +808,18 @@ int dvm_step_host(dvm_solver *s, const double *host_prim8, const double *host_rh
     return DVM_OK;
 }
 
-int dvm_plan_query(int nx, int ny, int nz, const dvm_vgrid *v, int target_ctas, int max_blocks, int rv, int order, int *counts5,
-                   int *items9, int max_items)
+int dvm_plan_query(int nx, int ny, int nz, const dvm_vgrid *v, int target_ctas, int max_blocks, int rv, int order, int wide_axis,
+                   int *counts5, int *items9, int max_items)
 {
-    if (!v || !counts5 || max_blocks < 0 || (rv != 0 && rv != 2 && rv != 4) || (order != 1 && order != 2) || (order == 2 && rv == 4) || nx <= 0 || ny <= 0 || nz <= 0 || v->mx <= 0 || v->my <= 0 || v->mz <= 0 || !v->xi_x || !v->xi_y || !v->xi_z)
+    if (wide_axis < 0 || wide_axis > 3) return fail(DVM_EINVAL, "bad argument");
+    if (!v || !counts5 || max_blocks < 0 || (rv != 0 && (rv < 2 || rv > 4)) || (order != 1 && order != 2) || (order == 2 && rv > 2) || nx <= 0 || ny <= 0 || nz <= 0 || v->mx <= 0 || v->my <= 0 || v->mz <= 0 || !v->xi_x || !v->xi_y || !v->xi_z)
         return fail(DVM_EINVAL, "bad argument");
     std::vector<double> xi[3];
     xi[0].assign(v->xi_x, v->xi_x + v->mx); xi[1].assign(v->xi_y, v->xi_y + v->my); xi[2].assign(v->xi_z, v->xi_z + v->mz);
     TilePlan tp;
-    if (rv == 0) rv = order == 2 ? 2 : choose_rv(xi);
-    if (tile_plan(nx, ny, nz, xi, target_ctas, max_blocks, rv, order, &tp)) return fail(DVM_EINVAL, "tile plan failed");
+    int wide = 0;
+    choose_variant(xi, order, rv, wide_axis - 1, &rv, &wide);
+    if (tile_plan(nx, ny, nz, xi, target_ctas, max_blocks, rv, order, wide, &tp)) return fail(DVM_EINVAL, "tile plan failed");
     counts5[0] = (int)tp.vblocks.size(); counts5[1] = tp.ntx; counts5[2] = tp.nty; counts5[3] = tp.P; counts5[4] = tp.batch;
     const int n = (int)tp.items.size();
     if (items9) {
@@ -815,21 +835,26 @@ int dvm_plan_query(int nx, int ny, int nz, const dvm_vgrid *v, int target_ctas, 
     return n;
 }
 
-int dvm_plan_vblocks(const dvm_vgrid *v, int rv, int order, int *boxes8, int max_blocks)
+int dvm_plan_vblocks(const dvm_vgrid *v, int rv, int order, int wide_axis, int *boxes8, int max_blocks)
 {
-    if (!v || max_blocks < 0 || (rv != 0 && rv != 2 && rv != 4) || (order != 1 && order != 2) || (order == 2 && rv == 4) || v->mx <= 0 || v->my <= 0 || v->mz <= 0 || !v->xi_x || !v->xi_y || !v->xi_z)
+    if (wide_axis < 0 || wide_axis > 3) return fail(DVM_EINVAL, "bad argument");
+    if (!v || max_blocks < 0 || (rv != 0 && (rv < 2 || rv > 4)) || (order != 1 && order != 2) || (order == 2 && rv > 2) || v->mx <= 0 || v->my <= 0 || v->mz <= 0 || !v->xi_x || !v->xi_y || !v->xi_z)
         return fail(DVM_EINVAL, "bad argument");
     std::vector<double> xi[3];
     xi[0].assign(v->xi_x, v->xi_x + v->mx); xi[1].assign(v->xi_y, v->xi_y + v->my); xi[2].assign(v->xi_z, v->xi_z + v->mz);
-    if (rv == 0) rv = order == 2 ? 2 : choose_rv(xi);
+    int wide = 0;
+    choose_variant(xi, order, rv, wide_axis - 1, &rv, &wide);
     TilePlan tp;
-    if (tile_plan(4, 4, 1, xi, 1, 0, rv, order, &tp)) return fail(DVM_EINVAL, "tile plan failed");
+    if (tile_plan(4, 4, 1, xi, 1, 0, rv, order, wide, &tp)) return fail(DVM_EINVAL, "tile plan failed");
     const int n = (int)tp.vblocks.size();
     if (boxes8)
         for (int e = 0; e < n && e < max_blocks; ++e) {
             const VBlock &b = tp.vblocks[e];
             int *o = boxes8 + 8 * e;
-            o[0] = b.a0; o[1] = b.na; o[2] = b.b0; o[3] = b.nb; o[4] = b.c0; o[5] = b.nc; o[6] = tile_na(rv); o[7] = b.nbb * 256 + b.ncb;
+            // node ranges in the order xi_x, xi_y, xi_z whatever the roles are
+            const int lo[3] = {b.a0, b.b0, b.c0}, cn[3] = {b.na, b.nb, b.nc};
+            for (int r = 0; r < 3; ++r) { o[2 * tp.ax[r]] = lo[r]; o[2 * tp.ax[r] + 1] = cn[r]; }
+            o[6] = tile_na(rv) + 65536 * (tp.ax[0] + 1); o[7] = b.nbb * 256 + b.ncb;
         }
     return n;
 }

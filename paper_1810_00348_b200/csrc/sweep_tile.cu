@@ -8,9 +8,9 @@
 //
 //  * work item = (velocity block of 512 velocities of one sign octant) x (4 x 4 z-column of cells); a CTA owns an
 //    item, a thread owns RV velocities (consecutive xi_x nodes) and keeps their 4 x 4 values of the current z-plane
-//    in registers: x-, y- and z-upwind operands of interior cells are register operands.  Two variants: RV = 4
-//    (128 threads, blocks of 16 x 32 nodes, 8 warps per SM) and RV = 2 (256 threads, blocks of 8 x 64 nodes, 16 warps
-//    per SM);
+//    in registers: x-, y- and z-upwind operands of interior cells are register operands.  Variants: RV = 4 (128
+//    threads, blocks of 16 x 32 nodes, 8 warps per SM), RV = 3 (128 threads, blocks of 12 x 32 nodes: fills 24-node sign
+//    halves), RV = 2 (256 threads, blocks of 8 x 64 nodes, 16 warps per SM), and RV = 2 at order 2 (128 threads);
 //  * what is carried is g = w_alpha f_alpha (the recurrence is linear in f), so quadrature weights cost nothing;
 //  * exp(-|xi-U|^2/T) and the Shakhov polynomial factorise per axis on the tensor velocity grid: tables.cu tabulates
 //    one entry (E, Q, e, a) per (cell, 1-D node) once per iteration; per level the CTA receives the entries of its
@@ -43,7 +43,7 @@ constexpr unsigned REC_ROW_BYTES = 4 * (unsigned)sizeof(CellRec);
 // Kernel variant: RV velocities per thread, ORD = order of the upwind sweep (sweep_tile.cuh)
 template <int RV, int ORD>
 struct KC {
-    static constexpr int THREADS = ORD == 2 ? 128 : TILE_NVB / RV;
+    static constexpr int THREADS = (ORD == 2 || RV >= 3) ? 128 : 256;
     static constexpr int WARPS = THREADS / 32;
     static constexpr int NVB = THREADS * RV;                 // velocities per block
     static constexpr int ES = ORD == 2 ? 48 : 32;            // bytes of a factor-table entry
@@ -174,6 +174,10 @@ __device__ __forceinline__ void red_f64(double *addr, double v)
 __device__ __forceinline__ void st_f64x2(double *addr, double a, double b)
 {
     asm volatile("st.global.v2.f64 [%0], {%1, %2};" ::"l"(addr), "d"(a), "d"(b));
+}
+__device__ __forceinline__ void st_f64(double *addr, double a)
+{
+    asm volatile("st.global.f64 [%0], %1;" ::"l"(addr), "d"(a));
 }
 
 // D (8 x 8) += A (8 x 4, row-major) * B (4 x 8, column-major) in fp64 on the tensor cores (DMMA).  Fragments of lane l:
@@ -360,24 +364,33 @@ __device__ __forceinline__ void decode_records(const TileParams &P, const ItemCt
 }
 
 // The RV values of a thread in a face row of NVB doubles are stored as RV / 2 pairs, pair h of thread t at double
-// (h * threads + t) * 2: every 16-byte access of a warp then covers 512 contiguous bytes (full sectors in L2 / HBM, no
-// bank conflict in shared memory).  row = start of the face row.
+// (h * threads + t) * 2 (odd RV: the last value of thread t follows the pairs, at pairs + t): every 16-byte access of a
+// warp then covers 512 contiguous bytes (full sectors in L2 / HBM, no bank conflict in shared memory).  row = start of the
+// face row.
 template <int RV, int ORD>
-__device__ __forceinline__ int face_index(int tid, int r) { return ((r >> 1) * KC<RV, ORD>::THREADS + tid) * 2 + (r & 1); }
+__device__ __forceinline__ int face_index(int tid, int r)
+{
+    constexpr int TH = KC<RV, ORD>::THREADS;
+    return r < 2 * (RV / 2) ? ((r >> 1) * TH + tid) * 2 + (r & 1) : (RV / 2) * TH * 2 + tid;
+}
 template <int RV, int ORD>
 __device__ __forceinline__ void load_face(const double *row, int tid, double (&v)[RV])
 {
+    constexpr int TH = KC<RV, ORD>::THREADS;
 #pragma unroll
     for (int h = 0; h < RV / 2; ++h) {
-        const double2 t = reinterpret_cast<const double2 *>(row)[h * KC<RV, ORD>::THREADS + tid];
+        const double2 t = reinterpret_cast<const double2 *>(row)[h * TH + tid];
         v[2 * h] = t.x; v[2 * h + 1] = t.y;
     }
+    if (RV & 1) v[RV - 1] = row[(RV / 2) * TH * 2 + tid];
 }
 template <int RV, int ORD>
 __device__ __forceinline__ void store_face(double *row, int tid, const double (&v)[RV])
 {
+    constexpr int TH = KC<RV, ORD>::THREADS;
 #pragma unroll
-    for (int h = 0; h < RV / 2; ++h) st_f64x2(row + (h * KC<RV, ORD>::THREADS + tid) * 2, v[2 * h], v[2 * h + 1]);
+    for (int h = 0; h < RV / 2; ++h) st_f64x2(row + (h * TH + tid) * 2, v[2 * h], v[2 * h + 1]);
+    if (RV & 1) st_f64(row + (RV / 2) * TH * 2 + tid, v[RV - 1]);
 }
 
 // Ghost values of the domain faces of level kp (buffer b) for a tile at the upwind x / y edge of the domain
@@ -468,7 +481,7 @@ __device__ __forceinline__ void emit_pair(const RowBuf<RV, ORD> &R, const int ro
 // table entries carry the stencil coefficients (cd, c1, c2) per direction, so the cell value is
 // g = [src + sum_d (c1_d g_1d + c2_d g_2d)] / (nu + sum_d cd_d); the recurrence along x is still one DFMA per value
 // (the c2 term uses the value two cells back, known a cell earlier).  YL: y-face layer this row's values go to (-1: none).
-template <int RV, int ORD, int YL>
+template <int RV, int ORD, int AX, int YL>
 __device__ __forceinline__ void compute_row(const RowBuf<RV, ORD> &R, const double *xin, const double *xin2, double (&zrow)[4][RV],
                                             double (&z2row)[4][RV], const double (&yup)[4][RV], const double (&yup2)[4][RV],
                                             const ThreadCtx<RV, ORD> &T, const int tid, const int lane, double *xout, const bool wx,
@@ -485,10 +498,11 @@ __device__ __forceinline__ void compute_row(const RowBuf<RV, ORD> &R, const doub
         const double4 zt = entry<RV, ORD>(R, T.zo[ii]);
         const double Eyz = yt.x * zt.x, Qyz = yt.y + zt.y, eyz = yt.z + zt.z;
         const double dyz = (yt.w + zt.w) + record<RV, ORD>(R, T.ro[ii]).nu;
-        double c1y = yt.w, c1z = zt.w, c2y = 0.0, c2z = 0.0;
+        // stencil coefficients of the entries of the roles B and C (one per cell) - and, below, A (one per node)
+        double c1B = yt.w, c1C = zt.w, c2B = 0.0, c2C = 0.0;
         if (ORD == 2) {
             const double2 yc = entry_c<RV, ORD>(R, T.yo[ii]), zc = entry_c<RV, ORD>(R, T.zo[ii]);
-            c1y = yc.x; c2y = yc.y; c1z = zc.x; c2z = zc.y;
+            c1B = yc.x; c2B = yc.y; c1C = zc.x; c2C = zc.y;
         }
         // Everything that does not depend on the x-upwind value, for the RV nodes of the thread in lock step (the fp64
         // pipe takes a warp instruction every 2 clocks and has a latency of ~10): the cell value is g = W g_xup + V with
@@ -522,21 +536,26 @@ __device__ __forceinline__ void compute_row(const RowBuf<RV, ORD> &R, const doub
         for (int r = 0; r < RV; ++r) V[r] = sE[r] * t1[r];
 #pragma unroll
         for (int r = 0; r < RV; ++r) y0[r] = fma(y0[r], e[r], y0[r]);       // 1 / den (MUFU seed + cubic Newton step)
+        // The entry of role A belongs to velocity axis AX, B and C to the other two in ascending order; the coefficient of the
+        // x- / y- / z-upwind value is the one of the entry that holds xi_x / xi_y / xi_z (compile-time selection).
+        double c1A[RV], c2A[RV];
 #pragma unroll
-        for (int r = 0; r < RV; ++r) V[r] = fma(c1y, yup[ii][r], V[r]);
+        for (int r = 0; r < RV; ++r) { c1A[r] = ORD == 2 ? xc[r].x : xt[r].w; c2A[r] = ORD == 2 ? xc[r].y : 0.0; }
+#pragma unroll
+        for (int r = 0; r < RV; ++r) V[r] = fma(AX == 0 ? c1B : AX == 1 ? c1A[r] : c1C, yup[ii][r], V[r]);
         if (ORD == 2) {
 #pragma unroll
-            for (int r = 0; r < RV; ++r) V[r] = fma(c2y, yup2[ii][r], V[r]);
+            for (int r = 0; r < RV; ++r) V[r] = fma(AX == 0 ? c2B : AX == 1 ? c2A[r] : c2C, yup2[ii][r], V[r]);
         }
 #pragma unroll
-        for (int r = 0; r < RV; ++r) W[r] = (ORD == 2 ? xc[r].x : xt[r].w) * y0[r];
+        for (int r = 0; r < RV; ++r) W[r] = (AX == 0 ? c1A[r] : c1B) * y0[r];
 #pragma unroll
-        for (int r = 0; r < RV; ++r) V[r] = fma(c1z, zrow[ii][r], V[r]);
+        for (int r = 0; r < RV; ++r) V[r] = fma(AX == 2 ? c1A[r] : c1C, zrow[ii][r], V[r]);
         if (ORD == 2) {
 #pragma unroll
-            for (int r = 0; r < RV; ++r) V[r] = fma(c2z, z2row[ii][r], V[r]);
+            for (int r = 0; r < RV; ++r) V[r] = fma(AX == 2 ? c2A[r] : c2C, z2row[ii][r], V[r]);
 #pragma unroll
-            for (int r = 0; r < RV; ++r) V[r] = fma(xc[r].y, fx2[r], V[r]);
+            for (int r = 0; r < RV; ++r) V[r] = fma(AX == 0 ? c2A[r] : c2B, fx2[r], V[r]);
         }
 #pragma unroll
         for (int r = 0; r < RV; ++r) V[r] *= y0[r];
@@ -565,7 +584,7 @@ __device__ __forceinline__ void compute_row(const RowBuf<RV, ORD> &R, const doub
 // the row before.  The B200 instruction cache holds 32 KB, and a level loop larger than that is fetch-bound at 1/3
 // instruction per clock and scheduler (profiles/r01_ifetch_microbench.txt): the instructions a level executes on
 // this path (about 1900 for RV = 4) stay below that; rolled variants with rotating row slots were slower (profiles/).
-template <int RV, int ORD>
+template <int RV, int ORD, int AX>
 __device__ __forceinline__ void compute_level(const LevelBuf<RV, ORD> &L, double (&pl)[TILE_TY][4][RV], double (&pl2)[ORD == 2 ? TILE_TY : 1][4][RV],
                                               const ThreadCtx<RV, ORD> &T, const int tid, const int lane, double *xout, const bool wx,
                                               double *yout, const bool wy)
@@ -581,21 +600,21 @@ __device__ __forceinline__ void compute_level(const LevelBuf<RV, ORD> &L, double
     }
     // y-face layer a row's values go to: the last row -> layer 0, the one before (order 2) -> layer 1
     if (TILE_TY == 1) {
-        compute_row<RV, ORD, 0>(L.row[0], L.xface[0][0], L.xface[L2][0], pl[0], pl2[0], yu, yu2, T, tid, lane, xout, wx, yout, wy);
+        compute_row<RV, ORD, AX, 0>(L.row[0], L.xface[0][0], L.xface[L2][0], pl[0], pl2[0], yu, yu2, T, tid, lane, xout, wx, yout, wy);
     } else {
-        compute_row<RV, ORD, (ORD == 2 && TILE_TY == 2) ? 1 : -1>(L.row[0], L.xface[0][0], L.xface[L2][0], pl[0], pl2[0], yu, yu2, T, tid, lane,
+        compute_row<RV, ORD, AX, (ORD == 2 && TILE_TY == 2) ? 1 : -1>(L.row[0], L.xface[0][0], L.xface[L2][0], pl[0], pl2[0], yu, yu2, T, tid, lane,
                                                                 xout, wx, yout, wy);
 #pragma unroll
         for (int jj = 1; jj < TILE_TY - 1; ++jj) {
             if (ORD == 2 && jj == TILE_TY - 2)
-                compute_row<RV, ORD, 1>(L.row[jj], L.xface[0][jj], L.xface[L2][jj], pl[jj], pl2[ORD == 2 ? jj : 0], pl[jj - 1], jj >= 2 ? pl[jj >= 2 ? jj - 2 : 0] : yu,
+                compute_row<RV, ORD, AX, 1>(L.row[jj], L.xface[0][jj], L.xface[L2][jj], pl[jj], pl2[ORD == 2 ? jj : 0], pl[jj - 1], jj >= 2 ? pl[jj >= 2 ? jj - 2 : 0] : yu,
                                         T, tid, lane, xout + jj * NVB, wx, yout, wy);
             else
-                compute_row<RV, ORD, -1>(L.row[jj], L.xface[0][jj], L.xface[L2][jj], pl[jj], pl2[ORD == 2 ? jj : 0], pl[jj - 1], jj >= 2 ? pl[jj >= 2 ? jj - 2 : 0] : yu,
+                compute_row<RV, ORD, AX, -1>(L.row[jj], L.xface[0][jj], L.xface[L2][jj], pl[jj], pl2[ORD == 2 ? jj : 0], pl[jj - 1], jj >= 2 ? pl[jj >= 2 ? jj - 2 : 0] : yu,
                                          T, tid, lane, xout + jj * NVB, wx, yout, wy);
         }
         constexpr int J = TILE_TY - 1;
-        compute_row<RV, ORD, 0>(L.row[J], L.xface[0][J], L.xface[L2][J], pl[J], pl2[ORD == 2 ? J : 0], pl[J - 1], J >= 2 ? pl[J >= 2 ? J - 2 : 0] : yu, T, tid, lane,
+        compute_row<RV, ORD, AX, 0>(L.row[J], L.xface[0][J], L.xface[L2][J], pl[J], pl2[ORD == 2 ? J : 0], pl[J - 1], J >= 2 ? pl[J >= 2 ? J - 2 : 0] : yu, T, tid, lane,
                                 xout + J * NVB, wx, yout, wy);
     }
 }
@@ -604,7 +623,7 @@ __device__ __forceinline__ void compute_level(const LevelBuf<RV, ORD> &L, double
 // written as compact loops over a copy of the plane(s) in local memory.  Rare (the surface of a masked body), so its
 // speed does not matter; keeping it out of the unrolled path halves the code the instruction cache has to hold.
 // A solid ghost replaces the first upwind value; the coefficient of the second one is 0 there (tables.cu).
-template <int RV, int ORD>
+template <int RV, int ORD, int AX>
 __device__ __forceinline__ void compute_level_slow(TileSmem<RV, ORD> &s, const LevelBuf<RV, ORD> &L, double *pl, double *pl2,
                                                    const ThreadCtx<RV, ORD> &T, const int tid, const int lane, double *xout, double *yout)
 {
@@ -630,10 +649,10 @@ __device__ __forceinline__ void compute_level_slow(TileSmem<RV, ORD> &s, const L
             const double4 yt = entry<RV, ORD>(R, yo);
             const double4 zt = entry<RV, ORD>(R, zo);
             const double Eyz = yt.x * zt.x, Qyz = yt.y + zt.y, eyz = yt.z + zt.z;
-            double c1y = yt.w, c1z = zt.w, c2y = 0.0, c2z = 0.0;
+            double c1B = yt.w, c1C = zt.w, c2B = 0.0, c2C = 0.0;
             if (ORD == 2) {
                 const double2 yc = entry_c<RV, ORD>(R, yo), zc = entry_c<RV, ORD>(R, zo);
-                c1y = yc.x; c2y = yc.y; c1z = zc.x; c2z = zc.y;
+                c1B = yc.x; c2B = yc.y; c1C = zc.x; c2C = zc.y;
             }
             const int ro = ii == 0 ? T.ro[0] : ii == 1 ? T.ro[1] : ii == 2 ? T.ro[2] : T.ro[3];
             const double dyz = (yt.w + zt.w) + record<RV, ORD>(R, ro).nu;
@@ -644,8 +663,10 @@ __device__ __forceinline__ void compute_level_slow(TileSmem<RV, ORD> &s, const L
             for (int r = 0; r < RV; ++r) {
                 const double Pg = s.g[3][0][RV * T.ag + r] * gyz;
                 const double4 xt = entry<RV, ORD>(R, xo + r * GA * ES);
-                double c1x = xt.w, c2x = 0.0;
-                if (ORD == 2) { const double2 xc = entry_c<RV, ORD>(R, xo + r * GA * ES); c1x = xc.x; c2x = xc.y; }
+                double c1A = xt.w, c2A = 0.0;
+                if (ORD == 2) { const double2 xc = entry_c<RV, ORD>(R, xo + r * GA * ES); c1A = xc.x; c2A = xc.y; }
+                const double c1x = AX == 0 ? c1A : c1B, c1y = AX == 0 ? c1B : AX == 1 ? c1A : c1C, c1z = AX == 2 ? c1A : c1C;
+                const double c2x = AX == 0 ? c2A : c2B, c2y = AX == 0 ? c2B : AX == 1 ? c2A : c2C, c2z = AX == 2 ? c2A : c2C;
                 double xu = fx[r], zu = pl[cell * RV + r];
                 double yu = jj == 0 ? L.yface[0][ii][face_index<RV, ORD>(tid, r)] : pl[(cell - 4) * RV + r];
                 double xu2 = fx2[r], zu2 = 0.0, yu2 = 0.0;
@@ -701,12 +722,16 @@ __device__ __forceinline__ void compute_level_slow(TileSmem<RV, ORD> &s, const L
     }
 }
 
-template <int RV, int ORD>
+template <int RV, int ORD, int AX>
 __global__ void __launch_bounds__(KC<RV, ORD>::THREADS, 2) sweep_tile_kernel(const TileParams P)
 {
     constexpr int NA = GA * RV, THREADS = KC<RV, ORD>::THREADS, XLEVEL_DOUBLES = KC<RV, ORD>::XLEVEL_DOUBLES, YLEVEL_DOUBLES = KC<RV, ORD>::YLEVEL_DOUBLES;
     (void)THREADS;
     using RB = RowBuf<RV, ORD>;
+    // velocity axis in the role A (AX), B, C and their node arrays
+    constexpr int AXB = AX == 0 ? 1 : 0, AXC = AX == 2 ? 1 : 2;
+    const double *xiA = AX == 0 ? P.xi_x : AX == 1 ? P.xi_y : P.xi_z;
+    const double *xiB = AXB == 0 ? P.xi_x : P.xi_y, *xiC = AXC == 1 ? P.xi_y : P.xi_z;
     // dynamic shared memory starts at offset 0 of the CTA's window (no static __shared__ in this kernel), so the
     // 128-byte alignment holds; casting without pointer arithmetic keeps the address space visible (LDS / STS)
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -765,24 +790,24 @@ __global__ void __launch_bounds__(KC<RV, ORD>::THREADS, 2) sweep_tile_kernel(con
             if (tid < 16) {
                 const bool ok = tid < vb.na;
                 const int idx = vb.a0 + tid;
-                s.xi_a[tid] = ok ? P.xi_x[idx] : 0.0;
+                s.xi_a[tid] = ok ? xiA[idx] : 0.0;
 #pragma unroll
-                for (int f = 0; f < 4; ++f) s.g[f][0][tid] = ok ? P.gtab[(long long)(slotid[f] * 3 + 0) * P.gstride + idx] : 0.0;
+                for (int f = 0; f < 4; ++f) s.g[f][0][tid] = ok ? P.gtab[(long long)(slotid[f] * 3 + AX) * P.gstride + idx] : 0.0;
             } else if (tid < 16 + vb.nbb) {
                 const int bl = tid - 16;
                 const bool ok = bl < vb.nb;
                 const int idx = vb.b0 + bl;
-                s.xi_bc[bl] = ok ? P.xi_y[idx] : 0.0;
+                s.xi_bc[bl] = ok ? xiB[idx] : 0.0;
 #pragma unroll
-                for (int f = 0; f < 4; ++f) s.g[f][1][bl] = ok ? P.gtab[(long long)(slotid[f] * 3 + 1) * P.gstride + idx] : 0.0;
+                for (int f = 0; f < 4; ++f) s.g[f][1][bl] = ok ? P.gtab[(long long)(slotid[f] * 3 + AXB) * P.gstride + idx] : 0.0;
             } else if (tid >= 32 && tid < 32 + vb.ncb) {
                 const int cl = tid - 32;
                 const bool ok = cl < vb.nc;
                 const int idx = vb.c0 + cl;
-                s.xi_bc[vb.nbb + cl] = ok ? P.xi_z[idx] : 0.0;
+                s.xi_bc[vb.nbb + cl] = ok ? xiC[idx] : 0.0;
 #pragma unroll
                 for (int f = 0; f < 4; ++f)
-                    s.g[f][2][vb.nbb + cl] = ok ? P.gtab[(long long)(slotid[f] * 3 + 2) * P.gstride + idx] : 0.0;
+                    s.g[f][2][vb.nbb + cl] = ok ? P.gtab[(long long)(slotid[f] * 3 + AXC) * P.gstride + idx] : 0.0;
             }
             rwb_store<RV, ORD>(s, 0, tid, rwb_load(P, I, 0, tid));
             rwb_store<RV, ORD>(s, 1, tid, rwb_load(P, I, 1, tid));
@@ -824,15 +849,26 @@ __global__ void __launch_bounds__(KC<RV, ORD>::THREADS, 2) sweep_tile_kernel(con
                         : j == 6 ? y * r2 : z * r2;
             }
             T.yz0 = mono[0]; T.yz1 = mono[1];
-            // results of this lane: D[p][2q], D[p][2q + 1] and their accumulator slots
-            int s0 = c_slot0[pw][q];
-            const int s1 = c_slot1[pw][q];
+            // results of this lane: D[p][2q], D[p][2q + 1] and their accumulator slots.  c_slot names the sums in terms of the
+            // roles (A, B, C) = (xi_AX, xi_AXB, xi_AXC); the accumulator row is in terms of (xi_x, xi_y, xi_z)
+            int s0 = c_slot0[pw][q], s1 = c_slot1[pw][q];
             const bool u0 = c_use0[pw][q], u1 = c_use1[pw][q];
+            const int axr[3] = {AX, AXB, AXC}, sgn[3] = {vb.sx, vb.sy, vb.sz};
+            auto physical = [&](int sl) {
+                if (sl >= 1 && sl <= 3) return 1 + axr[sl - 1];
+                if (sl >= 4 && sl <= 6) return 4 + axr[sl - 4];
+                if (sl == 7) return 6 + AX + AXB;      // {0,1} -> 7, {0,2} -> 8, {1,2} -> 9
+                if (sl == 8) return 6 + AX + AXC;
+                if (sl == 9) return 6 + AXB + AXC;
+                if (sl >= 10 && sl <= 12) return 10 + axr[sl - 10];
+                if (sl >= 13) return 13 + axr[sl - 13];
+                return sl;
+            };
             if (s0 >= 1 && s0 <= 3) {
                 // first moments: half-range slot by the sign of the block; an unneeded result goes to the other one
-                const int sg = s0 == 1 ? vb.sx : s0 == 2 ? vb.sy : vb.sz;
-                if ((sg < 0) == u0) s0 += 12;
+                if ((sgn[axr[s0 - 1]] < 0) == u0) s0 += 12;
             }
+            s0 = physical(s0); s1 = physical(s1);
             T.raw0 = P.raw16 + s0; T.raw1 = P.raw16 + s1;
             T.use0 = u0 ? 1.0 : 0.0; T.use1 = u1 ? 1.0 : 0.0;
         }
@@ -900,7 +936,7 @@ __global__ void __launch_bounds__(KC<RV, ORD>::THREADS, 2) sweep_tile_kernel(con
                         tmp[c * RV + r] = pl[c >> 2][c & 3][r];
                         if (ORD == 2) tmp2[c * RV + r] = pl2[ORD == 2 ? c >> 2 : 0][c & 3][r];
                     }
-                compute_level_slow<RV, ORD>(s, s.lv[b], tmp, tmp2, T, tid, lane, write_x ? xout : nullptr, write_y ? yout : nullptr);
+                compute_level_slow<RV, ORD, AX>(s, s.lv[b], tmp, tmp2, T, tid, lane, write_x ? xout : nullptr, write_y ? yout : nullptr);
 #pragma unroll
                 for (int c = 0; c < NCELL; ++c)
 #pragma unroll
@@ -909,7 +945,7 @@ __global__ void __launch_bounds__(KC<RV, ORD>::THREADS, 2) sweep_tile_kernel(con
                         if (ORD == 2) pl2[ORD == 2 ? c >> 2 : 0][c & 3][r] = tmp2[c * RV + r];
                     }
             } else {
-                compute_level<RV, ORD>(s.lv[b], pl, pl2, T, tid, lane, xout, write_x, yout, write_y);
+                compute_level<RV, ORD, AX>(s.lv[b], pl, pl2, T, tid, lane, xout, write_x, yout, write_y);
             }
             if (edge) {
                 rwb_store<RV, ORD>(s, b, tid, vrw);
@@ -929,31 +965,45 @@ __global__ void __launch_bounds__(KC<RV, ORD>::THREADS, 2) sweep_tile_kernel(con
     }
 }
 
-template <int RV, int ORD>
-cudaError_t configure(int *ctas_per_sm)
+template <int RV, int ORD, int AX>
+cudaError_t configure1(int *ctas_per_sm)
 {
-    cudaError_t e = cudaFuncSetAttribute(sweep_tile_kernel<RV, ORD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(TileSmem<RV, ORD>));
+    cudaError_t e = cudaFuncSetAttribute(sweep_tile_kernel<RV, ORD, AX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(TileSmem<RV, ORD>));
     if (e != cudaSuccess) return e;
-    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, sweep_tile_kernel<RV, ORD>, KC<RV, ORD>::THREADS, sizeof(TileSmem<RV, ORD>));
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, sweep_tile_kernel<RV, ORD, AX>, KC<RV, ORD>::THREADS, sizeof(TileSmem<RV, ORD>));
+}
+template <int RV, int ORD>
+cudaError_t configure(int ax, int *ctas_per_sm)
+{
+    return ax == 1 ? configure1<RV, ORD, 1>(ctas_per_sm) : ax == 2 ? configure1<RV, ORD, 2>(ctas_per_sm) : configure1<RV, ORD, 0>(ctas_per_sm);
+}
+template <int RV, int ORD>
+void launch(const TileParams &P, int ax, int grid, cudaStream_t st)
+{
+    if (ax == 1) sweep_tile_kernel<RV, ORD, 1><<<grid, KC<RV, ORD>::THREADS, sizeof(TileSmem<RV, ORD>), st>>>(P);
+    else if (ax == 2) sweep_tile_kernel<RV, ORD, 2><<<grid, KC<RV, ORD>::THREADS, sizeof(TileSmem<RV, ORD>), st>>>(P);
+    else sweep_tile_kernel<RV, ORD, 0><<<grid, KC<RV, ORD>::THREADS, sizeof(TileSmem<RV, ORD>), st>>>(P);
 }
 
 }  // namespace
 
 size_t tile_smem_bytes(int rv, int order)
 {
-    return order == 2 ? sizeof(TileSmem<2, 2>) : rv == 2 ? sizeof(TileSmem<2, 1>) : sizeof(TileSmem<4, 1>);
+    return order == 2 ? sizeof(TileSmem<2, 2>) : rv == 2 ? sizeof(TileSmem<2, 1>) : rv == 3 ? sizeof(TileSmem<3, 1>) : sizeof(TileSmem<4, 1>);
 }
 
-cudaError_t tile_configure(int rv, int order, int *ctas_per_sm)
+cudaError_t tile_configure(int rv, int order, int wide_axis, int *ctas_per_sm)
 {
-    return order == 2 ? configure<2, 2>(ctas_per_sm) : rv == 2 ? configure<2, 1>(ctas_per_sm) : configure<4, 1>(ctas_per_sm);
+    return order == 2 ? configure<2, 2>(wide_axis, ctas_per_sm) : rv == 2 ? configure<2, 1>(wide_axis, ctas_per_sm)
+         : rv == 3 ? configure<3, 1>(wide_axis, ctas_per_sm) : configure<4, 1>(wide_axis, ctas_per_sm);
 }
 
-cudaError_t launch_sweep_tile(const TileParams &P, int rv, int order, int grid, cudaStream_t st)
+cudaError_t launch_sweep_tile(const TileParams &P, int rv, int order, int wide_axis, int grid, cudaStream_t st)
 {
-    if (order == 2) sweep_tile_kernel<2, 2><<<grid, KC<2, 2>::THREADS, sizeof(TileSmem<2, 2>), st>>>(P);
-    else if (rv == 2) sweep_tile_kernel<2, 1><<<grid, KC<2, 1>::THREADS, sizeof(TileSmem<2, 1>), st>>>(P);
-    else sweep_tile_kernel<4, 1><<<grid, KC<4, 1>::THREADS, sizeof(TileSmem<4, 1>), st>>>(P);
+    if (order == 2) launch<2, 2>(P, wide_axis, grid, st);
+    else if (rv == 2) launch<2, 1>(P, wide_axis, grid, st);
+    else if (rv == 3) launch<3, 1>(P, wide_axis, grid, st);
+    else launch<4, 1>(P, wide_axis, grid, st);
     return cudaGetLastError();
 }
 

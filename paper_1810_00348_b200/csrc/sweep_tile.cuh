@@ -11,8 +11,9 @@
 // dependencies (x-face of (I'-1, J'), y-face of (I', J'-1)); done-flags in global memory gate the start of an item.
 // The equilibrium enters through 1-D factor tables (tables.cu) staged by TMA with the faces; velocity blocks may
 // sweep in batches that share face-slot sets when the f workspace is capped (DVM_OPT_MAX_F_MBYTES).
-// Two variants of the kernel (DVM_OPT_TILE_RV): RV = 4: CTAs of 128 threads, blocks of 16 x 32 nodes (nbb x ncb = 8 x 4
-// or 4 x 8); RV = 2: CTAs of 256 threads, blocks of 8 x 8 x 8 nodes, twice the warps per SM.
+// Variants of the kernel (DVM_OPT_TILE_RV): RV = 4: CTAs of 128 threads, blocks of 16 x 32 nodes (nbb x ncb = 8 x 4
+// or 4 x 8); RV = 3: 128 threads, blocks of 12 x 32 nodes; RV = 2: CTAs of 256 threads, blocks of 8 x 8 x 8 nodes, twice the
+// warps per SM.
 #pragma once
 #include <cuda_runtime.h>
 #include <vector>
@@ -37,9 +38,9 @@ inline void split_axis(const std::vector<double> &xi, int lo[2], int cnt[2])
     while (nneg < (int)xi.size() && xi[nneg] < 0.0) ++nneg;
     lo[0] = 0; cnt[0] = nneg; lo[1] = nneg; cnt[1] = (int)xi.size() - nneg;
 }
-// Kernel variants: (rv, order) = (4, 1): 128 threads x 4 velocities; (2, 1): 256 x 2; (2, 2): the second-order sweep
+// Kernel variants: (rv, order) = (4, 1): 128 threads x 4 velocities; (3, 1): 128 x 3; (2, 1): 256 x 2; (2, 2): the second-order sweep
 // (DVM_OPT_ORDER = 2) keeps two z-planes in registers: 128 threads x 2 velocities, 256 velocities per block.
-inline int tile_threads(int rv, int order = 1) { return order == 2 ? 128 : TILE_NVB / rv; }
+inline int tile_threads(int rv, int order = 1) { return (order == 2 || rv >= 3) ? 128 : 256; }
 inline int tile_nvb(int rv, int order = 1) { return tile_threads(rv, order) * rv; }   // velocities per block
 inline int tile_na(int rv) { return TILE_GA * rv; }          // xi_x nodes per velocity block
 inline int tile_npair(int rv, int order = 1) { return tile_threads(rv, order) / TILE_GA; }   // (xi_y, xi_z) pairs per block
@@ -58,7 +59,8 @@ struct CellRec {
 };
 static_assert(sizeof(CellRec) == 48, "CellRec rows must be 16-byte aligned");
 
-// velocity block: node-index box [a0, a0+na) x [b0, b0+nb) x [c0, c0+nc), na <= NA, nb <= nbb, nc <= ncb,
+// velocity block: node-index box [a0, a0+na) x [b0, b0+nb) x [c0, c0+nc) of the velocity axes in the roles A, B, C
+// (TilePlan::ax; A = xi_x unless another axis fills the wide role better), na <= NA, nb <= nbb, nc <= ncb,
 // nbb * ncb = pairs per block; lanes beyond the box carry weight 0
 struct VBlock {
     int a0, na, b0, nb, c0, nc;
@@ -82,9 +84,10 @@ struct TileItem {
 struct TilePlan {
     int ntx = 0, nty = 0, P = 1;
     int rv = 4, order = 1;             // kernel variant this plan is for: velocities per thread, order of the sweep
+    int ax[3] = {0, 1, 2};             // velocity axis in the role A (the wide one: RV nodes per thread x 4 lane groups), B, C
     int batch = 0;                     // velocity blocks in flight at once (= face-slot sets)
     int nbb = 8, ncb = 4;              // one (xi_y, xi_z) block shape for the whole problem
-    std::vector<int> xnode, ynode, znode;   // node index per 1-D block slot (-1 = padding): [nxb][NA], [nyb][nbb], [nzb][ncb];
+    std::vector<int> xnode, ynode, znode;   // node index (of the axis in role A, B, C) per 1-D block slot (-1 = padding): [nxb][NA], [nyb][nbb], [nzb][ncb];
                                             // xnode is in table order: slot r*4 + ag holds node RV*ag + r of the block
     std::vector<VBlock> vblocks;
     std::vector<TileItem> items;
@@ -124,6 +127,7 @@ struct TileParams {
 
 struct TableParams {
     int nx, ny, nz, nxp, nyp, na, nbb, ncb, nxb, nyb, nzb, order;
+    int ax[3];                    // velocity axis of the tables TX, TY, TZ (roles A, B, C)
     long long ncell;
     const double *coef;           // [NCOEF][ncell]
     const unsigned char *flags;   // bit 6: solid
@@ -141,11 +145,11 @@ struct TableParams {
 // flight at once (batches).  Pure host code (tests call it through
 // dvm_plan_query without a GPU).
 int tile_plan(int nx, int ny, int nz, const std::vector<double> xi[3], int target_ctas, int max_blocks, int rv, int order,
-              TilePlan *plan);
+              int wide_axis, TilePlan *plan);
 
 size_t tile_smem_bytes(int rv, int order);
-cudaError_t tile_configure(int rv, int order, int *ctas_per_sm);
-cudaError_t launch_sweep_tile(const TileParams &P, int rv, int order, int grid, cudaStream_t st);
+cudaError_t tile_configure(int rv, int order, int wide_axis, int *ctas_per_sm);
+cudaError_t launch_sweep_tile(const TileParams &P, int rv, int order, int wide_axis, int grid, cudaStream_t st);
 cudaError_t launch_tables(const TableParams &T, cudaStream_t st);
 
 }  // namespace dvm

@@ -1,9 +1,10 @@
 // tables.cu - the 1-D factor tables of the tile sweep kernel, rebuilt once per outer iteration from the per-cell pack
 // of step n (a1/a2 of DESIGN.md): on the tensor velocity grid the source term of Eq.(7) factorises,
 //   f^S / tau = [E_x E_y E_z] [1 + (Q_x + Q_y + Q_z)(e_x + e_y + e_z)]      (Eq.(2)),
-// so one entry (E, Q, e, a) per (cell, 1-D node) is all the sweep needs: E = w exp(-(xi-u)^2/T) (the x entry also
-// carries rho (pi T)^{-3/2} / tau), Q = q'(xi-u), e = 2 (xi-u)^2/T (- 5 in x), a = |xi| / cell width (Eq.(7),
-// PAPER.md:77; 0 where the upwind face is a zero-gradient boundary, i.e. the term is dropped).
+// so one entry (E, Q, e, a) per (cell, 1-D node) is all the sweep needs: E = w exp(-(xi-u)^2/T) (the entries of table
+// TX also carry rho (pi T)^{-3/2} / tau), Q = q'(xi-u), e = 2 (xi-u)^2/T (- 5 in TX), a = |xi| / cell width (Eq.(7),
+// PAPER.md:77; 0 where the upwind face is a zero-gradient boundary, i.e. the term is dropped).  TX, TY, TZ hold the velocity
+// axes T.ax[0..2]: TX the one that plays the wide role (A) in the sweep kernel, usually xi_x.
 // order = 2 (DVM_OPT_ORDER, reading G21): the transport term of Eq.(7) along d is
 // a_d (F(c) - F(c1)) with face values extrapolated from the two upwind centres, i.e. cd f_c - c1 f_c1 - c2 f_c2 with
 //   c1 fluid: psi = w_c / (w_c + w_c1), psi1 = w_c1 / (w_c1 + w_c2) if c2 is fluid else 0,
@@ -29,11 +30,12 @@ __global__ void __launch_bounds__(256) tables_kernel(const TableParams T)
         const int sl = (int)(idx - c * nslot);
         const int i = (int)(c % T.nx), j = (int)((c / T.nx) % T.ny), k = (int)(c / ((long long)T.nx * T.ny));
         const long long pc = ((long long)k * T.nyp + (j + TILE_PAD)) * T.nxp + (i + TILE_PAD);
-        int d, m, pos, width, blk;
+        int role, m, pos, width, blk;
         double *dst;
-        if (sl < sx) { d = 0; width = T.na; blk = sl / width; pos = sl - blk * width; m = T.xnode[sl]; dst = T.TX; }
-        else if (sl < sx + sy) { d = 1; width = T.nbb; const int t = sl - sx; blk = t / width; pos = t - blk * width; m = T.ynode[t]; dst = T.TY; }
-        else { d = 2; width = T.ncb; const int t = sl - sx - sy; blk = t / width; pos = t - blk * width; m = T.znode[t]; dst = T.TZ; }
+        if (sl < sx) { role = 0; width = T.na; blk = sl / width; pos = sl - blk * width; m = T.xnode[sl]; dst = T.TX; }
+        else if (sl < sx + sy) { role = 1; width = T.nbb; const int t = sl - sx; blk = t / width; pos = t - blk * width; m = T.ynode[t]; dst = T.TY; }
+        else { role = 2; width = T.ncb; const int t = sl - sx - sy; blk = t / width; pos = t - blk * width; m = T.znode[t]; dst = T.TZ; }
+        const int d = T.ax[role];   // velocity axis (= direction of the transport term) this table belongs to
         const bool solid = T.flags[c] & FLAG_SOLID;
         const double nu = T.coef[c];
         double ent[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
@@ -41,7 +43,7 @@ __global__ void __launch_bounds__(256) tables_kernel(const TableParams T)
             const double invT = T.coef[2 * n + c], u = T.coef[(3 + d) * n + c], q = T.coef[(6 + d) * n + c];
             const double xi = d == 0 ? T.xi_x[m] : d == 1 ? T.xi_y[m] : T.xi_z[m];
             double w = d == 0 ? T.w_x[m] : d == 1 ? T.w_y[m] : T.w_z[m];
-            if (d == 0) w *= nu * T.coef[n + c];
+            if (role == 0) w *= nu * T.coef[n + c];
             const int id = d == 0 ? i : d == 1 ? j : k, nd = d == 0 ? T.nx : d == 1 ? T.ny : T.nz;
             const double h = d == 0 ? T.invdx[i] : d == 1 ? T.invdy[j] : T.invdz[k];
             const bool pos_dir = xi >= 0.0;   // sweeps ascending: the upwind face is the low one
@@ -51,7 +53,7 @@ __global__ void __launch_bounds__(256) tables_kernel(const TableParams T)
             const double c1 = xi - u, t = c1 * c1 * invT;
             ent[0] = w * exp(-t);
             ent[1] = q * c1;
-            ent[2] = d == 0 ? 2.0 * t - 5.0 : 2.0 * t;
+            ent[2] = role == 0 ? 2.0 * t - 5.0 : 2.0 * t;
             const double a = drop ? 0.0 : fabs(xi) * h;
             ent[3] = a;
             if (T.order == 2) {

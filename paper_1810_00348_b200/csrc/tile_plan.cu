@@ -20,11 +20,16 @@ int ceil_div(int a, int b) { return (a + b - 1) / b; }
 }  // namespace
 
 int tile_plan(int nx, int ny, int nz, const std::vector<double> xi[3], int target_ctas, int max_blocks, int rv, int order,
-              TilePlan *plan)
+              int wide_axis, TilePlan *plan)
 {
-    if (nx <= 0 || ny <= 0 || nz <= 0 || !plan || (rv != 2 && rv != 4) || (order != 1 && order != 2) || (order == 2 && rv != 2)) return -1;
+    if (nx <= 0 || ny <= 0 || nz <= 0 || !plan || (rv < 2 || rv > 4) || (order != 1 && order != 2) || (order == 2 && rv != 2) ||
+        wide_axis < 0 || wide_axis > 2)
+        return -1;
     const int NA = tile_na(rv), NVB = tile_nvb(rv, order), npair = tile_npair(rv, order), layers = tile_face_layers(order);
     plan->rv = rv; plan->order = order;
+    // roles: A = the wide axis, B and C = the other two in ascending order
+    const int ax[3] = {wide_axis, wide_axis == 0 ? 1 : 0, wide_axis == 2 ? 1 : 2};
+    for (int r = 0; r < 3; ++r) plan->ax[r] = ax[r];
     plan->vblocks.clear();
     plan->items.clear();
     int lo[3][2], cnt[3][2];
@@ -39,7 +44,7 @@ int tile_plan(int nx, int ny, int nz, const std::vector<double> xi[3], int targe
         for (auto &s : (npair == 64 ? shapes2 : shapes4)) {
             long slots = 0;
             for (int oz = 0; oz < 2; ++oz) for (int oy = 0; oy < 2; ++oy)
-                slots += (long)ceil_div(cnt[1][oy], s[0]) * ceil_div(cnt[2][oz], s[1]);
+                slots += (long)ceil_div(cnt[ax[1]][oy], s[0]) * ceil_div(cnt[ax[2]][oz], s[1]);
             if (best < 0 || slots < best) { best = slots; best_bb = s[0]; best_cb = s[1]; }
         }
     }
@@ -48,32 +53,35 @@ int tile_plan(int nx, int ny, int nz, const std::vector<double> xi[3], int targe
     int first[3][2];
     const int width[3] = {NA, best_bb, best_cb};
     std::vector<int> *nodes[3] = {&plan->xnode, &plan->ynode, &plan->znode};
-    for (int d = 0; d < 3; ++d) {
-        nodes[d]->clear();
+    for (int r = 0; r < 3; ++r) {
+        const int d = ax[r];
+        nodes[r]->clear();
         int nblk = 0;
         for (int h = 0; h < 2; ++h) {
-            first[d][h] = nblk;
-            for (int k0 = 0; k0 < cnt[d][h]; k0 += width[d], ++nblk)
-                for (int sl = 0; sl < width[d]; ++sl) {
-                    // x: table slot r*4 + ag holds node RV*ag + r of the block (conflict-free reads, sweep_tile.cu)
-                    const int local = d == 0 ? rv * (sl & 3) + (sl >> 2) : sl;
-                    nodes[d]->push_back(k0 + local < cnt[d][h] ? lo[d][h] + k0 + local : -1);
+            first[r][h] = nblk;
+            for (int k0 = 0; k0 < cnt[d][h]; k0 += width[r], ++nblk)
+                for (int sl = 0; sl < width[r]; ++sl) {
+                    // A: table slot r*4 + ag holds node RV*ag + r of the block (conflict-free reads, sweep_tile.cu)
+                    const int local = r == 0 ? rv * (sl & 3) + (sl >> 2) : sl;
+                    nodes[r]->push_back(k0 + local < cnt[d][h] ? lo[d][h] + k0 + local : -1);
                 }
         }
     }
-    // ---- velocity blocks: per octant, chunks of NA x nbb x ncb node indices ----
-    for (int oz = 0; oz < 2; ++oz) for (int oy = 0; oy < 2; ++oy) for (int ox = 0; ox < 2; ++ox) {
-        const int na = cnt[0][ox], nb = cnt[1][oy], nc = cnt[2][oz];
+    // ---- velocity blocks: per octant, chunks of NA x nbb x ncb node indices of the axes in the roles A, B, C ----
+    for (int oc = 0; oc < 2; ++oc) for (int ob = 0; ob < 2; ++ob) for (int oa = 0; oa < 2; ++oa) {
+        const int na = cnt[ax[0]][oa], nb = cnt[ax[1]][ob], nc = cnt[ax[2]][oc];
         if (na == 0 || nb == 0 || nc == 0) continue;
+        int sgn[3];
+        sgn[ax[0]] = oa ? 1 : -1; sgn[ax[1]] = ob ? 1 : -1; sgn[ax[2]] = oc ? 1 : -1;
         for (int c0 = 0; c0 < nc; c0 += best_cb) for (int b0 = 0; b0 < nb; b0 += best_bb)
             for (int a0 = 0; a0 < na; a0 += NA) {
                 VBlock v{};
-                v.a0 = lo[0][ox] + a0; v.na = std::min(NA, na - a0);
-                v.b0 = lo[1][oy] + b0; v.nb = std::min(best_bb, nb - b0);
-                v.c0 = lo[2][oz] + c0; v.nc = std::min(best_cb, nc - c0);
+                v.a0 = lo[ax[0]][oa] + a0; v.na = std::min(NA, na - a0);
+                v.b0 = lo[ax[1]][ob] + b0; v.nb = std::min(best_bb, nb - b0);
+                v.c0 = lo[ax[2]][oc] + c0; v.nc = std::min(best_cb, nc - c0);
                 v.nbb = best_bb; v.ncb = best_cb;
-                v.sx = ox ? 1 : -1; v.sy = oy ? 1 : -1; v.sz = oz ? 1 : -1;
-                v.xb = first[0][ox] + a0 / NA; v.yb = first[1][oy] + b0 / best_bb; v.zb = first[2][oz] + c0 / best_cb;
+                v.sx = sgn[0]; v.sy = sgn[1]; v.sz = sgn[2];
+                v.xb = first[0][oa] + a0 / NA; v.yb = first[1][ob] + b0 / best_bb; v.zb = first[2][oc] + c0 / best_cb;
                 plan->vblocks.push_back(v);
             }
     }

@@ -28,13 +28,14 @@ OPT_MAX_F_MBYTES = 2
 OPT_TILE_RV = 3
 OPT_MAX_CTAS = 4
 OPT_ORDER = 5
+OPT_TILE_AXIS = 6
 
 # every symbol include/dvm.h declares (checked by tests/test_abi.py)
 SYMBOLS = (
     "dvm_create", "dvm_iterate", "dvm_moments", "dvm_residual", "dvm_num_faces", "dvm_iterations_done",
     "dvm_get_state", "dvm_set_state", "dvm_raw_moments", "dvm_wall_flux", "dvm_residual_history",
     "dvm_mass_scale", "dvm_step_host", "dvm_set_option", "dvm_workspace_bytes", "dvm_launch_count",
-    "dvm_kernel_used", "dvm_tile_rv", "dvm_plan_query", "dvm_plan_vblocks", "dvm_destroy", "dvm_last_error",
+    "dvm_kernel_used", "dvm_tile_rv", "dvm_tile_axis", "dvm_plan_query", "dvm_plan_vblocks", "dvm_destroy", "dvm_last_error",
 )
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
@@ -123,9 +124,10 @@ def lib():
         L.dvm_workspace_bytes.argtypes = [vp, C.POINTER(C.c_size_t), C.POINTER(C.c_size_t)]
         L.dvm_kernel_used.argtypes = [vp]
         L.dvm_tile_rv.argtypes = [vp]
-        L.dvm_plan_query.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(_VGrid), C.c_int, C.c_int, C.c_int, C.c_int,
+        L.dvm_tile_axis.argtypes = [vp]
+        L.dvm_plan_query.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(_VGrid), C.c_int, C.c_int, C.c_int, C.c_int, C.c_int,
                                      C.POINTER(C.c_int), C.POINTER(C.c_int), C.c_int]
-        L.dvm_plan_vblocks.argtypes = [C.POINTER(_VGrid), C.c_int, C.c_int, C.POINTER(C.c_int), C.c_int]
+        L.dvm_plan_vblocks.argtypes = [C.POINTER(_VGrid), C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int), C.c_int]
         L.dvm_launch_count.argtypes = [vp]
         L.dvm_launch_count.restype = C.c_longlong
         L.dvm_destroy.argtypes = [vp]
@@ -144,26 +146,27 @@ def _f64(a):
     return np.ascontiguousarray(a, dtype=np.float64)
 
 
-def plan_query(nx, ny, nz, xi_x, xi_y, xi_z, target_ctas=296, max_blocks=0, max_items=1 << 22, rv=0, order=1):
+def plan_query(nx, ny, nz, xi_x, xi_y, xi_z, target_ctas=296, max_blocks=0, max_items=1 << 22, rv=0, order=1, wide_axis=0):
     """dvm_plan_query: (counts dict, items int32 [n][9]) of the tile kernel's work decomposition (host only)."""
     keep = [_f64(a) for a in (xi_x, xi_y, xi_z)]
     v = _VGrid(len(keep[0]), len(keep[1]), len(keep[2]), *(a.ctypes.data_as(_dp) for a in keep), None, None, None)
     counts = (C.c_int * 5)()
-    n = _check(lib().dvm_plan_query(nx, ny, nz, C.byref(v), target_ctas, max_blocks, rv, order, counts, None, 0))
+    n = _check(lib().dvm_plan_query(nx, ny, nz, C.byref(v), target_ctas, max_blocks, rv, order, wide_axis, counts, None, 0))
     items = np.zeros((min(n, max_items), 9), dtype=np.int32)
-    _check(lib().dvm_plan_query(nx, ny, nz, C.byref(v), target_ctas, max_blocks, rv, order, counts,
+    _check(lib().dvm_plan_query(nx, ny, nz, C.byref(v), target_ctas, max_blocks, rv, order, wide_axis, counts,
                                 items.ctypes.data_as(C.POINTER(C.c_int)), len(items)))
     return {"n_vblocks": counts[0], "ntx": counts[1], "nty": counts[2], "P": counts[3], "batch": counts[4],
             "n_items": n}, items
 
 
-def plan_vblocks(xi_x, xi_y, xi_z, rv=0, order=1):
-    """dvm_plan_vblocks: int32 [n][8] = a0, na, b0, nb, c0, nc, NA, 256 nbb + ncb per velocity block (host only)."""
+def plan_vblocks(xi_x, xi_y, xi_z, rv=0, order=1, wide_axis=0):
+    """dvm_plan_vblocks: int32 [n][8] = x0, nx, y0, ny, z0, nz, NA + 65536 (1 + wide axis), 256 nbb + ncb per velocity block
+    (host only); wide_axis: 0 = the library's choice, 1 + axis otherwise."""
     keep = [_f64(a) for a in (xi_x, xi_y, xi_z)]
     v = _VGrid(len(keep[0]), len(keep[1]), len(keep[2]), *(a.ctypes.data_as(_dp) for a in keep), None, None, None)
-    n = _check(lib().dvm_plan_vblocks(C.byref(v), rv, order, None, 0))
+    n = _check(lib().dvm_plan_vblocks(C.byref(v), rv, order, wide_axis, None, 0))
     out = np.zeros((n, 8), dtype=np.int32)
-    _check(lib().dvm_plan_vblocks(C.byref(v), rv, order, out.ctypes.data_as(C.POINTER(C.c_int)), n))
+    _check(lib().dvm_plan_vblocks(C.byref(v), rv, order, wide_axis, out.ctypes.data_as(C.POINTER(C.c_int)), n))
     return out
 
 
@@ -171,7 +174,7 @@ class Solver:
     """dvm_create / dvm_iterate / dvm_moments / dvm_residual (+ support calls) for one workload record."""
 
     def __init__(self, wl, kernel: int = KERNEL_AUTO, device: str = "cuda:0", max_f_mbytes: int = 0, tile_rv: int = 0,
-                 max_ctas: int = 0, order: int = 0):
+                 max_ctas: int = 0, order: int = 0, tile_axis: int = 0):
         import torch
         if not torch.cuda.is_available():
             raise DvmError(ECUDA, "no CUDA device: the DVM solver has no CPU fallback")
@@ -228,6 +231,8 @@ class Solver:
             self.set_option(OPT_TILE_RV, int(tile_rv))
         if max_ctas:
             self.set_option(OPT_MAX_CTAS, int(max_ctas))
+        if tile_axis:
+            self.set_option(OPT_TILE_AXIS, int(tile_axis))
 
     # -- the four calls of the north star ---------------------------------------------------------
     def iterate(self, n: int = 1):
@@ -309,6 +314,9 @@ class Solver:
 
     def tile_rv(self):
         return _check(lib().dvm_tile_rv(self._h))
+
+    def tile_axis(self):
+        return _check(lib().dvm_tile_axis(self._h))
 
     def launch_count(self):
         return int(lib().dvm_launch_count(self._h))

@@ -211,10 +211,23 @@ def test_config4_full_size_stratified_step(oracle_mod, seed):
     lockstep(wl, 2, 1, oracle_mod, state=st, rho_w=None)
 
 
-def test_config3_stratified_step_two_velocities_per_thread(oracle_mod):
-    """The RV = 2 variant of the tile kernel (8 x 8 x 8 velocity blocks) on config 3 at full size, one velocity per block."""
-    wl = stratified(W.config(3), 1, rv=2)
-    lockstep(wl, 2, 1, oracle_mod, state=W.perturbed_state(wl, seed=33), rho_w=None, tile_rv=2)
+@pytest.mark.parametrize("rv", [2, 3])
+def test_config3_stratified_step_other_variants(oracle_mod, rv):
+    """The RV = 2 (8 x 8 x 8 velocity blocks) and RV = 3 (12 x 8 x 4) variants of the tile kernel on config 3 at full size, one
+    velocity per block."""
+    wl = stratified(W.config(3), 1, rv=rv)
+    lockstep(wl, 2, 1, oracle_mod, state=W.perturbed_state(wl, seed=33), rho_w=None, tile_rv=rv)
+
+
+def test_paper_cube_grid_runs_on_the_variant_chosen_for_it(oracle_mod):
+    """The paper's cube run has 24 nodes per sign half on every axis: the library picks the 12-wide RV = 3 variant for it
+    (no padded lanes); reduced-size grid with that velocity grid, in lock-step."""
+    wl = W.cube_flow_paper(5, 6, 6, 7, 48)
+    s = make(wl, 2)
+    s.iterate(1)
+    assert s.tile_rv() == 3
+    s.close()
+    lockstep(stratified(wl, 0), 2, 2, oracle_mod)
 
 
 @pytest.mark.parametrize("kernel", KERNELS)
@@ -327,7 +340,8 @@ def test_f_never_materialised(kernel):
 # ---------------------------------------------------------------------------------------------------------------------
 # Round 2: dense cases with several x-blocks per sign half, GPU counterparts of pins P13-P16, the one-step map along the
 # real trajectories, run-to-run reproducibility, the dependency protocol under stress.
-VARIANTS = [(1, {}), (2, {"tile_rv": 4}), (2, {"tile_rv": 2})]
+VARIANTS = [(1, {}), (2, {"tile_rv": 4, "tile_axis": 1}), (2, {"tile_rv": 3, "tile_axis": 1}), (2, {"tile_rv": 2, "tile_axis": 1}),
+            (2, {"tile_rv": 4, "tile_axis": 2}), (2, {"tile_rv": 3, "tile_axis": 3}), (2, {"tile_rv": 2, "tile_axis": 3})]
 
 
 @pytest.mark.parametrize("kernel,kw", VARIANTS)
@@ -437,7 +451,7 @@ def test_run_to_run_reproducibility():
 
 
 @pytest.mark.parametrize("ctas", [1, 4])
-@pytest.mark.parametrize("rv", [4, 2])
+@pytest.mark.parametrize("rv", [4, 3, 2])
 def test_dependency_protocol_under_stress(oracle_mod, ctas, rv):
     """compute-sanitizer is closed on this pool, so the done-flag / face-slot protocol of the tile kernel is stressed
     instead: many velocity blocks (5 x 3 x 5 per axis and octant pattern), tiny tiles (9 x 10 x 3 cells), a workspace cap
@@ -564,3 +578,17 @@ def test_full_weight_step_against_archived_oracle(cfg):
     assert_residual(s.residual(), gold["resid"], what=f"archived full-weight step of config {cfg}")
     assert abs(s.mass_scale() - gold["scale"]) <= 1e-12 * abs(gold["scale"])
     s.close()
+
+
+@pytest.mark.parametrize("axis", [1, 2, 3])
+@pytest.mark.parametrize("rv,order", [(4, 1), (3, 1), (2, 2)])
+def test_every_wide_axis_of_the_tile_kernel(oracle_mod, axis, rv, order):
+    """DVM_OPT_TILE_AXIS: the velocity axis that plays the wide role (RV nodes per thread x 4 lane groups) is a free choice;
+    every choice on a ragged stretched cavity with unequal node counts per axis (10 x 7 x 9), on the cube flow (shifted
+    xi_x, solid block: slow path) and on a wide grid with several blocks along each axis."""
+    kw = {"tile_rv": rv, "tile_axis": axis}
+    wl = W.cavity(0, 0, 0.075, stretch=1.5, nxyz=(13, 9, 11), mxyz=(10, 7, 9)).with_(order=order)
+    lockstep(wl, 2, 2, oracle_mod, **kw)
+    lockstep(W.cube_flow(4, 12, box=(6, 4, 4), vrange=8.0).with_(order=order), 2, 2, oracle_mod, **kw)
+    wide = W.cavity(0, 0, 0.3, nxyz=(6, 5, 7), mxyz=(18, 26, 34)).with_(order=order)
+    lockstep(wide, 2, 1, oracle_mod, state=W.perturbed_state(wide, seed=60 + axis, amp_q=0.01), rho_w=None, **kw)

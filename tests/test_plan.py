@@ -19,7 +19,7 @@ def plan(wl, target=296, max_blocks=0, rv=0, order=1):
     (W.config(1), 296, 5), (W.config(2), 296, 24), (W.config(0), 296, 1),
     (W.cavity(0, 0, 0.1, nxyz=(13, 9, 11), mxyz=(10, 7, 9)), 16, 3),
 ])
-@pytest.mark.parametrize("rv,order", [(4, 1), (2, 1), (2, 2)])
+@pytest.mark.parametrize("rv,order", [(4, 1), (3, 1), (2, 1), (2, 2)])
 def test_items_cover_everything_once_in_dependency_order(wl, target, max_blocks, rv, order):
     counts, items = plan(wl, target, max_blocks, rv, order)
     n = counts["n_items"]
@@ -81,7 +81,7 @@ def test_plan_rejects_bad_input():
 
 
 @pytest.mark.parametrize("cfg", [2, 3, 4])
-@pytest.mark.parametrize("rv", [4, 2])
+@pytest.mark.parametrize("rv", [4, 3, 2])
 def test_stratified_subset_puts_one_velocity_in_every_block(cfg, rv):
     """The full-size one-step parity cases keep one velocity per velocity block of the tile kernel (a zero-weight
     velocity is identically zero inside that kernel): exactly one kept velocity in each block of dvm_plan_vblocks, both
@@ -105,17 +105,22 @@ def test_stratified_subset_puts_one_velocity_in_every_block(cfg, rv):
     assert not np.array_equal(kept[0][0], kept[1][0])
 
 
-@pytest.mark.parametrize("rv,order,nvb,na", [(4, 1, 512, 16), (2, 1, 512, 8), (2, 2, 256, 8)])
+@pytest.mark.parametrize("rv,order,nvb,na", [(4, 1, 512, 16), (3, 1, 384, 12), (2, 1, 512, 8), (2, 2, 256, 8)])
 def test_velocity_block_boxes(rv, order, nvb, na):
     """dvm_plan_vblocks: the boxes tile the velocity grid exactly once, stay inside one sign octant, and fit the lanes of
     the kernel variant (NA x nbb x ncb = velocities per block)."""
     wl = W.config(3)
     boxes = dvm.plan_vblocks(wl.xi_x, wl.xi_y, wl.xi_z, rv, order)
     cover = np.zeros((wl.mx, wl.my, wl.mz), dtype=np.int32)
-    for a0, n_a, b0, n_b, c0, n_c, NA, shape in boxes:
+    for a0, n_a, b0, n_b, c0, n_c, code, shape in boxes:
         nbb, ncb = shape // 256, shape % 256
+        NA, wide = code % 65536, code // 65536 - 1
         assert NA == na and NA * nbb * ncb == nvb
-        assert 0 < n_a <= NA and 0 < n_b <= nbb and 0 < n_c <= ncb
+        lim = [0, 0, 0]
+        lim[wide] = NA
+        lim[[a for a in range(3) if a != wide][0]] = nbb
+        lim[[a for a in range(3) if a != wide][1]] = ncb
+        assert 0 < n_a <= lim[0] and 0 < n_b <= lim[1] and 0 < n_c <= lim[2]
         cover[a0:a0 + n_a, b0:b0 + n_b, c0:c0 + n_c] += 1
         for xi, lo, cnt in ((wl.xi_x, a0, n_a), (wl.xi_y, b0, n_b), (wl.xi_z, c0, n_c)):
             s = xi[lo:lo + cnt] >= 0
@@ -123,3 +128,32 @@ def test_velocity_block_boxes(rv, order, nvb, na):
     assert (cover == 1).all()
     with pytest.raises(dvm.DvmError):
         dvm.plan_vblocks(wl.xi_x, wl.xi_y, wl.xi_z, 4, 2)      # the second-order kernel carries 2 velocities per thread
+
+
+def test_library_picks_the_variant_that_fills_its_lanes():
+    """Config 3 (48 nodes per axis, xi_x shifted: 20 / 28 per sign, xi_y and xi_z 24 / 24): blocks 12 wide along xi_y or xi_z
+    with 4 x 8 (xi_x x the other) pairs have no padded lane at all; config 4 (32 per sign half) keeps 16-wide blocks
+    along xi_x; the paper's cube run (24 / 24 / 24) takes 12-wide blocks."""
+    for cfg, na, fill in ((3, 12, 1.0), (4, 16, 1.0), (5, 12, 1.0), (2, 16, 1.0)):
+        wl = W.config(cfg)
+        boxes = dvm.plan_vblocks(wl.xi_x, wl.xi_y, wl.xi_z)
+        NA, wide = boxes[0][6] % 65536, boxes[0][6] // 65536 - 1
+        nvb = NA * (boxes[0][7] // 256) * (boxes[0][7] % 256)
+        assert NA == na
+        assert wl.n_vel / (len(boxes) * nvb) == pytest.approx(fill)
+        if cfg == 3:
+            assert wide in (1, 2)
+
+
+@pytest.mark.parametrize("wide", [1, 2, 3])
+def test_plans_with_every_wide_axis(wide):
+    wl = W.cavity(0, 0, 0.1, nxyz=(13, 9, 11), mxyz=(10, 7, 9))
+    for rv, order in ((4, 1), (3, 1), (2, 2)):
+        boxes = dvm.plan_vblocks(wl.xi_x, wl.xi_y, wl.xi_z, rv, order, wide)
+        assert all(b[6] // 65536 == wide for b in boxes)
+        cover = np.zeros((wl.mx, wl.my, wl.mz), dtype=np.int32)
+        for a0, n_a, b0, n_b, c0, n_c, code, shape in boxes:
+            cover[a0:a0 + n_a, b0:b0 + n_b, c0:c0 + n_c] += 1
+        assert (cover == 1).all()
+        counts, items = dvm.plan_query(wl.nx, wl.ny, wl.nz, wl.xi_x, wl.xi_y, wl.xi_z, rv=rv, order=order, wide_axis=wide)
+        assert counts["n_vblocks"] == len(boxes)
