@@ -201,7 +201,7 @@ def run_gpu(args):
     wl = workload_for(args)
     kernel = {"auto": dvm.KERNEL_AUTO, "slice": dvm.KERNEL_SLICE, "tile": dvm.KERNEL_TILE}[args.kernel]
     s = dvm.Solver(wl, kernel=kernel, device=f"cuda:{local}", max_f_mbytes=args.max_f_mbytes, tile_rv=args.tile_rv,
-                   order=args.order)
+                   order=args.order, tile_axis=args.tile_axis)
     stream = torch.cuda.current_stream(dev)
 
     def barrier():
@@ -287,6 +287,7 @@ def run_gpu(args):
             "dtype": "f64", "data": "synthetic",
             "config": {"workload": wl.name, "physical_cells": [wl.nx, wl.ny, wl.nz], "velocity_nodes": [wl.mx, wl.my, wl.mz],
                        "phase_points_per_iteration": pts, "kernel": kname, "tile_rv": s.tile_rv() if kname == "tile" else None,
+                       "tile_axis": s.tile_axis() if kname == "tile" else None,
                        "order": args.order, "max_f_mbytes": args.max_f_mbytes,
                        "parallelism": "replicas only" if world > 1 else "1 GPU",
                        "l2": "inputs larger than L2 (f workspace %.1f GB, fields %.2f GB)" % (f_bytes / 1e9, (total_bytes - f_bytes) / 1e9)
@@ -321,7 +322,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--max-f-mbytes", type=int, default=0, help="cap (MiB) on the f workspace of the tile kernel (0 = none)")
     ap.add_argument("--tile-rv", type=int, default=0, choices=[0, 2, 3, 4], help="velocities per thread of the tile kernel (0 = library's choice)")
-    ap.add_argument("--order", type=int, default=1, choices=[1, 2], help="order of the upwind sweep (2: slice kernel)")
+    ap.add_argument("--tile-axis", type=int, default=0, choices=[0, 1, 2, 3], help="velocity axis in the wide role of the tile kernel (1 + axis; 0 = library's choice)")
+    ap.add_argument("--order", type=int, default=1, choices=[1, 2], help="order of the upwind sweep")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
