@@ -293,6 +293,14 @@ static void sweep_one(const odvm_problem *p, const face_tab *t, const double *pr
         gfs[b] = p->bc_type[b] == ODVM_FREESTREAM ? ghost_freestream(p, b, xi) : 0.0;
     }
     const double xi2 = xi[0] * xi[0] + xi[1] * xi[1] + xi[2] * xi[2];
+    /* f32 = 1 (reading G22 of DESIGN.md; "single precision computations"): the sweep runs in IEEE single.
+     * Every number the update of Eq.(7) takes in or produces - tau, f^S, the coefficients a_d, the ghost values, the
+     * running numerator and denominator, the quotient f_c - is rounded to single after the operation that makes it
+     * (a double operation on singles followed by this rounding IS the single operation for + - * /).  The velocity
+     * sums below stay in extended precision: only f is single. */
+    const int f32 = p->f32 != 0;
+#define SGL(x) (f32 ? (double)(float)(x) : (x))
+    for (int b = 0; b < 7; ++b) { gw[b] = SGL(gw[b]); gfs[b] = SGL(gfs[b]); }
     for (int kk = 0; kk < nz; ++kk) {
         const int k = sz > 0 ? kk : nz - 1 - kk;
         for (int jj = 0; jj < ny; ++jj) {
@@ -303,12 +311,12 @@ static void sweep_one(const odvm_problem *p, const face_tab *t, const double *pr
                 if (p->solid && p->solid[c]) { f[c] = 0.0; continue; }
                 double W[8];
                 for (int m = 0; m < 8; ++m) W[m] = prim8[m * n + c];
-                const double tau = odvm_tau(p, W[0], W[4]);
-                const double a[3] = {fabs(xi[0]) / (p->xf[i + 1] - p->xf[i]),
-                                     fabs(xi[1]) / (p->yf[j + 1] - p->yf[j]),
-                                     fabs(xi[2]) / (p->zf[k + 1] - p->zf[k])};
-                double num = odvm_feq(p, W, xi) / tau;
-                double den = 1.0 / tau;
+                const double tau = SGL(odvm_tau(p, W[0], W[4]));
+                const double a[3] = {SGL(fabs(xi[0]) / (p->xf[i + 1] - p->xf[i])),
+                                     SGL(fabs(xi[1]) / (p->yf[j + 1] - p->yf[j])),
+                                     SGL(fabs(xi[2]) / (p->zf[k + 1] - p->zf[k]))};
+                double num = SGL(SGL(odvm_feq(p, W, xi)) / tau);
+                double den = SGL(1.0 / tau);
                 int zg_face[3] = {-1, -1, -1};
                 double psi[3] = {0.0, 0.0, 0.0}, f1v[3] = {0.0, 0.0, 0.0};
                 for (int d = 0; d < 3; ++d) {
@@ -343,15 +351,15 @@ static void sweep_one(const odvm_problem *p, const face_tab *t, const double *pr
                         }
                     } else {
                         const int b = t->bc_slot[face];
-                        if (p->bc_type[b] == ODVM_WALL_DIFFUSE) fu = rho_w[face] * gw[b];
+                        if (p->bc_type[b] == ODVM_WALL_DIFFUSE) fu = SGL(rho_w[face] * gw[b]);
                         else if (p->bc_type[b] == ODVM_FREESTREAM) fu = gfs[b];
                         else { zg_face[d] = face; continue; } /* zero gradient: drop the term */
                         if (acc && acc->flux_in) acc->flux_in[face] += (long double)(w * fabs(xi[d]) * fu);
                     }
-                    num += a[d] * fu;
-                    den += a[d];
+                    num = SGL(num + SGL(a[d] * fu));
+                    den = SGL(den + a[d]);
                 }
-                const double fc = num / den;
+                const double fc = SGL(num / den);
                 f[c] = fc;
                 if (!acc) continue;
                 /* value at the downwind faces of the cell: f_c (order 1), extrapolated (order 2, G21) */
@@ -388,6 +396,7 @@ static void sweep_one(const odvm_problem *p, const face_tab *t, const double *pr
             }
         }
     }
+#undef SGL
 }
 
 int odvm_sweep_velocity(const odvm_problem *p, const double *prim8_in, const double *rho_w_in,
@@ -411,6 +420,7 @@ int odvm_step(const odvm_problem *p, const double *prim8_in, const double *rho_w
     const size_t n = (size_t)nx * ny * nz;
     const long nvel = (long)p->mx * p->my * p->mz;
     face_tab t;
+    if (p->f32 && p->order == 2) return -2; /* the single-precision sweep is stated for Eq.(7) only (G22) */
     if (build_faces(p, &t)) { free_faces(&t); return -1; }
     const int nface = t.nface;
     int nt = 1;

@@ -43,6 +43,8 @@ typedef struct {
     int rescale_mass;               /* 1 = apply the global mass rescale */
     int wall_norm;                  /* 0 = discrete Phi_unit (G4), 1 = analytic constant of Eq.(9) */
     int order;                      /* 1 = first-order upwind, Eq.(7); 2 = second-order upwind (reading G21) */
+    int f32;                        /* 0 = everything in double; 1 = the sweep of Eq.(7) in IEEE single, velocity sums in extended
+                                     * precision (the paper's timing precision; reading G22); order 1 only */
 } odvm_problem;
 
 /* number of boundary faces (domain + solid); fills nothing */

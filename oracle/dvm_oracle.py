@@ -34,6 +34,7 @@ class _Problem(C.Structure):
         ("bc_type", C.c_int * 7),
         ("bc_T", C.c_double * 7), ("bc_rho", C.c_double * 7), ("bc_u", (C.c_double * 3) * 7),
         ("rescale_mass", C.c_int), ("wall_norm", C.c_int), ("order", C.c_int),
+        ("f32", C.c_int),
     ]
 
 
@@ -112,6 +113,7 @@ class Oracle:
                 p.bc_u[b][d] = bc.u[d]
         p.rescale_mass, p.wall_norm = wl.rescale_mass, wl.wall_norm
         p.order = getattr(wl, "order", 1)
+        p.f32 = 1 if getattr(wl, "f32", False) else 0   # the sweep in IEEE single (reading G22), sums in extended precision
         self.p = p
         self.n = wl.n_cells
         self.nface = lib().odvm_num_faces(C.byref(p))

@@ -64,6 +64,7 @@ class Workload:
     wall_norm: int = 0
     iterations: int = 1
     order: int = 1          # 1 = first-order upwind Eq.(7); 2 = second-order upwind (G21)
+    f32: bool = False       # True = the sweep in IEEE single, velocity sums in double (G22)
 
     @property
     def nx(self):

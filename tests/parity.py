@@ -31,3 +31,10 @@ def assert_residual(r_gpu, r_cpu, what=""):
     """north_star 'residual histories agree to 1e-9': |r_gpu - r_cpu| <= 1e-9 r_cpu + 1e-13 (step 7)."""
     r_gpu, r_cpu = np.asarray(r_gpu), np.asarray(r_cpu)
     assert np.all(np.abs(r_gpu - r_cpu) <= 1e-9 * np.abs(r_cpu) + 1e-13), f"{what}: residual {r_gpu} vs {r_cpu}"
+
+
+def tol32(wl, K=16.0):
+    """Absolute tolerance (units of DESIGN.md section 2) of every field of the single-precision sweep against the double
+    oracle: K u L with u = 2^-24 and L = nx + ny + nz the longest upwind path (reading G22; derivation in
+    tests/test_oracle_f32.py)."""
+    return K * 2.0 ** -24 * (wl.nx + wl.ny + wl.nz)
