@@ -123,15 +123,19 @@ FP64_PEAK_TFLOPS = 2 * FP64_LANE_SLOTS_PEAK / 1e12
 #   traffic: dram__bytes_read.sum + dram__bytes_write.sum per sweep launch; inst / fp64 / dmma: thread-level instructions per
 #   point-update (smsp__inst_executed.sum x 32 / points, SASS opcode shares of the level loop); pipe / issue: ncu percentages
 NCU = {
-    "cfg4_cavity_128^3x64^3_Kn0.01": {"traffic": None, "inst_per_point": None, "fp64_inst_per_point": None, "dmma_per_point": None,
-                                      "pipe_fp64_active_pct": None, "pipe_tensor_active_pct": None, "issue_active_pct": None,
-                                      "commit": None},
+    "cfg4_cavity_128^3x64^3_Kn0.01": {"traffic": 4.3483e12, "inst_per_point": 30.2, "fp64_inst_per_point": 15.5, "dmma_per_point": 1.25,
+                                      "pipe_fp64_active_pct": 37.6, "pipe_tensor_active_pct": 24.2, "pipe_shared_active_pct": 59.9,
+                                      "issue_active_pct": 36.6, "commit": "8533099", "source": "profiles/r02_cfg4_counters.md"},
+    "cfg3_cube_96x64x64_v48^3_Ma2": {"traffic": 3.3827e11, "inst_per_point": 32.3, "fp64_inst_per_point": 16.2, "dmma_per_point": 1.25,
+                                     "pipe_fp64_active_pct": 35.4, "pipe_tensor_active_pct": 23.5, "pipe_shared_active_pct": 57.1,
+                                     "issue_active_pct": 35.3, "commit": "8533099", "source": "profiles/r02_cfg4_counters.md"},
 }
 FP64_SLOTS_PER_POINT = {"tile": 15.5, "slice": 70.0}   # executed fp64 instructions per point (SASS count)
 
 
-def algorithmic_bytes_per_point(kernel_name):
-    return {"slice": 16.0, "tile": 8.0}[kernel_name]
+def algorithmic_bytes_per_point(kernel_name, order=1):
+    # one face value written and read back per point (tile), one in-place slice value (slice); two of each at order 2
+    return {"slice": 16.0, "tile": 8.0}[kernel_name] * (2 if order == 2 else 1)
 
 
 # --------------------------------------------------------------------------------------------------
@@ -258,12 +262,14 @@ def run_gpu(args):
         peak, peak_src, _ = measured_peaks()
         # dominant kernel = the sweep (one launch per step); its duration is the step minus the small table / update launches,
         # measured here as the step itself (upper bound on the sweep time -> lower bound on achieved)
-        bpp = algorithmic_bytes_per_point(kname)
+        bpp = algorithmic_bytes_per_point(kname, args.order)
         secs = ms_per_step * 1e-3
         hbm_gbs = bpp * pts / secs / 1e9
         fp64_slots = FP64_SLOTS_PER_POINT[kname] * pts / secs            # executed fp64 lane slots per second
         frac_hbm, frac_alu = hbm_gbs / peak, fp64_slots / FP64_LANE_SLOTS_PEAK
-        ncu = NCU.get(wl.name, {})
+        # the ncu evidence belongs to the default variant (order 1, library's choice of the tile variant, no workspace cap)
+        default_variant = args.order == 1 and args.tile_rv == 0 and args.tile_axis == 0 and args.max_f_mbytes == 0 and kname == "tile"
+        ncu = NCU.get(wl.name, {}) if default_variant else {}
         if frac_hbm >= frac_alu:
             roof = {"bound": "hbm", "achieved": hbm_gbs, "peak": peak, "unit": "GB/s", "frac": frac_hbm,
                     "traffic": ncu.get("traffic"), "peak_source": peak_src}
