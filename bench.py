@@ -130,6 +130,8 @@ NCU = {
                                      "pipe_fp64_active_pct": 35.4, "pipe_tensor_active_pct": 23.5, "pipe_shared_active_pct": 57.1,
                                      "issue_active_pct": 35.3, "commit": "8533099", "source": "profiles/r02_cfg4_counters.md"},
 }
+FP32_SLOTS_PER_POINT = 11.0                         # --precision mixed: fp32 instructions per point of the tile kernel
+FP32_LANE_SLOTS_PEAK = 148 * 128 * 1.965e9          # fp32 FMA-lane issue slots per second
 FP64_SLOTS_PER_POINT = {"tile": 15.5, "slice": 70.0}   # executed fp64 instructions per point (SASS count)
 
 
@@ -205,7 +207,9 @@ def run_gpu(args):
     wl = workload_for(args)
     kernel = {"auto": dvm.KERNEL_AUTO, "slice": dvm.KERNEL_SLICE, "tile": dvm.KERNEL_TILE}[args.kernel]
     s = dvm.Solver(wl, kernel=kernel, device=f"cuda:{local}", max_f_mbytes=args.max_f_mbytes, tile_rv=args.tile_rv,
-                   order=args.order, tile_axis=args.tile_axis)
+                   order=args.order, tile_axis=args.tile_axis,
+                   precision=dvm.PREC_MIXED if args.precision == "mixed" else dvm.PREC_F64)
+    mixed = args.precision == "mixed"
     stream = torch.cuda.current_stream(dev)
 
     def barrier():
@@ -262,25 +266,32 @@ def run_gpu(args):
         peak, peak_src, _ = measured_peaks()
         # dominant kernel = the sweep (one launch per step); its duration is the step minus the small table / update launches,
         # measured here as the step itself (upper bound on the sweep time -> lower bound on achieved)
-        bpp = algorithmic_bytes_per_point(kname, args.order)
+        bpp = algorithmic_bytes_per_point(kname, args.order) * (0.5 if mixed else 1.0)   # single-precision faces
         secs = ms_per_step * 1e-3
         hbm_gbs = bpp * pts / secs / 1e9
         fp64_slots = FP64_SLOTS_PER_POINT[kname] * pts / secs            # executed fp64 lane slots per second
         frac_hbm, frac_alu = hbm_gbs / peak, fp64_slots / FP64_LANE_SLOTS_PEAK
+        if mixed:
+            # single-precision sweep: 11 fp32 instructions per point (SASS count: 3 FADD + 4 FMUL + 4 FFMA) on the 128-lane
+            # fp32 pipe; the fp64 side is one F2F (widening for the tensor-core sums) + 1.25 DMMA per point
+            fp64_slots = FP32_SLOTS_PER_POINT * pts / secs
+            frac_alu = fp64_slots / FP32_LANE_SLOTS_PEAK
         # the ncu evidence belongs to the default variant (order 1, library's choice of the tile variant, no workspace cap)
-        default_variant = args.order == 1 and args.tile_rv == 0 and args.tile_axis == 0 and args.max_f_mbytes == 0 and kname == "tile"
+        default_variant = not mixed and args.order == 1 and args.tile_rv == 0 and args.tile_axis == 0 and args.max_f_mbytes == 0 and kname == "tile"
         ncu = NCU.get(wl.name, {}) if default_variant else {}
         if frac_hbm >= frac_alu:
             roof = {"bound": "hbm", "achieved": hbm_gbs, "peak": peak, "unit": "GB/s", "frac": frac_hbm,
                     "traffic": ncu.get("traffic"), "peak_source": peak_src}
         else:
-            roof = {"bound": "alu", "achieved": 2.0 * fp64_slots / 1e12, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
-                    "frac": frac_alu, "traffic": ncu.get("traffic"),
-                    "peak_source": "derived: 148 SM x 64 fp64 lanes x 2 flop x 1.965 GHz (DESIGN.md section 6)"}
+            roof = {"bound": "alu", "achieved": 2.0 * fp64_slots / 1e12, "peak": 2e-12 * FP32_LANE_SLOTS_PEAK if mixed else FP64_PEAK_TFLOPS,
+                    "unit": "TFLOP/s", "frac": frac_alu, "traffic": ncu.get("traffic"),
+                    "peak_source": "derived: 148 SM x %d lanes x 2 flop x 1.965 GHz (DESIGN.md section 6)" % (128 if mixed else 64)}
         roof.update({"kernel": f"sweep_{kname}_kernel", "launch_ms": ms_per_step,
                      "algorithmic_bytes_per_point": bpp, "hbm_achieved_gbs": hbm_gbs, "hbm_peak_gbs": peak, "hbm_frac": frac_hbm,
-                     "fp64_executed_inst_per_point": FP64_SLOTS_PER_POINT[kname], "fp64_executed_tflops": 2.0 * fp64_slots / 1e12,
-                     "fp64_peak_tflops": FP64_PEAK_TFLOPS, "fp64_pipe_frac": frac_alu,
+                     ("fp32" if mixed else "fp64") + "_executed_inst_per_point": FP32_SLOTS_PER_POINT if mixed else FP64_SLOTS_PER_POINT[kname],
+                     ("fp32" if mixed else "fp64") + "_executed_tflops": 2.0 * fp64_slots / 1e12,
+                     ("fp32" if mixed else "fp64") + "_peak_tflops": 2e-12 * FP32_LANE_SLOTS_PEAK if mixed else FP64_PEAK_TFLOPS,
+                     ("fp32" if mixed else "fp64") + "_pipe_frac": frac_alu,
                      "algorithmic_equivalent": {"fp64_slots_per_point": ALGO_FP64_SLOTS_PER_POINT,
                                                 "tflops": 2.0 * ALGO_FP64_SLOTS_PER_POINT * pts / secs / 1e12,
                                                 "note": "SURVEY.md 8(d) count with one FMA per moment and a divide; not executed"},
@@ -290,9 +301,10 @@ def run_gpu(args):
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f64", "data": "synthetic",
+            "dtype": "f32 sweep, f64 moments" if mixed else "f64", "data": "synthetic",
             "config": {"workload": wl.name, "physical_cells": [wl.nx, wl.ny, wl.nz], "velocity_nodes": [wl.mx, wl.my, wl.mz],
-                       "phase_points_per_iteration": pts, "kernel": kname, "tile_rv": s.tile_rv() if kname == "tile" else None,
+                       "phase_points_per_iteration": pts, "kernel": kname, "precision": args.precision,
+                       "tile_rv": s.tile_rv() if kname == "tile" else None,
                        "tile_axis": s.tile_axis() if kname == "tile" else None,
                        "order": args.order, "max_f_mbytes": args.max_f_mbytes,
                        "parallelism": "replicas only" if world > 1 else "1 GPU",
@@ -330,6 +342,8 @@ def main():
     ap.add_argument("--tile-rv", type=int, default=0, choices=[0, 2, 3, 4], help="velocities per thread of the tile kernel (0 = library's choice)")
     ap.add_argument("--tile-axis", type=int, default=0, choices=[0, 1, 2, 3], help="velocity axis in the wide role of the tile kernel (1 + axis; 0 = library's choice)")
     ap.add_argument("--order", type=int, default=1, choices=[1, 2], help="order of the upwind sweep")
+    ap.add_argument("--precision", default="f64", choices=["f64", "mixed"],
+                    help="f64 (BASELINE.json's metric) or mixed = the paper's timing precision: single-precision sweep, double moments")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

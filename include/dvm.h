@@ -73,6 +73,16 @@ extern "C" {
                              threads, 12 x 8 x 4: fills sign halves of 12 k nodes) or 2 (256-thread CTAs, blocks of 8 x 8 x 8
                              nodes); 0 = the library chooses by lane use x measured speed of the variant (default) */
 
+#define DVM_OPT_PRECISION 7 /* precision f is carried in by the sweep: DVM_PREC_F64 (default) or DVM_PREC_MIXED = the paper's timing
+                             precision ("single precision computations"; reading G22): the factor tables, the
+                             faces, the plane in registers and the arithmetic of Eq.(7) are IEEE single; the velocity sums of Eq.(5)
+                             (tensor-core products, accumulator), the wall fluxes, the moment update and the residual stay double.
+                             Tile kernel, order 1, 3 or 4 velocities per thread; every other combination: DVM_EINVAL at the first
+                             dvm_iterate.  Fields then agree with the double result to 16 x 2^-24 x (nx + ny + nz) absolute
+                             (units of DESIGN.md section 2), not to 1e-11 */
+#define DVM_PREC_F64      0
+#define DVM_PREC_MIXED    1
+
 typedef struct dvm_solver dvm_solver; /* opaque */
 
 typedef struct {
@@ -164,6 +174,8 @@ int dvm_kernel_used(const dvm_solver *s);
 int dvm_tile_rv(const dvm_solver *s);
 /* 1 + velocity axis in the wide role of the tile kernel once planned (DVM_OPT_TILE_AXIS), the requested value before. */
 int dvm_tile_axis(const dvm_solver *s);
+/* DVM_PREC_F64 or DVM_PREC_MIXED (DVM_OPT_PRECISION). */
+int dvm_precision(const dvm_solver *s);
 /* Host-only (needs no device): the work decomposition the tile kernel would use for an nx x ny x nz grid and the
  * velocity nodes of v when target_ctas items should run concurrently, at most max_blocks velocity blocks are in
  * flight at once (0 = all; "smaller batches"), a thread carries rv velocities (2, 4, or 0 = the

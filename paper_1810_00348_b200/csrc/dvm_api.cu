@@ -80,6 +80,8 @@ struct dvm_solver {
     int tile_axis = 0;            // velocity axis in the wide role of the tile kernel: 0 = choose, 1 + axis
     int max_ctas = 0;             // cap on the persistent grid of the tile kernel (0 = all resident CTAs)
     int order = 1;                // 1: first-order upwind Eq.(7); 2: second-order upwind
+    int precision = DVM_PREC_F64; // DVM_PREC_MIXED: f carried in single precision by the tile kernel
+    size_t fvalue() const { return precision == DVM_PREC_MIXED ? sizeof(float) : sizeof(double); }
     bool planned = false;
     long long launches = 0;
     // device arrays
@@ -105,13 +107,13 @@ struct dvm_solver {
     VBlock *d_vblocks = nullptr;
     TileItem *d_items = nullptr;
     int *d_done = nullptr, *d_counter = nullptr;
-    double *d_xface = nullptr, *d_yface = nullptr;
+    void *d_xface = nullptr, *d_yface = nullptr;
     int tile_grid = 0, epoch = 0;
     std::vector<double> h_rho_w0;
     // factor tables of the tile kernel (tables.cu)
     std::vector<CellRec> h_rec;
     CellRec *d_rec = nullptr;
-    double *d_TX = nullptr, *d_TY = nullptr, *d_TZ = nullptr;
+    void *d_TX = nullptr, *d_TY = nullptr, *d_TZ = nullptr;
     int *d_xnode = nullptr, *d_ynode = nullptr, *d_znode = nullptr;
     int nxp = 0, nyp = 0, nxb = 0, nyb = 0, nzb = 0;
     size_t table_bytes = 0;
@@ -225,8 +227,8 @@ TileParams tile_params(dvm_solver *s)
     P.done = s->d_done; P.counter = s->d_counter; P.epoch = s->epoch;
     P.xface = s->d_xface; P.yface = s->d_yface;
     const int nvb = tile_nvb(s->tile.rv, s->tile.order), layers = tile_face_layers(s->tile.order);
-    P.xslot_doubles = (long long)s->nz * layers * TILE_TY * nvb;
-    P.yslot_doubles = (long long)s->nz * layers * TILE_TX * nvb;
+    P.xslot_values = (long long)s->nz * layers * TILE_TY * nvb;
+    P.yslot_values = (long long)s->nz * layers * TILE_TX * nvb;
     P.TX = s->d_TX; P.TY = s->d_TY; P.TZ = s->d_TZ; P.rec = s->d_rec;
     P.nxp = s->nxp; P.nyp = s->nyp; P.nbb = s->tile.nbb; P.ncb = s->tile.ncb;
     return P;
@@ -237,7 +239,7 @@ TableParams table_params(dvm_solver *s)
     TableParams T{};
     T.nx = s->nx; T.ny = s->ny; T.nz = s->nz; T.nxp = s->nxp; T.nyp = s->nyp;
     for (int r = 0; r < 3; ++r) T.ax[r] = s->tile.ax[r];
-    T.order = s->tile.order; T.dx = s->d_dx; T.dy = s->d_dy; T.dz = s->d_dz;
+    T.order = s->tile.order; T.f32 = s->precision == DVM_PREC_MIXED; T.dx = s->d_dx; T.dy = s->d_dy; T.dz = s->d_dz;
     T.na = tile_na(s->tile.rv); T.nbb = s->tile.nbb; T.ncb = s->tile.ncb; T.nxb = s->nxb; T.nyb = s->nyb; T.nzb = s->nzb;
     T.ncell = s->ncell; T.coef = s->d_coef; T.flags = s->d_flags;
     T.invdx = s->d_invdx; T.invdy = s->d_invdy; T.invdz = s->d_invdz;
@@ -254,7 +256,7 @@ TableParams table_params(dvm_solver *s)
 // or 8 x 64 nodes per sign octant, the wide side along the chosen velocity axis) x (measured throughput of the variant
 // relative to RV = 4 when all fill their blocks).  rv / axis > 0 (resp. >= 0) fix that part.
 constexpr double RV_SPEED[5] = {0.0, 0.0, 0.80, 0.90, 1.0};
-void choose_variant(const std::vector<double> xi[3], int order, int rv_fixed, int axis_fixed, int *rv_out, int *axis_out)
+void choose_variant(const std::vector<double> xi[3], int order, int rv_fixed, int axis_fixed, int *rv_out, int *axis_out, bool f32 = false)
 {
     if (rv_fixed == 0)
         if (const char *e = std::getenv("DVM_TILE_RV")) { const int v = std::atoi(e); if (v >= 2 && v <= 4) rv_fixed = v; }
@@ -266,6 +268,7 @@ void choose_variant(const std::vector<double> xi[3], int order, int rv_fixed, in
     double best_score = -1.0;
     for (int rv = 4; rv >= 2; --rv) {
         if (rv_fixed && rv != rv_fixed) continue;
+        if (!rv_fixed && !tile_variant_exists(rv, order, f32)) continue;
         for (int ax = 0; ax < 3; ++ax) {
             if (axis_fixed >= 0 && ax != axis_fixed) continue;
             TilePlan tp;
@@ -306,6 +309,9 @@ int plan_once(dvm_solver *s)
     if (kernel == DVM_KERNEL_AUTO) kernel = DVM_KERNEL_TILE;
     if (kernel == DVM_KERNEL_TILE && s->order == 2 && s->tile_rv > 2)
         return fail(DVM_EINVAL, "the second-order tile kernel carries 2 velocities per thread (DVM_OPT_TILE_RV = 2 or 0)");
+    const bool f32 = s->precision == DVM_PREC_MIXED;
+    if (f32 && (kernel != DVM_KERNEL_TILE || s->order != 1 || s->tile_rv == 2))
+        return fail(DVM_EINVAL, "DVM_PREC_MIXED is a mode of the first-order tile kernel with 3 or 4 velocities per thread");
     s->kernel = kernel;
     int lo[3][2], cnt[3][2];
     for (int d = 0; d < 3; ++d) split_axis(s->xi[d], lo[d], cnt[d]);
@@ -337,9 +343,9 @@ int plan_once(dvm_solver *s)
         int per_sm = 0, dev = 0, nsm = 0;
         const int order = s->order;
         int rv = 0, wide = 0;
-        choose_variant(s->xi, order, s->tile_rv, s->tile_axis - 1, &rv, &wide);
+        choose_variant(s->xi, order, s->tile_rv, s->tile_axis - 1, &rv, &wide, f32);
         s->tile_rv = rv; s->tile_axis = wide + 1;
-        CK(tile_configure(rv, order, wide, &per_sm));
+        CK(tile_configure(rv, order, f32, wide, &per_sm));
         CK(cudaGetDevice(&dev));
         CK(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
         if (per_sm < 1) return fail(DVM_ECUDA, "tile kernel does not fit on an SM");
@@ -348,15 +354,16 @@ int plan_once(dvm_solver *s)
         if (s->max_f_mbytes > 0) {
             // cap on the f workspace: fewer velocity blocks in flight (batches); the band height P
             // grows as the batch shrinks, so iterate to a fixed point; one block is the floor
-            const double cap = (double)s->max_f_mbytes * 1048576.0, lvl = (double)s->nz * tile_nvb(rv, order) * tile_face_layers(order) * 8.0;
+            const double vbytes = (double)s->fvalue();
+            const double cap = (double)s->max_f_mbytes * 1048576.0, lvl = (double)s->nz * tile_nvb(rv, order) * tile_face_layers(order) * vbytes;
             int B = (int)s->tile.vblocks.size();
             for (int pass = 0; pass < 8; ++pass) {
-                const double need = (double)(s->tile.xface_doubles + s->tile.yface_doubles) * 8.0;
+                const double need = (double)(s->tile.xface_values + s->tile.yface_values) * vbytes;
                 if (need <= cap || B == 1) break;
                 B = std::max(1, std::min(B - 1, (int)(cap / ((s->tile.P * TILE_TY + s->tile.ntx * TILE_TX) * lvl))));
                 if (tile_plan(s->nx, s->ny, s->nz, s->xi, resident, B, rv, order, wide, &s->tile)) return fail(DVM_EINVAL, "tile plan failed");
             }
-            const double need = (double)(s->tile.xface_doubles + s->tile.yface_doubles) * 8.0;
+            const double need = (double)(s->tile.xface_values + s->tile.yface_values) * vbytes;
             if (need > cap)
                 return fail(DVM_EINVAL, "the f workspace needs %.1f MiB even with one velocity block in flight: the cap of %lld MiB "
                             "(DVM_OPT_MAX_F_MBYTES) cannot be met", need / 1048576.0, s->max_f_mbytes);
@@ -364,9 +371,9 @@ int plan_once(dvm_solver *s)
         const size_t nitems = s->tile.items.size();
         s->tile_grid = (int)std::min<size_t>((size_t)resident, nitems);
         if (s->max_ctas > 0) s->tile_grid = std::min(s->tile_grid, s->max_ctas);
-        const size_t fbytes = (s->tile.xface_doubles + s->tile.yface_doubles) * sizeof(double);
-        s->d_xface = (double *)s->dalloc(s->tile.xface_doubles * sizeof(double));
-        s->d_yface = (double *)s->dalloc(s->tile.yface_doubles * sizeof(double));
+        const size_t fbytes = (s->tile.xface_values + s->tile.yface_values) * s->fvalue();
+        s->d_xface = s->dalloc(s->tile.xface_values * s->fvalue());
+        s->d_yface = s->dalloc(s->tile.yface_values * s->fvalue());
         if (!s->d_xface || !s->d_yface) return fail(DVM_ENOMEM, "tile face workspace of %zu bytes failed", fbytes);
         s->f_bytes = fbytes;
         // factor tables on the padded grid: [1-D block][nz][nyp][nxp][width] entries of 32 bytes, zero in the padding
@@ -375,10 +382,12 @@ int plan_once(dvm_solver *s)
             s->nyb = (int)s->tile.ynode.size() / s->tile.nbb;
             s->nzb = (int)s->tile.znode.size() / s->tile.ncb;
             const size_t npc = (size_t)s->nz * s->nyp * s->nxp;
-            const size_t ed = (size_t)tile_entry_doubles(order);
-            const size_t ex = npc * s->tile.xnode.size() * ed, ey = npc * s->tile.ynode.size() * ed, ez = npc * s->tile.znode.size() * ed;
-            if (dzeros(s, &s->d_TX, ex) || dzeros(s, &s->d_TY, ey) || dzeros(s, &s->d_TZ, ez)) return DVM_ENOMEM;
-            s->table_bytes = (ex + ey + ez) * sizeof(double);
+            const size_t eb = (size_t)tile_entry_values(order) * s->fvalue();   // bytes per entry
+            const size_t ex = npc * s->tile.xnode.size() * eb, ey = npc * s->tile.ynode.size() * eb, ez = npc * s->tile.znode.size() * eb;
+            unsigned char *tx = nullptr, *ty = nullptr, *tz = nullptr;
+            if (dzeros(s, &tx, ex) || dzeros(s, &ty, ey) || dzeros(s, &tz, ez)) return DVM_ENOMEM;
+            s->d_TX = tx; s->d_TY = ty; s->d_TZ = tz;
+            s->table_bytes = ex + ey + ez;
             if (upload(s, &s->d_rec, s->h_rec.data(), s->h_rec.size())) return DVM_ENOMEM;
             if (upload(s, &s->d_xnode, s->tile.xnode.data(), s->tile.xnode.size())) return DVM_ENOMEM;
             if (upload(s, &s->d_ynode, s->tile.ynode.data(), s->tile.ynode.size())) return DVM_ENOMEM;
@@ -512,7 +521,7 @@ int dvm_create(const dvm_grid *g, const dvm_vgrid *v, const dvm_gas *gas, const 
             const int ic = std::min(std::max(i, 0), nx - 1), jc = std::min(std::max(j, 0), ny - 1);
             const long long c = ((long long)k * ny + jc) * nx + ic;
             CellRec &r = s->h_rec[((size_t)k * s->nyp + jp) * s->nxp + ip];
-            r.nu = 1.0; r.cidx = (int)c; r.flags = REC_DEAD; r.pad[0] = r.pad[1] = 0;
+            r.nu = 1.0; r.nu32 = 1.0f; r.cidx = (int)c; r.flags = REC_DEAD; r.pad = 0;
             for (int d = 0; d < 6; ++d) r.face[d] = -1;
             if (!inside || s->solid[c]) continue;
             r.flags = (int)(flags[c] & 63) | ((int)(sflags[c] & 63) << 8);
@@ -648,6 +657,12 @@ int dvm_set_option(dvm_solver *s, int option, int value)
         s->order = value;
         return DVM_OK;
     }
+    if (option == DVM_OPT_PRECISION) {
+        if (s->planned) return fail(DVM_EINVAL, "the precision of the sweep must be chosen before the first iteration");
+        if (value != DVM_PREC_F64 && value != DVM_PREC_MIXED) return fail(DVM_EINVAL, "precision: DVM_PREC_F64 or DVM_PREC_MIXED");
+        s->precision = value;
+        return DVM_OK;
+    }
     if (option == DVM_OPT_MAX_CTAS) {
         if (s->planned) return fail(DVM_EINVAL, "the grid cap must be set before the first iteration");
         if (value < 0) return fail(DVM_EINVAL, "negative grid cap");
@@ -682,7 +697,7 @@ int dvm_iterate(dvm_solver *s, int niter)
             CK(cudaMemsetAsync(s->d_counter, 0, sizeof(int), s->stream));
             s->epoch += 1;
             const TileParams TP = tile_params(s);
-            CK(launch_sweep_tile(TP, s->tile_rv, s->order, s->tile.ax[0], s->tile_grid, s->stream));
+            CK(launch_sweep_tile(TP, s->tile_rv, s->order, s->precision == DVM_PREC_MIXED, s->tile.ax[0], s->tile_grid, s->stream));
             CK(launch_phi_from_raw(U, s->d_face_cell, s->d_face_dir, s->d_phi, s->order, s->stream));
             s->launches += 1;
         }
@@ -721,6 +736,7 @@ int dvm_iterations_done(const dvm_solver *s) { return s ? s->iters : fail(DVM_EI
 int dvm_kernel_used(const dvm_solver *s) { return s ? s->kernel : fail(DVM_EINVAL, "NULL solver"); }
 int dvm_tile_rv(const dvm_solver *s) { return s ? s->tile_rv : fail(DVM_EINVAL, "NULL solver"); }
 int dvm_tile_axis(const dvm_solver *s) { return s ? s->tile_axis : fail(DVM_EINVAL, "NULL solver"); }
+int dvm_precision(const dvm_solver *s) { return s ? s->precision : fail(DVM_EINVAL, "NULL solver"); }
 long long dvm_launch_count(const dvm_solver *s) { return s ? s->launches : -1; }
 
 int dvm_get_state(dvm_solver *s, double *dev_prim14, double *dev_rho_wall)

@@ -25,6 +25,10 @@
 //    read back by the downwind item with TMA bulk copies (cp.async.bulk + mbarrier) two levels ahead;
 //  * items are handed out by an atomic counter in dependency order (tile_plan.cu); done-flags gate their start.
 //
+//  * R = the type f is carried in: double, or float for DVM_OPT_PRECISION = DVM_PREC_MIXED (the paper's timing precision,
+//    PAPER.md:313; reading G22): factor tables, faces, the plane in registers and the arithmetic of Eq.(7) are then
+//    IEEE single, the velocity sums (DMMA operands, accumulator, REDs) stay double.
+//
 // Product code: shares nothing with oracle/.
 #include "sweep_tile.cuh"
 
@@ -40,17 +44,25 @@ constexpr int NCELL = TILE_NCELL;
 constexpr int GA = TILE_GA;
 constexpr unsigned REC_ROW_BYTES = 4 * (unsigned)sizeof(CellRec);
 
-// Kernel variant: RV velocities per thread, ORD = order of the upwind sweep (sweep_tile.cuh)
-template <int RV, int ORD>
+// vector types of the carried type
+template <typename R> struct Vec;
+template <> struct Vec<double> { using v2 = double2; using v4 = double4; };
+template <> struct Vec<float> { using v2 = float2; using v4 = float4; };
+
+// Kernel variant: RV velocities per thread, ORD = order of the upwind sweep, R = type f is carried in (sweep_tile.cuh)
+template <int RV, int ORD, typename R>
 struct KC {
     static constexpr int THREADS = (ORD == 2 || RV >= 3) ? 128 : 256;
     static constexpr int WARPS = THREADS / 32;
     static constexpr int NVB = THREADS * RV;                 // velocities per block
-    static constexpr int ES = ORD == 2 ? 48 : 32;            // bytes of a factor-table entry
+    static constexpr int ES = (ORD == 2 ? 6 : 4) * (int)sizeof(R);   // bytes of a factor-table entry
     static constexpr int LAYERS = ORD;                       // upwind values per direction carried through a face
-    static constexpr int XLEVEL_DOUBLES = LAYERS * TILE_TY * NVB;   // one level of an x-face slot
-    static constexpr int YLEVEL_DOUBLES = LAYERS * TILE_TX * NVB;   // one level of a y-face slot
-    static constexpr unsigned XLEVEL_BYTES = XLEVEL_DOUBLES * 8u, YLEVEL_BYTES = YLEVEL_DOUBLES * 8u;
+    static constexpr int XLEVEL_VALUES = LAYERS * TILE_TY * NVB;   // one level of an x-face slot
+    static constexpr int YLEVEL_VALUES = LAYERS * TILE_TX * NVB;   // one level of a y-face slot
+    static constexpr unsigned XLEVEL_BYTES = XLEVEL_VALUES * (unsigned)sizeof(R), YLEVEL_BYTES = YLEVEL_VALUES * (unsigned)sizeof(R);
+    // resident CTAs per SM the kernel is compiled for: the double plane takes 128 registers of a thread (2 CTAs of 128
+    // threads x 255 registers), the single plane half of that
+    static constexpr int MIN_CTAS = sizeof(R) == 4 ? DVM_TILE_F32_CTAS : 2;
 };
 
 // One TMA bulk copy per level: source of level 0, byte step per level, destination in a LevelBuf; bytes = 0: skipped.
@@ -64,29 +76,29 @@ constexpr int NCOPY = 4 * TILE_TY + 2;              // per row: x, y, z factor r
 
 // One tile row (4 cells along x) of one level: everything the row's arithmetic reads sits at a static offset from the
 // row's base address, whatever the row index and the level parity are.
-template <int RV, int ORD>
+template <int RV, int ORD, typename R>
 struct __align__(128) RowBuf {
     // ---- staged by TMA two levels ahead ----
-    alignas(16) unsigned char xtab[4 * GA * RV * KC<RV, ORD>::ES];   // per (cell', xi_x node): E, Q, e, a [order 2: E, Q, e, cd, c1,
-    alignas(16) unsigned char ytab[4 * 8 * KC<RV, ORD>::ES];         // c2] (slot r*4 + ag); cell' = position of the cell in ascending
-    alignas(16) unsigned char ztab[4 * 8 * KC<RV, ORD>::ES];         // absolute x;  y: [cell'][nbb], z: [cell'][ncb]
+    alignas(16) unsigned char xtab[4 * GA * RV * KC<RV, ORD, R>::ES];   // per (cell', xi_x node): E, Q, e, a [order 2: E, Q, e, cd, c1,
+    alignas(16) unsigned char ytab[4 * 8 * KC<RV, ORD, R>::ES];         // c2] (slot r*4 + ag); cell' = position of the cell in ascending
+    alignas(16) unsigned char ztab[4 * 8 * KC<RV, ORD, R>::ES];         // absolute x;  y: [cell'][nbb], z: [cell'][ncb]
     CellRec rec[4];                                // per cell': 1/tau, accumulator row, neighbour flags, boundary faces
     // ---- decoded by 16 threads on levels that hold a solid ghost (slow path; sweep-relative cell ii) ----
     double4 spec[4];                               // rho_w of a solid ghost in x, y, z
     int code[4];                                   // 1: x-up solid ghost, 2: y-up, 4: z-up, 8: dead cell
 };
 
-template <int RV, int ORD>
+template <int RV, int ORD, typename R>
 struct __align__(128) LevelBuf {
-    RowBuf<RV, ORD> row[TILE_TY];
-    double xface[KC<RV, ORD>::LAYERS][TILE_TY][KC<RV, ORD>::NVB];   // x-face input of the level (layer 0: nearest upwind cell)
-    double yface[KC<RV, ORD>::LAYERS][TILE_TX][KC<RV, ORD>::NVB];   // y-face input of the level
+    RowBuf<RV, ORD, R> row[TILE_TY];
+    alignas(16) R xface[KC<RV, ORD, R>::LAYERS][TILE_TY][KC<RV, ORD, R>::NVB];   // x-face input of the level (layer 0: nearest upwind cell)
+    alignas(16) R yface[KC<RV, ORD, R>::LAYERS][TILE_TX][KC<RV, ORD, R>::NVB];   // y-face input of the level
     double rwb[8];                                 // ghost densities of the domain faces: 4 x-face rows, 4 y-face columns
 };
 
-template <int RV, int ORD>
+template <int RV, int ORD, typename R>
 struct __align__(128) TileSmem {
-    LevelBuf<RV, ORD> lv[2];                            // index = level parity
+    LevelBuf<RV, ORD, R> lv[2];                            // index = level parity
     // ---- per item ----
     double xi_a[16];                               // nodes of the block (0 beyond the box)
     double xi_bc[TILE_MAXBC];
@@ -165,6 +177,20 @@ __device__ __forceinline__ double fast_rcp(double d)
     const double t = fma(e, e, e);
     return fma(y, t, y);
 }
+__device__ __forceinline__ float fast_rcp(float d)
+{
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(d));   // MUFU.RCP: 1 ulp
+    return y;
+}
+// MUFU seed of 1 / d in the carried type
+__device__ __forceinline__ double rcp_seed(double d)
+{
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(d));
+    return y;
+}
+__device__ __forceinline__ float rcp_seed(float d) { return fast_rcp(d); }
 // Global REDs and face stores are volatile asm statements: they keep their program order, so ptxas cannot sink the
 // stores of a whole level to its end, where the burst would stall the warp on the load/store unit.
 __device__ __forceinline__ void red_f64(double *addr, double v)
@@ -178,6 +204,18 @@ __device__ __forceinline__ void st_f64x2(double *addr, double a, double b)
 __device__ __forceinline__ void st_f64(double *addr, double a)
 {
     asm volatile("st.global.f64 [%0], %1;" ::"l"(addr), "d"(a));
+}
+__device__ __forceinline__ void st_f32x4(float *addr, float a, float b, float c, float d)
+{
+    asm volatile("st.global.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(addr), "f"(a), "f"(b), "f"(c), "f"(d));
+}
+__device__ __forceinline__ void st_f32x2(float *addr, float a, float b)
+{
+    asm volatile("st.global.v2.f32 [%0], {%1, %2};" ::"l"(addr), "f"(a), "f"(b));
+}
+__device__ __forceinline__ void st_f32(float *addr, float a)
+{
+    asm volatile("st.global.f32 [%0], %1;" ::"l"(addr), "f"(a));
 }
 
 // D (8 x 8) += A (8 x 4, row-major) * B (4 x 8, column-major) in fp64 on the tensor cores (DMMA).  Fragments of lane l:
@@ -252,8 +290,8 @@ __device__ __forceinline__ double rwb_load(const TileParams &P, const ItemCtx &I
     return v;
 }
 
-template <int RV, int ORD>
-__device__ __forceinline__ void rwb_store(TileSmem<RV, ORD> &s, int b, int tid, double v)
+template <int RV, int ORD, typename R>
+__device__ __forceinline__ void rwb_store(TileSmem<RV, ORD, R> &s, int b, int tid, double v)
 {
     if (tid >= 32 && tid < 40) s.lv[b].rwb[tid - 32] = v;
 }
@@ -261,18 +299,18 @@ __device__ __forceinline__ void rwb_store(TileSmem<RV, ORD> &s, int b, int tid, 
 // The TMA copies of a level are described once per item (setup_copies: per 4-cell row the x, y, z factor-table rows and
 // the cell records - tables.cu; every row is one contiguous run of the padded grid - plus the x- and y-face input) and
 // issued per level by lane q / WARPS of warp q % WARPS for copy q (issue_level), so the copies are spread over the warps.
-template <int RV, int ORD>
-__device__ __forceinline__ int copy_of_thread(int tid) { return (tid & 31) * KC<RV, ORD>::WARPS + (tid >> 5); }
+template <int RV, int ORD, typename R>
+__device__ __forceinline__ int copy_of_thread(int tid) { return (tid & 31) * KC<RV, ORD, R>::WARPS + (tid >> 5); }
 
-template <int RV, int ORD>
-__device__ __forceinline__ void setup_copies(const TileParams &P, const ItemCtx &I, TileSmem<RV, ORD> &s, const VBlock &vb, int tid,
-                                             const double *xsrc, const double *ysrc)
+template <int RV, int ORD, typename R>
+__device__ __forceinline__ void setup_copies(const TileParams &P, const ItemCtx &I, TileSmem<RV, ORD, R> &s, const VBlock &vb, int tid,
+                                             const R *xsrc, const R *ysrc)
 {
-    using RB = RowBuf<RV, ORD>;
-    using LB = LevelBuf<RV, ORD>;
-    constexpr int NA = GA * RV, ES = KC<RV, ORD>::ES;
-    constexpr unsigned XLEVEL_BYTES = KC<RV, ORD>::XLEVEL_BYTES, YLEVEL_BYTES = KC<RV, ORD>::YLEVEL_BYTES;
-    const int q = copy_of_thread<RV, ORD>(tid);
+    using RB = RowBuf<RV, ORD, R>;
+    using LB = LevelBuf<RV, ORD, R>;
+    constexpr int NA = GA * RV, ES = KC<RV, ORD, R>::ES;
+    constexpr unsigned XLEVEL_BYTES = KC<RV, ORD, R>::XLEVEL_BYTES, YLEVEL_BYTES = KC<RV, ORD, R>::YLEVEL_BYTES;
+    const int q = copy_of_thread<RV, ORD, R>(tid);
     if (q >= NCOPY) return;
     const unsigned xbytes = 4u * NA * ES, ybytes = 4u * vb.nbb * ES, zbytes = 4u * vb.ncb * ES;
     CopyDesc d;
@@ -292,7 +330,7 @@ __device__ __forceinline__ void setup_copies(const TileParams &P, const ItemCtx 
         const int k = I.sz > 0 ? 0 : P.nz - 1;
         const long long npc = (long long)P.nz * P.nyp * P.nxp, lvl = (long long)P.nyp * P.nxp * I.sz;
         const long long pc = ((long long)k * P.nyp + (j + TILE_PAD)) * P.nxp + (i + TILE_PAD);
-        const unsigned rowoff = (unsigned)(offsetof(LB, row) + jj * sizeof(RowBuf<RV, ORD>));
+        const unsigned rowoff = (unsigned)(offsetof(LB, row) + jj * sizeof(RowBuf<RV, ORD, R>));
         if (kind == 0) {
             d.src = reinterpret_cast<const unsigned char *>(P.TX) + ((long long)vb.xb * npc + pc) * NA * ES;
             d.step = lvl * NA * ES; d.dst = rowoff + (unsigned)offsetof(RB, xtab); d.bytes = xbytes;
@@ -314,10 +352,10 @@ __device__ __forceinline__ void setup_copies(const TileParams &P, const ItemCtx 
 }
 
 // issue the copies of level kp into buffer kp & 1 (the descriptors were written by the same threads)
-template <int RV, int ORD>
-__device__ __forceinline__ void issue_level(TileSmem<RV, ORD> &s, int kp, int tid)
+template <int RV, int ORD, typename R>
+__device__ __forceinline__ void issue_level(TileSmem<RV, ORD, R> &s, int kp, int tid)
 {
-    const int q = copy_of_thread<RV, ORD>(tid);
+    const int q = copy_of_thread<RV, ORD, R>(tid);
     if (q >= NCOPY) return;
     const int b = kp & 1;
     if (q == 0) mbar_expect_tx(&s.mbar[b], s.txbytes);
@@ -328,8 +366,8 @@ __device__ __forceinline__ void issue_level(TileSmem<RV, ORD> &s, int kp, int ti
 // Does the level staged in buffer b hold a fluid cell whose upwind neighbour is a masked cell?  Asked by lanes 0..15 of
 // warp 0 (one record each) right after they have waited for the level's copies; the answer reaches the other threads
 // through the CTA barrier that ends the level before.
-template <int RV, int ORD>
-__device__ __forceinline__ void detect_special(const ItemCtx &I, TileSmem<RV, ORD> &s, int b, int lane)
+template <int RV, int ORD, typename R>
+__device__ __forceinline__ void detect_special(const ItemCtx &I, TileSmem<RV, ORD, R> &s, int b, int lane)
 {
     const CellRec &r = s.lv[b].row[lane >> 2].rec[lane & 3];
     const int upmask = (1 << I.upx) | (1 << I.upy) | (1 << I.upz);
@@ -340,14 +378,14 @@ __device__ __forceinline__ void detect_special(const ItemCtx &I, TileSmem<RV, OR
 
 // Slow path only: per-cell ghost codes of the level in buffer b, decoded from the staged records by the first 16 threads
 // of the last warp.
-template <int RV, int ORD>
-__device__ __forceinline__ void decode_records(const TileParams &P, const ItemCtx &I, TileSmem<RV, ORD> &s, int b, int tid)
+template <int RV, int ORD, typename R>
+__device__ __forceinline__ void decode_records(const TileParams &P, const ItemCtx &I, TileSmem<RV, ORD, R> &s, int b, int tid)
 {
-    constexpr int T0 = KC<RV, ORD>::THREADS - 32;
+    constexpr int T0 = KC<RV, ORD, R>::THREADS - 32;
     if (tid >= T0 && tid < T0 + NCELL) {
         const int cell = tid - T0, ii = cell & 3, jj = cell >> 2;
-        RowBuf<RV, ORD> &R = s.lv[b].row[jj];
-        const CellRec &r = R.rec[I.sx > 0 ? ii : 3 - ii];
+        RowBuf<RV, ORD, R> &Rw = s.lv[b].row[jj];
+        const CellRec &r = Rw.rec[I.sx > 0 ? ii : 3 - ii];
         const bool dead = (r.flags & REC_DEAD) != 0;
         const int sfl = (r.flags >> 8) & 0xff;
         int code = 8;
@@ -358,8 +396,8 @@ __device__ __forceinline__ void decode_records(const TileParams &P, const ItemCt
             if (code & 2) sp.y = P.rho_w[r.face[I.upy]];
             if (code & 4) sp.z = P.rho_w[r.face[I.upz]];
         }
-        R.code[ii] = code;
-        R.spec[ii] = sp;
+        Rw.code[ii] = code;
+        Rw.spec[ii] = sp;
     }
 }
 
@@ -367,37 +405,53 @@ __device__ __forceinline__ void decode_records(const TileParams &P, const ItemCt
 // (h * threads + t) * 2 (odd RV: the last value of thread t follows the pairs, at pairs + t): every 16-byte access of a
 // warp then covers 512 contiguous bytes (full sectors in L2 / HBM, no bank conflict in shared memory).  row = start of the
 // face row.
-template <int RV, int ORD>
+// Single values with RV = 4: the four values of a thread are one 16-byte quad at tid * 4.
+__device__ __forceinline__ void st_pair(double *a, double x, double y) { st_f64x2(a, x, y); }
+__device__ __forceinline__ void st_pair(float *a, float x, float y) { st_f32x2(a, x, y); }
+__device__ __forceinline__ void st_one(double *a, double x) { st_f64(a, x); }
+__device__ __forceinline__ void st_one(float *a, float x) { st_f32(a, x); }
+template <int RV, int ORD, typename R>
 __device__ __forceinline__ int face_index(int tid, int r)
 {
-    constexpr int TH = KC<RV, ORD>::THREADS;
+    constexpr int TH = KC<RV, ORD, R>::THREADS;
+    if (sizeof(R) == 4 && RV == 4) return tid * 4 + r;
     return r < 2 * (RV / 2) ? ((r >> 1) * TH + tid) * 2 + (r & 1) : (RV / 2) * TH * 2 + tid;
 }
-template <int RV, int ORD>
-__device__ __forceinline__ void load_face(const double *row, int tid, double (&v)[RV])
+template <int RV, int ORD, typename R>
+__device__ __forceinline__ void load_face(const R *row, int tid, R (&v)[RV])
 {
-    constexpr int TH = KC<RV, ORD>::THREADS;
+    constexpr int TH = KC<RV, ORD, R>::THREADS;
+    using V2 = typename Vec<R>::v2;
+    if (sizeof(R) == 4 && RV == 4) {
+        const float4 t = reinterpret_cast<const float4 *>(row)[tid];
+        v[0] = t.x; v[1] = t.y; v[2 % RV] = t.z; v[3 % RV] = t.w;
+    } else {
 #pragma unroll
-    for (int h = 0; h < RV / 2; ++h) {
-        const double2 t = reinterpret_cast<const double2 *>(row)[h * TH + tid];
-        v[2 * h] = t.x; v[2 * h + 1] = t.y;
+        for (int h = 0; h < RV / 2; ++h) {
+            const V2 t = reinterpret_cast<const V2 *>(row)[h * TH + tid];
+            v[2 * h] = t.x; v[2 * h + 1] = t.y;
+        }
+        if (RV & 1) v[RV - 1] = row[(RV / 2) * TH * 2 + tid];
     }
-    if (RV & 1) v[RV - 1] = row[(RV / 2) * TH * 2 + tid];
 }
-template <int RV, int ORD>
-__device__ __forceinline__ void store_face(double *row, int tid, const double (&v)[RV])
+template <int RV, int ORD, typename R>
+__device__ __forceinline__ void store_face(R *row, int tid, const R (&v)[RV])
 {
-    constexpr int TH = KC<RV, ORD>::THREADS;
+    constexpr int TH = KC<RV, ORD, R>::THREADS;
+    if (sizeof(R) == 4 && RV == 4) {
+        st_f32x4(reinterpret_cast<float *>(row) + tid * 4, (float)v[0], (float)v[1], (float)v[2 % RV], (float)v[3 % RV]);
+    } else {
 #pragma unroll
-    for (int h = 0; h < RV / 2; ++h) st_f64x2(row + (h * TH + tid) * 2, v[2 * h], v[2 * h + 1]);
-    if (RV & 1) st_f64(row + (RV / 2) * TH * 2 + tid, v[RV - 1]);
+        for (int h = 0; h < RV / 2; ++h) st_pair(row + (h * TH + tid) * 2, v[2 * h], v[2 * h + 1]);
+        if (RV & 1) st_one(row + (RV / 2) * TH * 2 + tid, v[RV - 1]);
+    }
 }
 
 // Ghost values of the domain faces of level kp (buffer b) for a tile at the upwind x / y edge of the domain
-template <int RV, int ORD>
-__device__ __forceinline__ void fill_faces(const ItemCtx &I, TileSmem<RV, ORD> &s, int b, int tid, int ag, int yidx, int zidx)
+template <int RV, int ORD, typename R>
+__device__ __forceinline__ void fill_faces(const ItemCtx &I, TileSmem<RV, ORD, R> &s, int b, int tid, int ag, int yidx, int zidx)
 {
-    LevelBuf<RV, ORD> &L = s.lv[b];
+    LevelBuf<RV, ORD, R> &L = s.lv[b];
     if (I.first_x) {
         const double gyz = s.g[0][1][yidx] * s.g[0][2][zidx];
 #pragma unroll
@@ -405,8 +459,8 @@ __device__ __forceinline__ void fill_faces(const ItemCtx &I, TileSmem<RV, ORD> &
             const double G = s.g[0][0][RV * ag + r] * gyz;
 #pragma unroll
             for (int jj = 0; jj < TILE_TY; ++jj) {
-                L.xface[0][jj][face_index<RV, ORD>(tid, r)] = L.rwb[jj] * G;
-                if (ORD == 2) L.xface[ORD - 1][jj][face_index<RV, ORD>(tid, r)] = 0.0;   // second upwind value: its coefficient is 0
+                L.xface[0][jj][face_index<RV, ORD, R>(tid, r)] = (R)(L.rwb[jj] * G);
+                if (ORD == 2) L.xface[ORD - 1][jj][face_index<RV, ORD, R>(tid, r)] = (R)0;   // second upwind value: its coefficient is 0
             }
         }
     }
@@ -417,15 +471,15 @@ __device__ __forceinline__ void fill_faces(const ItemCtx &I, TileSmem<RV, ORD> &
             const double G = s.g[1][0][RV * ag + r] * gyz;
 #pragma unroll
             for (int ii = 0; ii < 4; ++ii) {
-                L.yface[0][ii][face_index<RV, ORD>(tid, r)] = L.rwb[4 + ii] * G;
-                if (ORD == 2) L.yface[ORD - 1][ii][face_index<RV, ORD>(tid, r)] = 0.0;
+                L.yface[0][ii][face_index<RV, ORD, R>(tid, r)] = (R)(L.rwb[4 + ii] * G);
+                if (ORD == 2) L.yface[ORD - 1][ii][face_index<RV, ORD, R>(tid, r)] = (R)0;
             }
         }
     }
 }
 
 // per-thread constants of an item
-template <int RV, int ORD>
+template <int RV, int ORD, typename R>
 struct ThreadCtx {
     double aX[RV];               // stage-1 A fragments per node r: xi_x^p, p = (lane >> 2) & 3
     double yz0, yz1;             // stage-2 B fragments: monomial lane >> 2 of the warp's pairs 2 (lane & 3), 2 (lane & 3) + 1
@@ -437,37 +491,40 @@ struct ThreadCtx {
     int xrev;                    // 3 if the sweep runs against x (table rows are in ascending absolute x), else 0
 };
 
-template <int RV, int ORD>
-__device__ __forceinline__ const double4 &entry(const RowBuf<RV, ORD> &R, int byte_off)
+template <int RV, int ORD, typename R>
+__device__ __forceinline__ const typename Vec<R>::v4 &entry(const RowBuf<RV, ORD, R> &B, int byte_off)
 {
-    return *reinterpret_cast<const double4 *>(reinterpret_cast<const unsigned char *>(&R) + byte_off);
+    return *reinterpret_cast<const typename Vec<R>::v4 *>(reinterpret_cast<const unsigned char *>(&B) + byte_off);
 }
 // order 2: the two stencil coefficients c1, c2 that follow (E, Q, e, cd) in an entry
-template <int RV, int ORD>
-__device__ __forceinline__ const double2 &entry_c(const RowBuf<RV, ORD> &R, int byte_off)
+template <int RV, int ORD, typename R>
+__device__ __forceinline__ const typename Vec<R>::v2 &entry_c(const RowBuf<RV, ORD, R> &B, int byte_off)
 {
-    return *reinterpret_cast<const double2 *>(reinterpret_cast<const unsigned char *>(&R) + byte_off + 32);
+    return *reinterpret_cast<const typename Vec<R>::v2 *>(reinterpret_cast<const unsigned char *>(&B) + byte_off + 4 * sizeof(R));
 }
-template <int RV, int ORD>
-__device__ __forceinline__ const CellRec &record(const RowBuf<RV, ORD> &R, int byte_off)
+template <int RV, int ORD, typename R>
+__device__ __forceinline__ const CellRec &record(const RowBuf<RV, ORD, R> &B, int byte_off)
 {
-    return *reinterpret_cast<const CellRec *>(reinterpret_cast<const unsigned char *>(&R) + byte_off);
+    return *reinterpret_cast<const CellRec *>(reinterpret_cast<const unsigned char *>(&B) + byte_off);
 }
+// 1/tau of a cell in the carried type (the record holds it in both)
+__device__ __forceinline__ void rec_nu(const CellRec &r, double &nu) { nu = r.nu; }
+__device__ __forceinline__ void rec_nu(const CellRec &r, float &nu) { nu = r.nu32; }
 
 // stage 2 for a pair of cells (A, B; roA, roB: their records) of a row and the REDs of its results (lanes 0..15: cell A,
 // 16..31: cell B).
 // No predicates and no branches (the row stays one basic block): a result the sums do not need is multiplied by 0 and
 // added to a slot no other lane of the instruction targets; dead cells have g = 0 and name a row of their own or, in
 // the padding, of the nearest cell of the grid.
-template <int RV, int ORD>
-__device__ __forceinline__ void emit_pair(const RowBuf<RV, ORD> &R, const int roA, const int roB, const double a0, const double a1,
-                                          const double b0, const double b1, const ThreadCtx<RV, ORD> &T, const int lane)
+template <int RV, int ORD, typename R>
+__device__ __forceinline__ void emit_pair(const RowBuf<RV, ORD, R> &Rw, const int roA, const int roB, const double a0, const double a1,
+                                          const double b0, const double b1, const ThreadCtx<RV, ORD, R> &T, const int lane)
 {
     const bool hi = lane & 16;
     double d0 = 0.0, d1 = 0.0;
     dmma(d0, d1, hi ? b0 : a0, T.yz0);
     dmma(d0, d1, hi ? b1 : a1, T.yz1);
-    const long long c = record<RV, ORD>(R, hi ? roB : roA).cidx;
+    const long long c = record<RV, ORD, R>(Rw, hi ? roB : roA).cidx;
     red_f64(T.raw0 + c * 16, d0 * T.use0);
     red_f64(T.raw1 + c * 16, d1 * T.use1);
 }
@@ -481,66 +538,77 @@ __device__ __forceinline__ void emit_pair(const RowBuf<RV, ORD> &R, const int ro
 // table entries carry the stencil coefficients (cd, c1, c2) per direction, so the cell value is
 // g = [src + sum_d (c1_d g_1d + c2_d g_2d)] / (nu + sum_d cd_d); the recurrence along x is still one DFMA per value
 // (the c2 term uses the value two cells back, known a cell earlier).  YL: y-face layer this row's values go to (-1: none).
-template <int RV, int ORD, int AX, int YL>
-__device__ __forceinline__ void compute_row(const RowBuf<RV, ORD> &R, const double *xin, const double *xin2, double (&zrow)[4][RV],
-                                            double (&z2row)[4][RV], const double (&yup)[4][RV], const double (&yup2)[4][RV],
-                                            const ThreadCtx<RV, ORD> &T, const int tid, const int lane, double *xout, const bool wx,
-                                            double *yout, const bool wy)
+template <int RV, int ORD, int AX, int YL, typename R>
+__device__ __forceinline__ void compute_row(const RowBuf<RV, ORD, R> &Rw, const R *xin, const R *xin2, R (&zrow)[4][RV],
+                                            R (&z2row)[4][RV], const R (&yup)[4][RV], const R (&yup2)[4][RV],
+                                            const ThreadCtx<RV, ORD, R> &T, const int tid, const int lane, R *xout, const bool wx,
+                                            R *yout, const bool wy)
 {
-    constexpr int NVB = KC<RV, ORD>::NVB, ES = KC<RV, ORD>::ES;
-    double fx[RV], fx2[RV];
-    load_face<RV, ORD>(xin, tid, fx);
-    if (ORD == 2) load_face<RV, ORD>(xin2, tid, fx2);
+    using V4 = typename Vec<R>::v4;
+    using V2 = typename Vec<R>::v2;
+    constexpr int NVB = KC<RV, ORD, R>::NVB, ES = KC<RV, ORD, R>::ES;
+    constexpr R ONE = (R)1, ZERO = (R)0;
+    R fx[RV], fx2[RV];
+    load_face<RV, ORD, R>(xin, tid, fx);
+    if (ORD == 2) load_face<RV, ORD, R>(xin2, tid, fx2);
     double acc[2][2];
 #pragma unroll
     for (int ii = 0; ii < 4; ++ii) {
-        const double4 yt = entry<RV, ORD>(R, T.yo[ii]);
-        const double4 zt = entry<RV, ORD>(R, T.zo[ii]);
-        const double Eyz = yt.x * zt.x, Qyz = yt.y + zt.y, eyz = yt.z + zt.z;
-        const double dyz = (yt.w + zt.w) + record<RV, ORD>(R, T.ro[ii]).nu;
+        const V4 yt = entry<RV, ORD, R>(Rw, T.yo[ii]);
+        const V4 zt = entry<RV, ORD, R>(Rw, T.zo[ii]);
+        R nu;
+        rec_nu(record<RV, ORD, R>(Rw, T.ro[ii]), nu);
+        const R Eyz = yt.x * zt.x, Qyz = yt.y + zt.y, eyz = yt.z + zt.z;
+        const R dyz = (yt.w + zt.w) + nu;
         // stencil coefficients of the entries of the roles B and C (one per cell) - and, below, A (one per node)
-        double c1B = yt.w, c1C = zt.w, c2B = 0.0, c2C = 0.0;
+        R c1B = yt.w, c1C = zt.w, c2B = ZERO, c2C = ZERO;
         if (ORD == 2) {
-            const double2 yc = entry_c<RV, ORD>(R, T.yo[ii]), zc = entry_c<RV, ORD>(R, T.zo[ii]);
+            const V2 yc = entry_c<RV, ORD, R>(Rw, T.yo[ii]), zc = entry_c<RV, ORD, R>(Rw, T.zo[ii]);
             c1B = yc.x; c2B = yc.y; c1C = zc.x; c2C = zc.y;
         }
         // Everything that does not depend on the x-upwind value, for the RV nodes of the thread in lock step (the fp64
         // pipe takes a warp instruction every 2 clocks and has a latency of ~10): the cell value is g = W g_xup + V with
         // W = a_x / den and V = (a_y g_yup + a_z g_zup + src) / den, Eq.(7) PAPER.md:75-79.
-        double4 xt[RV];
-        double2 xc[RV];
-        double t1[RV], t2[RV], d[RV], y0[RV], sE[RV], e[RV], W[RV], V[RV];
+        V4 xt[RV];
+        V2 xc[RV];
+        R t1[RV], t2[RV], d[RV], y0[RV], sE[RV], e[RV], W[RV], V[RV];
 #pragma unroll
-        for (int r = 0; r < RV; ++r) xt[r] = entry<RV, ORD>(R, T.xo[ii] + r * GA * ES);
+        for (int r = 0; r < RV; ++r) xt[r] = entry<RV, ORD, R>(Rw, T.xo[ii] + r * GA * ES);
         if (ORD == 2) {
 #pragma unroll
-            for (int r = 0; r < RV; ++r) xc[r] = entry_c<RV, ORD>(R, T.xo[ii] + r * GA * ES);
+            for (int r = 0; r < RV; ++r) xc[r] = entry_c<RV, ORD, R>(Rw, T.xo[ii] + r * GA * ES);
         }
 #pragma unroll
         for (int r = 0; r < RV; ++r) d[r] = xt[r].w + dyz;
 #pragma unroll
         for (int r = 0; r < RV; ++r) t1[r] = xt[r].y + Qyz;
 #pragma unroll
-        for (int r = 0; r < RV; ++r) asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y0[r]) : "d"(d[r]));
+        for (int r = 0; r < RV; ++r) y0[r] = rcp_seed(d[r]);
 #pragma unroll
         for (int r = 0; r < RV; ++r) t2[r] = xt[r].z + eyz;
 #pragma unroll
         for (int r = 0; r < RV; ++r) sE[r] = xt[r].x * Eyz;
+        if (sizeof(R) == 8) {
 #pragma unroll
-        for (int r = 0; r < RV; ++r) e[r] = fma(-d[r], y0[r], 1.0);
+            for (int r = 0; r < RV; ++r) e[r] = fma(-d[r], y0[r], ONE);
+        }
 #pragma unroll
-        for (int r = 0; r < RV; ++r) t1[r] = fma(t1[r], t2[r], 1.0);
+        for (int r = 0; r < RV; ++r) t1[r] = fma(t1[r], t2[r], ONE);
+        if (sizeof(R) == 8) {
 #pragma unroll
-        for (int r = 0; r < RV; ++r) e[r] = fma(e[r], e[r], e[r]);
+            for (int r = 0; r < RV; ++r) e[r] = fma(e[r], e[r], e[r]);
+        }
 #pragma unroll
         for (int r = 0; r < RV; ++r) V[r] = sE[r] * t1[r];
+        if (sizeof(R) == 8) {
 #pragma unroll
-        for (int r = 0; r < RV; ++r) y0[r] = fma(y0[r], e[r], y0[r]);       // 1 / den (MUFU seed + cubic Newton step)
+            for (int r = 0; r < RV; ++r) y0[r] = fma(y0[r], e[r], y0[r]);   // 1 / den (MUFU seed + cubic Newton step; single: the seed is exact to 1 ulp)
+        }
         // The entry of role A belongs to velocity axis AX, B and C to the other two in ascending order; the coefficient of the
         // x- / y- / z-upwind value is the one of the entry that holds xi_x / xi_y / xi_z (compile-time selection).
-        double c1A[RV], c2A[RV];
+        R c1A[RV], c2A[RV];
 #pragma unroll
-        for (int r = 0; r < RV; ++r) { c1A[r] = ORD == 2 ? xc[r].x : xt[r].w; c2A[r] = ORD == 2 ? xc[r].y : 0.0; }
+        for (int r = 0; r < RV; ++r) { c1A[r] = ORD == 2 ? xc[r].x : xt[r].w; c2A[r] = ORD == 2 ? xc[r].y : ZERO; }
 #pragma unroll
         for (int r = 0; r < RV; ++r) V[r] = fma(AX == 0 ? c1B : AX == 1 ? c1A[r] : c1C, yup[ii][r], V[r]);
         if (ORD == 2) {
@@ -559,23 +627,24 @@ __device__ __forceinline__ void compute_row(const RowBuf<RV, ORD> &R, const doub
         }
 #pragma unroll
         for (int r = 0; r < RV; ++r) V[r] *= y0[r];
-        // the recurrence along x: one DFMA per value
+        // the recurrence along x: one FMA per value
 #pragma unroll
         for (int r = 0; r < RV; ++r) {
-            const double gg = fma(W[r], fx[r], V[r]);
+            const R gg = fma(W[r], fx[r], V[r]);
             if (ORD == 2) { fx2[r] = fx[r]; z2row[ii][r] = zrow[ii][r]; }
             fx[r] = gg;
             zrow[ii][r] = gg;
         }
+        // velocity sums: always in double (a single value is widened exactly)
         acc[ii & 1][0] = 0.0; acc[ii & 1][1] = 0.0;
 #pragma unroll
-        for (int r = 0; r < RV; ++r) dmma(acc[ii & 1][0], acc[ii & 1][1], T.aX[r], zrow[ii][r]);
-        if (ii & 1) emit_pair<RV, ORD>(R, T.ro[ii - 1], T.ro[ii], acc[0][0], acc[0][1], acc[1][0], acc[1][1], T, lane);
-        if (YL >= 0 && wy) store_face<RV, ORD>(yout + (YL * TILE_TX + ii) * NVB, tid, zrow[ii]);
+        for (int r = 0; r < RV; ++r) dmma(acc[ii & 1][0], acc[ii & 1][1], T.aX[r], (double)zrow[ii][r]);
+        if (ii & 1) emit_pair<RV, ORD, R>(Rw, T.ro[ii - 1], T.ro[ii], acc[0][0], acc[0][1], acc[1][0], acc[1][1], T, lane);
+        if (YL >= 0 && wy) store_face<RV, ORD, R>(yout + (YL * TILE_TX + ii) * NVB, tid, zrow[ii]);
     }
     if (wx) {
-        store_face<RV, ORD>(xout, tid, fx);
-        if (ORD == 2) store_face<RV, ORD>(xout + TILE_TY * NVB, tid, fx2);
+        store_face<RV, ORD, R>(xout, tid, fx);
+        if (ORD == 2) store_face<RV, ORD, R>(xout + TILE_TY * NVB, tid, fx2);
     }
 }
 
@@ -584,37 +653,37 @@ __device__ __forceinline__ void compute_row(const RowBuf<RV, ORD> &R, const doub
 // the row before.  The B200 instruction cache holds 32 KB, and a level loop larger than that is fetch-bound at 1/3
 // instruction per clock and scheduler (profiles/r01_ifetch_microbench.txt): the instructions a level executes on
 // this path (about 1900 for RV = 4) stay below that; rolled variants with rotating row slots were slower (profiles/).
-template <int RV, int ORD, int AX>
-__device__ __forceinline__ void compute_level(const LevelBuf<RV, ORD> &L, double (&pl)[TILE_TY][4][RV], double (&pl2)[ORD == 2 ? TILE_TY : 1][4][RV],
-                                              const ThreadCtx<RV, ORD> &T, const int tid, const int lane, double *xout, const bool wx,
-                                              double *yout, const bool wy)
+template <int RV, int ORD, int AX, typename R>
+__device__ __forceinline__ void compute_level(const LevelBuf<RV, ORD, R> &L, R (&pl)[TILE_TY][4][RV], R (&pl2)[ORD == 2 ? TILE_TY : 1][4][RV],
+                                              const ThreadCtx<RV, ORD, R> &T, const int tid, const int lane, R *xout, const bool wx,
+                                              R *yout, const bool wy)
 {
-    constexpr int NVB = KC<RV, ORD>::NVB, L2 = ORD - 1;
+    constexpr int NVB = KC<RV, ORD, R>::NVB, L2 = ORD - 1;
     static_assert(TILE_TY >= 2 || ORD == 1, "the second-order tile kernel needs at least two rows per tile");
-    double yu[4][RV], yu2[4][RV];
+    R yu[4][RV], yu2[4][RV];
 #pragma unroll
-    for (int ii = 0; ii < 4; ++ii) load_face<RV, ORD>(&L.yface[0][ii][0], tid, yu[ii]);
+    for (int ii = 0; ii < 4; ++ii) load_face<RV, ORD, R>(&L.yface[0][ii][0], tid, yu[ii]);
     if (ORD == 2) {
 #pragma unroll
-        for (int ii = 0; ii < 4; ++ii) load_face<RV, ORD>(&L.yface[L2][ii][0], tid, yu2[ii]);
+        for (int ii = 0; ii < 4; ++ii) load_face<RV, ORD, R>(&L.yface[L2][ii][0], tid, yu2[ii]);
     }
     // y-face layer a row's values go to: the last row -> layer 0, the one before (order 2) -> layer 1
     if (TILE_TY == 1) {
-        compute_row<RV, ORD, AX, 0>(L.row[0], L.xface[0][0], L.xface[L2][0], pl[0], pl2[0], yu, yu2, T, tid, lane, xout, wx, yout, wy);
+        compute_row<RV, ORD, AX, 0, R>(L.row[0], L.xface[0][0], L.xface[L2][0], pl[0], pl2[0], yu, yu2, T, tid, lane, xout, wx, yout, wy);
     } else {
-        compute_row<RV, ORD, AX, (ORD == 2 && TILE_TY == 2) ? 1 : -1>(L.row[0], L.xface[0][0], L.xface[L2][0], pl[0], pl2[0], yu, yu2, T, tid, lane,
+        compute_row<RV, ORD, AX, (ORD == 2 && TILE_TY == 2) ? 1 : -1, R>(L.row[0], L.xface[0][0], L.xface[L2][0], pl[0], pl2[0], yu, yu2, T, tid, lane,
                                                                 xout, wx, yout, wy);
 #pragma unroll
         for (int jj = 1; jj < TILE_TY - 1; ++jj) {
             if (ORD == 2 && jj == TILE_TY - 2)
-                compute_row<RV, ORD, AX, 1>(L.row[jj], L.xface[0][jj], L.xface[L2][jj], pl[jj], pl2[ORD == 2 ? jj : 0], pl[jj - 1], jj >= 2 ? pl[jj >= 2 ? jj - 2 : 0] : yu,
+                compute_row<RV, ORD, AX, 1, R>(L.row[jj], L.xface[0][jj], L.xface[L2][jj], pl[jj], pl2[ORD == 2 ? jj : 0], pl[jj - 1], jj >= 2 ? pl[jj >= 2 ? jj - 2 : 0] : yu,
                                         T, tid, lane, xout + jj * NVB, wx, yout, wy);
             else
-                compute_row<RV, ORD, AX, -1>(L.row[jj], L.xface[0][jj], L.xface[L2][jj], pl[jj], pl2[ORD == 2 ? jj : 0], pl[jj - 1], jj >= 2 ? pl[jj >= 2 ? jj - 2 : 0] : yu,
+                compute_row<RV, ORD, AX, -1, R>(L.row[jj], L.xface[0][jj], L.xface[L2][jj], pl[jj], pl2[ORD == 2 ? jj : 0], pl[jj - 1], jj >= 2 ? pl[jj >= 2 ? jj - 2 : 0] : yu,
                                          T, tid, lane, xout + jj * NVB, wx, yout, wy);
         }
         constexpr int J = TILE_TY - 1;
-        compute_row<RV, ORD, AX, 0>(L.row[J], L.xface[0][J], L.xface[L2][J], pl[J], pl2[ORD == 2 ? J : 0], pl[J - 1], J >= 2 ? pl[J >= 2 ? J - 2 : 0] : yu, T, tid, lane,
+        compute_row<RV, ORD, AX, 0, R>(L.row[J], L.xface[0][J], L.xface[L2][J], pl[J], pl2[ORD == 2 ? J : 0], pl[J - 1], J >= 2 ? pl[J >= 2 ? J - 2 : 0] : yu, T, tid, lane,
                                 xout + J * NVB, wx, yout, wy);
     }
 }
@@ -623,20 +692,23 @@ __device__ __forceinline__ void compute_level(const LevelBuf<RV, ORD> &L, double
 // written as compact loops over a copy of the plane(s) in local memory.  Rare (the surface of a masked body), so its
 // speed does not matter; keeping it out of the unrolled path halves the code the instruction cache has to hold.
 // A solid ghost replaces the first upwind value; the coefficient of the second one is 0 there (tables.cu).
-template <int RV, int ORD, int AX>
-__device__ __forceinline__ void compute_level_slow(TileSmem<RV, ORD> &s, const LevelBuf<RV, ORD> &L, double *pl, double *pl2,
-                                                   const ThreadCtx<RV, ORD> &T, const int tid, const int lane, double *xout, double *yout)
+template <int RV, int ORD, int AX, typename R>
+__device__ __forceinline__ void compute_level_slow(TileSmem<RV, ORD, R> &s, const LevelBuf<RV, ORD, R> &L, R *pl, R *pl2,
+                                                   const ThreadCtx<RV, ORD, R> &T, const int tid, const int lane, R *xout, R *yout)
 {
-    constexpr int NVB = KC<RV, ORD>::NVB, ES = KC<RV, ORD>::ES, L2 = ORD - 1;
+    using V4 = typename Vec<R>::v4;
+    using V2 = typename Vec<R>::v2;
+    constexpr int NVB = KC<RV, ORD, R>::NVB, ES = KC<RV, ORD, R>::ES, L2 = ORD - 1;
+    constexpr R ONE = (R)1, ZERO = (R)0;
     const double gyz = s.g[3][1][T.yi] * s.g[3][2][T.zi];
 #pragma unroll 1
     for (int jj = 0; jj < TILE_TY; ++jj) {
-        const RowBuf<RV, ORD> &R = L.row[jj];
-        double fx[RV], fx2[RV];
+        const RowBuf<RV, ORD, R> &Rw = L.row[jj];
+        R fx[RV], fx2[RV];
 #pragma unroll
         for (int r = 0; r < RV; ++r) {
-            fx[r] = L.xface[0][jj][face_index<RV, ORD>(tid, r)];
-            fx2[r] = ORD == 2 ? L.xface[L2][jj][face_index<RV, ORD>(tid, r)] : 0.0;
+            fx[r] = L.xface[0][jj][face_index<RV, ORD, R>(tid, r)];
+            fx2[r] = ORD == 2 ? L.xface[L2][jj][face_index<RV, ORD, R>(tid, r)] : ZERO;
         }
         double accA0 = 0.0, accA1 = 0.0;
         int roPrev = 0;
@@ -646,41 +718,43 @@ __device__ __forceinline__ void compute_level_slow(TileSmem<RV, ORD> &s, const L
             const int xo = ii == 0 ? T.xo[0] : ii == 1 ? T.xo[1] : ii == 2 ? T.xo[2] : T.xo[3];
             const int yo = ii == 0 ? T.yo[0] : ii == 1 ? T.yo[1] : ii == 2 ? T.yo[2] : T.yo[3];
             const int zo = ii == 0 ? T.zo[0] : ii == 1 ? T.zo[1] : ii == 2 ? T.zo[2] : T.zo[3];
-            const double4 yt = entry<RV, ORD>(R, yo);
-            const double4 zt = entry<RV, ORD>(R, zo);
-            const double Eyz = yt.x * zt.x, Qyz = yt.y + zt.y, eyz = yt.z + zt.z;
-            double c1B = yt.w, c1C = zt.w, c2B = 0.0, c2C = 0.0;
+            const V4 yt = entry<RV, ORD, R>(Rw, yo);
+            const V4 zt = entry<RV, ORD, R>(Rw, zo);
+            const R Eyz = yt.x * zt.x, Qyz = yt.y + zt.y, eyz = yt.z + zt.z;
+            R c1B = yt.w, c1C = zt.w, c2B = ZERO, c2C = ZERO;
             if (ORD == 2) {
-                const double2 yc = entry_c<RV, ORD>(R, yo), zc = entry_c<RV, ORD>(R, zo);
+                const V2 yc = entry_c<RV, ORD, R>(Rw, yo), zc = entry_c<RV, ORD, R>(Rw, zo);
                 c1B = yc.x; c2B = yc.y; c1C = zc.x; c2C = zc.y;
             }
             const int ro = ii == 0 ? T.ro[0] : ii == 1 ? T.ro[1] : ii == 2 ? T.ro[2] : T.ro[3];
-            const double dyz = (yt.w + zt.w) + record<RV, ORD>(R, ro).nu;
-            const int code = R.code[ii];
-            const double4 sp = R.spec[ii];
+            R nu;
+            rec_nu(record<RV, ORD, R>(Rw, ro), nu);
+            const R dyz = (yt.w + zt.w) + nu;
+            const int code = Rw.code[ii];
+            const double4 sp = Rw.spec[ii];
             double c0 = 0.0, c1 = 0.0;
 #pragma unroll
             for (int r = 0; r < RV; ++r) {
                 const double Pg = s.g[3][0][RV * T.ag + r] * gyz;
-                const double4 xt = entry<RV, ORD>(R, xo + r * GA * ES);
-                double c1A = xt.w, c2A = 0.0;
-                if (ORD == 2) { const double2 xc = entry_c<RV, ORD>(R, xo + r * GA * ES); c1A = xc.x; c2A = xc.y; }
-                const double c1x = AX == 0 ? c1A : c1B, c1y = AX == 0 ? c1B : AX == 1 ? c1A : c1C, c1z = AX == 2 ? c1A : c1C;
-                const double c2x = AX == 0 ? c2A : c2B, c2y = AX == 0 ? c2B : AX == 1 ? c2A : c2C, c2z = AX == 2 ? c2A : c2C;
-                double xu = fx[r], zu = pl[cell * RV + r];
-                double yu = jj == 0 ? L.yface[0][ii][face_index<RV, ORD>(tid, r)] : pl[(cell - 4) * RV + r];
-                double xu2 = fx2[r], zu2 = 0.0, yu2 = 0.0;
+                const V4 xt = entry<RV, ORD, R>(Rw, xo + r * GA * ES);
+                R c1A = xt.w, c2A = ZERO;
+                if (ORD == 2) { const V2 xc = entry_c<RV, ORD, R>(Rw, xo + r * GA * ES); c1A = xc.x; c2A = xc.y; }
+                const R c1x = AX == 0 ? c1A : c1B, c1y = AX == 0 ? c1B : AX == 1 ? c1A : c1C, c1z = AX == 2 ? c1A : c1C;
+                const R c2x = AX == 0 ? c2A : c2B, c2y = AX == 0 ? c2B : AX == 1 ? c2A : c2C, c2z = AX == 2 ? c2A : c2C;
+                R xu = fx[r], zu = pl[cell * RV + r];
+                R yu = jj == 0 ? L.yface[0][ii][face_index<RV, ORD, R>(tid, r)] : pl[(cell - 4) * RV + r];
+                R xu2 = fx2[r], zu2 = ZERO, yu2 = ZERO;
                 if (ORD == 2) {
                     zu2 = pl2[cell * RV + r];
-                    yu2 = jj == 0 ? L.yface[L2][ii][face_index<RV, ORD>(tid, r)]
-                        : jj == 1 ? L.yface[0][ii][face_index<RV, ORD>(tid, r)] : pl[(cell - 8) * RV + r];
+                    yu2 = jj == 0 ? L.yface[L2][ii][face_index<RV, ORD, R>(tid, r)]
+                        : jj == 1 ? L.yface[0][ii][face_index<RV, ORD, R>(tid, r)] : pl[(cell - 8) * RV + r];
                 }
-                if (code & 1) xu = sp.x * Pg;
-                if (code & 2) yu = sp.y * Pg;
-                if (code & 4) zu = sp.z * Pg;
-                const double src = (xt.x * Eyz) * fma(xt.y + Qyz, xt.z + eyz, 1.0);
-                const double inv = fast_rcp(xt.w + dyz);
-                double num = fma(c1y, yu, src);
+                if (code & 1) xu = (R)(sp.x * Pg);
+                if (code & 2) yu = (R)(sp.y * Pg);
+                if (code & 4) zu = (R)(sp.z * Pg);
+                const R src = (xt.x * Eyz) * fma(xt.y + Qyz, xt.z + eyz, ONE);
+                const R inv = fast_rcp(xt.w + dyz);
+                R num = fma(c1y, yu, src);
                 num = fma(c1z, zu, num);
                 num = fma(c1x, xu, num);
                 if (ORD == 2) {
@@ -688,16 +762,16 @@ __device__ __forceinline__ void compute_level_slow(TileSmem<RV, ORD> &s, const L
                     num = fma(c2z, zu2, num);
                     num = fma(c2x, xu2, num);
                 }
-                double gg = num * inv;
-                if (code & 8) gg = 0.0;
+                R gg = num * inv;
+                if (code & 8) gg = ZERO;
                 fx2[r] = fx[r];
                 fx[r] = gg;
                 if (ORD == 2) pl2[cell * RV + r] = pl[cell * RV + r];
                 pl[cell * RV + r] = gg;
-                dmma(c0, c1, T.aX[r], gg);
+                dmma(c0, c1, T.aX[r], (double)gg);
             }
             if (ii & 1) {
-                emit_pair<RV, ORD>(R, roPrev, ro, accA0, accA1, c0, c1, T, lane);
+                emit_pair<RV, ORD, R>(Rw, roPrev, ro, accA0, accA1, c0, c1, T, lane);
             } else {
                 accA0 = c0; accA1 = c1;
             }
@@ -706,8 +780,8 @@ __device__ __forceinline__ void compute_level_slow(TileSmem<RV, ORD> &s, const L
         if (xout) {
 #pragma unroll
             for (int r = 0; r < RV; ++r) {
-                xout[jj * NVB + face_index<RV, ORD>(tid, r)] = fx[r];
-                if (ORD == 2) xout[(TILE_TY + jj) * NVB + face_index<RV, ORD>(tid, r)] = fx2[r];
+                xout[jj * NVB + face_index<RV, ORD, R>(tid, r)] = fx[r];
+                if (ORD == 2) xout[(TILE_TY + jj) * NVB + face_index<RV, ORD, R>(tid, r)] = fx2[r];
             }
         }
     }
@@ -716,18 +790,18 @@ __device__ __forceinline__ void compute_level_slow(TileSmem<RV, ORD> &s, const L
         for (int ii = 0; ii < 4; ++ii)
 #pragma unroll
             for (int r = 0; r < RV; ++r) {
-                yout[ii * NVB + face_index<RV, ORD>(tid, r)] = pl[((TILE_TY - 1) * 4 + ii) * RV + r];
-                if (ORD == 2) yout[(TILE_TX + ii) * NVB + face_index<RV, ORD>(tid, r)] = pl[((TILE_TY >= 2 ? TILE_TY - 2 : 0) * 4 + ii) * RV + r];
+                yout[ii * NVB + face_index<RV, ORD, R>(tid, r)] = pl[((TILE_TY - 1) * 4 + ii) * RV + r];
+                if (ORD == 2) yout[(TILE_TX + ii) * NVB + face_index<RV, ORD, R>(tid, r)] = pl[((TILE_TY >= 2 ? TILE_TY - 2 : 0) * 4 + ii) * RV + r];
             }
     }
 }
 
-template <int RV, int ORD, int AX>
-__global__ void __launch_bounds__(KC<RV, ORD>::THREADS, 2) sweep_tile_kernel(const TileParams P)
+template <int RV, int ORD, int AX, typename R>
+__global__ void __launch_bounds__(KC<RV, ORD, R>::THREADS, KC<RV, ORD, R>::MIN_CTAS) sweep_tile_kernel(const TileParams P)
 {
-    constexpr int NA = GA * RV, THREADS = KC<RV, ORD>::THREADS, XLEVEL_DOUBLES = KC<RV, ORD>::XLEVEL_DOUBLES, YLEVEL_DOUBLES = KC<RV, ORD>::YLEVEL_DOUBLES;
+    constexpr int NA = GA * RV, THREADS = KC<RV, ORD, R>::THREADS, XLEVEL_VALUES = KC<RV, ORD, R>::XLEVEL_VALUES, YLEVEL_VALUES = KC<RV, ORD, R>::YLEVEL_VALUES;
     (void)THREADS;
-    using RB = RowBuf<RV, ORD>;
+    using RB = RowBuf<RV, ORD, R>;
     // velocity axis in the role A (AX), B, C and their node arrays
     constexpr int AXB = AX == 0 ? 1 : 0, AXC = AX == 2 ? 1 : 2;
     const double *xiA = AX == 0 ? P.xi_x : AX == 1 ? P.xi_y : P.xi_z;
@@ -735,7 +809,7 @@ __global__ void __launch_bounds__(KC<RV, ORD>::THREADS, 2) sweep_tile_kernel(con
     // dynamic shared memory starts at offset 0 of the CTA's window (no static __shared__ in this kernel), so the
     // 128-byte alignment holds; casting without pointer arithmetic keeps the address space visible (LDS / STS)
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    TileSmem<RV, ORD> &s = *reinterpret_cast<TileSmem<RV, ORD> *>(smem_raw);
+    TileSmem<RV, ORD, R> &s = *reinterpret_cast<TileSmem<RV, ORD, R> *>(smem_raw);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     if (tid == 0) {
         mbar_init(&s.mbar[0], 1);
@@ -773,16 +847,16 @@ __global__ void __launch_bounds__(KC<RV, ORD>::THREADS, 2) sweep_tile_kernel(con
         I.tpx = P.bc_type[I.upx]; I.tpy = P.bc_type[I.upy]; I.tpz = P.bc_type[I.upz];
         I.first_x = it.ti == 0; I.first_y = it.tj == 0;
         I.nbb = vb.nbb; I.ncb = vb.ncb;
-        double *xdst = P.xface + ((long long)(it.vb % P.batch) * P.P + it.xslot) * P.xslot_doubles;
-        double *ydst = P.yface + ((long long)(it.vb % P.batch) * P.ntx + it.ti) * P.yslot_doubles;
+        R *xdst = static_cast<R *>(P.xface) + ((long long)(it.vb % P.batch) * P.P + it.xslot) * P.xslot_values;
+        R *ydst = static_cast<R *>(P.yface) + ((long long)(it.vb % P.batch) * P.ntx + it.ti) * P.yslot_values;
 
         // ---- TMA copies of levels 0 and 1 (the staging buffers are free: every thread passed the end-of-item
         //      barrier; the upwind items' face stores were made with the generic proxy) ----
-        setup_copies<RV, ORD>(P, I, s, vb, tid, xdst, ydst);
-        if (copy_of_thread<RV, ORD>(tid) < NCOPY) {
+        setup_copies<RV, ORD, R>(P, I, s, vb, tid, xdst, ydst);
+        if (copy_of_thread<RV, ORD, R>(tid) < NCOPY) {
             fence_proxy_async_global();
-            issue_level<RV, ORD>(s, 0, tid);
-            if (P.nz > 1) issue_level<RV, ORD>(s, 1, tid);
+            issue_level<RV, ORD, R>(s, 0, tid);
+            if (P.nz > 1) issue_level<RV, ORD, R>(s, 1, tid);
         }
         // ---- per-item tables: nodes, ghost factors; ghost densities of the domain faces of levels 0 and 1 ----
         {
@@ -809,12 +883,12 @@ __global__ void __launch_bounds__(KC<RV, ORD>::THREADS, 2) sweep_tile_kernel(con
                 for (int f = 0; f < 4; ++f)
                     s.g[f][2][vb.nbb + cl] = ok ? P.gtab[(long long)(slotid[f] * 3 + AXC) * P.gstride + idx] : 0.0;
             }
-            rwb_store<RV, ORD>(s, 0, tid, rwb_load(P, I, 0, tid));
-            rwb_store<RV, ORD>(s, 1, tid, rwb_load(P, I, 1, tid));
+            rwb_store<RV, ORD, R>(s, 0, tid, rwb_load(P, I, 0, tid));
+            rwb_store<RV, ORD, R>(s, 1, tid, rwb_load(P, I, 1, tid));
         }
         __syncthreads();
 
-        ThreadCtx<RV, ORD> T;
+        ThreadCtx<RV, ORD, R> T;
         T.ag = lane & 3;
         T.xrev = vb.sx > 0 ? 0 : 3;
         {
@@ -826,9 +900,9 @@ __global__ void __launch_bounds__(KC<RV, ORD>::THREADS, 2) sweep_tile_kernel(con
 #pragma unroll
             for (int ii = 0; ii < 4; ++ii) {
                 const int cp = ii ^ T.xrev;
-                T.xo[ii] = (int)offsetof(RB, xtab) + (cp * NA + T.ag) * KC<RV, ORD>::ES;
-                T.yo[ii] = (int)offsetof(RB, ytab) + (cp * vb.nbb + yl) * KC<RV, ORD>::ES;
-                T.zo[ii] = (int)offsetof(RB, ztab) + (cp * vb.ncb + zl) * KC<RV, ORD>::ES;
+                T.xo[ii] = (int)offsetof(RB, xtab) + (cp * NA + T.ag) * KC<RV, ORD, R>::ES;
+                T.yo[ii] = (int)offsetof(RB, ytab) + (cp * vb.nbb + yl) * KC<RV, ORD, R>::ES;
+                T.zo[ii] = (int)offsetof(RB, ztab) + (cp * vb.ncb + zl) * KC<RV, ORD, R>::ES;
                 T.ro[ii] = (int)offsetof(RB, rec) + cp * (int)sizeof(CellRec);
             }
             // stage-1 A fragments: xi_x^p of the thread's own nodes, p = (lane >> 2) & 3
@@ -879,18 +953,18 @@ __global__ void __launch_bounds__(KC<RV, ORD>::THREADS, 2) sweep_tile_kernel(con
         if (tid < NCELL) {
             mbar_wait(&s.mbar[0], par[0]);
             par[0] ^= 1u;
-            detect_special<RV, ORD>(I, s, 0, lane);
+            detect_special<RV, ORD, R>(I, s, 0, lane);
         }
-        fill_faces<RV, ORD>(I, s, 0, tid, T.ag, T.yi, T.zi);
+        fill_faces<RV, ORD, R>(I, s, 0, tid, T.ag, T.yi, T.zi);
         // plane = ghost of the upwind z face of the domain (order 2: the plane before it is never used, its coefficient
         // is 0 in the first level; it must only be finite)
-        double pl[TILE_TY][4][RV], pl2[ORD == 2 ? TILE_TY : 1][4][RV];
+        R pl[TILE_TY][4][RV], pl2[ORD == 2 ? TILE_TY : 1][4][RV];
 #pragma unroll
         for (int jj = 0; jj < (ORD == 2 ? TILE_TY : 1); ++jj)
 #pragma unroll
             for (int ii = 0; ii < 4; ++ii)
 #pragma unroll
-                for (int r = 0; r < RV; ++r) pl2[jj][ii][r] = 0.0;
+                for (int r = 0; r < RV; ++r) pl2[jj][ii][r] = (R)0;
         {
             const double gyz = s.g[2][1][T.yi] * s.g[2][2][T.zi];
             double G[RV];
@@ -904,7 +978,7 @@ __global__ void __launch_bounds__(KC<RV, ORD>::THREADS, 2) sweep_tile_kernel(con
                     double rw = 0.0;
                     if (cell_of(P, I, ii, jj, 0, i, j, k)) rw = face_density(P, I.tpz, P.foff[I.upz] + j * P.nx + i);
 #pragma unroll
-                    for (int r = 0; r < RV; ++r) pl[jj][ii][r] = rw * G[r];
+                    for (int r = 0; r < RV; ++r) pl[jj][ii][r] = (R)(rw * G[r]);
                 }
         }
         __syncthreads();
@@ -918,17 +992,17 @@ __global__ void __launch_bounds__(KC<RV, ORD>::THREADS, 2) sweep_tile_kernel(con
             if (tid < NCELL && kp + 1 < P.nz) {
                 mbar_wait(&s.mbar[b ^ 1], par[b ^ 1]);
                 par[b ^ 1] ^= 1u;
-                detect_special<RV, ORD>(I, s, b ^ 1, lane);
+                detect_special<RV, ORD, R>(I, s, b ^ 1, lane);
             }
             double vrw = 0.0;
             if (edge) vrw = rwb_load(P, I, kp + 2, tid);
             const int special = __shfl_sync(0xffffffffu, s.special[b], 0);
-            double *xout = xdst + (long long)kp * XLEVEL_DOUBLES, *yout = ydst + (long long)kp * YLEVEL_DOUBLES;
+            R *xout = xdst + (long long)kp * XLEVEL_VALUES, *yout = ydst + (long long)kp * YLEVEL_VALUES;
             if (special) {
                 // every thread of the CTA takes this branch together
-                decode_records<RV, ORD>(P, I, s, b, tid);
+                decode_records<RV, ORD, R>(P, I, s, b, tid);
                 __syncthreads();
-                double tmp[NCELL * RV], tmp2[ORD == 2 ? NCELL * RV : 1];
+                R tmp[NCELL * RV], tmp2[ORD == 2 ? NCELL * RV : 1];
 #pragma unroll
                 for (int c = 0; c < NCELL; ++c)
 #pragma unroll
@@ -936,7 +1010,7 @@ __global__ void __launch_bounds__(KC<RV, ORD>::THREADS, 2) sweep_tile_kernel(con
                         tmp[c * RV + r] = pl[c >> 2][c & 3][r];
                         if (ORD == 2) tmp2[c * RV + r] = pl2[ORD == 2 ? c >> 2 : 0][c & 3][r];
                     }
-                compute_level_slow<RV, ORD, AX>(s, s.lv[b], tmp, tmp2, T, tid, lane, write_x ? xout : nullptr, write_y ? yout : nullptr);
+                compute_level_slow<RV, ORD, AX, R>(s, s.lv[b], tmp, tmp2, T, tid, lane, write_x ? xout : nullptr, write_y ? yout : nullptr);
 #pragma unroll
                 for (int c = 0; c < NCELL; ++c)
 #pragma unroll
@@ -945,16 +1019,16 @@ __global__ void __launch_bounds__(KC<RV, ORD>::THREADS, 2) sweep_tile_kernel(con
                         if (ORD == 2) pl2[ORD == 2 ? c >> 2 : 0][c & 3][r] = tmp2[c * RV + r];
                     }
             } else {
-                compute_level<RV, ORD, AX>(s.lv[b], pl, pl2, T, tid, lane, xout, write_x, yout, write_y);
+                compute_level<RV, ORD, AX, R>(s.lv[b], pl, pl2, T, tid, lane, xout, write_x, yout, write_y);
             }
             if (edge) {
-                rwb_store<RV, ORD>(s, b, tid, vrw);
-                if (kp + 1 < P.nz) fill_faces<RV, ORD>(I, s, b ^ 1, tid, T.ag, T.yi, T.zi);
+                rwb_store<RV, ORD, R>(s, b, tid, vrw);
+                if (kp + 1 < P.nz) fill_faces<RV, ORD, R>(I, s, b ^ 1, tid, T.ag, T.yi, T.zi);
             }
             __syncthreads();
-            if (copy_of_thread<RV, ORD>(tid) < NCOPY && kp + 2 < P.nz) {
+            if (copy_of_thread<RV, ORD, R>(tid) < NCOPY && kp + 2 < P.nz) {
                 fence_proxy_async_smem();  // this level's reads of the staging buffers before the TMA overwrites them
-                issue_level<RV, ORD>(s, kp + 2, tid);
+                issue_level<RV, ORD, R>(s, kp + 2, tid);
             }
         }
         // ---- publish: faces of this item are complete ----
@@ -965,45 +1039,59 @@ __global__ void __launch_bounds__(KC<RV, ORD>::THREADS, 2) sweep_tile_kernel(con
     }
 }
 
-template <int RV, int ORD, int AX>
+template <int RV, int ORD, int AX, typename R>
 cudaError_t configure1(int *ctas_per_sm)
 {
-    cudaError_t e = cudaFuncSetAttribute(sweep_tile_kernel<RV, ORD, AX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(TileSmem<RV, ORD>));
+    cudaError_t e = cudaFuncSetAttribute(sweep_tile_kernel<RV, ORD, AX, R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(TileSmem<RV, ORD, R>));
     if (e != cudaSuccess) return e;
-    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, sweep_tile_kernel<RV, ORD, AX>, KC<RV, ORD>::THREADS, sizeof(TileSmem<RV, ORD>));
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, sweep_tile_kernel<RV, ORD, AX, R>, KC<RV, ORD, R>::THREADS, sizeof(TileSmem<RV, ORD, R>));
 }
-template <int RV, int ORD>
+template <int RV, int ORD, typename R>
 cudaError_t configure(int ax, int *ctas_per_sm)
 {
-    return ax == 1 ? configure1<RV, ORD, 1>(ctas_per_sm) : ax == 2 ? configure1<RV, ORD, 2>(ctas_per_sm) : configure1<RV, ORD, 0>(ctas_per_sm);
+    return ax == 1 ? configure1<RV, ORD, 1, R>(ctas_per_sm) : ax == 2 ? configure1<RV, ORD, 2, R>(ctas_per_sm) : configure1<RV, ORD, 0, R>(ctas_per_sm);
 }
-template <int RV, int ORD>
+template <int RV, int ORD, typename R>
 void launch(const TileParams &P, int ax, int grid, cudaStream_t st)
 {
-    if (ax == 1) sweep_tile_kernel<RV, ORD, 1><<<grid, KC<RV, ORD>::THREADS, sizeof(TileSmem<RV, ORD>), st>>>(P);
-    else if (ax == 2) sweep_tile_kernel<RV, ORD, 2><<<grid, KC<RV, ORD>::THREADS, sizeof(TileSmem<RV, ORD>), st>>>(P);
-    else sweep_tile_kernel<RV, ORD, 0><<<grid, KC<RV, ORD>::THREADS, sizeof(TileSmem<RV, ORD>), st>>>(P);
+    if (ax == 1) sweep_tile_kernel<RV, ORD, 1, R><<<grid, KC<RV, ORD, R>::THREADS, sizeof(TileSmem<RV, ORD, R>), st>>>(P);
+    else if (ax == 2) sweep_tile_kernel<RV, ORD, 2, R><<<grid, KC<RV, ORD, R>::THREADS, sizeof(TileSmem<RV, ORD, R>), st>>>(P);
+    else sweep_tile_kernel<RV, ORD, 0, R><<<grid, KC<RV, ORD, R>::THREADS, sizeof(TileSmem<RV, ORD, R>), st>>>(P);
 }
 
 }  // namespace
 
-size_t tile_smem_bytes(int rv, int order)
+// (rv, order, f32): the variants that exist: double (4 | 3 | 2, 1), (2, 2); single (4 | 3, 1)
+bool tile_variant_exists(int rv, int order, bool f32)
 {
-    return order == 2 ? sizeof(TileSmem<2, 2>) : rv == 2 ? sizeof(TileSmem<2, 1>) : rv == 3 ? sizeof(TileSmem<3, 1>) : sizeof(TileSmem<4, 1>);
+    if (f32) return order == 1 && (rv == 3 || rv == 4);
+    return order == 2 ? rv == 2 : (rv >= 2 && rv <= 4);
 }
 
-cudaError_t tile_configure(int rv, int order, int wide_axis, int *ctas_per_sm)
+size_t tile_smem_bytes(int rv, int order, bool f32)
 {
-    return order == 2 ? configure<2, 2>(wide_axis, ctas_per_sm) : rv == 2 ? configure<2, 1>(wide_axis, ctas_per_sm)
-         : rv == 3 ? configure<3, 1>(wide_axis, ctas_per_sm) : configure<4, 1>(wide_axis, ctas_per_sm);
+    if (f32) return rv == 3 ? sizeof(TileSmem<3, 1, float>) : sizeof(TileSmem<4, 1, float>);
+    return order == 2 ? sizeof(TileSmem<2, 2, double>) : rv == 2 ? sizeof(TileSmem<2, 1, double>) : rv == 3 ? sizeof(TileSmem<3, 1, double>) : sizeof(TileSmem<4, 1, double>);
 }
 
-cudaError_t launch_sweep_tile(const TileParams &P, int rv, int order, int wide_axis, int grid, cudaStream_t st)
+cudaError_t tile_configure(int rv, int order, bool f32, int wide_axis, int *ctas_per_sm)
 {
-    if (order == 2) launch<2, 2>(P, wide_axis, grid, st);
-    else if (rv == 2) launch<2, 1>(P, wide_axis, grid, st);
-    else if (rv == 3) launch<3, 1>(P, wide_axis, grid, st);
-    else launch<4, 1>(P, wide_axis, grid, st);
+    if (!tile_variant_exists(rv, order, f32)) return cudaErrorInvalidValue;
+    if (f32) return rv == 3 ? configure<3, 1, float>(wide_axis, ctas_per_sm) : configure<4, 1, float>(wide_axis, ctas_per_sm);
+    return order == 2 ? configure<2, 2, double>(wide_axis, ctas_per_sm) : rv == 2 ? configure<2, 1, double>(wide_axis, ctas_per_sm)
+         : rv == 3 ? configure<3, 1, double>(wide_axis, ctas_per_sm) : configure<4, 1, double>(wide_axis, ctas_per_sm);
+}
+
+cudaError_t launch_sweep_tile(const TileParams &P, int rv, int order, bool f32, int wide_axis, int grid, cudaStream_t st)
+{
+    if (!tile_variant_exists(rv, order, f32)) return cudaErrorInvalidValue;
+    if (f32) {
+        if (rv == 3) launch<3, 1, float>(P, wide_axis, grid, st);
+        else launch<4, 1, float>(P, wide_axis, grid, st);
+    } else if (order == 2) launch<2, 2, double>(P, wide_axis, grid, st);
+    else if (rv == 2) launch<2, 1, double>(P, wide_axis, grid, st);
+    else if (rv == 3) launch<3, 1, double>(P, wide_axis, grid, st);
+    else launch<4, 1, double>(P, wide_axis, grid, st);
     return cudaGetLastError();
 }
 

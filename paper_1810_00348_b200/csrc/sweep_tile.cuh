@@ -26,6 +26,9 @@ constexpr int TILE_TX = 4;                 // cells per tile along the sweep-rel
 #define DVM_TILE_TY 4
 #endif
 constexpr int TILE_TY = DVM_TILE_TY;        // cells per tile along the sweep-relative y
+#ifndef DVM_TILE_F32_CTAS
+#define DVM_TILE_F32_CTAS 3
+#endif                                      // resident CTAs per SM the single-precision variants are compiled for
 constexpr int TILE_NCELL = TILE_TX * TILE_TY;
 constexpr int TILE_GA = 4;                 // xi_x groups per lane quad
 constexpr int TILE_NVB = 512;              // velocities per block (incl. padding) = threads x RV, first-order kernels
@@ -44,7 +47,7 @@ inline int tile_threads(int rv, int order = 1) { return (order == 2 || rv >= 3) 
 inline int tile_nvb(int rv, int order = 1) { return tile_threads(rv, order) * rv; }   // velocities per block
 inline int tile_na(int rv) { return TILE_GA * rv; }          // xi_x nodes per velocity block
 inline int tile_npair(int rv, int order = 1) { return tile_threads(rv, order) / TILE_GA; }   // (xi_y, xi_z) pairs per block
-inline int tile_entry_doubles(int order) { return order == 2 ? 6 : 4; }   // factor-table entry: (E, Q, e, a) or (E, Q, e, cd, c1, c2)
+inline int tile_entry_values(int order) { return order == 2 ? 6 : 4; }   // factor-table entry: (E, Q, e, a) or (E, Q, e, cd, c1, c2)
 inline int tile_face_layers(int order) { return order == 2 ? 2 : 1; }     // upwind values per direction carried through a face
 
 // per-cell record of the padded grid, fetched by TMA with the factor tables (48 bytes)
@@ -55,7 +58,8 @@ struct CellRec {
                       // in the padding) produces exact zeros and names its own row / that of the nearest cell of the grid
     int flags;        // bits 0..5: neighbour in direction d is not fluid; bits 8..13: it is a solid cell; REC_DEAD
     int face[6];      // boundary-face slot in direction d or -1
-    int pad[2];       // 48 bytes: every row of records starts on a 16-byte boundary (TMA)
+    float nu32;       // nu rounded to single (DVM_PREC_MIXED)
+    int pad;          // 48 bytes: every row of records starts on a 16-byte boundary (TMA)
 };
 static_assert(sizeof(CellRec) == 48, "CellRec rows must be 16-byte aligned");
 
@@ -91,7 +95,7 @@ struct TilePlan {
                                             // xnode is in table order: slot r*4 + ag holds node RV*ag + r of the block
     std::vector<VBlock> vblocks;
     std::vector<TileItem> items;
-    size_t xface_doubles = 0, yface_doubles = 0;
+    size_t xface_values = 0, yface_values = 0;   // values of f the two face workspaces hold (8 or 4 bytes each)
 };
 
 struct TileParams {
@@ -117,16 +121,18 @@ struct TileParams {
     int *done;                    // [nitems] epoch of completion
     int *counter;                 // next item
     int epoch;
-    double *xface, *yface;
-    long long xslot_doubles, yslot_doubles;   // nz * layers * TILE_TY * NVB, nz * layers * TILE_TX * NVB
-    // factor tables of step n (tables_kernel), padded grid nxp x nyp x nz, entries (E, Q, e, a) [order 2: (E, Q, e, cd, c1, c2)]:
-    const double *TX, *TY, *TZ;   // [nxb][nz][nyp][nxp][NA][4 or 6], [nyb][nz][nyp][nxp][nbb][.], [nzb][nz][nyp][nxp][ncb][.]
+    void *xface, *yface;          // double, or float when f is carried in single precision (DVM_PREC_MIXED)
+    long long xslot_values, yslot_values;   // nz * layers * TILE_TY * NVB, nz * layers * TILE_TX * NVB
+    // factor tables of step n (tables_kernel), padded grid nxp x nyp x nz, entries (E, Q, e, a) [order 2: (E, Q, e, cd, c1, c2)],
+    // double or float like the faces:
+    const void *TX, *TY, *TZ;     // [nxb][nz][nyp][nxp][NA][4 or 6], [nyb][nz][nyp][nxp][nbb][.], [nzb][nz][nyp][nxp][ncb][.]
     const CellRec *rec;           // [nz][nyp][nxp]
     int nxp, nyp, nbb, ncb;
 };
 
 struct TableParams {
     int nx, ny, nz, nxp, nyp, na, nbb, ncb, nxb, nyb, nzb, order;
+    int f32;                      // 1: entries are written as float (DVM_PREC_MIXED)
     int ax[3];                    // velocity axis of the tables TX, TY, TZ (roles A, B, C)
     long long ncell;
     const double *coef;           // [NCOEF][ncell]
@@ -136,7 +142,7 @@ struct TableParams {
     const double *xi_x, *xi_y, *xi_z, *w_x, *w_y, *w_z;
     const int *xnode, *ynode, *znode;
     int bc_type[6];
-    double *TX, *TY, *TZ;
+    void *TX, *TY, *TZ;
     CellRec *rec;
 };
 
@@ -147,9 +153,11 @@ struct TableParams {
 int tile_plan(int nx, int ny, int nz, const std::vector<double> xi[3], int target_ctas, int max_blocks, int rv, int order,
               int wide_axis, TilePlan *plan);
 
-size_t tile_smem_bytes(int rv, int order);
-cudaError_t tile_configure(int rv, int order, int wide_axis, int *ctas_per_sm);
-cudaError_t launch_sweep_tile(const TileParams &P, int rv, int order, int wide_axis, int grid, cudaStream_t st);
+// f32: f carried in single precision (DVM_PREC_MIXED; order 1, rv 3 or 4)
+bool tile_variant_exists(int rv, int order, bool f32);
+size_t tile_smem_bytes(int rv, int order, bool f32);
+cudaError_t tile_configure(int rv, int order, bool f32, int wide_axis, int *ctas_per_sm);
+cudaError_t launch_sweep_tile(const TileParams &P, int rv, int order, bool f32, int wide_axis, int grid, cudaStream_t st);
 cudaError_t launch_tables(const TableParams &T, cudaStream_t st);
 
 }  // namespace dvm

@@ -31,7 +31,7 @@ __global__ void __launch_bounds__(256) tables_kernel(const TableParams T)
         const int i = (int)(c % T.nx), j = (int)((c / T.nx) % T.ny), k = (int)(c / ((long long)T.nx * T.ny));
         const long long pc = ((long long)k * T.nyp + (j + TILE_PAD)) * T.nxp + (i + TILE_PAD);
         int role, m, pos, width, blk;
-        double *dst;
+        void *dst;
         if (sl < sx) { role = 0; width = T.na; blk = sl / width; pos = sl - blk * width; m = T.xnode[sl]; dst = T.TX; }
         else if (sl < sx + sy) { role = 1; width = T.nbb; const int t = sl - sx; blk = t / width; pos = t - blk * width; m = T.ynode[t]; dst = T.TY; }
         else { role = 2; width = T.ncb; const int t = sl - sx - sy; blk = t / width; pos = t - blk * width; m = T.znode[t]; dst = T.TZ; }
@@ -74,9 +74,16 @@ __global__ void __launch_bounds__(256) tables_kernel(const TableParams T)
             }
         }
         const int es = T.order == 2 ? 6 : 4;
-        double *o = dst + (((long long)blk * npc + pc) * width + pos) * es;
-        for (int e = 0; e < es; ++e) o[e] = ent[e];
-        if (sl == 0) T.rec[pc].nu = solid ? 1.0 : nu;
+        const long long at = (((long long)blk * npc + pc) * width + pos) * es;
+        if (T.f32) {
+            // DVM_PREC_MIXED: the factors are evaluated in double and rounded once to single
+            float *o = static_cast<float *>(dst) + at;
+            for (int e = 0; e < es; ++e) o[e] = (float)ent[e];
+        } else {
+            double *o = static_cast<double *>(dst) + at;
+            for (int e = 0; e < es; ++e) o[e] = ent[e];
+        }
+        if (sl == 0) { T.rec[pc].nu = solid ? 1.0 : nu; T.rec[pc].nu32 = solid ? 1.0f : (float)nu; }
     }
 }
 

@@ -130,8 +130,8 @@ int tile_plan(int nx, int ny, int nz, const std::vector<double> xi[3], int targe
             }
         }
     }
-    plan->xface_doubles = (size_t)B * P * nz * layers * TILE_TY * NVB;
-    plan->yface_doubles = (size_t)B * ntx * nz * layers * TILE_TX * NVB;
+    plan->xface_values = (size_t)B * P * nz * layers * TILE_TY * NVB;
+    plan->yface_values = (size_t)B * ntx * nz * layers * TILE_TX * NVB;
     return 0;
 }
 

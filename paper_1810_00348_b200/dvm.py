@@ -29,13 +29,15 @@ OPT_TILE_RV = 3
 OPT_MAX_CTAS = 4
 OPT_ORDER = 5
 OPT_TILE_AXIS = 6
+OPT_PRECISION = 7
+PREC_F64, PREC_MIXED = 0, 1
 
 # every symbol include/dvm.h declares (checked by tests/test_abi.py)
 SYMBOLS = (
     "dvm_create", "dvm_iterate", "dvm_moments", "dvm_residual", "dvm_num_faces", "dvm_iterations_done",
     "dvm_get_state", "dvm_set_state", "dvm_raw_moments", "dvm_wall_flux", "dvm_residual_history",
     "dvm_mass_scale", "dvm_step_host", "dvm_set_option", "dvm_workspace_bytes", "dvm_launch_count",
-    "dvm_kernel_used", "dvm_tile_rv", "dvm_tile_axis", "dvm_plan_query", "dvm_plan_vblocks", "dvm_destroy", "dvm_last_error",
+    "dvm_kernel_used", "dvm_tile_rv", "dvm_tile_axis", "dvm_precision", "dvm_plan_query", "dvm_plan_vblocks", "dvm_destroy", "dvm_last_error",
 )
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
@@ -124,6 +126,7 @@ def lib():
         L.dvm_workspace_bytes.argtypes = [vp, C.POINTER(C.c_size_t), C.POINTER(C.c_size_t)]
         L.dvm_kernel_used.argtypes = [vp]
         L.dvm_tile_rv.argtypes = [vp]
+        L.dvm_precision.argtypes = [vp]
         L.dvm_tile_axis.argtypes = [vp]
         L.dvm_plan_query.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(_VGrid), C.c_int, C.c_int, C.c_int, C.c_int, C.c_int,
                                      C.POINTER(C.c_int), C.POINTER(C.c_int), C.c_int]
@@ -174,7 +177,7 @@ class Solver:
     """dvm_create / dvm_iterate / dvm_moments / dvm_residual (+ support calls) for one workload record."""
 
     def __init__(self, wl, kernel: int = KERNEL_AUTO, device: str = "cuda:0", max_f_mbytes: int = 0, tile_rv: int = 0,
-                 max_ctas: int = 0, order: int = 0, tile_axis: int = 0):
+                 max_ctas: int = 0, order: int = 0, tile_axis: int = 0, precision: int = -1):
         import torch
         if not torch.cuda.is_available():
             raise DvmError(ECUDA, "no CUDA device: the DVM solver has no CPU fallback")
@@ -233,6 +236,10 @@ class Solver:
             self.set_option(OPT_MAX_CTAS, int(max_ctas))
         if tile_axis:
             self.set_option(OPT_TILE_AXIS, int(tile_axis))
+        if precision < 0:
+            precision = PREC_MIXED if getattr(wl, "f32", False) else PREC_F64
+        if precision != PREC_F64:
+            self.set_option(OPT_PRECISION, int(precision))
 
     # -- the four calls of the north star ---------------------------------------------------------
     def iterate(self, n: int = 1):
@@ -317,6 +324,9 @@ class Solver:
 
     def tile_axis(self):
         return _check(lib().dvm_tile_axis(self._h))
+
+    def precision(self):
+        return _check(lib().dvm_precision(self._h))
 
     def launch_count(self):
         return int(lib().dvm_launch_count(self._h))
