@@ -208,7 +208,11 @@ def run_gpu(args):
     kernel = {"auto": dvm.KERNEL_AUTO, "slice": dvm.KERNEL_SLICE, "tile": dvm.KERNEL_TILE}[args.kernel]
     s = dvm.Solver(wl, kernel=kernel, device=f"cuda:{local}", max_f_mbytes=args.max_f_mbytes, tile_rv=args.tile_rv,
                    order=args.order, tile_axis=args.tile_axis,
-                   precision=dvm.PREC_MIXED if args.precision == "mixed" else dvm.PREC_F64)
+                   precision=dvm.PREC_MIXED if args.precision == "mixed" else dvm.PREC_F64,
+                   shard=(rank, world) if args.shard else None)
+    # --shard: ONE problem, its velocity blocks spread over the ranks, one NCCL all-reduce of the velocity sums per iteration
+    # (strong scaling).  Default: independent replicas (north_star: no sharding).
+    iterate = (lambda n: s.iterate_sharded(n)) if args.shard else s.iterate
     mixed = args.precision == "mixed"
     stream = torch.cuda.current_stream(dev)
 
@@ -219,7 +223,7 @@ def run_gpu(args):
         torch.cuda.synchronize(dev)
 
     # ---- device-resident timing: W warm-up steps, then exactly K steps ----
-    s.iterate(args.warmup)
+    iterate(args.warmup)
     barrier()
     l0 = s.launch_count()
     sampler = ClockSampler(local)
@@ -228,7 +232,7 @@ def run_gpu(args):
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
     ev[0].record(stream)
     for k in range(args.steps):
-        s.iterate(1)
+        iterate(1)
         ev[k + 1].record(stream)
     barrier()
     clocks = sampler.stop() if rank == 0 else None
@@ -246,11 +250,22 @@ def run_gpu(args):
     p14, rw = s.get_state()
     h_in.copy_(p14[:8].reshape(-1).cpu()); h_rw[: s.nface].copy_(rw.cpu())
     e2e_steps = max(1, min(args.steps, args.e2e_steps))
-    s.step_host(h_in, h_rw, 1, h_out, h_rw_out)  # warm
+
+    def step_host():
+        if not (args.shard and world > 1):
+            return s.step_host(h_in, h_rw, 1, h_out, h_rw_out)
+        # sharded: the same host -> device -> host round trip around the sweep / all-reduce / update of one iteration
+        s.set_state(h_in.view(8, -1).to(dev, non_blocking=True), h_rw[: s.nface].to(dev, non_blocking=True))
+        s.iterate_sharded(1)
+        p14_, rw_ = s.get_state()
+        h_out.copy_(p14_.reshape(-1), non_blocking=True); h_rw_out[: s.nface].copy_(rw_, non_blocking=True)
+        torch.cuda.synchronize(dev)
+
+    step_host()  # warm
     barrier()
     t0 = time.perf_counter()
     for k in range(e2e_steps):
-        s.step_host(h_in, h_rw, 1, h_out, h_rw_out)
+        step_host()
         h_in.copy_(h_out[:n8]); h_rw.copy_(h_rw_out)
     torch.cuda.synchronize(dev)
     e2e_ms = 1e3 * (time.perf_counter() - t0) / e2e_steps
@@ -261,7 +276,7 @@ def run_gpu(args):
     if rank == 0:
         pts = wl.phase_points
         ms_per_step = total_ms / args.steps
-        value = whole_job_value(world, pts, ms_per_step)
+        value = whole_job_value(1 if args.shard else world, pts, ms_per_step)
         kname = "slice" if s.kernel_used() == dvm.KERNEL_SLICE else "tile"
         peak, peak_src, _ = measured_peaks()
         # dominant kernel = the sweep (one launch per step); its duration is the step minus the small table / update launches,
@@ -300,21 +315,22 @@ def run_gpu(args):
                              "highest utilisation is named as the bound"})
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "strong" if args.shard else "weak", "vs_baseline": None,
             "dtype": "f32 sweep, f64 moments" if mixed else "f64", "data": "synthetic",
             "config": {"workload": wl.name, "physical_cells": [wl.nx, wl.ny, wl.nz], "velocity_nodes": [wl.mx, wl.my, wl.mz],
                        "phase_points_per_iteration": pts, "kernel": kname, "precision": args.precision,
                        "tile_rv": s.tile_rv() if kname == "tile" else None,
                        "tile_axis": s.tile_axis() if kname == "tile" else None,
                        "order": args.order, "max_f_mbytes": args.max_f_mbytes,
-                       "parallelism": "replicas only" if world > 1 else "1 GPU",
+                       "parallelism": ("velocity shards x%d, 1 all-reduce / iteration" % world) if args.shard and world > 1
+                       else "replicas only" if world > 1 else "1 GPU",
                        "l2": "inputs larger than L2 (f workspace %.1f GB, fields %.2f GB)" % (f_bytes / 1e9, (total_bytes - f_bytes) / 1e9)
                        if total_bytes > 126e6 else "working set smaller than L2 (config is a parity case)",
                        "workspace_bytes": total_bytes, "f_workspace_bytes": f_bytes,
                        "full_6d_f_bytes_never_allocated": 8 * wl.n_cells * wl.n_vel,
                        "residual_after_run": [float(x) for x in res], "step_ms": [round(x, 3) for x in step_ms]},
             "roofline": roof,
-            "e2e": {"value": whole_job_value(world, pts, e2e_ms), "unit": UNIT,
+            "e2e": {"value": whole_job_value(1 if args.shard else world, pts, e2e_ms), "unit": UNIT,
                     "h2d_bytes_per_step": 8 * (n8 + s.nface), "d2h_bytes_per_step": 8 * (n14 + s.nface)},
             "gpu_launches": int(launches),
             "clocks": clocks,
@@ -342,6 +358,9 @@ def main():
     ap.add_argument("--tile-rv", type=int, default=0, choices=[0, 2, 3, 4], help="velocities per thread of the tile kernel (0 = library's choice)")
     ap.add_argument("--tile-axis", type=int, default=0, choices=[0, 1, 2, 3], help="velocity axis in the wide role of the tile kernel (1 + axis; 0 = library's choice)")
     ap.add_argument("--order", type=int, default=1, choices=[1, 2], help="order of the upwind sweep")
+    ap.add_argument("--shard", action="store_true",
+                    help="with --gpus N: shard the velocity blocks of ONE problem over the N ranks (NCCL all-reduce of the velocity "
+                         "sums per iteration, strong scaling) instead of N independent replicas")
     ap.add_argument("--precision", default="f64", choices=["f64", "mixed"],
                     help="f64 (BASELINE.json's metric) or mixed = the paper's timing precision: single-precision sweep, double moments")
     args = ap.parse_args()

@@ -82,6 +82,13 @@ extern "C" {
                              (units of DESIGN.md section 2), not to 1e-11 */
 #define DVM_PREC_F64      0
 #define DVM_PREC_MIXED    1
+#define DVM_OPT_SHARD_COUNT 8 /* velocity-space sharding over several GPUs (the velocities are independent inside an
+                             iteration; the paper's MPI program decomposes the velocity space): number of ranks n >= 1
+                             (default 1).  With n > 1 this solver sweeps only the velocity blocks r, r + n, ... of the tile kernel
+                             (r = DVM_OPT_SHARD_RANK), all macroscopic state is replicated, and an iteration is
+                             dvm_sweep -> all-reduce (sum, fp64) of the buffer dvm_reduce_buffer names, over the ranks, by the caller
+                             (NCCL) -> dvm_update; dvm_iterate / dvm_step_host then return DVM_EINVAL.  Tile kernel only */
+#define DVM_OPT_SHARD_RANK  9 /* this solver's rank, 0 <= r < n; set DVM_OPT_SHARD_COUNT first */
 
 typedef struct dvm_solver dvm_solver; /* opaque */
 
@@ -130,6 +137,18 @@ int dvm_create(const dvm_grid *grid, const dvm_vgrid *vgrid, const dvm_gas *gas,
 
 /* n >= 0 outer iterations (Alg. 1 + moment update + residual), asynchronous on the stream. */
 int dvm_iterate(dvm_solver *s, int n);
+
+/* The two halves of one outer iteration, for velocity-space sharding (DVM_OPT_SHARD_COUNT): dvm_sweep clears the velocity-sum
+ * accumulator, rebuilds the factor tables and sweeps this rank's velocity blocks (rows a1-a5 of DESIGN.md); dvm_update converts
+ * the sums to the state n+1, wall densities, mass rescale and residual (rows a5-a7) - every rank does it redundantly after the
+ * all-reduce.  dvm_sweep; dvm_update with one rank is exactly dvm_iterate(1).  Asynchronous on the stream.  Tile kernel only
+ * (DVM_EINVAL for the slice kernel, whose wall fluxes are separate atomics). */
+int dvm_sweep(dvm_solver *s);
+int dvm_update(dvm_solver *s);
+/* The buffer the ranks must sum between dvm_sweep and dvm_update: *dev_ptr = the [ncell][16] fp64 accumulator (13 velocity
+ * sums + the half-range first moments the wall fluxes are read from), *count = 16 * ncell doubles.  The pointer is the start
+ * of an allocation made through dvm_device.alloc and stays valid for the life of the solver. */
+int dvm_reduce_buffer(dvm_solver *s, double **dev_ptr, size_t *count);
 
 /* Current macroscopic fields, dev_out[14][ncell]: rho, ux, uy, uz, T, qx, qy, qz, sxx, syy, szz, sxy, sxz, syz
  * (solid cells: zeros).  Asynchronous device-to-device copy on the stream. */
@@ -192,6 +211,9 @@ int dvm_plan_query(int nx, int ny, int nz, const dvm_vgrid *v, int target_ctas, 
  * nz, NA + 65536 (1 + wide axis), 256 nbb + ncb}: the block holds the nodes [x0, x0+nx) x [y0, y0+ny) x [z0, z0+nz) of xi_x,
  * xi_y, xi_z, all of one sign octant, in a box of NA (along the wide axis) x nbb x ncb lanes.  Returns the number of blocks. */
 int dvm_plan_vblocks(const dvm_vgrid *v, int rv, int order, int wide_axis, int *boxes8, int max_blocks);
+/* The same for rank shard_rank of shard_count (DVM_OPT_SHARD_COUNT): only that rank's velocity blocks. */
+int dvm_plan_shard_vblocks(const dvm_vgrid *v, int rv, int order, int wide_axis, int shard_rank, int shard_count, int *boxes8,
+                           int max_blocks);
 /* Bytes of device workspace held by the solver, and the part of it that holds distribution-function values. */
 int dvm_workspace_bytes(const dvm_solver *s, size_t *total, size_t *f_bytes);
 /* Number of kernel launches enqueued by this solver so far (bench.py's gpu_launches). */

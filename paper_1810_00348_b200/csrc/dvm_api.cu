@@ -81,6 +81,8 @@ struct dvm_solver {
     int max_ctas = 0;             // cap on the persistent grid of the tile kernel (0 = all resident CTAs)
     int order = 1;                // 1: first-order upwind Eq.(7); 2: second-order upwind
     int precision = DVM_PREC_F64; // DVM_PREC_MIXED: f carried in single precision by the tile kernel
+    int shard_rank = 0, shard_count = 1;   // velocity-space sharding (DVM_OPT_SHARD_COUNT / _RANK)
+    bool swept = false;           // dvm_sweep done, dvm_update pending
     size_t fvalue() const { return precision == DVM_PREC_MIXED ? sizeof(float) : sizeof(double); }
     bool planned = false;
     long long launches = 0;
@@ -312,6 +314,8 @@ int plan_once(dvm_solver *s)
     const bool f32 = s->precision == DVM_PREC_MIXED;
     if (f32 && (kernel != DVM_KERNEL_TILE || s->order != 1 || s->tile_rv == 2))
         return fail(DVM_EINVAL, "DVM_PREC_MIXED is a mode of the first-order tile kernel with 3 or 4 velocities per thread");
+    if (s->shard_count > 1 && kernel != DVM_KERNEL_TILE)
+        return fail(DVM_EINVAL, "velocity-space sharding (DVM_OPT_SHARD_COUNT) is a mode of the tile kernel");
     s->kernel = kernel;
     int lo[3][2], cnt[3][2];
     for (int d = 0; d < 3; ++d) split_axis(s->xi[d], lo[d], cnt[d]);
@@ -350,7 +354,8 @@ int plan_once(dvm_solver *s)
         CK(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
         if (per_sm < 1) return fail(DVM_ECUDA, "tile kernel does not fit on an SM");
         const int resident = per_sm * nsm;
-        if (tile_plan(s->nx, s->ny, s->nz, s->xi, resident, 0, rv, order, wide, &s->tile)) return fail(DVM_EINVAL, "tile plan failed");
+        if (tile_plan(s->nx, s->ny, s->nz, s->xi, resident, 0, rv, order, wide, &s->tile, s->shard_rank, s->shard_count))
+            return fail(DVM_EINVAL, s->shard_count > 1 ? "tile plan failed (more shards than velocity blocks?)" : "tile plan failed");
         if (s->max_f_mbytes > 0) {
             // cap on the f workspace: fewer velocity blocks in flight (batches); the band height P
             // grows as the batch shrinks, so iterate to a fixed point; one block is the floor
@@ -361,7 +366,8 @@ int plan_once(dvm_solver *s)
                 const double need = (double)(s->tile.xface_values + s->tile.yface_values) * vbytes;
                 if (need <= cap || B == 1) break;
                 B = std::max(1, std::min(B - 1, (int)(cap / ((s->tile.P * TILE_TY + s->tile.ntx * TILE_TX) * lvl))));
-                if (tile_plan(s->nx, s->ny, s->nz, s->xi, resident, B, rv, order, wide, &s->tile)) return fail(DVM_EINVAL, "tile plan failed");
+                if (tile_plan(s->nx, s->ny, s->nz, s->xi, resident, B, rv, order, wide, &s->tile, s->shard_rank, s->shard_count))
+                    return fail(DVM_EINVAL, "tile plan failed");
             }
             const double need = (double)(s->tile.xface_values + s->tile.yface_values) * vbytes;
             if (need > cap)
@@ -663,6 +669,18 @@ int dvm_set_option(dvm_solver *s, int option, int value)
         s->precision = value;
         return DVM_OK;
     }
+    if (option == DVM_OPT_SHARD_COUNT || option == DVM_OPT_SHARD_RANK) {
+        if (s->planned) return fail(DVM_EINVAL, "sharding must be set before the first iteration");
+        if (option == DVM_OPT_SHARD_COUNT) {
+            if (value < 1) return fail(DVM_EINVAL, "shard count must be >= 1");
+            s->shard_count = value;
+            if (s->shard_rank >= value) s->shard_rank = 0;
+        } else {
+            if (value < 0 || value >= s->shard_count) return fail(DVM_EINVAL, "shard rank must be in [0, shard count)");
+            s->shard_rank = value;
+        }
+        return DVM_OK;
+    }
     if (option == DVM_OPT_MAX_CTAS) {
         if (s->planned) return fail(DVM_EINVAL, "the grid cap must be set before the first iteration");
         if (value < 0) return fail(DVM_EINVAL, "negative grid cap");
@@ -678,35 +696,88 @@ int dvm_set_option(dvm_solver *s, int option, int value)
     return fail(DVM_EINVAL, "unknown option %d", option);
 }
 
+namespace {
+
+// first half of an outer iteration: clear the accumulators, (tile kernel) rebuild the factor tables, sweep
+int sweep_phase(dvm_solver *s)
+{
+    CK(cudaMemsetAsync(s->d_raw, 0, (size_t)16 * s->ncell * sizeof(double), s->stream));
+    CK(cudaMemsetAsync(s->d_phi, 0, (size_t)s->nface * sizeof(double), s->stream));
+    if (s->kernel == DVM_KERNEL_SLICE) {
+        const SweepParams P = sweep_params(s);
+        CK(launch_sweep_slice(P, (int)s->blocks.size(), s->nb_threads, s->stream));
+    } else {
+        CK(launch_tables(table_params(s), s->stream));
+        s->launches += 1;
+        CK(cudaMemsetAsync(s->d_counter, 0, sizeof(int), s->stream));
+        s->epoch += 1;
+        const TileParams TP = tile_params(s);
+        CK(launch_sweep_tile(TP, s->tile_rv, s->order, s->precision == DVM_PREC_MIXED, s->tile.ax[0], s->tile_grid, s->stream));
+    }
+    s->launches += 1;
+    return 0;
+}
+
+// second half: wall fluxes from the half-range sums (tile kernel), conversion, wall densities, rescale, residual
+int update_phase(dvm_solver *s)
+{
+    const UpdateParams U = update_params(s);
+    if (s->kernel != DVM_KERNEL_SLICE) {
+        CK(launch_phi_from_raw(U, s->d_face_cell, s->d_face_dir, s->d_phi, s->order, s->stream));
+        s->launches += 1;
+    }
+    int l = 0;
+    CK(launch_update(U, s->iters % HIST_CAP, s->stream, &l));
+    s->launches += l;
+    s->iters += 1;
+    return 0;
+}
+
+}  // namespace
+
 int dvm_iterate(dvm_solver *s, int niter)
 {
     if (!s || niter < 0) return fail(DVM_EINVAL, "bad argument");
     if (niter == 0) return DVM_OK;
+    if (s->shard_count > 1)
+        return fail(DVM_EINVAL, "this solver holds 1 of %d velocity shards: iterate with dvm_sweep / all-reduce / dvm_update", s->shard_count);
+    if (s->swept) return fail(DVM_EINVAL, "dvm_sweep without dvm_update");
     DeviceGuard guard(s->device);
     if (int rc = plan(s)) return rc;
-    const UpdateParams U = update_params(s);
-    const SweepParams P = sweep_params(s);
     for (int it = 0; it < niter; ++it) {
-        CK(cudaMemsetAsync(s->d_raw, 0, (size_t)16 * s->ncell * sizeof(double), s->stream));
-        CK(cudaMemsetAsync(s->d_phi, 0, (size_t)s->nface * sizeof(double), s->stream));
-        if (s->kernel == DVM_KERNEL_SLICE) {
-            CK(launch_sweep_slice(P, (int)s->blocks.size(), s->nb_threads, s->stream));
-        } else {
-            CK(launch_tables(table_params(s), s->stream));
-            s->launches += 1;
-            CK(cudaMemsetAsync(s->d_counter, 0, sizeof(int), s->stream));
-            s->epoch += 1;
-            const TileParams TP = tile_params(s);
-            CK(launch_sweep_tile(TP, s->tile_rv, s->order, s->precision == DVM_PREC_MIXED, s->tile.ax[0], s->tile_grid, s->stream));
-            CK(launch_phi_from_raw(U, s->d_face_cell, s->d_face_dir, s->d_phi, s->order, s->stream));
-            s->launches += 1;
-        }
-        s->launches += 1;
-        int l = 0;
-        CK(launch_update(U, s->iters % HIST_CAP, s->stream, &l));
-        s->launches += l;
-        s->iters += 1;
+        if (int rc = sweep_phase(s)) return rc;
+        if (int rc = update_phase(s)) return rc;
     }
+    return DVM_OK;
+}
+
+int dvm_sweep(dvm_solver *s)
+{
+    if (!s) return fail(DVM_EINVAL, "NULL solver");
+    if (s->swept) return fail(DVM_EINVAL, "dvm_sweep twice without dvm_update");
+    DeviceGuard guard(s->device);
+    if (int rc = plan(s)) return rc;
+    if (s->kernel == DVM_KERNEL_SLICE) return fail(DVM_EINVAL, "dvm_sweep / dvm_update are calls of the tile kernel");
+    if (int rc = sweep_phase(s)) return rc;
+    s->swept = true;
+    return DVM_OK;
+}
+
+int dvm_update(dvm_solver *s)
+{
+    if (!s) return fail(DVM_EINVAL, "NULL solver");
+    if (!s->swept) return fail(DVM_EINVAL, "dvm_update without dvm_sweep");
+    DeviceGuard guard(s->device);
+    if (int rc = update_phase(s)) return rc;
+    s->swept = false;
+    return DVM_OK;
+}
+
+int dvm_reduce_buffer(dvm_solver *s, double **dev_ptr, size_t *count)
+{
+    if (!s || !dev_ptr || !count) return fail(DVM_EINVAL, "NULL argument");
+    *dev_ptr = s->d_raw;
+    *count = (size_t)16 * (size_t)s->ncell;
     return DVM_OK;
 }
 
@@ -868,6 +939,30 @@ int dvm_plan_vblocks(const dvm_vgrid *v, int rv, int order, int wide_axis, int *
             const VBlock &b = tp.vblocks[e];
             int *o = boxes8 + 8 * e;
             // node ranges in the order xi_x, xi_y, xi_z whatever the roles are
+            const int lo[3] = {b.a0, b.b0, b.c0}, cn[3] = {b.na, b.nb, b.nc};
+            for (int r = 0; r < 3; ++r) { o[2 * tp.ax[r]] = lo[r]; o[2 * tp.ax[r] + 1] = cn[r]; }
+            o[6] = tile_na(rv) + 65536 * (tp.ax[0] + 1); o[7] = b.nbb * 256 + b.ncb;
+        }
+    return n;
+}
+
+int dvm_plan_shard_vblocks(const dvm_vgrid *v, int rv, int order, int wide_axis, int shard_rank, int shard_count, int *boxes8,
+                           int max_blocks)
+{
+    if (wide_axis < 0 || wide_axis > 3 || shard_count < 1 || shard_rank < 0 || shard_rank >= shard_count) return fail(DVM_EINVAL, "bad argument");
+    if (!v || max_blocks < 0 || (rv != 0 && (rv < 2 || rv > 4)) || (order != 1 && order != 2) || (order == 2 && rv > 2) || v->mx <= 0 || v->my <= 0 || v->mz <= 0 || !v->xi_x || !v->xi_y || !v->xi_z)
+        return fail(DVM_EINVAL, "bad argument");
+    std::vector<double> xi[3];
+    xi[0].assign(v->xi_x, v->xi_x + v->mx); xi[1].assign(v->xi_y, v->xi_y + v->my); xi[2].assign(v->xi_z, v->xi_z + v->mz);
+    int wide = 0;
+    choose_variant(xi, order, rv, wide_axis - 1, &rv, &wide);
+    TilePlan tp;
+    if (tile_plan(4, 4, 1, xi, 1, 0, rv, order, wide, &tp, shard_rank, shard_count)) return fail(DVM_EINVAL, "tile plan failed (more shards than velocity blocks?)");
+    const int n = (int)tp.vblocks.size();
+    if (boxes8)
+        for (int e = 0; e < n && e < max_blocks; ++e) {
+            const VBlock &b = tp.vblocks[e];
+            int *o = boxes8 + 8 * e;
             const int lo[3] = {b.a0, b.b0, b.c0}, cn[3] = {b.na, b.nb, b.nc};
             for (int r = 0; r < 3; ++r) { o[2 * tp.ax[r]] = lo[r]; o[2 * tp.ax[r] + 1] = cn[r]; }
             o[6] = tile_na(rv) + 65536 * (tp.ax[0] + 1); o[7] = b.nbb * 256 + b.ncb;

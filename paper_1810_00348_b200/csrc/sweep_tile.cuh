@@ -150,8 +150,9 @@ struct TableParams {
 // items that should be able to run concurrently (sets the band height P); max_blocks > 0 caps the velocity blocks in
 // flight at once (batches).  Pure host code (tests call it through
 // dvm_plan_query without a GPU).
+// shard_rank / shard_count: the plan holds only the velocity blocks of that rank (velocity-space sharding; -1 if it has none).
 int tile_plan(int nx, int ny, int nz, const std::vector<double> xi[3], int target_ctas, int max_blocks, int rv, int order,
-              int wide_axis, TilePlan *plan);
+              int wide_axis, TilePlan *plan, int shard_rank = 0, int shard_count = 1);
 
 // f32: f carried in single precision (DVM_PREC_MIXED; order 1, rv 3 or 4)
 bool tile_variant_exists(int rv, int order, bool f32);

@@ -20,10 +20,10 @@ int ceil_div(int a, int b) { return (a + b - 1) / b; }
 }  // namespace
 
 int tile_plan(int nx, int ny, int nz, const std::vector<double> xi[3], int target_ctas, int max_blocks, int rv, int order,
-              int wide_axis, TilePlan *plan)
+              int wide_axis, TilePlan *plan, int shard_rank, int shard_count)
 {
     if (nx <= 0 || ny <= 0 || nz <= 0 || !plan || (rv < 2 || rv > 4) || (order != 1 && order != 2) || (order == 2 && rv != 2) ||
-        wide_axis < 0 || wide_axis > 2)
+        wide_axis < 0 || wide_axis > 2 || shard_count < 1 || shard_rank < 0 || shard_rank >= shard_count)
         return -1;
     const int NA = tile_na(rv), NVB = tile_nvb(rv, order), npair = tile_npair(rv, order), layers = tile_face_layers(order);
     plan->rv = rv; plan->order = order;
@@ -84,6 +84,14 @@ int tile_plan(int nx, int ny, int nz, const std::vector<double> xi[3], int targe
                 v.xb = first[0][oa] + a0 / NA; v.yb = first[1][ob] + b0 / best_bb; v.zb = first[2][oc] + c0 / best_cb;
                 plan->vblocks.push_back(v);
             }
+    }
+    // velocity-space sharding (the paper's MPI program decomposes the velocity space): rank r
+    // of n sweeps the velocity blocks r, r + n, r + 2n, ... of the list (every octant is spread over the ranks); the factor
+    // tables stay complete
+    if (shard_count > 1) {
+        std::vector<VBlock> mine;
+        for (size_t e = (size_t)shard_rank; e < plan->vblocks.size(); e += (size_t)shard_count) mine.push_back(plan->vblocks[e]);
+        plan->vblocks.swap(mine);
     }
     const int nvb = (int)plan->vblocks.size();
     if (nvb == 0) return -1;

@@ -30,6 +30,8 @@ OPT_MAX_CTAS = 4
 OPT_ORDER = 5
 OPT_TILE_AXIS = 6
 OPT_PRECISION = 7
+OPT_SHARD_COUNT = 8
+OPT_SHARD_RANK = 9
 PREC_F64, PREC_MIXED = 0, 1
 
 # every symbol include/dvm.h declares (checked by tests/test_abi.py)
@@ -37,7 +39,8 @@ SYMBOLS = (
     "dvm_create", "dvm_iterate", "dvm_moments", "dvm_residual", "dvm_num_faces", "dvm_iterations_done",
     "dvm_get_state", "dvm_set_state", "dvm_raw_moments", "dvm_wall_flux", "dvm_residual_history",
     "dvm_mass_scale", "dvm_step_host", "dvm_set_option", "dvm_workspace_bytes", "dvm_launch_count",
-    "dvm_kernel_used", "dvm_tile_rv", "dvm_tile_axis", "dvm_precision", "dvm_plan_query", "dvm_plan_vblocks", "dvm_destroy", "dvm_last_error",
+    "dvm_kernel_used", "dvm_tile_rv", "dvm_tile_axis", "dvm_precision", "dvm_plan_query", "dvm_plan_vblocks",
+    "dvm_plan_shard_vblocks", "dvm_sweep", "dvm_update", "dvm_reduce_buffer", "dvm_destroy", "dvm_last_error",
 )
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
@@ -127,6 +130,10 @@ def lib():
         L.dvm_kernel_used.argtypes = [vp]
         L.dvm_tile_rv.argtypes = [vp]
         L.dvm_precision.argtypes = [vp]
+        L.dvm_sweep.argtypes = [vp]
+        L.dvm_update.argtypes = [vp]
+        L.dvm_reduce_buffer.argtypes = [vp, C.POINTER(vp), C.POINTER(C.c_size_t)]
+        L.dvm_plan_shard_vblocks.argtypes = [C.POINTER(_VGrid), C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int), C.c_int]
         L.dvm_tile_axis.argtypes = [vp]
         L.dvm_plan_query.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(_VGrid), C.c_int, C.c_int, C.c_int, C.c_int, C.c_int,
                                      C.POINTER(C.c_int), C.POINTER(C.c_int), C.c_int]
@@ -173,11 +180,21 @@ def plan_vblocks(xi_x, xi_y, xi_z, rv=0, order=1, wide_axis=0):
     return out
 
 
+def plan_shard_vblocks(xi_x, xi_y, xi_z, rank, count, rv=0, order=1, wide_axis=0):
+    """dvm_plan_shard_vblocks: the velocity blocks (as plan_vblocks) of rank `rank` of `count` (host only)."""
+    keep = [_f64(a) for a in (xi_x, xi_y, xi_z)]
+    v = _VGrid(len(keep[0]), len(keep[1]), len(keep[2]), *(a.ctypes.data_as(_dp) for a in keep), None, None, None)
+    n = _check(lib().dvm_plan_shard_vblocks(C.byref(v), rv, order, wide_axis, rank, count, None, 0))
+    out = np.zeros((n, 8), dtype=np.int32)
+    _check(lib().dvm_plan_shard_vblocks(C.byref(v), rv, order, wide_axis, rank, count, out.ctypes.data_as(C.POINTER(C.c_int)), n))
+    return out
+
+
 class Solver:
     """dvm_create / dvm_iterate / dvm_moments / dvm_residual (+ support calls) for one workload record."""
 
     def __init__(self, wl, kernel: int = KERNEL_AUTO, device: str = "cuda:0", max_f_mbytes: int = 0, tile_rv: int = 0,
-                 max_ctas: int = 0, order: int = 0, tile_axis: int = 0, precision: int = -1):
+                 max_ctas: int = 0, order: int = 0, tile_axis: int = 0, precision: int = -1, shard=None):
         import torch
         if not torch.cuda.is_available():
             raise DvmError(ECUDA, "no CUDA device: the DVM solver has no CPU fallback")
@@ -240,10 +257,43 @@ class Solver:
             precision = PREC_MIXED if getattr(wl, "f32", False) else PREC_F64
         if precision != PREC_F64:
             self.set_option(OPT_PRECISION, int(precision))
+        # velocity-space sharding: shard = (rank, count); this solver sweeps 1 of `count` parts of the velocity blocks
+        self.shard = (0, 1) if shard is None else (int(shard[0]), int(shard[1]))
+        if self.shard[1] > 1:
+            self.set_option(OPT_SHARD_COUNT, self.shard[1])
+            self.set_option(OPT_SHARD_RANK, self.shard[0])
 
     # -- the four calls of the north star ---------------------------------------------------------
     def iterate(self, n: int = 1):
         _check(lib().dvm_iterate(self._h, n))
+
+    # -- velocity-space sharding (DVM_OPT_SHARD_COUNT): sweep -> all-reduce over the ranks -> update ---------------
+    def sweep(self):
+        _check(lib().dvm_sweep(self._h))
+
+    def update(self):
+        _check(lib().dvm_update(self._h))
+
+    def reduce_buffer(self):
+        """The [ncell][16] fp64 accumulator the ranks must sum between sweep() and update(), as a torch view of the solver's
+        own allocation (no copy)."""
+        ptr, n = C.c_void_p(), C.c_size_t()
+        _check(lib().dvm_reduce_buffer(self._h, C.byref(ptr), C.byref(n)))
+        block = self._blocks[ptr.value]
+        return block[: 8 * n.value].view(self.torch.float64)
+
+    def iterate_sharded(self, n: int = 1, group=None):
+        """n outer iterations of a velocity-sharded solver: every rank sweeps its velocity blocks, one all-reduce (sum, fp64;
+        NCCL through torch.distributed, on the solver's stream) of the velocity sums per iteration, then every rank updates the
+        replicated macroscopic state.  With one rank this is iterate(n)."""
+        if self.shard[1] == 1:
+            return self.iterate(n)
+        import torch.distributed as dist
+        buf = self.reduce_buffer()
+        for _ in range(n):
+            self.sweep()
+            dist.all_reduce(buf, op=dist.ReduceOp.SUM, group=group)
+            self.update()
 
     def moments(self, out=None):
         out = self._dev_empty(14 * self.ncell) if out is None else out

@@ -592,3 +592,78 @@ def test_every_wide_axis_of_the_tile_kernel(oracle_mod, axis, rv, order):
     lockstep(W.cube_flow(4, 12, box=(6, 4, 4), vrange=8.0).with_(order=order), 2, 2, oracle_mod, **kw)
     wide = W.cavity(0, 0, 0.3, nxyz=(6, 5, 7), mxyz=(18, 26, 34)).with_(order=order)
     lockstep(wide, 2, 1, oracle_mod, state=W.perturbed_state(wide, seed=60 + axis, amp_q=0.01), rho_w=None, **kw)
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# Velocity-space sharding (DVM_OPT_SHARD_COUNT): one GPU stands in for n ranks.  The n
+# solvers run one after the other (no kernel waits on another); the sum of their accumulators stands in for the all-reduce.
+@pytest.mark.parametrize("nranks,case", [(2, "cfg0"), (3, "ragged"), (2, "cube"), (4, "cfg1"), (2, "mixed")])
+def test_velocity_shards_emulated_on_one_gpu(oracle_mod, nranks, case):
+    from paper_1810_00348_b200 import dvm
+    kw = {}
+    if case == "cfg0":
+        wl, iters = W.config(0), 5
+    elif case == "ragged":
+        wl, iters = W.cavity(0, 0, 0.075, stretch=1.5, nxyz=(13, 9, 11), mxyz=(10, 7, 9)), 3
+    elif case == "cube":
+        wl, iters = W.cube_flow(4, 12, box=(6, 4, 4), vrange=8.0), 3
+    elif case == "cfg1":
+        wl, iters = W.config(1), 2
+    else:
+        wl, iters, kw = W.config(0), 3, dict(precision=dvm.PREC_MIXED)
+    o = oracle_mod.Oracle(wl)
+    ranks = [dvm.Solver(wl, kernel=2, shard=(r, nranks), **kw) for r in range(nranks)]
+    fm = fluid_mask(wl)
+    for it in range(iters):
+        for s in ranks:
+            s.sweep()
+        total = sum(s.reduce_buffer() for s in ranks)          # stands in for the all-reduce
+        part_rho = [float(s.reduce_buffer().view(-1, 16)[:, 0].sum()) for s in ranks]
+        for s in ranks:
+            s.reduce_buffer().copy_(total)
+            s.update()
+        o.step()
+        what = f"{case} {nranks} ranks iteration {it + 1}"
+        assert all(0 < p < (1 - 1e-9) * sum(part_rho) for p in part_rho), what       # every rank holds a part, none all of it
+        g14 = ranks[0].moments().cpu().numpy()
+        if case == "mixed":
+            from tests.parity import tol32
+            assert np.abs(g14 - o.prim14).max() <= 3 * tol32(wl), what
+        else:
+            assert_fields(g14, o.prim14, fm, what=what)
+            assert_residual(ranks[0].residual(), o.resid, what=what)
+            assert np.abs(ranks[0].get_state()[1].cpu().numpy() - o.rho_w).max() <= 1e-11 * np.abs(o.rho_w).max(), what
+        # the replicated state is bit-identical on every rank (same sums, same update)
+        for s in ranks[1:]:
+            assert np.array_equal(s.moments().cpu().numpy(), g14), what
+    # a sharded solver refuses the unsharded calls
+    with pytest.raises(dvm.DvmError):
+        ranks[0].iterate(1)
+    with pytest.raises(dvm.DvmError):
+        ranks[0].update()
+    for s in ranks:
+        s.close()
+
+
+def test_sweep_update_is_iterate_with_one_rank(oracle_mod):
+    """dvm_sweep; dvm_update on an unsharded solver is dvm_iterate(1) (same launches): lock-step with the oracle; the slice
+    kernel refuses the split."""
+    from paper_1810_00348_b200 import dvm
+    wl = W.config(0)
+    o = oracle_mod.Oracle(wl)
+    s = make(wl, 2)
+    for it in range(3):
+        s.sweep()
+        with pytest.raises(dvm.DvmError):
+            s.sweep()
+        s.update()
+        o.step()
+        compare_step(s, o, f"sweep/update iteration {it + 1}")
+    s.iterate_sharded(1)
+    o.step()
+    compare_step(s, o, "iterate_sharded with one rank")
+    s.close()
+    s = make(wl, 1)
+    with pytest.raises(dvm.DvmError):
+        s.sweep()
+    s.close()
