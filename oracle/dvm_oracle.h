@@ -18,8 +18,9 @@
  *   then the faces between a fluid cell and a solid cell inside the domain, ordered by
  *   (fluid cell index ascending, direction id ascending).
  *
- * Pins (tests/test_oracle_pins.py, run with -m "not gpu"): P1-P9 of DESIGN.md.  The actual field
- * values of a cavity / cube solution are "parity unpinned": the paper prints none.
+ * Pins (run with -m "not gpu"): tests/test_oracle_pins.py (P1-P16 of DESIGN.md), tests/test_oracle_order2.py (order = 2),
+ * tests/test_oracle_f32.py (f32 = 1).  The actual field values of a cavity / cube solution are "parity unpinned": the paper
+ * prints none.
  */
 #ifndef DVM_ORACLE_H
 #define DVM_ORACLE_H

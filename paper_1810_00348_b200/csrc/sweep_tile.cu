@@ -218,6 +218,30 @@ __device__ __forceinline__ void st_f32(float *addr, float a)
     asm volatile("st.global.f32 [%0], %1;" ::"l"(addr), "f"(a));
 }
 
+// Lane <-> velocity mapping.  The fp64 MMA contracts over lane & 3, and stage 1 of the velocity sums contracts over the
+// xi_x groups, so the MMA wants the value of (xi_x group ag, pair n) in lane 4 n + ag, and by default the thread in that lane
+// owns that velocity.  A 128-bit shared-memory load whose address is shared by NON-adjacent lanes costs 4 wavefronts whatever
+// the number of distinct addresses (1 - 2 when ADJACENT lanes share it; micro-benchmark in profiles/r02_sweep_tile.md), and the
+// entries of the xi_x table - 3/4 of the shared-memory wavefronts - are shared by the lanes of one xi_x group.
+// -DDVM_TILE_XPOSE=1 gives the thread in lane l the velocity (ag = l >> 3, pair = l & 7) instead - the 8 lanes of a group are
+// adjacent - and hands every new value to the lane the MMA wants it in with one shuffle: 38 % fewer shared-memory wavefronts,
+// parity-green, and 7 % SLOWER on every config (cfg4 3.79e11 against 4.08e11): the shared-memory pipe is the most used unit
+// but not what limits the kernel.  Kept as a compile-time switch for the record; off.
+#ifndef DVM_TILE_XPOSE
+#define DVM_TILE_XPOSE 0
+#endif
+__device__ __forceinline__ int lane_ag(int lane) { return DVM_TILE_XPOSE ? lane >> 3 : lane & 3; }
+__device__ __forceinline__ int lane_pair(int lane) { return DVM_TILE_XPOSE ? lane & 7 : lane >> 2; }
+// the value the MMA wants from this lane (B fragment: k = lane & 3 = xi_x group, n = lane >> 2 = pair), widened to double
+__device__ __forceinline__ double mma_operand(double g, int lane)
+{
+    return DVM_TILE_XPOSE ? __shfl_sync(0xffffffffu, g, (lane & 3) * 8 + (lane >> 2)) : g;
+}
+__device__ __forceinline__ double mma_operand(float g, int lane)
+{
+    return (double)(DVM_TILE_XPOSE ? __shfl_sync(0xffffffffu, g, (lane & 3) * 8 + (lane >> 2)) : g);
+}
+
 // D (8 x 8) += A (8 x 4, row-major) * B (4 x 8, column-major) in fp64 on the tensor cores (DMMA).  Fragments of lane l:
 // A[l >> 2][l & 3], B[l & 3][l >> 2], C/D[l >> 2][2 (l & 3) + {0, 1}].
 __device__ __forceinline__ void dmma(double &c0, double &c1, const double a, const double b)
@@ -638,7 +662,7 @@ __device__ __forceinline__ void compute_row(const RowBuf<RV, ORD, R> &Rw, const 
         // velocity sums: always in double (a single value is widened exactly)
         acc[ii & 1][0] = 0.0; acc[ii & 1][1] = 0.0;
 #pragma unroll
-        for (int r = 0; r < RV; ++r) dmma(acc[ii & 1][0], acc[ii & 1][1], T.aX[r], (double)zrow[ii][r]);
+        for (int r = 0; r < RV; ++r) dmma(acc[ii & 1][0], acc[ii & 1][1], T.aX[r], mma_operand(zrow[ii][r], lane));
         if (ii & 1) emit_pair<RV, ORD, R>(Rw, T.ro[ii - 1], T.ro[ii], acc[0][0], acc[0][1], acc[1][0], acc[1][1], T, lane);
         if (YL >= 0 && wy) store_face<RV, ORD, R>(yout + (YL * TILE_TX + ii) * NVB, tid, zrow[ii]);
     }
@@ -768,7 +792,7 @@ __device__ __forceinline__ void compute_level_slow(TileSmem<RV, ORD, R> &s, cons
                 fx[r] = gg;
                 if (ORD == 2) pl2[cell * RV + r] = pl[cell * RV + r];
                 pl[cell * RV + r] = gg;
-                dmma(c0, c1, T.aX[r], (double)gg);
+                dmma(c0, c1, T.aX[r], mma_operand(gg, lane));
             }
             if (ii & 1) {
                 emit_pair<RV, ORD, R>(Rw, roPrev, ro, accA0, accA1, c0, c1, T, lane);
@@ -889,10 +913,10 @@ __global__ void __launch_bounds__(KC<RV, ORD, R>::THREADS, KC<RV, ORD, R>::MIN_C
         __syncthreads();
 
         ThreadCtx<RV, ORD, R> T;
-        T.ag = lane & 3;
+        T.ag = lane_ag(lane);
         T.xrev = vb.sx > 0 ? 0 : 3;
         {
-            const int pair = warp * 8 + (lane >> 2);
+            const int pair = warp * 8 + lane_pair(lane);
             const int yl = pair % vb.nbb, zl = pair / vb.nbb;
             T.yi = yl;
             T.zi = vb.nbb + zl;
@@ -909,7 +933,7 @@ __global__ void __launch_bounds__(KC<RV, ORD, R>::THREADS, KC<RV, ORD, R>::MIN_C
             const int row = lane >> 2, pw = row & 3;
 #pragma unroll
             for (int r = 0; r < RV; ++r) {
-                const double x = s.xi_a[RV * T.ag + r];
+                const double x = s.xi_a[RV * (lane & 3) + r];      // the MMA's view: k = lane & 3
                 T.aX[r] = pw == 0 ? 1.0 : pw == 1 ? x : pw == 2 ? x * x : x * x * x;
             }
             // stage-2 B fragments: monomial j = lane >> 2 of the (xi_y, xi_z) nodes of pairs 2q and 2q + 1 of this warp
