@@ -19,8 +19,9 @@
  *   (fluid cell index ascending, direction id ascending).
  *
  * Pins (run with -m "not gpu"): tests/test_oracle_pins.py (P1-P16 of DESIGN.md), tests/test_oracle_order2.py (order = 2),
- * tests/test_oracle_f32.py (f32 = 1).  The actual field values of a cavity / cube solution are "parity unpinned": the paper
- * prints none.
+ * tests/test_oracle_f32.py (f32 = 1).  Every function here is pinned.  The converged solution is pinned against its closed form in
+ * the free-molecular limit (P17, P18); for the cavity / cube fields at finite Kn the paper prints no value to pin against
+ * (PAPER.md:271, 295).
  */
 #ifndef DVM_ORACLE_H
 #define DVM_ORACLE_H

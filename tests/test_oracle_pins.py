@@ -518,3 +518,57 @@ def test_P16_mass_rescale_scales_everything_linear_in_f(oracle_mod):
         xin = comp[d] * (1.0 if d & 1 else -1.0)
         bf = (Wt * np.where(xin > 0, xin, 0.0) * (s * f6[..., c])).sum()
         assert o.rho_w[fidx] == pytest.approx(bf / phi_u[fidx], rel=1e-13)
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# P17, P18: the CONVERGED solution in the free-molecular limit against its textbook closed form.  Between two parallel
+# diffuse plates at Kn -> infinity the stationary distribution is the two half-range wall Maxwellians (Eq.(8)):
+# n_1 g_w1 for xi_x > 0, n_2 g_w2 for xi_x < 0, with n_1 sqrt(T_1) = n_2 sqrt(T_2) (no net mass flux, Eq.(9)) and
+# (n_1 + n_2) / 2 = rho.  Its moments are elementary half-range Gaussian integrals (speeds in v_m, section 2 of DESIGN.md):
+#   Couette (walls moving at -+U/2 in y, same T_w):  u = 0,  T = T_w + (2/3) (U/2)^2,  sigma_xy = -rho U / (2 sqrt(pi)),  q = 0
+#   Fourier (walls at rest, T_1 != T_2):  u = 0,  q_x = F (T_1 - T_2) / (2 sqrt(pi)),  F = 2 rho sqrt(T_1 T_2) / (sqrt T_1 + sqrt T_2),
+#            T = sqrt(T_1 T_2)
+# The oracle iterated to convergence at Kn = 1e9 on a 1-cell-thick channel must land on them up to the quadrature error of the
+# half-range trapezoid sums, which is second order in the node spacing h (P3): checked at two spacings.
+def _plates(oracle_mod, m, faces_x, iters=40):
+    wl = W.cavity(1, m, 1e9, nxyz=(6, 1, 1), vrange=7.0)
+    zg = W.FaceBC(W.ZERO_GRADIENT)
+    wl = wl.with_(faces=[faces_x[0], faces_x[1], zg, zg, zg, zg], rescale_mass=1)
+    o = oracle_mod.Oracle(wl)
+    for _ in range(iters):
+        p14 = o.step()
+    assert o.resid[0] < 1e-9 and o.resid[2] < 1e-9      # converged to the O(1 / Kn) the limit itself is approached with (the
+                                                        # momentum field is zero: its relative residual is noise)
+    assert np.abs(p14 - p14[:, :1]).max() < 1e-7        # collisionless: uniform across the gap
+    return p14[:, 0]
+
+
+def test_P17_free_molecular_couette_flow(oracle_mod):
+    U = 0.4
+    lo, hi = W.FaceBC(W.WALL_DIFFUSE, 1.0, 1.0, (0.0, -U / 2, 0.0)), W.FaceBC(W.WALL_DIFFUSE, 1.0, 1.0, (0.0, U / 2, 0.0))
+    errs = []
+    for m in (24, 48):
+        p = _plates(oracle_mod, m, (lo, hi))
+        rho, u, T, q, sig = p[0], p[1:4], p[4], p[5:8], p[8:14]
+        assert abs(rho - 1) < 1e-12 and np.abs(u).max() < 1e-8 and np.abs(q[[0, 2]]).max() < 1e-8 and abs(q[1]) < 1e-8
+        assert abs(T - (1 + (2 / 3) * (U / 2) ** 2)) < 1e-8          # full-range sums of one temperature: spectrally accurate
+        exact = -rho * U / (2 * math.sqrt(math.pi))
+        errs.append(abs(sig[3] - exact) / abs(exact))   # sigma_xy is component 3 of (xx, yy, zz, xy, xz, yz)
+        assert np.abs(sig[[4, 5]]).max() < 1e-10        # xz, yz vanish
+    assert errs[0] < 5e-2 and errs[1] < errs[0] / 3     # second order in h (3.3 %, 0.75 %): the sign and the factor 1 / (2 sqrt(pi)) are right
+
+
+def test_P18_free_molecular_heat_transfer(oracle_mod):
+    T1, T2 = 1.3, 0.8
+    lo, hi = W.FaceBC(W.WALL_DIFFUSE, T1, 1.0, (0.0, 0.0, 0.0)), W.FaceBC(W.WALL_DIFFUSE, T2, 1.0, (0.0, 0.0, 0.0))
+    errs, errT = [], []
+    for m in (24, 48):
+        p = _plates(oracle_mod, m, (lo, hi))
+        rho, u, T, q = p[0], p[1:4], p[4], p[5:8]
+        assert abs(rho - 1) < 1e-8 and np.abs(u).max() < 1e-8 and np.abs(q[1:]).max() < 1e-12
+        F = 2 * rho * math.sqrt(T1 * T2) / (math.sqrt(T1) + math.sqrt(T2))
+        exact = F * (T1 - T2) / (2 * math.sqrt(math.pi))          # heat flows from the hot plate (x-) to the cold one: q_x > 0
+        errs.append(abs(q[0] - exact) / abs(exact))
+        errT.append(abs(T - math.sqrt(T1 * T2)))
+    assert errs[0] < 5e-2 and errs[1] < errs[0] / 3
+    assert errT[0] < 5e-3 and errT[1] < errT[0] / 3

@@ -667,3 +667,32 @@ def test_sweep_update_is_iterate_with_one_rank(oracle_mod):
     with pytest.raises(dvm.DvmError):
         s.sweep()
     s.close()
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_free_molecular_plates_converged_solution(oracle_mod, kernel):
+    """GPU counterpart of pins P17 / P18: Couette flow and heat transfer between parallel plates at Kn = 1e9, 40 iterations on a
+    6 x 1 x 1 channel with 24^3 velocities: the converged GPU fields equal the oracle's (1e-11) and carry the textbook
+    free-molecular shear stress -rho U / (2 sqrt pi) and heat flux F (T1 - T2) / (2 sqrt pi) up to the 4 % quadrature error of
+    the half-range sums at this node spacing (P17 / P18 show that error is second order)."""
+    import math
+    zg = W.FaceBC(W.ZERO_GRADIENT)
+    U, T1, T2 = 0.4, 1.3, 0.8
+    cases = {"couette": (W.FaceBC(W.WALL_DIFFUSE, 1.0, 1.0, (0.0, -U / 2, 0.0)), W.FaceBC(W.WALL_DIFFUSE, 1.0, 1.0, (0.0, U / 2, 0.0))),
+             "fourier": (W.FaceBC(W.WALL_DIFFUSE, T1, 1.0, (0.0, 0.0, 0.0)), W.FaceBC(W.WALL_DIFFUSE, T2, 1.0, (0.0, 0.0, 0.0)))}
+    for name, (lo, hi) in cases.items():
+        wl = W.cavity(1, 24, 1e9, nxyz=(6, 1, 1), vrange=7.0).with_(faces=[lo, hi, zg, zg, zg, zg], rescale_mass=1)
+        o = oracle_mod.Oracle(wl)
+        s = make(wl, kernel)
+        s.iterate(40)
+        for _ in range(40):
+            o.step()
+        g = s.moments().cpu().numpy()
+        assert np.abs(g - o.prim14).max() <= 1e-11 * np.abs(o.prim14).max(), name
+        if name == "couette":
+            exact = -U / (2 * math.sqrt(math.pi))
+            assert abs(g[11, 0] - exact) < 0.04 * abs(exact) and g[11, 0] < 0
+        else:
+            exact = 2 * math.sqrt(T1 * T2) / (math.sqrt(T1) + math.sqrt(T2)) * (T1 - T2) / (2 * math.sqrt(math.pi))
+            assert abs(g[5, 0] - exact) < 0.04 * abs(exact) and g[5, 0] > 0
+        s.close()
