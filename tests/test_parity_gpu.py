@@ -696,3 +696,49 @@ def test_free_molecular_plates_converged_solution(oracle_mod, kernel):
             exact = 2 * math.sqrt(T1 * T2) / (math.sqrt(T1) + math.sqrt(T2)) * (T1 - T2) / (2 * math.sqrt(math.pi))
             assert abs(g[5, 0] - exact) < 0.04 * abs(exact) and g[5, 0] > 0
         s.close()
+
+
+_NCCL_ONE_RANK = r'''
+import os, sys, numpy as np, torch, torch.distributed as dist
+sys.path.insert(0, os.environ["DVM_ROOT"])
+from paper_1810_00348_b200 import dvm, workloads as W
+from oracle import dvm_oracle
+try:
+    dist.init_process_group("nccl", init_method="tcp://127.0.0.1:" + os.environ["DVM_PORT"], rank=0, world_size=1,
+                            device_id=torch.device("cuda:0"))
+except Exception as e:                       # no usable NCCL on this box: an environment matter, reported as such
+    print("NCCL-UNAVAILABLE", repr(e)); sys.exit(0)
+wl = W.config(0)
+o = dvm_oracle.Oracle(wl)
+s = dvm.Solver(wl, kernel=dvm.KERNEL_TILE)
+buf = s.reduce_buffer()
+assert buf.is_cuda and buf.dtype == torch.float64 and buf.is_contiguous() and buf.numel() == 16 * wl.n_cells
+for it in range(3):
+    s.sweep()
+    dist.all_reduce(buf, op=dist.ReduceOp.SUM)      # the collective of iterate_sharded, on the solver's own accumulator and stream
+    s.update()
+    o.step()
+    g = s.moments().cpu().numpy()
+    assert np.abs(g - o.prim14).max() <= 1e-11 * np.abs(o.prim14).max(), it
+s.close()
+dist.destroy_process_group()
+print("NCCL-OK")
+'''
+
+
+def test_allreduce_of_the_accumulator_through_nccl():
+    """The all-reduce step of the sharded iteration, on the real accumulator through NCCL (one rank: the sum is the identity, the
+    plumbing - a torch view of the solver's own allocation as the NCCL operand, ordered on the solver's stream - is the same)."""
+    import os
+    import socket
+    import subprocess
+    import sys
+    from pathlib import Path
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    env = dict(os.environ, DVM_ROOT=str(Path(__file__).resolve().parents[1]), DVM_PORT=str(port))
+    r = subprocess.run([sys.executable, "-c", _NCCL_ONE_RANK], env=env, capture_output=True, text=True, timeout=300)
+    if "NCCL-UNAVAILABLE" in r.stdout:
+        pytest.skip("NCCL could not be initialised on this box: " + r.stdout.strip()[-200:])
+    assert r.returncode == 0 and "NCCL-OK" in r.stdout, r.stdout[-2000:] + r.stderr[-2000:]
