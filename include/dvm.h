@@ -189,7 +189,7 @@ int dvm_set_option(dvm_solver *s, int option, int value);
 /* Sweep-kernel variant in use: DVM_KERNEL_SLICE / DVM_KERNEL_TILE once the first dvm_iterate has planned the
  * workspace, the requested value (possibly DVM_KERNEL_AUTO) before. */
 int dvm_kernel_used(const dvm_solver *s);
-/* Velocities per thread of the tile kernel: 2 or 4 once the first dvm_iterate has planned, the requested value before. */
+/* Velocities per thread of the tile kernel: 2, 3 or 4 once the first dvm_iterate has planned, the requested value before. */
 int dvm_tile_rv(const dvm_solver *s);
 /* 1 + velocity axis in the wide role of the tile kernel once planned (DVM_OPT_TILE_AXIS), the requested value before. */
 int dvm_tile_axis(const dvm_solver *s);
