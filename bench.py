@@ -132,7 +132,7 @@ NCU = {
 }
 FP32_SLOTS_PER_POINT = 12.25                        # --precision mixed: fp32 instructions per point of the tile kernel (ncu, profiles/r02_mixed_precision.md)
 FP32_LANE_SLOTS_PEAK = 148 * 128 * 1.965e9          # fp32 FMA-lane issue slots per second
-FP64_SLOTS_PER_POINT = {"tile": 15.5, "slice": 70.0}   # executed fp64 instructions per point (SASS count)
+FP64_SLOTS_PER_POINT = {"tile": 14.5, "slice": 70.0}   # executed fp64 instructions per point (SASS count)
 
 
 def algorithmic_bytes_per_point(kernel_name, order=1):

@@ -15,9 +15,9 @@
 //  * exp(-|xi-U|^2/T) and the Shakhov polynomial factorise per axis on the tensor velocity grid: tables.cu tabulates
 //    one entry (E, Q, e, a) per (cell, 1-D node) once per iteration; per level the CTA receives the entries of its
 //    16 cells as TMA row copies, together with the cell records (1/tau, cell index, faces);
-//  * the cell value is written as g = W g_xup + V, so that the recurrence along x is ONE fp64 FMA per value and
-//    everything else (W, V: source term, reciprocal of the denominator by MUFU.RCP64H + one cubic Newton step) is
-//    independent work, done for the RV nodes of a thread in lock step;
+//  * the cell value is written as g = (a_x g_xup + N) / den, so that the recurrence along x is one fp64 FMA and one
+//    multiplication per value and everything else (N: source term + y- and z-upwind terms; 1 / den by MUFU.RCP64H + one
+//    cubic Newton step) is independent work, done for the RV nodes of a thread in lock step;
 //  * the 13 velocity sums are two small matrix products on the fp64 tensor cores (mma.sync m8n8k4 = SASS DMMA, a
 //    pipe of its own beside the fp64 FMA pipe): powers of xi_x times the values over the lane quad, then monomials
 //    of (xi_y, xi_z) over the 8 pairs of a warp; results go to the [cell][16] accumulator in L2 / HBM as fp64 REDs;
@@ -247,6 +247,12 @@ __device__ __forceinline__ double mma_operand(float g, int lane)
 __device__ __forceinline__ void dmma(double &c0, double &c1, const double a, const double b)
 {
     asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+}
+
+// the first product of a chain: D = A * B (the zero accumulator is the zero register, not two moves)
+__device__ __forceinline__ void dmma0(double &c0, double &c1, const double a, const double b)
+{
+    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%4, %4};" : "=d"(c0), "=d"(c1) : "d"(a), "d"(b), "d"(0.0));
 }
 
 // Velocity sums of Eq.(5) as two small matrix products per pair of cells (A, B) and warp.
@@ -545,8 +551,8 @@ __device__ __forceinline__ void emit_pair(const RowBuf<RV, ORD, R> &Rw, const in
                                           const double b0, const double b1, const ThreadCtx<RV, ORD, R> &T, const int lane)
 {
     const bool hi = lane & 16;
-    double d0 = 0.0, d1 = 0.0;
-    dmma(d0, d1, hi ? b0 : a0, T.yz0);
+    double d0, d1;
+    dmma0(d0, d1, hi ? b0 : a0, T.yz0);
     dmma(d0, d1, hi ? b1 : a1, T.yz1);
     const long long c = record<RV, ORD, R>(Rw, hi ? roB : roA).cidx;
     red_f64(T.raw0 + c * 16, d0 * T.use0);
@@ -591,8 +597,8 @@ __device__ __forceinline__ void compute_row(const RowBuf<RV, ORD, R> &Rw, const 
             c1B = yc.x; c2B = yc.y; c1C = zc.x; c2C = zc.y;
         }
         // Everything that does not depend on the x-upwind value, for the RV nodes of the thread in lock step (the fp64
-        // pipe takes a warp instruction every 2 clocks and has a latency of ~10): the cell value is g = W g_xup + V with
-        // W = a_x / den and V = (a_y g_yup + a_z g_zup + src) / den, Eq.(7) PAPER.md:75-79.
+        // pipe has a latency of ~10 clocks): the cell value is g = (W g_xup + V) / den with W = a_x and
+        // V = a_y g_yup + a_z g_zup + src, Eq.(7) PAPER.md:75-79.
         V4 xt[RV];
         V2 xc[RV];
         R t1[RV], t2[RV], d[RV], y0[RV], sE[RV], e[RV], W[RV], V[RV];
@@ -640,7 +646,7 @@ __device__ __forceinline__ void compute_row(const RowBuf<RV, ORD, R> &Rw, const 
             for (int r = 0; r < RV; ++r) V[r] = fma(AX == 0 ? c2B : AX == 1 ? c2A[r] : c2C, yup2[ii][r], V[r]);
         }
 #pragma unroll
-        for (int r = 0; r < RV; ++r) W[r] = (AX == 0 ? c1A[r] : c1B) * y0[r];
+        for (int r = 0; r < RV; ++r) W[r] = AX == 0 ? c1A[r] : c1B;
 #pragma unroll
         for (int r = 0; r < RV; ++r) V[r] = fma(AX == 2 ? c1A[r] : c1C, zrow[ii][r], V[r]);
         if (ORD == 2) {
@@ -649,20 +655,20 @@ __device__ __forceinline__ void compute_row(const RowBuf<RV, ORD, R> &Rw, const 
 #pragma unroll
             for (int r = 0; r < RV; ++r) V[r] = fma(AX == 0 ? c2A[r] : c2B, fx2[r], V[r]);
         }
-#pragma unroll
-        for (int r = 0; r < RV; ++r) V[r] *= y0[r];
-        // the recurrence along x: one FMA per value
+        // the recurrence along x: one FMA and the multiplication by 1 / den per value (scaling W and V by 1 / den beforehand
+        // would take the multiplication off the recurrence at the price of one more per value: measured 3 % slower - the
+        // chain of a row is short against the work of a level)
 #pragma unroll
         for (int r = 0; r < RV; ++r) {
-            const R gg = fma(W[r], fx[r], V[r]);
+            const R gg = fma(W[r], fx[r], V[r]) * y0[r];
             if (ORD == 2) { fx2[r] = fx[r]; z2row[ii][r] = zrow[ii][r]; }
             fx[r] = gg;
             zrow[ii][r] = gg;
         }
         // velocity sums: always in double (a single value is widened exactly)
-        acc[ii & 1][0] = 0.0; acc[ii & 1][1] = 0.0;
+        dmma0(acc[ii & 1][0], acc[ii & 1][1], T.aX[0], mma_operand(zrow[ii][0], lane));
 #pragma unroll
-        for (int r = 0; r < RV; ++r) dmma(acc[ii & 1][0], acc[ii & 1][1], T.aX[r], mma_operand(zrow[ii][r], lane));
+        for (int r = 1; r < RV; ++r) dmma(acc[ii & 1][0], acc[ii & 1][1], T.aX[r], mma_operand(zrow[ii][r], lane));
         if (ii & 1) emit_pair<RV, ORD, R>(Rw, T.ro[ii - 1], T.ro[ii], acc[0][0], acc[0][1], acc[1][0], acc[1][1], T, lane);
         if (YL >= 0 && wy) store_face<RV, ORD, R>(yout + (YL * TILE_TX + ii) * NVB, tid, zrow[ii]);
     }
