@@ -198,3 +198,24 @@ def test_mixed_f_workspace_is_half(oracle_mod):
     a.iterate(1); b.iterate(1)
     assert b.workspace_bytes()[1] * 2 == a.workspace_bytes()[1]
     a.close(); b.close()
+
+
+def test_mixed_config2_runs_to_residual_1e6_like_the_double_run():
+    """BASELINE.json configs[2] "run to residual 1e-6" in single precision: the residual history follows the double run's to
+    the stated tolerance down to 1e-6 (reached at the same iteration +- 1), then stops at its rounding floor of ~1e-7
+    (G22) where the double run goes on falling; the converged fields of the two runs agree to 3 tol32."""
+    from paper_1810_00348_b200 import dvm
+    wl = W.config(2)
+    runs = {}
+    for prec in (dvm.PREC_F64, dvm.PREC_MIXED):
+        s = dvm.Solver(wl, kernel=TILE, precision=prec)
+        s.iterate(160)
+        runs[prec] = (s.residual_history().max(axis=1), s.moments().cpu().numpy())
+        s.close()
+    h64, h32 = runs[dvm.PREC_F64][0], runs[dvm.PREC_MIXED][0]
+    first64, first32 = int(np.argmax(h64 < 1e-6)) + 1, int(np.argmax(h32 < 1e-6)) + 1
+    assert h64[first64 - 1] < 1e-6 and h32[first32 - 1] < 1e-6 and abs(first64 - first32) <= 1, (first64, first32)
+    above = h64 > 2e-6
+    assert np.all(np.abs(h32[above] - h64[above]) <= 0.05 * h64[above])
+    assert h64[-1] < 1e-8 and 1e-8 < h32[-1] < 1e-6          # the double run keeps falling, the single one sits on its floor
+    assert np.abs(runs[dvm.PREC_MIXED][1] - runs[dvm.PREC_F64][1]).max() <= 3 * tol32(wl)
