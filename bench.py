@@ -123,12 +123,12 @@ FP64_PEAK_TFLOPS = 2 * FP64_LANE_SLOTS_PEAK / 1e12
 #   traffic: dram__bytes_read.sum + dram__bytes_write.sum per sweep launch; inst / fp64 / dmma: thread-level instructions per
 #   point-update (smsp__inst_executed.sum x 32 / points, SASS opcode shares of the level loop); pipe / issue: ncu percentages
 NCU = {
-    "cfg4_cavity_128^3x64^3_Kn0.01": {"traffic": 4.3480e12, "inst_per_point": 30.3, "fp64_inst_per_point": 15.5, "dmma_per_point": 1.25,
-                                      "pipe_fp64_active_pct": 37.5, "pipe_tensor_active_pct": 24.1, "pipe_shared_active_pct": 59.7,
-                                      "issue_active_pct": 36.6, "commit": "75e4cc2", "source": "profiles/r02_cfg4_counters.md"},
-    "cfg3_cube_96x64x64_v48^3_Ma2": {"traffic": 3.3874e11, "inst_per_point": 32.4, "fp64_inst_per_point": 16.2, "dmma_per_point": 1.25,
-                                     "pipe_fp64_active_pct": 35.9, "pipe_tensor_active_pct": 23.8, "pipe_shared_active_pct": 57.8,
-                                     "issue_active_pct": 35.8, "commit": "75e4cc2", "source": "profiles/r02_cfg4_counters.md"},
+    "cfg4_cavity_128^3x64^3_Kn0.01": {"traffic": 4.3476e12, "inst_per_point": 29.1, "fp64_inst_per_point": 14.5, "dmma_per_point": 1.25,
+                                      "pipe_fp64_active_pct": 36.6, "pipe_tensor_active_pct": 25.2, "pipe_shared_active_pct": 62.5,
+                                      "issue_active_pct": 36.8, "commit": "2d206e2", "source": "profiles/r02_cfg4_counters.md"},
+    "cfg3_cube_96x64x64_v48^3_Ma2": {"traffic": 3.3836e11, "inst_per_point": 31.2, "fp64_inst_per_point": 15.2, "dmma_per_point": 1.25,
+                                     "pipe_fp64_active_pct": 34.2, "pipe_tensor_active_pct": 24.2, "pipe_shared_active_pct": 58.8,
+                                     "issue_active_pct": 35.1, "commit": "2d206e2", "source": "profiles/r02_cfg4_counters.md"},
 }
 FP32_SLOTS_PER_POINT = 12.25                        # --precision mixed: fp32 instructions per point of the tile kernel (ncu, profiles/r02_mixed_precision.md)
 FP32_LANE_SLOTS_PEAK = 148 * 128 * 1.965e9          # fp32 FMA-lane issue slots per second
