@@ -597,7 +597,7 @@ def test_every_wide_axis_of_the_tile_kernel(oracle_mod, axis, rv, order):
 # ---------------------------------------------------------------------------------------------------------------------
 # Velocity-space sharding (DVM_OPT_SHARD_COUNT): one GPU stands in for n ranks.  The n
 # solvers run one after the other (no kernel waits on another); the sum of their accumulators stands in for the all-reduce.
-@pytest.mark.parametrize("nranks,case", [(2, "cfg0"), (3, "ragged"), (2, "cube"), (4, "cfg1"), (2, "mixed")])
+@pytest.mark.parametrize("nranks,case", [(2, "cfg0"), (3, "ragged"), (2, "cube"), (4, "cfg1"), (2, "mixed"), (3, "order2")])
 def test_velocity_shards_emulated_on_one_gpu(oracle_mod, nranks, case):
     from paper_1810_00348_b200 import dvm
     kw = {}
@@ -609,6 +609,8 @@ def test_velocity_shards_emulated_on_one_gpu(oracle_mod, nranks, case):
         wl, iters = W.cube_flow(4, 12, box=(6, 4, 4), vrange=8.0), 3
     elif case == "cfg1":
         wl, iters = W.config(1), 2
+    elif case == "order2":
+        wl, iters, kw = W.cavity(0, 0, 0.3, stretch=1.5, nxyz=(9, 6, 7), mxyz=(12, 8, 10)).with_(order=2), 3, dict(order=2)
     else:
         wl, iters, kw = W.config(0), 3, dict(precision=dvm.PREC_MIXED)
     o = oracle_mod.Oracle(wl)
