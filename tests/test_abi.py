@@ -50,6 +50,10 @@ def test_create_rejects_bad_input_without_gpu():
     assert L.dvm_create(None, None, None, None, None, ctypes.byref(h)) == dvm.EINVAL
     assert b"NULL" in L.dvm_last_error()
     assert L.dvm_iterate(None, 1) == dvm.EINVAL
+    assert L.dvm_sweep(None) == dvm.EINVAL and L.dvm_update(None) == dvm.EINVAL
+    assert L.dvm_reduce_buffer(None, None, None) == dvm.EINVAL
+    assert L.dvm_set_option(None, dvm.OPT_SHARD_COUNT, 2) == dvm.EINVAL
+    assert L.dvm_precision(None) == dvm.EINVAL
     assert L.dvm_destroy(None) == 0
 
 

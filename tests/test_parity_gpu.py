@@ -211,6 +211,15 @@ def test_config4_full_size_stratified_step(oracle_mod, seed):
     lockstep(wl, 2, 1, oracle_mod, state=st, rho_w=None)
 
 
+def test_paper_cube_full_size_stratified_step(oracle_mod):
+    """The paper's own cube workload (bench --config 5: 191 x 181 x 181 stretched cells with the 31^3 solid cube, 48^3
+    velocities: 6.9e11 phase points swept by the GPU) at full size in the launch configuration bench.py times (RV = 3), one
+    velocity in each of the 288 velocity blocks (the oracle sweeps those: 1.8e9 points), one step from a perturbed state with
+    heat flux."""
+    wl = stratified(W.config(5), 1)
+    lockstep(wl, 2, 1, oracle_mod, state=W.perturbed_state(wl, seed=55, amp_q=0.01), rho_w=None, check_raw=False)
+
+
 @pytest.mark.parametrize("rv", [2, 3])
 def test_config3_stratified_step_other_variants(oracle_mod, rv):
     """The RV = 2 (8 x 8 x 8 velocity blocks) and RV = 3 (12 x 8 x 4) variants of the tile kernel on config 3 at full size, one
