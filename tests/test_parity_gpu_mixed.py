@@ -219,3 +219,52 @@ def test_mixed_config2_runs_to_residual_1e6_like_the_double_run():
     assert np.all(np.abs(h32[above] - h64[above]) <= 0.05 * h64[above])
     assert h64[-1] < 1e-8 and 1e-8 < h32[-1] < 1e-6          # the double run keeps falling, the single one sits on its floor
     assert np.abs(runs[dvm.PREC_MIXED][1] - runs[dvm.PREC_F64][1]).max() <= 3 * tol32(wl)
+
+
+def _golden_full_steps():
+    from pathlib import Path
+    return sorted(int(p.stem.split("cfg")[1]) for p in (Path(__file__).parent / "golden").glob("full_step_cfg*.txt"))
+
+
+@pytest.mark.parametrize("cfg", _golden_full_steps())
+def test_mixed_full_weight_step_against_archived_double_oracle(cfg):
+    """The single-precision sweep over EVERY velocity of configs 2 - 4 (all lanes of all velocity blocks carry weight) against
+    the archived full-weight step of the DOUBLE oracle (tests/golden/full_step_cfg<N>.txt): sampled cells, wall densities,
+    field maxima, residual and rescale factor at tol32."""
+    from pathlib import Path
+    import importlib.util
+    spec = importlib.util.spec_from_file_location("make_goldens", Path(__file__).parent / "golden" / "make_full_step_goldens.py")
+    mg = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mg)
+    wl, prim, cells = mg.seeded_state(cfg)
+    gold = {"cell": {}, "face": {}, "field": {}}
+    for line in (Path(__file__).parent / "golden" / f"full_step_cfg{cfg}.txt").read_text().splitlines():
+        if line.startswith("#") or not line.strip():
+            continue
+        k, *v = line.split()
+        if k == "resid":
+            gold["resid"] = np.array([float(x) for x in v])
+        elif k == "scale":
+            gold["scale"] = float(v[0])
+        else:
+            gold[k][int(v[0])] = np.array([float(x) for x in v[1:]])
+    s = make(wl)
+    s.set_state(prim, None)
+    s.iterate(1)
+    g14 = s.moments().cpu().numpy()
+    rw = s.get_state()[1].cpu().numpy()
+    tol = tol32(wl)
+    worst = 0.0
+    for c, ref in gold["cell"].items():
+        err = np.abs(g14[:, c] - ref).max()
+        worst = max(worst, err)
+        assert err <= tol, (cfg, c, err, tol)
+    assert worst > 1e-10                               # single precision did take part
+    fluid = np.ones(wl.n_cells, bool) if wl.solid is None else wl.solid.reshape(-1) == 0
+    for m in range(14):
+        assert abs(np.abs(g14[m][fluid]).max() - gold["field"][m][0]) <= tol
+    for fidx, val in gold["face"].items():
+        assert abs(rw[fidx] - val[0]) <= tol * max(1.0, abs(val[0]))
+    assert np.all(np.abs(np.asarray(s.residual()) - gold["resid"]) <= 2 * tol * np.maximum(1.0, gold["resid"]))
+    assert abs(s.mass_scale() - gold["scale"]) <= tol * abs(gold["scale"])
+    s.close()
