@@ -5,7 +5,8 @@ perturbed state the GPU test reproduces.  Calls only oracle/ and the input gener
 
     python tests/golden/make_full_step_goldens.py --configs 2 3 4 [--out DIR] [--threads N]
 
-Cost on 16 host cores: config 2 ~2 min, config 3 ~9 min, config 4 ~1.9 h (5.5e11 phase points at ~8e7 points/s).
+Cost: config 2 ~4 min and config 3 ~23 min on 7 threads of an 8-core container; config 4 (5.5e11 phase points) 51 min on the 16 host
+threads of the GPU box (1.8e8 points/s).
 The file holds, as repr(float) text: residual triple, mass-rescale factor, per field (14) the maximum absolute value,
 the sum and the sum of squares over fluid cells, the 14 fields at SAMPLE_CELLS seeded fluid cells, and the wall density at
 SAMPLE_FACES seeded wall faces.  tests/test_parity_gpu.py::test_full_weight_step_against_archived_oracle compares the GPU
