@@ -130,7 +130,7 @@ NCU = {
                                      "pipe_fp64_active_pct": 34.2, "pipe_tensor_active_pct": 24.2, "pipe_shared_active_pct": 58.8,
                                      "issue_active_pct": 35.1, "commit": "2d206e2", "source": "profiles/r02_cfg4_counters.md"},
 }
-FP32_SLOTS_PER_POINT = 12.25                        # --precision mixed: fp32 instructions per point of the tile kernel (ncu, profiles/r02_mixed_precision.md)
+FP32_SLOTS_PER_POINT = 11.25                        # --precision mixed: fp32 instructions per point of the tile kernel (ncu, profiles/r02_mixed_precision.md)
 FP32_LANE_SLOTS_PEAK = 148 * 128 * 1.965e9          # fp32 FMA-lane issue slots per second
 FP64_SLOTS_PER_POINT = {"tile": 14.5, "slice": 70.0}   # executed fp64 instructions per point (SASS count)
 
@@ -287,7 +287,7 @@ def run_gpu(args):
         fp64_slots = FP64_SLOTS_PER_POINT[kname] * pts / secs            # executed fp64 lane slots per second
         frac_hbm, frac_alu = hbm_gbs / peak, fp64_slots / FP64_LANE_SLOTS_PEAK
         if mixed:
-            # single-precision sweep: 12.25 fp32 instructions per point (4 FADD + 4.25 FMUL + 4 FFMA, ncu) on the 128-lane
+            # single-precision sweep: 11.25 fp32 instructions per point (4 FADD + 3.25 FMUL + 4 FFMA, ncu) on the 128-lane
             # fp32 pipe; the fp64 side is one F2F (widening for the tensor-core sums) + 1.25 DMMA per point
             fp64_slots = FP32_SLOTS_PER_POINT * pts / secs
             frac_alu = fp64_slots / FP32_LANE_SLOTS_PEAK
