@@ -52,24 +52,26 @@ def test_f32_values_are_singles_and_order1_double_is_untouched(oracle_mod):
 
 
 def test_f32_one_dimensional_recurrence_in_numpy_float32(oracle_mod):
-    """NY = NZ = 1, zero-gradient y, z faces, uniform state (the P5 setting): Eq.(7) is the two-term recurrence
-    f_i = (S/tau + a f_{i-1}) / (1/tau + a).  Written out with numpy float32 scalars, one rounding per operation, it
-    must reproduce the oracle's single-precision sweep BIT FOR BIT: the rounding points are the ones G22 states."""
-    wl = W.cavity(1, 6, 0.5, nxyz=(12, 1, 1))
+    """NY = NZ = 1, zero-gradient y, z faces (the P5 setting), on a stretched grid with a different state in every cell:
+    Eq.(7) is the two-term recurrence f_i = (S_i/tau_i + a_i f_{i-1}) / (1/tau_i + a_i).  Written out with numpy float32
+    scalars, one rounding per operation, it must reproduce the oracle's single-precision sweep BIT FOR BIT for every
+    velocity of the grid: the rounding points are the ones G22 states.  Mutation-checked on a scratch copy of the oracle:
+    leaving out the rounding of tau, f^S, a_d, g_w, 1/tau, a_d f_up, either running sum or the quotient fails this test; only
+    the rounding of the product rho_w g_w can be left out unnoticed (it changes 4 of 108 ghost terms by half an ulp, which the
+    next rounding absorbs)."""
+    wl = W.cavity(1, 6, 0.5, nxyz=(12, 1, 1), stretch=1.5)
     zg = W.FaceBC(W.ZERO_GRADIENT)
     faces = [W.FaceBC(W.WALL_DIFFUSE, 1.2, 1.0, (0, 0, 0)), W.FaceBC(W.FREESTREAM, 0.9, 1.1, (0.1, 0, 0)), zg, zg, zg, zg]
     wl = wl.with_(faces=faces, rescale_mass=0, f32=True)
     o = oracle_mod.Oracle(wl)
-    Wst = np.array([1.1, 0.05, 0.02, -0.01, 0.9, 0.01, 0.0, 0.02])
-    prim = np.repeat(Wst[:, None], wl.n_cells, axis=1)
+    prim = W.perturbed_state(wl, seed=77, amp_q=0.01)
     rho_w = np.full(o.nface, 0.7)
     f4 = np.float32
-    tau = f4(o.tau(Wst[0], Wst[4]))
-    for (ia, ib, ic) in [(4, 1, 2), (1, 4, 3), (5, 5, 0)]:
+    widths = np.diff(wl.xf)
+    taus = [f4(o.tau(prim[0, i], prim[4, i])) for i in range(12)]
+    for (ia, ib, ic) in [(a_, b_, c_) for a_ in range(6) for b_ in range(6) for c_ in range(6)]:   # every velocity of the grid
         xi = (wl.xi_x[ia], wl.xi_y[ib], wl.xi_z[ic])
         f = o.sweep_velocity(ia, ib, ic, prim, rho_w)[0, 0, :]
-        S = f4(o.feq(Wst, xi))
-        widths = np.diff(wl.xf)
         if xi[0] > 0:
             up = f4(0.7 * float(f4(o.gwall(0, xi))))        # rho_w enters as a double; g_w and the product are rounded
             cells = range(12)
@@ -78,14 +80,15 @@ def test_f32_one_dimensional_recurrence_in_numpy_float32(oracle_mod):
             cells = range(11, -1, -1)
         out = np.zeros(12)
         for i in cells:
+            S = f4(o.feq(prim[:, i], xi))
             a = f4(abs(xi[0]) / widths[i])
-            num = f4(S / tau)
-            den = f4(f4(1.0) / tau)
+            num = f4(S / taus[i])
+            den = f4(f4(1.0) / taus[i])
             num = f4(num + f4(a * up))
             den = f4(den + a)
             up = f4(num / den)
             out[i] = float(up)
-        assert np.array_equal(f, out)
+        assert np.array_equal(f, out), (ia, ib, ic)
 
 
 def test_f32_step_stays_within_the_stated_bound_of_the_double_step(oracle_mod):
