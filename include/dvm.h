@@ -135,7 +135,9 @@ typedef struct {
 int dvm_create(const dvm_grid *grid, const dvm_vgrid *vgrid, const dvm_gas *gas, const dvm_bc *bc,
                const dvm_device *dev, dvm_solver **out);
 
-/* n >= 0 outer iterations (Alg. 1 + moment update + residual), asynchronous on the stream. */
+/* n >= 0 outer iterations (Alg. 1 + moment update + residual), asynchronous on the stream.  Tile kernel: the first call captures
+ * one iteration from the stream as a CUDA graph and every iteration is one graph launch from then on (DVM_GRAPH=0 in the
+ * environment: plain kernel launches). */
 int dvm_iterate(dvm_solver *s, int n);
 
 /* The two halves of one outer iteration, for velocity-space sharding (DVM_OPT_SHARD_COUNT): dvm_sweep clears the velocity-sum

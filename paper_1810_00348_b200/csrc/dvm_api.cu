@@ -83,6 +83,11 @@ struct dvm_solver {
     int precision = DVM_PREC_F64; // DVM_PREC_MIXED: f carried in single precision by the tile kernel
     int shard_rank = 0, shard_count = 1;   // velocity-space sharding (DVM_OPT_SHARD_COUNT / _RANK)
     bool swept = false;           // dvm_sweep done, dvm_update pending
+    // one outer iteration of the tile kernel as a CUDA graph: captured at the first dvm_iterate, replayed afterwards (the
+    // launch parameters of an iteration never change: constant flag epoch + flag reset, device-side history slot)
+    cudaGraphExec_t graph_exec = nullptr;
+    long long graph_launches = 0; // kernel launches inside the graph
+    bool graph_off = false;       // DVM_GRAPH=0 in the environment, or the capture failed: plain launches
     size_t fvalue() const { return precision == DVM_PREC_MIXED ? sizeof(float) : sizeof(double); }
     bool planned = false;
     long long launches = 0;
@@ -710,7 +715,9 @@ int sweep_phase(dvm_solver *s)
         CK(launch_tables(table_params(s), s->stream));
         s->launches += 1;
         CK(cudaMemsetAsync(s->d_counter, 0, sizeof(int), s->stream));
-        s->epoch += 1;
+        // completion flags back to 0; the epoch they are compared with stays 1 (constant launch parameters: CUDA graph)
+        CK(cudaMemsetAsync(s->d_done, 0, s->tile.items.size() * sizeof(int), s->stream));
+        s->epoch = 1;
         const TileParams TP = tile_params(s);
         CK(launch_sweep_tile(TP, s->tile_rv, s->order, s->precision == DVM_PREC_MIXED, s->tile.ax[0], s->tile_grid, s->stream));
     }
@@ -727,7 +734,7 @@ int update_phase(dvm_solver *s)
         s->launches += 1;
     }
     int l = 0;
-    CK(launch_update(U, s->iters % HIST_CAP, s->stream, &l));
+    CK(launch_update(U, HIST_CAP, s->stream, &l));
     s->launches += l;
     s->iters += 1;
     return 0;
@@ -744,7 +751,33 @@ int dvm_iterate(dvm_solver *s, int niter)
     if (s->swept) return fail(DVM_EINVAL, "dvm_sweep without dvm_update");
     DeviceGuard guard(s->device);
     if (int rc = plan(s)) return rc;
+    if (s->kernel == DVM_KERNEL_TILE && !s->graph_off && !s->graph_exec) {
+        // capture one iteration (3 + 1 memsets, factor tables, sweep, wall fluxes, 5 update kernels) and replay it from now
+        // on: one launch per iteration instead of twelve (configs 0 and 1 are launch-bound: 0.14 ms per iteration)
+        if (const char *e = std::getenv("DVM_GRAPH")) s->graph_off = std::atoi(e) == 0;
+        if (!s->graph_off) {
+            const long long l0 = s->launches;
+            const int it0 = s->iters;
+            cudaGraph_t g = nullptr;
+            bool ok = cudaStreamBeginCapture(s->stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
+            if (ok) {
+                const int rc1 = sweep_phase(s), rc2 = rc1 ? rc1 : update_phase(s);
+                ok = cudaStreamEndCapture(s->stream, &g) == cudaSuccess && rc2 == 0 && g != nullptr;
+            }
+            if (ok) ok = cudaGraphInstantiate(&s->graph_exec, g, 0) == cudaSuccess;
+            if (g) cudaGraphDestroy(g);
+            s->graph_launches = s->launches - l0;
+            s->launches = l0; s->iters = it0;           // nothing ran yet
+            if (!ok) { cudaGetLastError(); s->graph_exec = nullptr; s->graph_off = true; }
+        }
+    }
     for (int it = 0; it < niter; ++it) {
+        if (s->graph_exec) {
+            CK(cudaGraphLaunch(s->graph_exec, s->stream));
+            s->launches += s->graph_launches;
+            s->iters += 1;
+            continue;
+        }
         if (int rc = sweep_phase(s)) return rc;
         if (int rc = update_phase(s)) return rc;
     }
@@ -983,6 +1016,7 @@ int dvm_destroy(dvm_solver *s)
     if (!s) return DVM_OK;
     DeviceGuard guard(s->device);
     cudaStreamSynchronize(s->stream);
+    if (s->graph_exec) cudaGraphExecDestroy(s->graph_exec);
     s->dfree_all();
     delete s;
     return DVM_OK;

@@ -147,9 +147,12 @@ __global__ void __launch_bounds__(UB) finish_kernel(const UpdateParams U)
     }
 }
 
-// single block: residual of this iteration -> history[it], non-finite flag
-__global__ void __launch_bounds__(UB) residual_kernel(const UpdateParams U, int nparts, int slot)
+// single block: residual of this iteration -> history[slot].  The slot is a device-side counter (scal[3], an exact small
+// integer in a double) that the kernel advances itself, so that the launch parameters of an iteration do not change from
+// one iteration to the next and the whole iteration can be replayed as a CUDA graph (dvm_api.cu).
+__global__ void __launch_bounds__(UB) residual_kernel(const UpdateParams U, int nparts, int hist_cap)
 {
+    const int slot = (int)U.scal[3];
     __shared__ double sh[UB / 32];
     __shared__ double tot[6];
     for (int m = 0; m < 6; ++m) {
@@ -168,6 +171,7 @@ __global__ void __launch_bounds__(UB) residual_kernel(const UpdateParams U, int 
             U.hist[3 * slot + m] = r;
         }
         U.hist_scale[slot] = U.scal[0];
+        U.scal[3] = (double)((slot + 1) % hist_cap);
     }
 }
 
@@ -242,13 +246,13 @@ cudaError_t launch_phi_from_raw(const UpdateParams &U, const int *face_cell, con
     return cudaGetLastError();
 }
 
-cudaError_t launch_update(const UpdateParams &U, int hist_slot, cudaStream_t st, int *launches)
+cudaError_t launch_update(const UpdateParams &U, int hist_cap, cudaStream_t st, int *launches)
 {
     const int nb = nblk(U.ncell);
     convert_kernel<<<nb, UB, 0, st>>>(U);
     mass_kernel<<<1, UB, 0, st>>>(U, nb);
     finish_kernel<<<nb, UB, 0, st>>>(U);
-    residual_kernel<<<1, UB, 0, st>>>(U, nb, hist_slot);
+    residual_kernel<<<1, UB, 0, st>>>(U, nb, hist_cap);
     faces_kernel<<<nblk(U.nface), UB, 0, st>>>(U);
     *launches += 5;
     return cudaGetLastError();

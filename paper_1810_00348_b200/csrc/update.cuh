@@ -30,7 +30,7 @@ struct SweepParams;
 cudaError_t launch_raw_export(const double *raw16, double *out13, long long n, cudaStream_t st);
 cudaError_t launch_pack(const UpdateParams &U, cudaStream_t st);
 cudaError_t launch_phi_from_raw(const UpdateParams &U, const int *face_cell, const int *face_dir, double *phi, int order, cudaStream_t st);
-cudaError_t launch_update(const UpdateParams &U, int hist_slot, cudaStream_t st, int *launches);
+cudaError_t launch_update(const UpdateParams &U, int hist_cap, cudaStream_t st, int *launches);   // the history slot is a device-side counter
 cudaError_t launch_sweep_slice(const SweepParams &P, int nblocks, int nb, cudaStream_t st);
 
 }  // namespace dvm
