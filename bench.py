@@ -125,10 +125,10 @@ FP64_PEAK_TFLOPS = 2 * FP64_LANE_SLOTS_PEAK / 1e12
 NCU = {
     "cfg4_cavity_128^3x64^3_Kn0.01": {"traffic": 4.3476e12, "inst_per_point": 29.1, "fp64_inst_per_point": 14.5, "dmma_per_point": 1.25,
                                       "pipe_fp64_active_pct": 36.6, "pipe_tensor_active_pct": 25.2, "pipe_shared_active_pct": 62.5,
-                                      "issue_active_pct": 36.8, "commit": "2d206e2", "source": "profiles/r02_cfg4_counters.md"},
+                                      "issue_active_pct": 36.8, "commit": "42e5d51", "source": "profiles/r02_cfg4_counters.md"},
     "cfg3_cube_96x64x64_v48^3_Ma2": {"traffic": 3.3836e11, "inst_per_point": 31.2, "fp64_inst_per_point": 15.2, "dmma_per_point": 1.25,
                                      "pipe_fp64_active_pct": 34.2, "pipe_tensor_active_pct": 24.2, "pipe_shared_active_pct": 58.8,
-                                     "issue_active_pct": 35.1, "commit": "2d206e2", "source": "profiles/r02_cfg4_counters.md"},
+                                     "issue_active_pct": 35.1, "commit": "42e5d51", "source": "profiles/r02_cfg4_counters.md"},
 }
 FP32_SLOTS_PER_POINT = 11.25                        # --precision mixed: fp32 instructions per point of the tile kernel (ncu, profiles/r02_mixed_precision.md)
 FP32_LANE_SLOTS_PEAK = 148 * 128 * 1.965e9          # fp32 FMA-lane issue slots per second
