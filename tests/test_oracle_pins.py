@@ -363,6 +363,80 @@ def test_residual_definition(oracle_mod):
     assert o2.resid[1] == 1.0
 
 
+def test_residual_sums_are_unweighted_on_a_stretched_grid(oracle_mod):
+    """Step 7 on a NON-uniform grid (the criterion is written with plain sums over the cells, no cell volume in
+    it; reading G9).  On the uniform grid of test_residual_definition a cell-volume weight cancels out of every
+    ratio, so that test cannot tell the two apart; here the tanh-stretched cells differ in volume by more than a factor 10 and
+    the volume-weighted restatement must be visibly different (the assertion that this pin has teeth).  configs[2] and
+    configs[4] run on such grids."""
+    wl = W.cavity(5, 8, 1.0, stretch=1.5)
+    o = oracle_mod.Oracle(wl)
+    o.step()
+    a = o.prim8.copy()
+    b = o.step()
+    dx, dy, dz = np.diff(wl.xf), np.diff(wl.yf), np.diff(wl.zf)
+    vol = (dz[:, None, None] * dy[None, :, None] * dx[None, None, :]).reshape(-1)
+    assert vol.max() / vol.min() > 10.0
+
+    def cons(p):
+        rho, u, T = p[0], p[1:4], p[4]
+        return rho, rho * u, 0.75 * rho * T + 0.5 * rho * (u * u).sum(0)
+
+    def ratios(wgt):
+        out = []
+        for qa, qb in zip(cons(a), cons(b)):
+            num = (wgt * (qb - qa) ** 2).sum()
+            den = (wgt * qb ** 2).sum()
+            out.append(np.sqrt(num / den))
+        return np.array(out)
+
+    plain, weighted = ratios(1.0), ratios(vol)
+    assert np.allclose(o.resid, plain, rtol=1e-12)
+    assert np.all(np.abs(weighted - plain) > 1e-3 * plain), (plain, weighted)
+    assert not np.allclose(o.resid, weighted, rtol=1e-4)
+
+
+@pytest.mark.parametrize("m", [48, 96])
+def test_initial_wall_density_with_gas_moving_into_the_wall(oracle_mod, m):
+    """Step 1 with u_0 . n != 0 (Eq.(9): rho_w balances the flux the gas carries ONTO the wall; SURVEY 8(c)
+    step 1: rho_w^0 = Phi^0 / Phi_unit with Phi^0 the wall-incident flux of f^M(W^0)).  For a drifting Maxwellian the
+    half-range flux through a plane with outward normal n has the textbook closed form
+        Phi^0 = rho_0 [ sqrt(T_0 / 4 pi) exp(-S^2) + (U_n / 2)(1 + erf S) ],  S = U_n / sqrt(T_0),  U_n = u_0 . n,
+    and a stationary wall at T_w emits Phi_unit = sqrt(T_w / 4 pi) per unit rho_w.  A wall the gas moves TOWARDS therefore
+    starts with a much larger rho_w than the wall in its lee: with u_0 = (0.8, -0.3, 0), T_0 = 1.2 the x+ side gets 14 times
+    the x- side.  Swapping the direction of the incident flux in step 1 exchanges the two.  Checked on the six domain walls
+    and on the faces of a solid block, against the closed form to the second-order error of the half-range trapezoid sums
+    (halving the node spacing must quarter the error).  Every other pin that starts from the initial state has u_0 = 0 or
+    walls parallel to u_0; configs[3] (Mach-2 free stream onto the cube) is this case."""
+    from math import erf, exp, pi, sqrt
+    u0, T0, rho0, Tw = (0.8, -0.3, 0.0), 1.2, 1.1, 1.0
+    solid = np.zeros((4, 4, 4), dtype=np.uint8)
+    solid[1:3, 1:3, 2:3] = 1
+    wl = W.cavity(4, m, 1.0, vrange=7.0, U_w=0.0).with_(solid=solid, u0=u0, T0=T0, rho0=rho0)
+    o = oracle_mod.Oracle(wl)
+    cell, dirn, _ = o.face_table()
+    assert o.nface > 6 * 16 and (cell >= 0).sum() > 6 * 16 - 1      # domain faces + the block's faces
+
+    def closed(d):
+        un = u0[d // 2] * (1.0 if d & 1 else -1.0)
+        S = un / sqrt(T0)
+        return rho0 * (sqrt(T0 / (4 * pi)) * exp(-S * S) + 0.5 * un * (1.0 + erf(S))) / sqrt(Tw / (4 * pi))
+
+    h = 14.0 / (m - 1)
+    worst = 0.0
+    for d in range(6):
+        sel = (cell >= 0) & (dirn == d)
+        assert sel.sum() >= 16
+        vals = o.rho_w[sel]
+        assert np.ptp(vals) <= 1e-14 * vals.max()                    # uniform initial state: one value per direction
+        worst = max(worst, abs(vals[0] - closed(d)) / closed(d))
+    assert worst < 0.35 * h * h, (worst, h)                          # second order in the node spacing
+    by_dir = [o.rho_w[(cell >= 0) & (dirn == d)][0] for d in range(6)]
+    assert by_dir[1] > 12 * by_dir[0]          # x+ faces: the gas runs into them; x- faces: in the lee
+    assert by_dir[2] > 2 * by_dir[3]           # u_y < 0: the y- faces are hit harder
+    assert by_dir[4] == pytest.approx(by_dir[5], rel=1e-14)
+
+
 def test_config0_history_reference_digits(oracle_mod):
     """Config 0 runs its 20 iterations stably and monotonically; the mass-rescale factor settles at the value
     fixed by the 8-node quadrature (sum w f^S != rho)."""
