@@ -223,6 +223,34 @@ long long dvm_launch_count(const dvm_solver *s);
 int dvm_destroy(dvm_solver *s);
 const char *dvm_last_error(void);
 
+/* ---- convergence residual without a solver and without any allocation ---------------------------------------------------
+ * The residual of PAPER.md:269 (reading G9: r_rho = sqrt(sum (rho1 - rho0)^2 / sum rho1^2) over the cells, the same
+ * for the momentum rho u and the energy rho E = 3/4 rho T + 1/2 rho |u|^2, unweighted sums) between two macroscopic states
+ * the caller already holds, e.g. two outputs of dvm_moments.  It is the arithmetic and the two-level fixed-order reduction of
+ * the solver's own residual kernels; what differs is where the per-block partial sums go.
+ *
+ * This call never enters the CUDA allocator (no cudaMalloc / cudaFree, no allocating library routine), so it is usable by
+ * hosts that cannot allocate: a program that gave all device memory to its own pool at start-up (cudaMalloc would fail), a
+ * latency-critical loop (cudaMalloc / cudaFree stall the whole device), or code called from a context where the allocator
+ * may not be entered.  The partial sums live in a fixed 3 MiB array inside the library image; consequences:
+ *   - every GPU onto which libdvm_b200.so is loaded holds those 3 MiB until the process exits;
+ *   - ncell <= DVM_RESIDUAL_NOALLOC_MAX_CELLS (256^3); anything larger is refused with DVM_EINVAL and a message that names the
+ *     limit - use a solver's dvm_residual there;
+ *   - all calls share the array.  Calls are safe one after the other on one stream (no slot is read that the same call has not
+ *     written first, so nothing needs clearing between calls); two calls that may run at the same time on one GPU (different
+ *     streams, different host threads) race on it and return garbage - the caller serialises them;
+ *   - the first call on each GPU also does the one-time set-up for that GPU (it asks the runtime for the array's device address,
+ *     which makes the driver load the module).  Make that first call during start-up, before any stream capture begins.
+ *
+ * dev_prim_old, dev_prim_new: dev, SoA with field stride ncell, at least the first 5 fields of dvm_moments' layout (rho, ux, uy,
+ * uz, T at [m*ncell + c]; a prim8 or prim14 buffer fits as it is); solid cells must hold zeros in both (dvm_moments writes
+ * them so).  dev_out3: dev, 3 doubles = r_rho, r_mom, r_E; a zero denominator gives 0 (numerator 0) or +inf, a NaN in the
+ * input propagates (no DVM_ENONFINITE here: nothing is read back).  stream: cudaStream_t (0 = default stream).  All three buffers
+ * must belong to one GPU; the call runs there whatever device is current and restores the caller's device.  Asynchronous.
+ * Errors: DVM_EINVAL (NULL, ncell <= 0 or beyond the limit, a buffer that is not device memory of that GPU), DVM_ECUDA. */
+#define DVM_RESIDUAL_NOALLOC_MAX_CELLS 16777216LL
+int dvm_residual_noalloc(const double *dev_prim_old, const double *dev_prim_new, long long ncell, double *dev_out3, void *stream);
+
 #ifdef __cplusplus
 }
 #endif

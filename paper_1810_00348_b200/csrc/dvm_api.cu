@@ -60,6 +60,15 @@ const double PI = 3.14159265358979323846;
 
 }  // namespace
 
+namespace dvm {
+// for the other translation units of the library (residual_noalloc.cu): leave a message for dvm_last_error()
+int report_error(int code, const char *msg)
+{
+    g_err = msg;
+    return code;
+}
+}  // namespace dvm
+
 struct dvm_solver {
     int nx = 0, ny = 0, nz = 0, mx = 0, my = 0, mz = 0, nface = 0;
     long long ncell = 0;

@@ -41,6 +41,7 @@ SYMBOLS = (
     "dvm_mass_scale", "dvm_step_host", "dvm_set_option", "dvm_workspace_bytes", "dvm_launch_count",
     "dvm_kernel_used", "dvm_tile_rv", "dvm_tile_axis", "dvm_precision", "dvm_plan_query", "dvm_plan_vblocks",
     "dvm_plan_shard_vblocks", "dvm_sweep", "dvm_update", "dvm_reduce_buffer", "dvm_destroy", "dvm_last_error",
+    "dvm_residual_noalloc",
 )
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
@@ -142,6 +143,7 @@ def lib():
         L.dvm_launch_count.restype = C.c_longlong
         L.dvm_destroy.argtypes = [vp]
         L.dvm_last_error.restype = C.c_char_p
+        L.dvm_residual_noalloc.argtypes = [vp, vp, C.c_longlong, vp, vp]
         _lib = L
     return _lib
 
@@ -188,6 +190,36 @@ def plan_shard_vblocks(xi_x, xi_y, xi_z, rank, count, rv=0, order=1, wide_axis=0
     out = np.zeros((n, 8), dtype=np.int32)
     _check(lib().dvm_plan_shard_vblocks(C.byref(v), rv, order, wide_axis, rank, count, out.ctypes.data_as(C.POINTER(C.c_int)), n))
     return out
+
+
+RESIDUAL_NOALLOC_MAX_CELLS = 1 << 24
+
+
+def residual_noalloc(prim_old, prim_new, out3, stream=None):
+    """dvm_residual_noalloc: the residual triple (r_rho, r_mom, r_E) between two macroscopic states on the GPU,
+    written to `out3`, for hosts that cannot allocate device memory (all of HBM already in their own pool, a latency-critical
+    loop, a context where the CUDA allocator may not be entered): the call makes no allocation, its partial sums sit in a fixed
+    3 MiB array of the library image.  Limits that follow (include/dvm.h has the full text): at most RESIDUAL_NOALLOC_MAX_CELLS
+    cells (DvmError EINVAL beyond); every call shares that array, so calls that could overlap on the GPU must be serialised by the
+    caller; the first call on a GPU does a one-time set-up and belongs in start-up code, before any stream capture.
+
+    prim_old, prim_new: CUDA float64 tensors [>= 5][ncell] (rho, ux, uy, uz, T first; the outputs of Solver.moments() or
+    get_state() fit as they are), contiguous, same shape; out3: CUDA float64 tensor of 3 elements on the same GPU, supplied by the
+    caller - this function allocates nothing either.  stream: a torch.cuda.Stream (default: torch's current stream of that GPU).
+    Asynchronous; returns out3."""
+    import torch
+    if not (prim_old.is_cuda and prim_new.is_cuda and out3.is_cuda):
+        raise DvmError(EINVAL, "residual_noalloc: CUDA tensors required (there is no CPU fallback)")
+    if prim_old.dtype != torch.float64 or prim_new.dtype != torch.float64 or out3.dtype != torch.float64:
+        raise DvmError(EINVAL, "residual_noalloc: float64 tensors required")
+    if prim_old.shape != prim_new.shape or prim_old.dim() != 2 or prim_old.shape[0] < 5 or out3.numel() < 3:
+        raise DvmError(EINVAL, "residual_noalloc: prim_old / prim_new must be [>= 5][ncell] and alike, out3 must hold 3 values")
+    if not (prim_old.is_contiguous() and prim_new.is_contiguous() and out3.is_contiguous()):
+        raise DvmError(EINVAL, "residual_noalloc: contiguous tensors required")
+    st = torch.cuda.current_stream(out3.device) if stream is None else stream
+    _check(lib().dvm_residual_noalloc(prim_old.data_ptr(), prim_new.data_ptr(), int(prim_old.shape[1]), out3.data_ptr(),
+                                      st.cuda_stream))
+    return out3
 
 
 class Solver:
