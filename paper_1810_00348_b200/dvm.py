@@ -314,18 +314,38 @@ class Solver:
         block = self._blocks[ptr.value]
         return block[: 8 * n.value].view(self.torch.float64)
 
+    def plan_signature(self):
+        """What every rank of a sharded run must agree on for the ranks' velocity blocks to partition the velocity grid: kernel
+        variant, velocities per thread, wide axis, precision (valid once the first sweep has planned the workspace)."""
+        return (self.kernel_used(), self.tile_rv(), self.tile_axis(), self.precision())
+
     def iterate_sharded(self, n: int = 1, group=None):
         """n outer iterations of a velocity-sharded solver: every rank sweeps its velocity blocks, one all-reduce (sum, fp64;
-        NCCL through torch.distributed, on the solver's stream) of the velocity sums per iteration, then every rank updates the
-        replicated macroscopic state.  With one rank this is iterate(n)."""
+        NCCL through torch.distributed) of the velocity sums per iteration, then every rank updates the replicated macroscopic
+        state.  With one rank this is iterate(n).
+
+        Stream order: the kernels of dvm_sweep / dvm_update run on the stream the solver was created with, torch's collective
+        orders itself against torch's CURRENT stream; the loop therefore runs with the solver's stream made current, whatever
+        stream the caller is on.  After the first sweep (which plans the workspace) the ranks compare their plan_signature():
+        ranks that chose different block shapes would count velocities twice or not at all."""
         if self.shard[1] == 1:
             return self.iterate(n)
+        import contextlib
+        import torch
         import torch.distributed as dist
         buf = self.reduce_buffer()
-        for _ in range(n):
-            self.sweep()
-            dist.all_reduce(buf, op=dist.ReduceOp.SUM, group=group)
-            self.update()
+        on_stream = torch.cuda.stream(self.stream) if buf.is_cuda else contextlib.nullcontext()
+        with on_stream:
+            for _ in range(n):
+                self.sweep()
+                if not getattr(self, "_shard_plan_checked", False):
+                    sigs = [None] * dist.get_world_size(group)
+                    dist.all_gather_object(sigs, tuple(self.plan_signature()), group=group)
+                    if any(sg != sigs[0] for sg in sigs):
+                        raise DvmError(EINVAL, f"sharded ranks planned different sweeps (kernel, rv, axis, precision): {sigs}")
+                    self._shard_plan_checked = True
+                dist.all_reduce(buf, op=dist.ReduceOp.SUM, group=group)
+                self.update()
 
     def moments(self, out=None):
         out = self._dev_empty(14 * self.ncell) if out is None else out

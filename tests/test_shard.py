@@ -91,17 +91,28 @@ def _worker(rank, world, port, out):
             self.results.append(self.buf.clone().numpy()); self.calls.append("update")
         def reduce_buffer(self):
             return self.buf
+        def plan_signature(self):
+            return sig
         def close(self):
             pass
         def __del__(self):
             pass
 
+    sig = (2, 4, 1, 0)
     s = HostShard()
     s.iterate_sharded(2)
+    # ranks whose libraries planned different block shapes must be stopped before the first all-reduce
+    sig = (2, 4 - rank, 1, 0)
+    bad = HostShard()
+    try:
+        bad.iterate_sharded(1)
+        mismatch = "not detected"
+    except dvm.DvmError as e:
+        mismatch = "detected" if "different sweeps" in str(e) and bad.calls == ["sweep"] else f"wrong state {e} {bad.calls}"
     dist.barrier()
     dist.destroy_process_group()
     err = max(float(np.abs(r.reshape(13, -1) - full.raw13).max()) for r in s.results)
-    out.put((rank, s.calls, err, float(part[0].max()), float(full.raw13[0].max()), float(np.abs(full.raw13).max())))
+    out.put((rank, s.calls, err, float(part[0].max()), float(full.raw13[0].max()), float(np.abs(full.raw13).max()), mismatch))
 
 
 def test_sweep_allreduce_update_loop_over_two_gloo_ranks():
@@ -118,7 +129,8 @@ def test_sweep_allreduce_update_loop_over_two_gloo_ranks():
     for p in procs:
         p.join(timeout=60)
         assert p.exitcode == 0
-    for rank, calls, err, rho_part, rho_full, fmax in res:
+    for rank, calls, err, rho_part, rho_full, fmax, mismatch in res:
         assert calls == ["sweep", "update", "sweep", "update"]
+        assert mismatch == "detected"
         assert err <= 1e-13 * fmax
         assert rho_part < 0.75 * rho_full          # a rank alone holds only a part of the density sum
