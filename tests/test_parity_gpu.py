@@ -211,6 +211,35 @@ def test_config4_full_size_stratified_step(oracle_mod, seed):
     lockstep(wl, 2, 1, oracle_mod, state=st, rho_w=None)
 
 
+def test_initial_wall_density_closed_form_gpu(oracle_mod):
+    """rho_w^0 straight after dvm_create on configs[3] (Mach-2 free stream hitting the cube: u_0 . n != 0) against the closed
+    half-range flux of the drifting Maxwellian, rho_0 [sqrt(T_0/4 pi) e^{-S^2} + (U_n/2)(1 + erf S)] / sqrt(T_w/4 pi) with
+    S = U_n / sqrt T_0 (Eq.(9); oracle step 1; CPU pin test_initial_wall_density_with_gas_moving_into_the_wall):
+    the library computes rho_w^0 in its own host code, and lock-step tests only show that it equals the oracle's.  The cube's
+    upstream faces start at 6.48, its lee faces at 0.004, the side faces at 1; tolerance = the second-order error of the
+    half-range trapezoid sums, 0.02 h^2."""
+    from math import erf, exp, pi, sqrt
+    wl = W.config(3)
+    s = make(wl, 2)
+    o = oracle_mod.Oracle(wl)
+    cell, dirn, _ = o.face_table()
+    rw = s.get_state()[1].cpu().numpy()
+    s.close()
+    assert rw.shape == cell.shape
+    h = wl.xi_x[1] - wl.xi_x[0]
+    walls = np.flatnonzero((cell >= 0) & (rw > 0))
+    assert len(walls) == 6 * 16 * 16            # the faces of the 16^3 cube; the domain faces are not walls
+    for d in range(6):
+        un = wl.u0[d // 2] * (1.0 if d & 1 else -1.0)
+        S = un / sqrt(wl.T0)
+        closed = wl.rho0 * (sqrt(wl.T0 / (4 * pi)) * exp(-S * S) + 0.5 * un * (1.0 + erf(S))) / sqrt(wl.solid_bc.T / (4 * pi))
+        sel = walls[dirn[walls] == d]
+        assert len(sel) == 256
+        assert np.abs(rw[sel] - closed).max() <= 0.02 * h * h, (d, rw[sel][0], closed)
+    front, rear = rw[walls[dirn[walls] == 1]][0], rw[walls[dirn[walls] == 0]][0]
+    assert front > 1000 * rear
+
+
 def test_paper_cube_full_size_stratified_step(oracle_mod):
     """The paper's own cube workload (bench --config 5: 191 x 181 x 181 stretched cells with the 31^3 solid cube, 48^3
     velocities: 6.9e11 phase points swept by the GPU) at full size in the launch configuration bench.py times (RV = 3), one
