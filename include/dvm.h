@@ -220,6 +220,11 @@ int dvm_plan_shard_vblocks(const dvm_vgrid *v, int rv, int order, int wide_axis,
 int dvm_workspace_bytes(const dvm_solver *s, size_t *total, size_t *f_bytes);
 /* Number of kernel launches enqueued by this solver so far (bench.py's gpu_launches). */
 long long dvm_launch_count(const dvm_solver *s);
+/* How dvm_iterate issues an iteration: 1 = it replays the CUDA graph captured at the first dvm_iterate; 0 = plain kernel launches
+ * because no graph is in use (before the first dvm_iterate, slice kernel, DVM_GRAPH=0, sharded solver); 2 = plain kernel launches
+ * because the capture was tried and FAILED (e.g. the caller's stream was itself being captured) - results are the same, every
+ * iteration costs twelve launches instead of one, and dvm_last_error() held the reason when the first dvm_iterate returned. */
+int dvm_graph_active(const dvm_solver *s);
 int dvm_destroy(dvm_solver *s);
 const char *dvm_last_error(void);
 
@@ -250,6 +255,14 @@ const char *dvm_last_error(void);
  * Errors: DVM_EINVAL (NULL, ncell <= 0 or beyond the limit, a buffer that is not device memory of that GPU), DVM_ECUDA. */
 #define DVM_RESIDUAL_NOALLOC_MAX_CELLS 16777216LL
 int dvm_residual_noalloc(const double *dev_prim_old, const double *dev_prim_new, long long ncell, double *dev_out3, void *stream);
+
+/* ---- measurement aid (bench.py's roofline) ---------------------------------------------------------
+ * (syncs) The fp64 rate this board sustains on a register-resident stream of fused multiply-adds: every SM full (2048 threads),
+ * 8 independent chains per thread, `rounds` DFMAs per chain, no memory traffic, timed with CUDA events on the default stream of
+ * the current device.  *host_lane_ops_per_s = executed fp64 thread-instructions per second (one DFMA = one lane-operation; the
+ * nominal figure is 148 SM x 64 lanes x clock), *host_ms (may be NULL) = duration of the timed launch.  dev_sink: dev, >= 1 double,
+ * never written in practice.  rounds = 2 000 000 runs for about 0.3 s on a B200. */
+int dvm_fp64_peak_probe(double *dev_sink, long long rounds, double *host_lane_ops_per_s, double *host_ms);
 
 #ifdef __cplusplus
 }

@@ -97,6 +97,7 @@ struct dvm_solver {
     cudaGraphExec_t graph_exec = nullptr;
     long long graph_launches = 0; // kernel launches inside the graph
     bool graph_off = false;       // DVM_GRAPH=0 in the environment, or the capture failed: plain launches
+    bool graph_failed = false;    // the capture was tried and failed (dvm_graph_active reports it)
     size_t fvalue() const { return precision == DVM_PREC_MIXED ? sizeof(float) : sizeof(double); }
     bool planned = false;
     long long launches = 0;
@@ -274,10 +275,6 @@ TableParams table_params(dvm_solver *s)
 constexpr double RV_SPEED[5] = {0.0, 0.0, 0.80, 0.90, 1.0};
 void choose_variant(const std::vector<double> xi[3], int order, int rv_fixed, int axis_fixed, int *rv_out, int *axis_out, bool f32 = false)
 {
-    if (rv_fixed == 0)
-        if (const char *e = std::getenv("DVM_TILE_RV")) { const int v = std::atoi(e); if (v >= 2 && v <= 4) rv_fixed = v; }
-    if (axis_fixed < 0)
-        if (const char *e = std::getenv("DVM_TILE_AXIS")) { const int v = std::atoi(e); if (v >= 0 && v <= 2) axis_fixed = v; }
     if (order == 2) rv_fixed = 2;
     const long long nvel = (long long)xi[0].size() * xi[1].size() * xi[2].size();
     int best_rv = rv_fixed ? rv_fixed : 4, best_ax = axis_fixed >= 0 ? axis_fixed : 0;
@@ -299,11 +296,14 @@ void choose_variant(const std::vector<double> xi[3], int order, int rv_fixed, in
 int plan_once(dvm_solver *s);
 
 // Decide the kernel variant and build the block table + f workspace (once, before the first iteration).  A failed attempt
-// gives back what it allocated, so that the call can be repeated (e.g. with another workspace cap).
+// gives back what it allocated and puts back what the caller had requested (kernel, velocities per thread, wide axis: plan_once
+// replaces "the library chooses" by its choice), so that the call can be repeated, e.g. with another workspace cap or
+// precision, and is planned afresh.
 int plan(dvm_solver *s)
 {
     if (s->planned) return 0;
     const size_t nalloc = s->allocs.size(), bytes = s->total_bytes;
+    const int req_kernel = s->kernel, req_rv = s->tile_rv, req_axis = s->tile_axis;
     const int rc = plan_once(s);
     if (rc != 0) {
         cudaStreamSynchronize(s->stream);
@@ -314,6 +314,13 @@ int plan(dvm_solver *s)
         s->allocs.resize(nalloc);
         s->total_bytes = bytes;
         s->f_bytes = 0;
+        s->table_bytes = 0;
+        s->kernel = req_kernel; s->tile_rv = req_rv; s->tile_axis = req_axis;
+        // everything plan_once may have pointed at the memory just released
+        s->d_fbuf = nullptr; s->d_blocks = nullptr; s->d_xface = nullptr; s->d_yface = nullptr;
+        s->d_TX = nullptr; s->d_TY = nullptr; s->d_TZ = nullptr; s->d_rec = nullptr;
+        s->d_xnode = nullptr; s->d_ynode = nullptr; s->d_znode = nullptr;
+        s->d_vblocks = nullptr; s->d_items = nullptr; s->d_done = nullptr; s->d_counter = nullptr;
     }
     return rc;
 }
@@ -734,6 +741,18 @@ int sweep_phase(dvm_solver *s)
     return 0;
 }
 
+// (syncs) The history slot the NEXT residual_kernel will write, read from the counter that kernel advances itself (scal[3]):
+// the host's iteration count is not used to address the ring, so the two cannot drift apart.
+int history_next_slot(dvm_solver *s, int *next)
+{
+    double v = 0.0;
+    CK(cudaMemcpyAsync(&v, s->d_scal + 3, sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+    CK(cudaStreamSynchronize(s->stream));
+    if (!(v >= 0.0 && v < (double)HIST_CAP)) return fail(DVM_ECUDA, "history counter on the device is corrupt (%g)", v);
+    *next = (int)v;
+    return 0;
+}
+
 // second half: wall fluxes from the half-range sums (tile kernel), conversion, wall densities, rescale, residual
 int update_phase(dvm_solver *s)
 {
@@ -768,16 +787,34 @@ int dvm_iterate(dvm_solver *s, int niter)
             const long long l0 = s->launches;
             const int it0 = s->iters;
             cudaGraph_t g = nullptr;
-            bool ok = cudaStreamBeginCapture(s->stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
+            // The capture runs on a stream of its own, not on the solver's: the solver's stream is very often the legacy
+            // default stream (torch's current stream, dvm_device.stream = 0), which cannot be captured at all.  Nothing
+            // executes during a capture, so the stream it is recorded on does not matter; the graph is launched on the
+            // solver's stream.
+            cudaStream_t user = s->stream, cap = nullptr;
+            bool ok = cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking) == cudaSuccess;
             if (ok) {
-                const int rc1 = sweep_phase(s), rc2 = rc1 ? rc1 : update_phase(s);
-                ok = cudaStreamEndCapture(s->stream, &g) == cudaSuccess && rc2 == 0 && g != nullptr;
+                s->stream = cap;
+                ok = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
+                if (ok) {
+                    const int rc1 = sweep_phase(s), rc2 = rc1 ? rc1 : update_phase(s);
+                    ok = cudaStreamEndCapture(cap, &g) == cudaSuccess && rc2 == 0 && g != nullptr;
+                }
+                s->stream = user;
             }
             if (ok) ok = cudaGraphInstantiate(&s->graph_exec, g, 0) == cudaSuccess;
             if (g) cudaGraphDestroy(g);
+            if (cap) cudaStreamDestroy(cap);
             s->graph_launches = s->launches - l0;
             s->launches = l0; s->iters = it0;           // nothing ran yet
-            if (!ok) { cudaGetLastError(); s->graph_exec = nullptr; s->graph_off = true; }
+            if (!ok) {
+                // not an error of the iteration (plain launches follow), but it must not go unnoticed: dvm_graph_active() = 0
+                // and the reason stays readable through dvm_last_error() until the next failing call of this thread
+                const cudaError_t ce = cudaGetLastError();
+                s->graph_exec = nullptr; s->graph_off = true; s->graph_failed = true;
+                fail(DVM_OK, "CUDA-graph capture of the iteration failed (%s): iterating with plain kernel launches",
+                     ce == cudaSuccess ? "a launch inside the capture was refused" : cudaGetErrorString(ce));
+            }
         }
     }
     for (int it = 0; it < niter; ++it) {
@@ -836,7 +873,9 @@ int dvm_residual(dvm_solver *s, double *host_out3)
     if (!s || !host_out3) return fail(DVM_EINVAL, "NULL argument");
     DeviceGuard guard(s->device);
     if (s->iters == 0) return fail(DVM_EINVAL, "no iteration done yet");
-    const int slot = (s->iters - 1) % HIST_CAP;
+    int next = 0;
+    if (int rc = history_next_slot(s, &next)) return rc;
+    const int slot = (next + HIST_CAP - 1) % HIST_CAP;
     CK(cudaMemcpyAsync(host_out3, s->d_hist + 3 * slot, 3 * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
     CK(cudaStreamSynchronize(s->stream));
     for (int m = 0; m < 3; ++m)
@@ -851,6 +890,11 @@ int dvm_tile_rv(const dvm_solver *s) { return s ? s->tile_rv : fail(DVM_EINVAL, 
 int dvm_tile_axis(const dvm_solver *s) { return s ? s->tile_axis : fail(DVM_EINVAL, "NULL solver"); }
 int dvm_precision(const dvm_solver *s) { return s ? s->precision : fail(DVM_EINVAL, "NULL solver"); }
 long long dvm_launch_count(const dvm_solver *s) { return s ? s->launches : -1; }
+int dvm_graph_active(const dvm_solver *s)
+{
+    if (!s) return fail(DVM_EINVAL, "NULL solver");
+    return s->graph_exec ? 1 : (s->graph_failed ? 2 : 0);
+}
 
 int dvm_get_state(dvm_solver *s, double *dev_prim14, double *dev_rho_wall)
 {
@@ -864,6 +908,7 @@ int dvm_get_state(dvm_solver *s, double *dev_prim14, double *dev_rho_wall)
 int dvm_set_state(dvm_solver *s, const double *dev_prim8, const double *dev_rho_wall)
 {
     if (!s || !dev_prim8) return fail(DVM_EINVAL, "NULL argument");
+    if (s->swept) return fail(DVM_EINVAL, "dvm_sweep without dvm_update: the state cannot be replaced between the two");
     DeviceGuard guard(s->device);
     CK(cudaMemcpyAsync(s->d_prim, dev_prim8, (size_t)8 * s->ncell * sizeof(double), cudaMemcpyDeviceToDevice, s->stream));
     CK(cudaMemsetAsync(s->d_prim + 8 * s->ncell, 0, (size_t)6 * s->ncell * sizeof(double), s->stream));
@@ -897,7 +942,9 @@ int dvm_residual_history(dvm_solver *s, double *host_out, int max_n)
     DeviceGuard guard(s->device);
     const int count = std::min(std::min(max_n, s->iters), HIST_CAP);
     if (count > 0) {
-        const int slot = (s->iters - count) % HIST_CAP;
+        int next = 0;
+        if (int rc = history_next_slot(s, &next)) return rc;
+        const int slot = ((next - count) % HIST_CAP + HIST_CAP) % HIST_CAP;
         const int run1 = std::min(count, HIST_CAP - slot);
         CK(cudaMemcpyAsync(host_out, s->d_hist + 3 * slot, (size_t)3 * run1 * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
         if (count > run1)
@@ -921,6 +968,10 @@ int dvm_step_host(dvm_solver *s, const double *host_prim8, const double *host_rh
                   double *host_prim14_out, double *host_rho_wall_out)
 {
     if (!s || n < 0) return fail(DVM_EINVAL, "bad argument");
+    // refuse before the state is touched: a sharded solver's replicated state must not change on one rank only
+    if (s->shard_count > 1 && n > 0)
+        return fail(DVM_EINVAL, "this solver holds 1 of %d velocity shards: iterate with dvm_sweep / all-reduce / dvm_update", s->shard_count);
+    if (s->swept) return fail(DVM_EINVAL, "dvm_sweep without dvm_update: the state cannot be replaced between the two");
     DeviceGuard guard(s->device);
     if (host_prim8) {
         CK(cudaMemcpyAsync(s->d_prim, host_prim8, (size_t)8 * s->ncell * sizeof(double), cudaMemcpyHostToDevice, s->stream));

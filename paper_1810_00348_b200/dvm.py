@@ -41,7 +41,7 @@ SYMBOLS = (
     "dvm_mass_scale", "dvm_step_host", "dvm_set_option", "dvm_workspace_bytes", "dvm_launch_count",
     "dvm_kernel_used", "dvm_tile_rv", "dvm_tile_axis", "dvm_precision", "dvm_plan_query", "dvm_plan_vblocks",
     "dvm_plan_shard_vblocks", "dvm_sweep", "dvm_update", "dvm_reduce_buffer", "dvm_destroy", "dvm_last_error",
-    "dvm_residual_noalloc",
+    "dvm_residual_noalloc", "dvm_graph_active", "dvm_fp64_peak_probe",
 )
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
@@ -140,10 +140,12 @@ def lib():
                                      C.POINTER(C.c_int), C.POINTER(C.c_int), C.c_int]
         L.dvm_plan_vblocks.argtypes = [C.POINTER(_VGrid), C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int), C.c_int]
         L.dvm_launch_count.argtypes = [vp]
+        L.dvm_graph_active.argtypes = [vp]
         L.dvm_launch_count.restype = C.c_longlong
         L.dvm_destroy.argtypes = [vp]
         L.dvm_last_error.restype = C.c_char_p
         L.dvm_residual_noalloc.argtypes = [vp, vp, C.c_longlong, vp, vp]
+        L.dvm_fp64_peak_probe.argtypes = [vp, C.c_longlong, _dp, _dp]
         _lib = L
     return _lib
 
@@ -190,6 +192,17 @@ def plan_shard_vblocks(xi_x, xi_y, xi_z, rank, count, rv=0, order=1, wide_axis=0
     out = np.zeros((n, 8), dtype=np.int32)
     _check(lib().dvm_plan_shard_vblocks(C.byref(v), rv, order, wide_axis, rank, count, out.ctypes.data_as(C.POINTER(C.c_int)), n))
     return out
+
+
+def fp64_peak_probe(device="cuda:0", rounds: int = 2_000_000):
+    """dvm_fp64_peak_probe on `device`: (fp64 lane-operations per second the board sustains on register-resident DFMA chains,
+    milliseconds of the timed launch).  Measurement aid for bench.py's roofline."""
+    import torch
+    with torch.cuda.device(torch.device(device)):
+        sink = torch.zeros(1, dtype=torch.float64, device=device)
+        rate, ms = C.c_double(), C.c_double()
+        _check(lib().dvm_fp64_peak_probe(sink.data_ptr(), int(rounds), C.byref(rate), C.byref(ms)))
+    return rate.value, ms.value
 
 
 RESIDUAL_NOALLOC_MAX_CELLS = 1 << 24
@@ -432,6 +445,11 @@ class Solver:
 
     def launch_count(self):
         return int(lib().dvm_launch_count(self._h))
+
+    def graph_active(self):
+        """1: iterations replay the captured CUDA graph; 0: plain launches, no graph in use; 2: plain launches because the
+        capture failed (dvm_graph_active)."""
+        return _check(lib().dvm_graph_active(self._h))
 
     def close(self):
         if getattr(self, "_h", None):
