@@ -8,8 +8,9 @@ A "step" is one outer iteration (all of DESIGN.md's hot-path rows a1-a7) of the 
 BASELINE.json configs[4] (128^3 x 64^3 cavity, Kn = 0.01, memory-reduction path, f never materialised), the
 largest single-GPU configuration and the one the target is stated on; --config picks another (0-4: BASELINE.json;
 5: the paper's own cube run, 191 x 181 x 181 stretched cells x 48^3 velocities; 6: a 16-level slab of config 4 for ncu).
-The solver runs on one GPU with no sharding (replicas only): with --gpus N every rank
-runs an independent replica, timing is max over ranks, value = total units / that time.
+Default multi-GPU mode (replicas only): with --gpus N every rank runs an independent replica,
+timing is max over ranks, value = total units / that time ("scaling": "weak").  --shard instead splits the velocity blocks
+of ONE problem over the ranks (one fp64 all-reduce of the velocity sums per iteration; "scaling": "strong").
 Prints ONE JSON line.
 """
 from __future__ import annotations
@@ -203,6 +204,8 @@ def run_gpu(args):
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
     dist = None
+    if torch.cuda.device_count() <= local:
+        sys.exit(f"bench.py: rank {rank} needs cuda:{local} but this node shows {torch.cuda.device_count()} GPU(s); there is no CPU fallback")
     if world > 1:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
@@ -276,6 +279,19 @@ def run_gpu(args):
     e2e_ms = 1e3 * (time.perf_counter() - t0) / e2e_steps
 
     total_ms, e2e_ms = max_over_ranks([total_ms, e2e_ms], dist, dev)
+
+    # ---- fp64 peak of this board, measured: register-resident DFMA chains on every SM, ~0.3 s, after the timed
+    # region and under its own clock sampler, ~1.5 s (a pure fp64 stream is power-limited: the clock it holds is part of the result)
+    fp64_probe = None
+    if rank == 0 and not args.no_fp64_probe:
+        torch.cuda.synchronize(dev)
+        psampler = ClockSampler(local)
+        psampler.start()
+        dvm.fp64_peak_probe(f"cuda:{local}", rounds=1_000_000)                 # nvidia-smi comes up, clocks settle under the load
+        rate, pms = dvm.fp64_peak_probe(f"cuda:{local}", rounds=8_000_000)     # ~1.3 s: several clock samples
+        fp64_probe = {"lane_ops_per_s": rate, "tflops": 2e-12 * rate, "ms": pms, "clocks": psampler.stop(),
+                      "kernel": "dfma_probe_kernel (csrc/fp64_probe.cu): 8 DFMA chains per thread, 2048 threads per SM",
+                      "nominal_lane_ops_per_s": FP64_LANE_SLOTS_PEAK}
     total_bytes, f_bytes = s.workspace_bytes()
 
     if rank == 0:
@@ -289,29 +305,46 @@ def run_gpu(args):
         bpp = algorithmic_bytes_per_point(kname, args.order) * (0.5 if mixed else 1.0)   # single-precision faces
         secs = ms_per_step * 1e-3
         hbm_gbs = bpp * pts / secs / 1e9
-        fp64_slots = FP64_SLOTS_PER_POINT[kname] * pts / secs            # executed fp64 lane slots per second
-        frac_hbm, frac_alu = hbm_gbs / peak, fp64_slots / FP64_LANE_SLOTS_PEAK
+        # executed-instruction counts come from ncu captures of ONE variant per precision (order 1, the library's choice of the
+        # tile variant, no workspace cap - or the slice kernel); for any other variant they are not evidence and are left out
+        counted_variant = kname == "slice" or (args.order == 1 and args.tile_rv == 0 and args.tile_axis == 0 and args.max_f_mbytes == 0)
+        alu = "fp32" if mixed else "fp64"
         if mixed:
             # single-precision sweep: 11.25 fp32 instructions per point (4 FADD + 3.25 FMUL + 4 FFMA, ncu) on the 128-lane
             # fp32 pipe; the fp64 side is one F2F (widening for the tensor-core sums) + 1.25 DMMA per point
-            fp64_slots = FP32_SLOTS_PER_POINT * pts / secs
-            frac_alu = fp64_slots / FP32_LANE_SLOTS_PEAK
+            inst_per_point, lane_peak = FP32_SLOTS_PER_POINT, FP32_LANE_SLOTS_PEAK
+        else:
+            inst_per_point, lane_peak = FP64_SLOTS_PER_POINT[kname], FP64_LANE_SLOTS_PEAK      # executed fp64 lane slots
+        alu_slots = inst_per_point * pts / secs if counted_variant else None
+        frac_hbm = hbm_gbs / peak
+        alu_peak_src = "derived: 148 SM x %d lanes x 2 flop x 1.965 GHz (DESIGN.md section 6)" % (128 if mixed else 64)
+        if fp64_probe is not None and not mixed:
+            lane_peak = fp64_probe["lane_ops_per_s"]          # the fp64 denominator is the measured one
+            alu_peak_src = "measured in this run: dvm_fp64_peak_probe (roofline.fp64_peak_measured)"
+        frac_alu = alu_slots / lane_peak if counted_variant else None
         # the ncu evidence belongs to the default variant (order 1, library's choice of the tile variant, no workspace cap)
-        default_variant = not mixed and args.order == 1 and args.tile_rv == 0 and args.tile_axis == 0 and args.max_f_mbytes == 0 and kname == "tile"
+        default_variant = not mixed and counted_variant and kname == "tile"
         ncu = NCU.get(wl.name, {}) if default_variant else {}
-        if frac_hbm >= frac_alu:
+        if frac_alu is None or frac_hbm >= frac_alu:
             roof = {"bound": "hbm", "achieved": hbm_gbs, "peak": peak, "unit": "GB/s", "frac": frac_hbm,
                     "traffic": ncu.get("traffic"), "peak_source": peak_src}
         else:
-            roof = {"bound": "alu", "achieved": 2.0 * fp64_slots / 1e12, "peak": 2e-12 * FP32_LANE_SLOTS_PEAK if mixed else FP64_PEAK_TFLOPS,
+            roof = {"bound": "alu", "achieved": 2.0 * alu_slots / 1e12, "peak": 2e-12 * lane_peak,
                     "unit": "TFLOP/s", "frac": frac_alu, "traffic": ncu.get("traffic"),
-                    "peak_source": "derived: 148 SM x %d lanes x 2 flop x 1.965 GHz (DESIGN.md section 6)" % (128 if mixed else 64)}
+                    "peak_source": alu_peak_src}
         roof.update({"kernel": f"sweep_{kname}_kernel", "launch_ms": ms_per_step,
-                     "algorithmic_bytes_per_point": bpp, "hbm_achieved_gbs": hbm_gbs, "hbm_peak_gbs": peak, "hbm_frac": frac_hbm,
-                     ("fp32" if mixed else "fp64") + "_executed_inst_per_point": FP32_SLOTS_PER_POINT if mixed else FP64_SLOTS_PER_POINT[kname],
-                     ("fp32" if mixed else "fp64") + "_executed_tflops": 2.0 * fp64_slots / 1e12,
-                     ("fp32" if mixed else "fp64") + "_peak_tflops": 2e-12 * FP32_LANE_SLOTS_PEAK if mixed else FP64_PEAK_TFLOPS,
-                     ("fp32" if mixed else "fp64") + "_pipe_frac": frac_alu,
+                     "algorithmic_bytes_per_point": bpp,
+                     "algorithmic_bytes_source": "constant: the design's face traffic per point (DESIGN.md section 6); ncu dram bytes "
+                                                 "of the default variant are in 'traffic' (profiles/r02_cfg4_counters.md)",
+                     "hbm_achieved_gbs": hbm_gbs, "hbm_peak_gbs": peak, "hbm_frac": frac_hbm,
+                     alu + "_executed_inst_per_point": inst_per_point if counted_variant else None,
+                     alu + "_executed_tflops": 2.0 * alu_slots / 1e12 if counted_variant else None,
+                     alu + "_peak_tflops": 2e-12 * lane_peak,
+                     alu + "_pipe_frac": frac_alu,
+                     alu + "_peak_source": alu_peak_src,
+                     "fp64_peak_measured": fp64_probe,
+                     alu + "_counts_note": None if counted_variant else "no instruction count was taken for this variant "
+                                           "(order / velocities per thread / axis / workspace cap): pipe fraction not reported",
                      "algorithmic_equivalent": {"fp64_slots_per_point": ALGO_FP64_SLOTS_PER_POINT,
                                                 "tflops": 2.0 * ALGO_FP64_SLOTS_PER_POINT * pts / secs / 1e12,
                                                 "note": "SURVEY.md 8(d) count with one FMA per moment and a divide; not executed"},
@@ -348,6 +381,20 @@ def run_gpu(args):
         dist.destroy_process_group()
 
 
+def self_launch_command(gpus, argv, env):
+    """The command that starts `gpus` ranks of this script (the driver's own launch line: torch.distributed.run, one node, one
+    process per GPU, rendezvous on 127.0.0.1), or None when there is nothing to start: one GPU, or a launcher has already set
+    WORLD_SIZE.  Host logic only - tests/test_bench_ranks.py checks it without a GPU."""
+    if gpus <= 1 or "WORLD_SIZE" in env:
+        return None
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    return [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={gpus}", "--master-addr", "127.0.0.1",
+            "--master-port", str(port), str(Path(__file__).resolve()), *argv]
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -359,6 +406,7 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--ref-budget", type=float, default=15.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-fp64-probe", action="store_true", help="skip the 0.3 s fp64 peak measurement after the timed region")
     ap.add_argument("--max-f-mbytes", type=int, default=0, help="cap (MiB) on the f workspace of the tile kernel (0 = none)")
     ap.add_argument("--tile-rv", type=int, default=0, choices=[0, 2, 3, 4], help="velocities per thread of the tile kernel (0 = library's choice)")
     ap.add_argument("--tile-axis", type=int, default=0, choices=[0, 1, 2, 3], help="velocity axis in the wide role of the tile kernel (1 + axis; 0 = library's choice)")
@@ -371,8 +419,16 @@ def main():
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
-    else:
-        run_gpu(args)
+        return
+    cmd = self_launch_command(args.gpus, sys.argv[1:], os.environ)
+    if cmd is not None:
+        # --gpus N without a launcher: start the N ranks here (one process per GPU, NCCL) and pass their output through;
+        # rank 0 prints the one JSON line with n_gpus = N
+        sys.exit(subprocess.run(cmd, env=dict(os.environ, NCCL_DEBUG=os.environ.get("NCCL_DEBUG", "WARN"))).returncode)
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if world != args.gpus:
+        sys.exit(f"bench.py: --gpus {args.gpus} but the launcher started WORLD_SIZE = {world} ranks")
+    run_gpu(args)
 
 
 if __name__ == "__main__":

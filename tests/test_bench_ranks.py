@@ -52,3 +52,29 @@ def test_reference_arm_other_ranks_do_no_work():
     r = subprocess.run([sys.executable, str(ROOT / "bench.py"), "--impl", "reference", "--gpus", "2", "--steps", "1",
                         "--warmup", "0"], env=env, capture_output=True, text=True, timeout=120)
     assert r.returncode == 0 and r.stdout.strip() == ""
+
+
+def test_gpus_n_starts_n_ranks_itself():
+    """`python bench.py --gpus N` without a launcher re-executes itself under torch.distributed.run with N processes (so the line
+    it prints says n_gpus = N); under a launcher (WORLD_SIZE set) and for one GPU it starts nothing."""
+    sys.path.insert(0, str(ROOT))
+    import bench
+    argv = ["--gpus", "4", "--steps", "2", "--warmup", "3", "--shard"]
+    cmd = bench.self_launch_command(4, argv, {})
+    assert cmd[:3] == [sys.executable, "-m", "torch.distributed.run"]
+    assert "--nproc-per-node=4" in cmd and "--nnodes=1" in cmd
+    assert cmd[cmd.index("--master-addr") + 1] == "127.0.0.1" and int(cmd[cmd.index("--master-port") + 1]) > 0
+    assert cmd[-len(argv) - 1:] == [str(ROOT / "bench.py"), *argv]
+    assert bench.self_launch_command(4, argv, {"WORLD_SIZE": "4"}) is None
+    assert bench.self_launch_command(1, ["--gpus", "1"], {}) is None
+
+
+def test_gpus_n_on_a_box_without_gpus_fails_loudly():
+    """The self-started ranks find no device: non-zero exit and a message, never a CPU result."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    r = subprocess.run([sys.executable, str(ROOT / "bench.py"), "--gpus", "2", "--steps", "1", "--warmup", "0", "--config", "0"],
+                       capture_output=True, text=True, timeout=300)
+    assert r.returncode != 0 and "no CPU fallback" in (r.stderr + r.stdout)
+    assert "point-updates/s" not in r.stdout
